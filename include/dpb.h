@@ -1,0 +1,135 @@
+/* include/dpb.h — C ABI of libdpb.so: one Deep Potential (smooth edition, se_a) energy / force / virial
+ * evaluation over a periodic box on one NVIDIA B200 (sm_100a).
+ *
+ * What is computed (arXiv 2004.11658, cited as PAPER.md:<line>; readings R1..R26 are listed in DESIGN.md):
+ *   E = sum_i E_i,  E_i = N_{alpha_i}( D( R~_i ) )                                  Eq. 1
+ *   neighbour list L~(i,:): type-sorted, distance-sorted, index-tie-broken, padded     Alg. 1
+ *   environment matrix R~_i (Nm x 4), rows s(r)(1, x/r, y/r, z/r), zero when padded    Eq. 5 / Alg. 2, :98-105, :212-238
+ *   embedding net G (1 -> s1 -> 2 s1 -> 4 s1 = M, tanh, concat skip)                   Eq. 6-9, :105-121
+ *   descriptor D_i = (G^T R~)(R~^T G^<)  (M x M^<, row-major flatten b*M^< + a)        Eq. 4, :94-96
+ *   fitting net (D -> w -> w -> w -> 1, tanh, identity skip on the square layers)       Eq. 2-3, :84-92
+ *   F_i = -dE/dr_i by back-propagation, virial Xi = -sum_{i,k} d_ik (x) dE_i/dd_ik      Eq. 10, :125-135; ProdForce/ProdVirial :240
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  All calls return 0 on success or a
+ * negative dpb_status; on error the outputs are undefined and dpb_last_error() describes the failure.
+ * Nothing here throws or aborts.  Units: Angstrom, eV, eV/Angstrom.  All matrices row-major.
+ */
+#ifndef DPB_H
+#define DPB_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dpb_model dpb_model;   /* opaque; owns device copies of the weights and a grow-only workspace */
+
+typedef enum {
+  DPB_FP64 = 0,   /* everything in fp64 (the paper's precision)                              */
+  DPB_TF32 = 1,   /* reserved: embedding / fitting GEMM operands in TF32, fp32 accumulate (BASELINE cfg 3) */
+  DPB_BF16 = 2    /* reserved: same with BF16 operands                                                     */
+} dpb_precision;
+
+typedef enum {
+  DPB_OK = 0,
+  DPB_EINVAL = -1,   /* bad argument, shape or type index                                                  */
+  DPB_EBOX = -2,     /* box not orthorhombic, or r_c >= min(L)/2 (reading R18: minimum image must be unique) */
+  DPB_ENOMEM = -3,   /* device or host allocation failed                                                   */
+  DPB_ECUDA = -4,    /* a CUDA runtime call or kernel launch failed                                        */
+  DPB_ECAP = -5,     /* an atom has more in-range candidates than the neighbour staging capacity           */
+  DPB_ENOTIMPL = -6  /* precision / model shape not supported by this build                                */
+} dpb_status;
+
+/* Model description.  All pointers are HOST pointers, read during dpb_model_create only (not retained). */
+typedef struct {
+  int32_t ntypes;             /* number of species (Remark 1)                                 */
+  double rcut;                /* r_c                                                          */
+  double rcut_smth;           /* r_cs: the gate w(r) of Eq. 5 is 1 below it (reading R1)                    */
+  const int32_t *sel;         /* sel[ntypes]: padded slot count per neighbour type; Nm = sum */
+  int32_t emb_s1;             /* embedding widths s1 -> 2 s1 -> 4 s1 = M (Eq. 8-9)        */
+  int32_t m_axis;             /* M^<, 1 <= M^< <= M                                          */
+  int32_t fit_width;          /* fitting hidden width (240)                                   */
+  const double *emb_weights;  /* ntypes^2 nets; net (a = centre type, t = neighbour type) at a*ntypes + t:
+                                 W0[1][s1] b0[s1] W1[s1][2s1] b1[2s1] W2[2s1][4s1] b2[4s1], [in][out]       */
+  const double *fit_weights;  /* ntypes nets: W0[M*M^<][w] b0[w] W1[w][w] b1[w] W2[w][w] b2[w] w3[w] b3[1]   */
+} dpb_model_desc;
+
+/* Filled by dpb_eval when info != NULL (this makes the call synchronise the stream). */
+typedef struct {
+  int64_t n_real_pairs;       /* number of non-padded neighbour slots over all atoms                        */
+  int64_t n_overflow;         /* neighbours dropped because a type section was full (reading R8)            */
+  int32_t max_nei[8];         /* max over atoms of in-range neighbours of type t (before truncation), t < 8 */
+  int32_t n_chunks;           /* atom chunks the evaluation was split into                                  */
+  int32_t reserved;
+} dpb_eval_info;
+
+/* Create / destroy.  dpb_model_create copies (and re-lays-out) the weights to the current CUDA device.
+ * Errors: DPB_EINVAL (shape), DPB_ENOTIMPL (precision != DPB_FP64 in this build), DPB_ENOMEM, DPB_ECUDA. */
+int dpb_model_create(const dpb_model_desc *desc, int precision, dpb_model **out);
+int dpb_model_destroy(dpb_model *model);
+
+/* Nm = sum_t sel[t]. */
+int dpb_model_nm(const dpb_model *model);
+
+/* Upper bound on the atoms processed per pass (bounds the workspace: about 80 KB per atom for copper).
+ * Default 32768.  Returns DPB_EINVAL if chunk < 1. */
+int dpb_model_set_chunk(dpb_model *model, int64_t chunk_atoms);
+
+/* Select the kernel generation: 0 = plain reference kernels ("v0": unfused, thread-per-output FMA loops),
+ * 1 = fused DMMA kernels (default).  Both compute the same path; tests compare each with the oracle. */
+int dpb_model_set_variant(dpb_model *model, int variant);
+
+/* One evaluation (the paper's problem statement: coordinates, types and box in; E, E_i, F_i and the virial out).
+ *   stream       cudaStream_t (as void*) on which all work is enqueued; NULL = the legacy default stream
+ *   natoms       N >= 0
+ *   coord        DEVICE fp64 [N][3], raw (unwrapped is allowed) Cartesian positions
+ *   type         DEVICE int32 [N], 0 <= type < ntypes, any order
+ *   box          HOST fp64 [9], rows = cell vectors; must be orthorhombic with r_c < min(L)/2 (DPB_EBOX otherwise)
+ *   energy       DEVICE fp64 [1]            E                      (may be NULL)
+ *   atom_energy  DEVICE fp64 [N]            E_i                    (may be NULL)
+ *   force        DEVICE fp64 [N][3]         F_i = -dE/dr_i         (may be NULL)
+ *   virial       DEVICE fp64 [9]            Xi[a][b] = -sum_i sum_k d_ik[a] dE_i/dd_ik[b]  (may be NULL)
+ *   nlist        DEVICE int32 [N][Nm]       formatted neighbour list, -1 padded  (may be NULL)
+ *   info         HOST, may be NULL; non-NULL synchronises the stream before returning
+ * The caller owns every buffer; the library neither frees nor retains them.  Work is asynchronous with
+ * respect to the host unless info != NULL.  Neighbour overflow is not an error: the nearest sel[t] are kept. */
+int dpb_eval(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,
+             const double box[9], double *energy, double *atom_energy, double *force, double *virial,
+             int32_t *nlist, dpb_eval_info *info);
+
+/* Same call with HOST buffers for coord/type and for every output (end-to-end entry: host->device copies of the
+ * inputs, the evaluation, and device->host copies of the requested outputs, all on `stream`, then a stream
+ * synchronise).  Pinned host memory makes the copies asynchronous, pageable memory is accepted. */
+int dpb_eval_host(dpb_model *model, void *stream, int64_t natoms, const double *coord_h, const int32_t *type_h,
+                  const double box[9], double *energy_h, double *atom_energy_h, double *force_h, double *virial_h,
+                  int32_t *nlist_h, dpb_eval_info *info);
+
+/* Alg. 1 only (cell binning + neighbour search + format): nlist DEVICE int32 [N][Nm].  n_overflow HOST, may be
+ * NULL (non-NULL synchronises). */
+int dpb_build_nlist(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,
+                    const double box[9], int32_t *nlist, int64_t *n_overflow);
+
+/* Test / profiling hook, not part of the contract: DEVICE buffers (any may be NULL) that the following
+ * dpb_eval calls also fill, indexed by the ORIGINAL atom index:
+ *   T  [N][M][4]   = G^T R~                    (Eq. 4, left factor)
+ *   D  [N][M*M^<]  = descriptor                (only written by variant 0)
+ *   dT [N][M][4]   = dE_i/dT_i
+ * Pass all NULL to switch it off. */
+int dpb_set_debug_buffers(dpb_model *model, double *T, double *D, double *dT);
+
+/* Per-stage device time of the last dpb_eval that was given info != NULL, in microseconds (CUDA events on the
+ * caller's stream): [0] cell binning, [1] neighbour search + format, [2] env + embedding + T, [3] descriptor +
+ * fitting fwd/bwd + dT, [4] embedding backward + force/virial, [5] reductions.  Requires dpb_model_set_timing(1). */
+int dpb_model_set_timing(dpb_model *model, int on);
+int dpb_model_stage_us(const dpb_model *model, float stage_us[8]);
+
+/* Thread-local description of the last error returned on this thread; valid until the next call. */
+const char *dpb_last_error(void);
+
+/* Version string of the library ("dpb <n> sm_100a"). */
+const char *dpb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DPB_H */

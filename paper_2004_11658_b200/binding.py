@@ -1,0 +1,218 @@
+"""ctypes binding of libdpb.so — same names as include/dpb.h, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+STATUS = {0: "DPB_OK", -1: "DPB_EINVAL", -2: "DPB_EBOX", -3: "DPB_ENOMEM", -4: "DPB_ECUDA", -5: "DPB_ECAP",
+          -6: "DPB_ENOTIMPL"}
+FP64, TF32, BF16 = 0, 1, 2
+
+
+class DPBError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class _Desc(C.Structure):
+    _fields_ = [("ntypes", C.c_int32), ("rcut", C.c_double), ("rcut_smth", C.c_double),
+                ("sel", C.POINTER(C.c_int32)), ("emb_s1", C.c_int32), ("m_axis", C.c_int32),
+                ("fit_width", C.c_int32), ("emb_weights", C.POINTER(C.c_double)),
+                ("fit_weights", C.POINTER(C.c_double))]
+
+
+class _Info(C.Structure):
+    _fields_ = [("n_real_pairs", C.c_int64), ("n_overflow", C.c_int64), ("max_nei", C.c_int32 * 8),
+                ("n_chunks", C.c_int32), ("reserved", C.c_int32)]
+
+
+@dataclass
+class EvalInfo:
+    n_real_pairs: int
+    n_overflow: int
+    max_nei: tuple
+    n_chunks: int
+
+
+def lib_path() -> str:
+    return os.path.join(HERE, "libdpb.so")
+
+
+_LIB = None
+
+
+def load_library():
+    """Load libdpb.so (built in-tree by paper_2004_11658_b200/build.py).  Raises if it is missing: no fallback."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = lib_path()
+    if not os.path.exists(path):
+        raise DPBError(-4, f"{path} not found: build it with `python -m paper_2004_11658_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int
+    lib.dpb_model_create.argtypes = [C.POINTER(_Desc), i32, C.POINTER(vp)]
+    lib.dpb_model_destroy.argtypes = [vp]
+    lib.dpb_model_nm.argtypes = [vp]
+    lib.dpb_model_set_chunk.argtypes = [vp, i64]
+    lib.dpb_model_set_variant.argtypes = [vp, i32]
+    lib.dpb_model_set_timing.argtypes = [vp, i32]
+    lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.dpb_set_debug_buffers.argtypes = [vp, vp, vp, vp]
+    lib.dpb_eval.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp, C.POINTER(_Info)]
+    lib.dpb_eval_host.argtypes = lib.dpb_eval.argtypes
+    lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
+    lib.dpb_last_error.restype = C.c_char_p
+    lib.dpb_version.restype = C.c_char_p
+    _LIB = lib
+    return lib
+
+
+def _torch():
+    import torch
+    return torch
+
+
+class DPModel:
+    """One DP model on the current CUDA device (dpb_model_create / dpb_eval / dpb_model_destroy)."""
+
+    def __init__(self, ntypes, rcut, rcut_smth, sel, emb_s1, m_axis, fit_width, emb_weights, fit_weights,
+                 precision: int = FP64):
+        self.lib = load_library()
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise DPBError(-4, "no CUDA device: this library has no CPU path")
+        self.ntypes = int(ntypes)
+        self.sel = np.ascontiguousarray(sel, dtype=np.int32)
+        self.nm = int(self.sel.sum())
+        self.s1, self.m_axis, self.fit_width = int(emb_s1), int(m_axis), int(fit_width)
+        self.M = 4 * self.s1
+        self.dim = self.M * self.m_axis
+        emb = np.ascontiguousarray(emb_weights, dtype=np.float64)
+        fit = np.ascontiguousarray(fit_weights, dtype=np.float64)
+        desc = _Desc(self.ntypes, float(rcut), float(rcut_smth), self.sel.ctypes.data_as(C.POINTER(C.c_int32)),
+                     self.s1, self.m_axis, self.fit_width, emb.ctypes.data_as(C.POINTER(C.c_double)),
+                     fit.ctypes.data_as(C.POINTER(C.c_double)))
+        self._h = C.c_void_p()
+        self._chk(self.lib.dpb_model_create(C.byref(desc), int(precision), C.byref(self._h)))
+
+    @classmethod
+    def from_spec(cls, spec, emb, fit, precision: int = FP64):
+        return cls(spec.ntypes, spec.rcut, spec.rcut_smth, spec.sel, spec.emb_s1, spec.m_axis, spec.fit_width,
+                   emb, fit, precision)
+
+    def _chk(self, rc):
+        if rc != 0:
+            raise DPBError(rc, self.lib.dpb_last_error().decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self.lib.dpb_model_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_chunk(self, n: int):
+        self._chk(self.lib.dpb_model_set_chunk(self._h, int(n)))
+
+    def set_variant(self, v: int):
+        self._chk(self.lib.dpb_model_set_variant(self._h, int(v)))
+
+    def set_timing(self, on: bool):
+        self._chk(self.lib.dpb_model_set_timing(self._h, int(bool(on))))
+
+    def stage_us(self):
+        buf = (C.c_float * 8)()
+        self._chk(self.lib.dpb_model_stage_us(self._h, buf))
+        return list(buf)
+
+    def set_debug_buffers(self, T=None, D=None, dT=None):
+        p = [None if t is None else C.c_void_p(t.data_ptr()) for t in (T, D, dT)]
+        self._debug_keep = (T, D, dT)
+        self._chk(self.lib.dpb_set_debug_buffers(self._h, *p))
+
+    @staticmethod
+    def _box(box):
+        b = np.ascontiguousarray(box, dtype=np.float64).reshape(9)
+        return b, b.ctypes.data_as(C.POINTER(C.c_double))
+
+    @staticmethod
+    def _stream():
+        torch = _torch()
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    def eval(self, coord, types, box, want_nlist=False, want_info=False, out=None):
+        """dpb_eval on torch CUDA tensors (coord float64 [N,3], types int32 [N]); returns a dict of CUDA tensors.
+
+        `out` may hold preallocated tensors (energy, atom_energy, force, virial, nlist) to reuse between calls.
+        """
+        torch = _torch()
+        assert coord.is_cuda and coord.dtype == torch.float64 and coord.is_contiguous()
+        assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
+        n = int(coord.shape[0])
+        dev = coord.device
+        o = out if out is not None else {}
+        if "energy" not in o:
+            o["energy"] = torch.empty(1, dtype=torch.float64, device=dev)
+            o["atom_energy"] = torch.empty(n, dtype=torch.float64, device=dev)
+            o["force"] = torch.empty((n, 3), dtype=torch.float64, device=dev)
+            o["virial"] = torch.empty((3, 3), dtype=torch.float64, device=dev)
+        if want_nlist and "nlist" not in o:
+            o["nlist"] = torch.empty((n, self.nm), dtype=torch.int32, device=dev)
+        b, bp = self._box(box)
+        info = _Info() if want_info else None
+        nl = C.c_void_p(o["nlist"].data_ptr()) if want_nlist else None
+        rc = self.lib.dpb_eval(self._h, self._stream(), n, C.c_void_p(coord.data_ptr()), C.c_void_p(types.data_ptr()),
+                               bp, C.c_void_p(o["energy"].data_ptr()), C.c_void_p(o["atom_energy"].data_ptr()),
+                               C.c_void_p(o["force"].data_ptr()), C.c_void_p(o["virial"].data_ptr()), nl,
+                               C.byref(info) if want_info else None)
+        self._chk(rc)
+        if want_info:
+            o["info"] = EvalInfo(int(info.n_real_pairs), int(info.n_overflow), tuple(info.max_nei), int(info.n_chunks))
+        return o
+
+    def eval_host(self, coord, types, box, out=None, want_nlist=False):
+        """dpb_eval_host on HOST arrays (numpy or pinned torch CPU tensors): H2D, evaluation, D2H, synchronise."""
+        torch = _torch()
+
+        def ptr(a):
+            return C.c_void_p(a.data_ptr()) if isinstance(a, torch.Tensor) else C.c_void_p(a.ctypes.data)
+
+        n = int(coord.shape[0])
+        o = out if out is not None else {}
+        if "energy" not in o:
+            o["energy"] = np.empty(1)
+            o["atom_energy"] = np.empty(n)
+            o["force"] = np.empty((n, 3))
+            o["virial"] = np.empty((3, 3))
+        if want_nlist and "nlist" not in o:
+            o["nlist"] = np.empty((n, self.nm), dtype=np.int32)
+        b, bp = self._box(box)
+        rc = self.lib.dpb_eval_host(self._h, self._stream(), n, ptr(coord), ptr(types), bp, ptr(o["energy"]),
+                                    ptr(o["atom_energy"]), ptr(o["force"]), ptr(o["virial"]),
+                                    ptr(o["nlist"]) if want_nlist else None, None)
+        self._chk(rc)
+        return o
+
+    def build_nlist(self, coord, types, box):
+        """dpb_build_nlist: returns (nlist CUDA int32 [N][Nm], n_overflow)."""
+        torch = _torch()
+        n = int(coord.shape[0])
+        nlist = torch.empty((n, self.nm), dtype=torch.int32, device=coord.device)
+        b, bp = self._box(box)
+        ovf = C.c_int64(0)
+        rc = self.lib.dpb_build_nlist(self._h, self._stream(), n, C.c_void_p(coord.data_ptr()),
+                                      C.c_void_p(types.data_ptr()), bp, C.c_void_p(nlist.data_ptr()), C.byref(ovf))
+        self._chk(rc)
+        return nlist, int(ovf.value)

@@ -1,0 +1,392 @@
+// api.cu — the C ABI of libdpb.so (include/dpb.h): model object, grow-only device workspace, host dispatcher.
+// One dpb_eval = S1 (cell sort) once, then for each chunk of atoms (sorted by type, then cell):
+//   S2 nlist -> S3-S5 pass 1 (T) -> S5-S7 fitting fwd/bwd (E_i, dT) -> S8-S9 pass 2 (F, virial); finally E = sum E_i.
+// Everything is enqueued on the caller's stream; no host synchronisation unless the caller asks for `info`.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "v1_kernels.cuh"
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+extern "C" const char *dpb_last_error(void) { return g_err; }
+extern "C" const char *dpb_version(void) { return "dpb 1 sm_100a"; }
+
+struct Buf {
+  void *p = nullptr;
+  size_t cap = 0;
+  cudaError_t reserve(size_t bytes) {
+    if (bytes <= cap) return cudaSuccess;
+    if (p) cudaFree(p);
+    p = nullptr; cap = 0;
+    size_t want = bytes + bytes / 8 + 256;
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e == cudaSuccess) cap = want;
+    return e;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+  template <class T> T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+struct dpb_model {
+  DevModel P;
+  int precision = 0, variant = 0, timing = 0;
+  int64_t chunk = 32768;
+  int device = 0;
+  Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
+  V1Weights v1;                 // re-laid-out weights of the fused kernels
+  // workspace
+  Buf key, count, start, cursor, s_idx, s_xyz, stats, ei;
+  Buf nl, dr, nreal, T, dT;
+  Buf v0[9];
+  Buf v1ws;
+  Buf h_coord, h_type, h_out;   // device staging of dpb_eval_host
+  double *dbgT = nullptr, *dbgD = nullptr, *dbgdT = nullptr;
+  std::vector<cudaEvent_t> evs;   // stage timers: [0] start, [1] after S1, then 4 per chunk, then the end
+  int ev_chunks = 0;              // chunks of the last timed evaluation
+  float stage_us[8] = {};
+};
+
+static int nm_of(const DevModel &P) { return P.nm; }
+
+extern "C" int dpb_model_nm(const dpb_model *m) { return m ? nm_of(m->P) : DPB_EINVAL; }
+
+extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_model **out) {
+  if (!d || !out) return fail(DPB_EINVAL, "dpb_model_create: null argument");
+  *out = nullptr;
+  if (precision != DPB_FP64) return fail(DPB_ENOTIMPL, "dpb_model_create: only DPB_FP64 is built");
+  if (d->ntypes < 1 || d->ntypes > DPB_MAX_TYPES) return fail(DPB_EINVAL, "ntypes must be in [1, %d]", DPB_MAX_TYPES);
+  if (!d->sel || !d->emb_weights || !d->fit_weights) return fail(DPB_EINVAL, "null sel / weights");
+  if (d->emb_s1 < 1 || d->emb_s1 > 64) return fail(DPB_EINVAL, "emb_s1 must be in [1, 64]");
+  if (d->m_axis < 1 || d->m_axis > 4 * d->emb_s1) return fail(DPB_EINVAL, "m_axis must be in [1, 4 s1]");
+  if (d->fit_width < 1 || d->fit_width > 1024) return fail(DPB_EINVAL, "fit_width must be in [1, 1024]");
+  if (!(d->rcut > 0.0) || !(d->rcut_smth >= 0.0) || !(d->rcut_smth < d->rcut))
+    return fail(DPB_EINVAL, "need 0 <= rcut_smth < rcut");
+  dpb_model *m = new (std::nothrow) dpb_model();
+  if (!m) return fail(DPB_ENOMEM, "host allocation failed");
+  DevModel &P = m->P;
+  memset(&P, 0, sizeof(P));
+  P.ntypes = d->ntypes; P.s1 = d->emb_s1; P.M = 4 * d->emb_s1; P.Ma = d->m_axis; P.dim = P.M * P.Ma;
+  P.fw = d->fit_width; P.rc = d->rcut; P.rcs = d->rcut_smth;
+  int nm = 0;
+  for (int t = 0; t < P.ntypes; ++t) {
+    if (d->sel[t] < 0) { delete m; return fail(DPB_EINVAL, "sel[%d] < 0", t); }
+    P.sel[t] = d->sel[t]; P.sec_start[t] = nm; nm += d->sel[t];
+  }
+  P.sec_start[P.ntypes] = nm;
+  for (int t = P.ntypes + 1; t <= DPB_MAX_TYPES; ++t) P.sec_start[t] = nm;
+  P.nm = nm;
+  const long long s1 = P.s1;
+  P.emb_net_size = s1 + s1 + s1 * 2 * s1 + 2 * s1 + 2 * s1 * 4 * s1 + 4 * s1;
+  P.fit_net_size = (long long)P.dim * P.fw + P.fw + 2 * ((long long)P.fw * P.fw + P.fw) + P.fw + 1;
+  cudaGetDevice(&m->device);
+  const size_t eb = sizeof(double) * (size_t)P.emb_net_size * P.ntypes * P.ntypes;
+  const size_t fb = sizeof(double) * (size_t)P.fit_net_size * P.ntypes;
+  cudaError_t e = m->emb.reserve(eb);
+  if (e == cudaSuccess) e = m->fit.reserve(fb);
+  if (e == cudaSuccess) e = m->stats.reserve(sizeof(DevStats));
+  if (e == cudaSuccess) e = cudaMemcpy(m->emb.p, d->emb_weights, eb, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(m->fit.p, d->fit_weights, fb, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = v1_prepare_weights(P, d->emb_weights, d->fit_weights, m->v1);
+  if (e != cudaSuccess) {
+    int code = (e == cudaErrorMemoryAllocation) ? DPB_ENOMEM : DPB_ECUDA;
+    dpb_model_destroy(m);
+    return fail(code, "dpb_model_create: %s", cudaGetErrorString(e));
+  }
+  *out = m;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_destroy(dpb_model *m) {
+  if (!m) return DPB_OK;
+  Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
+                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->h_coord, &m->h_type, &m->h_out};
+  for (Buf *b : all) b->release();
+  for (Buf &b : m->v0) b.release();
+  v1_release_weights(m->v1);
+  for (cudaEvent_t &e : m->evs) cudaEventDestroy(e);
+  delete m;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_chunk(dpb_model *m, int64_t chunk) {
+  if (!m || chunk < 1) return fail(DPB_EINVAL, "dpb_model_set_chunk: chunk must be >= 1");
+  m->chunk = chunk;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_variant(dpb_model *m, int variant) {
+  if (!m || variant < 0 || variant > 1) return fail(DPB_EINVAL, "dpb_model_set_variant: variant must be 0 or 1");
+  m->variant = variant;
+  return DPB_OK;
+}
+
+extern "C" int dpb_set_debug_buffers(dpb_model *m, double *T, double *D, double *dT) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  m->dbgT = T; m->dbgD = D; m->dbgdT = dT;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_timing(dpb_model *m, int on) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  m->timing = on ? 1 : 0;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_stage_us(const dpb_model *m, float us[8]) {
+  if (!m || !us) return fail(DPB_EINVAL, "null argument");
+  memcpy(us, m->stage_us, sizeof(float) * 8);
+  return DPB_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static int make_grid(const DevModel &P, const double box[9], DevGrid &G) {
+  if (box[1] != 0.0 || box[2] != 0.0 || box[3] != 0.0 || box[5] != 0.0 || box[6] != 0.0 || box[7] != 0.0)
+    return fail(DPB_EBOX, "box must be orthorhombic (off-diagonal entries are not zero)");
+  G.L[0] = box[0]; G.L[1] = box[4]; G.L[2] = box[8];
+  long long ncell = 1;
+  for (int c = 0; c < 3; ++c) {
+    if (!(G.L[c] > 0.0) || !(P.rc < 0.5 * G.L[c]))
+      return fail(DPB_EBOX, "need rcut < L/2 in every dimension (L[%d] = %g, rcut = %g)", c, G.L[c], P.rc);
+    // cell edge >= rc (1 + 1e-6): the +-1 stencil then covers every r <= rc even when rounding moves an atom that
+    // sits on a cell face into the neighbouring cell
+    double f = floor(G.L[c] / (P.rc * (1.0 + 1e-6)));
+    int n = f < 1.0 ? 1 : (f > 512.0 ? 512 : (int)f);
+    G.nc[c] = n;
+    ncell *= n;
+  }
+  while (ncell * P.ntypes > (1ll << 22)) {           // bound the histogram: coarser cells are still correct
+    int big = 0;
+    for (int c = 1; c < 3; ++c) if (G.nc[c] > G.nc[big]) big = c;
+    ncell = ncell / G.nc[big];
+    G.nc[big] = (G.nc[big] + 1) / 2;
+    ncell *= G.nc[big];
+  }
+  for (int c = 0; c < 3; ++c) G.lo_mode[c] = G.nc[c] >= 3 ? 1 : 0;
+  G.ncell = (int)ncell;
+  return DPB_OK;
+}
+
+static int cuda_fail(cudaError_t e, const char *what) {
+  return fail(e == cudaErrorMemoryAllocation ? DPB_ENOMEM : DPB_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+#define CU(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, what); } while (0)
+
+static int neighbour_cap(const DevModel &P) {
+  int cap = 2 * P.nm;
+  if (cap < 256) cap = 256;
+  if (cap > 12288) cap = 12288;       // 16 B per hit: 192 KB of shared memory at most
+  return cap;
+}
+
+static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double *coord, const int32_t *type,
+                    const double box[9], double *energy, double *atom_energy, double *force, double *virial,
+                    int32_t *nlist, bool nlist_only) {
+  const DevModel &P = m->P;
+  if (natoms < 0 || natoms > 2000000000ll) return fail(DPB_EINVAL, "natoms out of range");
+  if (natoms > 0 && (!coord || !type)) return fail(DPB_EINVAL, "null coord / type");
+  DevGrid G;
+  int rc = make_grid(P, box, G);
+  if (rc != DPB_OK) return rc;
+  const int N = (int)natoms;
+  const int nkeys = P.ntypes * G.ncell;
+  const int64_t chunk = m->chunk < natoms ? m->chunk : (natoms > 0 ? natoms : 1);
+
+  CU(m->key.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
+  CU(m->count.reserve(sizeof(int) * (size_t)(nkeys + 1)), "workspace");
+  CU(m->start.reserve(sizeof(int) * (size_t)(nkeys + 1 + P.ntypes + 1)), "workspace");
+  CU(m->cursor.reserve(sizeof(int) * (size_t)(nkeys + 1)), "workspace");
+  CU(m->s_idx.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
+  CU(m->s_xyz.reserve(sizeof(double) * 3 * (size_t)(N + 1)), "workspace");
+  CU(m->ei.reserve(sizeof(double) * (size_t)(N + 1)), "workspace");
+  CU(m->nl.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
+  CU(m->dr.reserve(sizeof(double4) * (size_t)chunk * P.nm), "workspace");
+  CU(m->nreal.reserve(sizeof(int) * (size_t)chunk * P.ntypes), "workspace");
+  if (!nlist_only) {
+    CU(m->T.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
+    CU(m->dT.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
+    if (m->variant == 0) {
+      CU(m->v0[0].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
+      CU(m->v0[1].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
+      for (int k = 2; k < 9; ++k) CU(m->v0[k].reserve(sizeof(double) * (size_t)chunk * P.fw), "workspace");
+    } else {
+      CU(m->v1ws.reserve(v1_workspace_bytes(P, chunk)), "workspace");
+    }
+  }
+  DevStats *stats = m->stats.as<DevStats>();
+  CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");
+  const bool timing = m->timing && !nlist_only;
+  const int nchunks = (int)((natoms + chunk - 1) / chunk);
+  if (timing) {
+    const size_t need = 3 + 4 * (size_t)nchunks;
+    while (m->evs.size() < need) {
+      cudaEvent_t e;
+      CU(cudaEventCreate(&e), "cudaEventCreate");
+      m->evs.push_back(e);
+    }
+    m->ev_chunks = nchunks;
+    cudaEventRecord(m->evs[0], st);
+  }
+
+  int *start = m->start.as<int>();
+  CU(launch_cell_sort(P, G, natoms, coord, type, m->key.as<int>(), m->count.as<int>(), start, m->cursor.as<int>(),
+                      m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st), "cell sort");
+  if (timing) cudaEventRecord(m->evs[1], st);
+
+  double *ei = atom_energy ? atom_energy : m->ei.as<double>();
+  if (!nlist_only) {
+    if (force) CU(cudaMemsetAsync(force, 0, sizeof(double) * 3 * (size_t)natoms, st), "memset force");
+    if (virial) CU(cudaMemsetAsync(virial, 0, sizeof(double) * 9, st), "memset virial");
+  }
+  const int cap = neighbour_cap(P);
+  int ci = 0;
+  for (int64_t p0 = 0; p0 < natoms; p0 += chunk, ++ci) {
+    ChunkView C;
+    C.p0 = (int)p0;
+    C.n = (int)((natoms - p0) < chunk ? (natoms - p0) : chunk);
+    C.s_idx = m->s_idx.as<int>();
+    C.type_start = start + nkeys + 1;
+    C.nl = m->nl.as<int>();
+    C.dr = m->dr.as<double4>();
+    C.nreal = m->nreal.as<int>();
+    C.T = m->T.as<double>();
+    C.dT = m->dT.as<double>();
+    CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st), "nlist");
+    if (nlist_only) continue;
+    if (timing) cudaEventRecord(m->evs[2 + 4 * ci], st);
+    if (m->variant == 0) {
+      V0Scratch S;
+      S.D = m->v0[0].as<double>(); S.dD = m->v0[1].as<double>();
+      S.Z0 = m->v0[2].as<double>(); S.U1 = m->v0[3].as<double>(); S.Z1 = m->v0[4].as<double>();
+      S.U2 = m->v0[5].as<double>(); S.Z2 = m->v0[6].as<double>(); S.G = m->v0[7].as<double>();
+      S.dZ = m->v0[8].as<double>();
+      CU(launch_pass1_v0(P, C, m->emb.as<double>(), st), "pass1 v0");
+      if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);
+      CU(launch_fit_v0(P, C, m->fit.as<double>(), S, ei, m->dbgD, st), "fit v0");
+      CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
+      if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
+      CU(launch_pass2_v0(P, C, m->emb.as<double>(), force, virial, st), "pass2 v0");
+      if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
+    } else {
+      CU(v1_pass1(P, C, m->v1, st), "pass1");
+      if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);
+      CU(v1_fit(P, C, m->v1, m->fit.as<double>(), m->v1ws.p, ei, st), "fit");
+      CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
+      if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
+      CU(v1_pass2(P, C, m->v1, force, virial, st), "pass2");
+      if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
+    }
+  }
+  if (!nlist_only) {
+    if (energy) CU(launch_reduce_energy(natoms, ei, energy, st), "energy reduction");
+    if (timing) cudaEventRecord(m->evs[2 + 4 * nchunks], st);
+  }
+  return DPB_OK;
+}
+
+static int finish_info(dpb_model *m, cudaStream_t st, int64_t natoms, dpb_eval_info *info) {
+  DevStats hs;
+  CU(cudaMemcpyAsync(&hs, m->stats.p, sizeof(DevStats), cudaMemcpyDeviceToHost, st), "stats copy");
+  CU(cudaStreamSynchronize(st), "stream synchronise");
+  if (hs.err_type) return fail(DPB_EINVAL, "an atom has a type index outside [0, ntypes)");
+  if (hs.err_cap) return fail(DPB_ECAP, "an atom has more in-range candidates than the staging capacity (%d)",
+                              neighbour_cap(m->P));
+  if (info) {
+    memset(info, 0, sizeof(*info));
+    info->n_real_pairs = (int64_t)hs.n_real_pairs;
+    info->n_overflow = (int64_t)hs.n_overflow;
+    for (int t = 0; t < 8 && t < DPB_MAX_TYPES; ++t) info->max_nei[t] = hs.max_nei[t];
+    const int64_t chunk = m->chunk;
+    info->n_chunks = (int32_t)((natoms + chunk - 1) / chunk);
+  }
+  if (m->timing && m->ev_chunks > 0 && m->evs.size() >= 3 + 4 * (size_t)m->ev_chunks) {
+    float ms = 0.f;
+    memset(m->stage_us, 0, sizeof(m->stage_us));
+    if (cudaEventElapsedTime(&ms, m->evs[0], m->evs[1]) == cudaSuccess) m->stage_us[0] = ms * 1e3f;
+    for (int c = 0; c < m->ev_chunks; ++c) {
+      const int b = 2 + 4 * c;
+      if (cudaEventElapsedTime(&ms, m->evs[b - 1], m->evs[b]) == cudaSuccess) m->stage_us[1] += ms * 1e3f;
+      for (int k = 0; k < 3; ++k)
+        if (cudaEventElapsedTime(&ms, m->evs[b + k], m->evs[b + k + 1]) == cudaSuccess) m->stage_us[2 + k] += ms * 1e3f;
+    }
+    const int last = 2 + 4 * m->ev_chunks;
+    if (cudaEventElapsedTime(&ms, m->evs[last - 1], m->evs[last]) == cudaSuccess) m->stage_us[5] = ms * 1e3f;
+  }
+  return DPB_OK;
+}
+
+extern "C" int dpb_eval(dpb_model *m, void *stream, int64_t natoms, const double *coord, const int32_t *type,
+                        const double box[9], double *energy, double *atom_energy, double *force, double *virial,
+                        int32_t *nlist, dpb_eval_info *info) {
+  if (!m || !box) return fail(DPB_EINVAL, "dpb_eval: null model / box");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  int rc = run_eval(m, st, natoms, coord, type, box, energy, atom_energy, force, virial, nlist, false);
+  if (rc != DPB_OK) return rc;
+  if (info) return finish_info(m, st, natoms, info);
+  return DPB_OK;
+}
+
+extern "C" int dpb_build_nlist(dpb_model *m, void *stream, int64_t natoms, const double *coord, const int32_t *type,
+                               const double box[9], int32_t *nlist, int64_t *n_overflow) {
+  if (!m || !box || !nlist) return fail(DPB_EINVAL, "dpb_build_nlist: null argument");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  int rc = run_eval(m, st, natoms, coord, type, box, nullptr, nullptr, nullptr, nullptr, nlist, true);
+  if (rc != DPB_OK) return rc;
+  if (n_overflow) {
+    dpb_eval_info info;
+    rc = finish_info(m, st, natoms, &info);
+    if (rc != DPB_OK) return rc;
+    *n_overflow = info.n_overflow;
+  }
+  return DPB_OK;
+}
+
+extern "C" int dpb_eval_host(dpb_model *m, void *stream, int64_t natoms, const double *coord_h, const int32_t *type_h,
+                             const double box[9], double *energy_h, double *atom_energy_h, double *force_h,
+                             double *virial_h, int32_t *nlist_h, dpb_eval_info *info) {
+  if (!m || !box) return fail(DPB_EINVAL, "dpb_eval_host: null model / box");
+  if (natoms < 0) return fail(DPB_EINVAL, "natoms < 0");
+  if (natoms > 0 && (!coord_h || !type_h)) return fail(DPB_EINVAL, "null coord / type");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const size_t n = (size_t)natoms;
+  CU(m->h_coord.reserve(sizeof(double) * 3 * (n + 1)), "staging");
+  CU(m->h_type.reserve(sizeof(int) * (n + 1)), "staging");
+  // outputs: E[1] (padded to 2), virial[9] (padded to 10), E_i[N], F[N][3], then nlist
+  const size_t out_d = 2 + 10 + n + 3 * n;
+  const size_t nl_bytes = nlist_h ? sizeof(int) * n * (size_t)m->P.nm : 0;
+  CU(m->h_out.reserve(sizeof(double) * out_d + nl_bytes + 16), "staging");
+  double *d_e = m->h_out.as<double>(), *d_v = d_e + 2, *d_ei = d_v + 10, *d_f = d_ei + n;
+  int *d_nl = nlist_h ? reinterpret_cast<int *>(d_f + 3 * n) : nullptr;
+  if (natoms > 0) {
+    CU(cudaMemcpyAsync(m->h_coord.p, coord_h, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, st), "H2D coord");
+    CU(cudaMemcpyAsync(m->h_type.p, type_h, sizeof(int) * n, cudaMemcpyHostToDevice, st), "H2D type");
+  }
+  int rc = run_eval(m, st, natoms, m->h_coord.as<double>(), m->h_type.as<int>(), box, energy_h ? d_e : nullptr,
+                    atom_energy_h ? d_ei : nullptr, force_h ? d_f : nullptr, virial_h ? d_v : nullptr, d_nl, false);
+  if (rc != DPB_OK) return rc;
+  if (energy_h) CU(cudaMemcpyAsync(energy_h, d_e, sizeof(double), cudaMemcpyDeviceToHost, st), "D2H energy");
+  if (virial_h) CU(cudaMemcpyAsync(virial_h, d_v, sizeof(double) * 9, cudaMemcpyDeviceToHost, st), "D2H virial");
+  if (atom_energy_h && natoms > 0)
+    CU(cudaMemcpyAsync(atom_energy_h, d_ei, sizeof(double) * n, cudaMemcpyDeviceToHost, st), "D2H atom energy");
+  if (force_h && natoms > 0)
+    CU(cudaMemcpyAsync(force_h, d_f, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, st), "D2H force");
+  if (nlist_h && natoms > 0)
+    CU(cudaMemcpyAsync(nlist_h, d_nl, nl_bytes, cudaMemcpyDeviceToHost, st), "D2H nlist");
+  if (info) return finish_info(m, st, natoms, info);
+  CU(cudaStreamSynchronize(st), "stream synchronise");
+  return DPB_OK;
+}

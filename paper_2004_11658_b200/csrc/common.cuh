@@ -1,0 +1,101 @@
+// common.cuh — internal declarations shared by the translation units of libdpb.so (CUDA, sm_100a).
+// Not installed; the public interface is include/dpb.h.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dpb.h"
+
+#define DPB_MAX_TYPES 8
+
+// Model parameters passed to kernels by value.
+struct DevModel {
+  int ntypes, nm, s1, M, Ma, dim, fw;
+  double rc, rcs;
+  int sel[DPB_MAX_TYPES];
+  int sec_start[DPB_MAX_TYPES + 1];   // slot offset of neighbour-type section t; sec_start[ntypes] = nm
+  long long emb_net_size, fit_net_size;
+};
+
+// Cell grid of one evaluation (orthorhombic box).
+struct DevGrid {
+  double L[3];
+  int nc[3];
+  int ncell;
+  int lo_mode[3];   // 1: nc >= 3, use the +-1 stencil; 0: fewer than 3 cells, visit every cell of that dimension once
+};
+
+// Stats accumulated on the device by the neighbour kernel.
+struct DevStats {
+  unsigned long long n_real_pairs;
+  unsigned long long n_overflow;
+  int max_nei[DPB_MAX_TYPES];
+  int err_type;      // an atom had a type index outside [0, ntypes)
+  int err_cap;       // an atom had more in-range candidates than the staging capacity
+};
+
+// Per-chunk views (chunk = sorted positions [p0, p0 + n)).
+struct ChunkView {
+  int p0, n;
+  const int *s_idx;        // [N] original atom index of sorted position p
+  const int *type_start;   // [ntypes + 1] first sorted position of each type (device)
+  int *nl;                 // [n][nm] neighbour index per slot (chunk-local copy of the nlist rows)
+  double4 *dr;             // [n][nm] (dx, dy, dz, r) of real slots
+  int *nreal;              // [n][ntypes] real (non-padded) slots per section
+  double *T;               // [n][M][4]
+  double *dT;              // [n][M][4]
+};
+
+// ---- launchers implemented in the .cu files (all asynchronous on `st`; return cudaGetLastError()) ----------
+cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
+                             int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
+                             DevStats *stats, cudaStream_t st);
+cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
+                         const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st);
+
+// variant 0 ("v0"): plain unfused kernels
+struct V0Scratch {
+  double *D, *dD;                       // [n][dim]
+  double *Z0, *U1, *Z1, *U2, *Z2;       // [n][fw]
+  double *G, *dZ;                       // [n][fw]
+};
+cudaError_t launch_pass1_v0(const DevModel &P, const ChunkView &C, const double *emb, cudaStream_t st);
+cudaError_t launch_fit_v0(const DevModel &P, const ChunkView &C, const double *fit, const V0Scratch &S,
+                          double *atom_energy, double *dbgD, cudaStream_t st);
+cudaError_t launch_pass2_v0(const DevModel &P, const ChunkView &C, const double *emb, double *force, double *virial,
+                            cudaStream_t st);
+
+cudaError_t launch_scatter_debug(const DevModel &P, const ChunkView &C, double *dbgT, double *dbgdT, cudaStream_t st);
+cudaError_t launch_reduce_energy(int64_t natoms, const double *atom_energy, double *energy, cudaStream_t st);
+
+// ---- device helpers ---------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+// Minimum-image displacement d = r_j - r_i and |d| (Alg. 1 line 3-4), one pinned sequence of
+// IEEE-754 operations on the raw coordinates (reading R2) so that the neighbour list is reproducible bit for bit:
+//   d = x_j - x_i;  k = rint(d / L);  d = fma(-k, L, d);  r2 = fma(dz,dz, fma(dy,dy, dx*dx));  r = sqrt(r2).
+__device__ __forceinline__ void dp_displacement(const double xi[3], const double xj[3], const double L[3], double d[3],
+                                                double &r) {
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    double dc = __dsub_rn(xj[c], xi[c]);
+    double k = rint(__ddiv_rn(dc, L[c]));
+    d[c] = __fma_rn(-k, L[c], dc);
+  }
+  double r2 = __fma_rn(d[2], d[2], __fma_rn(d[1], d[1], __dmul_rn(d[0], d[0])));
+  r = __dsqrt_rn(r2);
+}
+
+// Gate w(r) of Eq. 5, reading R1: quintic between r_cs and r_c.
+__device__ __forceinline__ void dp_switch(double r, double rcs, double rc, double &w, double &dw) {
+  if (r < rcs) {
+    w = 1.0; dw = 0.0;
+  } else if (r < rc) {
+    double inv = 1.0 / (rc - rcs);
+    double u = (r - rcs) * inv;
+    w = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+    dw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * inv;
+  } else {
+    w = 0.0; dw = 0.0;
+  }
+}
+#endif
