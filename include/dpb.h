@@ -117,14 +117,18 @@ int dpb_build_nlist(dpb_model *model, void *stream, int64_t natoms, const double
  * Pass all NULL to switch it off. */
 int dpb_set_debug_buffers(dpb_model *model, double *T, double *D, double *dT);
 
-/* Per-stage device time of the last dpb_eval that was given info != NULL, in microseconds (CUDA events on the
- * caller's stream): [0] cell binning, [1] neighbour search + format, [2] env + embedding + T, [3] descriptor +
- * fitting fwd/bwd + dT, [4] embedding backward + force/virial, [5] reductions.  Requires dpb_model_set_timing(1). */
+/* Per-stage device time of the last dpb_eval issued after dpb_model_set_timing(model, 1), in microseconds (CUDA
+ * events recorded on the caller's stream between the stages; the caller must have synchronised that stream):
+ * [0] cell binning, [1] neighbour search + format, [2] env + embedding + T, [3] descriptor + fitting fwd/bwd + dT,
+ * [4] embedding backward + force/virial, [5] energy reduction; summed over chunks.  DPB_ECUDA if not complete. */
 int dpb_model_set_timing(dpb_model *model, int on);
 int dpb_model_stage_us(const dpb_model *model, float stage_us[8]);
 
 /* Thread-local description of the last error returned on this thread; valid until the next call. */
 const char *dpb_last_error(void);
+
+/* Number of CUDA kernels this library has launched in this process so far (all models, all calls). */
+int64_t dpb_kernel_launches(void);
 
 /* Version string of the library ("dpb <n> sm_100a"). */
 const char *dpb_version(void);

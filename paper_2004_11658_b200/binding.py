@@ -69,6 +69,7 @@ def load_library():
     lib.dpb_eval.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp, C.POINTER(_Info)]
     lib.dpb_eval_host.argtypes = lib.dpb_eval.argtypes
     lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
+    lib.dpb_kernel_launches.restype = C.c_int64
     lib.dpb_last_error.restype = C.c_char_p
     lib.dpb_version.restype = C.c_char_p
     _LIB = lib
@@ -136,6 +137,9 @@ class DPModel:
         buf = (C.c_float * 8)()
         self._chk(self.lib.dpb_model_stage_us(self._h, buf))
         return list(buf)
+
+    def kernel_launches(self) -> int:
+        return int(self.lib.dpb_kernel_launches())
 
     def set_debug_buffers(self, T=None, D=None, dT=None):
         p = [None if t is None else C.c_void_p(t.data_ptr()) for t in (T, D, dT)]

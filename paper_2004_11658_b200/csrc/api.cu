@@ -22,6 +22,9 @@ static int fail(int code, const char *fmt, ...) {
   return code;
 }
 
+unsigned long long g_dpb_launches = 0;
+extern "C" int64_t dpb_kernel_launches(void) { return (int64_t)g_dpb_launches; }
+
 extern "C" const char *dpb_last_error(void) { return g_err; }
 extern "C" const char *dpb_version(void) { return "dpb 1 sm_100a"; }
 
@@ -57,7 +60,6 @@ struct dpb_model {
   double *dbgT = nullptr, *dbgD = nullptr, *dbgdT = nullptr;
   std::vector<cudaEvent_t> evs;   // stage timers: [0] start, [1] after S1, then 4 per chunk, then the end
   int ev_chunks = 0;              // chunks of the last timed evaluation
-  float stage_us[8] = {};
 };
 
 static int nm_of(const DevModel &P) { return P.nm; }
@@ -148,7 +150,21 @@ extern "C" int dpb_model_set_timing(dpb_model *m, int on) {
 
 extern "C" int dpb_model_stage_us(const dpb_model *m, float us[8]) {
   if (!m || !us) return fail(DPB_EINVAL, "null argument");
-  memcpy(us, m->stage_us, sizeof(float) * 8);
+  memset(us, 0, sizeof(float) * 8);
+  if (m->ev_chunks <= 0 || m->evs.size() < 3 + 4 * (size_t)m->ev_chunks)
+    return fail(DPB_EINVAL, "no timed evaluation yet (dpb_model_set_timing)");
+  float ms = 0.f;
+  cudaError_t e = cudaEventElapsedTime(&ms, m->evs[0], m->evs[1]);
+  if (e != cudaSuccess) return fail(DPB_ECUDA, "stage events not complete: %s", cudaGetErrorString(e));
+  us[0] = ms * 1e3f;
+  for (int c = 0; c < m->ev_chunks; ++c) {
+    const int b = 2 + 4 * c;
+    if (cudaEventElapsedTime(&ms, m->evs[b - 1], m->evs[b]) == cudaSuccess) us[1] += ms * 1e3f;
+    for (int k = 0; k < 3; ++k)
+      if (cudaEventElapsedTime(&ms, m->evs[b + k], m->evs[b + k + 1]) == cudaSuccess) us[2 + k] += ms * 1e3f;
+  }
+  const int last = 2 + 4 * m->ev_chunks;
+  if (cudaEventElapsedTime(&ms, m->evs[last - 1], m->evs[last]) == cudaSuccess) us[5] = ms * 1e3f;
   return DPB_OK;
 }
 
@@ -312,19 +328,6 @@ static int finish_info(dpb_model *m, cudaStream_t st, int64_t natoms, dpb_eval_i
     for (int t = 0; t < 8 && t < DPB_MAX_TYPES; ++t) info->max_nei[t] = hs.max_nei[t];
     const int64_t chunk = m->chunk;
     info->n_chunks = (int32_t)((natoms + chunk - 1) / chunk);
-  }
-  if (m->timing && m->ev_chunks > 0 && m->evs.size() >= 3 + 4 * (size_t)m->ev_chunks) {
-    float ms = 0.f;
-    memset(m->stage_us, 0, sizeof(m->stage_us));
-    if (cudaEventElapsedTime(&ms, m->evs[0], m->evs[1]) == cudaSuccess) m->stage_us[0] = ms * 1e3f;
-    for (int c = 0; c < m->ev_chunks; ++c) {
-      const int b = 2 + 4 * c;
-      if (cudaEventElapsedTime(&ms, m->evs[b - 1], m->evs[b]) == cudaSuccess) m->stage_us[1] += ms * 1e3f;
-      for (int k = 0; k < 3; ++k)
-        if (cudaEventElapsedTime(&ms, m->evs[b + k], m->evs[b + k + 1]) == cudaSuccess) m->stage_us[2 + k] += ms * 1e3f;
-    }
-    const int last = 2 + 4 * m->ev_chunks;
-    if (cudaEventElapsedTime(&ms, m->evs[last - 1], m->evs[last]) == cudaSuccess) m->stage_us[5] = ms * 1e3f;
   }
   return DPB_OK;
 }

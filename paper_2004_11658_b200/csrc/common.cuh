@@ -46,6 +46,10 @@ struct ChunkView {
   double *dT;              // [n][M][4]
 };
 
+// Process-wide count of kernels launched by this library (reported by dpb_kernel_launches()).
+extern unsigned long long g_dpb_launches;
+#define DPB_LAUNCHED(n) (g_dpb_launches += (unsigned long long)(n))
+
 // ---- launchers implemented in the .cu files (all asynchronous on `st`; return cudaGetLastError()) ----------
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,

@@ -84,6 +84,7 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
   // type_start lives right behind start[nkeys + 1]
   k_scan<<<1, 1024, 0, st>>>(nkeys, G.ncell, P.ntypes, count, start, cursor, start + nkeys + 1);
   if (n > 0) k_fill<<<(n + 255) / 256, 256, 0, st>>>(n, coord, key, cursor, s_idx, s_xyz);
+  DPB_LAUNCHED(n > 0 ? 3 : 1);
   return cudaGetLastError();
 }
 
@@ -221,6 +222,7 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
     configured = smem;
   }
   k_nlist<<<C.n, NL_THREADS, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
@@ -241,6 +243,7 @@ __global__ void k_reduce_energy(long long n, const double *__restrict__ ei, doub
 
 cudaError_t launch_reduce_energy(int64_t natoms, const double *atom_energy, double *energy, cudaStream_t st) {
   k_reduce_energy<<<1, 1024, 0, st>>>((long long)natoms, atom_energy, energy);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
@@ -258,5 +261,6 @@ __global__ void k_scatter_debug(DevModel P, ChunkView C, double *dbgT, double *d
 cudaError_t launch_scatter_debug(const DevModel &P, const ChunkView &C, double *dbgT, double *dbgdT, cudaStream_t st) {
   if (C.n <= 0 || (!dbgT && !dbgdT)) return cudaSuccess;
   k_scatter_debug<<<C.n, 128, 0, st>>>(P, C, dbgT, dbgdT);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }

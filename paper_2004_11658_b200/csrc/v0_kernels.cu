@@ -90,6 +90,7 @@ cudaError_t launch_pass1_v0(const DevModel &P, const ChunkView &C, const double 
   const int threads = ((P.M + 31) / 32) * 32;
   const size_t smem = sizeof(double) * (RG * 4 + RG * P.s1 + RG * 2 * P.s1);
   k_pass1_v0<<<C.n, threads, smem, st>>>(P, C, emb);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
@@ -256,6 +257,7 @@ cudaError_t launch_pass2_v0(const DevModel &P, const ChunkView &C, const double 
   if (threads < 64) threads = 64;
   const size_t smem = sizeof(double) * (RG * 4 + 2 * RG * P.s1 + 2 * RG * 2 * P.s1 + (threads / 32) * RG * 5 + RG * 5);
   k_pass2_v0<<<C.n, threads, smem, st>>>(P, C, emb, force, virial);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
@@ -422,5 +424,6 @@ cudaError_t launch_fit_v0(const DevModel &P, const ChunkView &C, const double *f
     k_gemm_v0<3, true><<<g_dim, 256, 0, st>>>(C, ty, dim, fw, S.G, fw, W0, fw, nullptr, nullptr, S.dD, nullptr, dim);
   }
   k_dT_v0<<<C.n, 256, 0, st>>>(P, C, S.dD);
+  DPB_LAUNCHED(2 + 9 * P.ntypes);
   return cudaGetLastError();
 }

@@ -1,0 +1,260 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle on the same
+seeded inputs.  Bars (BASELINE.json north_star): nlist bit-exact including order and padding; fp64: relative error
+<= 1e-10 on E, absolute error <= 1e-9 eV/A on F.  We also bound E_i, the virial, T and dT.
+
+Both kernel generations are checked: variant 0 (plain unfused kernels) and variant 1 (fused DMMA kernels)."""
+import numpy as np
+import pytest
+
+import gen
+from gen.weights import MODELS, ModelSpec
+
+from conftest import small_model, random_box
+
+pytestmark = pytest.mark.gpu
+
+E_REL = 1e-10
+F_ABS = 1e-9
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (the library has no CPU fallback)")
+    return torch
+
+
+def _models(spec, emb, fit, variant):
+    from oracle import Oracle
+    from paper_2004_11658_b200 import DPModel
+    m = DPModel.from_spec(spec, emb, fit)
+    m.set_variant(variant)
+    return Oracle.from_spec(spec, emb, fit), m
+
+
+def _gpu_eval(m, coord, types, box, debug=False, spec=None):
+    torch = _torch()
+    dc = torch.tensor(coord, device="cuda")
+    dt = torch.tensor(types, device="cuda")
+    dbg = None
+    if debug:
+        n = coord.shape[0]
+        T = torch.zeros((n, spec.m, 4), dtype=torch.float64, device="cuda")
+        dT = torch.zeros_like(T)
+        m.set_debug_buffers(T, None, dT)
+        dbg = (T, dT)
+    out = m.eval(dc, dt, box, want_nlist=True, want_info=True)
+    torch.cuda.synchronize()
+    res = {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in out.items()}
+    if debug:
+        res["T"], res["dT"] = dbg[0].cpu().numpy(), dbg[1].cpu().numpy()
+        m.set_debug_buffers(None, None, None)
+    return res
+
+
+def _check_full(ref, got, n_overflow=0):
+    assert got["nlist"].dtype == np.int32
+    assert np.array_equal(got["nlist"], ref["nlist"]), "nlist must be bit-exact (order and padding)"
+    assert got["info"].n_overflow == n_overflow
+    e_ref = ref["energy"]
+    assert abs(e_ref) >= 1e-3 * np.abs(ref["atom_energy"]).sum()          # reading R20: E is not a cancellation
+    assert abs(got["energy"][0] - e_ref) <= E_REL * abs(e_ref)
+    assert np.abs(got["atom_energy"] - ref["atom_energy"]).max() <= E_REL * np.abs(ref["atom_energy"]).max()
+    assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
+    assert np.abs(got["virial"] - ref["virial"]).max() <= 1e-10 * max(1.0, np.abs(ref["virial"]).max())
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("conditioned", [False, True])
+def test_water192_full_parity(variant, conditioned):
+    """BASELINE config 0 (W192), literal and conditioned weight sets: every output element against the oracle."""
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    if conditioned:
+        fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, variant)
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box, debug=True, spec=spec)
+    _check_full(ref, got)
+    ar = orc.atom_rows(coord, types, box, None, ref["nlist"], want_T=True)
+    assert np.abs(got["T"] - ar["T"]).max() <= 1e-12 * np.abs(ar["T"]).max()
+    assert np.abs(got["dT"] - ar["dT"]).max() <= 1e-11 * np.abs(ar["dT"]).max()
+    assert got["info"].n_real_pairs == int((ref["nlist"] >= 0).sum())
+    m.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_copper_small_full_parity(variant):
+    """Copper model (sel 512, 32-64-128) on a 6x6x6-cell FCC box (864 atoms, several row tiles + ragged tail)."""
+    spec = MODELS["Cu32k"]
+    coord, types, box = gen.copper_box(6, 0.05, seed=gen.SEED_BASE + 2)
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, variant)
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box)
+    _check_full(ref, got)
+    assert got["info"].max_nei[0] == int((ref["nlist"] >= 0).sum(1).max())
+    m.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("chunk", [1, 7, 100000])
+def test_chunking_does_not_change_results(variant, chunk):
+    """Atom chunking (the memory bound for the 864k-atom config) must give the same result for any chunk size,
+    including chunks that straddle a species boundary."""
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, variant)
+    m.set_chunk(chunk)
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box)
+    _check_full(ref, got)
+    m.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_tiny_model_three_types_random_box(variant):
+    """A small 3-species model with odd widths (s1 = 5, M^< = 3, width 9) on a random box with unsorted types:
+    exercises padding of every tile dimension and ntypes^2 = 9 embedding nets (Remark 1)."""
+    spec, emb, fit = small_model(ntypes=3, s1=5, m_axis=3, fit_width=9, sel=(7, 12, 9), rcut=3.5, rcut_smth=0.8,
+                                 seed=11, fit_scale=0.02)
+    coord, types, box = random_box(150, 9.0, 3, seed=5, min_dist=0.9)
+    orc, m = _models(spec, emb, fit, variant)
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box)
+    assert np.array_equal(got["nlist"], ref["nlist"])
+    assert abs(got["energy"][0] - ref["energy"]) <= E_REL * abs(ref["energy"])
+    assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
+    assert np.abs(got["virial"] - ref["virial"]).max() <= 1e-10 * max(1.0, np.abs(ref["virial"]).max())
+    m.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_neighbour_overflow_keeps_nearest(variant):
+    """Reading R8: more neighbours than sel[t] -> the nearest sel[t] are kept and the drops are counted."""
+    spec, emb, fit = small_model(ntypes=2, s1=4, m_axis=3, fit_width=8, sel=(3, 4), rcut=4.0, rcut_smth=1.0, seed=3)
+    coord, types, box = random_box(120, 10.0, 2, seed=9, min_dist=0.9)
+    orc, m = _models(spec, emb, fit, variant)
+    nl_ref, ovf_ref = orc.build_nlist(coord, types, box)
+    assert ovf_ref > 0
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box)
+    assert np.array_equal(got["nlist"], nl_ref)
+    assert got["info"].n_overflow == ovf_ref
+    assert abs(got["energy"][0] - ref["energy"]) <= E_REL * abs(ref["energy"])
+    assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
+    m.close()
+
+
+def test_unwrapped_coordinates_and_exact_ties():
+    """Raw coordinates outside [0, L) are allowed; a simple-cubic lattice with exactly representable coordinates
+    gives exact distance ties, broken by atom index."""
+    torch = _torch()
+    n = 6
+    g = np.stack(np.meshgrid(*[np.arange(n)] * 3, indexing="ij"), -1).reshape(-1, 3).astype(np.float64) * 2.0
+    rng = np.random.default_rng(3)
+    g_shift = g + 12.0 * rng.integers(-2, 3, size=g.shape)        # whole box vectors: same bits after min-image
+    types = np.zeros(len(g), dtype=np.int32)
+    box = np.diag([2.0 * n] * 3).reshape(9)
+    spec = ModelSpec("sc", 1, 4.5, 1.0, (64,), 4, 2, 8, 0)
+    emb, fit = gen.make_weights(spec, seed=1)
+    orc, m = _models(spec, emb, fit, 0)
+    for c in (g, g_shift):
+        nl_ref, _ = orc.build_nlist(c, types, box)
+        nl, ovf = m.build_nlist(torch.tensor(c, device="cuda"), torch.tensor(types, device="cuda"), box)
+        assert np.array_equal(nl.cpu().numpy(), nl_ref)
+    m.close()
+
+
+def test_empty_and_isolated_inputs():
+    """N = 0 is legal; an isolated atom has D = 0, E_i = N(0), F = 0 (SURVEY.md §8(c) pins)."""
+    torch = _torch()
+    spec, emb, fit = small_model()
+    orc, m = _models(spec, emb, fit, 1)
+    box = np.diag([20.0] * 3).reshape(9)
+    out = m.eval(torch.zeros((0, 3), dtype=torch.float64, device="cuda"),
+                 torch.zeros((0,), dtype=torch.int32, device="cuda"), box, want_info=True)
+    torch.cuda.synchronize()
+    assert out["energy"].item() == 0.0
+    coord = np.array([[1.0, 2.0, 3.0], [11.0, 12.0, 13.0]])
+    types = np.array([0, 1], dtype=np.int32)
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box)
+    assert np.all(got["nlist"] == -1)
+    assert np.abs(got["atom_energy"] - ref["atom_energy"]).max() <= 1e-14
+    assert np.all(got["force"] == 0.0)
+    m.close()
+
+
+def test_errors_are_reported_not_thrown_from_c():
+    from paper_2004_11658_b200 import DPBError
+    torch = _torch()
+    spec, emb, fit = small_model()
+    _, m = _models(spec, emb, fit, 1)
+    coord = torch.zeros((4, 3), dtype=torch.float64, device="cuda")
+    types = torch.zeros((4,), dtype=torch.int32, device="cuda")
+    with pytest.raises(DPBError) as e:
+        m.eval(coord, types, np.diag([7.0] * 3).reshape(9))                  # r_c = 4 >= L/2
+    assert e.value.status == -2
+    skew = np.diag([20.0] * 3); skew[0, 1] = 1.0
+    with pytest.raises(DPBError) as e:
+        m.eval(coord, types, skew.reshape(9))
+    assert e.value.status == -2
+    bad = torch.full((4,), 5, dtype=torch.int32, device="cuda")
+    with pytest.raises(DPBError) as e:
+        m.eval(torch.rand((4, 3), dtype=torch.float64, device="cuda") * 20, bad, np.diag([20.0] * 3).reshape(9),
+               want_info=True)
+    assert e.value.status == -1
+    m.close()
+
+
+@pytest.mark.parametrize("name", ["W24k", "Cu32k"])
+def test_full_size_sampled_parity(name):
+    """BASELINE configs 1 and 2 at full size, in the launch configuration bench.py times (variant 1, default chunk):
+    sampled atoms against the oracle (nlist rows bit-exact, E_i, T, dT), plus whole-system properties that hold at
+    any size: sum F = 0, symmetric virial, force parity between the two kernel generations."""
+    torch = _torch()
+    spec = MODELS[name]
+    coord, types, box = gen.make_system(name)
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, 1)
+    got = _gpu_eval(m, coord, types, box, debug=True, spec=spec)
+    n = coord.shape[0]
+    rows = np.random.default_rng(1).choice(n, 48, replace=False).astype(np.int64)
+    nl_ref, _ = orc.build_nlist(coord, types, box, rows=rows)
+    assert np.array_equal(got["nlist"][rows], nl_ref)
+    ar = orc.atom_rows(coord, types, box, rows, nl_ref, want_T=True)
+    assert np.abs(got["atom_energy"][rows] - ar["atom_energy"]).max() <= E_REL * np.abs(ar["atom_energy"]).max()
+    assert np.abs(got["T"][rows] - ar["T"]).max() <= 1e-12 * np.abs(ar["T"]).max()
+    assert np.abs(got["dT"][rows] - ar["dT"]).max() <= 1e-11 * np.abs(ar["dT"]).max()
+    # forces of the sampled atoms' own slots: F_i gets contributions from neighbours' lists too, so compare the two
+    # independent kernel generations on every atom instead, and check the conservation laws
+    assert np.abs(got["force"].sum(0)).max() <= 1e-9
+    assert np.abs(got["virial"] - got["virial"].T).max() <= 1e-9 * np.abs(got["virial"]).max()
+    assert abs(got["energy"][0] - got["atom_energy"].sum()) <= 1e-12 * np.abs(got["atom_energy"]).sum()
+    m0 = _models(spec, emb, fit, 0)[1]
+    got0 = _gpu_eval(m0, coord, types, box)
+    assert np.array_equal(got0["nlist"], got["nlist"])
+    assert np.abs(got0["force"] - got["force"]).max() <= F_ABS
+    assert abs(got0["energy"][0] - got["energy"][0]) <= E_REL * abs(got0["energy"][0])
+    m.close(); m0.close()
+
+
+def test_eval_host_matches_device_entry():
+    """dpb_eval_host (host buffers, copies inside) returns the same numbers as dpb_eval."""
+    torch = _torch()
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    _, m = _models(spec, emb, fit, 1)
+    dev = _gpu_eval(m, coord, types, box)
+    host = m.eval_host(coord, types, box, want_nlist=True)
+    assert np.array_equal(host["nlist"], dev["nlist"])
+    assert np.abs(host["force"] - dev["force"]).max() <= 1e-12
+    assert abs(host["energy"][0] - dev["energy"][0]) <= 1e-12 * abs(dev["energy"][0])
+    m.close()
