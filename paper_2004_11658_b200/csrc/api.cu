@@ -46,7 +46,7 @@ struct Buf {
 
 struct dpb_model {
   DevModel P;
-  int precision = 0, variant = 0, timing = 0;
+  int precision = 0, variant = 1, timing = 0;
   int64_t chunk = 32768;
   int device = 0;
   Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
@@ -235,7 +235,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   if (!nlist_only) {
     CU(m->T.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
     CU(m->dT.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
-    if (m->variant == 0) {
+    if (m->variant == 0 || !m->v1.ready) {
       CU(m->v0[0].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
       CU(m->v0[1].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
       for (int k = 2; k < 9; ++k) CU(m->v0[k].reserve(sizeof(double) * (size_t)chunk * P.fw), "workspace");
@@ -284,7 +284,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st), "nlist");
     if (nlist_only) continue;
     if (timing) cudaEventRecord(m->evs[2 + 4 * ci], st);
-    if (m->variant == 0) {
+    if (m->variant == 0 || !m->v1.ready) {
       V0Scratch S;
       S.D = m->v0[0].as<double>(); S.dD = m->v0[1].as<double>();
       S.Z0 = m->v0[2].as<double>(); S.U1 = m->v0[3].as<double>(); S.Z1 = m->v0[4].as<double>();

@@ -1,0 +1,570 @@
+// embed_dmma.cu — variant 1 of S3+S4+S5 (pass 1) and S8+S9 (pass 2): the embedding net on fp64 tensor-core tiles
+// (mma.sync m8n8k4 = SASS DMMA.8x8x4, the only fp64 MMA primitive of sm_100a; tcgen05 has no f64 kind), fused with
+// the env matrix, the G^T R~ reduction and the force / virial chain so that G never leaves the SM.
+//
+// Fragment layout of m8n8k4 (g = lane / 4, q = lane % 4):  A[row g][k q]   B[k q][col g]   C[row g][cols 2q, 2q+1].
+// Rows are neighbours.  The output of one layer (C layout: thread (g, q) holds, for n-block nb, the columns 2q and
+// 2q+1, called "slots" 2nb and 2nb+1 of lane quarter q) feeds the next layer as A operand WITHOUT any shuffle: the
+// k-step `ks` of the next GEMM takes, from lane quarter q, its slot ks — a permutation of the contraction index that
+// the weight rows follow.  Features are placed so that the concat skip [x || x] of Eq. 9 stays inside the thread:
+//   feature o of a layer of width 2^l s1:  copy c = o / s1, r = o % s1  ->  quarter q = r % 4, slot = c * SP + r / 4,
+// with SP = ceil(s1 / 4) slots per copy (pads are zero weights, zero bias: their activations are exactly 0).
+// The padded weight matrices in shared memory are  W_l[4 * ks + q][8 * nb + 2 q' + e]  (input slot ks of quarter q,
+// output slot 2 nb + e of quarter q'), leading dimension = 4 (mod 16) doubles so that B-fragment loads are
+// conflict-free.
+//
+// Pass 2 differentiates the embedding net in forward mode: its input is the scalar s(r), so the tangent row
+// h' = dh/dx runs through the same GEMM chain as the value row (second m-block, same B fragments), and
+//   dE/dx = sum_o (dT R~)[o] g'[o],   dE/dR~[c] = sum_o dT[o][c] g[o]          (O9 of DESIGN.md / SURVEY.md §8(c)).
+#include "v1_kernels.cuh"
+
+#include <vector>
+
+#define EMB_WARPS 8
+#define EMB_THREADS (32 * EMB_WARPS)
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, const double a, const double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+      : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// tanh(x) = 1 - 2 / (exp(2x) + 1), exp through 2^n p(f); absolute error <= 5e-15 (measured against libdevice over
+// [-25, 25] and [-0.025, 0.025], profiles/r1_fp64_peaks.md).  About half the fp64-pipe slots of libdevice's tanh.
+__device__ __forceinline__ double dp_tanh(double x) {
+  double t = x * 2.8853900817779268;                 // 2 log2(e)
+  t = fmin(fmax(t, -64.0), 64.0);                    // beyond |x| > 22 the result is +-1 in fp64
+  const double tm = t + 6755399441055744.0;          // 1.5 * 2^52: rounds t to an integer, kept in the low word
+  const int ni = __double2loint(tm);
+  const double n = tm - 6755399441055744.0;
+  const double f = (t - n) * 0.6931471805599453;     // f ln 2 in [-0.347, 0.347]
+  double p = 2.505210838544172e-8;                   // Taylor of exp, degree 12 (remainder 1.7e-16)
+  p = fma(p, f, 2.755731922398589e-7);
+  p = fma(p, f, 2.7557319223985893e-6);
+  p = fma(p, f, 2.48015873015873e-5);
+  p = fma(p, f, 1.984126984126984e-4);
+  p = fma(p, f, 1.388888888888889e-3);
+  p = fma(p, f, 8.333333333333333e-3);
+  p = fma(p, f, 4.1666666666666664e-2);
+  p = fma(p, f, 1.6666666666666666e-1);
+  p = fma(p, f, 0.5);
+  p = fma(p, f, 1.0);
+  p = fma(p, f, 1.0);
+  const double e = __hiloint2double(__double2hiint(p) + ni * 1048576, __double2loint(p));
+  const double d = e + 1.0;
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+  double err = fma(-d, r, 1.0);
+  r = fma(r, err, r);
+  err = fma(-d, r, 1.0);
+  r = fma(r, err, r);
+  return fma(-2.0, r, 1.0);
+}
+
+template <int SP>
+struct EL {
+  static constexpr int S0 = SP, S1 = 2 * SP, S2 = 4 * SP;
+  static constexpr int NB1 = SP, NB2 = 2 * SP;
+  static constexpr int LD1 = 8 * NB1 + 4, LD2 = 8 * NB2 + 4;
+  static constexpr int oW0 = 0;                          // [4 SP]  position 4 s + q
+  static constexpr int ob0 = 4 * SP;                     // [4 SP]
+  static constexpr int oW1 = 8 * SP;                     // [4 SP][LD1]
+  static constexpr int ob1 = oW1 + 4 * SP * LD1;         // [8 NB1]
+  static constexpr int oW2 = ob1 + 8 * NB1;              // [8 SP][LD2]
+  static constexpr int ob2 = oW2 + 8 * SP * LD2;         // [8 NB2]
+  static constexpr int total = ob2 + 8 * NB2;
+  static constexpr int LDG = 8 * SP + 4;                 // leading dimension of the per-warp g tile (one N chunk)
+  static constexpr int tile1 = 16 * LDG + 16 * 4;        // pass 1, per warp: g tile [16][LDG] + env tile [16][4]
+  static constexpr int tile2 = 16 * SP * 4;              // pass 2, per warp: dT tile [16 SP][4]
+};
+
+static int sp_for(int s1) {
+  if (s1 <= 8) return 2;
+  if (s1 <= 16) return 4;
+  if (s1 <= 28) return 7;
+  if (s1 <= 32) return 8;
+  return 0;                                              // wider nets: variant 0 kernels
+}
+
+// feature index held by (quarter q, slot s) of a layer with `copies` copies of s1, or -1 for a pad
+static inline int feat_of(int q, int s, int SP, int s1, int copies) {
+  const int c = s / SP, r = (s % SP) * 4 + q;
+  if (c >= copies || r >= s1) return -1;
+  return c * s1 + r;
+}
+
+template <int SP>
+static void pack_net(const double *net, int s1, std::vector<double> &out) {
+  using L = EL<SP>;
+  out.assign(L::total, 0.0);
+  const double *W0 = net, *b0 = W0 + s1, *W1 = b0 + s1, *b1 = W1 + (size_t)s1 * 2 * s1, *W2 = b1 + 2 * s1,
+               *b2 = W2 + (size_t)2 * s1 * 4 * s1;
+  for (int s = 0; s < SP; ++s)
+    for (int q = 0; q < 4; ++q) {
+      const int f = feat_of(q, s, SP, s1, 1);
+      if (f >= 0) { out[L::oW0 + 4 * s + q] = W0[f]; out[L::ob0 + 4 * s + q] = b0[f]; }
+    }
+  for (int nb = 0; nb < L::NB1; ++nb)
+    for (int qo = 0; qo < 4; ++qo)
+      for (int e = 0; e < 2; ++e) {
+        const int fo = feat_of(qo, 2 * nb + e, SP, s1, 2), col = 8 * nb + 2 * qo + e;
+        if (fo < 0) continue;
+        out[L::ob1 + col] = b1[fo];
+        for (int ks = 0; ks < SP; ++ks)
+          for (int q = 0; q < 4; ++q) {
+            const int fi = feat_of(q, ks, SP, s1, 1);
+            if (fi >= 0) out[L::oW1 + (4 * ks + q) * L::LD1 + col] = W1[(size_t)fi * 2 * s1 + fo];
+          }
+      }
+  for (int nb = 0; nb < L::NB2; ++nb)
+    for (int qo = 0; qo < 4; ++qo)
+      for (int e = 0; e < 2; ++e) {
+        const int fo = feat_of(qo, 2 * nb + e, SP, s1, 4), col = 8 * nb + 2 * qo + e;
+        if (fo < 0) continue;
+        out[L::ob2 + col] = b2[fo];
+        for (int ks = 0; ks < 2 * SP; ++ks)
+          for (int q = 0; q < 4; ++q) {
+            const int fi = feat_of(q, ks, SP, s1, 2);
+            if (fi >= 0) out[L::oW2 + (4 * ks + q) * L::LD2 + col] = W2[(size_t)fi * 4 * s1 + fo];
+          }
+      }
+}
+
+cudaError_t v1_prepare_weights(const DevModel &P, const double *emb_h, const double *fit_h, V1Weights &W) {
+  (void)fit_h;
+  W.SP = sp_for(P.s1);
+  W.ready = false;
+  if (W.SP == 0) return cudaSuccess;
+  std::vector<double> one, all;
+  const int nets = P.ntypes * P.ntypes;
+  for (int k = 0; k < nets; ++k) {
+    const double *net = emb_h + (size_t)k * P.emb_net_size;
+    switch (W.SP) {
+      case 2: pack_net<2>(net, P.s1, one); break;
+      case 4: pack_net<4>(net, P.s1, one); break;
+      case 7: pack_net<7>(net, P.s1, one); break;
+      default: pack_net<8>(net, P.s1, one); break;
+    }
+    W.net_stride = (long long)one.size();
+    all.insert(all.end(), one.begin(), one.end());
+  }
+  cudaError_t e = cudaMalloc(&W.emb, sizeof(double) * all.size());
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(W.emb, all.data(), sizeof(double) * all.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  W.ready = true;
+  return cudaSuccess;
+}
+
+void v1_release_weights(V1Weights &W) {
+  if (W.emb) cudaFree(W.emb);
+  W.emb = nullptr;
+  W.ready = false;
+}
+
+// Env-matrix row (Eq. 5) from the stored (d, r) of a real slot.
+__device__ __forceinline__ void env_row4(const DevModel &P, const double4 v, double e[4]) {
+  double w, dw;
+  dp_switch(v.w, P.rcs, P.rc, w, dw);
+  const double ir = 1.0 / v.w;
+  const double s = w * ir;
+  const double sr = s * ir;
+  e[0] = s; e[1] = sr * v.x; e[2] = sr * v.y; e[3] = sr * v.z;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Pass 1.  One launch per (centre type a, neighbour type t): the CTA keeps net (a, t) in shared memory, each warp
+// takes atoms of type a round-robin and walks the real slots of section t in blocks of 16 rows (two m-blocks that
+// share every B fragment).  T_i is accumulated in registers (lane-owned features) through a per-warp g tile.
+template <int SP>
+__global__ void __launch_bounds__(EMB_THREADS, 1)
+k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate) {
+  using L = EL<SP>;
+  extern __shared__ __align__(16) double smem[];
+  double *W = smem;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
+  double *gt = smem + ((L::total + 1) & ~1) + warp * L::tile1;     // [16][LDG]
+  double *envt = gt + 16 * L::LDG;                                 // [16][4]
+  for (int k = tid; k < L::total; k += EMB_THREADS) W[k] = netp[k];
+  __syncthreads();
+  const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
+               *b2p = W + L::ob2;
+  const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
+  const int s1 = P.s1, M = P.M;
+
+  for (int qa = row_lo + blockIdx.x * EMB_WARPS + warp; qa < row_hi; qa += gridDim.x * EMB_WARPS) {
+    const int n = C.nreal[(size_t)qa * P.ntypes + t];
+    const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
+    double Tacc[2][2][4];
+#pragma unroll
+    for (int ch = 0; ch < 2; ++ch)
+#pragma unroll
+      for (int u = 0; u < 2; ++u)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) Tacc[ch][u][c] = 0.0;
+
+    for (int r0 = 0; r0 < n; r0 += 16) {
+      const bool second = r0 + 8 < n;                    // warp-uniform: the second m-block holds real rows
+      double x[2];
+#pragma unroll
+      for (int rb = 0; rb < 2; ++rb) {
+        const int row = r0 + g + 8 * rb;
+        double e[4] = {0.0, 0.0, 0.0, 0.0};
+        if (row < n) env_row4(P, dr[row], e);
+        x[rb] = e[0];
+        if (q == 0) {
+          double *dst = envt + (g + 8 * rb) * 4;
+          dst[0] = e[0]; dst[1] = e[1]; dst[2] = e[2]; dst[3] = e[3];
+        }
+      }
+      // layer 0 (Eq. 8): h0 = tanh(x W0 + b0)
+      double h0[2][SP];
+#pragma unroll
+      for (int s = 0; s < SP; ++s) {
+        const double w0 = W0p[4 * s + q], bb = b0p[4 * s + q];
+        h0[0][s] = dp_tanh(fma(x[0], w0, bb));
+        h0[1][s] = second ? dp_tanh(fma(x[1], w0, bb)) : 0.0;
+      }
+      // layer 1 (Eq. 9): h1 = (h0, h0) + tanh(h0 W1 + b1)
+      double h1[2][2 * SP];
+#pragma unroll
+      for (int nb = 0; nb < L::NB1; ++nb) {
+        const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
+        h1[0][2 * nb] = bb.x; h1[0][2 * nb + 1] = bb.y;
+        h1[1][2 * nb] = bb.x; h1[1][2 * nb + 1] = bb.y;
+      }
+#pragma unroll
+      for (int ks = 0; ks < SP; ++ks) {
+#pragma unroll
+        for (int nb = 0; nb < L::NB1; ++nb) {
+          const double b = W1p[(4 * ks + q) * L::LD1 + 8 * nb + g];
+          dmma884(h1[0][2 * nb], h1[0][2 * nb + 1], h0[0][ks], b);
+          if (second) dmma884(h1[1][2 * nb], h1[1][2 * nb + 1], h0[1][ks], b);
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < 2 * SP; ++s) h1[0][s] = h0[0][s % SP] + dp_tanh(h1[0][s]);
+      if (second) {
+#pragma unroll
+        for (int s = 0; s < 2 * SP; ++s) h1[1][s] = h0[1][s % SP] + dp_tanh(h1[1][s]);
+      }
+      // layer 2 (Eq. 9) in two N chunks of SP n-blocks: g = (h1, h1) + tanh(h1 W2 + b2); T += g (x) R~
+#pragma unroll
+      for (int ch = 0; ch < 2; ++ch) {
+        double acc[2][2 * SP];
+#pragma unroll
+        for (int nb = 0; nb < SP; ++nb) {
+          const double2 bb = *reinterpret_cast<const double2 *>(b2p + 8 * (ch * SP + nb) + 2 * q);
+          acc[0][2 * nb] = bb.x; acc[0][2 * nb + 1] = bb.y;
+          acc[1][2 * nb] = bb.x; acc[1][2 * nb + 1] = bb.y;
+        }
+#pragma unroll
+        for (int ks = 0; ks < 2 * SP; ++ks) {
+#pragma unroll
+          for (int nb = 0; nb < SP; ++nb) {
+            const double b = W2p[(4 * ks + q) * L::LD2 + 8 * (ch * SP + nb) + g];
+            dmma884(acc[0][2 * nb], acc[0][2 * nb + 1], h1[0][ks], b);
+            if (second) dmma884(acc[1][2 * nb], acc[1][2 * nb + 1], h1[1][ks], b);
+          }
+        }
+        __syncwarp();                                    // previous chunk's T update has finished reading gt
+        // slot ch*2SP + s of layer 2 takes its skip from slot s of layer 1 (same copy structure)
+#pragma unroll
+        for (int s = 0; s < 2 * SP; ++s) gt[g * L::LDG + 4 * s + q] = h1[0][s] + dp_tanh(acc[0][s]);
+        if (second) {
+#pragma unroll
+          for (int s = 0; s < 2 * SP; ++s) gt[(g + 8) * L::LDG + 4 * s + q] = h1[1][s] + dp_tanh(acc[1][s]);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          if (half == 1 && !second) break;
+#pragma unroll
+          for (int rr = 0; rr < 8; ++rr) {
+            const int row = 8 * half + rr;
+            const double4 e4a = *reinterpret_cast<const double4 *>(envt + row * 4);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+              const int p = lane + 32 * u;
+              if (p < 8 * SP) {
+                const double gv = gt[row * L::LDG + p];
+                Tacc[ch][u][0] = fma(gv, e4a.x, Tacc[ch][u][0]);
+                Tacc[ch][u][1] = fma(gv, e4a.y, Tacc[ch][u][1]);
+                Tacc[ch][u][2] = fma(gv, e4a.z, Tacc[ch][u][2]);
+                Tacc[ch][u][3] = fma(gv, e4a.w, Tacc[ch][u][3]);
+              }
+            }
+          }
+        }
+      }
+      __syncwarp();                                      // envt / gt are rewritten by the next row block
+    }
+    // T_i rows of the lane-owned features (position p = 4 s + q inside chunk ch)
+#pragma unroll
+    for (int ch = 0; ch < 2; ++ch)
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int p = lane + 32 * u;
+        if (p < 8 * SP) {
+          const int s = ch * 2 * SP + (p >> 2), qq = p & 3;
+          const int c = s / SP, r = (s % SP) * 4 + qq;
+          if (r < s1) {
+            double *dst = C.T + ((size_t)qa * M + c * s1 + r) * 4;
+            if (accumulate) {
+              dst[0] += Tacc[ch][u][0]; dst[1] += Tacc[ch][u][1]; dst[2] += Tacc[ch][u][2]; dst[3] += Tacc[ch][u][3];
+            } else {
+              dst[0] = Tacc[ch][u][0]; dst[1] = Tacc[ch][u][1]; dst[2] = Tacc[ch][u][2]; dst[3] = Tacc[ch][u][3];
+            }
+          }
+        }
+      }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Pass 2.  Same launch structure; per warp 8 neighbours at a time: m-block 0 carries the values, m-block 1 the
+// tangents d/dx.  Epilogue per N chunk: partial dots with the atom's dT tile (shared memory), quad reduction, then
+// one lane per neighbour chains to the displacement (O10) and scatters force / virial (O11).
+template <int SP>
+__global__ void __launch_bounds__(EMB_THREADS, 1)
+k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
+             double *__restrict__ virial) {
+  using L = EL<SP>;
+  extern __shared__ __align__(16) double smem[];
+  double *W = smem;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
+  double *dTt = smem + ((L::total + 1) & ~1) + warp * L::tile2;    // [16 SP][4], position 4 s + q
+  __shared__ double vred[EMB_WARPS][9];
+  for (int k = tid; k < L::total; k += EMB_THREADS) W[k] = netp[k];
+  __syncthreads();
+  const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
+               *b2p = W + L::ob2;
+  const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
+  const int s1 = P.s1, M = P.M;
+  double vir[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+
+  for (int qa = row_lo + blockIdx.x * EMB_WARPS + warp; qa < row_hi; qa += gridDim.x * EMB_WARPS) {
+    const int n = C.nreal[(size_t)qa * P.ntypes + t];
+    if (n == 0) continue;
+    const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
+    const int *nl = C.nl + (size_t)qa * P.nm + P.sec_start[t];
+    __syncwarp();
+    for (int p = lane; p < 16 * SP; p += 32) {
+      const int s = p >> 2, qq = p & 3;
+      const int c = s / SP, r = (s % SP) * 4 + qq;
+      double4 v = make_double4(0.0, 0.0, 0.0, 0.0);
+      if (r < s1) {
+        const double *src = C.dT + ((size_t)qa * M + c * s1 + r) * 4;
+        v = make_double4(src[0], src[1], src[2], src[3]);
+      }
+      *reinterpret_cast<double4 *>(dTt + 4 * p) = v;
+    }
+    __syncwarp();
+    double fi[3] = {0.0, 0.0, 0.0};
+
+    for (int r0 = 0; r0 < n; r0 += 8) {
+      const int row = r0 + g;
+      const bool valid = row < n;
+      double e[4] = {0.0, 0.0, 0.0, 0.0};
+      double4 dv = make_double4(0.0, 0.0, 0.0, 1.0);
+      if (valid) { dv = dr[row]; env_row4(P, dv, e); }
+      // layer 0 and its tangent: h0' = (1 - t0^2) W0   (d tanh = 1 - tanh^2)
+      double h0v[SP], h0t[SP];
+#pragma unroll
+      for (int s = 0; s < SP; ++s) {
+        const double w0 = W0p[4 * s + q], bb = b0p[4 * s + q];
+        const double t0 = dp_tanh(fma(e[0], w0, bb));
+        h0v[s] = t0;
+        h0t[s] = fma(-t0, t0, 1.0) * w0;
+      }
+      double h1v[2 * SP], h1t[2 * SP];
+#pragma unroll
+      for (int nb = 0; nb < L::NB1; ++nb) {
+        const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
+        h1v[2 * nb] = bb.x; h1v[2 * nb + 1] = bb.y;
+        h1t[2 * nb] = 0.0; h1t[2 * nb + 1] = 0.0;
+      }
+#pragma unroll
+      for (int ks = 0; ks < SP; ++ks) {
+#pragma unroll
+        for (int nb = 0; nb < L::NB1; ++nb) {
+          const double b = W1p[(4 * ks + q) * L::LD1 + 8 * nb + g];
+          dmma884(h1v[2 * nb], h1v[2 * nb + 1], h0v[ks], b);
+          dmma884(h1t[2 * nb], h1t[2 * nb + 1], h0t[ks], b);
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < 2 * SP; ++s) {
+        const double t1 = dp_tanh(h1v[s]);
+        h1v[s] = h0v[s % SP] + t1;
+        h1t[s] = fma(fma(-t1, t1, 1.0), h1t[s], h0t[s % SP]);
+      }
+      double pr[5] = {0.0, 0.0, 0.0, 0.0, 0.0};         // partial dR~[0..3], dx over this thread's features
+#pragma unroll
+      for (int ch = 0; ch < 2; ++ch) {
+        double av[2 * SP], at[2 * SP];
+#pragma unroll
+        for (int nb = 0; nb < SP; ++nb) {
+          const double2 bb = *reinterpret_cast<const double2 *>(b2p + 8 * (ch * SP + nb) + 2 * q);
+          av[2 * nb] = bb.x; av[2 * nb + 1] = bb.y;
+          at[2 * nb] = 0.0; at[2 * nb + 1] = 0.0;
+        }
+#pragma unroll
+        for (int ks = 0; ks < 2 * SP; ++ks) {
+#pragma unroll
+          for (int nb = 0; nb < SP; ++nb) {
+            const double b = W2p[(4 * ks + q) * L::LD2 + 8 * (ch * SP + nb) + g];
+            dmma884(av[2 * nb], av[2 * nb + 1], h1v[ks], b);
+            dmma884(at[2 * nb], at[2 * nb + 1], h1t[ks], b);
+          }
+        }
+#pragma unroll
+        for (int s = 0; s < 2 * SP; ++s) {
+          const double t2 = dp_tanh(av[s]);
+          const double gv = h1v[s] + t2;
+          const double gp = fma(fma(-t2, t2, 1.0), at[s], h1t[s]);
+          const double4 d4 = *reinterpret_cast<const double4 *>(dTt + 4 * (4 * (ch * 2 * SP + s) + q));
+          pr[0] = fma(d4.x, gv, pr[0]);
+          pr[1] = fma(d4.y, gv, pr[1]);
+          pr[2] = fma(d4.z, gv, pr[2]);
+          pr[3] = fma(d4.w, gv, pr[3]);
+          const double dg = fma(d4.x, e[0], fma(d4.y, e[1], fma(d4.z, e[2], d4.w * e[3])));
+          pr[4] = fma(dg, gp, pr[4]);
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        pr[k] += __shfl_xor_sync(0xffffffffu, pr[k], 1);
+        pr[k] += __shfl_xor_sync(0xffffffffu, pr[k], 2);
+      }
+      if (valid && q == 0) {
+        // O10: derivative of R~ with respect to the displacement; f_ik[c] = sum_m dR~[m] dR~_m / dd_c
+        const double r = dv.w, ir = 1.0 / r;
+        double w, dw;
+        dp_switch(r, P.rcs, P.rc, w, dw);
+        const double s = w * ir, qq = s * ir;
+        const double sp = dw * ir - w * ir * ir;
+        const double qp = sp * ir - s * ir * ir;
+        const double dR0 = pr[0] + pr[4];
+        const double dot = pr[1] * dv.x + pr[2] * dv.y + pr[3] * dv.z;
+        const double cm = (dR0 * sp + qp * dot) * ir;
+        const double f0 = fma(cm, dv.x, qq * pr[1]), f1 = fma(cm, dv.y, qq * pr[2]), f2 = fma(cm, dv.z, qq * pr[3]);
+        const int j = nl[row];
+        if (force) {
+          atomicAdd(&force[3 * (size_t)j + 0], -f0);
+          atomicAdd(&force[3 * (size_t)j + 1], -f1);
+          atomicAdd(&force[3 * (size_t)j + 2], -f2);
+        }
+        fi[0] += f0; fi[1] += f1; fi[2] += f2;
+        vir[0] -= dv.x * f0; vir[1] -= dv.x * f1; vir[2] -= dv.x * f2;
+        vir[3] -= dv.y * f0; vir[4] -= dv.y * f1; vir[5] -= dv.y * f2;
+        vir[6] -= dv.z * f0; vir[7] -= dv.z * f1; vir[8] -= dv.z * f2;
+      }
+    }
+    // F_i += sum_k f_ik (ProdForce)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      double v = fi[k];                                 // only the q == 0 lanes hold contributions
+      v += __shfl_xor_sync(0xffffffffu, v, 1);
+      v += __shfl_xor_sync(0xffffffffu, v, 2);
+      v += __shfl_xor_sync(0xffffffffu, v, 4);
+      v += __shfl_xor_sync(0xffffffffu, v, 8);
+      v += __shfl_xor_sync(0xffffffffu, v, 16);
+      fi[k] = v;
+    }
+    if (lane < 3 && force) atomicAdd(&force[3 * (size_t)C.s_idx[C.p0 + qa] + lane], lane == 0 ? fi[0] : (lane == 1 ? fi[1] : fi[2]));
+  }
+  // virial (ProdVirial): warp -> block -> one atomic per component and CTA
+#pragma unroll
+  for (int k = 0; k < 9; ++k) {
+    double v = vir[k];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if (lane == 0) vred[warp][k] = v;
+  }
+  __syncthreads();
+  if (tid < 9 && virial) {
+    double v = 0.0;
+    for (int w = 0; w < EMB_WARPS; ++w) v += vred[w][tid];
+    atomicAdd(&virial[tid], v);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static int g_sm_count = 0;
+
+template <int SP>
+static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weights &W, cudaStream_t st) {
+  using L = EL<SP>;
+  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + EMB_WARPS * L::tile1);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int grid = min(g_sm_count, (C.n + EMB_WARPS - 1) / EMB_WARPS);
+  for (int a = 0; a < P.ntypes; ++a)
+    for (int t = 0; t < P.ntypes; ++t) {
+      k_pass1_dmma<SP><<<grid, EMB_THREADS, smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
+                                                        t > 0);
+      DPB_LAUNCHED(1);
+    }
+  return cudaGetLastError();
+}
+
+template <int SP>
+static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weights &W, double *force, double *virial,
+                             cudaStream_t st) {
+  using L = EL<SP>;
+  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + EMB_WARPS * L::tile2);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int grid = min(g_sm_count, (C.n + EMB_WARPS - 1) / EMB_WARPS);
+  for (int a = 0; a < P.ntypes; ++a)
+    for (int t = 0; t < P.ntypes; ++t) {
+      k_pass2_dmma<SP><<<grid, EMB_THREADS, smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
+                                                        force, virial);
+      DPB_LAUNCHED(1);
+    }
+  return cudaGetLastError();
+}
+
+static cudaError_t ensure_sm_count() {
+  if (g_sm_count > 0) return cudaSuccess;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  return cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
+}
+
+cudaError_t v1_pass1(const DevModel &P, const ChunkView &C, const V1Weights &W, cudaStream_t st) {
+  if (C.n <= 0) return cudaSuccess;
+  if (!W.ready) return cudaErrorNotSupported;                  // api.cu routes nets wider than 32 to variant 0
+  cudaError_t e = ensure_sm_count();
+  if (e != cudaSuccess) return e;
+  switch (W.SP) {
+    case 2: return run_pass1<2>(P, C, W, st);
+    case 4: return run_pass1<4>(P, C, W, st);
+    case 7: return run_pass1<7>(P, C, W, st);
+    default: return run_pass1<8>(P, C, W, st);
+  }
+}
+
+cudaError_t v1_pass2(const DevModel &P, const ChunkView &C, const V1Weights &W, double *force, double *virial,
+                     cudaStream_t st) {
+  if (C.n <= 0) return cudaSuccess;
+  cudaError_t e = ensure_sm_count();
+  if (e != cudaSuccess) return e;
+  switch (W.SP) {
+    case 2: return run_pass2<2>(P, C, W, force, virial, st);
+    case 4: return run_pass2<4>(P, C, W, force, virial, st);
+    case 7: return run_pass2<7>(P, C, W, force, virial, st);
+    default: return run_pass2<8>(P, C, W, force, virial, st);
+  }
+}
