@@ -173,9 +173,10 @@ __device__ __forceinline__ void env_row4(const DevModel &P, const double4 v, dou
 
 // ---------------------------------------------------------------------------------------------------------
 // Pass 1.  One launch per (centre type a, neighbour type t): the CTA keeps net (a, t) in shared memory, each warp
-// takes atoms of type a round-robin and walks the real slots of section t in blocks of 16 rows (two m-blocks that
+// takes atoms of type a round-robin and walks the real slots of section t in blocks of 8 * RB rows (RB m-blocks that
 // share every B fragment).  T_i is accumulated in registers (lane-owned features) through a per-warp g tile.
-template <int SP>
+// RB = 1 keeps the fully unrolled loop body inside the instruction cache (RB = 2 measured 49 % stall_no_inst).
+template <int SP, int RB>
 __global__ void __launch_bounds__(EMB_THREADS, 1)
 k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate) {
   using L = EL<SP>;
@@ -202,11 +203,10 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 #pragma unroll
         for (int c = 0; c < 4; ++c) Tacc[ch][u][c] = 0.0;
 
-    for (int r0 = 0; r0 < n; r0 += 16) {
-      const bool second = r0 + 8 < n;                    // warp-uniform: the second m-block holds real rows
-      double x[2];
+    for (int r0 = 0; r0 < n; r0 += 8 * RB) {
+      double x[RB];
 #pragma unroll
-      for (int rb = 0; rb < 2; ++rb) {
+      for (int rb = 0; rb < RB; ++rb) {
         const int row = r0 + g + 8 * rb;
         double e[4] = {0.0, 0.0, 0.0, 0.0};
         if (row < n) env_row4(P, dr[row], e);
@@ -217,81 +217,72 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         }
       }
       // layer 0 (Eq. 8): h0 = tanh(x W0 + b0)
-      double h0[2][SP];
+      double h0[RB][SP];
 #pragma unroll
       for (int s = 0; s < SP; ++s) {
         const double w0 = W0p[4 * s + q], bb = b0p[4 * s + q];
-        h0[0][s] = dp_tanh(fma(x[0], w0, bb));
-        h0[1][s] = second ? dp_tanh(fma(x[1], w0, bb)) : 0.0;
+#pragma unroll
+        for (int rb = 0; rb < RB; ++rb) h0[rb][s] = dp_tanh(fma(x[rb], w0, bb));
       }
       // layer 1 (Eq. 9): h1 = (h0, h0) + tanh(h0 W1 + b1)
-      double h1[2][2 * SP];
+      double h1[RB][2 * SP];
 #pragma unroll
       for (int nb = 0; nb < L::NB1; ++nb) {
         const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
-        h1[0][2 * nb] = bb.x; h1[0][2 * nb + 1] = bb.y;
-        h1[1][2 * nb] = bb.x; h1[1][2 * nb + 1] = bb.y;
+#pragma unroll
+        for (int rb = 0; rb < RB; ++rb) { h1[rb][2 * nb] = bb.x; h1[rb][2 * nb + 1] = bb.y; }
       }
 #pragma unroll
       for (int ks = 0; ks < SP; ++ks) {
 #pragma unroll
         for (int nb = 0; nb < L::NB1; ++nb) {
           const double b = W1p[(4 * ks + q) * L::LD1 + 8 * nb + g];
-          dmma884(h1[0][2 * nb], h1[0][2 * nb + 1], h0[0][ks], b);
-          if (second) dmma884(h1[1][2 * nb], h1[1][2 * nb + 1], h0[1][ks], b);
+#pragma unroll
+          for (int rb = 0; rb < RB; ++rb) dmma884(h1[rb][2 * nb], h1[rb][2 * nb + 1], h0[rb][ks], b);
         }
       }
 #pragma unroll
-      for (int s = 0; s < 2 * SP; ++s) h1[0][s] = h0[0][s % SP] + dp_tanh(h1[0][s]);
-      if (second) {
+      for (int s = 0; s < 2 * SP; ++s)
 #pragma unroll
-        for (int s = 0; s < 2 * SP; ++s) h1[1][s] = h0[1][s % SP] + dp_tanh(h1[1][s]);
-      }
+        for (int rb = 0; rb < RB; ++rb) h1[rb][s] = h0[rb][s % SP] + dp_tanh(h1[rb][s]);
       // layer 2 (Eq. 9) in two N chunks of SP n-blocks: g = (h1, h1) + tanh(h1 W2 + b2); T += g (x) R~
 #pragma unroll
       for (int ch = 0; ch < 2; ++ch) {
-        double acc[2][2 * SP];
+        double acc[RB][2 * SP];
 #pragma unroll
         for (int nb = 0; nb < SP; ++nb) {
           const double2 bb = *reinterpret_cast<const double2 *>(b2p + 8 * (ch * SP + nb) + 2 * q);
-          acc[0][2 * nb] = bb.x; acc[0][2 * nb + 1] = bb.y;
-          acc[1][2 * nb] = bb.x; acc[1][2 * nb + 1] = bb.y;
+#pragma unroll
+          for (int rb = 0; rb < RB; ++rb) { acc[rb][2 * nb] = bb.x; acc[rb][2 * nb + 1] = bb.y; }
         }
 #pragma unroll
         for (int ks = 0; ks < 2 * SP; ++ks) {
 #pragma unroll
           for (int nb = 0; nb < SP; ++nb) {
             const double b = W2p[(4 * ks + q) * L::LD2 + 8 * (ch * SP + nb) + g];
-            dmma884(acc[0][2 * nb], acc[0][2 * nb + 1], h1[0][ks], b);
-            if (second) dmma884(acc[1][2 * nb], acc[1][2 * nb + 1], h1[1][ks], b);
+#pragma unroll
+            for (int rb = 0; rb < RB; ++rb) dmma884(acc[rb][2 * nb], acc[rb][2 * nb + 1], h1[rb][ks], b);
           }
         }
         __syncwarp();                                    // previous chunk's T update has finished reading gt
         // slot ch*2SP + s of layer 2 takes its skip from slot s of layer 1 (same copy structure)
 #pragma unroll
-        for (int s = 0; s < 2 * SP; ++s) gt[g * L::LDG + 4 * s + q] = h1[0][s] + dp_tanh(acc[0][s]);
-        if (second) {
+        for (int s = 0; s < 2 * SP; ++s)
 #pragma unroll
-          for (int s = 0; s < 2 * SP; ++s) gt[(g + 8) * L::LDG + 4 * s + q] = h1[1][s] + dp_tanh(acc[1][s]);
-        }
+          for (int rb = 0; rb < RB; ++rb) gt[(g + 8 * rb) * L::LDG + 4 * s + q] = h1[rb][s] + dp_tanh(acc[rb][s]);
         __syncwarp();
 #pragma unroll
-        for (int half = 0; half < 2; ++half) {
-          if (half == 1 && !second) break;
+        for (int row = 0; row < 8 * RB; ++row) {
+          const double4 e4a = *reinterpret_cast<const double4 *>(envt + row * 4);
 #pragma unroll
-          for (int rr = 0; rr < 8; ++rr) {
-            const int row = 8 * half + rr;
-            const double4 e4a = *reinterpret_cast<const double4 *>(envt + row * 4);
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-              const int p = lane + 32 * u;
-              if (p < 8 * SP) {
-                const double gv = gt[row * L::LDG + p];
-                Tacc[ch][u][0] = fma(gv, e4a.x, Tacc[ch][u][0]);
-                Tacc[ch][u][1] = fma(gv, e4a.y, Tacc[ch][u][1]);
-                Tacc[ch][u][2] = fma(gv, e4a.z, Tacc[ch][u][2]);
-                Tacc[ch][u][3] = fma(gv, e4a.w, Tacc[ch][u][3]);
-              }
+          for (int u = 0; u < 2; ++u) {
+            const int p = lane + 32 * u;
+            if (p < 8 * SP) {
+              const double gv = gt[row * L::LDG + p];
+              Tacc[ch][u][0] = fma(gv, e4a.x, Tacc[ch][u][0]);
+              Tacc[ch][u][1] = fma(gv, e4a.y, Tacc[ch][u][1]);
+              Tacc[ch][u][2] = fma(gv, e4a.z, Tacc[ch][u][2]);
+              Tacc[ch][u][3] = fma(gv, e4a.w, Tacc[ch][u][3]);
             }
           }
         }
@@ -500,14 +491,14 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
   const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + EMB_WARPS * L::tile1);
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
   const int grid = min(g_sm_count, (C.n + EMB_WARPS - 1) / EMB_WARPS);
   for (int a = 0; a < P.ntypes; ++a)
     for (int t = 0; t < P.ntypes; ++t) {
-      k_pass1_dmma<SP><<<grid, EMB_THREADS, smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
+      k_pass1_dmma<SP, 1><<<grid, EMB_THREADS, smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
                                                         t > 0);
       DPB_LAUNCHED(1);
     }
