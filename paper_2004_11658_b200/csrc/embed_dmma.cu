@@ -130,10 +130,13 @@ static void pack_net(const double *net, int s1, std::vector<double> &out) {
 }
 
 cudaError_t v1_prepare_weights(const DevModel &P, const double *emb_h, const double *fit_h, V1Weights &W) {
-  (void)fit_h;
   W.SP = sp_for(P.s1);
   W.ready = false;
   if (W.SP == 0) return cudaSuccess;
+  {
+    cudaError_t ef = v1_prepare_fit(P, fit_h, W);
+    if (ef != cudaSuccess) return ef;
+  }
   std::vector<double> one, all;
   const int nets = P.ntypes * P.ntypes;
   for (int k = 0; k < nets; ++k) {
@@ -156,6 +159,7 @@ cudaError_t v1_prepare_weights(const DevModel &P, const double *emb_h, const dou
 }
 
 void v1_release_weights(V1Weights &W) {
+  v1_release_fit(W);
   if (W.emb) cudaFree(W.emb);
   W.emb = nullptr;
   W.ready = false;

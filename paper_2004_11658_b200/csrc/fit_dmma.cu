@@ -1,25 +1,356 @@
-// fit_dmma.cu — variant 1 of S5 (D = T T^<T), S6 (fitting net forward), S7 (fitting backward + dT).
-// TEMPORARY: routes to the variant-0 GEMM kernels until the DMMA fitting kernels land.
+// fit_dmma.cu — variant 1 of S5 (D = T T^<T), S6 (fitting net forward, Eq. 2-3) and S7 (fitting
+// backward + dT): six GEMMs per species on fp64 tensor-core tiles (DMMA m8n8k4) with the activation,
+// skip and d tanh = 1 - tanh^2 work fused into the epilogues:
+//   G1  Z0 = tanh(D W0 + b0)                                   [rows x dim] [dim x w]
+//   G2  U1 = tanh(Z0 W1 + b1),  Z1 = Z0 + U1
+//   G3  U2 = tanh(Z1 W2 + b2),  Z2 = Z1 + U2,  Q2 = w3 (1 - U2^2)          E_i = Z2 . w3 + b3 (row dot)
+//   G4  dZ1 = w3 + Q2 W2^T,     Q1 = dZ1 (1 - U1^2)
+//   G5  dZ0 = dZ1 + Q1 W1^T,    Q0 = dZ0 (1 - Z0^2)
+//   G6  dD = Q0 W0^T                                           [rows x w] [w x dim]
+// Weights are re-laid-out once at model creation: zero-padded to multiples of 16, 16-byte aligned, and the
+// transposes are stored explicitly so that every GEMM reads a row-major B.  Rows = the chunk's atoms of one species
+// (a contiguous range of sorted positions, read from the device: no host synchronisation).
+//
+// Kernel: CTA tile 64 rows x (16 NBW) columns, 8 warps as 4 (rows) x 2 (columns), warp tile 16 x (8 NBW): two
+// m-blocks share every B fragment, one A fragment feeds NBW n-blocks.  K tiles of 16 through a 3-stage cp.async
+// pipeline; shared-memory leading dimensions are 4 (mod 16) doubles, which makes the fragment loads conflict-free.
 #include "v1_kernels.cuh"
 
+#include <vector>
+
+#define FIT_BM 64
+#define FIT_BK 16
+#define FIT_STAGES 3
+#define FIT_LDA (FIT_BK + 4)
+
+struct FitNet {            // device pointers into the padded fitting weights of one species
+  const double *W0, *b0, *W1, *b1, *W2, *b2, *w3, *W0T, *W1T, *W2T;
+  double b3;
+};
+
+struct FitWeights {
+  double *buf = nullptr;
+  int fwp = 0, dimp = 0;
+  std::vector<FitNet> nets;
+};
+
+__device__ __forceinline__ void dmma884f(double &c0, double &c1, const double a, const double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+      : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc, bool valid) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  const int sz = valid ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gsrc), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+enum { EPI_TANH = 0, EPI_TANH_SKIP = 1, EPI_L3 = 2, EPI_BWD = 3, EPI_STORE = 4 };
+
+struct GemmArgs {
+  const double *A; int lda;          // [rows][lda], K columns used
+  const double *B; int ldb;          // [K][ldb] row-major, N columns used
+  int K, N;                          // multiples of 16 / 8
+  const double *bias;                // [N] or null
+  const double *in0; const double *in1; int ldi;
+  double *out0; double *out1; int ldo;
+};
+
+template <int NBW, int EPI>
+__global__ void __launch_bounds__(256, 1)
+k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
+  constexpr int BN = 16 * NBW, LDB = BN + 4;
+  extern __shared__ __align__(16) double smem[];
+  double *As = smem;                                        // [STAGES][BM][LDA]
+  double *Bs = smem + FIT_STAGES * FIT_BM * FIT_LDA;        // [STAGES][BK][LDB]
+  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  const int m0 = row_lo + blockIdx.x * FIT_BM;
+  if (m0 >= row_hi) return;
+  const int n0 = blockIdx.y * BN;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gq = lane >> 2, q = lane & 3;
+  const int wm = warp >> 1, wn = warp & 1;                  // warp tile: rows 16 wm .., cols 8 NBW wn ..
+  const int nkt = g.K / FIT_BK;
+
+  auto load_tile = [&](int kt, int stage) {
+    double *as = As + stage * FIT_BM * FIT_LDA;
+    double *bs = Bs + stage * FIT_BK * LDB;
+    const int k0 = kt * FIT_BK;
+    for (int c = tid; c < FIT_BM * (FIT_BK / 2); c += 256) {
+      const int m = c >> 3, kk = (c & 7) * 2;
+      const bool ok = m0 + m < row_hi;
+      cp_async16(as + m * FIT_LDA + kk, g.A + (size_t)(ok ? m0 + m : m0) * g.lda + k0 + kk, ok);
+    }
+    for (int c = tid; c < FIT_BK * (BN / 2); c += 256) {
+      const int k = c / (BN / 2), nn = (c - k * (BN / 2)) * 2;
+      const bool ok = n0 + nn < g.N;
+      cp_async16(bs + k * LDB + nn, g.B + (size_t)(k0 + k) * g.ldb + (ok ? n0 + nn : 0), ok);
+    }
+  };
+
+  double acc[2][NBW][2];
+#pragma unroll
+  for (int mb = 0; mb < 2; ++mb)
+#pragma unroll
+    for (int nb = 0; nb < NBW; ++nb) { acc[mb][nb][0] = 0.0; acc[mb][nb][1] = 0.0; }
+
+#pragma unroll
+  for (int s = 0; s < FIT_STAGES - 1; ++s) {
+    if (s < nkt) load_tile(s, s);
+    cp_async_commit();
+  }
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_async_wait<FIT_STAGES - 2>();
+    __syncthreads();
+    {
+      const int nk = kt + FIT_STAGES - 1;
+      if (nk < nkt) load_tile(nk, nk % FIT_STAGES);
+      cp_async_commit();
+    }
+    const double *as = As + (kt % FIT_STAGES) * FIT_BM * FIT_LDA + (16 * wm + gq) * FIT_LDA + q;
+    const double *bs = Bs + (kt % FIT_STAGES) * FIT_BK * LDB + q * LDB + 8 * NBW * wn + gq;
+#pragma unroll
+    for (int ks = 0; ks < FIT_BK / 4; ++ks) {
+      const double a0 = as[4 * ks], a1 = as[8 * FIT_LDA + 4 * ks];
+#pragma unroll
+      for (int nb = 0; nb < NBW; ++nb) {
+        const double b = bs[4 * ks * LDB + 8 * nb];
+        dmma884f(acc[0][nb][0], acc[0][nb][1], a0, b);
+        dmma884f(acc[1][nb][0], acc[1][nb][1], a1, b);
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  // epilogue: thread (gq, q) holds rows 16 wm + gq (+8), columns n0 + 8 NBW wn + 8 nb + 2 q (+1)
+#pragma unroll
+  for (int mb = 0; mb < 2; ++mb) {
+    const int m = m0 + 16 * wm + gq + 8 * mb;
+    if (m >= row_hi) continue;
+#pragma unroll
+    for (int nb = 0; nb < NBW; ++nb) {
+      const int n = n0 + 8 * NBW * wn + 8 * nb + 2 * q;
+      if (n >= g.N) continue;
+      double v0 = acc[mb][nb][0], v1 = acc[mb][nb][1];
+      const size_t oi = (size_t)m * g.ldi + n, oo = (size_t)m * g.ldo + n;
+      if (EPI == EPI_TANH) {
+        const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
+        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(tanh(v0 + b.x), tanh(v1 + b.y));
+      } else if (EPI == EPI_TANH_SKIP) {
+        const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
+        const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi);
+        const double u0 = tanh(v0 + b.x), u1 = tanh(v1 + b.y);
+        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(u0, u1);
+        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(z.x + u0, z.y + u1);
+      } else if (EPI == EPI_L3) {
+        // bias = b2, in1 = w3 (as a [N] vector), in0 = Z1: out1 = Z2 = Z1 + U2, out0 = Q2 = w3 (1 - U2^2)
+        const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
+        const double2 w = *reinterpret_cast<const double2 *>(g.in1 + n);
+        const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi);
+        const double u0 = tanh(v0 + b.x), u1 = tanh(v1 + b.y);
+        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(z.x + u0, z.y + u1);
+        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(w.x * (1.0 - u0 * u0), w.y * (1.0 - u1 * u1));
+      } else if (EPI == EPI_BWD) {
+        // dz = acc + bias[n] (w3, first backward step) + in0 (dZ of the next layer); out0 = dz; out1 = dz (1 - in1^2)
+        if (g.bias) { const double2 b = *reinterpret_cast<const double2 *>(g.bias + n); v0 += b.x; v1 += b.y; }
+        if (g.in0) { const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi); v0 += z.x; v1 += z.y; }
+        const double2 u = *reinterpret_cast<const double2 *>(g.in1 + oi);
+        if (g.out0) *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0, v1);
+        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(v0 * (1.0 - u.x * u.x), v1 * (1.0 - u.y * u.y));
+      } else {
+        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0, v1);
+      }
+    }
+  }
+}
+
+// S5: D[b][a] = sum_c T[b][c] T[a][c] (Eq. 4; flatten b M^< + a, reading R7), zero-padded to dimp.
+__global__ void k_descr_v1(DevModel P, ChunkView C, int dimp, double *__restrict__ D) {
+  const int q = blockIdx.x;
+  __shared__ double Ts[1024 + 16];
+  const double *T = C.T + (size_t)q * P.M * 4;
+  for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
+  __syncthreads();
+  for (int e = threadIdx.x; e < dimp; e += blockDim.x) {
+    double acc = 0.0;
+    if (e < P.dim) {
+      const int b = e / P.Ma, a = e - b * P.Ma;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) acc += Ts[b * 4 + c] * Ts[a * 4 + c];
+    }
+    D[(size_t)q * dimp + e] = acc;
+  }
+}
+
+// S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c].
+__global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restrict__ dD) {
+  const int q = blockIdx.x;
+  extern __shared__ double sm2[];
+  double *Ts = sm2;                 // [M][4]
+  double *dd = sm2 + P.M * 4;       // [dim]
+  const double *T = C.T + (size_t)q * P.M * 4;
+  for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
+  for (int k = threadIdx.x; k < P.dim; k += blockDim.x) dd[k] = dD[(size_t)q * dimp + k];
+  __syncthreads();
+  for (int e = threadIdx.x; e < P.M * 4; e += blockDim.x) {
+    const int b = e >> 2, c = e & 3;
+    double acc = 0.0;
+    for (int a = 0; a < P.Ma; ++a) acc += dd[b * P.Ma + a] * Ts[a * 4 + c];
+    if (b < P.Ma)
+      for (int bp = 0; bp < P.M; ++bp) acc += dd[bp * P.Ma + b] * Ts[bp * 4 + c];
+    C.dT[(size_t)q * P.M * 4 + e] = acc;
+  }
+}
+
+// E_i = Z2 . w3 + b3 (output layer, reading R4): one warp per atom.
+__global__ void k_rowdot_v1(ChunkView C, int ty, int fwp, const double *__restrict__ Z2, const double *__restrict__ w3,
+                            double b3, double *__restrict__ atom_energy) {
+  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  const int q = row_lo + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (q >= row_hi) return;
+  const int lane = threadIdx.x & 31;
+  double s = 0.0;
+  for (int o = lane; o < fwp; o += 32) s += Z2[(size_t)q * fwp + o] * w3[o];
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0) atom_energy[C.s_idx[C.p0 + q]] = s + b3;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// The padded fitting weights hang off V1Weights::fit (opaque pointer declared in v1_kernels.cuh).
+cudaError_t v1_prepare_fit(const DevModel &P, const double *fit_h, V1Weights &W) {
+  FitWeights *F = new FitWeights();
+  const int fw = P.fw, dim = P.dim, fwp = round_up(fw, 16), dimp = round_up(dim, 16);
+  F->fwp = fwp; F->dimp = dimp;
+  const size_t per = (size_t)dimp * fwp * 2 + (size_t)fwp * fwp * 4 + 4 * (size_t)fwp;
+  std::vector<double> h(per * P.ntypes, 0.0);
+  std::vector<size_t> off;
+  for (int ty = 0; ty < P.ntypes; ++ty) {
+    const double *W0 = fit_h + (size_t)ty * P.fit_net_size;
+    const double *b0 = W0 + (size_t)dim * fw, *W1 = b0 + fw, *b1 = W1 + (size_t)fw * fw, *W2 = b1 + fw,
+                 *b2 = W2 + (size_t)fw * fw, *w3 = b2 + fw;
+    double *base = h.data() + per * ty;
+    double *pW0 = base, *pW0T = pW0 + (size_t)dimp * fwp, *pW1 = pW0T + (size_t)dimp * fwp,
+           *pW1T = pW1 + (size_t)fwp * fwp, *pW2 = pW1T + (size_t)fwp * fwp, *pW2T = pW2 + (size_t)fwp * fwp,
+           *pb0 = pW2T + (size_t)fwp * fwp, *pb1 = pb0 + fwp, *pb2 = pb1 + fwp, *pw3 = pb2 + fwp;
+    for (int d = 0; d < dim; ++d)
+      for (int o = 0; o < fw; ++o) {
+        pW0[(size_t)d * fwp + o] = W0[(size_t)d * fw + o];
+        pW0T[(size_t)o * dimp + d] = W0[(size_t)d * fw + o];
+      }
+    for (int a = 0; a < fw; ++a)
+      for (int o = 0; o < fw; ++o) {
+        pW1[(size_t)a * fwp + o] = W1[(size_t)a * fw + o];
+        pW1T[(size_t)o * fwp + a] = W1[(size_t)a * fw + o];
+        pW2[(size_t)a * fwp + o] = W2[(size_t)a * fw + o];
+        pW2T[(size_t)o * fwp + a] = W2[(size_t)a * fw + o];
+      }
+    for (int o = 0; o < fw; ++o) { pb0[o] = b0[o]; pb1[o] = b1[o]; pb2[o] = b2[o]; pw3[o] = w3[o]; }
+  }
+  cudaError_t e = cudaMalloc(&F->buf, sizeof(double) * h.size());
+  if (e != cudaSuccess) { delete F; return e; }
+  e = cudaMemcpy(F->buf, h.data(), sizeof(double) * h.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(F->buf); delete F; return e; }
+  for (int ty = 0; ty < P.ntypes; ++ty) {
+    const double *base = F->buf + per * ty;
+    FitNet n;
+    n.W0 = base; n.W0T = n.W0 + (size_t)dimp * fwp; n.W1 = n.W0T + (size_t)dimp * fwp;
+    n.W1T = n.W1 + (size_t)fwp * fwp; n.W2 = n.W1T + (size_t)fwp * fwp; n.W2T = n.W2 + (size_t)fwp * fwp;
+    n.b0 = n.W2T + (size_t)fwp * fwp; n.b1 = n.b0 + fwp; n.b2 = n.b1 + fwp; n.w3 = n.b2 + fwp;
+    n.b3 = fit_h[(size_t)ty * P.fit_net_size + P.fit_net_size - 1];
+    F->nets.push_back(n);
+  }
+  W.fit = F;
+  return cudaSuccess;
+}
+
+void v1_release_fit(V1Weights &W) {
+  FitWeights *F = reinterpret_cast<FitWeights *>(W.fit);
+  if (F) {
+    if (F->buf) cudaFree(F->buf);
+    delete F;
+  }
+  W.fit = nullptr;
+}
+
 size_t v1_workspace_bytes(const DevModel &P, int64_t chunk) {
-  return sizeof(double) * (size_t)chunk * (2 * (size_t)P.dim + 7 * (size_t)P.fw) + 256;
+  const size_t fwp = round_up(P.fw, 16), dimp = round_up(P.dim, 16);
+  return sizeof(double) * (size_t)chunk * (2 * dimp + 6 * fwp) + 256;
+}
+
+template <int NBW, int EPI>
+static cudaError_t gemm(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st) {
+  constexpr int BN = 16 * NBW;
+  const size_t smem = sizeof(double) * FIT_STAGES * (FIT_BM * FIT_LDA + FIT_BK * (BN + 4));
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_fit_gemm<NBW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid((C.n + FIT_BM - 1) / FIT_BM, (g.N + BN - 1) / BN);
+  k_fit_gemm<NBW, EPI><<<grid, 256, smem, st>>>(C, ty, g);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
 }
 
 cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, const double *fit, void *ws,
                    double *atom_energy, cudaStream_t st) {
-  (void)W;
-  double *p = reinterpret_cast<double *>(ws);
+  (void)fit;
+  if (C.n <= 0) return cudaSuccess;
+  const FitWeights *F = reinterpret_cast<const FitWeights *>(W.fit);
+  if (!F) return cudaErrorNotSupported;
+  const int fwp = F->fwp, dimp = F->dimp;
   const size_t n = (size_t)C.n;
-  V0Scratch S;
-  S.D = p; p += n * P.dim;
-  S.dD = p; p += n * P.dim;
-  S.Z0 = p; p += n * P.fw;
-  S.U1 = p; p += n * P.fw;
-  S.Z1 = p; p += n * P.fw;
-  S.U2 = p; p += n * P.fw;
-  S.Z2 = p; p += n * P.fw;
-  S.G = p; p += n * P.fw;
-  S.dZ = p;
-  return launch_fit_v0(P, C, fit, S, atom_energy, nullptr, st);
+  double *p = reinterpret_cast<double *>(ws);
+  double *D = p; p += n * dimp;          // later reused as dD's input? no: dD has its own buffer
+  double *dD = p; p += n * dimp;
+  double *Z0 = p; p += n * fwp;
+  double *U1 = p; p += n * fwp;
+  double *Z1 = p; p += n * fwp;          // later dZ1
+  double *Z2 = p; p += n * fwp;
+  double *Q = p; p += n * fwp;           // Q2, then Q1 (ping-pong with Q')
+  double *Q2 = p;                        // second Q buffer
+  cudaError_t e;
+
+  k_descr_v1<<<C.n, 256, 0, st>>>(P, C, dimp, D);
+  DPB_LAUNCHED(1);
+  for (int ty = 0; ty < P.ntypes; ++ty) {
+    const FitNet &N = F->nets[ty];
+    GemmArgs g;
+    // G1: Z0 = tanh(D W0 + b0)
+    g = GemmArgs{D, dimp, N.W0, fwp, dimp, fwp, N.b0, nullptr, nullptr, fwp, Z0, nullptr, fwp};
+    if ((e = gemm<15, EPI_TANH>(C, ty, g, st)) != cudaSuccess) return e;
+    // G2: U1 = tanh(Z0 W1 + b1); Z1 = Z0 + U1
+    g = GemmArgs{Z0, fwp, N.W1, fwp, fwp, fwp, N.b1, Z0, nullptr, fwp, U1, Z1, fwp};
+    if ((e = gemm<15, EPI_TANH_SKIP>(C, ty, g, st)) != cudaSuccess) return e;
+    // G3: U2 = tanh(Z1 W2 + b2); Z2 = Z1 + U2; Q = w3 (1 - U2^2)
+    g = GemmArgs{Z1, fwp, N.W2, fwp, fwp, fwp, N.b2, Z1, N.w3, fwp, Q, Z2, fwp};
+    if ((e = gemm<15, EPI_L3>(C, ty, g, st)) != cudaSuccess) return e;
+    k_rowdot_v1<<<(C.n + 7) / 8, 256, 0, st>>>(C, ty, fwp, Z2, N.w3, N.b3, atom_energy);
+    DPB_LAUNCHED(1);
+    // G4: dZ1 = w3 + Q W2^T (-> Z1 buffer); Q' = dZ1 (1 - U1^2)
+    g = GemmArgs{Q, fwp, N.W2T, fwp, fwp, fwp, N.w3, nullptr, U1, fwp, Z1, Q2, fwp};
+    if ((e = gemm<15, EPI_BWD>(C, ty, g, st)) != cudaSuccess) return e;
+    // G5: dZ0 = dZ1 + Q' W1^T; Q = dZ0 (1 - Z0^2)
+    g = GemmArgs{Q2, fwp, N.W1T, fwp, fwp, fwp, nullptr, Z1, Z0, fwp, nullptr, Q, fwp};
+    if ((e = gemm<15, EPI_BWD>(C, ty, g, st)) != cudaSuccess) return e;
+    // G6: dD = Q W0^T
+    g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
+    if ((e = gemm<8, EPI_STORE>(C, ty, g, st)) != cudaSuccess) return e;
+  }
+  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + P.dim);
+  static size_t configured = 0;
+  if (sm > 48 * 1024 && sm > configured) {
+    e = cudaFuncSetAttribute(k_dT_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    configured = sm;
+  }
+  k_dT_v1<<<C.n, 256, sm, st>>>(P, C, dimp, dD);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
 }

@@ -8,7 +8,11 @@ struct V1Weights {
   long long net_stride = 0;   // doubles per padded net
   int SP = 0;                 // feature slots per lane quarter and copy: ceil(s1 / 4)
   bool ready = false;
+  void *fit = nullptr;        // padded fitting weights (fit_dmma.cu)
 };
+
+cudaError_t v1_prepare_fit(const DevModel &P, const double *fit_h, V1Weights &W);
+void v1_release_fit(V1Weights &W);
 
 cudaError_t v1_prepare_weights(const DevModel &P, const double *emb_h, const double *fit_h, V1Weights &W);
 void v1_release_weights(V1Weights &W);
