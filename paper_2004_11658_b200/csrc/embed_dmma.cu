@@ -28,35 +28,35 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, const double a, 
       : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// tanh(x) = 1 - 2 / (exp(2x) + 1), exp through 2^n p(f); absolute error <= 5e-15 (measured against libdevice over
-// [-25, 25] and [-0.025, 0.025], profiles/r1_fp64_peaks.md).  About half the fp64-pipe slots of libdevice's tanh.
+// tanh(x) = 1 - 2 / (exp(2x) + 1) with exp(2x) = 2^n 2^f: n = rint(2x log2 e) by the 1.5 * 2^52 trick, 2^f by a
+// degree-10 polynomial on [-0.5, 0.5] (relative error 2.9e-16), the reciprocal from MUFU.RCP64H refined by one cubic
+// step.  19 fp64-pipe instructions; absolute error <= 4.5e-16 against libdevice on [-25, 25], [-1, 1], [-0.01, 0.01]
+// and [-1e-6, 1e-6] (4e7 points each, profiles/r1_fp64_peaks.md); libdevice's tanh costs 2.2x the pipe slots.
 __device__ __forceinline__ double dp_tanh(double x) {
-  double t = x * 2.8853900817779268;                 // 2 log2(e)
-  t = fmin(fmax(t, -64.0), 64.0);                    // beyond |x| > 22 the result is +-1 in fp64
-  const double tm = t + 6755399441055744.0;          // 1.5 * 2^52: rounds t to an integer, kept in the low word
+  const int hi = __double2hiint(x);
+  const bool big = (hi & 0x7fffffff) >= 0x40340000;                 // |x| >= 20: tanh = +-1 in fp64
+  const double xc = big ? __hiloint2double((hi & 0x80000000) | 0x40340000, 0) : x;
+  const double t = xc * 2.8853900817779268;                          // 2 log2(e)
+  const double tm = t + 6755399441055744.0;                          // 1.5 * 2^52
   const int ni = __double2loint(tm);
-  const double n = tm - 6755399441055744.0;
-  const double f = (t - n) * 0.6931471805599453;     // f ln 2 in [-0.347, 0.347]
-  double p = 2.505210838544172e-8;                   // Taylor of exp, degree 12 (remainder 1.7e-16)
-  p = fma(p, f, 2.755731922398589e-7);
-  p = fma(p, f, 2.7557319223985893e-6);
-  p = fma(p, f, 2.48015873015873e-5);
-  p = fma(p, f, 1.984126984126984e-4);
-  p = fma(p, f, 1.388888888888889e-3);
-  p = fma(p, f, 8.333333333333333e-3);
-  p = fma(p, f, 4.1666666666666664e-2);
-  p = fma(p, f, 1.6666666666666666e-1);
-  p = fma(p, f, 0.5);
+  const double f = t - (tm - 6755399441055744.0);
+  double p = 7.0725859492692236999e-9;
+  p = fma(p, f, 1.0208690299958305835e-7);
+  p = fma(p, f, 1.3215442587921689653e-6);
+  p = fma(p, f, 0.000015252657260200837064);
+  p = fma(p, f, 0.00015403530441736050155);
+  p = fma(p, f, 0.0013333558230164973899);
+  p = fma(p, f, 0.0096181291076068885273);
+  p = fma(p, f, 0.055504108664447719166);
+  p = fma(p, f, 0.2402265069591009822);
+  p = fma(p, f, 0.69314718055994998286);
   p = fma(p, f, 1.0);
-  p = fma(p, f, 1.0);
-  const double e = __hiloint2double(__double2hiint(p) + ni * 1048576, __double2loint(p));
-  const double d = e + 1.0;
+  const double d = __hiloint2double(__double2hiint(p) + ni * 1048576, __double2loint(p)) + 1.0;
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-  double err = fma(-d, r, 1.0);
-  r = fma(r, err, r);
-  err = fma(-d, r, 1.0);
-  r = fma(r, err, r);
+  const double err = fma(-d, r, 1.0);
+  const double tq = fma(err, err, err);
+  r = fma(r, tq, r);
   return fma(-2.0, r, 1.0);
 }
 
