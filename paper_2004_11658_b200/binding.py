@@ -41,7 +41,8 @@ class EvalInfo:
 
 
 def lib_path() -> str:
-    return os.path.join(HERE, "libdpb.so")
+    # DPB_LIBRARY selects another build of the same library (kernel-tuning experiments); default: the in-tree build
+    return os.environ.get("DPB_LIBRARY") or os.path.join(HERE, "libdpb.so")
 
 
 _LIB = None

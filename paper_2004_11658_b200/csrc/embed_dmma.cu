@@ -20,8 +20,12 @@
 
 #include <vector>
 
-#define EMB_WARPS 8
-#define EMB_THREADS (32 * EMB_WARPS)
+#ifndef P1_WARPS
+#define P1_WARPS 8            // warps per CTA, pass 1
+#endif
+#ifndef P2_WARPS
+#define P2_WARPS 8            // warps per CTA, pass 2
+#endif
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, const double a, const double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -73,7 +77,8 @@ struct EL {
   static constexpr int ob2 = oW2 + 8 * SP * LD2;         // [8 NB2]
   static constexpr int total = ob2 + 8 * NB2;
   static constexpr int LDG = 8 * SP + 4;                 // leading dimension of the per-warp g tile (one N chunk)
-  static constexpr int tile1 = 16 * LDG + 16 * 4;        // pass 1, per warp: g tile [16][LDG] + env tile [16][4]
+  static constexpr int tile1 = 16 * LDG + 16 * 4;        // pass 1, per warp: g tile [16][LDG] + env tile [16][4] (RB = 2)
+  static constexpr int tile1s = 8 * LDG + 8 * 4;         // same for RB = 1
   static constexpr int tile2 = 16 * SP * 4;              // pass 2, per warp: dT tile [16 SP][4]
 };
 
@@ -181,22 +186,22 @@ __device__ __forceinline__ void env_row4(const DevModel &P, const double4 v, dou
 // share every B fragment).  T_i is accumulated in registers (lane-owned features) through a per-warp g tile.
 // RB = 1 keeps the fully unrolled loop body inside the instruction cache (RB = 2 measured 49 % stall_no_inst).
 template <int SP, int RB>
-__global__ void __launch_bounds__(EMB_THREADS, 1)
+__global__ void __launch_bounds__((32 * P1_WARPS), 1)
 k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate) {
   using L = EL<SP>;
   extern __shared__ __align__(16) double smem[];
   double *W = smem;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
-  double *gt = smem + ((L::total + 1) & ~1) + warp * L::tile1;     // [16][LDG]
-  double *envt = gt + 16 * L::LDG;                                 // [16][4]
-  for (int k = tid; k < L::total; k += EMB_THREADS) W[k] = netp[k];
+  double *gt = smem + ((L::total + 1) & ~1) + warp * (RB == 1 ? L::tile1s : L::tile1);     // [8 RB][LDG]
+  double *envt = gt + 8 * RB * L::LDG;                             // [8 RB][4]
+  for (int k = tid; k < L::total; k += (32 * P1_WARPS)) W[k] = netp[k];
   __syncthreads();
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
   const int s1 = P.s1, M = P.M;
 
-  for (int qa = row_lo + blockIdx.x * EMB_WARPS + warp; qa < row_hi; qa += gridDim.x * EMB_WARPS) {
+  for (int qa = row_lo + blockIdx.x * P1_WARPS + warp; qa < row_hi; qa += gridDim.x * P1_WARPS) {
     const int n = C.nreal[(size_t)qa * P.ntypes + t];
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
     double Tacc[2][2][4];
@@ -320,7 +325,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 // tangents d/dx.  Epilogue per N chunk: partial dots with the atom's dT tile (shared memory), quad reduction, then
 // one lane per neighbour chains to the displacement (O10) and scatters force / virial (O11).
 template <int SP>
-__global__ void __launch_bounds__(EMB_THREADS, 1)
+__global__ void __launch_bounds__((32 * P2_WARPS), 1)
 k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
              double *__restrict__ virial) {
   using L = EL<SP>;
@@ -328,8 +333,8 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   double *W = smem;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
   double *dTt = smem + ((L::total + 1) & ~1) + warp * L::tile2;    // [16 SP][4], position 4 s + q
-  __shared__ double vred[EMB_WARPS][9];
-  for (int k = tid; k < L::total; k += EMB_THREADS) W[k] = netp[k];
+  __shared__ double vred[P2_WARPS][9];
+  for (int k = tid; k < L::total; k += (32 * P2_WARPS)) W[k] = netp[k];
   __syncthreads();
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
@@ -339,7 +344,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 #pragma unroll
   for (int k = 0; k < 9; ++k) vir[k] = 0.0;
 
-  for (int qa = row_lo + blockIdx.x * EMB_WARPS + warp; qa < row_hi; qa += gridDim.x * EMB_WARPS) {
+  for (int qa = row_lo + blockIdx.x * P2_WARPS + warp; qa < row_hi; qa += gridDim.x * P2_WARPS) {
     const int n = C.nreal[(size_t)qa * P.ntypes + t];
     if (n == 0) continue;
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
@@ -481,7 +486,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   __syncthreads();
   if (tid < 9 && virial) {
     double v = 0.0;
-    for (int w = 0; w < EMB_WARPS; ++w) v += vred[w][tid];
+    for (int w = 0; w < P2_WARPS; ++w) v += vred[w][tid];
     atomicAdd(&virial[tid], v);
   }
 }
@@ -492,17 +497,17 @@ static int g_sm_count = 0;
 template <int SP>
 static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weights &W, cudaStream_t st) {
   using L = EL<SP>;
-  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + EMB_WARPS * L::tile1);
+  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P1_WARPS * L::tile1s);
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  const int grid = min(g_sm_count, (C.n + EMB_WARPS - 1) / EMB_WARPS);
+  const int grid = min(g_sm_count, (C.n + P1_WARPS - 1) / P1_WARPS);
   for (int a = 0; a < P.ntypes; ++a)
     for (int t = 0; t < P.ntypes; ++t) {
-      k_pass1_dmma<SP, 1><<<grid, EMB_THREADS, smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
+      k_pass1_dmma<SP, 1><<<grid, (32 * P1_WARPS), smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
                                                         t > 0);
       DPB_LAUNCHED(1);
     }
@@ -513,17 +518,17 @@ template <int SP>
 static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weights &W, double *force, double *virial,
                              cudaStream_t st) {
   using L = EL<SP>;
-  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + EMB_WARPS * L::tile2);
+  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * L::tile2);
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  const int grid = min(g_sm_count, (C.n + EMB_WARPS - 1) / EMB_WARPS);
+  const int grid = min(g_sm_count, (C.n + P2_WARPS - 1) / P2_WARPS);
   for (int a = 0; a < P.ntypes; ++a)
     for (int t = 0; t < P.ntypes; ++t) {
-      k_pass2_dmma<SP><<<grid, EMB_THREADS, smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
+      k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
                                                         force, virial);
       DPB_LAUNCHED(1);
     }

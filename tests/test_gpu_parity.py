@@ -258,3 +258,53 @@ def test_eval_host_matches_device_entry():
     assert np.abs(host["force"] - dev["force"]).max() <= 1e-12
     assert abs(host["energy"][0] - dev["energy"][0]) <= 1e-12 * abs(dev["energy"][0])
     m.close()
+
+
+def test_config5_copper_864k_sampled():
+    """BASELINE configs[4]: 864,000-atom copper box (27 chunks of 32,768 atoms).  Sampled rows against the oracle
+    (nlist bit-exact, E_i), conservation laws, and extensivity: the box is NOT a replica of config 2 (independent
+    jitter), so extensivity is checked on E / N against the 32,000-atom box only loosely (same lattice, same model)."""
+    torch = _torch()
+    spec = MODELS["Cu864k"]
+    coord, types, box = gen.make_system("Cu864k")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, 1)
+    dc = torch.tensor(coord, device="cuda")
+    dt = torch.tensor(types, device="cuda")
+    out = m.eval(dc, dt, box, want_nlist=True, want_info=True)
+    torch.cuda.synchronize()
+    info = out["info"]
+    assert info.n_overflow == 0 and info.n_chunks == 27
+    rows = np.random.default_rng(2).choice(coord.shape[0], 12, replace=False).astype(np.int64)
+    nl_ref, _ = orc.build_nlist(coord, types, box, rows=rows)
+    nl = out["nlist"][torch.tensor(rows, device="cuda")].cpu().numpy()
+    assert np.array_equal(nl, nl_ref)
+    ar = orc.atom_rows(coord, types, box, rows, nl_ref)
+    ei = out["atom_energy"].cpu().numpy()
+    assert np.abs(ei[rows] - ar["atom_energy"]).max() <= E_REL * np.abs(ar["atom_energy"]).max()
+    f = out["force"].cpu().numpy()
+    assert np.abs(f.sum(0)).max() <= 1e-9
+    v = out["virial"].cpu().numpy()
+    assert np.abs(v - v.T).max() <= 1e-9 * np.abs(v).max()
+    assert abs(out["energy"].item() - ei.sum()) <= 1e-11 * np.abs(ei).sum()
+    m.close()
+
+
+def test_replication_extensivity_gpu():
+    """A 2x2x2 periodic replication gives exactly 8 E and replicated forces (PBC + cell list + chunking), here with
+    a chunk size that does not divide the atom count."""
+    torch = _torch()
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    _, m = _models(spec, emb, fit, 1)
+    small = _gpu_eval(m, coord, types, box)
+    big_c, big_t, big_b = gen.replicate(coord, types, box, 2)
+    m.set_chunk(500)
+    big = _gpu_eval(m, big_c, big_t, big_b)
+    assert abs(big["energy"][0] - 8 * small["energy"][0]) <= 1e-11 * abs(8 * small["energy"][0])
+    assert np.abs(big["force"].reshape(8, -1, 3) - small["force"][None]).max() <= 1e-10
+    assert np.abs(big["virial"] - 8 * small["virial"]).max() <= 1e-10 * np.abs(8 * small["virial"]).max()
+    m.close()
