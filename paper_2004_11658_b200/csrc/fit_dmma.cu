@@ -184,22 +184,34 @@ __global__ void k_descr_v1(DevModel P, ChunkView C, int dimp, double *__restrict
   }
 }
 
-// S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c].
+// S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c].  The second term (M^< x 4 outputs, M terms
+// each) is split over all threads in partial sums so that it does not serialise behind M^< x 4 threads.
 __global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restrict__ dD) {
   const int q = blockIdx.x;
   extern __shared__ double sm2[];
-  double *Ts = sm2;                 // [M][4]
-  double *dd = sm2 + P.M * 4;       // [dim]
+  double *Ts = sm2;                      // [M][4]
+  double *dd = sm2 + P.M * 4;            // [dim]
+  double *part = dd + P.dim;             // [nparts][Ma * 4]
   const double *T = C.T + (size_t)q * P.M * 4;
   for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
   for (int k = threadIdx.x; k < P.dim; k += blockDim.x) dd[k] = dD[(size_t)q * dimp + k];
+  __syncthreads();
+  const int nout2 = P.Ma * 4;
+  const int nparts = max(1, (int)blockDim.x / nout2);
+  for (int idx = threadIdx.x; idx < nparts * nout2; idx += blockDim.x) {
+    const int pt = idx / nout2, o = idx - pt * nout2, bcol = o >> 2, c = o & 3;
+    const int per = (P.M + nparts - 1) / nparts, lo = pt * per, hi = min(P.M, lo + per);
+    double acc = 0.0;
+    for (int bp = lo; bp < hi; ++bp) acc += dd[bp * P.Ma + bcol] * Ts[bp * 4 + c];
+    part[idx] = acc;
+  }
   __syncthreads();
   for (int e = threadIdx.x; e < P.M * 4; e += blockDim.x) {
     const int b = e >> 2, c = e & 3;
     double acc = 0.0;
     for (int a = 0; a < P.Ma; ++a) acc += dd[b * P.Ma + a] * Ts[a * 4 + c];
     if (b < P.Ma)
-      for (int bp = 0; bp < P.M; ++bp) acc += dd[bp * P.Ma + b] * Ts[bp * 4 + c];
+      for (int pt = 0; pt < nparts; ++pt) acc += part[pt * nout2 + e];
     C.dT[(size_t)q * P.M * 4 + e] = acc;
   }
 }
@@ -343,7 +355,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
     if ((e = gemm<8, EPI_STORE>(C, ty, g, st)) != cudaSuccess) return e;
   }
-  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + P.dim);
+  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + P.dim + 256 + 4 * P.Ma);
   static size_t configured = 0;
   if (sm > 48 * 1024 && sm > configured) {
     e = cudaFuncSetAttribute(k_dT_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);

@@ -8,6 +8,29 @@
 // The displacement uses dp_displacement (reading R2) on a cell-sorted COPY of the raw coordinates (same bits).
 #include "common.cuh"
 
+// dp_displacement with the division and the square root skipped where their result is known in advance — the
+// values produced are bit-identical to the pinned sequence (reading R2):
+//   |d| < 0.4999 L          =>  |RN(d / L)| < 0.5            =>  k = rint(d / L) = 0
+//   0.5001 L < |d| < 1.4999 L  =>  0.5 < |RN(d / L)| < 1.5   =>  k = +-1
+//   r2 > rc^2 (1 + 1e-9)    =>  sqrt(r2) > rc                =>  not a neighbour, r is not needed (returns false)
+__device__ __forceinline__ bool displacement_in_range(const double xi[3], const double xj[3], const double L[3],
+                                                      double rc2_hi, double d[3], double &r) {
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const double dc = __dsub_rn(xj[c], xi[c]);
+    const double a = fabs(dc);
+    double k;
+    if (a < 0.4999 * L[c]) k = 0.0;
+    else if (a > 0.5001 * L[c] && a < 1.4999 * L[c]) k = copysign(1.0, dc);
+    else k = rint(__ddiv_rn(dc, L[c]));
+    d[c] = __fma_rn(-k, L[c], dc);
+  }
+  const double r2 = __fma_rn(d[2], d[2], __fma_rn(d[1], d[1], __dmul_rn(d[0], d[0])));
+  if (r2 > rc2_hi) return false;
+  r = __dsqrt_rn(r2);
+  return true;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 __global__ void k_keys(DevModel P, DevGrid G, int n, const double *__restrict__ coord, const int *__restrict__ type,
                        int *__restrict__ key, int *__restrict__ count, DevStats *stats) {
@@ -111,7 +134,9 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   const int i = C.s_idx[p];
   const double xi[3] = {s_xyz[3 * (size_t)p], s_xyz[3 * (size_t)p + 1], s_xyz[3 * (size_t)p + 2]};
 
-  if (tid == 0) {
+  // stencil ranges: one thread per (type, stencil cell), then a serial compaction of the <= 27 ntypes entries
+  __shared__ int c_start[NL_MAX_RANGES], c_cnt[NL_MAX_RANGES];
+  for (int ent = tid; ent < 27 * P.ntypes; ent += NL_THREADS) {
     // cell of atom i, recomputed exactly as in k_keys
     int ic[3], lo[3], num[3];
 #pragma unroll
@@ -123,21 +148,30 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
       ic[c] = v >= G.nc[c] ? G.nc[c] - 1 : v;
       if (G.lo_mode[c]) { lo[c] = ic[c] - 1; num[c] = 3; } else { lo[c] = 0; num[c] = G.nc[c]; }
     }
+    const int t = ent / 27, w = ent - 27 * t;
+    const int a = w / 9, b = (w / 3) % 3, c = w % 3;
+    int cntv = 0, s0 = 0;
+    if (a < num[0] && b < num[1] && c < num[2]) {      // fewer than 3 cells in a dimension: each cell once
+      const int ja = (lo[0] + a + G.nc[0]) % G.nc[0];
+      const int jb = (lo[1] + b + G.nc[1]) % G.nc[1];
+      const int jc = (lo[2] + c + G.nc[2]) % G.nc[2];
+      const int k = t * G.ncell + (ja * G.nc[1] + jb) * G.nc[2] + jc;
+      s0 = start[k];
+      cntv = start[k + 1] - s0;
+    }
+    c_start[ent] = s0;
+    c_cnt[ent] = cntv;
+  }
+  __syncthreads();
+  if (tid == 0) {
     int nr = 0, run = 0;
-    for (int t = 0; t < P.ntypes; ++t)
-      for (int a = 0; a < num[0]; ++a)
-        for (int b = 0; b < num[1]; ++b)
-          for (int c = 0; c < num[2]; ++c) {
-            int ja = (lo[0] + a + G.nc[0]) % G.nc[0];
-            int jb = (lo[1] + b + G.nc[1]) % G.nc[1];
-            int jc = (lo[2] + c + G.nc[2]) % G.nc[2];
-            int k = t * G.ncell + (ja * G.nc[1] + jb) * G.nc[2] + jc;
-            int s0 = start[k], s1 = start[k + 1];
-            if (s1 > s0) {
-              r_start[nr] = s0; r_pref[nr] = run; r_type[nr] = t;
-              run += s1 - s0; ++nr;
-            }
-          }
+    for (int e = 0; e < 27 * P.ntypes; ++e) {
+      const int cv = c_cnt[e];
+      if (cv > 0) {
+        r_start[nr] = c_start[e]; r_pref[nr] = run; r_type[nr] = e / 27;
+        run += cv; ++nr;
+      }
+    }
     r_pref[nr] = run;
     n_ranges = nr;
     n_hit = 0;
@@ -145,6 +179,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   }
   __syncthreads();
 
+  const double rc2_hi = P.rc * P.rc * (1.0 + 1e-9);
   const int ncand = r_pref[n_ranges];
   int rp = 0;
   for (int c = tid; c < ncand; c += NL_THREADS) {
@@ -153,8 +188,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
     if (pj == p) continue;                                         // j != i (reading R19)
     const double xj[3] = {s_xyz[3 * (size_t)pj], s_xyz[3 * (size_t)pj + 1], s_xyz[3 * (size_t)pj + 2]};
     double d[3], r;
-    dp_displacement(xi, xj, G.L, d, r);
-    if (r <= P.rc) {                                               // "<=" as printed, PAPER.md:80 (reading R9)
+    if (displacement_in_range(xi, xj, G.L, rc2_hi, d, r) && r <= P.rc) {   // "<=" as printed, PAPER.md:80 (R9)
       const int t = r_type[rp];
       atomicAdd(&cnt[t], 1);
       const int h = atomicAdd(&n_hit, 1);
