@@ -11,6 +11,7 @@
 
 #include "common.cuh"
 #include "v1_kernels.cuh"
+#include "tc_kernels.cuh"
 
 static thread_local char g_err[512] = "";
 
@@ -51,11 +52,13 @@ struct dpb_model {
   int device = 0;
   Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
   V1Weights v1;                 // re-laid-out weights of the fused kernels
+  TCWeights tcw;                // mixed precision: TF32 hi / lo operand images (embed_tc.cu)
   // workspace
   Buf key, count, start, cursor, s_idx, s_xyz, stats, ei;
   Buf nl, dr, nreal, T, dT;
   Buf v0[9];
   Buf v1ws;
+  Buf pairs;                    // mixed precision: flattened real-slot lists of the chunk
   Buf h_coord, h_type, h_out;   // device staging of dpb_eval_host
   double *dbgT = nullptr, *dbgD = nullptr, *dbgdT = nullptr;
   std::vector<cudaEvent_t> evs;   // stage timers: [0] start, [1] after S1, then 4 per chunk, then the end
@@ -69,7 +72,8 @@ extern "C" int dpb_model_nm(const dpb_model *m) { return m ? nm_of(m->P) : DPB_E
 extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_model **out) {
   if (!d || !out) return fail(DPB_EINVAL, "dpb_model_create: null argument");
   *out = nullptr;
-  if (precision != DPB_FP64) return fail(DPB_ENOTIMPL, "dpb_model_create: only DPB_FP64 is built");
+  if (precision != DPB_FP64 && precision != DPB_TF32)
+    return fail(DPB_ENOTIMPL, "dpb_model_create: precision must be DPB_FP64 or DPB_TF32 (DPB_BF16 is not built)");
   if (d->ntypes < 1 || d->ntypes > DPB_MAX_TYPES) return fail(DPB_EINVAL, "ntypes must be in [1, %d]", DPB_MAX_TYPES);
   if (!d->sel || !d->emb_weights || !d->fit_weights) return fail(DPB_EINVAL, "null sel / weights");
   if (d->emb_s1 < 1 || d->emb_s1 > 64) return fail(DPB_EINVAL, "emb_s1 must be in [1, 64]");
@@ -103,6 +107,14 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
   if (e == cudaSuccess) e = cudaMemcpy(m->emb.p, d->emb_weights, eb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(m->fit.p, d->fit_weights, fb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = v1_prepare_weights(P, d->emb_weights, d->fit_weights, m->v1);
+  m->precision = precision;
+  if (e == cudaSuccess && precision == DPB_TF32) {
+    e = tc_prepare_weights(P, d->emb_weights, m->tcw);
+    if (e == cudaErrorNotSupported || !m->v1.ready) {
+      dpb_model_destroy(m);
+      return fail(DPB_ENOTIMPL, "DPB_TF32 is built for emb_s1 in {8, 16, 25, 32} (got %d)", d->emb_s1);
+    }
+  }
   if (e != cudaSuccess) {
     int code = (e == cudaErrorMemoryAllocation) ? DPB_ENOMEM : DPB_ECUDA;
     dpb_model_destroy(m);
@@ -115,10 +127,11 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->h_coord, &m->h_type, &m->h_out};
+                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->h_coord, &m->h_type, &m->h_out};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
+  tc_release_weights(m->tcw);
   for (cudaEvent_t &e : m->evs) cudaEventDestroy(e);
   delete m;
   return DPB_OK;
@@ -235,13 +248,14 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   if (!nlist_only) {
     CU(m->T.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
     CU(m->dT.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
-    if (m->variant == 0 || !m->v1.ready) {
+    if (m->precision == DPB_FP64 && (m->variant == 0 || !m->v1.ready)) {
       CU(m->v0[0].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
       CU(m->v0[1].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
       for (int k = 2; k < 9; ++k) CU(m->v0[k].reserve(sizeof(double) * (size_t)chunk * P.fw), "workspace");
     } else {
       CU(m->v1ws.reserve(v1_workspace_bytes(P, chunk)), "workspace");
     }
+    if (m->precision == DPB_TF32) CU(m->pairs.reserve(tc_pair_workspace_bytes(P, chunk)), "workspace");
   }
   DevStats *stats = m->stats.as<DevStats>();
   CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");
@@ -284,7 +298,16 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st), "nlist");
     if (nlist_only) continue;
     if (timing) cudaEventRecord(m->evs[2 + 4 * ci], st);
-    if (m->variant == 0 || !m->v1.ready) {
+    if (m->precision == DPB_TF32) {
+      CU(tc_build_pairs(P, C, m->pairs.p, st), "pair list");
+      CU(tc_pass1(P, C, m->tcw, m->pairs.p, st), "pass1 tf32");
+      if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);
+      CU(v1_fit(P, C, m->v1, m->fit.as<double>(), m->v1ws.p, ei, st), "fit");
+      CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
+      if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
+      CU(v1_pass2(P, C, m->v1, force, virial, st), "pass2");
+      if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
+    } else if (m->variant == 0 || !m->v1.ready) {
       V0Scratch S;
       S.D = m->v0[0].as<double>(); S.dD = m->v0[1].as<double>();
       S.Z0 = m->v0[2].as<double>(); S.U1 = m->v0[3].as<double>(); S.Z1 = m->v0[4].as<double>();

@@ -1,0 +1,381 @@
+// embed_tc.cu — mixed-precision (DPB_TF32) embedding passes on the 5th-generation tensor cores (BASELINE.json
+// configs[3]).  S3-S5 (pass 1) and S8-S9 (pass 2) of the hot path:
+//   * env matrix R~ (Eq. 5), the chain to the displacement (O10), and every accumulation of T, F, Xi stay in fp64;
+//   * the embedding GEMMs (Eq. 8-9) run as tcgen05.mma kind::tf32 with fp32 accumulators in TMEM,
+//     operands split x = hi + lo (3xTF32, tc_common.cuh) so that the contraction is accurate to fp32 rounding;
+//   * tanh in fp32 (ex2.approx / rcp.approx).
+// Work decomposition: the real (non-padded) slots of section t of all centre atoms of type a are flattened into one
+// pair list (k_pair_scan / k_pair_expand); a tile is 128 consecutive pairs = the 128 TMEM lanes; thread r of a
+// warpgroup owns row r through the whole net (layer outputs come back with tcgen05.ld 32x32b, one row per thread,
+// so the concat skip [x || x] of Eq. 9 is a register add).  Two warpgroups per CTA work on independent tiles (own
+// 64 KB operand slot, own TMEM columns, own mbarrier): while one waits for its MMAs the other runs its tanh epilogue.
+#include <cstring>
+#include <vector>
+
+#include "tc_common.cuh"
+#include "tc_kernels.cuh"
+
+template <int S1>
+struct TL {
+  static constexpr int N1 = (2 * S1 + 7) / 8 * 8, N2 = (4 * S1 + 7) / 8 * 8;
+  static constexpr int KS1 = (S1 + 7) / 8, KS2 = (2 * S1 + 7) / 8, PAN2 = (KS2 + 3) / 4;
+  static constexpr int W1B = N1 * 128, W2P = N2 * 128, W2B = PAN2 * W2P;       // bytes of one hi (or lo) image
+  static constexpr int oW1h = 0, oW1l = W1B, oW2h = 2 * W1B, oW2l = 2 * W1B + W2B, oVec = 2 * W1B + 2 * W2B;
+  static constexpr int vW0 = 0, vb0 = 32, vb1 = 64, vb2 = 64 + N1, nvec = 64 + N1 + N2;          // floats
+  static constexpr int img_bytes = (oVec + 4 * nvec + 1023) / 1024 * 1024;
+  static constexpr int SLOT = 65536;                       // per-warpgroup operand slot
+  static constexpr int oSlot = img_bytes, oEnv = oSlot + 2 * SLOT, oIds = oEnv + 2 * 128 * 32,
+                       oBar = oIds + 2 * 128 * 4, oTmem = oBar + 16, smem_bytes = oTmem + 16;
+  static_assert(S1 <= 32, "layer-1 operand is one 32-wide panel");
+  static_assert(N2 <= 128 && PAN2 <= 2, "layer-2 operand: two 32-wide panels, 128 output columns");
+};
+
+// ---- host: pack one net into its shared-memory image ---------------------------------------------------------
+template <int S1>
+static void pack_net_tc(const double *net, std::vector<float> &out) {
+  using L = TL<S1>;
+  out.assign(L::img_bytes / 4, 0.0f);
+  const double *W0 = net, *b0 = W0 + S1, *W1 = b0 + S1, *b1 = W1 + (size_t)S1 * 2 * S1, *W2 = b1 + 2 * S1,
+               *b2 = W2 + (size_t)2 * S1 * 4 * S1;
+  auto put = [&](int byte_base, int n, int k, double w) {
+    const float hi = tc_host_tf32((float)w);
+    const float lo = tc_host_tf32((float)(w - (double)hi));
+    (void)lo;
+    out[(byte_base + tc::sw128_offset(n, k)) / 4] = hi;
+  };
+  auto put_lo = [&](int byte_base, int n, int k, double w) {
+    const float hi = tc_host_tf32((float)w);
+    out[(byte_base + tc::sw128_offset(n, k)) / 4] = tc_host_tf32((float)(w - (double)hi));
+  };
+  for (int k = 0; k < S1; ++k)
+    for (int n = 0; n < 2 * S1; ++n) {
+      put(L::oW1h, n, k, W1[(size_t)k * 2 * S1 + n]);
+      put_lo(L::oW1l, n, k, W1[(size_t)k * 2 * S1 + n]);
+    }
+  for (int k = 0; k < 2 * S1; ++k)
+    for (int n = 0; n < 4 * S1; ++n) {
+      const int pan = k / 32, kk = k % 32;
+      put(L::oW2h + pan * L::W2P, n, kk, W2[(size_t)k * 4 * S1 + n]);
+      put_lo(L::oW2l + pan * L::W2P, n, kk, W2[(size_t)k * 4 * S1 + n]);
+    }
+  float *vec = out.data() + L::oVec / 4;
+  for (int s = 0; s < S1; ++s) { vec[L::vW0 + s] = (float)W0[s]; vec[L::vb0 + s] = (float)b0[s]; }
+  for (int o = 0; o < 2 * S1; ++o) vec[L::vb1 + o] = (float)b1[o];
+  for (int o = 0; o < 4 * S1; ++o) vec[L::vb2 + o] = (float)b2[o];
+}
+
+static bool tc_supported_s1(int s1) { return s1 == 8 || s1 == 16 || s1 == 25 || s1 == 32; }
+
+cudaError_t tc_prepare_weights(const DevModel &P, const double *emb_h, TCWeights &W) {
+  W.ready = false;
+  if (!tc_supported_s1(P.s1)) return cudaErrorNotSupported;
+  std::vector<float> one, all;
+  const int nets = P.ntypes * P.ntypes;
+  for (int k = 0; k < nets; ++k) {
+    const double *net = emb_h + (size_t)k * P.emb_net_size;
+    switch (P.s1) {
+      case 8: pack_net_tc<8>(net, one); break;
+      case 16: pack_net_tc<16>(net, one); break;
+      case 25: pack_net_tc<25>(net, one); break;
+      default: pack_net_tc<32>(net, one); break;
+    }
+    W.net_stride = one.size();
+    all.insert(all.end(), one.begin(), one.end());
+  }
+  cudaError_t e = cudaMalloc(&W.emb, sizeof(float) * all.size());
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(W.emb, all.data(), sizeof(float) * all.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  W.ready = true;
+  return cudaSuccess;
+}
+
+void tc_release_weights(TCWeights &W) {
+  if (W.emb) cudaFree(W.emb);
+  W.emb = nullptr;
+  W.ready = false;
+}
+
+// ---- pair list -----------------------------------------------------------------------------------------------
+// off[t][q] = number of real slots of section t over the chunk's atoms before sorted position q (q in [0, n]).
+__global__ void __launch_bounds__(1024) k_pair_scan(int n, int ntypes, const int *__restrict__ nreal, int *__restrict__ off) {
+  const int t = blockIdx.x, tid = threadIdx.x;
+  __shared__ int part[1024];
+  const int per = (n + 1023) / 1024, lo = min(n, tid * per), hi = min(n, lo + per);
+  int s = 0;
+  for (int q = lo; q < hi; ++q) s += nreal[(size_t)q * ntypes + t];
+  part[tid] = s;
+  __syncthreads();
+  for (int d = 1; d < 1024; d <<= 1) {
+    const int v = tid >= d ? part[tid - d] : 0;
+    __syncthreads();
+    part[tid] += v;
+    __syncthreads();
+  }
+  int run = part[tid] - s;
+  int *o = off + (size_t)t * (n + 1);
+  for (int q = lo; q < hi; ++q) { o[q] = run; run += nreal[(size_t)q * ntypes + t]; }
+  if (tid == 1023) o[n] = part[1023];
+}
+
+// pidx[n sec_start[t] + off[t][q] + k] = q Nm + sec_start[t] + k  for every real slot k of section t of atom q.
+__global__ void k_pair_expand(DevModel P, int n, const int *__restrict__ nreal, const int *__restrict__ off,
+                              int *__restrict__ pidx) {
+  const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= (long long)n * P.nm) return;
+  const int q = (int)(g / P.nm), slot = (int)(g - (long long)q * P.nm);
+  int t = 0;
+  while (t + 1 < P.ntypes && slot >= P.sec_start[t + 1]) ++t;
+  const int k = slot - P.sec_start[t];
+  if (k < nreal[(size_t)q * P.ntypes + t])
+    pidx[(size_t)n * P.sec_start[t] + off[(size_t)t * (n + 1) + q] + k] = (int)g;
+}
+
+size_t tc_pair_workspace_bytes(const DevModel &P, int64_t chunk) {
+  return sizeof(int) * ((size_t)P.ntypes * (chunk + 1) + (size_t)chunk * P.nm) + 256;
+}
+
+cudaError_t tc_build_pairs(const DevModel &P, const ChunkView &C, void *ws, cudaStream_t st) {
+  if (C.n <= 0) return cudaSuccess;
+  int *off = reinterpret_cast<int *>(ws);
+  int *pidx = off + (size_t)P.ntypes * (C.n + 1);
+  k_pair_scan<<<P.ntypes, 1024, 0, st>>>(C.n, P.ntypes, C.nreal, off);
+  const long long tot = (long long)C.n * P.nm;
+  k_pair_expand<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(P, C.n, C.nreal, off, pidx);
+  DPB_LAUNCHED(2);
+  return cudaGetLastError();
+}
+
+// ---- device helpers ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void env_row4_tc(const DevModel &P, const double4 v, double e[4]) {
+  double w, dw;
+  dp_switch(v.w, P.rcs, P.rc, w, dw);
+  const double ir = 1.0 / v.w;
+  const double s = w * ir;
+  const double sr = s * ir;
+  e[0] = s; e[1] = sr * v.x; e[2] = sr * v.y; e[3] = sr * v.z;
+}
+
+// write 4 consecutive K entries (one 16-byte chunk j of the 128-byte row) of a SW128 K-major panel, hi and lo
+__device__ __forceinline__ void store_split4(uint8_t *pan_hi, uint8_t *pan_lo, uint32_t rowbase, uint32_t r7, int j,
+                                             float v0, float v1, float v2, float v3) {
+  float4 h, l;
+  tc::split_tf32(v0, h.x, l.x);
+  tc::split_tf32(v1, h.y, l.y);
+  tc::split_tf32(v2, h.z, l.z);
+  tc::split_tf32(v3, h.w, l.w);
+  const uint32_t off = rowbase + ((((uint32_t)j ^ r7) & 7u) << 4);
+  *reinterpret_cast<float4 *>(pan_hi + off) = h;
+  *reinterpret_cast<float4 *>(pan_lo + off) = l;
+}
+
+// D (+)= A B with the 3xTF32 split: hi hi + lo hi + hi lo.  One thread issues.
+__device__ __forceinline__ void mma3(uint32_t tmem_d, uint32_t a_hi, uint32_t a_lo, uint32_t b_hi, uint32_t b_lo,
+                                     uint32_t idesc, bool first) {
+  const uint64_t dah = tc::make_desc_sw128(a_hi), dal = tc::make_desc_sw128(a_lo);
+  const uint64_t dbh = tc::make_desc_sw128(b_hi), dbl = tc::make_desc_sw128(b_lo);
+  tc::mma_tf32_ss(tmem_d, dal, dbh, idesc, first ? 0u : 1u);
+  tc::mma_tf32_ss(tmem_d, dah, dbl, idesc, 1u);
+  tc::mma_tf32_ss(tmem_d, dah, dbh, idesc, 1u);
+}
+
+// ---- pass 1 ----------------------------------------------------------------------------------------------------
+template <int S1>
+__global__ void __launch_bounds__(256, 1)
+k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int *__restrict__ off_t,
+           const int *__restrict__ pidx_t, int a, int t) {
+  using L = TL<S1>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  const int tid = threadIdx.x, wg = tid >> 7, wt = tid & 127, warp = tid >> 5;
+  const float *vec = reinterpret_cast<const float *>(smem + L::oVec);
+  uint8_t *slot = smem + L::oSlot + wg * L::SLOT;
+  double *envt = reinterpret_cast<double *>(smem + L::oEnv) + wg * 128 * 4;
+  int *ids = reinterpret_cast<int *>(smem + L::oIds) + wg * 128;
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + L::oBar) + wg;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::oTmem);
+
+  for (int k = tid; k < L::img_bytes / 16; k += 256)
+    reinterpret_cast<int4 *>(smem)[k] = reinterpret_cast<const int4 *>(net_img)[k];
+  if (warp == 0) tc::tmem_alloc<512>(tmem_slot);
+  if (tid == 0) {
+    tc::mbar_init(reinterpret_cast<uint64_t *>(smem + L::oBar), 1);
+    tc::mbar_init(reinterpret_cast<uint64_t *>(smem + L::oBar) + 1, 1);
+    tc::fence_mbar_init();
+  }
+  tc::fence_proxy_async();
+  tc::fence_before_sync();
+  __syncthreads();
+  tc::fence_after_sync();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t tD1 = tmem + wg * 256, tD2 = tD1 + 64;
+  const uint32_t lane_sel = (uint32_t)(32 * (warp & 3)) << 16;
+  const uint32_t slot_a = tc::smem_u32(slot), img_a = tc::smem_u32(smem);
+  const uint32_t rowbase = (uint32_t)(wt >> 3) * 1024u + (uint32_t)(wt & 7) * 128u, r7 = wt & 7;
+
+  const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
+  int flat0 = 0, flat1 = 0;
+  if (row_hi > row_lo) { flat0 = off_t[row_lo]; flat1 = off_t[row_hi]; }
+  const int ntiles = (flat1 - flat0 + 127) >> 7;
+  uint32_t phase = 0;
+
+  for (int tile = blockIdx.x * 2 + wg; tile < ntiles; tile += gridDim.x * 2) {
+    const int p = flat0 + tile * 128 + wt;
+    const bool valid = p < flat1;
+    const int nrows = min(128, flat1 - (flat0 + tile * 128));
+    double e[4] = {0.0, 0.0, 0.0, 0.0};
+    int qa = -1;
+    if (valid) {
+      const int idx = pidx_t[p];
+      qa = idx / P.nm;
+      env_row4_tc(P, C.dr[idx], e);
+    }
+    ids[wt] = qa;
+    *reinterpret_cast<double2 *>(envt + 4 * wt) = make_double2(e[0], e[1]);
+    *reinterpret_cast<double2 *>(envt + 4 * wt + 2) = make_double2(e[2], e[3]);
+    const float x = (float)e[0];
+    // layer 0 (Eq. 8): h0 = tanh(x W0 + b0)
+    float h0[32];
+#pragma unroll
+    for (int s = 0; s < 32; ++s) h0[s] = s < S1 ? tc::tanh_f32(fmaf(x, vec[L::vW0 + s], vec[L::vb0 + s])) : 0.0f;
+#pragma unroll
+    for (int j = 0; j < 2 * L::KS1; ++j)
+      store_split4(slot, slot + 16384, rowbase, r7, j, h0[4 * j], h0[4 * j + 1], h0[4 * j + 2], h0[4 * j + 3]);
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    tc::bar_sync(1 + wg, 128);
+    if (wt == 0) {
+      tc::fence_after_sync();
+      constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N1);
+#pragma unroll
+      for (int ks = 0; ks < L::KS1; ++ks)
+        mma3(tD1, slot_a + ks * 32, slot_a + 16384 + ks * 32, img_a + L::oW1h + ks * 32, img_a + L::oW1l + ks * 32, idesc,
+             ks == 0);
+      tc::mma_commit(mbar);
+    }
+    tc::mbar_wait(mbar, phase);
+    phase ^= 1;
+    tc::fence_after_sync();
+    // layer 1 (Eq. 9): h1 = (h0, h0) + tanh(h0 W1 + b1)
+    float h1[2 * S1];
+#pragma unroll
+    for (int c8 = 0; c8 < L::N1 / 8; ++c8) {
+      float v[8];
+      tc::tmem_ld8(tD1 + lane_sel + 8 * c8, v);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int o = 8 * c8 + i;
+        if (o < 2 * S1) h1[o] = h0[o % S1] + tc::tanh_f32(v[i] + vec[L::vb1 + o]);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 2 * L::KS2; ++j) {
+      const int pan = j >> 3;
+      auto H = [&](int o) { return o < 2 * S1 ? h1[o] : 0.0f; };
+      store_split4(slot + pan * 16384, slot + 32768 + pan * 16384, rowbase, r7, j & 7, H(4 * j), H(4 * j + 1), H(4 * j + 2),
+                   H(4 * j + 3));
+    }
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    tc::bar_sync(1 + wg, 128);
+    if (wt == 0) {
+      tc::fence_after_sync();
+      constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N2);
+#pragma unroll
+      for (int ks = 0; ks < L::KS2; ++ks) {
+        const uint32_t ao = (ks >> 2) * 16384 + (ks & 3) * 32, bo = (ks >> 2) * L::W2P + (ks & 3) * 32;
+        mma3(tD2, slot_a + ao, slot_a + 32768 + ao, img_a + L::oW2h + bo, img_a + L::oW2l + bo, idesc, ks == 0);
+      }
+      tc::mma_commit(mbar);
+    }
+    tc::mbar_wait(mbar, phase);
+    phase ^= 1;
+    tc::fence_after_sync();
+    // layer 2 (Eq. 9): g = (h1, h1) + tanh(h1 W2 + b2), written to the slot as a [128][128] fp32 tile whose 16-byte
+    // chunks are XOR-swizzled with the row (conflict-free row-wise stores and column-wise loads)
+    float *gt = reinterpret_cast<float *>(slot);
+#pragma unroll
+    for (int c8 = 0; c8 < L::N2 / 8; ++c8) {
+      float v[8];
+      tc::tmem_ld8(tD2 + lane_sel + 8 * c8, v);
+      float gv[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int o = 8 * c8 + i;
+        gv[i] = o < 4 * S1 ? h1[o % (2 * S1)] + tc::tanh_f32(v[i] + vec[L::vb2 + o]) : 0.0f;
+      }
+      *reinterpret_cast<float4 *>(gt + wt * 128 + (((2 * c8) ^ r7) << 2)) = make_float4(gv[0], gv[1], gv[2], gv[3]);
+      *reinterpret_cast<float4 *>(gt + wt * 128 + (((2 * c8 + 1) ^ r7) << 2)) = make_float4(gv[4], gv[5], gv[6], gv[7]);
+    }
+    tc::fence_before_sync();
+    tc::bar_sync(1 + wg, 128);
+    // S5: T_i += sum_rows g (x) R~ in fp64; thread b owns feature b and walks the rows, one segment per centre atom
+    if (wt < 4 * S1) {
+      const int b = wt;
+      double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+      int prev = ids[0];
+      for (int row = 0; row < nrows; ++row) {
+        const int cur = ids[row];
+        if (cur != prev) {
+          double *dst = C.T + ((size_t)prev * P.M + b) * 4;
+          atomicAdd(dst + 0, acc0); atomicAdd(dst + 1, acc1); atomicAdd(dst + 2, acc2); atomicAdd(dst + 3, acc3);
+          acc0 = acc1 = acc2 = acc3 = 0.0;
+          prev = cur;
+        }
+        const double gvd = (double)gt[row * 128 + ((((b >> 2) ^ (row & 7))) << 2) + (b & 3)];
+        const double2 e01 = *reinterpret_cast<const double2 *>(envt + 4 * row);
+        const double2 e23 = *reinterpret_cast<const double2 *>(envt + 4 * row + 2);
+        acc0 = fma(gvd, e01.x, acc0); acc1 = fma(gvd, e01.y, acc1);
+        acc2 = fma(gvd, e23.x, acc2); acc3 = fma(gvd, e23.y, acc3);
+      }
+      double *dst = C.T + ((size_t)prev * P.M + b) * 4;
+      atomicAdd(dst + 0, acc0); atomicAdd(dst + 1, acc1); atomicAdd(dst + 2, acc2); atomicAdd(dst + 3, acc3);
+    }
+    tc::bar_sync(1 + wg, 128);                              // slot, env tile and ids are rewritten by the next tile
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  if (warp == 0) tc::tmem_dealloc<512>(tmem);
+}
+
+static int g_tc_sms = 0;
+
+template <int S1>
+static cudaError_t run_pass1_tc(const DevModel &P, const ChunkView &C, const TCWeights &W, const int *off,
+                                const int *pidx, cudaStream_t st) {
+  using L = TL<S1>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_tc<S1>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::smem_bytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  for (int a = 0; a < P.ntypes; ++a)
+    for (int t = 0; t < P.ntypes; ++t) {
+      k_pass1_tc<S1><<<g_tc_sms, 256, L::smem_bytes, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride,
+                                                          off + (size_t)t * (C.n + 1), pidx + (size_t)C.n * P.sec_start[t],
+                                                          a, t);
+      DPB_LAUNCHED(1);
+    }
+  return cudaGetLastError();
+}
+
+cudaError_t tc_pass1(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, cudaStream_t st) {
+  if (C.n <= 0) return cudaSuccess;
+  if (!W.ready) return cudaErrorNotSupported;
+  if (g_tc_sms == 0) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g_tc_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+  }
+  cudaError_t e = cudaMemsetAsync(C.T, 0, sizeof(double) * (size_t)C.n * P.M * 4, st);
+  if (e != cudaSuccess) return e;
+  const int *off = reinterpret_cast<const int *>(pair_ws);
+  const int *pidx = off + (size_t)P.ntypes * (C.n + 1);
+  switch (P.s1) {
+    case 8: return run_pass1_tc<8>(P, C, W, off, pidx, st);
+    case 16: return run_pass1_tc<16>(P, C, W, off, pidx, st);
+    case 25: return run_pass1_tc<25>(P, C, W, off, pidx, st);
+    default: return run_pass1_tc<32>(P, C, W, off, pidx, st);
+  }
+}
