@@ -25,7 +25,7 @@ struct TL {
   static constexpr int img_bytes = (oVec + 4 * nvec + 1023) / 1024 * 1024;
   static constexpr int SLOT = 65536;                       // per-warpgroup operand slot
   static constexpr int oSlot = img_bytes, oEnv = oSlot + 2 * SLOT, oIds = oEnv + 2 * 128 * 32,
-                       oBar = oIds + 2 * 128 * 4, oTmem = oBar + 16, smem_bytes = oTmem + 16;
+                       oBar = oIds + 2 * 256 * 4, oTmem = oBar + 16, smem_bytes = oTmem + 16;
   static_assert(S1 <= 32, "layer-1 operand is one 32-wide panel");
   static_assert(N2 <= 128 && PAN2 <= 2, "layer-2 operand: two 32-wide panels, 128 output columns");
 };
@@ -179,6 +179,12 @@ __device__ __forceinline__ void mma3(uint32_t tmem_d, uint32_t a_hi, uint32_t a_
   tc::mma_tf32_ss(tmem_d, dah, dbh, idesc, 1u);
 }
 
+#ifdef TC_PROF
+#include <cstdio>
+#define TCP(i) tp[i] = clock64()
+#else
+#define TCP(i)
+#endif
 // ---- pass 1 ----------------------------------------------------------------------------------------------------
 template <int S1>
 __global__ void __launch_bounds__(256, 1)
@@ -189,8 +195,8 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
   const int tid = threadIdx.x, wg = tid >> 7, wt = tid & 127, warp = tid >> 5;
   const float *vec = reinterpret_cast<const float *>(smem + L::oVec);
   uint8_t *slot = smem + L::oSlot + wg * L::SLOT;
-  double *envt = reinterpret_cast<double *>(smem + L::oEnv) + wg * 128 * 4;
-  int *ids = reinterpret_cast<int *>(smem + L::oIds) + wg * 128;
+  float4 *envt = reinterpret_cast<float4 *>(smem + L::oEnv) + wg * 128;   // fp32 copy of the tile's R~ rows
+  int *ids = reinterpret_cast<int *>(smem + L::oIds) + wg * 256, *segs = ids + 128;
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + L::oBar) + wg;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::oTmem);
 
@@ -217,21 +223,34 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
   if (row_hi > row_lo) { flat0 = off_t[row_lo]; flat1 = off_t[row_hi]; }
   const int ntiles = (flat1 - flat0 + 127) >> 7;
   uint32_t phase = 0;
+#ifdef TC_PROF
+  long long tp[11];
+#endif
 
+  int nx_idx = 0;
+  double4 nx_dv = make_double4(0.0, 0.0, 0.0, 1.0);
+  bool nx_valid = false;
+  {
+    const int t0 = blockIdx.x * 2 + wg, p0 = flat0 + t0 * 128 + wt;
+    nx_valid = t0 < ntiles && p0 < flat1;
+    if (nx_valid) { nx_idx = pidx_t[p0]; nx_dv = C.dr[nx_idx]; }
+  }
   for (int tile = blockIdx.x * 2 + wg; tile < ntiles; tile += gridDim.x * 2) {
-    const int p = flat0 + tile * 128 + wt;
-    const bool valid = p < flat1;
+    const bool valid = nx_valid;
     const int nrows = min(128, flat1 - (flat0 + tile * 128));
     double e[4] = {0.0, 0.0, 0.0, 0.0};
     int qa = -1;
+    TCP(0);
     if (valid) {
-      const int idx = pidx_t[p];
-      qa = idx / P.nm;
-      env_row4_tc(P, C.dr[idx], e);
+      qa = nx_idx / P.nm;
+      env_row4_tc(P, nx_dv, e);
     }
     ids[wt] = qa;
-    *reinterpret_cast<double2 *>(envt + 4 * wt) = make_double2(e[0], e[1]);
-    *reinterpret_cast<double2 *>(envt + 4 * wt + 2) = make_double2(e[2], e[3]);
+    if (valid) {
+      const int tile0 = flat0 + tile * 128, seg_lo = off_t[qa] - tile0, seg_hi = off_t[qa + 1] - tile0;
+      segs[wt] = min(nrows, seg_hi) | ((seg_lo >= 0 && seg_hi <= 128) ? 256 : 0);
+    }
+    envt[wt] = make_float4((float)e[0], (float)e[1], (float)e[2], (float)e[3]);
     const float x = (float)e[0];
     // layer 0 (Eq. 8): h0 = tanh(x W0 + b0)
     float h0[32];
@@ -240,9 +259,11 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
 #pragma unroll
     for (int j = 0; j < 2 * L::KS1; ++j)
       store_split4(slot, slot + 16384, rowbase, r7, j, h0[4 * j], h0[4 * j + 1], h0[4 * j + 2], h0[4 * j + 3]);
+    TCP(1);
     tc::fence_proxy_async();
     tc::fence_before_sync();
     tc::bar_sync(1 + wg, 128);
+    TCP(2);
     if (wt == 0) {
       tc::fence_after_sync();
       constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N1);
@@ -255,18 +276,17 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
     tc::mbar_wait(mbar, phase);
     phase ^= 1;
     tc::fence_after_sync();
+    TCP(3);
     // layer 1 (Eq. 9): h1 = (h0, h0) + tanh(h0 W1 + b1)
     float h1[2 * S1];
+    {
+      uint32_t v[L::N1];
+      tc::tmem_ld_cols_nowait<L::N1>(tD1 + lane_sel, v);
+      tc::tmem_wait_ld();
 #pragma unroll
-    for (int c8 = 0; c8 < L::N1 / 8; ++c8) {
-      float v[8];
-      tc::tmem_ld8(tD1 + lane_sel + 8 * c8, v);
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int o = 8 * c8 + i;
-        if (o < 2 * S1) h1[o] = h0[o % S1] + tc::tanh_f32(v[i] + vec[L::vb1 + o]);
-      }
+      for (int o = 0; o < 2 * S1; ++o) h1[o] = h0[o % S1] + tc::tanh_f32(__uint_as_float(v[o]) + vec[L::vb1 + o]);
     }
+    TCP(4);
 #pragma unroll
     for (int j = 0; j < 2 * L::KS2; ++j) {
       const int pan = j >> 3;
@@ -274,6 +294,7 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
       store_split4(slot + pan * 16384, slot + 32768 + pan * 16384, rowbase, r7, j & 7, H(4 * j), H(4 * j + 1), H(4 * j + 2),
                    H(4 * j + 3));
     }
+    TCP(5);
     tc::fence_proxy_async();
     tc::fence_before_sync();
     tc::bar_sync(1 + wg, 128);
@@ -290,47 +311,104 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
     tc::mbar_wait(mbar, phase);
     phase ^= 1;
     tc::fence_after_sync();
+    TCP(6);
     // layer 2 (Eq. 9): g = (h1, h1) + tanh(h1 W2 + b2), written to the slot as a [128][128] fp32 tile whose 16-byte
     // chunks are XOR-swizzled with the row (conflict-free row-wise stores and column-wise loads)
     float *gt = reinterpret_cast<float *>(slot);
+    {
+      constexpr int CH = 32, NCH = (L::N2 + CH - 1) / CH;
+      uint32_t va[CH], vb[CH];
+      tc::tmem_ld_cols_nowait<(L::N2 < CH ? L::N2 : CH)>(tD2 + lane_sel, va);
+      tc::tmem_wait_ld();
 #pragma unroll
-    for (int c8 = 0; c8 < L::N2 / 8; ++c8) {
-      float v[8];
-      tc::tmem_ld8(tD2 + lane_sel + 8 * c8, v);
-      float gv[8];
+      for (int c = 0; c < NCH; ++c) {
+        uint32_t *cur = (c & 1) ? vb : va, *nxt = (c & 1) ? va : vb;
+        constexpr int dummy = 0;
+        (void)dummy;
+        if (c + 1 < NCH) {
+          if (L::N2 - (c + 1) * CH >= CH) tc::tmem_ld_cols_nowait<CH>(tD2 + lane_sel + (c + 1) * CH, nxt);
+          else tc::tmem_ld_cols_nowait<(L::N2 % CH == 0 ? CH : L::N2 % CH)>(tD2 + lane_sel + (c + 1) * CH, nxt);
+        }
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int o = 8 * c8 + i;
-        gv[i] = o < 4 * S1 ? h1[o % (2 * S1)] + tc::tanh_f32(v[i] + vec[L::vb2 + o]) : 0.0f;
+        for (int j = 0; j < CH / 4; ++j) {
+          const int o = c * CH + 4 * j;
+          if (o < L::N2) {
+            float gv[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+              gv[i] = o + i < 4 * S1 ? h1[(o + i) % (2 * S1)] + tc::tanh_f32(__uint_as_float(cur[4 * j + i]) + vec[L::vb2 + o + i]) : 0.0f;
+            *reinterpret_cast<float4 *>(gt + wt * 128 + (((o >> 2) ^ r7) << 2)) = make_float4(gv[0], gv[1], gv[2], gv[3]);
+          }
+        }
+        if (c + 1 < NCH) tc::tmem_wait_ld();
       }
-      *reinterpret_cast<float4 *>(gt + wt * 128 + (((2 * c8) ^ r7) << 2)) = make_float4(gv[0], gv[1], gv[2], gv[3]);
-      *reinterpret_cast<float4 *>(gt + wt * 128 + (((2 * c8 + 1) ^ r7) << 2)) = make_float4(gv[4], gv[5], gv[6], gv[7]);
     }
+    TCP(7);
     tc::fence_before_sync();
     tc::bar_sync(1 + wg, 128);
-    // S5: T_i += sum_rows g (x) R~ in fp64; thread b owns feature b and walks the rows, one segment per centre atom
+    TCP(8);
+    // prefetch the next tile's pair (two dependent global loads) behind the accumulation below
+    {
+      const int tn = tile + gridDim.x * 2, pn = flat0 + tn * 128 + wt;
+      nx_valid = tn < ntiles && pn < flat1;
+      if (nx_valid) { nx_idx = pidx_t[pn]; nx_dv = C.dr[nx_idx]; }
+    }
+    // S5: T_i += sum_rows g (x) R~.  Thread b owns feature b; rows are grouped by centre atom (segments, from the pair
+    // offsets).  Aligned blocks of 8 rows: products and the 8-row partial sum in fp32, accumulation across blocks in
+    // fp64; blocks cut by a segment boundary are masked.
     if (wt < 4 * S1) {
       const int b = wt;
-      double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-      int prev = ids[0];
-      for (int row = 0; row < nrows; ++row) {
+      const float *gp = gt + (b & 3);
+      int col[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) col[i] = i * 128 + ((((b >> 2) ^ i)) << 2);
+      int row = 0;
+      while (row < nrows) {
         const int cur = ids[row];
-        if (cur != prev) {
-          double *dst = C.T + ((size_t)prev * P.M + b) * 4;
-          atomicAdd(dst + 0, acc0); atomicAdd(dst + 1, acc1); atomicAdd(dst + 2, acc2); atomicAdd(dst + 3, acc3);
-          acc0 = acc1 = acc2 = acc3 = 0.0;
-          prev = cur;
+        const int se = segs[row];                           // end row of this atom's segment; bit 8: whole section in the tile
+        const int hi = se & 255;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        for (int r0 = row & ~7; r0 < hi; r0 += 8) {
+          const float *gb = gp + r0 * 128;
+          const float4 *eb = envt + r0;
+          float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+          if (r0 >= row && r0 + 8 <= hi) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const float gv = gb[col[i]];
+              const float4 ev = eb[i];
+              s0 = fmaf(gv, ev.x, s0); s1 = fmaf(gv, ev.y, s1); s2 = fmaf(gv, ev.z, s2); s3 = fmaf(gv, ev.w, s3);
+            }
+          } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const float gv = (r0 + i >= row && r0 + i < hi) ? gb[col[i]] : 0.f;
+              const float4 ev = eb[i];
+              s0 = fmaf(gv, ev.x, s0); s1 = fmaf(gv, ev.y, s1); s2 = fmaf(gv, ev.z, s2); s3 = fmaf(gv, ev.w, s3);
+            }
+          }
+          a0 += (double)s0; a1 += (double)s1; a2 += (double)s2; a3 += (double)s3;
         }
-        const double gvd = (double)gt[row * 128 + ((((b >> 2) ^ (row & 7))) << 2) + (b & 3)];
-        const double2 e01 = *reinterpret_cast<const double2 *>(envt + 4 * row);
-        const double2 e23 = *reinterpret_cast<const double2 *>(envt + 4 * row + 2);
-        acc0 = fma(gvd, e01.x, acc0); acc1 = fma(gvd, e01.y, acc1);
-        acc2 = fma(gvd, e23.x, acc2); acc3 = fma(gvd, e23.y, acc3);
+        double *dst = C.T + ((size_t)cur * P.M + b) * 4;
+        if (t == 0 && (se & 256)) {
+          // first section and the whole section of this atom lies inside the tile: nobody else writes T[cur][b][:] yet
+          double2 *d2 = reinterpret_cast<double2 *>(dst);
+          d2[0] = make_double2(a0, a1);
+          d2[1] = make_double2(a2, a3);
+        } else {
+          atomicAdd(dst + 0, a0); atomicAdd(dst + 1, a1); atomicAdd(dst + 2, a2); atomicAdd(dst + 3, a3);
+        }
+        row = hi;
       }
-      double *dst = C.T + ((size_t)prev * P.M + b) * 4;
-      atomicAdd(dst + 0, acc0); atomicAdd(dst + 1, acc1); atomicAdd(dst + 2, acc2); atomicAdd(dst + 3, acc3);
     }
+    TCP(9);
     tc::bar_sync(1 + wg, 128);                              // slot, env tile and ids are rewritten by the next tile
+    TCP(10);
+#ifdef TC_PROF
+    if (blockIdx.x == 3 && wt == 0 && tile == blockIdx.x * 2 + wg + 4 * gridDim.x * 2)
+      printf("wg %d a %d t %d: env+l0 %lld bar %lld mma1 %lld ld1+tanh %lld st2 %lld mma2 %lld ld2+tanh+g %lld bar %lld Tacc %lld bar %lld\n", wg, a, t,
+             tp[1]-tp[0], tp[2]-tp[1], tp[3]-tp[2], tp[4]-tp[3], tp[5]-tp[4], tp[6]-tp[5], tp[7]-tp[6], tp[8]-tp[7], tp[9]-tp[8], tp[10]-tp[9]);
+#endif
   }
   tc::fence_before_sync();
   __syncthreads();
