@@ -58,6 +58,7 @@ struct dpb_model {
   Buf nl, dr, nreal, T, dT;
   Buf v0[9];
   Buf v1ws;
+  Buf dT32;                     // mixed precision: fp32 copy of dE/dT of the chunk
   Buf pairs;                    // mixed precision: flattened real-slot lists of the chunk
   Buf h_coord, h_type, h_out;   // device staging of dpb_eval_host
   double *dbgT = nullptr, *dbgD = nullptr, *dbgdT = nullptr;
@@ -127,7 +128,7 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->h_coord, &m->h_type, &m->h_out};
+                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->h_coord, &m->h_type, &m->h_out};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
@@ -255,7 +256,10 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     } else {
       CU(m->v1ws.reserve(v1_workspace_bytes(P, chunk)), "workspace");
     }
-    if (m->precision == DPB_TF32) CU(m->pairs.reserve(tc_pair_workspace_bytes(P, chunk)), "workspace");
+    if (m->precision == DPB_TF32) {
+      CU(m->pairs.reserve(tc_pair_workspace_bytes(P, chunk)), "workspace");
+      CU(m->dT32.reserve(tc_pass2_workspace_bytes(P, chunk)), "workspace");
+    }
   }
   DevStats *stats = m->stats.as<DevStats>();
   CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");
@@ -305,7 +309,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       CU(v1_fit(P, C, m->v1, m->fit.as<double>(), m->v1ws.p, ei, st), "fit");
       CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
       if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
-      CU(v1_pass2(P, C, m->v1, force, virial, st), "pass2");
+      CU(tc_pass2(P, C, m->tcw, m->pairs.p, m->dT32.p, force, virial, st), "pass2 tf32");
       if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
     } else if (m->variant == 0 || !m->v1.ready) {
       V0Scratch S;

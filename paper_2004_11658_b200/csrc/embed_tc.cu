@@ -457,3 +457,306 @@ cudaError_t tc_pass1(const DevModel &P, const ChunkView &C, const TCWeights &W, 
     default: return run_pass1_tc<32>(P, C, W, off, pidx, st);
   }
 }
+
+// ---- pass 2 ----------------------------------------------------------------------------------------------------
+// S8 + S9 in mixed precision.  Forward-mode derivative of the embedding net (its input is the scalar s(r)): the value
+// row h and the tangent row h' = dh/dx go through the same tensor-core GEMMs (separate accumulators in TMEM), then
+//   dE/dR~[c] = sum_o dT[o][c] g[o],   dE/dx = sum_o (dT R~)[o] g'[o]                     (O9, fp32 dots per row)
+// and the chain to the displacement (O10), the force scatter and the virial (O11, ProdForce / ProdVirial,
+// PAPER.md:240) in fp64.  dT32 is the fp32 copy of dE/dT written by the fitting stage.
+__global__ void k_dT_to_f32(long long n, const double *__restrict__ src, float *__restrict__ dst) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = (float)src[i];
+}
+
+template <int S1>
+__global__ void __launch_bounds__(256, 1)
+k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int *__restrict__ off_t,
+           const int *__restrict__ pidx_t, const float *__restrict__ dT32, int a, int t, double *__restrict__ force,
+           double *__restrict__ virial) {
+  using L = TL<S1>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  const int tid = threadIdx.x, wg = tid >> 7, wt = tid & 127, warp = tid >> 5, lane = tid & 31;
+  const float *vec = reinterpret_cast<const float *>(smem + L::oVec);
+  uint8_t *slot = smem + L::oSlot + wg * L::SLOT;
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + L::oBar) + wg;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::oTmem);
+  double *vred = reinterpret_cast<double *>(smem + L::oEnv);           // [8 warps][9], used after the tile loop
+
+  for (int k = tid; k < L::img_bytes / 16; k += 256)
+    reinterpret_cast<int4 *>(smem)[k] = reinterpret_cast<const int4 *>(net_img)[k];
+  if (warp == 0) tc::tmem_alloc<512>(tmem_slot);
+  if (tid == 0) {
+    tc::mbar_init(reinterpret_cast<uint64_t *>(smem + L::oBar), 1);
+    tc::mbar_init(reinterpret_cast<uint64_t *>(smem + L::oBar) + 1, 1);
+    tc::fence_mbar_init();
+  }
+  tc::fence_proxy_async();
+  tc::fence_before_sync();
+  __syncthreads();
+  tc::fence_after_sync();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t tD1v = tmem + wg * 256, tD1t = tD1v + 64, tD2v = tD1v, tD2t = tD1v + 128;
+  const uint32_t lane_sel = (uint32_t)(32 * (warp & 3)) << 16;
+  const uint32_t slot_a = tc::smem_u32(slot), img_a = tc::smem_u32(smem);
+  const uint32_t rowbase = (uint32_t)(wt >> 3) * 1024u + (uint32_t)(wt & 7) * 128u, r7 = wt & 7;
+
+  const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
+  int flat0 = 0, flat1 = 0;
+  if (row_hi > row_lo) { flat0 = off_t[row_lo]; flat1 = off_t[row_hi]; }
+  const int ntiles = (flat1 - flat0 + 127) >> 7;
+  uint32_t phase = 0;
+  double vir[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+
+  int nx_idx = 0;
+  double4 nx_dv = make_double4(0.0, 0.0, 0.0, 1.0);
+  bool nx_valid = false;
+  {
+    const int t0 = blockIdx.x * 2 + wg, p0 = flat0 + t0 * 128 + wt;
+    nx_valid = t0 < ntiles && p0 < flat1;
+    if (nx_valid) { nx_idx = pidx_t[p0]; nx_dv = C.dr[nx_idx]; }
+  }
+  for (int tile = blockIdx.x * 2 + wg; tile < ntiles; tile += gridDim.x * 2) {
+    const bool valid = nx_valid;
+    const int idx = nx_idx;
+    const double4 dv = nx_dv;
+    const int qa = valid ? idx / P.nm : -1;
+    double ed[4] = {0.0, 0.0, 0.0, 0.0};
+    if (valid) env_row4_tc(P, dv, ed);
+    const float e0 = (float)ed[0], e1 = (float)ed[1], e2 = (float)ed[2], e3 = (float)ed[3];
+    // layer 0 and its tangent: h0' = (1 - t0^2) W0   (d tanh = 1 - tanh^2)
+    float h0v[32], h0t[32];
+#pragma unroll
+    for (int s = 0; s < 32; ++s) {
+      if (s < S1) {
+        const float w0 = vec[L::vW0 + s];
+        const float t0 = tc::tanh_f32(fmaf(e0, w0, vec[L::vb0 + s]));
+        h0v[s] = t0;
+        h0t[s] = fmaf(-t0, t0, 1.0f) * w0;
+      } else {
+        h0v[s] = 0.0f; h0t[s] = 0.0f;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 2 * L::KS1; ++j) {
+      store_split4(slot, slot + 16384, rowbase, r7, j, h0v[4 * j], h0v[4 * j + 1], h0v[4 * j + 2], h0v[4 * j + 3]);
+      store_split4(slot + 32768, slot + 49152, rowbase, r7, j, h0t[4 * j], h0t[4 * j + 1], h0t[4 * j + 2], h0t[4 * j + 3]);
+    }
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    tc::bar_sync(1 + wg, 128);
+    if (wt == 0) {
+      tc::fence_after_sync();
+      constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N1);
+#pragma unroll
+      for (int ks = 0; ks < L::KS1; ++ks) {
+        mma3(tD1v, slot_a + ks * 32, slot_a + 16384 + ks * 32, img_a + L::oW1h + ks * 32, img_a + L::oW1l + ks * 32, idesc,
+             ks == 0);
+        mma3(tD1t, slot_a + 32768 + ks * 32, slot_a + 49152 + ks * 32, img_a + L::oW1h + ks * 32, img_a + L::oW1l + ks * 32,
+             idesc, ks == 0);
+      }
+      tc::mma_commit(mbar);
+    }
+    tc::mbar_wait(mbar, phase);
+    phase ^= 1;
+    tc::fence_after_sync();
+    // layer 1: h1 = (h0, h0) + t1, h1' = (h0', h0') + (1 - t1^2) (h0' W1)
+    float h1v[2 * S1], h1t[2 * S1];
+    {
+      uint32_t v[L::N1], w[L::N1];
+      tc::tmem_ld_cols_nowait<L::N1>(tD1v + lane_sel, v);
+      tc::tmem_ld_cols_nowait<L::N1>(tD1t + lane_sel, w);
+      tc::tmem_wait_ld();
+#pragma unroll
+      for (int o = 0; o < 2 * S1; ++o) {
+        const float t1 = tc::tanh_f32(__uint_as_float(v[o]) + vec[L::vb1 + o]);
+        h1v[o] = h0v[o % S1] + t1;
+        h1t[o] = fmaf(fmaf(-t1, t1, 1.0f), __uint_as_float(w[o]), h0t[o % S1]);
+      }
+    }
+    // layer 2, value rows
+#pragma unroll
+    for (int j = 0; j < 2 * L::KS2; ++j) {
+      const int pan = j >> 3;
+      auto H = [&](int o) { return o < 2 * S1 ? h1v[o] : 0.0f; };
+      store_split4(slot + pan * 16384, slot + 32768 + pan * 16384, rowbase, r7, j & 7, H(4 * j), H(4 * j + 1), H(4 * j + 2),
+                   H(4 * j + 3));
+    }
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    tc::bar_sync(1 + wg, 128);
+    if (wt == 0) {
+      tc::fence_after_sync();
+      constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N2);
+#pragma unroll
+      for (int ks = 0; ks < L::KS2; ++ks) {
+        const uint32_t ao = (ks >> 2) * 16384 + (ks & 3) * 32, bo = (ks >> 2) * L::W2P + (ks & 3) * 32;
+        mma3(tD2v, slot_a + ao, slot_a + 32768 + ao, img_a + L::oW2h + bo, img_a + L::oW2l + bo, idesc, ks == 0);
+      }
+      tc::mma_commit(mbar);
+    }
+    tc::mbar_wait(mbar, phase);
+    phase ^= 1;
+    tc::fence_after_sync();
+    // layer 2, tangent rows (the operand slot is free again: the value MMAs have completed)
+#pragma unroll
+    for (int j = 0; j < 2 * L::KS2; ++j) {
+      const int pan = j >> 3;
+      auto H = [&](int o) { return o < 2 * S1 ? h1t[o] : 0.0f; };
+      store_split4(slot + pan * 16384, slot + 32768 + pan * 16384, rowbase, r7, j & 7, H(4 * j), H(4 * j + 1), H(4 * j + 2),
+                   H(4 * j + 3));
+    }
+    tc::fence_proxy_async();
+    tc::fence_before_sync();
+    tc::bar_sync(1 + wg, 128);
+    if (wt == 0) {
+      tc::fence_after_sync();
+      constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N2);
+#pragma unroll
+      for (int ks = 0; ks < L::KS2; ++ks) {
+        const uint32_t ao = (ks >> 2) * 16384 + (ks & 3) * 32, bo = (ks >> 2) * L::W2P + (ks & 3) * 32;
+        mma3(tD2t, slot_a + ao, slot_a + 32768 + ao, img_a + L::oW2h + bo, img_a + L::oW2l + bo, idesc, ks == 0);
+      }
+      tc::mma_commit(mbar);
+    }
+    // prefetch the next tile's pair behind the MMA wait
+    {
+      const int tn = tile + gridDim.x * 2, pn = flat0 + tn * 128 + wt;
+      nx_valid = tn < ntiles && pn < flat1;
+      if (nx_valid) { nx_idx = pidx_t[pn]; nx_dv = C.dr[nx_idx]; }
+    }
+    tc::mbar_wait(mbar, phase);
+    phase ^= 1;
+    tc::fence_after_sync();
+    // epilogue: g = (h1, h1) + t2, g' = (h1', h1') + (1 - t2^2) (h1' W2); dots with the atom's dT rows
+    float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f, pr3 = 0.f, dx = 0.f;
+    const float4 *dTrow = reinterpret_cast<const float4 *>(dT32) + (size_t)(valid ? qa : 0) * P.M;
+    {
+      constexpr int CH = 16, NCH = (4 * S1 + CH - 1) / CH;
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) {
+        uint32_t v[CH], w[CH];
+        constexpr int dummy = 0;
+        (void)dummy;
+        if (L::N2 - c * CH >= CH) {
+          tc::tmem_ld_cols_nowait<CH>(tD2v + lane_sel + c * CH, v);
+          tc::tmem_ld_cols_nowait<CH>(tD2t + lane_sel + c * CH, w);
+        } else {
+          tc::tmem_ld_cols_nowait<8>(tD2v + lane_sel + c * CH, v);
+          tc::tmem_ld_cols_nowait<8>(tD2t + lane_sel + c * CH, w);
+        }
+        tc::tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < CH; ++i) {
+          const int o = c * CH + i;
+          if (o < 4 * S1) {
+            const float t2 = tc::tanh_f32(__uint_as_float(v[i]) + vec[L::vb2 + o]);
+            const float gv = h1v[o % (2 * S1)] + t2;
+            const float gp = fmaf(fmaf(-t2, t2, 1.0f), __uint_as_float(w[i]), h1t[o % (2 * S1)]);
+            const float4 d4 = __ldg(dTrow + o);
+            pr0 = fmaf(d4.x, gv, pr0); pr1 = fmaf(d4.y, gv, pr1); pr2 = fmaf(d4.z, gv, pr2); pr3 = fmaf(d4.w, gv, pr3);
+            const float dg = fmaf(d4.x, e0, fmaf(d4.y, e1, fmaf(d4.z, e2, d4.w * e3)));
+            dx = fmaf(dg, gp, dx);
+          }
+        }
+      }
+    }
+    tc::fence_before_sync();                                // TMEM reads done before the next tile's MMAs overwrite
+    // O10 / O11 in fp64: f_ik = sum_m dR~[m] dR~_m/dd; F_j -= f, F_i += f, Xi -= d (x) f
+    double f0 = 0.0, f1 = 0.0, f2 = 0.0;
+    if (valid) {
+      const double r = dv.w, ir = 1.0 / r;
+      double w, dw;
+      dp_switch(r, P.rcs, P.rc, w, dw);
+      const double s = w * ir, qq = s * ir;
+      const double sp = dw * ir - w * ir * ir;
+      const double qp = sp * ir - s * ir * ir;
+      const double dR0 = (double)pr0 + (double)dx, dR1 = (double)pr1, dR2 = (double)pr2, dR3 = (double)pr3;
+      const double dot = dR1 * dv.x + dR2 * dv.y + dR3 * dv.z;
+      const double cm = (dR0 * sp + qp * dot) * ir;
+      f0 = fma(cm, dv.x, qq * dR1); f1 = fma(cm, dv.y, qq * dR2); f2 = fma(cm, dv.z, qq * dR3);
+      if (force) {
+        const int j = C.nl[idx];
+        atomicAdd(&force[3 * (size_t)j + 0], -f0);
+        atomicAdd(&force[3 * (size_t)j + 1], -f1);
+        atomicAdd(&force[3 * (size_t)j + 2], -f2);
+      }
+      vir[0] -= dv.x * f0; vir[1] -= dv.x * f1; vir[2] -= dv.x * f2;
+      vir[3] -= dv.y * f0; vir[4] -= dv.y * f1; vir[5] -= dv.y * f2;
+      vir[6] -= dv.z * f0; vir[7] -= dv.z * f1; vir[8] -= dv.z * f2;
+    }
+    // F_i += sum_k f_ik: rows of one atom are contiguous lanes -> segmented warp reduction, one RED per run head
+    if (force) {
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const int qo = __shfl_down_sync(0xffffffffu, qa, off);
+        const double g0 = __shfl_down_sync(0xffffffffu, f0, off), g1 = __shfl_down_sync(0xffffffffu, f1, off),
+                     g2 = __shfl_down_sync(0xffffffffu, f2, off);
+        if (lane + off < 32 && qo == qa) { f0 += g0; f1 += g1; f2 += g2; }
+      }
+      const int qprev = __shfl_up_sync(0xffffffffu, qa, 1);
+      if (valid && (lane == 0 || qprev != qa)) {
+        const size_t i = (size_t)C.s_idx[C.p0 + qa];
+        atomicAdd(&force[3 * i + 0], f0); atomicAdd(&force[3 * i + 1], f1); atomicAdd(&force[3 * i + 2], f2);
+      }
+    }
+  }
+  // virial: warp -> block -> one atomic per component and CTA
+#pragma unroll
+  for (int k = 0; k < 9; ++k) {
+    double v = vir[k];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if (lane == 0) vred[warp * 9 + k] = v;
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  if (tid < 9 && virial) {
+    double v = 0.0;
+    for (int w = 0; w < 8; ++w) v += vred[w * 9 + tid];
+    atomicAdd(&virial[tid], v);
+  }
+  if (warp == 0) tc::tmem_dealloc<512>(tmem);
+}
+
+size_t tc_pass2_workspace_bytes(const DevModel &P, int64_t chunk) { return sizeof(float) * (size_t)chunk * P.M * 4 + 256; }
+
+template <int S1>
+static cudaError_t run_pass2_tc(const DevModel &P, const ChunkView &C, const TCWeights &W, const int *off,
+                                const int *pidx, const float *dT32, double *force, double *virial, cudaStream_t st) {
+  using L = TL<S1>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass2_tc<S1>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::smem_bytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  for (int a = 0; a < P.ntypes; ++a)
+    for (int t = 0; t < P.ntypes; ++t) {
+      k_pass2_tc<S1><<<g_tc_sms, 256, L::smem_bytes, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride,
+                                                          off + (size_t)t * (C.n + 1), pidx + (size_t)C.n * P.sec_start[t],
+                                                          dT32, a, t, force, virial);
+      DPB_LAUNCHED(1);
+    }
+  return cudaGetLastError();
+}
+
+cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, void *ws2,
+                     double *force, double *virial, cudaStream_t st) {
+  if (C.n <= 0) return cudaSuccess;
+  if (!W.ready) return cudaErrorNotSupported;
+  const int *off = reinterpret_cast<const int *>(pair_ws);
+  const int *pidx = off + (size_t)P.ntypes * (C.n + 1);
+  float *dT32 = reinterpret_cast<float *>(ws2);
+  const long long tot = (long long)C.n * P.M * 4;
+  k_dT_to_f32<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(tot, C.dT, dT32);
+  DPB_LAUNCHED(1);
+  switch (P.s1) {
+    case 8: return run_pass2_tc<8>(P, C, W, off, pidx, dT32, force, virial, st);
+    case 16: return run_pass2_tc<16>(P, C, W, off, pidx, dT32, force, virial, st);
+    case 25: return run_pass2_tc<25>(P, C, W, off, pidx, dT32, force, virial, st);
+    default: return run_pass2_tc<32>(P, C, W, off, pidx, dT32, force, virial, st);
+  }
+}

@@ -17,5 +17,6 @@ size_t tc_pair_workspace_bytes(const DevModel &P, int64_t chunk);
 cudaError_t tc_build_pairs(const DevModel &P, const ChunkView &C, void *pair_ws, cudaStream_t st);
 
 cudaError_t tc_pass1(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, cudaStream_t st);
-cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, double *force,
-                     double *virial, cudaStream_t st);
+size_t tc_pass2_workspace_bytes(const DevModel &P, int64_t chunk);      // fp32 copy of dT
+cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, void *ws2,
+                     double *force, double *virial, cudaStream_t st);
