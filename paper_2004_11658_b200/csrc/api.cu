@@ -58,6 +58,7 @@ struct dpb_model {
   Buf nl, dr, nreal, T, dT;
   Buf v0[9];
   Buf v1ws;
+  Buf tcfit;                    // mixed precision: operand images and activations of the fitting stage
   Buf dT32;                     // mixed precision: fp32 copy of dE/dT of the chunk
   Buf pairs;                    // mixed precision: flattened real-slot lists of the chunk
   Buf h_coord, h_type, h_out;   // device staging of dpb_eval_host
@@ -111,9 +112,11 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
   m->precision = precision;
   if (e == cudaSuccess && precision == DPB_TF32) {
     e = tc_prepare_weights(P, d->emb_weights, m->tcw);
-    if (e == cudaErrorNotSupported || !m->v1.ready) {
+    if (e == cudaSuccess) e = tc_prepare_fit(P, d->fit_weights, m->tcw);
+    if (e == cudaErrorNotSupported) {
       dpb_model_destroy(m);
-      return fail(DPB_ENOTIMPL, "DPB_TF32 is built for emb_s1 in {8, 16, 25, 32} (got %d)", d->emb_s1);
+      return fail(DPB_ENOTIMPL, "DPB_TF32 is built for emb_s1 in {8, 16, 25, 32}, m_axis in {4, 8, 16} and "
+                                "fit_width %% 4 == 0, <= 256 (got %d, %d, %d)", d->emb_s1, d->m_axis, d->fit_width);
     }
   }
   if (e != cudaSuccess) {
@@ -128,7 +131,7 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->h_coord, &m->h_type, &m->h_out};
+                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
@@ -259,6 +262,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     if (m->precision == DPB_TF32) {
       CU(m->pairs.reserve(tc_pair_workspace_bytes(P, chunk)), "workspace");
       CU(m->dT32.reserve(tc_pass2_workspace_bytes(P, chunk)), "workspace");
+      CU(m->tcfit.reserve(tc_fit_workspace_bytes(P, chunk)), "workspace");
     }
   }
   DevStats *stats = m->stats.as<DevStats>();
@@ -306,10 +310,10 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       CU(tc_build_pairs(P, C, m->pairs.p, st), "pair list");
       CU(tc_pass1(P, C, m->tcw, m->pairs.p, st), "pass1 tf32");
       if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);
-      CU(v1_fit(P, C, m->v1, m->fit.as<double>(), m->v1ws.p, ei, st), "fit");
+      CU(tc_fit(P, C, m->tcw, m->tcfit.p, m->dT32.as<float>(), ei, st), "fit tf32");
       CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
       if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
-      CU(tc_pass2(P, C, m->tcw, m->pairs.p, m->dT32.p, force, virial, st), "pass2 tf32");
+      CU(tc_pass2(P, C, m->tcw, m->pairs.p, m->dT32.as<float>(), force, virial, st), "pass2 tf32");
       if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
     } else if (m->variant == 0 || !m->v1.ready) {
       V0Scratch S;

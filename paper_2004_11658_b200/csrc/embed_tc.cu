@@ -91,6 +91,7 @@ cudaError_t tc_prepare_weights(const DevModel &P, const double *emb_h, TCWeights
 }
 
 void tc_release_weights(TCWeights &W) {
+  tc_release_fit(W);
   if (W.emb) cudaFree(W.emb);
   W.emb = nullptr;
   W.ready = false;
@@ -464,10 +465,6 @@ cudaError_t tc_pass1(const DevModel &P, const ChunkView &C, const TCWeights &W, 
 //   dE/dR~[c] = sum_o dT[o][c] g[o],   dE/dx = sum_o (dT R~)[o] g'[o]                     (O9, fp32 dots per row)
 // and the chain to the displacement (O10), the force scatter and the virial (O11, ProdForce / ProdVirial,
 // PAPER.md:240) in fp64.  dT32 is the fp32 copy of dE/dT written by the fitting stage.
-__global__ void k_dT_to_f32(long long n, const double *__restrict__ src, float *__restrict__ dst) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) dst[i] = (float)src[i];
-}
 
 template <int S1>
 __global__ void __launch_bounds__(256, 1)
@@ -532,9 +529,10 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
     for (int s = 0; s < 32; ++s) {
       if (s < S1) {
         const float w0 = vec[L::vW0 + s];
-        const float t0 = tc::tanh_f32(fmaf(e0, w0, vec[L::vb0 + s]));
+        float t0, d0;
+        tc::tanh_d_f32(fmaf(e0, w0, vec[L::vb0 + s]), t0, d0);
         h0v[s] = t0;
-        h0t[s] = fmaf(-t0, t0, 1.0f) * w0;
+        h0t[s] = d0 * w0;
       } else {
         h0v[s] = 0.0f; h0t[s] = 0.0f;
       }
@@ -571,9 +569,10 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
       tc::tmem_wait_ld();
 #pragma unroll
       for (int o = 0; o < 2 * S1; ++o) {
-        const float t1 = tc::tanh_f32(__uint_as_float(v[o]) + vec[L::vb1 + o]);
+        float t1, d1;
+        tc::tanh_d_f32(__uint_as_float(v[o]) + vec[L::vb1 + o], t1, d1);
         h1v[o] = h0v[o % S1] + t1;
-        h1t[o] = fmaf(fmaf(-t1, t1, 1.0f), __uint_as_float(w[o]), h0t[o % S1]);
+        h1t[o] = fmaf(d1, __uint_as_float(w[o]), h0t[o % S1]);
       }
     }
     // layer 2, value rows
@@ -652,9 +651,10 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
         for (int i = 0; i < CH; ++i) {
           const int o = c * CH + i;
           if (o < 4 * S1) {
-            const float t2 = tc::tanh_f32(__uint_as_float(v[i]) + vec[L::vb2 + o]);
+            float t2, d2;
+            tc::tanh_d_f32(__uint_as_float(v[i]) + vec[L::vb2 + o], t2, d2);
             const float gv = h1v[o % (2 * S1)] + t2;
-            const float gp = fmaf(fmaf(-t2, t2, 1.0f), __uint_as_float(w[i]), h1t[o % (2 * S1)]);
+            const float gp = fmaf(d2, __uint_as_float(w[i]), h1t[o % (2 * S1)]);
             const float4 d4 = __ldg(dTrow + o);
             pr0 = fmaf(d4.x, gv, pr0); pr1 = fmaf(d4.y, gv, pr1); pr2 = fmaf(d4.z, gv, pr2); pr3 = fmaf(d4.w, gv, pr3);
             const float dg = fmaf(d4.x, e0, fmaf(d4.y, e1, fmaf(d4.z, e2, d4.w * e3)));
@@ -743,16 +743,12 @@ static cudaError_t run_pass2_tc(const DevModel &P, const ChunkView &C, const TCW
   return cudaGetLastError();
 }
 
-cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, void *ws2,
+cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, const float *dT32,
                      double *force, double *virial, cudaStream_t st) {
   if (C.n <= 0) return cudaSuccess;
   if (!W.ready) return cudaErrorNotSupported;
   const int *off = reinterpret_cast<const int *>(pair_ws);
   const int *pidx = off + (size_t)P.ntypes * (C.n + 1);
-  float *dT32 = reinterpret_cast<float *>(ws2);
-  const long long tot = (long long)C.n * P.M * 4;
-  k_dT_to_f32<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(tot, C.dT, dT32);
-  DPB_LAUNCHED(1);
   switch (P.s1) {
     case 8: return run_pass2_tc<8>(P, C, W, off, pidx, dT32, force, virial, st);
     case 16: return run_pass2_tc<16>(P, C, W, off, pidx, dT32, force, virial, st);

@@ -1,0 +1,533 @@
+// fit_tc.cu — mixed-precision (DPB_TF32) S5 (D = T T^<T), S6 (fitting net forward, Eq. 2-3) and S7
+// (fitting backward + dT) on the 5th-generation tensor cores.  Same six GEMMs as fit_dmma.cu:
+//   G1  Z0 = tanh(D W0 + b0)                    G4  dZ1 = w3 + Q2 W2^T,  Q1 = dZ1 S1,  S1 = 1 - U1^2
+//   G2  U1 = tanh(Z0 W1 + b1), Z1 = Z0 + U1     G5  dZ0 = dZ1 + Q1 W1^T, Q0 = dZ0 S0,  S0 = 1 - Z0^2
+//   G3  U2 = tanh(Z1 W2 + b2), E_i = (Z1 + U2) . w3 + b3,  Q2 = w3 (1 - U2^2)
+//   G6  dD = Q0 W0^T
+// each as tcgen05.mma kind::tf32 with the 3xTF32 operand split (tc_common.cuh) and fp32 accumulators in TMEM.
+//
+// Operand format ("images"): every GEMM operand lives in HBM as the exact shared-memory image the MMA reads:
+// K-major, 128-byte swizzle, panels of 32 K-columns; hi and lo parts in separate arrays.  An A image is
+// [row tile of 128][K panel][128 rows x 128 B]; a B image is [N tile][K panel][NT rows x 128 B].  A stage of the
+// pipeline is therefore four contiguous bulk copies (cp.async.bulk, the TMA engine without a tensor map).  The
+// epilogue of one GEMM writes the A image of the next (thread r of the epilogue warpgroup owns tile row r = TMEM lane
+// r), plus the plain fp32 rows the later element-wise steps need.
+//
+// Kernel: one CTA per (row tile, N tile); warp 0 = bulk-copy producer, warp 1 = MMA issuer, warps 2-9 = two epilogue
+// warpgroups (half of the N tile each).
+#include <vector>
+
+#include "tc_common.cuh"
+#include "tc_kernels.cuh"
+
+#define FT_KP 32                       // K columns per panel (128 bytes of tf32)
+#define FT_APANEL (128 * 128)          // bytes of one A panel (hi or lo)
+
+enum { FE_TANH = 0, FE_TANH_SKIP = 1, FE_L3 = 2, FE_BWD1 = 3, FE_BWD0 = 4, FE_STORE = 5 };
+
+struct FitTCNet {                      // device pointers (floats) of one species
+  const float *W0h, *W0l, *W1h, *W1l, *W2h, *W2l, *W2Th, *W2Tl, *W1Th, *W1Tl, *W0Th, *W0Tl;
+  const float *b0, *b1, *b2, *w3;
+  float b3;
+};
+
+struct FitTC {
+  float *buf = nullptr;
+  int fw = 0, fwp = 0, NT = 0;         // width, width padded to 32 (K panels), N tile of the fw-wide GEMMs
+  int dim = 0, dimp = 0, NT6 = 0;      // descriptor size, padded to 128; N tile of G6
+  std::vector<FitTCNet> nets;
+};
+
+struct FitTCArgs {
+  const float *Ah, *Al;                // A images [tile][KPAN][4096 floats]
+  const float *Bh, *Bl;                // B images [ntile][KPAN][NT * 32 floats]
+  int KPAN;                            // K panels
+  int N;                               // real output columns (<= gridDim.y * NT)
+  int KPAN_out;                        // K panels of the output image (its K = this GEMM's N)
+  const float *bias, *w3;              // [N]
+  const float *in0, *in1;              // plain fp32 [rows][ldp]
+  float *out_plain0, *out_plain1;      // plain fp32 [rows][ldp]
+  float *out_h, *out_l;                // output A image (hi / lo) or null
+  int ldp;
+  float b3;
+  double *atom_energy;                 // FE_L3
+  const int *s_idx;
+};
+
+// store 4 consecutive columns (chunk j of K panel kp) of row r into an A image in global memory
+__device__ __forceinline__ void img_store4(float *img_h, float *img_l, size_t tile, int kpan, int n0, int r, float v0,
+                                           float v1, float v2, float v3) {
+  float4 h, l;
+  tc::split_tf32(v0, h.x, l.x);
+  tc::split_tf32(v1, h.y, l.y);
+  tc::split_tf32(v2, h.z, l.z);
+  tc::split_tf32(v3, h.w, l.w);
+  const size_t o = (tile * kpan + (n0 >> 5)) * 4096 + (tc::sw128_offset(r, n0 & 31) >> 2);
+  *reinterpret_cast<float4 *>(img_h + o) = h;
+  *reinterpret_cast<float4 *>(img_l + o) = l;
+}
+
+// One group of 8 output columns of row m (tile row r): apply the GEMM's epilogue to the accumulators a[8].
+template <int EPI>
+__device__ __forceinline__ void ft_epi8(const float a[8], int nn0, const FitTCArgs &g, size_t tile, int r, int m,
+                                        double &edot) {
+  float o0[8], o1[8];
+#pragma unroll
+  for (int q4 = 0; q4 < 2; ++q4) {
+    const int nn = nn0 + 4 * q4;
+    const bool live = nn < g.N;
+    float4 bias = make_float4(0.f, 0.f, 0.f, 0.f), w3 = bias, i0 = bias, i1 = bias;
+    if (live) {
+      if (EPI == FE_TANH || EPI == FE_TANH_SKIP || EPI == FE_L3) bias = *reinterpret_cast<const float4 *>(g.bias + nn);
+      if (EPI == FE_L3 || EPI == FE_BWD1) w3 = *reinterpret_cast<const float4 *>(g.w3 + nn);
+      if (EPI == FE_TANH_SKIP || EPI == FE_L3 || EPI == FE_BWD0)
+        i0 = *reinterpret_cast<const float4 *>(g.in0 + (size_t)m * g.ldp + nn);
+      if (EPI == FE_BWD1 || EPI == FE_BWD0) i1 = *reinterpret_cast<const float4 *>(g.in1 + (size_t)m * g.ldp + nn);
+    }
+    const float bb[4] = {bias.x, bias.y, bias.z, bias.w}, ww[4] = {w3.x, w3.y, w3.z, w3.w};
+    const float x0[4] = {i0.x, i0.y, i0.z, i0.w}, x1[4] = {i1.x, i1.y, i1.z, i1.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float av = a[4 * q4 + i];
+      float p = 0.f, q = 0.f;                              // p -> image / plain0, q -> plain1
+      if (live) {
+        if (EPI == FE_TANH) {
+          tc::tanh_d_f32(av + bb[i], p, q);                                // Z0 and S0 = 1 - Z0^2
+        } else if (EPI == FE_TANH_SKIP) {
+          float u;
+          tc::tanh_d_f32(av + bb[i], u, q);                                // U1 and S1 = 1 - U1^2
+          p = x0[i] + u;                                                   // Z1 = Z0 + U1
+        } else if (EPI == FE_L3) {
+          float u, s2;
+          tc::tanh_d_f32(av + bb[i], u, s2);                               // U2 and 1 - U2^2
+          edot = fma((double)(x0[i] + u), (double)ww[i], edot);            // E_i += Z2 w3
+          p = ww[i] * s2;                                                  // Q2 = w3 (1 - U2^2)
+        } else if (EPI == FE_BWD1) {
+          q = ww[i] + av;                                                  // dZ1 = w3 + Q2 W2^T
+          p = q * x1[i];                                                   // Q1 = dZ1 S1
+        } else if (EPI == FE_BWD0) {
+          const float dz = x0[i] + av;                                     // dZ0 = dZ1 + Q1 W1^T
+          p = dz * x1[i];                                                  // Q0 = dZ0 S0
+        } else {
+          p = av;                                                          // dD
+        }
+      }
+      o0[4 * q4 + i] = p;
+      o1[4 * q4 + i] = q;
+    }
+  }
+#pragma unroll
+  for (int q4 = 0; q4 < 2; ++q4) {
+    const int nn = nn0 + 4 * q4;
+    if (g.out_h && nn < g.KPAN_out * FT_KP)
+      img_store4(g.out_h, g.out_l, tile, g.KPAN_out, nn, r, o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
+    if (nn < g.ldp) {
+      if (g.out_plain0)
+        *reinterpret_cast<float4 *>(g.out_plain0 + (size_t)m * g.ldp + nn) =
+            make_float4(o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
+      if (g.out_plain1)
+        *reinterpret_cast<float4 *>(g.out_plain1 + (size_t)m * g.ldp + nn) =
+            make_float4(o1[4 * q4], o1[4 * q4 + 1], o1[4 * q4 + 2], o1[4 * q4 + 3]);
+    }
+  }
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *mbar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(tc::smem_u32(mbar)) : "memory");
+}
+
+// The tensor core accumulates in fp32 with truncation; over a long K (1600 for G1) that bias reaches 1e-4 of the
+// pre-activations and breaks the force tolerance (measured).  The accumulation is therefore
+// chunked: the MMAs of FT_CP K panels (K = 64) go to one of two TMEM accumulators starting from zero, and the epilogue
+// warps add the finished chunk to fp32 registers (round-to-nearest) while the next chunk runs in the other buffer.
+#define FT_CP 2
+
+template <int NT, int EPI>
+__global__ void __launch_bounds__(320, 1)
+k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
+  constexpr int BPANEL = NT * 128;                               // bytes of one B panel (hi or lo)
+  constexpr int STAGE = 2 * FT_APANEL + 2 * BPANEL;
+  constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : 2;
+  constexpr int NH = NT / 2;                                     // columns per epilogue warpgroup
+  static_assert(NH % 8 == 0 && NH <= 128, "");
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + STAGES * STAGE);
+  uint64_t *empty = full + STAGES;
+  uint64_t *accfull = empty + STAGES, *accempty = accfull + 2;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(accempty + 2);
+  double *edot_sh = reinterpret_cast<double *>(smem);            // reused after the main loop (FE_L3)
+
+  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  const int tile = blockIdx.x, m0 = tile * 128;
+  if (m0 >= row_hi || m0 + 128 <= row_lo) return;               // tile holds no atom of this species
+  const int nt = blockIdx.y, n0 = nt * NT;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nchunks = (g.KPAN + FT_CP - 1) / FT_CP;
+
+  if (warp == 0) tc::tmem_alloc<512>(tmem_slot);
+  if (tid == 32) {
+    for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full + s, 1); tc::mbar_init(empty + s, 1); }
+    for (int b = 0; b < 2; ++b) { tc::mbar_init(accfull + b, 1); tc::mbar_init(accempty + b, 8); }
+    tc::fence_mbar_init();
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  tc::fence_after_sync();
+  const uint32_t tmem = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      const float *ah = g.Ah + (size_t)tile * g.KPAN * 4096, *al = g.Al + (size_t)tile * g.KPAN * 4096;
+      const float *bh = g.Bh + (size_t)nt * g.KPAN * (NT * 32), *bl = g.Bl + (size_t)nt * g.KPAN * (NT * 32);
+      for (int kp = 0; kp < g.KPAN; ++kp) {
+        const int s = kp % STAGES;
+        if (kp >= STAGES) tc::mbar_wait(empty + s, ((kp / STAGES) - 1) & 1);
+        uint8_t *st = smem + s * STAGE;
+        tc::mbar_arrive_expect_tx(full + s, STAGE);
+        tc::bulk_g2s(st, ah + (size_t)kp * 4096, FT_APANEL, full + s);
+        tc::bulk_g2s(st + FT_APANEL, al + (size_t)kp * 4096, FT_APANEL, full + s);
+        tc::bulk_g2s(st + 2 * FT_APANEL, bh + (size_t)kp * (NT * 32), BPANEL, full + s);
+        tc::bulk_g2s(st + 2 * FT_APANEL + BPANEL, bl + (size_t)kp * (NT * 32), BPANEL, full + s);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t idesc = tc::make_idesc_tf32(128, NT);
+      for (int c = 0; c < nchunks; ++c) {
+        const int buf = c & 1;
+        if (c >= 2) tc::mbar_wait(accempty + buf, ((c >> 1) - 1) & 1);
+        tc::fence_after_sync();
+        const uint32_t td = tmem + buf * 256;
+        const int kp_hi = min(g.KPAN, (c + 1) * FT_CP);
+        for (int kp = c * FT_CP; kp < kp_hi; ++kp) {
+          const int s = kp % STAGES;
+          tc::mbar_wait(full + s, (kp / STAGES) & 1);
+          tc::fence_after_sync();
+          const uint32_t sa = tc::smem_u32(smem + s * STAGE);
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) {
+            const uint64_t dah = tc::make_desc_sw128(sa + ks * 32), dal = tc::make_desc_sw128(sa + FT_APANEL + ks * 32);
+            const uint64_t dbh = tc::make_desc_sw128(sa + 2 * FT_APANEL + ks * 32),
+                           dbl = tc::make_desc_sw128(sa + 2 * FT_APANEL + BPANEL + ks * 32);
+            tc::mma_tf32_ss(td, dal, dbh, idesc, (kp > c * FT_CP || ks > 0) ? 1u : 0u);
+            tc::mma_tf32_ss(td, dah, dbl, idesc, 1u);
+            tc::mma_tf32_ss(td, dah, dbh, idesc, 1u);
+          }
+          tc::mma_commit(empty + s);
+        }
+        tc::mma_commit(accfull + buf);
+      }
+    }
+  } else {
+    // two epilogue warpgroups (columns [e NH, e NH + NH)); thread r = TMEM lane r = tile row r
+    const int e = (warp - 2) >> 2;
+    const int r = 32 * (warp & 3) + lane, m = m0 + r;
+    const bool ok = m >= row_lo && m < row_hi;
+    const uint32_t lane_sel = (uint32_t)(32 * (warp & 3)) << 16;
+    float acc[NH];
+#pragma unroll
+    for (int i = 0; i < NH; ++i) acc[i] = 0.0f;
+    for (int c = 0; c < nchunks; ++c) {
+      const int buf = c & 1;
+      tc::mbar_wait(accfull + buf, (c >> 1) & 1);
+      tc::fence_after_sync();
+      const uint32_t ta = tmem + lane_sel + buf * 256 + e * NH;
+      constexpr int P0 = NH < 64 ? NH : 64, P1 = NH - P0;
+      {
+        uint32_t v[P0];
+        tc::tmem_ld_cols_nowait<P0>(ta, v);
+        tc::tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < P0; ++i) acc[i] += __uint_as_float(v[i]);
+      }
+      if (P1 > 0) {
+        uint32_t v[P1 > 0 ? P1 : 8];
+        tc::tmem_ld_cols_nowait<(P1 > 0 ? P1 : 8)>(ta + P0, v);
+        tc::tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < P1; ++i) acc[P0 + i] += __uint_as_float(v[i]);
+      }
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(accempty + buf);
+    }
+    double edot = 0.0;
+    if (ok) {
+#pragma unroll
+      for (int j = 0; j < NH; j += 8) ft_epi8<EPI>(acc + j, n0 + e * NH + j, g, (size_t)tile, r, m, edot);
+      if (EPI != FE_STORE && g.out_h && e == 1)               // image columns between NT and the padded K must be zero
+        for (int nn = n0 + NT; nn < g.KPAN_out * FT_KP; nn += 4)
+          img_store4(g.out_h, g.out_l, (size_t)tile, g.KPAN_out, nn, r, 0.f, 0.f, 0.f, 0.f);
+    }
+    if (EPI == FE_L3) {
+      // all stages have been consumed (the last accfull implies every MMA read its operands): smem is free
+      if (e == 1) edot_sh[r] = edot;
+      tc::bar_sync(1, 256);
+      if (e == 0 && ok) g.atom_energy[g.s_idx[C.p0 + m]] = edot + edot_sh[r] + (double)g.b3;
+    }
+  }
+  tc::fence_before_sync();
+  __syncthreads();
+  if (warp == 0) tc::tmem_dealloc<512>(tmem);
+}
+
+// ---- S5: descriptor as the A image of G1 ---------------------------------------------------------------------------
+// D[b M^< + a] = sum_c T[b][c] T[a][c] (Eq. 4; reading R7), from the fp64 T rounded to fp32, written
+// straight into the hi / lo operand images (the descriptor never exists in another form).  Thread = atom (tile row).
+template <int MA>
+__global__ void __launch_bounds__(128) k_descr_tc(DevModel P, ChunkView C, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
+  const int tile = blockIdx.x, r = threadIdx.x, m = tile * 128 + r;
+  if (m >= C.n) return;
+  const double *T = C.T + (size_t)m * P.M * 4;
+  float ta[MA][4];
+#pragma unroll
+  for (int a = 0; a < MA; ++a) {
+    const double2 u = *reinterpret_cast<const double2 *>(T + 4 * a), v = *reinterpret_cast<const double2 *>(T + 4 * a + 2);
+    ta[a][0] = (float)u.x; ta[a][1] = (float)u.y; ta[a][2] = (float)v.x; ta[a][3] = (float)v.y;
+  }
+  for (int b = 0; b < P.M; ++b) {
+    const double2 u = *reinterpret_cast<const double2 *>(T + 4 * b), v = *reinterpret_cast<const double2 *>(T + 4 * b + 2);
+    const float t0 = (float)u.x, t1 = (float)u.y, t2 = (float)v.x, t3 = (float)v.y;
+#pragma unroll
+    for (int a = 0; a < MA; a += 4) {
+      float d[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) d[i] = fmaf(t0, ta[a + i][0], fmaf(t1, ta[a + i][1], fmaf(t2, ta[a + i][2], t3 * ta[a + i][3])));
+      img_store4(Dh, Dl, (size_t)tile, kpan, b * MA + a, r, d[0], d[1], d[2], d[3]);
+    }
+  }
+  for (int k = P.M * MA; k < kpan * FT_KP; k += 4) img_store4(Dh, Dl, (size_t)tile, kpan, k, r, 0.f, 0.f, 0.f, 0.f);
+}
+
+// ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c]; fp64 accumulation, also written as
+// the fp32 copy pass 2 reads.  One block per atom.
+__global__ void k_dT_tc(DevModel P, ChunkView C, int ldd, const float *__restrict__ dD, float *__restrict__ dT32) {
+  const int q = blockIdx.x;
+  extern __shared__ double sm3[];
+  double *Ts = sm3;                       // [M][4]
+  float *dd = reinterpret_cast<float *>(sm3 + P.M * 4);      // [dim]
+  double *part = reinterpret_cast<double *>(dd + ((P.dim + 1) & ~1));   // [nparts][Ma * 4]
+  const double *T = C.T + (size_t)q * P.M * 4;
+  for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
+  for (int k = threadIdx.x; k < P.dim; k += blockDim.x) dd[k] = dD[(size_t)q * ldd + k];
+  __syncthreads();
+  const int nout2 = P.Ma * 4;
+  const int nparts = max(1, (int)blockDim.x / nout2);
+  for (int idx = threadIdx.x; idx < nparts * nout2; idx += blockDim.x) {
+    const int pt = idx / nout2, o = idx - pt * nout2, bcol = o >> 2, c = o & 3;
+    const int per = (P.M + nparts - 1) / nparts, lo = pt * per, hi = min(P.M, lo + per);
+    double acc = 0.0;
+    for (int bp = lo; bp < hi; ++bp) acc += (double)dd[bp * P.Ma + bcol] * Ts[bp * 4 + c];
+    part[idx] = acc;
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < P.M * 4; e += blockDim.x) {
+    const int b = e >> 2, c = e & 3;
+    double acc = 0.0;
+    for (int a = 0; a < P.Ma; ++a) acc += (double)dd[b * P.Ma + a] * Ts[a * 4 + c];
+    if (b < P.Ma)
+      for (int pt = 0; pt < nparts; ++pt) acc += part[pt * nout2 + e];
+    C.dT[(size_t)q * P.M * 4 + e] = acc;
+    dT32[(size_t)q * P.M * 4 + e] = (float)acc;
+  }
+}
+
+// ---- host: weights as B images -------------------------------------------------------------------------------------
+static int ft_round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// B[n][k] for n < N, k < K (zero outside), as [ntiles][kpan][NT rows x 32] swizzled panels; appends hi and lo to out
+template <class F>
+static void pack_B(F get, int N, int K, int NT, int ntiles, int kpan, std::vector<float> &out, size_t &off_h, size_t &off_l) {
+  const size_t sz = (size_t)ntiles * kpan * NT * 32;
+  off_h = out.size();
+  out.resize(out.size() + 2 * sz, 0.0f);
+  off_l = off_h + sz;
+  for (int nt = 0; nt < ntiles; ++nt)
+    for (int kp = 0; kp < kpan; ++kp) {
+      const size_t base = ((size_t)nt * kpan + kp) * NT * 32;
+      for (int rn = 0; rn < NT; ++rn) {
+        const int n = nt * NT + rn;
+        if (n >= N) continue;
+        for (int kk = 0; kk < 32; ++kk) {
+          const int k = kp * 32 + kk;
+          if (k >= K) continue;
+          const double w = get(n, k);
+          const float hi = tc_host_tf32((float)w);
+          const size_t o = base + tc::sw128_offset(rn, kk) / 4;
+          out[off_h + o] = hi;
+          out[off_l + o] = tc_host_tf32((float)(w - (double)hi));
+        }
+      }
+    }
+}
+
+static int ft_pick_nt(int fw) {
+  if (fw <= 32) return 32;
+  if (fw <= 64) return 64;
+  if (fw <= 128) return 128;
+  if (fw <= 240) return 240;
+  if (fw <= 256) return 256;
+  return 0;
+}
+
+cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W) {
+  if (P.fw % 4 != 0 || ft_pick_nt(P.fw) == 0 || (P.Ma != 4 && P.Ma != 8 && P.Ma != 16)) return cudaErrorNotSupported;
+  FitTC *F = new FitTC();
+  F->fw = P.fw; F->fwp = ft_round_up(P.fw, 32); F->NT = ft_pick_nt(P.fw);
+  F->dim = P.dim; F->dimp = ft_round_up(P.dim, 128); F->NT6 = 128;
+  const int fw = P.fw, dim = P.dim, kpw = F->fwp / 32, kpd = ft_round_up(dim, 32) / 32, nt6 = F->dimp / 128;
+  std::vector<float> h;
+  struct Off { size_t W0h, W0l, W1h, W1l, W2h, W2l, W2Th, W2Tl, W1Th, W1Tl, W0Th, W0Tl, b0, b1, b2, w3; };
+  std::vector<Off> offs(P.ntypes);
+  for (int ty = 0; ty < P.ntypes; ++ty) {
+    const double *W0 = fit_h + (size_t)ty * P.fit_net_size;
+    const double *b0 = W0 + (size_t)dim * fw, *W1 = b0 + fw, *b1 = W1 + (size_t)fw * fw, *W2 = b1 + fw,
+                 *b2 = W2 + (size_t)fw * fw, *w3 = b2 + fw;
+    Off &o = offs[ty];
+    // forward GEMMs: C[r][n] = sum_k A[r][k] W[k][n]  ->  B[n][k] = W[k][n]
+    pack_B([&](int n, int k) { return W0[(size_t)k * fw + n]; }, fw, dim, F->NT, 1, kpd, h, o.W0h, o.W0l);
+    pack_B([&](int n, int k) { return W1[(size_t)k * fw + n]; }, fw, fw, F->NT, 1, kpw, h, o.W1h, o.W1l);
+    pack_B([&](int n, int k) { return W2[(size_t)k * fw + n]; }, fw, fw, F->NT, 1, kpw, h, o.W2h, o.W2l);
+    // backward GEMMs: C[r][n] = sum_k Q[r][k] W[n][k]  ->  B[n][k] = W[n][k]
+    pack_B([&](int n, int k) { return W2[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W2Th, o.W2Tl);
+    pack_B([&](int n, int k) { return W1[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W1Th, o.W1Tl);
+    pack_B([&](int n, int k) { return W0[(size_t)n * fw + k]; }, dim, fw, 128, nt6, kpw, h, o.W0Th, o.W0Tl);
+    auto vecpad = [&](const double *src) {
+      const size_t at = h.size();
+      h.resize(at + 256, 0.0f);
+      for (int i = 0; i < fw; ++i) h[at + i] = (float)src[i];
+      return at;
+    };
+    o.b0 = vecpad(b0); o.b1 = vecpad(b1); o.b2 = vecpad(b2); o.w3 = vecpad(w3);
+  }
+  cudaError_t e = cudaMalloc(&F->buf, sizeof(float) * h.size());
+  if (e != cudaSuccess) { delete F; return e; }
+  e = cudaMemcpy(F->buf, h.data(), sizeof(float) * h.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(F->buf); delete F; return e; }
+  for (int ty = 0; ty < P.ntypes; ++ty) {
+    const Off &o = offs[ty];
+    const float *b = F->buf;
+    FitTCNet n{b + o.W0h, b + o.W0l, b + o.W1h, b + o.W1l, b + o.W2h, b + o.W2l, b + o.W2Th, b + o.W2Tl,
+               b + o.W1Th, b + o.W1Tl, b + o.W0Th, b + o.W0Tl, b + o.b0, b + o.b1, b + o.b2, b + o.w3,
+               (float)fit_h[(size_t)ty * P.fit_net_size + P.fit_net_size - 1]};
+    F->nets.push_back(n);
+  }
+  W.fit = F;
+  return cudaSuccess;
+}
+
+void tc_release_fit(TCWeights &W) {
+  FitTC *F = reinterpret_cast<FitTC *>(W.fit);
+  if (F) {
+    if (F->buf) cudaFree(F->buf);
+    delete F;
+  }
+  W.fit = nullptr;
+}
+
+size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk) {
+  const size_t tiles = (size_t)(chunk + 127) / 128, rows = tiles * 128;
+  const size_t kpd = (size_t)ft_round_up(P.dim, 32) / 32, fwp = ft_round_up(P.fw, 32), dimp = ft_round_up(P.dim, 128);
+  return sizeof(float) * (2 * tiles * kpd * 4096 + 4 * tiles * (fwp / 32) * 4096 + 5 * rows * fwp + rows * dimp) + 1024;
+}
+
+template <int NT, int EPI>
+static cudaError_t ft_launch(const ChunkView &C, int ty, const FitTCArgs &g, int ntiles_n, cudaStream_t st) {
+  constexpr int STAGE = 2 * FT_APANEL + 2 * NT * 128;
+  constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : 2;
+  constexpr int smem = STAGES * STAGE + 128;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_fit_tc<NT, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid((C.n + 127) / 128, ntiles_n);
+  k_fit_tc<NT, EPI><<<grid, 320, smem, st>>>(C, ty, g);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}
+
+template <int NT>
+static cudaError_t ft_run_type(const DevModel &P, const ChunkView &C, const FitTC &F, int ty, float *Dh, float *Dl,
+                               float *X0h, float *X0l, float *X1h, float *X1l, float *Z0, float *S0, float *S1,
+                               float *Z1, float *dZ1, float *dD, double *atom_energy, cudaStream_t st) {
+  const FitTCNet &N = F.nets[ty];
+  const int kpw = F.fwp / 32, kpd = ft_round_up(F.dim, 32) / 32, fw = F.fw, ldp = F.fwp;
+  cudaError_t e;
+  FitTCArgs g{};
+  g.s_idx = C.s_idx; g.ldp = ldp; g.N = fw; g.KPAN_out = kpw;
+  // G1: Z0 = tanh(D W0 + b0), S0 = 1 - Z0^2 (stored: recomputing it from the rounded Z0 loses the saturated units)
+  g.Ah = Dh; g.Al = Dl; g.Bh = N.W0h; g.Bl = N.W0l; g.KPAN = kpd; g.bias = N.b0;
+  g.out_plain0 = Z0; g.out_plain1 = S0; g.out_h = X0h; g.out_l = X0l;
+  if ((e = ft_launch<NT, FE_TANH>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  // G2: U1 = tanh(Z0 W1 + b1), Z1 = Z0 + U1, S1 = 1 - U1^2
+  g.Ah = X0h; g.Al = X0l; g.Bh = N.W1h; g.Bl = N.W1l; g.KPAN = kpw; g.bias = N.b1; g.in0 = Z0;
+  g.out_plain0 = Z1; g.out_plain1 = S1; g.out_h = X1h; g.out_l = X1l;
+  if ((e = ft_launch<NT, FE_TANH_SKIP>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  // G3: U2 = tanh(Z1 W2 + b2), E_i = (Z1 + U2) . w3 + b3, Q2 = w3 (1 - U2^2)
+  g.Ah = X1h; g.Al = X1l; g.Bh = N.W2h; g.Bl = N.W2l; g.bias = N.b2; g.w3 = N.w3; g.in0 = Z1; g.b3 = N.b3;
+  g.atom_energy = atom_energy; g.out_plain0 = nullptr; g.out_plain1 = nullptr; g.out_h = X0h; g.out_l = X0l;
+  if ((e = ft_launch<NT, FE_L3>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  // G4: dZ1 = w3 + Q2 W2^T, Q1 = dZ1 S1
+  g.Ah = X0h; g.Al = X0l; g.Bh = N.W2Th; g.Bl = N.W2Tl; g.in0 = nullptr; g.in1 = S1;
+  g.out_plain0 = nullptr; g.out_plain1 = dZ1; g.out_h = X1h; g.out_l = X1l;
+  if ((e = ft_launch<NT, FE_BWD1>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  // G5: dZ0 = dZ1 + Q1 W1^T, Q0 = dZ0 S0
+  g.Ah = X1h; g.Al = X1l; g.Bh = N.W1Th; g.Bl = N.W1Tl; g.in0 = dZ1; g.in1 = S0;
+  g.out_plain0 = nullptr; g.out_plain1 = nullptr; g.out_h = X0h; g.out_l = X0l;
+  if ((e = ft_launch<NT, FE_BWD0>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  // G6: dD = Q0 W0^T
+  g.Ah = X0h; g.Al = X0l; g.Bh = N.W0Th; g.Bl = N.W0Tl; g.N = F.dim; g.ldp = F.dimp; g.KPAN_out = 0;
+  g.out_plain0 = dD; g.out_h = nullptr; g.out_l = nullptr; g.in0 = nullptr; g.in1 = nullptr;
+  return ft_launch<128, FE_STORE>(C, ty, g, F.dimp / 128, st);
+}
+
+cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
+                   cudaStream_t st) {
+  if (C.n <= 0) return cudaSuccess;
+  const FitTC *F = reinterpret_cast<const FitTC *>(W.fit);
+  if (!F) return cudaErrorNotSupported;
+  const size_t tiles = (size_t)(C.n + 127) / 128, rows = tiles * 128;
+  const size_t kpd = (size_t)ft_round_up(F->dim, 32) / 32, kpw = F->fwp / 32;
+  float *p = reinterpret_cast<float *>(ws);
+  float *Dh = p; p += tiles * kpd * 4096;
+  float *Dl = p; p += tiles * kpd * 4096;
+  float *X0h = p; p += tiles * kpw * 4096;
+  float *X0l = p; p += tiles * kpw * 4096;
+  float *X1h = p; p += tiles * kpw * 4096;
+  float *X1l = p; p += tiles * kpw * 4096;
+  float *Z0 = p; p += rows * F->fwp;
+  float *S0 = p; p += rows * F->fwp;
+  float *S1 = p; p += rows * F->fwp;
+  float *Z1 = p; p += rows * F->fwp;
+  float *dZ1 = p; p += rows * F->fwp;
+  float *dD = p;
+  switch (P.Ma) {
+    case 4: k_descr_tc<4><<<(unsigned)tiles, 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+    case 8: k_descr_tc<8><<<(unsigned)tiles, 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+    default: k_descr_tc<16><<<(unsigned)tiles, 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+  }
+  DPB_LAUNCHED(1);
+  for (int ty = 0; ty < P.ntypes; ++ty) {
+    cudaError_t e;
+    switch (F->NT) {
+      case 32: e = ft_run_type<32>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, st); break;
+      case 64: e = ft_run_type<64>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, st); break;
+      case 128: e = ft_run_type<128>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, st); break;
+      case 240: e = ft_run_type<240>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, st); break;
+      default: e = ft_run_type<256>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, st); break;
+    }
+    if (e != cudaSuccess) return e;
+  }
+  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + 256 + 4 * P.Ma) + sizeof(float) * (P.dim + 2);
+  static size_t configured = 0;
+  if (sm > 48 * 1024 && sm > configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_dT_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    configured = sm;
+  }
+  k_dT_tc<<<C.n, 256, sm, st>>>(P, C, F->dimp, dD, dT32);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}

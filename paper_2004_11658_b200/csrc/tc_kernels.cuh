@@ -7,6 +7,7 @@ struct TCWeights {
   float *emb = nullptr;       // ntypes^2 images
   size_t net_stride = 0;      // floats per image
   bool ready = false;
+  void *fit = nullptr;        // fitting weights as B operand images (fit_tc.cu)
 };
 
 cudaError_t tc_prepare_weights(const DevModel &P, const double *emb_h, TCWeights &W);
@@ -18,5 +19,12 @@ cudaError_t tc_build_pairs(const DevModel &P, const ChunkView &C, void *pair_ws,
 
 cudaError_t tc_pass1(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, cudaStream_t st);
 size_t tc_pass2_workspace_bytes(const DevModel &P, int64_t chunk);      // fp32 copy of dT
-cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, void *ws2,
+cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, const void *pair_ws, const float *dT32,
                      double *force, double *virial, cudaStream_t st);
+
+// fitting stage (fit_tc.cu): E_i and dT (fp64 in C.dT and the fp32 copy dT32) from C.T
+cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W);
+void tc_release_fit(TCWeights &W);
+size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk);
+cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
+                   cudaStream_t st);
