@@ -2,6 +2,7 @@
 """bench.py — throughput of one DP energy / force / virial evaluation (the whole hot path, S1..S9) on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload W24k|Cu32k|W192|Cu864k] [--variant 0|1]
+                    [--precision fp64|tf32]      # tf32 = BASELINE.json configs[3] (mixed precision, tcgen05 kernels)
     python bench.py --impl reference ...     # times the CPU oracle (the baseline arm) on a bounded sample
 
 A "step" is one dpb_eval over one freshly perturbed copy of the workload's box (BASELINE.json config: positions
@@ -34,6 +35,15 @@ from gen.weights import MODELS  # noqa: E402
 
 METRIC = "atom-steps/s"
 FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; measured 37.0
+
+
+def tf32_peak_tflops():
+    """Dense TF32 tensor peak = the measured bf16 cuBLAS burst figure (MEASURED_PEAKS.json) x the nominal ratio 1/2
+    (B200_PROFILING.md: 2.25 PF bf16, 1.1 PF tf32); fallback 1590 / 2."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["bf16_tflops"]) / 2.0, "measured bf16 x 1/2"
+    except Exception:
+        return 1590.0 / 2.0, "fallback bf16 x 1/2"
 
 
 # ---- algorithmic work (SURVEY.md §8(d); DESIGN.md "Algorithmic work per unit") -------------------------------
@@ -163,7 +173,8 @@ def workload_config(name, args):
             "weights": "random-init N(0,1/fan_in), biases N(0,1), seeded",
             "perturbation_sigma_A": 0.01, "neighbour_build": "every step",
             "parallelism": "replicas only (1 GPU per replica, no collectives)",
-            "l2": "flushed between timed steps (256 MiB write)", "variant": getattr(args, "variant", 1)}
+            "l2": "flushed between timed steps (256 MiB write)", "variant": getattr(args, "variant", 1),
+            "precision": getattr(args, "precision", "fp64")}
 
 
 # ---- the CUDA arm ---------------------------------------------------------------------------------------------
@@ -187,7 +198,8 @@ def run_cuda(args):
     coord, types, box = gen.make_system(name, seed=gen.SEED_BASE + gen.CONFIGS[name].config_id + 7919 * rank)
     emb, fit = gen.make_weights(spec)
     n = coord.shape[0]
-    model = DPModel.from_spec(spec, emb, fit)
+    mixed = args.precision == "tf32"
+    model = DPModel.from_spec(spec, emb, fit, precision=1 if mixed else 0)
     model.set_variant(args.variant)
     model.set_timing(True)
 
@@ -279,13 +291,14 @@ def run_cuda(args):
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get(f"{name}:v{args.variant}:{dom[0]}")
+                traffic = json.load(open(tpath)).get(f"{name}:{'tf32' if mixed else 'v' + str(args.variant)}:{dom[0]}")
             except Exception:
                 traffic = None
         line = {
             "metric": METRIC, "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(name, args),
+            "vs_baseline": None, "dtype": "tf32x3+f32acc (env/force/accumulations f64)" if mixed else "f64",
+            "data": "synthetic", "config": workload_config(name, args),
             "natoms_per_gpu": n, "real_pairs": info.n_real_pairs, "wall_s": wall,
             "algorithmic_tflops": total_flops / (ms_per_step * 1e-3) / 1e12,
             "fp64_frac_of_peak": total_flops / (ms_per_step * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
@@ -302,6 +315,15 @@ def run_cuda(args):
                        "reasons": clocks.get("reasons", []), "samples": clocks.get("samples", 0),
                        "power_w_max": clocks.get("power_w_max")},
         }
+        if mixed:
+            # the GEMMs run on the tensor pipe: 3 TF32 MMAs per algorithmic product (3xTF32 split)
+            peak, how = tf32_peak_tflops()
+            line["roofline"] = {"bound": "tensor", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                                "note": f"algorithmic flops of the stage / its CUDA-event time against the dense TF32 peak "
+                                        f"({how}); the tensor pipe executes 3x these flops (3xTF32 split); the stage is bound "
+                                        f"by MUFU (fp32 tanh) and instruction issue, not by the tensor pipe (DESIGN.md)"}
+            line.pop("fp64_frac_of_peak", None)
         if world == 1 and not args.no_cpu_baseline:
             step, k, desc, threads = oracle_step_sampler(name, gen.SEED_BASE, args.ref_sample)
             step()
@@ -325,6 +347,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="W24k", choices=sorted(MODELS))
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "tf32"])
     ap.add_argument("--variant", type=int, default=int(os.environ.get("DPB_VARIANT", "1")))
     ap.add_argument("--ref-sample", type=int, default=2048, help="atoms per step of the CPU oracle arm")
     ap.add_argument("--stage-every", type=int, default=10, help="read the stage timers every n-th step (0: never)")

@@ -26,8 +26,11 @@ typedef struct dpb_model dpb_model;   /* opaque; owns device copies of the weigh
 
 typedef enum {
   DPB_FP64 = 0,   /* everything in fp64 (the paper's precision)                              */
-  DPB_TF32 = 1,   /* reserved: embedding / fitting GEMM operands in TF32, fp32 accumulate (BASELINE cfg 3) */
-  DPB_BF16 = 2    /* reserved: same with BF16 operands                                                     */
+  DPB_TF32 = 1,   /* mixed precision (BASELINE.json configs[3]): embedding and fitting GEMM operands in TF32 with
+                     the error-compensated 3xTF32 split, fp32 accumulate (tcgen05 / TMEM), tanh in fp32; neighbour
+                     list, env matrix, chain to the displacement and the T, F, virial, E accumulations in fp64.
+                     Built for emb_s1 in {8, 16, 25, 32}, m_axis in {4, 8, 16}, fit_width % 4 == 0 and <= 256.   */
+  DPB_BF16 = 2    /* reserved (BF16 operand variant): DPB_ENOTIMPL in this build                             */
 } dpb_precision;
 
 typedef enum {
@@ -64,7 +67,7 @@ typedef struct {
 } dpb_eval_info;
 
 /* Create / destroy.  dpb_model_create copies (and re-lays-out) the weights to the current CUDA device.
- * Errors: DPB_EINVAL (shape), DPB_ENOTIMPL (precision != DPB_FP64 in this build), DPB_ENOMEM, DPB_ECUDA. */
+ * Errors: DPB_EINVAL (shape), DPB_ENOTIMPL (DPB_BF16; DPB_TF32 with an unsupported shape), DPB_ENOMEM, DPB_ECUDA. */
 int dpb_model_create(const dpb_model_desc *desc, int precision, dpb_model **out);
 int dpb_model_destroy(dpb_model *model);
 

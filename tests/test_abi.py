@@ -41,7 +41,7 @@ def test_version_and_error_strings(lib):
 
 
 def test_create_rejects_bad_arguments_without_a_gpu(lib):
-    """Argument validation happens before any CUDA call: EINVAL for null pointers, ENOTIMPL for reserved precisions."""
+    """Argument validation happens before any CUDA call: EINVAL for null pointers, ENOTIMPL for precisions that are not built."""
     out = ctypes.c_void_p()
     assert lib.dpb_model_create(None, 0, ctypes.byref(out)) == -1
 
@@ -50,7 +50,8 @@ def test_create_rejects_bad_arguments_without_a_gpu(lib):
                     ("sel", ctypes.c_void_p), ("emb_s1", ctypes.c_int32), ("m_axis", ctypes.c_int32),
                     ("fit_width", ctypes.c_int32), ("emb", ctypes.c_void_p), ("fit", ctypes.c_void_p)]
     d = Desc(1, 6.0, 0.5, None, 25, 16, 240, None, None)
-    assert lib.dpb_model_create(ctypes.byref(d), 1, ctypes.byref(out)) == -6      # TF32 reserved
+    assert lib.dpb_model_create(ctypes.byref(d), 2, ctypes.byref(out)) == -6      # BF16 variant: not built
+    assert lib.dpb_model_create(ctypes.byref(d), 1, ctypes.byref(out)) == -1      # TF32 is built: null sel / weights
     assert lib.dpb_model_create(ctypes.byref(d), 0, ctypes.byref(out)) == -1      # null sel / weights
     assert not out.value
 
@@ -66,6 +67,23 @@ def test_sass_is_sm100a_with_fp64_tensor_core_tiles():
     out = subprocess.run([cuobjdump, "-lelf", build.build()], capture_output=True, text=True).stdout
     archs = set(re.findall(r"sm_\d+a?", out))
     assert archs == {"sm_100a"}, archs
+
+
+def test_mixed_precision_kernels_use_tcgen05_and_tmem():
+    """The DPB_TF32 kernels are Blackwell-native: tcgen05.mma (SASS UTC*MMA), TMEM loads (LDTM) and bulk copies
+    (UBLKCP) appear in the SASS of the embedding / fitting objects; no legacy HMMA path."""
+    import shutil
+    import subprocess
+    from paper_2004_11658_b200 import build
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    build.build()
+    for obj, must in (("embed_tc.o", ("UTCHMMA", "LDTM")), ("fit_tc.o", ("UTCHMMA", "LDTM", "UBLKCP"))):
+        sass = subprocess.run([cuobjdump, "-sass", os.path.join(build.OBJ, obj)], capture_output=True, text=True).stdout
+        for mnem in must:
+            assert mnem in sass, (obj, mnem)
+        assert " HMMA" not in sass
 
 
 def test_binding_fails_loudly_without_cuda():

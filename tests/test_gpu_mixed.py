@@ -1,0 +1,167 @@
+"""GPU parity tests of the mixed-precision path (BASELINE.json configs[3], DPB_TF32): embedding and fitting GEMMs on
+tcgen05 with TF32 operands (3xTF32 split) and fp32 accumulate, tanh in fp32; neighbour list, environment matrix,
+chain to the displacement and the T / F / virial / E accumulations in fp64.
+
+Bars (BASELINE.json north_star, mixed precision): nlist bit-exact; relative error <= 1e-5 on E; absolute error
+<= 1e-3 eV/A on F — against the fp64 CPU oracle, on the literal AND the conditioned weight set."""
+import numpy as np
+import pytest
+
+import gen
+from gen.weights import MODELS, ModelSpec
+
+from conftest import random_box
+
+pytestmark = pytest.mark.gpu
+
+E_REL = 1e-5
+F_ABS = 1e-3
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (the library has no CPU fallback)")
+    return torch
+
+
+def _model(spec, emb, fit, precision):
+    from paper_2004_11658_b200 import DPModel
+    return DPModel.from_spec(spec, emb, fit, precision=precision)
+
+
+def _eval(m, coord, types, box, spec=None, debug=False):
+    torch = _torch()
+    dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda")
+    dbg = None
+    if debug:
+        T = torch.zeros((coord.shape[0], spec.m, 4), dtype=torch.float64, device="cuda")
+        dT = torch.zeros_like(T)
+        m.set_debug_buffers(T, None, dT)
+        dbg = (T, dT)
+    out = m.eval(dc, dt, box, want_nlist=True, want_info=True)
+    torch.cuda.synchronize()
+    res = {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in out.items()}
+    if debug:
+        res["T"], res["dT"] = dbg[0].cpu().numpy(), dbg[1].cpu().numpy()
+        m.set_debug_buffers(None, None, None)
+    return res
+
+
+def _check(ref, got):
+    assert np.array_equal(got["nlist"], ref["nlist"]), "nlist must be bit-exact also in mixed precision"
+    e_ref = ref["energy"]
+    assert abs(e_ref) >= 1e-3 * np.abs(ref["atom_energy"]).sum()
+    assert abs(got["energy"][0] - e_ref) <= E_REL * abs(e_ref)
+    assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
+    assert np.abs(got["atom_energy"] - ref["atom_energy"]).max() <= 1e-4 * max(1.0, np.abs(ref["atom_energy"]).max())
+    assert np.abs(got["virial"] - ref["virial"]).max() <= 1e-4 * max(1.0, np.abs(ref["virial"]).max())
+    assert np.abs(got["force"].sum(0)).max() <= 1e-9          # F_j -= f, F_i += f in fp64: exact up to fp64 rounding
+
+
+@pytest.mark.parametrize("conditioned", [False, True])
+def test_water192_mixed_vs_oracle(conditioned):
+    from oracle import Oracle
+    from paper_2004_11658_b200.binding import TF32
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    if conditioned:
+        fit = gen.condition_fit_w0(spec, fit)
+    orc = Oracle.from_spec(spec, emb, fit)
+    ref = orc.eval(coord, types, box)
+    m = _model(spec, emb, fit, TF32)
+    got = _eval(m, coord, types, box, spec=spec, debug=True)
+    _check(ref, got)
+    ar = orc.atom_rows(coord, types, box, None, ref["nlist"], want_T=True)
+    assert np.abs(got["T"] - ar["T"]).max() <= 2e-6 * np.abs(ar["T"]).max()        # fp32-level, not TF32-level
+    assert np.abs(got["dT"] - ar["dT"]).max() <= 1e-3 * np.abs(ar["dT"]).max()
+    m.close()
+
+
+@pytest.mark.parametrize("conditioned", [False, True])
+def test_copper_small_mixed_vs_oracle(conditioned):
+    """Copper model (sel 512, 32-64-128, one species) on a 6x6x6-cell FCC box: 864 atoms = 7 row tiles with a ragged
+    tail; every atom's neighbour section (176+ rows) spans two 128-pair tiles."""
+    from oracle import Oracle
+    from paper_2004_11658_b200.binding import TF32
+    spec = MODELS["Cu32k"]
+    coord, types, box = gen.copper_box(6, 0.05, seed=gen.SEED_BASE + 2)
+    emb, fit = gen.make_weights(spec)
+    if conditioned:
+        fit = gen.condition_fit_w0(spec, fit)
+    ref = Oracle.from_spec(spec, emb, fit).eval(coord, types, box)
+    m = _model(spec, emb, fit, TF32)
+    _check(ref, _eval(m, coord, types, box))
+    m.close()
+
+
+@pytest.mark.parametrize("chunk", [1, 100, 100000])
+def test_mixed_chunking(chunk):
+    """Chunks that straddle the species boundary and 128-row tiles holding both species."""
+    from oracle import Oracle
+    from paper_2004_11658_b200.binding import TF32
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    ref = Oracle.from_spec(spec, emb, fit).eval(coord, types, box)
+    m = _model(spec, emb, fit, TF32)
+    m.set_chunk(chunk)
+    _check(ref, _eval(m, coord, types, box))
+    m.close()
+
+
+def test_mixed_small_widths_three_types():
+    """s1 = 8, M^< = 4, fitting width 32, three species on a random box with unsorted types: the smallest shapes the
+    tensor-core kernels are instantiated for (padding of every operand panel, ntypes^2 = 9 nets)."""
+    from oracle import Oracle
+    from paper_2004_11658_b200.binding import TF32
+    spec = ModelSpec("tiny3", 3, 3.5, 0.8, (8, 12, 9), 8, 4, 32, 0)
+    emb, fit = gen.make_weights(spec, seed=21)
+    fit = gen.condition_fit_w0(spec, fit, scale=0.05)
+    coord, types, box = random_box(200, 9.5, 3, seed=6, min_dist=0.9)
+    ref = Oracle.from_spec(spec, emb, fit).eval(coord, types, box)
+    m = _model(spec, emb, fit, TF32)
+    _check(ref, _eval(m, coord, types, box))
+    m.close()
+
+
+@pytest.mark.parametrize("name", ["W24k", "Cu32k"])
+def test_mixed_full_size(name):
+    """BASELINE configs[3] (W24k in mixed precision; Cu32k as well) at full size in the launch configuration bench.py
+    times: sampled atoms against the oracle (nlist rows bit-exact, E_i), and E / F of every atom against the fp64
+    CUDA path (itself held to 1e-10 / 1e-9 against the oracle by test_gpu_parity.py), literal weights."""
+    from oracle import Oracle
+    from paper_2004_11658_b200.binding import TF32, FP64
+    spec = MODELS[name]
+    coord, types, box = gen.make_system(name)
+    emb, fit = gen.make_weights(spec)
+    orc = Oracle.from_spec(spec, emb, fit)
+    m = _model(spec, emb, fit, TF32)
+    got = _eval(m, coord, types, box)
+    m.close()
+    m64 = _model(spec, emb, fit, FP64)
+    r64 = _eval(m64, coord, types, box)
+    m64.close()
+    rows = np.random.default_rng(4).choice(coord.shape[0], 32, replace=False).astype(np.int64)
+    nl_ref, _ = orc.build_nlist(coord, types, box, rows=rows)
+    assert np.array_equal(got["nlist"][rows], nl_ref)
+    ar = orc.atom_rows(coord, types, box, rows, nl_ref)
+    assert np.abs(got["atom_energy"][rows] - ar["atom_energy"]).max() <= 1e-4 * max(1.0, np.abs(ar["atom_energy"]).max())
+    assert np.array_equal(got["nlist"], r64["nlist"])
+    assert abs(got["energy"][0] - r64["energy"][0]) <= E_REL * abs(r64["energy"][0])
+    assert np.abs(got["force"] - r64["force"]).max() <= F_ABS
+    assert np.abs(got["force"].sum(0)).max() <= 1e-8
+    assert np.abs(got["virial"] - r64["virial"]).max() <= 1e-4 * np.abs(r64["virial"]).max()
+
+
+def test_mixed_unsupported_shapes_and_bf16_are_reported():
+    from paper_2004_11658_b200 import DPBError
+    from paper_2004_11658_b200.binding import TF32, BF16
+    from conftest import small_model
+    spec, emb, fit = small_model(ntypes=1, s1=5, m_axis=3, fit_width=9)
+    for prec in (TF32, BF16):
+        with pytest.raises(DPBError) as e:
+            _model(spec, emb, fit, prec)
+        assert e.value.status == -6
