@@ -299,36 +299,65 @@ __global__ void __launch_bounds__(128) k_descr_tc(DevModel P, ChunkView C, int k
   for (int k = P.M * MA; k < kpan * FT_KP; k += 4) img_store4(Dh, Dl, (size_t)tile, kpan, k, r, 0.f, 0.f, 0.f, 0.f);
 }
 
-// ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c]; fp64 accumulation, also written as
-// the fp32 copy pass 2 reads.  One block per atom.
-__global__ void k_dT_tc(DevModel P, ChunkView C, int ldd, const float *__restrict__ dD, float *__restrict__ dT32) {
-  const int q = blockIdx.x;
-  extern __shared__ double sm3[];
-  double *Ts = sm3;                       // [M][4]
-  float *dd = reinterpret_cast<float *>(sm3 + P.M * 4);      // [dim]
-  double *part = reinterpret_cast<double *>(dd + ((P.dim + 1) & ~1));   // [nparts][Ma * 4]
-  const double *T = C.T + (size_t)q * P.M * 4;
-  for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
-  for (int k = threadIdx.x; k < P.dim; k += blockDim.x) dd[k] = dD[(size_t)q * ldd + k];
-  __syncthreads();
-  const int nout2 = P.Ma * 4;
-  const int nparts = max(1, (int)blockDim.x / nout2);
-  for (int idx = threadIdx.x; idx < nparts * nout2; idx += blockDim.x) {
-    const int pt = idx / nout2, o = idx - pt * nout2, bcol = o >> 2, c = o & 3;
-    const int per = (P.M + nparts - 1) / nparts, lo = pt * per, hi = min(P.M, lo + per);
-    double acc = 0.0;
-    for (int bp = lo; bp < hi; ++bp) acc += (double)dd[bp * P.Ma + bcol] * Ts[bp * 4 + c];
-    part[idx] = acc;
+// ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c] (one of the S7 contractions: fp32
+// products and sums like the GEMMs), written as fp64 (debug / ABI view) and as the fp32 copy pass 2 reads.
+// One WARP per atom, no block barrier: the atom's dD row (row stride M^< + 1: conflict-free column access) and an fp32
+// copy of T are staged in the warp's shared-memory slice.  First term: lane = b, all four c (one broadcast float4 of
+// T[a] per a).  Second term: lane = (a, half of the b' range), halves combined by one shuffle.  M^< in {4, 8, 16}.
+#define DT_WARPS 8
+__global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C, int ldd, int log2ma,
+                                                         const float *__restrict__ dD, float *__restrict__ dT32) {
+  extern __shared__ float4 sm4[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int q = blockIdx.x * DT_WARPS + warp;
+  if (q >= C.n) return;
+  const int M = P.M, Ma = 1 << log2ma, dim = P.dim, ldr = Ma + 1;
+  const int per4 = M + Ma + (M * ldr + 3) / 4;                  // float4 per warp slice
+  float4 *Ts = sm4 + warp * per4;                               // [M]   T[b][0..3] in fp32
+  float4 *t2 = Ts + M;                                          // [Ma]  second term
+  float *dd = reinterpret_cast<float *>(t2 + Ma);               // [M][Ma + 1]
+  const double2 *T = reinterpret_cast<const double2 *>(C.T + (size_t)q * M * 4);
+  for (int k = lane; k < M; k += 32) {
+    const double2 u = T[2 * k], v = T[2 * k + 1];
+    Ts[k] = make_float4((float)u.x, (float)u.y, (float)v.x, (float)v.y);
   }
-  __syncthreads();
-  for (int e = threadIdx.x; e < P.M * 4; e += blockDim.x) {
-    const int b = e >> 2, c = e & 3;
-    double acc = 0.0;
-    for (int a = 0; a < P.Ma; ++a) acc += (double)dd[b * P.Ma + a] * Ts[a * 4 + c];
-    if (b < P.Ma)
-      for (int pt = 0; pt < nparts; ++pt) acc += part[pt * nout2 + e];
-    C.dT[(size_t)q * P.M * 4 + e] = acc;
-    dT32[(size_t)q * P.M * 4 + e] = (float)acc;
+  const float4 *src = reinterpret_cast<const float4 *>(dD + (size_t)q * ldd);
+  for (int k4 = lane; k4 < dim / 4; k4 += 32) {
+    const float4 v = src[k4];
+    const int k = 4 * k4, o = (k >> log2ma) * ldr + (k & (Ma - 1));      // 4 | Ma: the four values stay in one row
+    dd[o] = v.x; dd[o + 1] = v.y; dd[o + 2] = v.z; dd[o + 3] = v.w;
+  }
+  __syncwarp();
+  // second term: lane = a + Ma * h (h < 32 / Ma parts of the b' range)
+  {
+    const int a = lane & (Ma - 1), h = lane >> log2ma, parts = 32 >> log2ma;
+    const int perp = (M + parts - 1) / parts, lo = h * perp, hi = min(M, lo + perp);
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+    for (int bp = lo; bp < hi; ++bp) {
+      const float d = dd[bp * ldr + a];
+      const float4 tv = Ts[bp];
+      s0 = fmaf(d, tv.x, s0); s1 = fmaf(d, tv.y, s1); s2 = fmaf(d, tv.z, s2); s3 = fmaf(d, tv.w, s3);
+    }
+    for (int off = Ma; off < 32; off <<= 1) {
+      s0 += __shfl_xor_sync(0xffffffffu, s0, off); s1 += __shfl_xor_sync(0xffffffffu, s1, off);
+      s2 += __shfl_xor_sync(0xffffffffu, s2, off); s3 += __shfl_xor_sync(0xffffffffu, s3, off);
+    }
+    if (lane < Ma) t2[a] = make_float4(s0, s1, s2, s3);
+  }
+  __syncwarp();
+  for (int b = lane; b < M; b += 32) {
+    const float *row = dd + b * ldr;
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+    for (int a = 0; a < Ma; ++a) {
+      const float d = row[a];
+      const float4 tv = Ts[a];
+      s0 = fmaf(d, tv.x, s0); s1 = fmaf(d, tv.y, s1); s2 = fmaf(d, tv.z, s2); s3 = fmaf(d, tv.w, s3);
+    }
+    if (b < Ma) { const float4 u = t2[b]; s0 += u.x; s1 += u.y; s2 += u.z; s3 += u.w; }
+    double2 *o = reinterpret_cast<double2 *>(C.dT + ((size_t)q * M + b) * 4);
+    o[0] = make_double2((double)s0, (double)s1);
+    o[1] = make_double2((double)s2, (double)s3);
+    reinterpret_cast<float4 *>(dT32)[(size_t)q * M + b] = make_float4(s0, s1, s2, s3);
   }
 }
 
@@ -520,14 +549,15 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
     }
     if (e != cudaSuccess) return e;
   }
-  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + 256 + 4 * P.Ma) + sizeof(float) * (P.dim + 2);
+  const int log2ma = P.Ma == 4 ? 2 : (P.Ma == 8 ? 3 : 4);
+  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma + ((size_t)P.M * (P.Ma + 1) + 3) / 4);
   static size_t configured = 0;
   if (sm > 48 * 1024 && sm > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_dT_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     configured = sm;
   }
-  k_dT_tc<<<C.n, 256, sm, st>>>(P, C, F->dimp, dD, dT32);
+  k_dT_tc<<<(C.n + DT_WARPS - 1) / DT_WARPS, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, log2ma, dD, dT32);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
