@@ -222,7 +222,7 @@ static int cuda_fail(cudaError_t e, const char *what) {
 static int neighbour_cap(const DevModel &P) {
   int cap = 2 * P.nm;
   if (cap < 256) cap = 256;
-  if (cap > 12288) cap = 12288;       // 16 B per hit: 192 KB of shared memory at most
+  if (cap > 11000) cap = 11000;       // 20 B per hit: 215 KB of shared memory at most
   return cap;
 }
 

@@ -112,35 +112,37 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// S2.  One block per atom (sorted position p).  Shared memory: the stencil's (type, cell) ranges with a prefix sum,
+// S2.  One block per atom (sorted position p).  Shared memory: the stencil's (type, cell-run) ranges with a prefix sum,
 // then the in-range hits S(i,k) = (alpha_j, |r_ij|, j) of Alg. 1 line 4.
+// Cells are numbered z-fastest, so the three z-neighbours of a stencil column are one contiguous run of sorted
+// positions (two runs when the column wraps around the box): 9 x 2 entries per type instead of 27.
 #define NL_THREADS 128
-#define NL_MAX_RANGES (27 * DPB_MAX_TYPES)
+#define NL_ENTRIES (18 * DPB_MAX_TYPES)
+
+struct __align__(16) NlHit { double r; int j; int t; };
 
 __global__ void __launch_bounds__(NL_THREADS)
 k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, const int *__restrict__ start, int cap,
         int *__restrict__ nlist_out, DevStats *stats) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double *hr = reinterpret_cast<double *>(smem_raw);            // [cap] distance
-  int *hj = reinterpret_cast<int *>(hr + cap);                    // [cap] atom index j
-  int *hp = hj + cap;                                             // [cap] sorted position of j
-  int *ht = hp + cap;                                             // [cap] type of j
-  __shared__ int r_start[NL_MAX_RANGES], r_pref[NL_MAX_RANGES + 1], r_type[NL_MAX_RANGES];
+  NlHit *hit = reinterpret_cast<NlHit *>(smem_raw);               // [cap] (distance, atom index j, type of j)
+  int *hp = reinterpret_cast<int *>(hit + cap);                   // [cap] sorted position of j
+  __shared__ int r_start[NL_ENTRIES], r_pref[NL_ENTRIES + 1], r_type[NL_ENTRIES];
   __shared__ int n_ranges, n_hit, cnt[DPB_MAX_TYPES];
 
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31;
   const int q = blockIdx.x;             // row inside the chunk
   const int p = C.p0 + q;               // sorted position
   const int i = C.s_idx[p];
   const double xi[3] = {s_xyz[3 * (size_t)p], s_xyz[3 * (size_t)p + 1], s_xyz[3 * (size_t)p + 2]};
 
-  // stencil ranges: one thread per (type, stencil cell), then a serial compaction of the <= 27 ntypes entries
-  __shared__ int c_start[NL_MAX_RANGES], c_cnt[NL_MAX_RANGES];
-  for (int ent = tid; ent < 27 * P.ntypes; ent += NL_THREADS) {
-    // cell of atom i, recomputed exactly as in k_keys
+  if (tid < DPB_MAX_TYPES) cnt[tid] = 0;
+  if (tid == 0) n_hit = 0;
+  // stencil ranges, built and compacted by warp 0 (ballot + warp scan): entry = (type, x offset, y offset, part)
+  if (tid < 32) {
     int ic[3], lo[3], num[3];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
+    for (int c = 0; c < 3; ++c) {                                  // cell of atom i, recomputed exactly as in k_keys
       double f = xi[c] / G.L[c];
       f -= floor(f);
       int v = (int)(f * G.nc[c]);
@@ -148,34 +150,44 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
       ic[c] = v >= G.nc[c] ? G.nc[c] - 1 : v;
       if (G.lo_mode[c]) { lo[c] = ic[c] - 1; num[c] = 3; } else { lo[c] = 0; num[c] = G.nc[c]; }
     }
-    const int t = ent / 27, w = ent - 27 * t;
-    const int a = w / 9, b = (w / 3) % 3, c = w % 3;
-    int cntv = 0, s0 = 0;
-    if (a < num[0] && b < num[1] && c < num[2]) {      // fewer than 3 cells in a dimension: each cell once
-      const int ja = (lo[0] + a + G.nc[0]) % G.nc[0];
-      const int jb = (lo[1] + b + G.nc[1]) % G.nc[1];
-      const int jc = (lo[2] + c + G.nc[2]) % G.nc[2];
-      const int k = t * G.ncell + (ja * G.nc[1] + jb) * G.nc[2] + jc;
-      s0 = start[k];
-      cntv = start[k + 1] - s0;
-    }
-    c_start[ent] = s0;
-    c_cnt[ent] = cntv;
-  }
-  __syncthreads();
-  if (tid == 0) {
+    // z runs: [z0, z0 + len0) and, if the stencil wraps, [z1, z1 + len1)
+    int z0, len0, z1 = 0, len1 = 0;
+    if (!G.lo_mode[2]) { z0 = 0; len0 = G.nc[2]; }
+    else if (lo[2] < 0) { z0 = 0; len0 = 2; z1 = G.nc[2] - 1; len1 = 1; }
+    else if (lo[2] + 2 >= G.nc[2]) { z0 = lo[2]; len0 = 2; z1 = 0; len1 = 1; }
+    else { z0 = lo[2]; len0 = 3; }
+    const int nent = 18 * P.ntypes;
     int nr = 0, run = 0;
-    for (int e = 0; e < 27 * P.ntypes; ++e) {
-      const int cv = c_cnt[e];
-      if (cv > 0) {
-        r_start[nr] = c_start[e]; r_pref[nr] = run; r_type[nr] = e / 27;
-        run += cv; ++nr;
+    for (int base = 0; base < nent; base += 32) {
+      const int ent = base + lane;
+      int cntv = 0, s0 = 0, t = 0;
+      if (ent < nent) {
+        t = ent / 18;
+        const int w = ent - 18 * t, part = w & 1, ab = w >> 1, a = ab / 3, b = ab - 3 * a;
+        const int zz = part ? z1 : z0, ln = part ? len1 : len0;
+        if (a < num[0] && b < num[1] && ln > 0) {                  // fewer than 3 cells in a dimension: each cell once
+          const int ja = (lo[0] + a + G.nc[0]) % G.nc[0];
+          const int jb = (lo[1] + b + G.nc[1]) % G.nc[1];
+          const int k = t * G.ncell + (ja * G.nc[1] + jb) * G.nc[2] + zz;
+          s0 = start[k];
+          cntv = start[k + ln] - s0;
+        }
       }
+      const unsigned m = __ballot_sync(0xffffffffu, cntv > 0);
+      int incl = cntv;                                             // inclusive warp scan of the counts
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += v;
+      }
+      if (cntv > 0) {
+        const int pos = nr + __popc(m & ((1u << lane) - 1u));
+        r_start[pos] = s0; r_pref[pos] = run + incl - cntv; r_type[pos] = t;
+      }
+      nr += __popc(m);
+      run += __shfl_sync(0xffffffffu, incl, 31);
     }
-    r_pref[nr] = run;
-    n_ranges = nr;
-    n_hit = 0;
-    for (int t = 0; t < DPB_MAX_TYPES; ++t) cnt[t] = 0;
+    if (lane == 0) { r_pref[nr] = run; n_ranges = nr; }
   }
   __syncthreads();
 
@@ -192,7 +204,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
       const int t = r_type[rp];
       atomicAdd(&cnt[t], 1);
       const int h = atomicAdd(&n_hit, 1);
-      if (h < cap) { hr[h] = r; hj[h] = C.s_idx[pj]; hp[h] = pj; ht[h] = t; }
+      if (h < cap) { hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t; hp[h] = pj; }
     }
   }
   __syncthreads();
@@ -209,17 +221,23 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   // Alg. 1 line 7: order by (type, distance, index).  rank = number of hits of the same type that
   // precede this one; the first sel[t] go to section t (line 8-9, :186-193), the others are dropped (reading R8).
   for (int h = tid; h < nh; h += NL_THREADS) {
-    const double r = hr[h];
-    const int j = hj[h], t = ht[h];
-    int rank = 0;
-    for (int g = 0; g < nh; ++g) {
-      const double rg = hr[g];
-      rank += (ht[g] == t) && (rg < r || (rg == r && hj[g] < j));
+    const NlHit me = hit[h];
+    int rank0 = 0, rank1 = 0;
+    int g = 0;
+    for (; g + 1 < nh; g += 2) {
+      const NlHit u = hit[g], v = hit[g + 1];
+      rank0 += (u.t == me.t) & ((u.r < me.r) | ((u.r == me.r) & (u.j < me.j)));
+      rank1 += (v.t == me.t) & ((v.r < me.r) | ((v.r == me.r) & (v.j < me.j)));
     }
+    if (g < nh) {
+      const NlHit u = hit[g];
+      rank0 += (u.t == me.t) & ((u.r < me.r) | ((u.r == me.r) & (u.j < me.j)));
+    }
+    const int rank = rank0 + rank1, t = me.t;
     if (rank < P.sel[t]) {
       const int slot = P.sec_start[t] + rank;
-      nl_row[slot] = j;
-      if (out_row) out_row[slot] = j;
+      nl_row[slot] = me.j;
+      if (out_row) out_row[slot] = me.j;
       const int pj = hp[h];
       const double xj[3] = {s_xyz[3 * (size_t)pj], s_xyz[3 * (size_t)pj + 1], s_xyz[3 * (size_t)pj + 2]};
       double d[3], rr;
@@ -248,7 +266,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
                          const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st) {
   if (C.n <= 0) return cudaSuccess;
-  const size_t smem = (size_t)cap * (sizeof(double) + 3 * sizeof(int));
+  const size_t smem = (size_t)cap * (sizeof(NlHit) + sizeof(int));
   static size_t configured = 0;
   if (smem > 48 * 1024 && smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_nlist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
