@@ -32,38 +32,6 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, const double a, 
       : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// tanh(x) = 1 - 2 / (exp(2x) + 1) with exp(2x) = 2^n 2^f: n = rint(2x log2 e) by the 1.5 * 2^52 trick, 2^f by a
-// degree-10 polynomial on [-0.5, 0.5] (relative error 2.9e-16), the reciprocal from MUFU.RCP64H refined by one cubic
-// step.  19 fp64-pipe instructions; absolute error <= 4.5e-16 against libdevice on [-25, 25], [-1, 1], [-0.01, 0.01]
-// and [-1e-6, 1e-6] (4e7 points each, profiles/r1_fp64_peaks.md); libdevice's tanh costs 2.2x the pipe slots.
-__device__ __forceinline__ double dp_tanh(double x) {
-  const int hi = __double2hiint(x);
-  const bool big = (hi & 0x7fffffff) >= 0x40340000;                 // |x| >= 20: tanh = +-1 in fp64
-  const double xc = big ? __hiloint2double((hi & 0x80000000) | 0x40340000, 0) : x;
-  const double t = xc * 2.8853900817779268;                          // 2 log2(e)
-  const double tm = t + 6755399441055744.0;                          // 1.5 * 2^52
-  const int ni = __double2loint(tm);
-  const double f = t - (tm - 6755399441055744.0);
-  double p = 7.0725859492692236999e-9;
-  p = fma(p, f, 1.0208690299958305835e-7);
-  p = fma(p, f, 1.3215442587921689653e-6);
-  p = fma(p, f, 0.000015252657260200837064);
-  p = fma(p, f, 0.00015403530441736050155);
-  p = fma(p, f, 0.0013333558230164973899);
-  p = fma(p, f, 0.0096181291076068885273);
-  p = fma(p, f, 0.055504108664447719166);
-  p = fma(p, f, 0.2402265069591009822);
-  p = fma(p, f, 0.69314718055994998286);
-  p = fma(p, f, 1.0);
-  const double d = __hiloint2double(__double2hiint(p) + ni * 1048576, __double2loint(p)) + 1.0;
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-  const double err = fma(-d, r, 1.0);
-  const double tq = fma(err, err, err);
-  r = fma(r, tq, r);
-  return fma(-2.0, r, 1.0);
-}
-
 template <int SP>
 struct EL {
   static constexpr int S0 = SP, S1 = 2 * SP, S2 = 4 * SP;

@@ -18,7 +18,11 @@
 
 #include <vector>
 
-#define FIT_BM 64
+#ifndef FIT_WM
+#define FIT_WM 2            // warp rows per CTA: CTA tile = 16 FIT_WM rows, 64 FIT_WM threads
+#endif
+#define FIT_BM (16 * FIT_WM)
+#define FIT_THREADS (64 * FIT_WM)
 #define FIT_BK 16
 #define FIT_STAGES 3
 #define FIT_LDA (FIT_BK + 4)
@@ -60,7 +64,7 @@ struct GemmArgs {
 };
 
 template <int NBW, int EPI>
-__global__ void __launch_bounds__(256, 1)
+__global__ void __launch_bounds__(FIT_THREADS, FIT_WM <= 2 ? 2 : 1)
 k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
   constexpr int BN = 16 * NBW, LDB = BN + 4;
   extern __shared__ __align__(16) double smem[];
@@ -78,12 +82,12 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
     double *as = As + stage * FIT_BM * FIT_LDA;
     double *bs = Bs + stage * FIT_BK * LDB;
     const int k0 = kt * FIT_BK;
-    for (int c = tid; c < FIT_BM * (FIT_BK / 2); c += 256) {
+    for (int c = tid; c < FIT_BM * (FIT_BK / 2); c += FIT_THREADS) {
       const int m = c >> 3, kk = (c & 7) * 2;
       const bool ok = m0 + m < row_hi;
       cp_async16(as + m * FIT_LDA + kk, g.A + (size_t)(ok ? m0 + m : m0) * g.lda + k0 + kk, ok);
     }
-    for (int c = tid; c < FIT_BK * (BN / 2); c += 256) {
+    for (int c = tid; c < FIT_BK * (BN / 2); c += FIT_THREADS) {
       const int k = c / (BN / 2), nn = (c - k * (BN / 2)) * 2;
       const bool ok = n0 + nn < g.N;
       cp_async16(bs + k * LDB + nn, g.B + (size_t)(k0 + k) * g.ldb + (ok ? n0 + nn : 0), ok);
@@ -137,11 +141,11 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
       const size_t oi = (size_t)m * g.ldi + n, oo = (size_t)m * g.ldo + n;
       if (EPI == EPI_TANH) {
         const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
-        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(tanh(v0 + b.x), tanh(v1 + b.y));
+        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(dp_tanh(v0 + b.x), dp_tanh(v1 + b.y));
       } else if (EPI == EPI_TANH_SKIP) {
         const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
         const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi);
-        const double u0 = tanh(v0 + b.x), u1 = tanh(v1 + b.y);
+        const double u0 = dp_tanh(v0 + b.x), u1 = dp_tanh(v1 + b.y);
         *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(u0, u1);
         *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(z.x + u0, z.y + u1);
       } else if (EPI == EPI_L3) {
@@ -149,7 +153,7 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
         const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
         const double2 w = *reinterpret_cast<const double2 *>(g.in1 + n);
         const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi);
-        const double u0 = tanh(v0 + b.x), u1 = tanh(v1 + b.y);
+        const double u0 = dp_tanh(v0 + b.x), u1 = dp_tanh(v1 + b.y);
         *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(z.x + u0, z.y + u1);
         *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(w.x * (1.0 - u0 * u0), w.y * (1.0 - u1 * u1));
       } else if (EPI == EPI_BWD) {
@@ -305,7 +309,7 @@ static cudaError_t gemm(const ChunkView &C, int ty, const GemmArgs &g, cudaStrea
     configured = true;
   }
   dim3 grid((C.n + FIT_BM - 1) / FIT_BM, (g.N + BN - 1) / BN);
-  k_fit_gemm<NBW, EPI><<<grid, 256, smem, st>>>(C, ty, g);
+  k_fit_gemm<NBW, EPI><<<grid, FIT_THREADS, smem, st>>>(C, ty, g);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
