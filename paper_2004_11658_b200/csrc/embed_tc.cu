@@ -21,7 +21,9 @@ struct TL {
   static constexpr int KS1 = (S1 + 7) / 8, KS2 = (2 * S1 + 7) / 8, PAN2 = (KS2 + 3) / 4;
   static constexpr int W1B = N1 * 128, W2P = N2 * 128, W2B = PAN2 * W2P;       // bytes of one hi (or lo) image
   static constexpr int oW1h = 0, oW1l = W1B, oW2h = 2 * W1B, oW2l = 2 * W1B + W2B, oVec = 2 * W1B + 2 * W2B;
-  static constexpr int vW0 = 0, vb0 = 32, vb1 = 64, vb2 = 64 + N1, nvec = 64 + N1 + N2;          // floats
+  static constexpr int vW0 = 0, vb0 = 32, vb1 = 64, vb2 = 64 + N1, nv1 = 64 + N1 + N2;           // floats
+  // the same vectors scaled by 2 log2(e) (pass 1 feeds them straight into ex2)
+  static constexpr int sW0 = nv1, sb0 = nv1 + 32, sb1 = nv1 + 64, sb2 = nv1 + 64 + N1, nvec = 2 * nv1;
   static constexpr int img_bytes = (oVec + 4 * nvec + 1023) / 1024 * 1024;
   static constexpr int SLOT = 65536;                       // per-warpgroup operand slot
   static constexpr int oSlot = img_bytes, oEnv = oSlot + 2 * SLOT, oIds = oEnv + 2 * 128 * 32,
@@ -62,6 +64,10 @@ static void pack_net_tc(const double *net, std::vector<float> &out) {
   for (int s = 0; s < S1; ++s) { vec[L::vW0 + s] = (float)W0[s]; vec[L::vb0 + s] = (float)b0[s]; }
   for (int o = 0; o < 2 * S1; ++o) vec[L::vb1 + o] = (float)b1[o];
   for (int o = 0; o < 4 * S1; ++o) vec[L::vb2 + o] = (float)b2[o];
+  const double c2 = 2.8853900817779268;
+  for (int s = 0; s < S1; ++s) { vec[L::sW0 + s] = (float)(c2 * W0[s]); vec[L::sb0 + s] = (float)(c2 * b0[s]); }
+  for (int o = 0; o < 2 * S1; ++o) vec[L::sb1 + o] = (float)(c2 * b1[o]);
+  for (int o = 0; o < 4 * S1; ++o) vec[L::sb2 + o] = (float)(c2 * b2[o]);
 }
 
 static bool tc_supported_s1(int s1) { return s1 == 8 || s1 == 16 || s1 == 25 || s1 == 32; }
@@ -251,12 +257,15 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
       const int tile0 = flat0 + tile * 128, seg_lo = off_t[qa] - tile0, seg_hi = off_t[qa + 1] - tile0;
       segs[wt] = min(nrows, seg_hi) | ((seg_lo >= 0 && seg_hi <= 128) ? 256 : 0);
     }
-    envt[wt] = make_float4((float)e[0], (float)e[1], (float)e[2], (float)e[3]);
+    {
+      float *ef = reinterpret_cast<float *>(envt);            // transposed: [component][row]
+      ef[wt] = (float)e[0]; ef[128 + wt] = (float)e[1]; ef[256 + wt] = (float)e[2]; ef[384 + wt] = (float)e[3];
+    }
     const float x = (float)e[0];
     // layer 0 (Eq. 8): h0 = tanh(x W0 + b0)
     float h0[32];
 #pragma unroll
-    for (int s = 0; s < 32; ++s) h0[s] = s < S1 ? tc::tanh_f32(fmaf(x, vec[L::vW0 + s], vec[L::vb0 + s])) : 0.0f;
+    for (int s = 0; s < 32; ++s) h0[s] = s < S1 ? tc::tanh_prescaled_f32(fmaf(x, vec[L::sW0 + s], vec[L::sb0 + s])) : 0.0f;
 #pragma unroll
     for (int j = 0; j < 2 * L::KS1; ++j)
       store_split4(slot, slot + 16384, rowbase, r7, j, h0[4 * j], h0[4 * j + 1], h0[4 * j + 2], h0[4 * j + 3]);
@@ -285,7 +294,7 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
       tc::tmem_ld_cols_nowait<L::N1>(tD1 + lane_sel, v);
       tc::tmem_wait_ld();
 #pragma unroll
-      for (int o = 0; o < 2 * S1; ++o) h1[o] = h0[o % S1] + tc::tanh_f32(__uint_as_float(v[o]) + vec[L::vb1 + o]);
+      for (int o = 0; o < 2 * S1; ++o) h1[o] = h0[o % S1] + tc::tanh_prescaled_f32(fmaf(__uint_as_float(v[o]), TC_2LOG2E, vec[L::sb1 + o]));
     }
     TCP(4);
 #pragma unroll
@@ -313,33 +322,30 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
     phase ^= 1;
     tc::fence_after_sync();
     TCP(6);
-    // layer 2 (Eq. 9): g = (h1, h1) + tanh(h1 W2 + b2), written to the slot as a [128][128] fp32 tile whose 16-byte
-    // chunks are XOR-swizzled with the row (conflict-free row-wise stores and column-wise loads)
+    // layer 2 (Eq. 9): g = (h1, h1) + tanh(h1 W2 + b2), written to the slot TRANSPOSED: gT[feature][row], 128 floats per
+    // feature, the 16-byte chunk (4 rows) XOR-swizzled with the feature (conflict-free 4-byte stores by row threads and
+    // 16-byte loads by feature threads)
     float *gt = reinterpret_cast<float *>(slot);
     {
       constexpr int CH = 32, NCH = (L::N2 + CH - 1) / CH;
       uint32_t va[CH], vb[CH];
       tc::tmem_ld_cols_nowait<(L::N2 < CH ? L::N2 : CH)>(tD2 + lane_sel, va);
       tc::tmem_wait_ld();
+      float *gdst = gt + (wt & 3);
+      const int rch = wt >> 2;
 #pragma unroll
       for (int c = 0; c < NCH; ++c) {
         uint32_t *cur = (c & 1) ? vb : va, *nxt = (c & 1) ? va : vb;
-        constexpr int dummy = 0;
-        (void)dummy;
         if (c + 1 < NCH) {
           if (L::N2 - (c + 1) * CH >= CH) tc::tmem_ld_cols_nowait<CH>(tD2 + lane_sel + (c + 1) * CH, nxt);
           else tc::tmem_ld_cols_nowait<(L::N2 % CH == 0 ? CH : L::N2 % CH)>(tD2 + lane_sel + (c + 1) * CH, nxt);
         }
 #pragma unroll
-        for (int j = 0; j < CH / 4; ++j) {
-          const int o = c * CH + 4 * j;
-          if (o < L::N2) {
-            float gv[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-              gv[i] = o + i < 4 * S1 ? h1[(o + i) % (2 * S1)] + tc::tanh_f32(__uint_as_float(cur[4 * j + i]) + vec[L::vb2 + o + i]) : 0.0f;
-            *reinterpret_cast<float4 *>(gt + wt * 128 + (((o >> 2) ^ r7) << 2)) = make_float4(gv[0], gv[1], gv[2], gv[3]);
-          }
+        for (int j = 0; j < CH; ++j) {
+          const int o = c * CH + j;
+          if (o < 4 * S1)
+            gdst[o * 128 + ((rch ^ (o & 7)) << 2)] =
+                h1[o % (2 * S1)] + tc::tanh_prescaled_f32(fmaf(__uint_as_float(cur[j]), TC_2LOG2E, vec[L::sb2 + o]));
         }
         if (c + 1 < NCH) tc::tmem_wait_ld();
       }
@@ -355,41 +361,45 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
       if (nx_valid) { nx_idx = pidx_t[pn]; nx_dv = C.dr[nx_idx]; }
     }
     // S5: T_i += sum_rows g (x) R~.  Thread b owns feature b; rows are grouped by centre atom (segments, from the pair
-    // offsets).  Aligned blocks of 8 rows: products and the 8-row partial sum in fp32, accumulation across blocks in
-    // fp64; blocks cut by a segment boundary are masked.
+    // offsets).  Four rows per step: one 16-byte load of gT, four broadcast loads of the transposed R~ tile, eight
+    // packed FMAs (FFMA2); products and partial sums of up to 8 rows in fp32, accumulation across them in fp64
+    // (DESIGN.md "Mixed precision"); steps cut by a segment boundary take the masked path.
     if (wt < 4 * S1) {
       const int b = wt;
-      const float *gp = gt + (b & 3);
-      int col[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) col[i] = i * 128 + ((((b >> 2) ^ i)) << 2);
+      const float4 *grow = reinterpret_cast<const float4 *>(gt + b * 128);
+      const float4 *et = reinterpret_cast<const float4 *>(envt);       // [4][32]: component c, rows 4 k .. 4 k + 3
+      const int sw = b & 7;
       int row = 0;
       while (row < nrows) {
         const int cur = ids[row];
         const int se = segs[row];                           // end row of this atom's segment; bit 8: whole section in the tile
         const int hi = se & 255;
         double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        for (int r0 = row & ~7; r0 < hi; r0 += 8) {
-          const float *gb = gp + r0 * 128;
-          const float4 *eb = envt + r0;
-          float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-          if (r0 >= row && r0 + 8 <= hi) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const float gv = gb[col[i]];
-              const float4 ev = eb[i];
-              s0 = fmaf(gv, ev.x, s0); s1 = fmaf(gv, ev.y, s1); s2 = fmaf(gv, ev.z, s2); s3 = fmaf(gv, ev.w, s3);
-            }
-          } else {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const float gv = (r0 + i >= row && r0 + i < hi) ? gb[col[i]] : 0.f;
-              const float4 ev = eb[i];
-              s0 = fmaf(gv, ev.x, s0); s1 = fmaf(gv, ev.y, s1); s2 = fmaf(gv, ev.z, s2); s3 = fmaf(gv, ev.w, s3);
-            }
+        float2 s01 = make_float2(0.f, 0.f), s23 = s01;
+        for (int k = row >> 2; 4 * k < hi; ++k) {
+          float4 g4 = grow[k ^ sw];
+          const int r0 = 4 * k;
+          if (r0 < row || r0 + 4 > hi) {                    // uniform over the warp: boundary step
+            if (r0 < row || r0 >= hi) g4.x = 0.f;
+            if (r0 + 1 < row || r0 + 1 >= hi) g4.y = 0.f;
+            if (r0 + 2 < row || r0 + 2 >= hi) g4.z = 0.f;
+            if (r0 + 3 < row || r0 + 3 >= hi) g4.w = 0.f;
           }
-          a0 += (double)s0; a1 += (double)s1; a2 += (double)s2; a3 += (double)s3;
+          const float4 e0 = et[k], e1 = et[32 + k], e2 = et[64 + k], e3 = et[96 + k];
+          s01 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e0.x, e1.x), s01);
+          s23 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e2.x, e3.x), s23);
+          s01 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e0.y, e1.y), s01);
+          s23 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e2.y, e3.y), s23);
+          s01 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e0.z, e1.z), s01);
+          s23 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e2.z, e3.z), s23);
+          s01 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e0.w, e1.w), s01);
+          s23 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e2.w, e3.w), s23);
+          if (k & 1) {
+            a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
+            s01 = make_float2(0.f, 0.f); s23 = s01;
+          }
         }
+        a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
         double *dst = C.T + ((size_t)cur * P.M + b) * 4;
         if (t == 0 && (se & 256)) {
           // first section and the whole section of this atom lies inside the tile: nobody else writes T[cur][b][:] yet

@@ -210,6 +210,28 @@ __device__ __forceinline__ float tanh_f32(float x) {
   return copysignf((1.0f - u) * r, x);
 }
 
+// tanh of an argument that is already scaled by 2 log2(e): 1 - 2 / (2^a + 1).  ex2, add, rcp, fma.
+__device__ __forceinline__ float tanh_prescaled_f32(float a) {
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(a));
+  const float d = e + 1.0f;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(d));
+  return fmaf(-2.0f, r, 1.0f);
+}
+#define TC_2LOG2E 2.885390081777927f
+
+// packed fp32 FMA (FFMA2): (d.x, d.y) = (a.x b.x + c.x, a.y b.y + c.y)
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+  unsigned long long ua, ub, uc, ud;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
+  float2 d;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
+  return d;
+}
+
 }  // namespace tc
 
 // host-side TF32 rounding (round to nearest, ties away from zero: what cvt.rna.tf32.f32 does)
