@@ -5,8 +5,8 @@ random network weights (recipes: DESIGN.md "Input recipe"; BASELINE.json `config
 the CUDA path receive the very same numpy arrays, so no cross-language RNG matching is needed.
 """
 from .systems import (CONFIGS, SEED_BASE, SystemSpec, make_system, perturbed, water_box, copper_box,
-                      replicate)
+                      replicate, MASSES, AMU_A2_FS2_IN_EV, KB_EV, maxwell_boltzmann)
 from .weights import ModelSpec, make_weights, emb_net_size, fit_net_size, condition_fit_w0
 
 __all__ = ["CONFIGS", "SEED_BASE", "SystemSpec", "make_system", "perturbed", "water_box", "copper_box",
-           "replicate", "ModelSpec", "make_weights", "emb_net_size", "fit_net_size", "condition_fit_w0"]
+           "replicate", "MASSES", "AMU_A2_FS2_IN_EV", "KB_EV", "maxwell_boltzmann", "ModelSpec", "make_weights", "emb_net_size", "fit_net_size", "condition_fit_w0"]

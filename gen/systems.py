@@ -117,3 +117,25 @@ def replicate(coord: np.ndarray, types: np.ndarray, box: np.ndarray, reps: int):
     shifts = np.stack(np.meshgrid(np.arange(reps), np.arange(reps), np.arange(reps), indexing="ij"), -1).reshape(-1, 3)
     big = (coord[None, :, :] + shifts[:, None, :] * L).reshape(-1, 3)
     return np.ascontiguousarray(big), np.tile(types, shifts.shape[0]).astype(np.int32), np.diag(L * reps).reshape(9)
+
+
+# ---- molecular dynamics inputs (330 K) ------------------------------------
+MASSES = {"W192": (15.999, 1.008), "W24k": (15.999, 1.008), "Cu32k": (63.546,), "Cu864k": (63.546,)}   # amu
+
+# CODATA 2018: atomic mass constant, elementary charge, Boltzmann constant
+_AMU_KG, _E_C, _KB_J = 1.66053906660e-27, 1.602176634e-19, 1.380649e-23
+AMU_A2_FS2_IN_EV = _AMU_KG * 1e10 / _E_C            # 1 amu A^2 / fs^2 in eV (103.6427)
+KB_EV = _KB_J / _E_C                                # eV / K
+
+
+def maxwell_boltzmann(types: np.ndarray, masses, temperature: float, seed: int) -> np.ndarray:
+    """Velocities [N][3] in A/fs drawn from the Maxwell-Boltzmann distribution at `temperature` (K), with the total
+    momentum removed and then rescaled so that 2 E_kin / (3 N k_B) equals `temperature` exactly."""
+    rng = np.random.default_rng(seed)
+    m = np.asarray(masses, dtype=np.float64)[np.asarray(types)]
+    sigma = np.sqrt(KB_EV * temperature / (m * AMU_A2_FS2_IN_EV))
+    v = rng.standard_normal((len(m), 3)) * sigma[:, None]
+    v -= (m[:, None] * v).sum(0) / m.sum()
+    ek = 0.5 * (m[:, None] * v * v).sum() * AMU_A2_FS2_IN_EV
+    v *= np.sqrt(1.5 * len(m) * KB_EV * temperature / ek)
+    return np.ascontiguousarray(v)
