@@ -127,6 +127,38 @@ int dpb_set_debug_buffers(dpb_model *model, double *T, double *D, double *dT);
 int dpb_model_set_timing(dpb_model *model, int on);
 int dpb_model_stage_us(const dpb_model *model, float stage_us[8]);
 
+/* ---- molecular dynamics with the DP forces ---------------------------------
+ * Velocity-Verlet, NVE: v += (dt/2) F/m; x += dt v; F = F(x); v += (dt/2) F/m.  Units: Angstrom, fs, amu, eV
+ * (1 amu A^2/fs^2 = 103.6426965268 eV; T = 2 E_kin / (3 N k_B), k_B = 8.617333262e-5 eV/K).
+ * Neighbour reuse (2 A skin, rebuilt every 50 steps): with rebuild_every > 1 the cell search runs
+ * over r_c + skin every rebuild_every steps and stores a raw list; the steps in between format that raw list (Alg. 1).
+ * The formatted list equals a fresh search as long as no atom moves more than skin / 2 between rebuilds
+ * (reported in dpb_md_info, not enforced).  rebuild_every == 1: fresh cell search every step, skin unused. */
+typedef struct {
+  double dt_fs;              /* time step                                                                  */
+  int32_t nsteps;            /* number of steps (>= 0)                                                     */
+  int32_t thermo_every;      /* thermo rows at steps 0, thermo_every, 2 thermo_every, ... (>= 1)           */
+  int32_t rebuild_every;     /* >= 1                                                                       */
+  int32_t reserved;
+  double skin;               /* Angstrom; needs r_c + skin < min(L) / 2 when rebuild_every > 1             */
+} dpb_md_params;
+
+typedef struct {
+  int32_t n_thermo;          /* rows written to thermo                                                     */
+  int32_t n_rebuilds;        /* neighbour searches from the cell list                                      */
+  int32_t skin_violated;     /* 1 if some atom moved more than skin / 2 between two rebuilds               */
+  int32_t reserved;
+  double max_displacement;   /* largest displacement of an atom since the rebuild before it (Angstrom)     */
+} dpb_md_info;
+
+/* coord DEVICE fp64 [N][3] and vel DEVICE fp64 [N][3] (A/fs) are updated in place; type DEVICE int32 [N]; mass HOST
+ * [ntypes] (amu); box HOST [9]; thermo HOST [nsteps / thermo_every + 1][3] = (E_pot, E_kin, T) or NULL; info HOST or
+ * NULL.  All work is enqueued on `stream`; the call returns after the stream has been synchronised.  The model must
+ * not be used by another call while the run is in flight.  Errors as dpb_eval. */
+int dpb_md_run(dpb_model *model, void *stream, int64_t natoms, double *coord, double *vel, const int32_t *type,
+               const double *mass, const double box[9], const dpb_md_params *params, double *thermo,
+               dpb_md_info *info);
+
 /* Thread-local description of the last error returned on this thread; valid until the next call. */
 const char *dpb_last_error(void);
 

@@ -27,6 +27,16 @@ class _Desc(C.Structure):
                 ("fit_weights", C.POINTER(C.c_double))]
 
 
+class _MDParams(C.Structure):
+    _fields_ = [("dt_fs", C.c_double), ("nsteps", C.c_int32), ("thermo_every", C.c_int32),
+                ("rebuild_every", C.c_int32), ("reserved", C.c_int32), ("skin", C.c_double)]
+
+
+class _MDInfo(C.Structure):
+    _fields_ = [("n_thermo", C.c_int32), ("n_rebuilds", C.c_int32), ("skin_violated", C.c_int32),
+                ("reserved", C.c_int32), ("max_displacement", C.c_double)]
+
+
 class _Info(C.Structure):
     _fields_ = [("n_real_pairs", C.c_int64), ("n_overflow", C.c_int64), ("max_nei", C.c_int32 * 8),
                 ("n_chunks", C.c_int32), ("reserved", C.c_int32)]
@@ -70,6 +80,8 @@ def load_library():
     lib.dpb_eval.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp, C.POINTER(_Info)]
     lib.dpb_eval_host.argtypes = lib.dpb_eval.argtypes
     lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
+    lib.dpb_md_run.argtypes = [vp, vp, i64, vp, vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                               C.POINTER(_MDParams), vp, C.POINTER(_MDInfo)]
     lib.dpb_kernel_launches.restype = C.c_int64
     lib.dpb_last_error.restype = C.c_char_p
     lib.dpb_version.restype = C.c_char_p
@@ -221,3 +233,23 @@ class DPModel:
                                       C.c_void_p(types.data_ptr()), bp, C.c_void_p(nlist.data_ptr()), C.byref(ovf))
         self._chk(rc)
         return nlist, int(ovf.value)
+
+    def md_run(self, coord, vel, types, mass, box, dt_fs, nsteps, thermo_every=1, rebuild_every=1, skin=0.0):
+        """dpb_md_run: velocity-Verlet NVE on torch CUDA tensors coord / vel (float64 [N,3], updated IN PLACE).
+        Returns (thermo numpy [k][3] = (E_pot, E_kin, T), info dict)."""
+        torch = _torch()
+        assert coord.is_cuda and coord.dtype == torch.float64 and coord.is_contiguous()
+        assert vel.is_cuda and vel.dtype == torch.float64 and vel.is_contiguous()
+        assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
+        n = int(coord.shape[0])
+        b, bp = self._box(box)
+        m = np.ascontiguousarray(mass, dtype=np.float64)
+        prm = _MDParams(float(dt_fs), int(nsteps), int(thermo_every), int(rebuild_every), 0, float(skin))
+        thermo = np.zeros((nsteps // thermo_every + 1, 3))
+        info = _MDInfo()
+        rc = self.lib.dpb_md_run(self._h, self._stream(), n, C.c_void_p(coord.data_ptr()), C.c_void_p(vel.data_ptr()),
+                                 C.c_void_p(types.data_ptr()), m.ctypes.data_as(C.POINTER(C.c_double)), bp,
+                                 C.byref(prm), C.c_void_p(thermo.ctypes.data), C.byref(info))
+        self._chk(rc)
+        return thermo, dict(n_thermo=info.n_thermo, n_rebuilds=info.n_rebuilds, skin_violated=bool(info.skin_violated),
+                            max_displacement=info.max_displacement)

@@ -62,6 +62,11 @@ struct dpb_model {
   Buf dT32;                     // mixed precision: fp32 copy of dE/dT of the chunk
   Buf pairs;                    // mixed precision: flattened real-slot lists of the chunk
   Buf h_coord, h_type, h_out;   // device staging of dpb_eval_host
+  // molecular dynamics driver (dpb_md_run): skin list of the last rebuild, forces, thermo output
+  Buf md_raw, md_nraw, md_xyz0, md_force, md_scal, md_mass;
+  int md_cap_raw = 0;
+  double md_skin = 0.0;
+  DevGrid md_grid;
   double *dbgT = nullptr, *dbgD = nullptr, *dbgdT = nullptr;
   std::vector<cudaEvent_t> evs;   // stage timers: [0] start, [1] after S1, then 4 per chunk, then the end
   int ev_chunks = 0;              // chunks of the last timed evaluation
@@ -131,7 +136,8 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out};
+                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
+                &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
@@ -186,17 +192,18 @@ extern "C" int dpb_model_stage_us(const dpb_model *m, float us[8]) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-static int make_grid(const DevModel &P, const double box[9], DevGrid &G) {
+static int make_grid(const DevModel &P, const double box[9], DevGrid &G, double rsearch) {
   if (box[1] != 0.0 || box[2] != 0.0 || box[3] != 0.0 || box[5] != 0.0 || box[6] != 0.0 || box[7] != 0.0)
     return fail(DPB_EBOX, "box must be orthorhombic (off-diagonal entries are not zero)");
   G.L[0] = box[0]; G.L[1] = box[4]; G.L[2] = box[8];
   long long ncell = 1;
   for (int c = 0; c < 3; ++c) {
-    if (!(G.L[c] > 0.0) || !(P.rc < 0.5 * G.L[c]))
-      return fail(DPB_EBOX, "need rcut < L/2 in every dimension (L[%d] = %g, rcut = %g)", c, G.L[c], P.rc);
+    if (!(G.L[c] > 0.0) || !(rsearch < 0.5 * G.L[c]))
+      return fail(DPB_EBOX, "need rcut (+ skin) < L/2 in every dimension (L[%d] = %g, search radius = %g)", c, G.L[c],
+                  rsearch);
     // cell edge >= rc (1 + 1e-6): the +-1 stencil then covers every r <= rc even when rounding moves an atom that
     // sits on a cell face into the neighbouring cell
-    double f = floor(G.L[c] / (P.rc * (1.0 + 1e-6)));
+    double f = floor(G.L[c] / (rsearch * (1.0 + 1e-6)));
     int n = f < 1.0 ? 1 : (f > 512.0 ? 512 : (int)f);
     G.nc[c] = n;
     ncell *= n;
@@ -226,15 +233,19 @@ static int neighbour_cap(const DevModel &P) {
   return cap;
 }
 
+// nl_mode 0: neighbour search from the cell list (every dpb_eval); 1 / 2: MD rebuild / reuse step (md.cu).
 static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double *coord, const int32_t *type,
                     const double box[9], double *energy, double *atom_energy, double *force, double *virial,
-                    int32_t *nlist, bool nlist_only) {
+                    int32_t *nlist, bool nlist_only, int nl_mode = 0) {
   const DevModel &P = m->P;
   if (natoms < 0 || natoms > 2000000000ll) return fail(DPB_EINVAL, "natoms out of range");
   if (natoms > 0 && (!coord || !type)) return fail(DPB_EINVAL, "null coord / type");
   DevGrid G;
-  int rc = make_grid(P, box, G);
+  int rc = DPB_OK;
+  if (nl_mode == 2) G = m->md_grid;
+  else rc = make_grid(P, box, G, nl_mode == 1 ? P.rc + m->md_skin : P.rc);
   if (rc != DPB_OK) return rc;
+  if (nl_mode == 1) m->md_grid = G;
   const int N = (int)natoms;
   const int nkeys = P.ntypes * G.ncell;
   const int64_t chunk = m->chunk < natoms ? m->chunk : (natoms > 0 ? natoms : 1);
@@ -266,7 +277,13 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     }
   }
   DevStats *stats = m->stats.as<DevStats>();
-  CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");
+  if (nl_mode == 0) CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");   // MD: kept over the run
+  NlRaw raw{};
+  if (nl_mode != 0) {
+    raw.raw = m->md_raw.as<int>(); raw.nraw = m->md_nraw.as<int>(); raw.cap = m->md_cap_raw;
+    const double rs = P.rc + m->md_skin;
+    raw.rs2_hi = rs * rs * (1.0 + 1e-9);
+  }
   const bool timing = m->timing && !nlist_only;
   const int nchunks = (int)((natoms + chunk - 1) / chunk);
   if (timing) {
@@ -281,8 +298,16 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   }
 
   int *start = m->start.as<int>();
-  CU(launch_cell_sort(P, G, natoms, coord, type, m->key.as<int>(), m->count.as<int>(), start, m->cursor.as<int>(),
-                      m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st), "cell sort");
+  if (nl_mode == 2) {
+    CU(launch_gather_sorted(natoms, coord, m->s_idx.as<int>(), m->s_xyz.as<double>(), m->md_xyz0.as<double>(), stats,
+                            st), "gather");
+  } else {
+    CU(launch_cell_sort(P, G, natoms, coord, type, m->key.as<int>(), m->count.as<int>(), start, m->cursor.as<int>(),
+                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st), "cell sort");
+    if (nl_mode == 1 && natoms > 0)
+      CU(cudaMemcpyAsync(m->md_xyz0.p, m->s_xyz.p, sizeof(double) * 3 * (size_t)natoms, cudaMemcpyDeviceToDevice, st),
+         "copy of the rebuild coordinates");
+  }
   if (timing) cudaEventRecord(m->evs[1], st);
 
   double *ei = atom_energy ? atom_energy : m->ei.as<double>();
@@ -303,7 +328,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.nreal = m->nreal.as<int>();
     C.T = m->T.as<double>();
     C.dT = m->dT.as<double>();
-    CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st), "nlist");
+    CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st, nl_mode, nl_mode ? &raw : nullptr),
+       "nlist");
     if (nlist_only) continue;
     if (timing) cudaEventRecord(m->evs[2 + 4 * ci], st);
     if (m->precision == DPB_TF32) {
@@ -422,5 +448,80 @@ extern "C" int dpb_eval_host(dpb_model *m, void *stream, int64_t natoms, const d
     CU(cudaMemcpyAsync(nlist_h, d_nl, nl_bytes, cudaMemcpyDeviceToHost, st), "D2H nlist");
   if (info) return finish_info(m, st, natoms, info);
   CU(cudaStreamSynchronize(st), "stream synchronise");
+  return DPB_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// molecular dynamics.  Velocity-Verlet NVE; one force evaluation per step
+// through run_eval; with rebuild_every > 1 the neighbour search runs on a skin list (cells and raw list over
+// r_c + skin, rebuilt every rebuild_every steps; in between, Alg. 1 formats the raw list).  Everything is enqueued on
+// the stream without host synchronisation until the thermo output is copied back at the end.
+extern "C" int dpb_md_run(dpb_model *m, void *stream, int64_t natoms, double *coord, double *vel, const int32_t *type,
+                          const double *mass_h, const double box[9], const dpb_md_params *prm, double *thermo_h,
+                          dpb_md_info *info) {
+  if (!m || !box || !prm || !mass_h) return fail(DPB_EINVAL, "dpb_md_run: null argument");
+  if (natoms < 0 || (natoms > 0 && (!coord || !vel || !type))) return fail(DPB_EINVAL, "dpb_md_run: null coord / vel / type");
+  if (!(prm->dt_fs > 0.0) || prm->nsteps < 0 || prm->thermo_every < 1 || prm->rebuild_every < 1 || !(prm->skin >= 0.0))
+    return fail(DPB_EINVAL, "dpb_md_run: need dt > 0, nsteps >= 0, thermo_every >= 1, rebuild_every >= 1, skin >= 0");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const DevModel &P = m->P;
+  const bool reuse = prm->rebuild_every > 1;
+  const size_t n = (size_t)natoms;
+  const int nth = prm->nsteps / prm->thermo_every + 1;
+  const double AMU = 103.6426965268;
+  std::vector<double> hm(2 * DPB_MAX_TYPES, 0.0);              // [0..8): (dt/2)/(m AMU); [8..16): m AMU
+  for (int t = 0; t < P.ntypes; ++t) {
+    if (!(mass_h[t] > 0.0)) return fail(DPB_EINVAL, "dpb_md_run: mass[%d] must be positive", t);
+    hm[t] = 0.5 * prm->dt_fs / (mass_h[t] * AMU);
+    hm[DPB_MAX_TYPES + t] = mass_h[t] * AMU;
+  }
+  CU(m->md_force.reserve(sizeof(double) * 3 * (n + 1)), "md workspace");
+  CU(m->md_scal.reserve(sizeof(double) * (2 + 3 * (size_t)nth)), "md workspace");
+  CU(m->md_mass.reserve(sizeof(double) * 2 * DPB_MAX_TYPES), "md workspace");
+  CU(cudaMemcpyAsync(m->md_mass.p, hm.data(), sizeof(double) * 2 * DPB_MAX_TYPES, cudaMemcpyHostToDevice, st), "H2D masses");
+  if (reuse) {
+    const double f = (P.rc + prm->skin) / P.rc;
+    long long cap = (long long)(1.3 * f * f * f * P.nm) + 32;
+    if (cap > 8192) cap = 8192;
+    m->md_cap_raw = (int)cap;
+    m->md_skin = prm->skin;
+    CU(m->md_raw.reserve(sizeof(int) * (n + 1) * (size_t)cap), "md skin list");
+    CU(m->md_nraw.reserve(sizeof(int) * (n + 1)), "md skin list");
+    CU(m->md_xyz0.reserve(sizeof(double) * 3 * (n + 1)), "md skin list");
+  }
+  double *force = m->md_force.as<double>(), *epot = m->md_scal.as<double>(), *thermo = epot + 2;
+  const double *d_hm = m->md_mass.as<double>(), *d_mev = d_hm + DPB_MAX_TYPES;
+  CU(cudaMemsetAsync(m->stats.p, 0, sizeof(DevStats), st), "memset stats");
+  int rebuilds = 0;
+  auto eval = [&](int step) -> int {
+    int mode = 0;
+    if (reuse) { mode = (step % prm->rebuild_every == 0) ? 1 : 2; rebuilds += mode == 1; }
+    else CU(cudaMemsetAsync(m->stats.p, 0, sizeof(DevStats), st), "memset stats");
+    return run_eval(m, st, natoms, coord, type, box, epot, nullptr, force, nullptr, nullptr, false, mode);
+  };
+  int rc = eval(0);
+  if (rc != DPB_OK) return rc;
+  int slot = 0;
+  for (int step = 0;; ++step) {
+    if (step % prm->thermo_every == 0) CU(launch_md_thermo(natoms, vel, type, d_mev, epot, thermo, slot++, st), "thermo");
+    if (step == prm->nsteps) break;
+    CU(launch_md_kick_drift(natoms, coord, vel, force, type, d_hm, prm->dt_fs, st), "kick + drift");
+    rc = eval(step + 1);
+    if (rc != DPB_OK) return rc;
+    CU(launch_md_kick(natoms, vel, force, type, d_hm, st), "kick");
+  }
+  if (thermo_h) CU(cudaMemcpyAsync(thermo_h, thermo, sizeof(double) * 3 * (size_t)nth, cudaMemcpyDeviceToHost, st), "D2H thermo");
+  DevStats hs;
+  CU(cudaMemcpyAsync(&hs, m->stats.p, sizeof(DevStats), cudaMemcpyDeviceToHost, st), "stats copy");
+  CU(cudaStreamSynchronize(st), "stream synchronise");
+  if (hs.err_type) return fail(DPB_EINVAL, "an atom has a type index outside [0, ntypes)");
+  if (hs.err_cap) return fail(DPB_ECAP, "an atom has more candidates than the staging / skin-list capacity");
+  if (info) {
+    memset(info, 0, sizeof(*info));
+    info->n_thermo = nth;
+    info->n_rebuilds = reuse ? rebuilds : prm->nsteps + 1;
+    info->max_displacement = sqrt(hs.max_disp2);
+    info->skin_violated = reuse && info->max_displacement > 0.5 * prm->skin;
+  }
   return DPB_OK;
 }

@@ -32,6 +32,15 @@ struct DevStats {
   int max_nei[DPB_MAX_TYPES];
   int err_type;      // an atom had a type index outside [0, ntypes)
   int err_cap;       // an atom had more in-range candidates than the staging capacity
+  double max_disp2;  // MD: largest squared displacement of an atom since the last neighbour rebuild (bits ordered as u64)
+};
+
+// Raw (skin) neighbour list of the MD driver: sorted positions of the atoms within r_c + skin at the last rebuild.
+struct NlRaw {
+  int *raw;          // [N][cap]
+  int *nraw;         // [N]
+  int cap;
+  double rs2_hi;     // (r_c + skin)^2 (1 + 1e-9)
 };
 
 // Per-chunk views (chunk = sorted positions [p0, p0 + n)).
@@ -55,7 +64,10 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
                              DevStats *stats, cudaStream_t st);
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
-                         const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st);
+                         const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode = 0,
+                         const NlRaw *raw = nullptr);
+cudaError_t launch_gather_sorted(int64_t natoms, const double *coord, const int *s_idx, double *s_xyz,
+                                 const double *xyz0, DevStats *stats, cudaStream_t st);
 
 // variant 0 ("v0"): plain unfused kernels
 struct V0Scratch {
@@ -71,6 +83,14 @@ cudaError_t launch_pass2_v0(const DevModel &P, const ChunkView &C, const double 
 
 cudaError_t launch_scatter_debug(const DevModel &P, const ChunkView &C, double *dbgT, double *dbgdT, cudaStream_t st);
 cudaError_t launch_reduce_energy(int64_t natoms, const double *atom_energy, double *energy, cudaStream_t st);
+
+// molecular-dynamics driver (md.cu)
+cudaError_t launch_md_kick_drift(int64_t n, double *coord, double *vel, const double *force, const int *type,
+                                 const double *hm, double dt, cudaStream_t st);
+cudaError_t launch_md_kick(int64_t n, double *vel, const double *force, const int *type, const double *hm,
+                           cudaStream_t st);
+cudaError_t launch_md_thermo(int64_t n, const double *vel, const int *type, const double *mass_ev, const double *epot,
+                             double *thermo, int slot, cudaStream_t st);
 
 // ---- device helpers ---------------------------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -1,0 +1,69 @@
+// md.cu — kernels of the molecular-dynamics driver dpb_md_run (velocity-Verlet,
+// NVE).  Units: Angstrom, fs, amu, eV; 1 amu A^2/fs^2 = 103.6426965268 eV (CODATA 2018), k_B = 8.617333262e-5 eV/K.
+#include "common.cuh"
+
+// v <- v + (dt/2) F/m;  x <- x + dt v     (hm[t] = (dt/2) / (m_t 103.64...))
+__global__ void k_md_kick_drift(int n, double *__restrict__ coord, double *__restrict__ vel,
+                                const double *__restrict__ force, const int *__restrict__ type,
+                                const double *__restrict__ hm, double dt) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= 3 * n) return;
+  const double v = fma(hm[type[k / 3]], force[k], vel[k]);
+  vel[k] = v;
+  coord[k] = fma(dt, v, coord[k]);
+}
+
+// v <- v + (dt/2) F/m
+__global__ void k_md_kick(int n, double *__restrict__ vel, const double *__restrict__ force,
+                          const int *__restrict__ type, const double *__restrict__ hm) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= 3 * n) return;
+  vel[k] = fma(hm[type[k / 3]], force[k], vel[k]);
+}
+
+// thermo[slot] = (E_pot, E_kin, T): fixed-order reduction by one block
+__global__ void k_md_thermo(int n, const double *__restrict__ vel, const int *__restrict__ type,
+                            const double *__restrict__ mass_ev, const double *__restrict__ epot,
+                            double *__restrict__ thermo, int slot) {
+  __shared__ double part[1024];
+  double s = 0.0;
+  for (int i = threadIdx.x; i < n; i += 1024) {
+    const double vx = vel[3 * (size_t)i], vy = vel[3 * (size_t)i + 1], vz = vel[3 * (size_t)i + 2];
+    s += 0.5 * mass_ev[type[i]] * (vx * vx + vy * vy + vz * vz);
+  }
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int off = 512; off > 0; off >>= 1) {
+    if ((int)threadIdx.x < off) part[threadIdx.x] += part[threadIdx.x + off];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const double ek = part[0];
+    thermo[3 * slot + 0] = *epot;
+    thermo[3 * slot + 1] = ek;
+    thermo[3 * slot + 2] = n > 0 ? 2.0 * ek / (3.0 * (double)n * 8.617333262e-5) : 0.0;
+  }
+}
+
+cudaError_t launch_md_kick_drift(int64_t n, double *coord, double *vel, const double *force, const int *type,
+                                 const double *hm, double dt, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_md_kick_drift<<<(unsigned)((3 * n + 255) / 256), 256, 0, st>>>((int)n, coord, vel, force, type, hm, dt);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_md_kick(int64_t n, double *vel, const double *force, const int *type, const double *hm,
+                           cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  k_md_kick<<<(unsigned)((3 * n + 255) / 256), 256, 0, st>>>((int)n, vel, force, type, hm);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_md_thermo(int64_t n, const double *vel, const int *type, const double *mass_ev, const double *epot,
+                             double *thermo, int slot, cudaStream_t st) {
+  k_md_thermo<<<1, 1024, 0, st>>>((int)n, vel, type, mass_ev, epot, thermo, slot);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}

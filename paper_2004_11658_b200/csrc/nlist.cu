@@ -121,14 +121,19 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
 
 struct __align__(16) NlHit { double r; int j; int t; };
 
+
+// MODE 0: candidates from the cell stencil (cells >= r_c).  MODE 1 (MD, rebuild step): cells >= r_c + skin; every
+// candidate within r_c + skin is also appended to the atom's raw list (the paper's LAMMPS skin list, PAPER.md:193,
+// :298).  MODE 2 (MD, reuse step): candidates are the raw list — Alg. 1 proper: format a raw list.
+template <int MODE>
 __global__ void __launch_bounds__(NL_THREADS)
 k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, const int *__restrict__ start, int cap,
-        int *__restrict__ nlist_out, DevStats *stats) {
+        int *__restrict__ nlist_out, DevStats *stats, NlRaw R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   NlHit *hit = reinterpret_cast<NlHit *>(smem_raw);               // [cap] (distance, atom index j, type of j)
   int *hp = reinterpret_cast<int *>(hit + cap);                   // [cap] sorted position of j
   __shared__ int r_start[NL_ENTRIES], r_pref[NL_ENTRIES + 1], r_type[NL_ENTRIES];
-  __shared__ int n_ranges, n_hit, cnt[DPB_MAX_TYPES];
+  __shared__ int n_ranges, n_hit, n_raw, cnt[DPB_MAX_TYPES];
 
   const int tid = threadIdx.x, lane = tid & 31;
   const int q = blockIdx.x;             // row inside the chunk
@@ -137,9 +142,9 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   const double xi[3] = {s_xyz[3 * (size_t)p], s_xyz[3 * (size_t)p + 1], s_xyz[3 * (size_t)p + 2]};
 
   if (tid < DPB_MAX_TYPES) cnt[tid] = 0;
-  if (tid == 0) n_hit = 0;
+  if (tid == 0) { n_hit = 0; n_raw = 0; }
   // stencil ranges, built and compacted by warp 0 (ballot + warp scan): entry = (type, x offset, y offset, part)
-  if (tid < 32) {
+  if (MODE != 2 && tid < 32) {
     int ic[3], lo[3], num[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {                                  // cell of atom i, recomputed exactly as in k_keys
@@ -192,19 +197,44 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   __syncthreads();
 
   const double rc2_hi = P.rc * P.rc * (1.0 + 1e-9);
-  const int ncand = r_pref[n_ranges];
-  int rp = 0;
-  for (int c = tid; c < ncand; c += NL_THREADS) {
-    while (c >= r_pref[rp + 1]) ++rp;
-    const int pj = r_start[rp] + (c - r_pref[rp]);
-    if (pj == p) continue;                                         // j != i (reading R19)
-    const double xj[3] = {s_xyz[3 * (size_t)pj], s_xyz[3 * (size_t)pj + 1], s_xyz[3 * (size_t)pj + 2]};
-    double d[3], r;
-    if (displacement_in_range(xi, xj, G.L, rc2_hi, d, r) && r <= P.rc) {   // "<=" as printed, PAPER.md:80 (R9)
-      const int t = r_type[rp];
-      atomicAdd(&cnt[t], 1);
-      const int h = atomicAdd(&n_hit, 1);
-      if (h < cap) { hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t; hp[h] = pj; }
+  if (MODE != 2) {
+    const int ncand = r_pref[n_ranges];
+    const double lim = MODE == 1 ? R.rs2_hi : rc2_hi;
+    int *raw_row = MODE == 1 ? R.raw + (size_t)p * R.cap : nullptr;
+    int rp = 0;
+    for (int c = tid; c < ncand; c += NL_THREADS) {
+      while (c >= r_pref[rp + 1]) ++rp;
+      const int pj = r_start[rp] + (c - r_pref[rp]);
+      if (pj == p) continue;                                         // j != i (reading R19)
+      const double xj[3] = {s_xyz[3 * (size_t)pj], s_xyz[3 * (size_t)pj + 1], s_xyz[3 * (size_t)pj + 2]};
+      double d[3], r;
+      if (displacement_in_range(xi, xj, G.L, lim, d, r)) {
+        if (MODE == 1) {
+          const int k = atomicAdd(&n_raw, 1);
+          if (k < R.cap) raw_row[k] = pj;
+        }
+        if (r <= P.rc) {                                             // "<=" as printed, PAPER.md:80 (R9)
+          const int t = r_type[rp];
+          atomicAdd(&cnt[t], 1);
+          const int h = atomicAdd(&n_hit, 1);
+          if (h < cap) { hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t; hp[h] = pj; }
+        }
+      }
+    }
+  } else {
+    const int ncand = min(R.nraw[p], R.cap);
+    const int *raw_row = R.raw + (size_t)p * R.cap;
+    for (int c = tid; c < ncand; c += NL_THREADS) {
+      const int pj = raw_row[c];
+      const double xj[3] = {s_xyz[3 * (size_t)pj], s_xyz[3 * (size_t)pj + 1], s_xyz[3 * (size_t)pj + 2]};
+      double d[3], r;
+      if (displacement_in_range(xi, xj, G.L, rc2_hi, d, r) && r <= P.rc) {
+        int t = 0;
+        while (t + 1 < P.ntypes && pj >= C.type_start[t + 1]) ++t;   // sorted positions are grouped by type
+        atomicAdd(&cnt[t], 1);
+        const int h = atomicAdd(&n_hit, 1);
+        if (h < cap) { hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t; hp[h] = pj; }
+      }
     }
   }
   __syncthreads();
@@ -213,6 +243,10 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   if (nh > cap) {
     if (tid == 0) atomicExch(&stats->err_cap, 1);
     nh = cap;
+  }
+  if (MODE == 1 && tid == 0) {
+    R.nraw[p] = n_raw;
+    if (n_raw > R.cap) atomicExch(&stats->err_cap, 1);
   }
   int *nl_row = C.nl + (size_t)q * P.nm;
   double4 *dr_row = C.dr + (size_t)q * P.nm;
@@ -264,16 +298,54 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
 }
 
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
-                         const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st) {
+                         const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode,
+                         const NlRaw *raw) {
   if (C.n <= 0) return cudaSuccess;
   const size_t smem = (size_t)cap * (sizeof(NlHit) + sizeof(int));
   static size_t configured = 0;
   if (smem > 48 * 1024 && smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_nlist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_nlist<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_nlist<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_nlist<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  k_nlist<<<C.n, NL_THREADS, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats);
+  NlRaw R{};
+  if (raw) R = *raw;
+  if (mode == 1) k_nlist<1><<<C.n, NL_THREADS, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R);
+  else if (mode == 2) k_nlist<2><<<C.n, NL_THREADS, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R);
+  else k_nlist<0><<<C.n, NL_THREADS, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}
+
+// MD reuse step: refresh the cell-sorted coordinate copy from the current coordinates (the sorted order of the last
+// rebuild stays) and track the largest displacement since that rebuild (skin criterion: must stay below skin / 2).
+__global__ void k_gather_sorted(int n, const double *__restrict__ coord, const int *__restrict__ s_idx,
+                                double *__restrict__ s_xyz, const double *__restrict__ xyz0, DevStats *stats) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  double d2 = 0.0;
+  if (p < n) {
+    const int i = s_idx[p];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double x = coord[3 * (size_t)i + c];
+      s_xyz[3 * (size_t)p + c] = x;
+      const double d = x - xyz0[3 * (size_t)p + c];
+      d2 += d * d;
+    }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) d2 = fmax(d2, __shfl_xor_sync(0xffffffffu, d2, off));
+  if ((threadIdx.x & 31) == 0 && d2 > 0.0)
+    atomicMax(reinterpret_cast<unsigned long long *>(&stats->max_disp2), (unsigned long long)__double_as_longlong(d2));
+}
+
+cudaError_t launch_gather_sorted(int64_t natoms, const double *coord, const int *s_idx, double *s_xyz,
+                                 const double *xyz0, DevStats *stats, cudaStream_t st) {
+  const int n = (int)natoms;
+  if (n <= 0) return cudaSuccess;
+  k_gather_sorted<<<(n + 255) / 256, 256, 0, st>>>(n, coord, s_idx, s_xyz, xyz0, stats);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
