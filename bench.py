@@ -177,6 +177,43 @@ def workload_config(name, args):
             "precision": getattr(args, "precision", "fp64")}
 
 
+# ---- molecular dynamics: the paper's own unit, steps/s and ns/day ----------------------
+def run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed):
+    """Random-init weights are not a physical potential: with the literal N(0, 1/fan_in) set the forces are ~4 eV/A rms
+    and the box heats to 1e5 K within 500 steps.  The MD leg therefore uses the conditioned weight set (fitting W0 / Nm,
+    DESIGN.md section 3: forces ~0.2 eV/A rms); the kernels and their cost are the same."""
+    import torch
+    from paper_2004_11658_b200 import DPModel
+    model = DPModel.from_spec(spec, emb, gen.condition_fit_w0(spec, fit), precision=1 if mixed else 0)
+    masses = gen.MASSES[name]
+    dt_fs = 0.5 if spec.ntypes == 2 else 1.0                     # PAPER.md:298: 0.5 fs water, 1.0 fs copper
+    vel = gen.maxwell_boltzmann(types, masses, 330.0, seed=gen.SEED_BASE + 500)
+    out = {}
+    for label, kw in (("skin2A_rebuild50", dict(rebuild_every=50, skin=2.0)), ("search_every_step", dict())):
+        if label.startswith("skin") and not (spec.rcut + 2.0 < 0.5 * min(box[0], box[4], box[8])):
+            out[label] = "r_c + skin >= L/2 for this box"
+            continue
+        dc, dv = torch.tensor(coord, device=dev), torch.tensor(vel, device=dev)
+        dt = torch.tensor(types, device=dev)
+        wc, wv = dc.clone(), dv.clone()
+        model.md_run(wc, wv, dt, masses, box, dt_fs, 10, thermo_every=10, **kw)          # warm-up on a copy
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        thermo, info = model.md_run(dc, dv, dt, masses, box, dt_fs, args.md_steps, thermo_every=20, **kw)
+        wall = time.perf_counter() - t0
+        etot = thermo[:, 0] + thermo[:, 1]
+        out[label] = {"steps": args.md_steps, "steps_per_s": args.md_steps / wall, "ms_per_step": wall / args.md_steps * 1e3,
+                      "ns_per_day": args.md_steps / wall * dt_fs * 1e-6 * 86400.0, "dt_fs": dt_fs,
+                      "atom_steps_per_s": coord.shape[0] * args.md_steps / wall,
+                      "rebuilds": info["n_rebuilds"], "max_displacement_A": info["max_displacement"],
+                      "skin_violated": info["skin_violated"],
+                      "etot_drift_rel_to_ekin": float(np.abs(etot - etot[0]).max() / thermo[0, 1]),
+                      "T_first_last_K": [float(thermo[0, 2]), float(thermo[-1, 2])]}
+    model.close()
+    out["weights"] = "conditioned (fitting W0 / Nm)"
+    return out
+
+
 # ---- the CUDA arm ---------------------------------------------------------------------------------------------
 def run_cuda(args):
     import torch
@@ -324,6 +361,8 @@ def run_cuda(args):
                                         f"({how}); the tensor pipe executes 3x these flops (3xTF32 split); the stage is bound "
                                         f"by MUFU (fp32 tanh) and instruction issue, not by the tensor pipe (DESIGN.md)"}
             line.pop("fp64_frac_of_peak", None)
+        if args.md_steps > 0:
+            line["md"] = run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed)
         if world == 1 and not args.no_cpu_baseline:
             step, k, desc, threads = oracle_step_sampler(name, gen.SEED_BASE, args.ref_sample)
             step()
@@ -352,6 +391,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=2048, help="atoms per step of the CPU oracle arm")
     ap.add_argument("--stage-every", type=int, default=10, help="read the stage timers every n-th step (0: never)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--md-steps", type=int, default=0,
+                    help="also run this many velocity-Verlet steps (dpb_md_run; PAPER.md:298: 330 K, 0.5 / 1.0 fs, 2 A skin "
+                         "rebuilt every 50 steps) and report steps/s and ns/day in an extra 'md' object")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
