@@ -29,6 +29,8 @@ CONFIGS = {
     "W24k":   SystemSpec("W24k",   "water",  16, True,  62.1,  0.10, 1),
     "Cu32k":  SystemSpec("Cu32k",  "copper", 20, False, 20 * 3.634, 0.05, 2),
     "Cu864k": SystemSpec("Cu864k", "copper", 60, False, 60 * 3.634, 0.05, 4),
+    # same box as Cu32k; the model is the paper's own copper model (gen.weights.COPPER_PAPER), SURVEY.md §8(f) NEXT #4
+    "Cu32k-paper": SystemSpec("Cu32k-paper", "copper", 20, False, 20 * 3.634, 0.05, 2),
 }
 
 _OH = 0.96                      # O-H bond length, Angstrom
@@ -120,7 +122,8 @@ def replicate(coord: np.ndarray, types: np.ndarray, box: np.ndarray, reps: int):
 
 
 # ---- molecular dynamics inputs (330 K) ------------------------------------
-MASSES = {"W192": (15.999, 1.008), "W24k": (15.999, 1.008), "Cu32k": (63.546,), "Cu864k": (63.546,)}   # amu
+MASSES = {"W192": (15.999, 1.008), "W24k": (15.999, 1.008), "Cu32k": (63.546,), "Cu864k": (63.546,),
+          "Cu32k-paper": (63.546,)}   # amu
 
 # CODATA 2018: atomic mass constant, elementary charge, Boltzmann constant
 _AMU_KG, _E_C, _KB_J = 1.66053906660e-27, 1.602176634e-19, 1.380649e-23

@@ -38,7 +38,10 @@ class ModelSpec:
 
 WATER = ModelSpec("water", 2, 6.0, 0.5, (46, 92), 25, 16, 240, 0)
 COPPER = ModelSpec("copper", 1, 8.0, 2.0, (512,), 32, 16, 240, 2)
-MODELS = {"W192": WATER, "W24k": WATER, "Cu32k": COPPER, "Cu864k": COPPER}
+# the copper model as the paper states it (PAPER.md:294 embedding 25-50-100, :296 Nm = 500);
+# BASELINE.json's copper configs use 32-64-128 and sel 512 (readings R16, R17).
+COPPER_PAPER = ModelSpec("copper-paper", 1, 8.0, 2.0, (500,), 25, 16, 240, 2)
+MODELS = {"W192": WATER, "W24k": WATER, "Cu32k": COPPER, "Cu864k": COPPER, "Cu32k-paper": COPPER_PAPER}
 
 
 def emb_net_size(s1: int) -> int:

@@ -165,3 +165,28 @@ def test_mixed_unsupported_shapes_and_bf16_are_reported():
         with pytest.raises(DPBError) as e:
             _model(spec, emb, fit, prec)
         assert e.value.status == -6
+
+
+def test_mixed_config5_copper_864k_against_fp64_path():
+    """BASELINE configs[4] (864,000 copper atoms, 27 chunks) in mixed precision: nlist identical to the fp64 path's
+    (compared on the device), E within 1e-5 and every force within 1e-3 eV/A of the fp64 CUDA path (which
+    test_gpu_parity.py::test_config5_copper_864k_sampled holds to the oracle)."""
+    torch = _torch()
+    from paper_2004_11658_b200.binding import TF32, FP64
+    spec = MODELS["Cu864k"]
+    coord, types, box = gen.make_system("Cu864k")
+    emb, fit = gen.make_weights(spec)
+    dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda")
+    res = {}
+    for name, prec in (("f64", FP64), ("tf32", TF32)):
+        m = _model(spec, emb, fit, prec)
+        out = m.eval(dc, dt, box, want_nlist=True, want_info=True)
+        torch.cuda.synchronize()
+        assert out["info"].n_overflow == 0 and out["info"].n_chunks == 27
+        res[name] = {k: v.clone() for k, v in out.items() if hasattr(v, "clone")}
+        m.close()
+    assert torch.equal(res["f64"]["nlist"], res["tf32"]["nlist"])
+    e64, e32 = res["f64"]["energy"].item(), res["tf32"]["energy"].item()
+    assert abs(e32 - e64) <= E_REL * abs(e64)
+    assert (res["tf32"]["force"] - res["f64"]["force"]).abs().max().item() <= F_ABS
+    assert res["tf32"]["force"].sum(0).abs().max().item() <= 1e-7
