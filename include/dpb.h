@@ -82,6 +82,13 @@ int dpb_model_set_chunk(dpb_model *model, int64_t chunk_atoms);
  * 1 = fused DMMA kernels (default).  Both compute the same path; tests compare each with the oracle. */
 int dpb_model_set_variant(dpb_model *model, int variant);
 
+/* Deterministic reduction (DPB_FP64, variant 1): forces and virial are summed in a fixed order instead of with fp64
+ * atomics, so two evaluations of the same input agree bit for bit (the paper reports E / F / virial reproducible to
+ * 15 / 10 / 13 digits; the default atomics mode differs at the 1e-16 relative level from run to run).
+ * Costs about N * Nm * 28 bytes of extra workspace and one gather kernel.  Exact only when no neighbour was dropped
+ * by a full type section (info.n_overflow == 0).  Other precisions / variants: dpb_eval returns DPB_ENOTIMPL. */
+int dpb_model_set_deterministic(dpb_model *model, int on);
+
 /* One evaluation (the paper's problem statement: coordinates, types and box in; E, E_i, F_i and the virial out).
  *   stream       cudaStream_t (as void*) on which all work is enqueued; NULL = the legacy default stream
  *   natoms       N >= 0

@@ -74,6 +74,7 @@ def load_library():
     lib.dpb_model_nm.argtypes = [vp]
     lib.dpb_model_set_chunk.argtypes = [vp, i64]
     lib.dpb_model_set_variant.argtypes = [vp, i32]
+    lib.dpb_model_set_deterministic.argtypes = [vp, i32]
     lib.dpb_model_set_timing.argtypes = [vp, i32]
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
     lib.dpb_set_debug_buffers.argtypes = [vp, vp, vp, vp]
@@ -142,6 +143,9 @@ class DPModel:
 
     def set_variant(self, v: int):
         self._chk(self.lib.dpb_model_set_variant(self._h, int(v)))
+
+    def set_deterministic(self, on: bool):
+        self._chk(self.lib.dpb_model_set_deterministic(self._h, int(bool(on))))
 
     def set_timing(self, on: bool):
         self._chk(self.lib.dpb_model_set_timing(self._h, int(bool(on))))

@@ -47,7 +47,7 @@ struct Buf {
 
 struct dpb_model {
   DevModel P;
-  int precision = 0, variant = 1, timing = 0;
+  int precision = 0, variant = 1, timing = 0, deterministic = 0;
   int64_t chunk = 32768;
   int device = 0;
   Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
@@ -63,6 +63,8 @@ struct dpb_model {
   Buf pairs;                    // mixed precision: flattened real-slot lists of the chunk
   Buf h_coord, h_type, h_out;   // device staging of dpb_eval_host
   // molecular dynamics driver (dpb_md_run): skin list of the last rebuild, forces, thermo output
+  // deterministic mode: inverse of s_idx, full-size lists, per-slot dE_i/dd_ik, per-atom virial parts
+  Buf pos_of, nl_all, nreal_all, fslot, vpart;
   Buf md_raw, md_nraw, md_xyz0, md_force, md_scal, md_mass;
   int md_cap_raw = 0;
   double md_skin = 0.0;
@@ -137,6 +139,7 @@ extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
                 &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
+                &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
                 &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
@@ -156,6 +159,12 @@ extern "C" int dpb_model_set_chunk(dpb_model *m, int64_t chunk) {
 extern "C" int dpb_model_set_variant(dpb_model *m, int variant) {
   if (!m || variant < 0 || variant > 1) return fail(DPB_EINVAL, "dpb_model_set_variant: variant must be 0 or 1");
   m->variant = variant;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_deterministic(dpb_model *m, int on) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  m->deterministic = on ? 1 : 0;
   return DPB_OK;
 }
 
@@ -257,6 +266,16 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   CU(m->s_idx.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
   CU(m->s_xyz.reserve(sizeof(double) * 3 * (size_t)(N + 1)), "workspace");
   CU(m->ei.reserve(sizeof(double) * (size_t)(N + 1)), "workspace");
+  const bool det = m->deterministic && !nlist_only;
+  if (det && (m->precision != DPB_FP64 || m->variant != 1 || !m->v1.ready))
+    return fail(DPB_ENOTIMPL, "the deterministic reduction is built for DPB_FP64, variant 1");
+  if (det) {
+    CU(m->pos_of.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
+    CU(m->nl_all.reserve(sizeof(int) * (size_t)(N + 1) * P.nm), "workspace");
+    CU(m->nreal_all.reserve(sizeof(int) * (size_t)(N + 1) * P.ntypes), "workspace");
+    CU(m->fslot.reserve(sizeof(double) * 3 * (size_t)(N + 1) * P.nm), "workspace");
+    CU(m->vpart.reserve(sizeof(double) * 9 * (size_t)(N + 1)), "workspace");
+  }
   CU(m->nl.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
   CU(m->dr.reserve(sizeof(double4) * (size_t)chunk * P.nm), "workspace");
   CU(m->nreal.reserve(sizeof(int) * (size_t)chunk * P.ntypes), "workspace");
@@ -303,7 +322,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
                             st), "gather");
   } else {
     CU(launch_cell_sort(P, G, natoms, coord, type, m->key.as<int>(), m->count.as<int>(), start, m->cursor.as<int>(),
-                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st), "cell sort");
+                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st, det ? m->pos_of.as<int>() : nullptr),
+       "cell sort");
     if (nl_mode == 1 && natoms > 0)
       CU(cudaMemcpyAsync(m->md_xyz0.p, m->s_xyz.p, sizeof(double) * 3 * (size_t)natoms, cudaMemcpyDeviceToDevice, st),
          "copy of the rebuild coordinates");
@@ -328,6 +348,12 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.nreal = m->nreal.as<int>();
     C.T = m->T.as<double>();
     C.dT = m->dT.as<double>();
+    C.fslot = nullptr;
+    if (det) {                                           // full-size lists: the gather needs every atom's row
+      C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
+      C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;
+      C.fslot = m->fslot.as<double>() + 3 * (size_t)p0 * P.nm;
+    }
     CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st, nl_mode, nl_mode ? &raw : nullptr),
        "nlist");
     if (nlist_only) continue;
@@ -364,6 +390,10 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
     }
   }
+  if (det)
+    CU(launch_force_gather(P, G, natoms, m->s_idx.as<int>(), m->pos_of.as<int>(), start + nkeys + 1,
+                           m->s_xyz.as<double>(), m->nl_all.as<int>(), m->nreal_all.as<int>(), m->fslot.as<double>(),
+                           force, m->vpart.as<double>(), virial, st), "deterministic force gather");
   if (!nlist_only) {
     if (energy) CU(launch_reduce_energy(natoms, ei, energy, st), "energy reduction");
     if (timing) cudaEventRecord(m->evs[2 + 4 * nchunks], st);

@@ -53,6 +53,7 @@ struct ChunkView {
   int *nreal;              // [n][ntypes] real (non-padded) slots per section
   double *T;               // [n][M][4]
   double *dT;              // [n][M][4]
+  double *fslot;           // deterministic mode: [n][nm][3] dE_i/dd_ik per slot (pass 2 stores instead of scattering)
 };
 
 // Process-wide count of kernels launched by this library (reported by dpb_kernel_launches()).
@@ -62,7 +63,11 @@ extern unsigned long long g_dpb_launches;
 // ---- launchers implemented in the .cu files (all asynchronous on `st`; return cudaGetLastError()) ----------
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
-                             DevStats *stats, cudaStream_t st);
+                             DevStats *stats, cudaStream_t st, int *pos_of = nullptr);
+// deterministic force / virial reduction (det.cu)
+cudaError_t launch_force_gather(const DevModel &P, const DevGrid &G, int64_t natoms, const int *s_idx, const int *pos_of,
+                                const int *type_start, const double *s_xyz, const int *nl_all, const int *nreal_all,
+                                const double *fslot, double *force, double *vpart, double *virial, cudaStream_t st);
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
                          const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode = 0,
                          const NlRaw *raw = nullptr);

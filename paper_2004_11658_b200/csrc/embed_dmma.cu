@@ -418,6 +418,11 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         const double dot = pr[1] * dv.x + pr[2] * dv.y + pr[3] * dv.z;
         const double cm = (dR0 * sp + qp * dot) * ir;
         const double f0 = fma(cm, dv.x, qq * pr[1]), f1 = fma(cm, dv.y, qq * pr[2]), f2 = fma(cm, dv.z, qq * pr[3]);
+        if (C.fslot) {
+          // deterministic mode: keep dE_i/dd_ik per slot; forces and virial are gathered in a fixed order afterwards
+          double *fs = C.fslot + ((size_t)qa * P.nm + P.sec_start[t] + row) * 3;
+          fs[0] = f0; fs[1] = f1; fs[2] = f2;
+        } else {
         const int j = nl[row];
         if (force) {
           atomicAdd(&force[3 * (size_t)j + 0], -f0);
@@ -428,6 +433,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         vir[0] -= dv.x * f0; vir[1] -= dv.x * f1; vir[2] -= dv.x * f2;
         vir[3] -= dv.y * f0; vir[4] -= dv.y * f1; vir[5] -= dv.y * f2;
         vir[6] -= dv.z * f0; vir[7] -= dv.z * f1; vir[8] -= dv.z * f2;
+        }
       }
     }
     // F_i += sum_k f_ik (ProdForce)
@@ -441,7 +447,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
       v += __shfl_xor_sync(0xffffffffu, v, 16);
       fi[k] = v;
     }
-    if (lane < 3 && force) atomicAdd(&force[3 * (size_t)C.s_idx[C.p0 + qa] + lane], lane == 0 ? fi[0] : (lane == 1 ? fi[1] : fi[2]));
+    if (lane < 3 && force && !C.fslot) atomicAdd(&force[3 * (size_t)C.s_idx[C.p0 + qa] + lane], lane == 0 ? fi[0] : (lane == 1 ? fi[1] : fi[2]));
   }
   // virial (ProdVirial): warp -> block -> one atomic per component and CTA
 #pragma unroll
@@ -452,7 +458,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
     if (lane == 0) vred[warp][k] = v;
   }
   __syncthreads();
-  if (tid < 9 && virial) {
+  if (tid < 9 && virial && !C.fslot) {
     double v = 0.0;
     for (int w = 0; w < P2_WARPS; ++w) v += vred[w][tid];
     atomicAdd(&virial[tid], v);

@@ -86,11 +86,12 @@ __global__ void k_scan(int nkeys, int ncell, int ntypes, const int *__restrict__
 }
 
 __global__ void k_fill(int n, const double *__restrict__ coord, const int *__restrict__ key, int *__restrict__ cursor,
-                       int *__restrict__ s_idx, double *__restrict__ s_xyz) {
+                       int *__restrict__ s_idx, double *__restrict__ s_xyz, int *__restrict__ pos_of) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int p = atomicAdd(&cursor[key[i]], 1);   // order inside a (type, cell) bucket is irrelevant: Alg. 1's key is total
   s_idx[p] = i;
+  if (pos_of) pos_of[i] = p;
   s_xyz[3 * (size_t)p + 0] = coord[3 * (size_t)i + 0];
   s_xyz[3 * (size_t)p + 1] = coord[3 * (size_t)i + 1];
   s_xyz[3 * (size_t)p + 2] = coord[3 * (size_t)i + 2];
@@ -98,7 +99,7 @@ __global__ void k_fill(int n, const double *__restrict__ coord, const int *__res
 
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
-                             DevStats *stats, cudaStream_t st) {
+                             DevStats *stats, cudaStream_t st, int *pos_of) {
   const int nkeys = P.ntypes * G.ncell;
   cudaError_t e = cudaMemsetAsync(count, 0, sizeof(int) * (size_t)nkeys, st);
   if (e != cudaSuccess) return e;
@@ -106,7 +107,7 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
   if (n > 0) k_keys<<<(n + 255) / 256, 256, 0, st>>>(P, G, n, coord, type, key, count, stats);
   // type_start lives right behind start[nkeys + 1]
   k_scan<<<1, 1024, 0, st>>>(nkeys, G.ncell, P.ntypes, count, start, cursor, start + nkeys + 1);
-  if (n > 0) k_fill<<<(n + 255) / 256, 256, 0, st>>>(n, coord, key, cursor, s_idx, s_xyz);
+  if (n > 0) k_fill<<<(n + 255) / 256, 256, 0, st>>>(n, coord, key, cursor, s_idx, s_xyz, pos_of);
   DPB_LAUNCHED(n > 0 ? 3 : 1);
   return cudaGetLastError();
 }

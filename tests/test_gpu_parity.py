@@ -308,3 +308,58 @@ def test_replication_extensivity_gpu():
     assert np.abs(big["force"].reshape(8, -1, 3) - small["force"][None]).max() <= 1e-10
     assert np.abs(big["virial"] - 8 * small["virial"]).max() <= 1e-10 * np.abs(8 * small["virial"]).max()
     m.close()
+
+
+@pytest.mark.parametrize("chunk", [100000, 50])
+def test_deterministic_reduction(chunk):
+    """SURVEY.md §7 hard part 6: forces and virial gathered in a fixed order (no atomics).  Two evaluations agree bit for
+    bit, the result matches the oracle to the fp64 bar and the atomics mode to rounding; also with chunks that cut the
+    species ranges (the gather needs every atom's row)."""
+    torch = _torch()
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, 1)
+    m.set_chunk(chunk)
+    ref = orc.eval(coord, types, box)
+    atom = _gpu_eval(m, coord, types, box)
+    m.set_deterministic(True)
+    d1 = _gpu_eval(m, coord, types, box)
+    d2 = _gpu_eval(m, coord, types, box)
+    _check_full(ref, d1)
+    assert np.array_equal(d1["force"], d2["force"]) and np.array_equal(d1["virial"], d2["virial"])
+    assert d1["energy"][0] == d2["energy"][0]
+    assert np.abs(d1["force"] - atom["force"]).max() <= 1e-12
+    assert np.abs(d1["virial"] - atom["virial"]).max() <= 1e-12 * np.abs(atom["virial"]).max()
+    m.close()
+
+
+def test_deterministic_reduction_full_size_is_bitwise_reproducible():
+    """W24k: the atomics mode differs between two runs in the last bits of some forces; the deterministic mode does not."""
+    torch = _torch()
+    spec = MODELS["W24k"]
+    coord, types, box = gen.make_system("W24k")
+    emb, fit = gen.make_weights(spec)
+    _, m = _models(spec, emb, fit, 1)
+    a1 = _gpu_eval(m, coord, types, box)
+    m.set_deterministic(True)
+    d1 = _gpu_eval(m, coord, types, box)
+    d2 = _gpu_eval(m, coord, types, box)
+    assert np.array_equal(d1["force"], d2["force"]) and np.array_equal(d1["virial"], d2["virial"])
+    assert np.abs(d1["force"] - a1["force"]).max() <= 1e-11
+    assert np.abs(d1["force"].sum(0)).max() <= 1e-9
+    m.close()
+
+
+def test_deterministic_mode_is_refused_where_it_is_not_built():
+    from paper_2004_11658_b200 import DPBError
+    torch = _torch()
+    spec, emb, fit = small_model()
+    _, m = _models(spec, emb, fit, 0)
+    m.set_deterministic(True)
+    coord, types, box = random_box(40, 10.0, 2, seed=2, min_dist=1.0)
+    with pytest.raises(DPBError) as e:
+        m.eval(torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda"), box)
+    assert e.value.status == -6
+    m.close()
