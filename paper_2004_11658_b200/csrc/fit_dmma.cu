@@ -173,16 +173,16 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
 // S5: D[b][a] = sum_c T[b][c] T[a][c] (Eq. 4; flatten b M^< + a, reading R7), zero-padded to dimp.
 __global__ void k_descr_v1(DevModel P, ChunkView C, int dimp, double *__restrict__ D) {
   const int q = blockIdx.x;
-  __shared__ double Ts[1024 + 16];
+  __shared__ double Ts[256 * 5 + 16];            // row stride 5 doubles: the 16 rows a = 0..15 hit 16 distinct bank pairs
   const double *T = C.T + (size_t)q * P.M * 4;
-  for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
+  for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[(k >> 2) * 5 + (k & 3)] = T[k];
   __syncthreads();
   for (int e = threadIdx.x; e < dimp; e += blockDim.x) {
     double acc = 0.0;
     if (e < P.dim) {
       const int b = e / P.Ma, a = e - b * P.Ma;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) acc += Ts[b * 4 + c] * Ts[a * 4 + c];
+      for (int c = 0; c < 4; ++c) acc += Ts[b * 5 + c] * Ts[a * 5 + c];
     }
     D[(size_t)q * dimp + e] = acc;
   }
@@ -194,11 +194,12 @@ __global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restr
   const int q = blockIdx.x;
   extern __shared__ double sm2[];
   double *Ts = sm2;                      // [M][4]
-  double *dd = sm2 + P.M * 4;            // [dim]
-  double *part = dd + P.dim;             // [nparts][Ma * 4]
+  const int ldr = P.Ma + 1;              // padded row stride: rows b, b + 1, ... fall into different banks
+  double *dd = sm2 + P.M * 4;            // [M][Ma + 1]
+  double *part = dd + P.M * ldr;         // [nparts][Ma * 4]
   const double *T = C.T + (size_t)q * P.M * 4;
   for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[k] = T[k];
-  for (int k = threadIdx.x; k < P.dim; k += blockDim.x) dd[k] = dD[(size_t)q * dimp + k];
+  for (int k = threadIdx.x; k < P.dim; k += blockDim.x) dd[(k / P.Ma) * ldr + (k % P.Ma)] = dD[(size_t)q * dimp + k];
   __syncthreads();
   const int nout2 = P.Ma * 4;
   const int nparts = max(1, (int)blockDim.x / nout2);
@@ -206,14 +207,14 @@ __global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restr
     const int pt = idx / nout2, o = idx - pt * nout2, bcol = o >> 2, c = o & 3;
     const int per = (P.M + nparts - 1) / nparts, lo = pt * per, hi = min(P.M, lo + per);
     double acc = 0.0;
-    for (int bp = lo; bp < hi; ++bp) acc += dd[bp * P.Ma + bcol] * Ts[bp * 4 + c];
+    for (int bp = lo; bp < hi; ++bp) acc += dd[bp * ldr + bcol] * Ts[bp * 4 + c];
     part[idx] = acc;
   }
   __syncthreads();
   for (int e = threadIdx.x; e < P.M * 4; e += blockDim.x) {
     const int b = e >> 2, c = e & 3;
     double acc = 0.0;
-    for (int a = 0; a < P.Ma; ++a) acc += dd[b * P.Ma + a] * Ts[a * 4 + c];
+    for (int a = 0; a < P.Ma; ++a) acc += dd[b * ldr + a] * Ts[a * 4 + c];
     if (b < P.Ma)
       for (int pt = 0; pt < nparts; ++pt) acc += part[pt * nout2 + e];
     C.dT[(size_t)q * P.M * 4 + e] = acc;
@@ -359,7 +360,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
     if ((e = gemm<8, EPI_STORE>(C, ty, g, st)) != cudaSuccess) return e;
   }
-  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + P.dim + 256 + 4 * P.Ma);
+  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
   static size_t configured = 0;
   if (sm > 48 * 1024 && sm > configured) {
     e = cudaFuncSetAttribute(k_dT_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
