@@ -238,7 +238,7 @@ static int cuda_fail(cudaError_t e, const char *what) {
 static int neighbour_cap(const DevModel &P) {
   int cap = 2 * P.nm;
   if (cap < 256) cap = 256;
-  if (cap > 11000) cap = 11000;       // 20 B per hit: 215 KB of shared memory at most
+  if (cap > 9000) cap = 9000;         // 24 B per hit: 211 KB of shared memory at most
   return cap;
 }
 

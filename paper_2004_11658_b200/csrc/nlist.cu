@@ -119,6 +119,7 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
 // positions (two runs when the column wraps around the box): 9 x 2 entries per type instead of 27.
 #define NL_THREADS 128
 #define NL_ENTRIES (18 * DPB_MAX_TYPES)
+#define NL_BUCKETS 32           // distance buckets per type, uniform in r^3: the ranking only compares inside a bucket
 
 struct __align__(16) NlHit { double r; int j; int t; };
 
@@ -133,6 +134,8 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   extern __shared__ __align__(16) unsigned char smem_raw[];
   NlHit *hit = reinterpret_cast<NlHit *>(smem_raw);               // [cap] (distance, atom index j, type of j)
   int *hp = reinterpret_cast<int *>(hit + cap);                   // [cap] sorted position of j
+  int *order = hp + cap;                                          // [cap] hits grouped by (type, distance bucket)
+  __shared__ int bcnt[DPB_MAX_TYPES * NL_BUCKETS], bstart[DPB_MAX_TYPES * NL_BUCKETS + 1];
   __shared__ int r_start[NL_ENTRIES], r_pref[NL_ENTRIES + 1], r_type[NL_ENTRIES];
   __shared__ int n_ranges, n_hit, n_raw, cnt[DPB_MAX_TYPES];
 
@@ -143,6 +146,8 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   const double xi[3] = {s_xyz[3 * (size_t)p], s_xyz[3 * (size_t)p + 1], s_xyz[3 * (size_t)p + 2]};
 
   if (tid < DPB_MAX_TYPES) cnt[tid] = 0;
+  for (int k = tid; k < DPB_MAX_TYPES * NL_BUCKETS; k += NL_THREADS) bcnt[k] = 0;
+  const double binv = (double)NL_BUCKETS / (P.rc * P.rc * P.rc);
   if (tid == 0) { n_hit = 0; n_raw = 0; }
   // stencil ranges, built and compacted by warp 0 (ballot + warp scan): entry = (type, x offset, y offset, part)
   if (MODE != 2 && tid < 32) {
@@ -218,7 +223,11 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
           const int t = r_type[rp];
           atomicAdd(&cnt[t], 1);
           const int h = atomicAdd(&n_hit, 1);
-          if (h < cap) { hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t; hp[h] = pj; }
+          if (h < cap) {
+            const int b = min(NL_BUCKETS - 1, (int)(r * r * r * binv));     // monotone in r: consistent with the order
+            hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t * NL_BUCKETS + b; hp[h] = pj;
+            atomicAdd(&bcnt[t * NL_BUCKETS + b], 1);
+          }
         }
       }
     }
@@ -234,7 +243,11 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
         while (t + 1 < P.ntypes && pj >= C.type_start[t + 1]) ++t;   // sorted positions are grouped by type
         atomicAdd(&cnt[t], 1);
         const int h = atomicAdd(&n_hit, 1);
-        if (h < cap) { hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t; hp[h] = pj; }
+        if (h < cap) {
+          const int b = min(NL_BUCKETS - 1, (int)(r * r * r * binv));
+          hit[h].r = r; hit[h].j = C.s_idx[pj]; hit[h].t = t * NL_BUCKETS + b; hp[h] = pj;
+          atomicAdd(&bcnt[t * NL_BUCKETS + b], 1);
+        }
       }
     }
   }
@@ -253,22 +266,41 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   double4 *dr_row = C.dr + (size_t)q * P.nm;
   int *out_row = nlist_out ? nlist_out + (size_t)i * P.nm : nullptr;
 
-  // Alg. 1 line 7: order by (type, distance, index).  rank = number of hits of the same type that
-  // precede this one; the first sel[t] go to section t (line 8-9, :186-193), the others are dropped (reading R8).
+  // Alg. 1 line 7: order by (type, distance, index).  Hits are grouped by (type, bucket of r^3) with a
+  // counting sort; the rank of a hit inside its type = hits in earlier buckets + hits of its own bucket that precede
+  // it under the exact key (r as fp64, then j).  The first sel[t] go to section t (line 8-9, :186-193), the others are
+  // dropped (reading R8).
+  const int nb = P.ntypes * NL_BUCKETS;
+  if (tid < 32) {                                             // exclusive scan of the bucket counts (<= 256 entries)
+    const int per = (nb + 31) / 32, lo = tid * per;
+    int sum = 0;
+    for (int k = lo; k < min(nb, lo + per); ++k) sum += bcnt[k];
+    int incl = sum;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int v = __shfl_up_sync(0xffffffffu, incl, off);
+      if (lane >= off) incl += v;
+    }
+    int run = incl - sum;
+    for (int k = lo; k < min(nb, lo + per); ++k) { bstart[k] = run; run += bcnt[k]; bcnt[k] = 0; }
+    if (tid == 31) bstart[nb] = incl;
+  }
+  __syncthreads();
   for (int h = tid; h < nh; h += NL_THREADS) {
+    const int bk = hit[h].t;
+    order[bstart[bk] + atomicAdd(&bcnt[bk], 1)] = h;
+  }
+  __syncthreads();
+  for (int pos = tid; pos < nh; pos += NL_THREADS) {
+    const int h = order[pos];
     const NlHit me = hit[h];
-    int rank0 = 0, rank1 = 0;
-    int g = 0;
-    for (; g + 1 < nh; g += 2) {
-      const NlHit u = hit[g], v = hit[g + 1];
-      rank0 += (u.t == me.t) & ((u.r < me.r) | ((u.r == me.r) & (u.j < me.j)));
-      rank1 += (v.t == me.t) & ((v.r < me.r) | ((v.r == me.r) & (v.j < me.j)));
+    const int t = me.t / NL_BUCKETS, lo = bstart[me.t], hi = bstart[me.t + 1];
+    int less = 0;
+    for (int g = lo; g < hi; ++g) {
+      const NlHit u = hit[order[g]];
+      less += (u.r < me.r) | ((u.r == me.r) & (u.j < me.j));
     }
-    if (g < nh) {
-      const NlHit u = hit[g];
-      rank0 += (u.t == me.t) & ((u.r < me.r) | ((u.r == me.r) & (u.j < me.j)));
-    }
-    const int rank = rank0 + rank1, t = me.t;
+    const int rank = lo - bstart[t * NL_BUCKETS] + less;
     if (rank < P.sel[t]) {
       const int slot = P.sec_start[t] + rank;
       nl_row[slot] = me.j;
@@ -302,7 +334,7 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
                          const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode,
                          const NlRaw *raw) {
   if (C.n <= 0) return cudaSuccess;
-  const size_t smem = (size_t)cap * (sizeof(NlHit) + sizeof(int));
+  const size_t smem = (size_t)cap * (sizeof(NlHit) + 2 * sizeof(int));
   static size_t configured = 0;
   if (smem > 48 * 1024 && smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_nlist<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
