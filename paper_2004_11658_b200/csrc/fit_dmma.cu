@@ -128,39 +128,55 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
   }
   cp_async_wait<0>();
 
-  // epilogue: thread (gq, q) holds rows 16 wm + gq (+8), columns n0 + 8 NBW wn + 8 nb + 2 q (+1)
+  // epilogue: thread (gq, q) holds rows 16 wm + gq (+8), columns n0 + 8 NBW wn + 8 nb + 2 q (+1).
+  // The element-wise inputs of one m-block are loaded first, all at once (the stores below may alias them as far as
+  // the compiler knows, so loads interleaved with stores would serialise NBW global round trips per row).
+  const double2 zero2 = make_double2(0.0, 0.0);
 #pragma unroll
   for (int mb = 0; mb < 2; ++mb) {
     const int m = m0 + 16 * wm + gq + 8 * mb;
     if (m >= row_hi) continue;
+    const int nbase = n0 + 8 * NBW * wn + 2 * q;
+    double2 x0[NBW], x1[NBW];
 #pragma unroll
     for (int nb = 0; nb < NBW; ++nb) {
-      const int n = n0 + 8 * NBW * wn + 8 * nb + 2 * q;
+      const int n = nbase + 8 * nb;
+      const size_t oi = (size_t)m * g.ldi + n;
+      x0[nb] = zero2; x1[nb] = zero2;
+      if (n < g.N) {
+        if (EPI == EPI_TANH_SKIP || EPI == EPI_L3) x0[nb] = *reinterpret_cast<const double2 *>(g.in0 + oi);
+        if (EPI == EPI_BWD) {
+          if (g.in0) x0[nb] = *reinterpret_cast<const double2 *>(g.in0 + oi);
+          x1[nb] = *reinterpret_cast<const double2 *>(g.in1 + oi);
+        }
+      }
+    }
+#pragma unroll
+    for (int nb = 0; nb < NBW; ++nb) {
+      const int n = nbase + 8 * nb;
       if (n >= g.N) continue;
       double v0 = acc[mb][nb][0], v1 = acc[mb][nb][1];
-      const size_t oi = (size_t)m * g.ldi + n, oo = (size_t)m * g.ldo + n;
+      const size_t oo = (size_t)m * g.ldo + n;
       if (EPI == EPI_TANH) {
         const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
         *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(dp_tanh(v0 + b.x), dp_tanh(v1 + b.y));
       } else if (EPI == EPI_TANH_SKIP) {
         const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
-        const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi);
         const double u0 = dp_tanh(v0 + b.x), u1 = dp_tanh(v1 + b.y);
         *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(u0, u1);
-        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(z.x + u0, z.y + u1);
+        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(x0[nb].x + u0, x0[nb].y + u1);
       } else if (EPI == EPI_L3) {
         // bias = b2, in1 = w3 (as a [N] vector), in0 = Z1: out1 = Z2 = Z1 + U2, out0 = Q2 = w3 (1 - U2^2)
         const double2 b = *reinterpret_cast<const double2 *>(g.bias + n);
         const double2 w = *reinterpret_cast<const double2 *>(g.in1 + n);
-        const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi);
         const double u0 = dp_tanh(v0 + b.x), u1 = dp_tanh(v1 + b.y);
-        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(z.x + u0, z.y + u1);
+        *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(x0[nb].x + u0, x0[nb].y + u1);
         *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(w.x * (1.0 - u0 * u0), w.y * (1.0 - u1 * u1));
       } else if (EPI == EPI_BWD) {
         // dz = acc + bias[n] (w3, first backward step) + in0 (dZ of the next layer); out0 = dz; out1 = dz (1 - in1^2)
         if (g.bias) { const double2 b = *reinterpret_cast<const double2 *>(g.bias + n); v0 += b.x; v1 += b.y; }
-        if (g.in0) { const double2 z = *reinterpret_cast<const double2 *>(g.in0 + oi); v0 += z.x; v1 += z.y; }
-        const double2 u = *reinterpret_cast<const double2 *>(g.in1 + oi);
+        v0 += x0[nb].x; v1 += x0[nb].y;
+        const double2 u = x1[nb];
         if (g.out0) *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0, v1);
         *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(v0 * (1.0 - u.x * u.x), v1 * (1.0 - u.y * u.y));
       } else {
