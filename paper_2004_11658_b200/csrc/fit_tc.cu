@@ -274,6 +274,7 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
 // ---- S5: descriptor as the A image of G1 ---------------------------------------------------------------------------
 // D[b M^< + a] = sum_c T[b][c] T[a][c] (Eq. 4; reading R7), from the fp64 T rounded to fp32, written
 // straight into the hi / lo operand images (the descriptor never exists in another form).  Thread = atom (tile row).
+#define DESCR_BS 8
 template <int MA>
 __global__ void __launch_bounds__(128) k_descr_tc(DevModel P, ChunkView C, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
   const int tile = blockIdx.x, r = threadIdx.x, m = tile * 128 + r;
@@ -285,18 +286,31 @@ __global__ void __launch_bounds__(128) k_descr_tc(DevModel P, ChunkView C, int k
     const double2 u = *reinterpret_cast<const double2 *>(T + 4 * a), v = *reinterpret_cast<const double2 *>(T + 4 * a + 2);
     ta[a][0] = (float)u.x; ta[a][1] = (float)u.y; ta[a][2] = (float)v.x; ta[a][3] = (float)v.y;
   }
-  for (int b = 0; b < P.M; ++b) {
+  // blockIdx.y splits the b range into slices of DESCR_BS rows (192 row tiles alone would leave most of the GPU idle);
+  // the slice's T rows are loaded up front: the image stores below may alias T as far as the compiler knows
+  const int b_lo = blockIdx.y * DESCR_BS;
+  float tb[DESCR_BS][4];
+#pragma unroll
+  for (int i = 0; i < DESCR_BS; ++i) {
+    const int b = min(b_lo + i, P.M - 1);
     const double2 u = *reinterpret_cast<const double2 *>(T + 4 * b), v = *reinterpret_cast<const double2 *>(T + 4 * b + 2);
-    const float t0 = (float)u.x, t1 = (float)u.y, t2 = (float)v.x, t3 = (float)v.y;
+    tb[i][0] = (float)u.x; tb[i][1] = (float)u.y; tb[i][2] = (float)v.x; tb[i][3] = (float)v.y;
+  }
+#pragma unroll
+  for (int i = 0; i < DESCR_BS; ++i) {
+    const int b = b_lo + i;
+    if (b >= P.M) break;
 #pragma unroll
     for (int a = 0; a < MA; a += 4) {
       float d[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) d[i] = fmaf(t0, ta[a + i][0], fmaf(t1, ta[a + i][1], fmaf(t2, ta[a + i][2], t3 * ta[a + i][3])));
+      for (int k = 0; k < 4; ++k)
+        d[k] = fmaf(tb[i][0], ta[a + k][0], fmaf(tb[i][1], ta[a + k][1], fmaf(tb[i][2], ta[a + k][2], tb[i][3] * ta[a + k][3])));
       img_store4(Dh, Dl, (size_t)tile, kpan, b * MA + a, r, d[0], d[1], d[2], d[3]);
     }
   }
-  for (int k = P.M * MA; k < kpan * FT_KP; k += 4) img_store4(Dh, Dl, (size_t)tile, kpan, k, r, 0.f, 0.f, 0.f, 0.f);
+  if (blockIdx.y == gridDim.y - 1)
+    for (int k = P.M * MA; k < kpan * FT_KP; k += 4) img_store4(Dh, Dl, (size_t)tile, kpan, k, r, 0.f, 0.f, 0.f, 0.f);
 }
 
 // ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c] (one of the S7 contractions: fp32
@@ -533,9 +547,9 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
   float *dZ1 = p; p += rows * F->fwp;
   float *dD = p;
   switch (P.Ma) {
-    case 4: k_descr_tc<4><<<(unsigned)tiles, 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
-    case 8: k_descr_tc<8><<<(unsigned)tiles, 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
-    default: k_descr_tc<16><<<(unsigned)tiles, 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+    case 4: k_descr_tc<4><<<dim3((unsigned)tiles, (unsigned)((P.M + DESCR_BS - 1) / DESCR_BS)), 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+    case 8: k_descr_tc<8><<<dim3((unsigned)tiles, (unsigned)((P.M + DESCR_BS - 1) / DESCR_BS)), 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+    default: k_descr_tc<16><<<dim3((unsigned)tiles, (unsigned)((P.M + DESCR_BS - 1) / DESCR_BS)), 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
   }
   DPB_LAUNCHED(1);
   for (int ty = 0; ty < P.ntypes; ++ty) {
