@@ -97,6 +97,11 @@ def test_md_mixed_precision_tracks_fp64():
     assert np.abs(x1 - x0).max() <= 1e-4
     e0, e1 = th0[:, 0] + th0[:, 1], th1[:, 0] + th1[:, 1]
     assert np.abs(e1 - e1[0]).max() <= 3 * np.abs(e0 - e0[0]).max() + 1e-3
+    # skin list in mixed precision (r_c + skin = 6.2 A < L/2 = 6.21 A): same trajectory as searching every step
+    x2, v2, th2, i2 = _gpu_md(spec, emb, fit, coord, vel, types, box, mass, precision=1, rebuild_every=2, skin=0.2, **kw)
+    assert i2["n_rebuilds"] == 11 and not i2["skin_violated"], i2
+    # the skin grid sorts the atoms differently, so the 128-pair tiles (and their fp32 partial sums) differ: fp32-level
+    assert np.abs(x2 - x1).max() <= 1e-6
 
 
 def test_md_argument_errors():
