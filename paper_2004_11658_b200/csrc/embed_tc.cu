@@ -195,8 +195,8 @@ __device__ __forceinline__ void mma3(uint32_t tmem_d, uint32_t a_hi, uint32_t a_
 // ---- pass 1 ----------------------------------------------------------------------------------------------------
 template <int S1>
 __global__ void __launch_bounds__(256, 1)
-k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int *__restrict__ off_t,
-           const int *__restrict__ pidx_t, int a, int t) {
+k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t net_stride,
+           const int *__restrict__ off_all, const int *__restrict__ pidx_all) {
   using L = TL<S1>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const int tid = threadIdx.x, wg = tid >> 7, wt = tid & 127, warp = tid >> 5;
@@ -207,8 +207,6 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + L::oBar) + wg;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::oTmem);
 
-  for (int k = tid; k < L::img_bytes / 16; k += 256)
-    reinterpret_cast<int4 *>(smem)[k] = reinterpret_cast<const int4 *>(net_img)[k];
   if (warp == 0) tc::tmem_alloc<512>(tmem_slot);
   if (tid == 0) {
     tc::mbar_init(reinterpret_cast<uint64_t *>(smem + L::oBar), 1);
@@ -225,11 +223,24 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
   const uint32_t slot_a = tc::smem_u32(slot), img_a = tc::smem_u32(smem);
   const uint32_t rowbase = (uint32_t)(wt >> 3) * 1024u + (uint32_t)(wt & 7) * 128u, r7 = wt & 7;
 
+  // one launch walks all ntypes^2 nets (a = centre type, t = neighbour type): the CTA reloads the weight image at a net
+  // switch, so only the last net has a tail in which SMs idle (four launches per pass had four)
+  uint32_t phase = 0;
+  for (int net = 0; net < P.ntypes * P.ntypes; ++net) {
+  const int a = net / P.ntypes, t = net - a * P.ntypes;
+  const int *off_t = off_all + (size_t)t * (C.n + 1), *pidx_t = pidx_all + (size_t)C.n * P.sec_start[t];
+  __syncthreads();                                          // every MMA that read the previous image has completed
+  {
+    const float *net_img = all_img + (size_t)net * net_stride;
+    for (int k = tid; k < L::img_bytes / 16; k += 256)
+      reinterpret_cast<int4 *>(smem)[k] = reinterpret_cast<const int4 *>(net_img)[k];
+  }
+  tc::fence_proxy_async();
+  __syncthreads();
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
   int flat0 = 0, flat1 = 0;
   if (row_hi > row_lo) { flat0 = off_t[row_lo]; flat1 = off_t[row_hi]; }
   const int ntiles = (flat1 - flat0 + 127) >> 7;
-  uint32_t phase = 0;
 #ifdef TC_PROF
   long long tp[11];
 #endif
@@ -401,8 +412,8 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
         }
         a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
         double *dst = C.T + ((size_t)cur * P.M + b) * 4;
-        if (t == 0 && (se & 256)) {
-          // first section and the whole section of this atom lies inside the tile: nobody else writes T[cur][b][:] yet
+        if (P.ntypes == 1 && (se & 256)) {
+          // one net only and the whole section of this atom lies inside the tile: nobody else writes T[cur][b][:]
           double2 *d2 = reinterpret_cast<double2 *>(dst);
           d2[0] = make_double2(a0, a1);
           d2[1] = make_double2(a2, a3);
@@ -421,6 +432,7 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
              tp[1]-tp[0], tp[2]-tp[1], tp[3]-tp[2], tp[4]-tp[3], tp[5]-tp[4], tp[6]-tp[5], tp[7]-tp[6], tp[8]-tp[7], tp[9]-tp[8], tp[10]-tp[9]);
 #endif
   }
+  }                                                         // nets
   tc::fence_before_sync();
   __syncthreads();
   if (warp == 0) tc::tmem_dealloc<512>(tmem);
@@ -438,13 +450,8 @@ static cudaError_t run_pass1_tc(const DevModel &P, const ChunkView &C, const TCW
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  for (int a = 0; a < P.ntypes; ++a)
-    for (int t = 0; t < P.ntypes; ++t) {
-      k_pass1_tc<S1><<<g_tc_sms, 256, L::smem_bytes, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride,
-                                                          off + (size_t)t * (C.n + 1), pidx + (size_t)C.n * P.sec_start[t],
-                                                          a, t);
-      DPB_LAUNCHED(1);
-    }
+  k_pass1_tc<S1><<<g_tc_sms, 256, L::smem_bytes, st>>>(P, C, W.emb, W.net_stride, off, pidx);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
@@ -478,9 +485,9 @@ cudaError_t tc_pass1(const DevModel &P, const ChunkView &C, const TCWeights &W, 
 
 template <int S1>
 __global__ void __launch_bounds__(256, 1)
-k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int *__restrict__ off_t,
-           const int *__restrict__ pidx_t, const float *__restrict__ dT32, int a, int t, double *__restrict__ force,
-           double *__restrict__ virial) {
+k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t net_stride,
+           const int *__restrict__ off_all, const int *__restrict__ pidx_all, const float *__restrict__ dT32,
+           double *__restrict__ force, double *__restrict__ virial) {
   using L = TL<S1>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const int tid = threadIdx.x, wg = tid >> 7, wt = tid & 127, warp = tid >> 5, lane = tid & 31;
@@ -490,8 +497,6 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::oTmem);
   double *vred = reinterpret_cast<double *>(smem + L::oEnv);           // [8 warps][9], used after the tile loop
 
-  for (int k = tid; k < L::img_bytes / 16; k += 256)
-    reinterpret_cast<int4 *>(smem)[k] = reinterpret_cast<const int4 *>(net_img)[k];
   if (warp == 0) tc::tmem_alloc<512>(tmem_slot);
   if (tid == 0) {
     tc::mbar_init(reinterpret_cast<uint64_t *>(smem + L::oBar), 1);
@@ -508,14 +513,27 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
   const uint32_t slot_a = tc::smem_u32(slot), img_a = tc::smem_u32(smem);
   const uint32_t rowbase = (uint32_t)(wt >> 3) * 1024u + (uint32_t)(wt & 7) * 128u, r7 = wt & 7;
 
+  double vir[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+  // one launch walks all ntypes^2 nets (a = centre type, t = neighbour type): the CTA reloads the weight image at a net
+  // switch, so only the last net has a tail in which SMs idle (four launches per pass had four)
+  uint32_t phase = 0;
+  for (int net = 0; net < P.ntypes * P.ntypes; ++net) {
+  const int a = net / P.ntypes, t = net - a * P.ntypes;
+  const int *off_t = off_all + (size_t)t * (C.n + 1), *pidx_t = pidx_all + (size_t)C.n * P.sec_start[t];
+  __syncthreads();                                          // every MMA that read the previous image has completed
+  {
+    const float *net_img = all_img + (size_t)net * net_stride;
+    for (int k = tid; k < L::img_bytes / 16; k += 256)
+      reinterpret_cast<int4 *>(smem)[k] = reinterpret_cast<const int4 *>(net_img)[k];
+  }
+  tc::fence_proxy_async();
+  __syncthreads();
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
   int flat0 = 0, flat1 = 0;
   if (row_hi > row_lo) { flat0 = off_t[row_lo]; flat1 = off_t[row_hi]; }
   const int ntiles = (flat1 - flat0 + 127) >> 7;
-  uint32_t phase = 0;
-  double vir[9];
-#pragma unroll
-  for (int k = 0; k < 9; ++k) vir[k] = 0.0;
 
   int nx_idx = 0;
   double4 nx_dv = make_double4(0.0, 0.0, 0.0, 1.0);
@@ -713,6 +731,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ net_img, const int
       }
     }
   }
+  }                                                         // nets
   // virial: warp -> block -> one atomic per component and CTA
 #pragma unroll
   for (int k = 0; k < 9; ++k) {
@@ -743,13 +762,8 @@ static cudaError_t run_pass2_tc(const DevModel &P, const ChunkView &C, const TCW
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  for (int a = 0; a < P.ntypes; ++a)
-    for (int t = 0; t < P.ntypes; ++t) {
-      k_pass2_tc<S1><<<g_tc_sms, 256, L::smem_bytes, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride,
-                                                          off + (size_t)t * (C.n + 1), pidx + (size_t)C.n * P.sec_start[t],
-                                                          dT32, a, t, force, virial);
-      DPB_LAUNCHED(1);
-    }
+  k_pass2_tc<S1><<<g_tc_sms, 256, L::smem_bytes, st>>>(P, C, W.emb, W.net_stride, off, pidx, dT32, force, virial);
+  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
