@@ -208,7 +208,8 @@ def run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed):
                       "rebuilds": info["n_rebuilds"], "max_displacement_A": info["max_displacement"],
                       "skin_violated": info["skin_violated"],
                       "etot_drift_rel_to_ekin": float(np.abs(etot - etot[0]).max() / thermo[0, 1]),
-                      "T_first_last_K": [float(thermo[0, 2]), float(thermo[-1, 2])]}
+                      "T_first_last_K": [float(thermo[0, 2]), float(thermo[-1, 2])],
+                      "P_first_last_bar": [float(thermo[0, 3]), float(thermo[-1, 3])]}
     model.close()
     out["weights"] = "conditioned (fitting W0 / Nm)"
     return out

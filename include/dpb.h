@@ -136,7 +136,8 @@ int dpb_model_stage_us(const dpb_model *model, float stage_us[8]);
 
 /* ---- molecular dynamics with the DP forces ---------------------------------
  * Velocity-Verlet, NVE: v += (dt/2) F/m; x += dt v; F = F(x); v += (dt/2) F/m.  Units: Angstrom, fs, amu, eV
- * (1 amu A^2/fs^2 = 103.6426965268 eV; T = 2 E_kin / (3 N k_B), k_B = 8.617333262e-5 eV/K).
+ * (1 amu A^2/fs^2 = 103.6426965268 eV; T = 2 E_kin / (3 N k_B), k_B = 8.617333262e-5 eV/K; pressure from the virial
+ * theorem, P = (2 E_kin + tr Xi) / (3 V), 1 eV/A^3 = 1.602176634e6 bar — the thermo quantities of PAPER.md:298).
  * Neighbour reuse (2 A skin, rebuilt every 50 steps): with rebuild_every > 1 the cell search runs
  * over r_c + skin every rebuild_every steps and stores a raw list; the steps in between format that raw list (Alg. 1).
  * The formatted list equals a fresh search as long as no atom moves more than skin / 2 between rebuilds
@@ -159,7 +160,7 @@ typedef struct {
 } dpb_md_info;
 
 /* coord DEVICE fp64 [N][3] and vel DEVICE fp64 [N][3] (A/fs) are updated in place; type DEVICE int32 [N]; mass HOST
- * [ntypes] (amu); box HOST [9]; thermo HOST [nsteps / thermo_every + 1][3] = (E_pot, E_kin, T) or NULL; info HOST or
+ * [ntypes] (amu); box HOST [9]; thermo HOST [nsteps / thermo_every + 1][4] = (E_pot [eV], E_kin [eV], T [K], P [bar]) or NULL; info HOST or
  * NULL.  All work is enqueued on `stream`; the call returns after the stream has been synchronised.  The model must
  * not be used by another call while the run is in flight.  Errors as dpb_eval. */
 int dpb_md_run(dpb_model *model, void *stream, int64_t natoms, double *coord, double *vel, const int32_t *type,

@@ -594,9 +594,12 @@ done:
  * every 50 steps, gives the same list as long as no atom moves more than half the skin).
  * Units: Angstrom, fs, amu, eV:  1 amu A^2/fs^2 = 103.6426965268 eV (CODATA 2018: 1.66053906660e-27 kg x 1e10 m^2/s^2 / 1.602176634e-19 C),
  * k_B = 8.617333262e-5 eV/K, T = 2 E_kin / (3 N k_B).  Coordinates are not wrapped (reading R2 takes raw values).
- * thermo[k][3] = (E_pot, E_kin, T) at steps 0, thermo_every, 2 thermo_every, ... <= nsteps. */
+ * thermo[k][4] = (E_pot, E_kin, T, P) at steps 0, thermo_every, 2 thermo_every, ... <= nsteps ("kinetic
+ * energy, potential energy, temperature, pressure ... every 20 time steps").  Pressure from the virial theorem,
+ * P = (2 E_kin + tr Xi) / (3 V) with Xi = -sum d_ik (x) dE_i/dd_ik (reading R14), in bar: 1 eV/A^3 = 1.602176634e6 bar. */
 #define DPO_AMU_A2_FS2_IN_EV 103.6426965268
 #define DPO_KB_EV 8.617333262e-5
+#define DPO_EV_A3_IN_BAR 1.602176634e6
 
 int dpo_md_run(const dpo_model_desc *m, int64_t natoms, double *coord, double *vel, const int32_t *type,
                const double *mass, const double box[9], double dt_fs, int64_t nsteps, int64_t thermo_every,
@@ -604,8 +607,9 @@ int dpo_md_run(const dpo_model_desc *m, int64_t natoms, double *coord, double *v
   if (natoms < 0 || nsteps < 0 || !(dt_fs > 0.0) || thermo_every < 1) return DPO_EINVAL;
   double *force = (double *)malloc((size_t)(natoms > 0 ? natoms : 1) * 3 * sizeof(double));
   if (!force) return DPO_ENOMEM;
-  double epot = 0.0;
-  int rc = dpo_eval(m, natoms, coord, type, box, &epot, NULL, force, NULL, NULL, use_cells);
+  double epot = 0.0, vir[9];
+  const double volume = box[0] * box[4] * box[8];
+  int rc = dpo_eval(m, natoms, coord, type, box, &epot, NULL, force, vir, NULL, use_cells);
   int64_t nt = 0;
   for (int64_t step = 0; rc == DPO_OK; ++step) {
     if (step % thermo_every == 0 && thermo) {
@@ -615,9 +619,10 @@ int dpo_md_run(const dpo_model_desc *m, int64_t natoms, double *coord, double *v
         ek += 0.5 * mass[type[i]] * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
       }
       ek *= DPO_AMU_A2_FS2_IN_EV;
-      thermo[3 * nt + 0] = epot;
-      thermo[3 * nt + 1] = ek;
-      thermo[3 * nt + 2] = natoms > 0 ? 2.0 * ek / (3.0 * (double)natoms * DPO_KB_EV) : 0.0;
+      thermo[4 * nt + 0] = epot;
+      thermo[4 * nt + 1] = ek;
+      thermo[4 * nt + 2] = natoms > 0 ? 2.0 * ek / (3.0 * (double)natoms * DPO_KB_EV) : 0.0;
+      thermo[4 * nt + 3] = (2.0 * ek + vir[0] + vir[4] + vir[8]) / (3.0 * volume) * DPO_EV_A3_IN_BAR;
       ++nt;
     }
     if (step == nsteps) break;
@@ -628,7 +633,7 @@ int dpo_md_run(const dpo_model_desc *m, int64_t natoms, double *coord, double *v
         coord[3 * i + c] += dt_fs * vel[3 * i + c];
       }
     }
-    rc = dpo_eval(m, natoms, coord, type, box, &epot, NULL, force, NULL, NULL, use_cells);
+    rc = dpo_eval(m, natoms, coord, type, box, &epot, NULL, force, vir, NULL, use_cells);
     if (rc != DPO_OK) break;
     for (int64_t i = 0; i < natoms; ++i) {
       const double h = 0.5 * dt_fs / (mass[type[i]] * DPO_AMU_A2_FS2_IN_EV);

@@ -82,8 +82,8 @@ int dpo_eval(const dpo_model_desc *m, int64_t natoms, const double *coord, const
              int32_t *nlist_out, int use_cells);
 
 /* NEXT #1: velocity-Verlet NVE molecular dynamics with the DP forces.
- * coord [N][3] (A) and vel [N][3] (A/fs) are updated in place; mass[ntypes] in amu; thermo [nsteps / thermo_every + 1][3]
- * = (E_pot, E_kin, T) at steps 0, thermo_every, ... (may be NULL).  Neighbours are searched from scratch every step. */
+ * coord [N][3] (A) and vel [N][3] (A/fs) are updated in place; mass[ntypes] in amu; thermo [nsteps / thermo_every + 1][4]
+ * = (E_pot [eV], E_kin [eV], T [K], P [bar]) at steps 0, thermo_every, ... (may be NULL).  Neighbours are searched from scratch every step. */
 int dpo_md_run(const dpo_model_desc *m, int64_t natoms, double *coord, double *vel, const int32_t *type,
                const double *mass, const double box[9], double dt_fs, int64_t nsteps, int64_t thermo_every,
                double *thermo, int use_cells);

@@ -167,13 +167,13 @@ class Oracle:
         return out
 
     def md_run(self, coord, vel, types, mass, box, dt_fs, nsteps, thermo_every=1, cells=False):
-        """Velocity-Verlet NVE MD (dpo_md_run).  Returns (coord, vel, thermo[k][3] = (E_pot, E_kin, T))."""
+        """Velocity-Verlet NVE MD (dpo_md_run).  Returns (coord, vel, thermo[k][4] = (E_pot, E_kin, T, P [bar]))."""
         coord, types, box = self._inputs(coord, types, box)
         coord = coord.copy()
         vel = np.ascontiguousarray(vel, dtype=np.float64).reshape(-1, 3).copy()
         mass = np.ascontiguousarray(mass, dtype=np.float64)
         nt = nsteps // thermo_every + 1
-        thermo = np.zeros((nt, 3))
+        thermo = np.zeros((nt, 4))
         rc = self.lib.dpo_md_run(C.byref(self.desc), C.c_int64(coord.shape[0]), _d(coord), _d(vel), _i(types),
                                  _d(mass), _d(box), C.c_double(dt_fs), C.c_int64(nsteps), C.c_int64(thermo_every),
                                  _d(thermo), C.c_int(1 if cells else 0))

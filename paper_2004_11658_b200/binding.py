@@ -240,7 +240,7 @@ class DPModel:
 
     def md_run(self, coord, vel, types, mass, box, dt_fs, nsteps, thermo_every=1, rebuild_every=1, skin=0.0):
         """dpb_md_run: velocity-Verlet NVE on torch CUDA tensors coord / vel (float64 [N,3], updated IN PLACE).
-        Returns (thermo numpy [k][3] = (E_pot, E_kin, T), info dict)."""
+        Returns (thermo numpy [k][4] = (E_pot, E_kin, T, P [bar]), info dict)."""
         torch = _torch()
         assert coord.is_cuda and coord.dtype == torch.float64 and coord.is_contiguous()
         assert vel.is_cuda and vel.dtype == torch.float64 and vel.is_contiguous()
@@ -249,7 +249,7 @@ class DPModel:
         b, bp = self._box(box)
         m = np.ascontiguousarray(mass, dtype=np.float64)
         prm = _MDParams(float(dt_fs), int(nsteps), int(thermo_every), int(rebuild_every), 0, float(skin))
-        thermo = np.zeros((nsteps // thermo_every + 1, 3))
+        thermo = np.zeros((nsteps // thermo_every + 1, 4))
         info = _MDInfo()
         rc = self.lib.dpb_md_run(self._h, self._stream(), n, C.c_void_p(coord.data_ptr()), C.c_void_p(vel.data_ptr()),
                                  C.c_void_p(types.data_ptr()), m.ctypes.data_as(C.POINTER(C.c_double)), bp,

@@ -506,7 +506,7 @@ extern "C" int dpb_md_run(dpb_model *m, void *stream, int64_t natoms, double *co
     hm[DPB_MAX_TYPES + t] = mass_h[t] * AMU;
   }
   CU(m->md_force.reserve(sizeof(double) * 3 * (n + 1)), "md workspace");
-  CU(m->md_scal.reserve(sizeof(double) * (2 + 3 * (size_t)nth)), "md workspace");
+  CU(m->md_scal.reserve(sizeof(double) * (12 + 4 * (size_t)nth)), "md workspace");
   CU(m->md_mass.reserve(sizeof(double) * 2 * DPB_MAX_TYPES), "md workspace");
   CU(cudaMemcpyAsync(m->md_mass.p, hm.data(), sizeof(double) * 2 * DPB_MAX_TYPES, cudaMemcpyHostToDevice, st), "H2D masses");
   if (reuse) {
@@ -519,7 +519,8 @@ extern "C" int dpb_md_run(dpb_model *m, void *stream, int64_t natoms, double *co
     CU(m->md_nraw.reserve(sizeof(int) * (n + 1)), "md skin list");
     CU(m->md_xyz0.reserve(sizeof(double) * 3 * (n + 1)), "md skin list");
   }
-  double *force = m->md_force.as<double>(), *epot = m->md_scal.as<double>(), *thermo = epot + 2;
+  double *force = m->md_force.as<double>(), *epot = m->md_scal.as<double>(), *vir = epot + 2, *thermo = epot + 12;
+  const double volume = box[0] * box[4] * box[8];
   const double *d_hm = m->md_mass.as<double>(), *d_mev = d_hm + DPB_MAX_TYPES;
   CU(cudaMemsetAsync(m->stats.p, 0, sizeof(DevStats), st), "memset stats");
   int rebuilds = 0;
@@ -527,20 +528,20 @@ extern "C" int dpb_md_run(dpb_model *m, void *stream, int64_t natoms, double *co
     int mode = 0;
     if (reuse) { mode = (step % prm->rebuild_every == 0) ? 1 : 2; rebuilds += mode == 1; }
     else CU(cudaMemsetAsync(m->stats.p, 0, sizeof(DevStats), st), "memset stats");
-    return run_eval(m, st, natoms, coord, type, box, epot, nullptr, force, nullptr, nullptr, false, mode);
+    return run_eval(m, st, natoms, coord, type, box, epot, nullptr, force, vir, nullptr, false, mode);
   };
   int rc = eval(0);
   if (rc != DPB_OK) return rc;
   int slot = 0;
   for (int step = 0;; ++step) {
-    if (step % prm->thermo_every == 0) CU(launch_md_thermo(natoms, vel, type, d_mev, epot, thermo, slot++, st), "thermo");
+    if (step % prm->thermo_every == 0) CU(launch_md_thermo(natoms, vel, type, d_mev, epot, vir, volume, thermo, slot++, st), "thermo");
     if (step == prm->nsteps) break;
     CU(launch_md_kick_drift(natoms, coord, vel, force, type, d_hm, prm->dt_fs, st), "kick + drift");
     rc = eval(step + 1);
     if (rc != DPB_OK) return rc;
     CU(launch_md_kick(natoms, vel, force, type, d_hm, st), "kick");
   }
-  if (thermo_h) CU(cudaMemcpyAsync(thermo_h, thermo, sizeof(double) * 3 * (size_t)nth, cudaMemcpyDeviceToHost, st), "D2H thermo");
+  if (thermo_h) CU(cudaMemcpyAsync(thermo_h, thermo, sizeof(double) * 4 * (size_t)nth, cudaMemcpyDeviceToHost, st), "D2H thermo");
   DevStats hs;
   CU(cudaMemcpyAsync(&hs, m->stats.p, sizeof(DevStats), cudaMemcpyDeviceToHost, st), "stats copy");
   CU(cudaStreamSynchronize(st), "stream synchronise");

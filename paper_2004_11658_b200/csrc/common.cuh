@@ -95,7 +95,7 @@ cudaError_t launch_md_kick_drift(int64_t n, double *coord, double *vel, const do
 cudaError_t launch_md_kick(int64_t n, double *vel, const double *force, const int *type, const double *hm,
                            cudaStream_t st);
 cudaError_t launch_md_thermo(int64_t n, const double *vel, const int *type, const double *mass_ev, const double *epot,
-                             double *thermo, int slot, cudaStream_t st);
+                             const double *virial, double volume, double *thermo, int slot, cudaStream_t st);
 
 // ---- device helpers ---------------------------------------------------------------------------------------
 #ifdef __CUDACC__

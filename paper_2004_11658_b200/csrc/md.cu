@@ -21,10 +21,10 @@ __global__ void k_md_kick(int n, double *__restrict__ vel, const double *__restr
   vel[k] = fma(hm[type[k / 3]], force[k], vel[k]);
 }
 
-// thermo[slot] = (E_pot, E_kin, T): fixed-order reduction by one block
+// thermo[slot] = (E_pot, E_kin, T, P [bar]): fixed-order reduction by one block; P = (2 E_kin + tr Xi) / (3 V)
 __global__ void k_md_thermo(int n, const double *__restrict__ vel, const int *__restrict__ type,
                             const double *__restrict__ mass_ev, const double *__restrict__ epot,
-                            double *__restrict__ thermo, int slot) {
+                            const double *__restrict__ virial, double volume, double *__restrict__ thermo, int slot) {
   __shared__ double part[1024];
   double s = 0.0;
   for (int i = threadIdx.x; i < n; i += 1024) {
@@ -39,9 +39,10 @@ __global__ void k_md_thermo(int n, const double *__restrict__ vel, const int *__
   }
   if (threadIdx.x == 0) {
     const double ek = part[0];
-    thermo[3 * slot + 0] = *epot;
-    thermo[3 * slot + 1] = ek;
-    thermo[3 * slot + 2] = n > 0 ? 2.0 * ek / (3.0 * (double)n * 8.617333262e-5) : 0.0;
+    thermo[4 * slot + 0] = *epot;
+    thermo[4 * slot + 1] = ek;
+    thermo[4 * slot + 2] = n > 0 ? 2.0 * ek / (3.0 * (double)n * 8.617333262e-5) : 0.0;
+    thermo[4 * slot + 3] = (2.0 * ek + virial[0] + virial[4] + virial[8]) / (3.0 * volume) * 1.602176634e6;
   }
 }
 
@@ -62,8 +63,8 @@ cudaError_t launch_md_kick(int64_t n, double *vel, const double *force, const in
 }
 
 cudaError_t launch_md_thermo(int64_t n, const double *vel, const int *type, const double *mass_ev, const double *epot,
-                             double *thermo, int slot, cudaStream_t st) {
-  k_md_thermo<<<1, 1024, 0, st>>>((int)n, vel, type, mass_ev, epot, thermo, slot);
+                             const double *virial, double volume, double *thermo, int slot, cudaStream_t st) {
+  k_md_thermo<<<1, 1024, 0, st>>>((int)n, vel, type, mass_ev, epot, virial, volume, thermo, slot);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }

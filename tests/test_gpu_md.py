@@ -50,6 +50,7 @@ def test_md_trajectory_matches_oracle():
     assert np.abs(th[:, 0] - tr[:, 0]).max() <= 1e-10 * np.abs(tr[:, 0]).max()
     assert np.abs(th[:, 1] - tr[:, 1]).max() <= 1e-10 * np.abs(tr[:, 1]).max()
     assert abs(th[0, 2] - 330.0) < 1e-6
+    assert np.abs(th[:, 3] - tr[:, 3]).max() <= 1e-9 * np.abs(tr[:, 3]).max()        # pressure (bar)
 
 
 def test_md_energy_conservation_and_order():

@@ -90,3 +90,29 @@ def test_one_step_against_hand_written_update():
     v1 = vh + 0.5 * dt * f1 / m
     x, v, th = o.md_run(coord, vel, types, MASS2, box, dt, 1)
     assert np.abs(x - x1).max() < 1e-13 and np.abs(v - v1).max() < 1e-13
+
+
+def test_pressure_ideal_gas_and_virial_part():
+    """thermo column 3 = P in bar (PAPER.md:298 lists the pressure among the thermo data).  Zero-force model: the ideal
+    gas law P V = N k_B T with CODATA constants (1 eV/A^3 = e / 1e-30 m^3 = 1.602176634e11 Pa).  Atoms at rest: the
+    virial part alone, P = -dE/dV, by central differences of the oracle's energy under an isotropic scaling."""
+    spec, emb, fit, coord, types, box, vel = _setup()
+    from gen.weights import fit_net_size
+    per = fit_net_size(spec.dim_descrpt, spec.fit_width)
+    fit0 = np.zeros_like(fit)
+    fit0[per - 1] = 0.3
+    o0 = Oracle.from_spec(spec, np.zeros_like(emb), fit0)
+    _, _, th = o0.md_run(coord, vel, types, MASS2, box, 0.5, 0)
+    V = box[0] * box[4] * box[8]
+    p_ideal = len(types) * (1.380649e-23 / 1.602176634e-19) * 330.0 / V * (1.602176634e-19 / 1e-30 / 1e5)
+    assert abs(th[0, 3] - p_ideal) < 1e-9 * p_ideal
+
+    o = Oracle.from_spec(spec, emb, fit)
+    _, _, th = o.md_run(coord, np.zeros_like(vel), types, MASS2, box, 0.5, 0)
+    h = 1e-5
+    e = []
+    for s in (1 + h, 1 - h):
+        e.append(o.eval(coord * s, types, box * s)["energy"])
+    dEdV = (e[0] - e[1]) / (V * ((1 + h) ** 3 - (1 - h) ** 3))
+    p_fd = -dEdV * 1.602176634e6
+    assert abs(th[0, 3] - p_fd) < 1e-6 * max(1.0, abs(p_fd)), (th[0, 3], p_fd)
