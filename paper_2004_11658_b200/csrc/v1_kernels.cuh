@@ -26,16 +26,15 @@ cudaError_t v1_pass2(const DevModel &P, const ChunkView &C, const V1Weights &W, 
 #ifdef __CUDACC__
 // tanh(x) = 1 - 2 / (exp(2x) + 1) with exp(2x) = 2^n 2^f: n = rint(2x log2 e) by the 1.5 * 2^52 trick, 2^f by a
 // degree-10 polynomial on [-0.5, 0.5] (relative error 2.9e-16), the reciprocal from MUFU.RCP64H refined by one cubic
-// step.  19 fp64-pipe instructions; absolute error <= 4.5e-16 against libdevice on [-25, 25], [-1, 1], [-0.01, 0.01]
+// step.  18 fp64-pipe instructions; absolute error <= 4.5e-16 against libdevice on [-25, 25], [-1, 1], [-0.01, 0.01]
 // and [-1e-6, 1e-6] (4e7 points each, profiles/r1_fp64_peaks.md); libdevice's tanh costs 2.2x the pipe slots.
 __device__ __forceinline__ double dp_tanh(double x) {
   const int hi = __double2hiint(x);
   const bool big = (hi & 0x7fffffff) >= 0x40340000;                 // |x| >= 20: tanh = +-1 in fp64
   const double xc = big ? __hiloint2double((hi & 0x80000000) | 0x40340000, 0) : x;
-  const double t = xc * 2.8853900817779268;                          // 2 log2(e)
-  const double tm = t + 6755399441055744.0;                          // 1.5 * 2^52
+  const double tm = fma(xc, 2.8853900817779268, 6755399441055744.0); // 2 log2(e) x + 1.5 * 2^52
   const int ni = __double2loint(tm);
-  const double f = t - (tm - 6755399441055744.0);
+  const double f = fma(xc, 2.8853900817779268, 6755399441055744.0 - tm);   // t - rint(t), one rounding
   double p = 7.0725859492692236999e-9;
   p = fma(p, f, 1.0208690299958305835e-7);
   p = fma(p, f, 1.3215442587921689653e-6);
