@@ -34,7 +34,7 @@ struct FitTCNet {                      // device pointers (floats) of one specie
 struct FitTC {
   float *buf = nullptr;
   int fw = 0, fwp = 0, NT = 0;         // width, width padded to 32 (K panels), N tile of the fw-wide GEMMs
-  int dim = 0, dimp = 0, NT6 = 0;      // descriptor size, padded to 128; N tile of G6
+  int dim = 0, dimp = 0, NT6 = 0;      // descriptor size, padded to the N tile of G6 (240: fewer re-reads of A than 128)
   std::vector<FitTCNet> nets;
 };
 
@@ -417,8 +417,9 @@ cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W)
   if (P.fw % 4 != 0 || ft_pick_nt(P.fw) == 0 || (P.Ma != 4 && P.Ma != 8 && P.Ma != 16)) return cudaErrorNotSupported;
   FitTC *F = new FitTC();
   F->fw = P.fw; F->fwp = ft_round_up(P.fw, 32); F->NT = ft_pick_nt(P.fw);
-  F->dim = P.dim; F->dimp = ft_round_up(P.dim, 128); F->NT6 = 128;
-  const int fw = P.fw, dim = P.dim, kpw = F->fwp / 32, kpd = ft_round_up(dim, 32) / 32, nt6 = F->dimp / 128;
+  F->NT6 = P.dim >= 960 ? 240 : 128;
+  F->dim = P.dim; F->dimp = ft_round_up(P.dim, F->NT6);
+  const int fw = P.fw, dim = P.dim, kpw = F->fwp / 32, kpd = ft_round_up(dim, 32) / 32, nt6 = F->dimp / F->NT6;
   std::vector<float> h;
   struct Off { size_t W0h, W0l, W1h, W1l, W2h, W2l, W2Th, W2Tl, W1Th, W1Tl, W0Th, W0Tl, b0, b1, b2, w3; };
   std::vector<Off> offs(P.ntypes);
@@ -434,7 +435,7 @@ cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W)
     // backward GEMMs: C[r][n] = sum_k Q[r][k] W[n][k]  ->  B[n][k] = W[n][k]
     pack_B([&](int n, int k) { return W2[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W2Th, o.W2Tl);
     pack_B([&](int n, int k) { return W1[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W1Th, o.W1Tl);
-    pack_B([&](int n, int k) { return W0[(size_t)n * fw + k]; }, dim, fw, 128, nt6, kpw, h, o.W0Th, o.W0Tl);
+    pack_B([&](int n, int k) { return W0[(size_t)n * fw + k]; }, dim, fw, F->NT6, nt6, kpw, h, o.W0Th, o.W0Tl);
     auto vecpad = [&](const double *src) {
       const size_t at = h.size();
       h.resize(at + 256, 0.0f);
@@ -470,7 +471,7 @@ void tc_release_fit(TCWeights &W) {
 
 size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk) {
   const size_t tiles = (size_t)(chunk + 127) / 128, rows = tiles * 128;
-  const size_t kpd = (size_t)ft_round_up(P.dim, 32) / 32, fwp = ft_round_up(P.fw, 32), dimp = ft_round_up(P.dim, 128);
+  const size_t kpd = (size_t)ft_round_up(P.dim, 32) / 32, fwp = ft_round_up(P.fw, 32), dimp = ft_round_up(P.dim, P.dim >= 960 ? 240 : 128);
   return sizeof(float) * (2 * tiles * kpd * 4096 + 4 * tiles * (fwp / 32) * 4096 + 5 * rows * fwp + rows * dimp) + 1024;
 }
 
@@ -523,6 +524,7 @@ static cudaError_t ft_run_type(const DevModel &P, const ChunkView &C, const FitT
   // G6: dD = Q0 W0^T
   g.Ah = X0h; g.Al = X0l; g.Bh = N.W0Th; g.Bl = N.W0Tl; g.N = F.dim; g.ldp = F.dimp; g.KPAN_out = 0;
   g.out_plain0 = dD; g.out_h = nullptr; g.out_l = nullptr; g.in0 = nullptr; g.in1 = nullptr;
+  if (F.NT6 == 240) return ft_launch<240, FE_STORE>(C, ty, g, F.dimp / 240, st);
   return ft_launch<128, FE_STORE>(C, ty, g, F.dimp / 128, st);
 }
 
