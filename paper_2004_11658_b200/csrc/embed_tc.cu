@@ -496,6 +496,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + L::oBar) + wg;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::oTmem);
   double *vred = reinterpret_cast<double *>(smem + L::oEnv);           // [8 warps][9], used after the tile loop
+  int *ids = reinterpret_cast<int *>(smem + L::oIds) + wg * 256;       // centre atom of every tile row
 
   if (warp == 0) tc::tmem_alloc<512>(tmem_slot);
   if (tid == 0) {
@@ -548,6 +549,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     const int idx = nx_idx;
     const double4 dv = nx_dv;
     const int qa = valid ? idx / P.nm : -1;
+    ids[wt] = qa;
     double ed[4] = {0.0, 0.0, 0.0, 0.0};
     if (valid) env_row4_tc(P, dv, ed);
     const float e0 = (float)ed[0], e1 = (float)ed[1], e2 = (float)ed[2], e3 = (float)ed[3];
@@ -657,9 +659,24 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     tc::mbar_wait(mbar, phase);
     phase ^= 1;
     tc::fence_after_sync();
+    // The operand slot is free again (the tangent MMAs have completed): stage the dT rows of the tile's centre atoms in
+    // it (coalesced), so that the epilogue reads them from shared memory — with 221 KB of shared memory in use the L1
+    // holds almost nothing and the per-feature global loads were the largest phase of the tile.
+    const float4 *dT4 = reinterpret_cast<const float4 *>(dT32);
+    float4 *stage = reinterpret_cast<float4 *>(slot);
+    constexpr int CAP_AT = L::SLOT / (4 * S1 * 16);            // atoms whose rows fit the slot
+    const int nrows_t = min(128, flat1 - (flat0 + tile * 128));
+    const int qa0 = ids[0];
+    const int nat = min(ids[nrows_t - 1] - qa0 + 1, CAP_AT);
+    {
+      const float4 *src = dT4 + (size_t)qa0 * P.M;
+      for (int k = wt; k < nat * 4 * S1; k += 128) stage[k] = src[k];
+    }
+    tc::bar_sync(1 + wg, 128);
     // epilogue: g = (h1, h1) + t2, g' = (h1', h1') + (1 - t2^2) (h1' W2); dots with the atom's dT rows
     float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f, pr3 = 0.f, dx = 0.f;
-    const float4 *dTrow = reinterpret_cast<const float4 *>(dT32) + (size_t)(valid ? qa : 0) * P.M;
+    const bool staged = valid && qa - qa0 < nat;
+    const float4 *dTrow = staged ? stage + (qa - qa0) * (4 * S1) : dT4 + (size_t)(valid ? qa : 0) * P.M;
     {
       constexpr int CH = 16, NCH = (4 * S1 + CH - 1) / CH;
 #pragma unroll
@@ -683,7 +700,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
             tc::tanh_d_f32(__uint_as_float(v[i]) + vec[L::vb2 + o], t2, d2);
             const float gv = h1v[o % (2 * S1)] + t2;
             const float gp = fmaf(d2, __uint_as_float(w[i]), h1t[o % (2 * S1)]);
-            const float4 d4 = __ldg(dTrow + o);
+            const float4 d4 = dTrow[o];
             pr0 = fmaf(d4.x, gv, pr0); pr1 = fmaf(d4.y, gv, pr1); pr2 = fmaf(d4.z, gv, pr2); pr3 = fmaf(d4.w, gv, pr3);
             const float dg = fmaf(d4.x, e0, fmaf(d4.y, e1, fmaf(d4.z, e2, d4.w * e3)));
             dx = fmaf(dg, gp, dx);
@@ -692,6 +709,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       }
     }
     tc::fence_before_sync();                                // TMEM reads done before the next tile's MMAs overwrite
+    tc::bar_sync(1 + wg, 128);                              // ... and the staged dT rows before the next tile's operands
     // O10 / O11 in fp64: f_ik = sum_m dR~[m] dR~_m/dd; F_j -= f, F_i += f, Xi -= d (x) f
     double f0 = 0.0, f1 = 0.0, f2 = 0.0;
     if (valid) {
