@@ -68,6 +68,9 @@ __device__ __forceinline__ void img_store4(float *img_h, float *img_l, size_t ti
 }
 
 // One group of 8 output columns of row m (tile row r): apply the GEMM's epilogue to the accumulators a[8].
+// The plain fp32 activation arrays (Z0, S0, S1, Z1, dZ1) are private to these epilogues, which all map thread r to tile
+// row r; they are stored tile-wise transposed, [tile][column / 4][row][4], so that the 32 lanes of a warp (32 rows) touch
+// 512 contiguous bytes per access instead of 32 separate lines.  dD (FE_STORE) stays row-major for k_dT_tc.
 template <int EPI>
 __device__ __forceinline__ void ft_epi8(const float a[8], int nn0, const FitTCArgs &g, size_t tile, int r, int m,
                                         double &edot) {
@@ -77,12 +80,13 @@ __device__ __forceinline__ void ft_epi8(const float a[8], int nn0, const FitTCAr
     const int nn = nn0 + 4 * q4;
     const bool live = nn < g.N;
     float4 bias = make_float4(0.f, 0.f, 0.f, 0.f), w3 = bias, i0 = bias, i1 = bias;
+    const size_t pt = ((tile * (size_t)(g.ldp >> 2) + (size_t)(nn >> 2)) * 128 + (size_t)r) * 4;   // tiled offset
     if (live) {
       if (EPI == FE_TANH || EPI == FE_TANH_SKIP || EPI == FE_L3) bias = *reinterpret_cast<const float4 *>(g.bias + nn);
       if (EPI == FE_L3 || EPI == FE_BWD1) w3 = *reinterpret_cast<const float4 *>(g.w3 + nn);
       if (EPI == FE_TANH_SKIP || EPI == FE_L3 || EPI == FE_BWD0)
-        i0 = *reinterpret_cast<const float4 *>(g.in0 + (size_t)m * g.ldp + nn);
-      if (EPI == FE_BWD1 || EPI == FE_BWD0) i1 = *reinterpret_cast<const float4 *>(g.in1 + (size_t)m * g.ldp + nn);
+        i0 = *reinterpret_cast<const float4 *>(g.in0 + pt);
+      if (EPI == FE_BWD1 || EPI == FE_BWD0) i1 = *reinterpret_cast<const float4 *>(g.in1 + pt);
     }
     const float bb[4] = {bias.x, bias.y, bias.z, bias.w}, ww[4] = {w3.x, w3.y, w3.z, w3.w};
     const float x0[4] = {i0.x, i0.y, i0.z, i0.w}, x1[4] = {i1.x, i1.y, i1.z, i1.w};
@@ -122,12 +126,12 @@ __device__ __forceinline__ void ft_epi8(const float a[8], int nn0, const FitTCAr
     if (g.out_h && nn < g.KPAN_out * FT_KP)
       img_store4(g.out_h, g.out_l, tile, g.KPAN_out, nn, r, o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
     if (nn < g.ldp) {
+      const size_t po = EPI == FE_STORE ? (size_t)m * g.ldp + nn
+                                        : ((tile * (size_t)(g.ldp >> 2) + (size_t)(nn >> 2)) * 128 + (size_t)r) * 4;
       if (g.out_plain0)
-        *reinterpret_cast<float4 *>(g.out_plain0 + (size_t)m * g.ldp + nn) =
-            make_float4(o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
+        *reinterpret_cast<float4 *>(g.out_plain0 + po) = make_float4(o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
       if (g.out_plain1)
-        *reinterpret_cast<float4 *>(g.out_plain1 + (size_t)m * g.ldp + nn) =
-            make_float4(o1[4 * q4], o1[4 * q4 + 1], o1[4 * q4 + 2], o1[4 * q4 + 3]);
+        *reinterpret_cast<float4 *>(g.out_plain1 + po) = make_float4(o1[4 * q4], o1[4 * q4 + 1], o1[4 * q4 + 2], o1[4 * q4 + 3]);
     }
   }
 }
