@@ -218,7 +218,11 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
   __syncthreads();
   tc::fence_after_sync();
   const uint32_t tmem = *tmem_slot;
-  const uint32_t tD1 = tmem + wg * 256, tD2 = tD1 + 64;
+  // TMEM columns of this warpgroup: A1 hi [0,32) lo [32,64), D1 [64,128); then A2 hi [0,64) lo [64,128) over them (the
+  // layer-1 operands and accumulator are dead by then), D2 [128,256).  The A operands are written with tcgen05.st, one
+  // row per thread, and the MMA reads them from tensor memory: no swizzled stores, no proxy fence, and half of the
+  // shared-memory operand traffic of an SS-mode MMA.
+  const uint32_t tA = tmem + wg * 256, tD1 = tA + 64, tD2 = tA + 128;
   const uint32_t lane_sel = (uint32_t)(32 * (warp & 3)) << 16;
   const uint32_t slot_a = tc::smem_u32(slot), img_a = tc::smem_u32(smem);
   const uint32_t rowbase = (uint32_t)(wt >> 3) * 1024u + (uint32_t)(wt & 7) * 128u, r7 = wt & 7;
@@ -277,11 +281,17 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     float h0[32];
 #pragma unroll
     for (int s = 0; s < 32; ++s) h0[s] = s < S1 ? tc::tanh_prescaled_f32(fmaf(x, vec[L::sW0 + s], vec[L::sb0 + s])) : 0.0f;
+    {
+      uint32_t w[32];
 #pragma unroll
-    for (int j = 0; j < 2 * L::KS1; ++j)
-      store_split4(slot, slot + 16384, rowbase, r7, j, h0[4 * j], h0[4 * j + 1], h0[4 * j + 2], h0[4 * j + 3]);
+      for (int s = 0; s < 32; ++s) { float fh, fl; tc::split_tf32(h0[s], fh, fl); w[s] = __float_as_uint(fh); }
+      tc::tmem_st32_nowait(tA + lane_sel, w);
+#pragma unroll
+      for (int s = 0; s < 32; ++s) { float fh, fl; tc::split_tf32(h0[s], fh, fl); w[s] = __float_as_uint(fl); }
+      tc::tmem_st32_nowait(tA + lane_sel + 32, w);
+      tc::tmem_wait_st();
+    }
     TCP(1);
-    tc::fence_proxy_async();
     tc::fence_before_sync();
     tc::bar_sync(1 + wg, 128);
     TCP(2);
@@ -289,9 +299,12 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       tc::fence_after_sync();
       constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N1);
 #pragma unroll
-      for (int ks = 0; ks < L::KS1; ++ks)
-        mma3(tD1, slot_a + ks * 32, slot_a + 16384 + ks * 32, img_a + L::oW1h + ks * 32, img_a + L::oW1l + ks * 32, idesc,
-             ks == 0);
+      for (int ks = 0; ks < L::KS1; ++ks) {
+        const uint64_t dbh = tc::make_desc_sw128(img_a + L::oW1h + ks * 32), dbl = tc::make_desc_sw128(img_a + L::oW1l + ks * 32);
+        tc::mma_tf32_ts(tD1, tA + 32 + 8 * ks, dbh, idesc, ks == 0 ? 0u : 1u);
+        tc::mma_tf32_ts(tD1, tA + 8 * ks, dbl, idesc, 1u);
+        tc::mma_tf32_ts(tD1, tA + 8 * ks, dbh, idesc, 1u);
+      }
       tc::mma_commit(mbar);
     }
     tc::mbar_wait(mbar, phase);
@@ -308,15 +321,25 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       for (int o = 0; o < 2 * S1; ++o) h1[o] = h0[o % S1] + tc::tanh_prescaled_f32(fmaf(__uint_as_float(v[o]), TC_2LOG2E, vec[L::sb1 + o]));
     }
     TCP(4);
+    {
+      uint32_t w[32];
 #pragma unroll
-    for (int j = 0; j < 2 * L::KS2; ++j) {
-      const int pan = j >> 3;
-      auto H = [&](int o) { return o < 2 * S1 ? h1[o] : 0.0f; };
-      store_split4(slot + pan * 16384, slot + 32768 + pan * 16384, rowbase, r7, j & 7, H(4 * j), H(4 * j + 1), H(4 * j + 2),
-                   H(4 * j + 3));
+      for (int half = 0; half < (8 * L::KS2 > 32 ? 2 : 1); ++half) {
+#pragma unroll
+        for (int lo = 0; lo < 2; ++lo) {
+#pragma unroll
+          for (int s = 0; s < 32; ++s) {
+            const int o = 32 * half + s;
+            float fh, fl;
+            tc::split_tf32(o < 2 * S1 ? h1[o] : 0.0f, fh, fl);
+            w[s] = __float_as_uint(lo ? fl : fh);
+          }
+          tc::tmem_st32_nowait(tA + lane_sel + 64 * lo + 32 * half, w);
+        }
+      }
+      tc::tmem_wait_st();
     }
     TCP(5);
-    tc::fence_proxy_async();
     tc::fence_before_sync();
     tc::bar_sync(1 + wg, 128);
     if (wt == 0) {
@@ -324,8 +347,11 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N2);
 #pragma unroll
       for (int ks = 0; ks < L::KS2; ++ks) {
-        const uint32_t ao = (ks >> 2) * 16384 + (ks & 3) * 32, bo = (ks >> 2) * L::W2P + (ks & 3) * 32;
-        mma3(tD2, slot_a + ao, slot_a + 32768 + ao, img_a + L::oW2h + bo, img_a + L::oW2l + bo, idesc, ks == 0);
+        const uint32_t bo = (ks >> 2) * L::W2P + (ks & 3) * 32;
+        const uint64_t dbh = tc::make_desc_sw128(img_a + L::oW2h + bo), dbl = tc::make_desc_sw128(img_a + L::oW2l + bo);
+        tc::mma_tf32_ts(tD2, tA + 64 + 8 * ks, dbh, idesc, ks == 0 ? 0u : 1u);
+        tc::mma_tf32_ts(tD2, tA + 8 * ks, dbl, idesc, 1u);
+        tc::mma_tf32_ts(tD2, tA + 8 * ks, dbh, idesc, 1u);
       }
       tc::mma_commit(mbar);
     }
