@@ -586,6 +586,62 @@ done:
   return rc;
 }
 
+/* ---- NEXT #2 / #3: evaluation of one sub-region with explicit ghost atoms ------------
+ * The paper's parallel formulation: a sub-region owns its "local" atoms; the atoms of the
+ * neighbouring sub-regions (and the periodic images) that lie within r_c of it are present as explicit "ghost" atoms.
+ * Atoms 0 .. nloc-1 are local, nloc .. nall-1 are ghosts.  There is no box: every displacement is the plain difference
+ * r_j - r_i.  E = sum over LOCAL atoms of E_i; force[nall][3] = -dE/dr for local and ghost atoms alike (the ghost part
+ * is what the reverse exchange sends home: grad_{r_i} E_j != -grad_{r_j} E_i, so it cannot be dropped);
+ * virial = -sum over local i, slots k of d_ik (x) dE_i/dd_ik (reading R14).  Summed over the sub-regions of a periodic
+ * system these give E, F and the virial of dpo_eval on the whole box: that identity is the pin (tests/test_oracle_local.py).
+ * Implementation: dpo_displacement with box edges of 1e300 A, for which k = rint(dc / L) = 0 and fma(-0, L, dc) = dc. */
+#define DPO_OPEN_EDGE 1e300
+
+int dpo_eval_local(const dpo_model_desc *m, int64_t nloc, int64_t nall, const double *coord, const int32_t *type,
+                   double *energy, double *atom_energy, double *force, double *virial, int32_t *nlist_out) {
+  if (nloc < 0 || nall < nloc) return DPO_EINVAL;
+  const double box[9] = {DPO_OPEN_EDGE, 0, 0, 0, DPO_OPEN_EDGE, 0, 0, 0, DPO_OPEN_EDGE};
+  double L[3];
+  int rc = check_inputs(m, box, L);
+  if (rc != DPO_OK) return rc;
+  const int nm = dpo_nm(m);
+  const size_t nrow = (size_t)(nloc > 0 ? nloc : 1);
+  int32_t *nlist = nlist_out ? nlist_out : (int32_t *)malloc(nrow * nm * sizeof(int32_t));
+  double *fslot = (double *)malloc(nrow * nm * 3 * sizeof(double));
+  double *ei = atom_energy ? atom_energy : (double *)malloc(nrow * sizeof(double));
+  if (!nlist || !fslot || !ei) { rc = DPO_ENOMEM; goto done; }
+  /* neighbours of the local atoms among ALL atoms; rows == NULL: atoms 0 .. nloc-1 */
+  rc = dpo_build_nlist_rows(m, nall, coord, type, box, nloc, NULL, nlist, NULL);
+  if (rc != DPO_OK) goto done;
+  rc = dpo_atom_rows(m, nall, coord, type, box, nloc, NULL, nlist, ei, fslot, NULL, NULL, NULL);
+  if (rc != DPO_OK) goto done;
+  {
+    double e = 0.0;
+    for (int64_t i = 0; i < nloc; ++i) e += ei[i];
+    if (energy) *energy = e;
+  }
+  if (force) memset(force, 0, (size_t)nall * 3 * sizeof(double));
+  if (virial) memset(virial, 0, 9 * sizeof(double));
+  for (int64_t i = 0; i < nloc; ++i)
+    for (int k = 0; k < nm; ++k) {
+      int32_t j = nlist[i * nm + k];
+      if (j < 0) continue;
+      const double *f = fslot + ((size_t)i * nm + k) * 3;
+      if (force)
+        for (int c = 0; c < 3; ++c) { force[3 * i + c] += f[c]; force[3 * (int64_t)j + c] -= f[c]; }
+      if (virial)
+        for (int a = 0; a < 3; ++a) {
+          const double da = coord[3 * (int64_t)j + a] - coord[3 * i + a];
+          for (int b = 0; b < 3; ++b) virial[3 * a + b] -= da * f[b];
+        }
+    }
+done:
+  if (!nlist_out) free(nlist);
+  if (!atom_energy) free(ei);
+  free(fslot);
+  return rc;
+}
+
 /* ---- NEXT #1: molecular dynamics driver --------------------------------------------------
  * Velocity-Verlet integration of Newton's equations with the DP forces, NVE, as the paper runs it (PAPER.md:298:
  * velocity-Verlet, 0.5 fs for water, 1.0 fs for copper; thermo output every 20 steps).  One step:

@@ -81,6 +81,12 @@ int dpo_eval(const dpo_model_desc *m, int64_t natoms, const double *coord, const
              const double box[9], double *energy, double *atom_energy, double *force, double *virial,
              int32_t *nlist_out, int use_cells);
 
+/* NEXT #2 / #3: one sub-region with explicit ghost atoms, no box.  Atoms
+ * 0..nloc-1 are local, nloc..nall-1 ghosts; energy[1] and atom_energy[nloc] cover the local atoms, force[nall][3] is
+ * -dE/dr of that energy on local and ghost atoms, virial[9] the local atoms' part; nlist_out [nloc][Nm] or NULL. */
+int dpo_eval_local(const dpo_model_desc *m, int64_t nloc, int64_t nall, const double *coord, const int32_t *type,
+                   double *energy, double *atom_energy, double *force, double *virial, int32_t *nlist_out);
+
 /* NEXT #1: velocity-Verlet NVE molecular dynamics with the DP forces.
  * coord [N][3] (A) and vel [N][3] (A/fs) are updated in place; mass[ntypes] in amu; thermo [nsteps / thermo_every + 1][4]
  * = (E_pot [eV], E_kin [eV], T [K], P [bar]) at steps 0, thermo_every, ... (may be NULL).  Neighbours are searched from scratch every step. */

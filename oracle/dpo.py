@@ -166,6 +166,23 @@ class Oracle:
             out["nlist"] = nlist
         return out
 
+    def eval_local(self, coord, types, nloc, want_nlist=True):
+        """One sub-region with explicit ghost atoms, no box (dpo_eval_local): atoms [0, nloc) are
+        local.  Returns dict(energy, atom_energy[nloc], force[nall], virial[, nlist[nloc]])."""
+        coord = np.ascontiguousarray(coord, dtype=np.float64).reshape(-1, 3)
+        types = np.ascontiguousarray(types, dtype=np.int32)
+        nall = coord.shape[0]
+        e = C.c_double(0.0)
+        ei, f, vir = np.empty(max(nloc, 1)), np.empty((nall, 3)), np.empty(9)
+        nlist = np.empty((max(nloc, 1), self.nm), dtype=np.int32) if want_nlist else None
+        rc = self.lib.dpo_eval_local(C.byref(self.desc), C.c_int64(nloc), C.c_int64(nall), _d(coord), _i(types),
+                                     C.byref(e), _d(ei), _d(f), _d(vir), _i(nlist))
+        self._chk(rc, "dpo_eval_local")
+        out = {"energy": e.value, "atom_energy": ei[:nloc], "force": f, "virial": vir.reshape(3, 3)}
+        if want_nlist:
+            out["nlist"] = nlist[:nloc]
+        return out
+
     def md_run(self, coord, vel, types, mass, box, dt_fs, nsteps, thermo_every=1, cells=False):
         """Velocity-Verlet NVE MD (dpo_md_run).  Returns (coord, vel, thermo[k][4] = (E_pot, E_kin, T, P [bar]))."""
         coord, types, box = self._inputs(coord, types, box)
