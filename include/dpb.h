@@ -114,6 +114,25 @@ int dpb_eval_host(dpb_model *model, void *stream, int64_t natoms, const double *
                   const double box[9], double *energy_h, double *atom_energy_h, double *force_h, double *virial_h,
                   int32_t *nlist_h, dpb_eval_info *info);
 
+/* One sub-region with explicit ghost atoms (a sub-region owns
+ * its local atoms, the atoms of neighbouring sub-regions and the periodic images within r_c of it are present as
+ * ghosts; the ghost forces go home in the reverse exchange).  There is no box and no minimum image: displacements are
+ * plain differences, so r_c >= L/2 is handled by supplying the images as ghosts.
+ *   nloc, nall   atoms [0, nloc) are local, [nloc, nall) ghosts (nall >= nloc >= 0)
+ *   coord, type  DEVICE, [nall][3] / [nall]
+ *   bounds       HOST fp64 [6]: lo[3], hi[3] of a region that contains every one of the nall atoms (e.g. the brick
+ *                widened by r_c); an atom outside it is DPB_EBOX, reported when info != NULL
+ *   energy       DEVICE fp64 [1]       sum of E_i over the LOCAL atoms
+ *   atom_energy  DEVICE fp64 [nloc]
+ *   force        DEVICE fp64 [nall][3] -dE/dr of that energy, on local and ghost atoms
+ *   virial       DEVICE fp64 [9]       the local atoms' part, -sum_{i<nloc} sum_k d_ik (x) dE_i/dd_ik
+ *   nlist        DEVICE int32 [nloc][Nm], indices into [0, nall)
+ * Summed over the sub-regions of a periodic system (ghost forces added to their owners) the outputs equal dpb_eval's.
+ * Ownership, asynchrony and info as for dpb_eval.  Not available with the deterministic reduction (DPB_ENOTIMPL). */
+int dpb_eval_local(dpb_model *model, void *stream, int64_t nloc, int64_t nall, const double *coord,
+                   const int32_t *type, const double bounds[6], double *energy, double *atom_energy, double *force,
+                   double *virial, int32_t *nlist, dpb_eval_info *info);
+
 /* Alg. 1 only (cell binning + neighbour search + format): nlist DEVICE int32 [N][Nm].  n_overflow HOST, may be
  * NULL (non-NULL synchronises). */
 int dpb_build_nlist(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,

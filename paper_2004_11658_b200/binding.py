@@ -79,6 +79,8 @@ def load_library():
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
     lib.dpb_set_debug_buffers.argtypes = [vp, vp, vp, vp]
     lib.dpb_eval.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp, C.POINTER(_Info)]
+    lib.dpb_eval_local.argtypes = [vp, vp, i64, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp,
+                                   C.POINTER(_Info)]
     lib.dpb_eval_host.argtypes = lib.dpb_eval.argtypes
     lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
     lib.dpb_md_run.argtypes = [vp, vp, i64, vp, vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double),
@@ -198,6 +200,32 @@ class DPModel:
                                bp, C.c_void_p(o["energy"].data_ptr()), C.c_void_p(o["atom_energy"].data_ptr()),
                                C.c_void_p(o["force"].data_ptr()), C.c_void_p(o["virial"].data_ptr()), nl,
                                C.byref(info) if want_info else None)
+        self._chk(rc)
+        if want_info:
+            o["info"] = EvalInfo(int(info.n_real_pairs), int(info.n_overflow), tuple(info.max_nei), int(info.n_chunks))
+        return o
+
+    def eval_local(self, coord, types, nloc, bounds, want_nlist=False, want_info=True):
+        """dpb_eval_local: atoms [0, nloc) local, the rest ghosts; bounds = (lo[3], hi[3]) containing all of them."""
+        torch = _torch()
+        assert coord.is_cuda and coord.dtype == torch.float64 and coord.is_contiguous()
+        assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
+        nall = int(coord.shape[0])
+        dev = coord.device
+        o = {"energy": torch.empty(1, dtype=torch.float64, device=dev),
+             "atom_energy": torch.empty(max(nloc, 1), dtype=torch.float64, device=dev)[:nloc],
+             "force": torch.empty((max(nall, 1), 3), dtype=torch.float64, device=dev)[:nall],
+             "virial": torch.empty((3, 3), dtype=torch.float64, device=dev)}
+        if want_nlist:
+            o["nlist"] = torch.empty((max(nloc, 1), self.nm), dtype=torch.int32, device=dev)[:nloc]
+        bnd = (C.c_double * 6)(*[float(v) for v in np.asarray(bounds, dtype=np.float64).reshape(-1)])
+        info = _Info() if want_info else None
+        rc = self.lib.dpb_eval_local(self._h, self._stream(), C.c_int64(nloc), C.c_int64(nall),
+                                     C.c_void_p(coord.data_ptr()), C.c_void_p(types.data_ptr()), bnd,
+                                     C.c_void_p(o["energy"].data_ptr()), C.c_void_p(o["atom_energy"].data_ptr()),
+                                     C.c_void_p(o["force"].data_ptr()), C.c_void_p(o["virial"].data_ptr()),
+                                     C.c_void_p(o["nlist"].data_ptr()) if want_nlist else None,
+                                     C.byref(info) if want_info else None)
         self._chk(rc)
         if want_info:
             o["info"] = EvalInfo(int(info.n_real_pairs), int(info.n_overflow), tuple(info.max_nei), int(info.n_chunks))

@@ -226,6 +226,27 @@ static int make_grid(const DevModel &P, const double box[9], DevGrid &G, double 
   }
   for (int c = 0; c < 3; ++c) G.lo_mode[c] = G.nc[c] >= 3 ? 1 : 0;
   G.ncell = (int)ncell;
+  for (int c = 0; c < 3; ++c) { G.org[c] = 0.0; G.ext[c] = G.L[c]; }
+  G.open = 0; G.ngrp = 1; G.nloc = 0;
+  return DPB_OK;
+}
+
+// Sub-region mode: the atoms lie in [lo, hi]; the grid is that of a periodic box of edge max(hi - lo + 1.001 rc,
+// 2.002 rc) at origin lo.  Two atoms inside the bounds are less than L - 1.001 rc apart in every coordinate, so every
+// periodic image other than the pair itself is farther than r_c: the minimum image is the plain difference wherever
+// it matters, and rc < L / 2 holds.
+static int make_grid_open(const DevModel &P, const double bounds[6], int64_t nloc, DevGrid &G) {
+  double box[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  for (int c = 0; c < 3; ++c) {
+    const double ext = bounds[3 + c] - bounds[c];
+    if (!(ext >= 0.0) || !(ext < 1e15)) return fail(DPB_EBOX, "bounds: need lo <= hi, finite (dimension %d)", c);
+    const double a = ext + 1.001 * P.rc, b = 2.002 * P.rc;
+    box[4 * c] = a > b ? a : b;
+  }
+  int rc = make_grid(P, box, G, P.rc);
+  if (rc != DPB_OK) return rc;
+  for (int c = 0; c < 3; ++c) { G.org[c] = bounds[c]; G.ext[c] = bounds[3 + c] - bounds[c]; }
+  G.open = 1; G.ngrp = 2; G.nloc = (int)nloc;
   return DPB_OK;
 }
 
@@ -245,23 +266,27 @@ static int neighbour_cap(const DevModel &P) {
 // nl_mode 0: neighbour search from the cell list (every dpb_eval); 1 / 2: MD rebuild / reuse step (md.cu).
 static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double *coord, const int32_t *type,
                     const double box[9], double *energy, double *atom_energy, double *force, double *virial,
-                    int32_t *nlist, bool nlist_only, int nl_mode = 0) {
+                    int32_t *nlist, bool nlist_only, int nl_mode = 0, int64_t nloc = -1) {
+  // nloc >= 0: sub-region mode (dpb_eval_local): `box` holds the bounds (lo[3], hi[3]); atoms [0, nloc) are the centres
   const DevModel &P = m->P;
   if (natoms < 0 || natoms > 2000000000ll) return fail(DPB_EINVAL, "natoms out of range");
   if (natoms > 0 && (!coord || !type)) return fail(DPB_EINVAL, "null coord / type");
+  if (nloc > natoms) return fail(DPB_EINVAL, "nloc > nall");
   DevGrid G;
   int rc = DPB_OK;
-  if (nl_mode == 2) G = m->md_grid;
+  if (nloc >= 0) rc = make_grid_open(P, box, nloc, G);
+  else if (nl_mode == 2) G = m->md_grid;
   else rc = make_grid(P, box, G, nl_mode == 1 ? P.rc + m->md_skin : P.rc);
   if (rc != DPB_OK) return rc;
   if (nl_mode == 1) m->md_grid = G;
   const int N = (int)natoms;
-  const int nkeys = P.ntypes * G.ncell;
-  const int64_t chunk = m->chunk < natoms ? m->chunk : (natoms > 0 ? natoms : 1);
+  const int nkeys = P.ntypes * G.ngrp * G.ncell;
+  const int64_t ncentre = nloc >= 0 ? nloc : natoms;
+  const int64_t chunk = m->chunk < ncentre ? m->chunk : (ncentre > 0 ? ncentre : 1);
 
   CU(m->key.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
   CU(m->count.reserve(sizeof(int) * (size_t)(nkeys + 1)), "workspace");
-  CU(m->start.reserve(sizeof(int) * (size_t)(nkeys + 1 + P.ntypes + 1)), "workspace");
+  CU(m->start.reserve(sizeof(int) * (size_t)(nkeys + 1 + P.ntypes * G.ngrp + 1)), "workspace");
   CU(m->cursor.reserve(sizeof(int) * (size_t)(nkeys + 1)), "workspace");
   CU(m->s_idx.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
   CU(m->s_xyz.reserve(sizeof(double) * 3 * (size_t)(N + 1)), "workspace");
@@ -269,6 +294,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   const bool det = m->deterministic && !nlist_only;
   if (det && (m->precision != DPB_FP64 || m->variant != 1 || !m->v1.ready))
     return fail(DPB_ENOTIMPL, "the deterministic reduction is built for DPB_FP64, variant 1");
+  if (det && nloc >= 0) return fail(DPB_ENOTIMPL, "the deterministic reduction is built for the periodic box");
   if (det) {
     CU(m->pos_of.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
     CU(m->nl_all.reserve(sizeof(int) * (size_t)(N + 1) * P.nm), "workspace");
@@ -304,7 +330,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     raw.rs2_hi = rs * rs * (1.0 + 1e-9);
   }
   const bool timing = m->timing && !nlist_only;
-  const int nchunks = (int)((natoms + chunk - 1) / chunk);
+  const int nchunks = (int)((ncentre + chunk - 1) / chunk);
   if (timing) {
     const size_t need = 3 + 4 * (size_t)nchunks;
     while (m->evs.size() < need) {
@@ -337,10 +363,10 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   }
   const int cap = neighbour_cap(P);
   int ci = 0;
-  for (int64_t p0 = 0; p0 < natoms; p0 += chunk, ++ci) {
+  for (int64_t p0 = 0; p0 < ncentre; p0 += chunk, ++ci) {
     ChunkView C;
     C.p0 = (int)p0;
-    C.n = (int)((natoms - p0) < chunk ? (natoms - p0) : chunk);
+    C.n = (int)((ncentre - p0) < chunk ? (ncentre - p0) : chunk);
     C.s_idx = m->s_idx.as<int>();
     C.type_start = start + nkeys + 1;
     C.nl = m->nl.as<int>();
@@ -395,7 +421,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
                            m->s_xyz.as<double>(), m->nl_all.as<int>(), m->nreal_all.as<int>(), m->fslot.as<double>(),
                            force, m->vpart.as<double>(), virial, st), "deterministic force gather");
   if (!nlist_only) {
-    if (energy) CU(launch_reduce_energy(natoms, ei, energy, st), "energy reduction");
+    if (energy) CU(launch_reduce_energy(ncentre, ei, energy, st), "energy reduction");
     if (timing) cudaEventRecord(m->evs[2 + 4 * nchunks], st);
   }
   return DPB_OK;
@@ -408,6 +434,7 @@ static int finish_info(dpb_model *m, cudaStream_t st, int64_t natoms, dpb_eval_i
   if (hs.err_type) return fail(DPB_EINVAL, "an atom has a type index outside [0, ntypes)");
   if (hs.err_cap) return fail(DPB_ECAP, "an atom has more in-range candidates than the staging capacity (%d)",
                               neighbour_cap(m->P));
+  if (hs.err_bounds) return fail(DPB_EBOX, "an atom lies outside the bounds given to dpb_eval_local");
   if (info) {
     memset(info, 0, sizeof(*info));
     info->n_real_pairs = (int64_t)hs.n_real_pairs;
@@ -427,6 +454,18 @@ extern "C" int dpb_eval(dpb_model *m, void *stream, int64_t natoms, const double
   int rc = run_eval(m, st, natoms, coord, type, box, energy, atom_energy, force, virial, nlist, false);
   if (rc != DPB_OK) return rc;
   if (info) return finish_info(m, st, natoms, info);
+  return DPB_OK;
+}
+
+extern "C" int dpb_eval_local(dpb_model *m, void *stream, int64_t nloc, int64_t nall, const double *coord,
+                              const int32_t *type, const double bounds[6], double *energy, double *atom_energy,
+                              double *force, double *virial, int32_t *nlist, dpb_eval_info *info) {
+  if (!m || !bounds) return fail(DPB_EINVAL, "dpb_eval_local: null model / bounds");
+  if (nloc < 0) return fail(DPB_EINVAL, "dpb_eval_local: nloc < 0");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  int rc = run_eval(m, st, nall, coord, type, bounds, energy, atom_energy, force, virial, nlist, false, 0, nloc);
+  if (rc != DPB_OK) return rc;
+  if (info) return finish_info(m, st, nloc, info);
   return DPB_OK;
 }
 

@@ -23,6 +23,14 @@ struct DevGrid {
   int nc[3];
   int ncell;
   int lo_mode[3];   // 1: nc >= 3, use the +-1 stencil; 0: fewer than 3 cells, visit every cell of that dimension once
+  // Sub-region mode (dpb_eval_local): no periodic box.  The atoms live in [org, org + ext]; L is that
+  // extent padded by more than r_c, so that the minimum image of any pair within r_c is the pair itself and the
+  // periodic kernels serve unchanged.  Atoms [0, nloc) are local, the rest ghosts: the sort key puts the ghosts behind
+  // all local atoms (ngrp = 2 groups of ntypes pseudo-types), so the sorted positions [0, nloc) are the centres.
+  double org[3], ext[3];
+  int open;         // 1: sub-region mode
+  int ngrp;         // 1 (periodic) or 2 (local, ghost)
+  int nloc;
 };
 
 // Stats accumulated on the device by the neighbour kernel.
@@ -32,6 +40,7 @@ struct DevStats {
   int max_nei[DPB_MAX_TYPES];
   int err_type;      // an atom had a type index outside [0, ntypes)
   int err_cap;       // an atom had more in-range candidates than the staging capacity
+  int err_bounds;    // sub-region mode: an atom lies outside the bounds the caller gave
   double max_disp2;  // MD: largest squared displacement of an atom since the last neighbour rebuild (bits ordered as u64)
 };
 

@@ -39,7 +39,9 @@ __global__ void k_keys(DevModel P, DevGrid G, int n, const double *__restrict__ 
   int ic[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    double f = coord[3 * (size_t)i + c] / G.L[c];
+    const double x = coord[3 * (size_t)i + c] - G.org[c];
+    if (G.open && !(x >= 0.0 && x <= G.ext[c])) atomicExch(&stats->err_bounds, 1);
+    double f = x / G.L[c];
     f -= floor(f);
     int v = (int)(f * G.nc[c]);
     v = v < 0 ? 0 : v;
@@ -50,6 +52,7 @@ __global__ void k_keys(DevModel P, DevGrid G, int n, const double *__restrict__ 
     atomicExch(&stats->err_type, 1);
     t = 0;
   }
+  if (G.ngrp == 2 && i >= G.nloc) t += P.ntypes;                   // ghosts: behind every local atom
   int k = t * G.ncell + (ic[0] * G.nc[1] + ic[1]) * G.nc[2] + ic[2];
   key[i] = k;
   atomicAdd(&count[k], 1);
@@ -100,13 +103,13 @@ __global__ void k_fill(int n, const double *__restrict__ coord, const int *__res
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
                              DevStats *stats, cudaStream_t st, int *pos_of) {
-  const int nkeys = P.ntypes * G.ncell;
+  const int nkeys = P.ntypes * G.ngrp * G.ncell;
   cudaError_t e = cudaMemsetAsync(count, 0, sizeof(int) * (size_t)nkeys, st);
   if (e != cudaSuccess) return e;
   const int n = (int)natoms;
   if (n > 0) k_keys<<<(n + 255) / 256, 256, 0, st>>>(P, G, n, coord, type, key, count, stats);
   // type_start lives right behind start[nkeys + 1]
-  k_scan<<<1, 1024, 0, st>>>(nkeys, G.ncell, P.ntypes, count, start, cursor, start + nkeys + 1);
+  k_scan<<<1, 1024, 0, st>>>(nkeys, G.ncell, P.ntypes * G.ngrp, count, start, cursor, start + nkeys + 1);
   if (n > 0) k_fill<<<(n + 255) / 256, 256, 0, st>>>(n, coord, key, cursor, s_idx, s_xyz, pos_of);
   DPB_LAUNCHED(n > 0 ? 3 : 1);
   return cudaGetLastError();
@@ -118,7 +121,7 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
 // Cells are numbered z-fastest, so the three z-neighbours of a stencil column are one contiguous run of sorted
 // positions (two runs when the column wraps around the box): 9 x 2 entries per type instead of 27.
 #define NL_THREADS 128
-#define NL_ENTRIES (18 * DPB_MAX_TYPES)
+#define NL_ENTRIES (2 * 18 * DPB_MAX_TYPES)       // x 2: local and ghost groups of the sub-region mode
 #define NL_BUCKETS 32           // distance buckets per type, uniform in r^3: the ranking only compares inside a bucket
 
 struct __align__(16) NlHit { double r; int j; int t; };
@@ -154,7 +157,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
     int ic[3], lo[3], num[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {                                  // cell of atom i, recomputed exactly as in k_keys
-      double f = xi[c] / G.L[c];
+      double f = (xi[c] - G.org[c]) / G.L[c];
       f -= floor(f);
       int v = (int)(f * G.nc[c]);
       v = v < 0 ? 0 : v;
@@ -167,19 +170,20 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
     else if (lo[2] < 0) { z0 = 0; len0 = 2; z1 = G.nc[2] - 1; len1 = 1; }
     else if (lo[2] + 2 >= G.nc[2]) { z0 = lo[2]; len0 = 2; z1 = 0; len1 = 1; }
     else { z0 = lo[2]; len0 = 3; }
-    const int nent = 18 * P.ntypes;
+    const int nent = 18 * P.ntypes * G.ngrp;
     int nr = 0, run = 0;
     for (int base = 0; base < nent; base += 32) {
       const int ent = base + lane;
       int cntv = 0, s0 = 0, t = 0;
       if (ent < nent) {
-        t = ent / 18;
-        const int w = ent - 18 * t, part = w & 1, ab = w >> 1, a = ab / 3, b = ab - 3 * a;
+        const int pt = ent / 18;                                     // pseudo-type: (group, type)
+        t = pt >= P.ntypes ? pt - P.ntypes : pt;
+        const int w = ent - 18 * pt, part = w & 1, ab = w >> 1, a = ab / 3, b = ab - 3 * a;
         const int zz = part ? z1 : z0, ln = part ? len1 : len0;
         if (a < num[0] && b < num[1] && ln > 0) {                  // fewer than 3 cells in a dimension: each cell once
           const int ja = (lo[0] + a + G.nc[0]) % G.nc[0];
           const int jb = (lo[1] + b + G.nc[1]) % G.nc[1];
-          const int k = t * G.ncell + (ja * G.nc[1] + jb) * G.nc[2] + zz;
+          const int k = pt * G.ncell + (ja * G.nc[1] + jb) * G.nc[2] + zz;
           s0 = start[k];
           cntv = start[k + ln] - s0;
         }

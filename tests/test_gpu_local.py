@@ -1,0 +1,185 @@
+"""GPU parity tests of dpb_eval_local (one sub-region with explicit ghost atoms, no box; SURVEY.md §8(e) / §8(f) NEXT
+#2, #3) against the oracle's dpo_eval_local, through the C ABI.  Bars as for dpb_eval: the neighbour
+list bit-exact; fp64: 1e-10 relative on E, 1e-9 eV/A on F (local AND ghost atoms); mixed precision: 1e-5 / 1e-3.
+The ghost shells are built by brute force over the 27 periodic images (tests/test_oracle_local.py)."""
+import numpy as np
+import pytest
+
+import gen
+from gen.weights import MODELS
+
+from conftest import small_model, random_box
+from test_oracle_local import brute_force_domain, bricks
+
+pytestmark = pytest.mark.gpu
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (the library has no CPU fallback)")
+    return torch
+
+
+def _bars(precision):
+    from paper_2004_11658_b200.binding import FP64
+    return (1e-10, 1e-9, 1e-10) if precision == FP64 else (1e-5, 1e-3, 1e-5)
+
+
+def _gpu_local(m, x, t, nloc, bounds):
+    torch = _torch()
+    out = m.eval_local(torch.tensor(x, device="cuda"), torch.tensor(t.astype(np.int32), device="cuda"), nloc, bounds,
+                       want_nlist=True)
+    torch.cuda.synchronize()
+    return {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in out.items()}
+
+
+def _domain(coord, types, box, lo, hi, rc):
+    loc, own, gxyz, w = brute_force_domain(coord, box, lo, hi, rc)
+    x = np.ascontiguousarray(np.concatenate([w[loc], gxyz]))
+    t = np.concatenate([types[loc], types[own]]).astype(np.int32)
+    bounds = np.concatenate([lo - rc, hi + rc])
+    return loc, own, x, t, bounds
+
+
+def _check(ref, got, precision):
+    e_rel, f_abs, v_rel = _bars(precision)
+    assert np.array_equal(got["nlist"], ref["nlist"]), "nlist must be bit-exact"
+    assert abs(got["energy"][0] - ref["energy"]) <= e_rel * abs(ref["energy"])
+    assert np.abs(got["atom_energy"] - ref["atom_energy"]).max() <= e_rel * np.abs(ref["atom_energy"]).max()
+    assert np.abs(got["force"] - ref["force"]).max() <= f_abs
+    assert np.abs(got["virial"] - ref["virial"]).max() <= v_rel * max(1.0, np.abs(ref["virial"]).max())
+
+
+@pytest.mark.parametrize("precision_name", ["FP64", "TF32"])
+@pytest.mark.parametrize("grid", [(2, 1, 1), (2, 2, 2)])
+def test_water192_subregions_against_the_oracle(precision_name, grid):
+    """BASELINE config 0 (W192, conditioned weights) cut into bricks: every brick, every output element, ghost forces
+    included; then the partition identity against dpb_eval on the periodic box."""
+    import paper_2004_11658_b200 as pk
+    from oracle import Oracle
+    torch = _torch()
+    from paper_2004_11658_b200 import binding
+    precision = getattr(binding, precision_name)
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc = Oracle.from_spec(spec, emb, fit)
+    m = pk.DPModel.from_spec(spec, emb, fit, precision=precision)
+    n = len(coord)
+    E, F, V = 0.0, np.zeros((n, 3)), np.zeros((3, 3))
+    for lo, hi in bricks(box, grid):
+        loc, own, x, t, bounds = _domain(coord, types, box, lo, hi, spec.rcut)
+        ref = orc.eval_local(x, t, len(loc))
+        got = _gpu_local(m, x, t, len(loc), bounds)
+        assert got["force"].shape == (len(x), 3) and np.abs(ref["force"][len(loc):]).max() > 1e-3
+        _check(ref, got, precision)
+        E += got["energy"][0]
+        V += got["virial"]
+        np.add.at(F, np.concatenate([loc, own]), got["force"])
+    per = m.eval(torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda"), box)
+    torch.cuda.synchronize()
+    e_rel, f_abs, v_rel = _bars(precision)
+    assert abs(E - per["energy"].item()) <= 2 * e_rel * abs(E)
+    assert np.abs(F - per["force"].cpu().numpy()).max() <= 2 * f_abs
+    assert np.abs(V - per["virial"].cpu().numpy()).max() <= 2 * v_rel * max(1.0, np.abs(V).max())
+
+
+def test_cutoff_beyond_half_the_box():
+    """r_c >= L/2 (refused by dpb_eval: DPB_EBOX) through explicit images, the paper's formulation:
+    one brick = the whole box, every ghost a periodic image; an atom then sees several images of the same neighbour."""
+    import paper_2004_11658_b200 as pk
+    from oracle import Oracle
+    torch = _torch()
+    spec, emb, fit = small_model(ntypes=2, s1=8, m_axis=4, fit_width=16, sel=(40, 60), rcut=4.0, rcut_smth=1.0, seed=5,
+                                 fit_scale=0.05)
+    coord, types, box = random_box(30, 6.5, 2, seed=11, min_dist=1.2)         # L = 6.5 < 2 r_c
+    orc = Oracle.from_spec(spec, emb, fit)
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    with pytest.raises(pk.DPBError):
+        m.eval(torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda"), box)
+    lo, hi = np.zeros(3), np.array([box[0], box[4], box[8]])
+    loc, own, x, t, bounds = _domain(coord, types, box, lo, hi, spec.rcut)
+    assert len(loc) == 30 and len(own) > 60
+    ref = orc.eval_local(x, t, 30)
+    ids = np.concatenate([loc, own])
+    row = ref["nlist"][0]
+    owners = ids[row[row >= 0]]
+    assert len(set(owners)) < len(owners)                                    # the same atom twice, as two images
+    got = _gpu_local(m, x, t, 30, bounds)
+    _check(ref, got, 0)
+
+
+def test_isolated_cluster_and_degenerate_cases():
+    import paper_2004_11658_b200 as pk
+    from oracle import Oracle
+    spec, emb, fit = small_model(ntypes=2, s1=8, m_axis=4, fit_width=16, sel=(30, 40), rcut=4.0, rcut_smth=1.0, seed=6,
+                                 fit_scale=0.05)
+    coord, types, box = random_box(50, 9.0, 2, seed=3, min_dist=1.2)
+    orc = Oracle.from_spec(spec, emb, fit)
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    x = coord - 200.0                                                         # negative coordinates, far from the origin
+    bounds = np.concatenate([x.min(axis=0), x.max(axis=0)])                   # tight: atoms sit ON the bounds
+    ref = orc.eval_local(x, types, 50)
+    got = _gpu_local(m, x, types, 50, bounds)
+    _check(ref, got, 0)
+    assert np.abs(got["force"].sum(axis=0)).max() < 1e-9
+    # ghosts only
+    got0 = _gpu_local(m, x, types, 0, bounds)
+    assert got0["energy"][0] == 0.0 and not got0["force"].any() and not got0["virial"].any()
+    # a lone atom, and nothing at all
+    one = _gpu_local(m, x[:1], types[:1], 1, np.concatenate([x[0], x[0]]))
+    ref1 = orc.eval_local(x[:1], types[:1], 1)
+    assert abs(one["energy"][0] - ref1["energy"]) <= 1e-10 * max(1.0, abs(ref1["energy"])) and not one["force"].any()
+    none = _gpu_local(m, x[:0], types[:0], 0, np.zeros(6))
+    assert none["energy"][0] == 0.0
+    # an atom outside the bounds is reported, not silently mis-binned
+    bad = bounds.copy()
+    bad[3] -= 1.0
+    with pytest.raises(pk.DPBError):
+        _gpu_local(m, x, types, 50, bad)
+    # sub-region mode and the deterministic reduction do not combine
+    m.set_deterministic(True)
+    with pytest.raises(pk.DPBError):
+        _gpu_local(m, x, types, 50, bounds)
+    m.set_deterministic(False)
+
+
+def test_water24k_slab_identity():
+    """BASELINE configs[1] (W24k) cut into 2 x 2 x 1 bricks in the launch configuration bench.py uses (default chunk,
+    fp64): ghost shells from the 27 images, sum over the bricks against dpb_eval on the periodic box, and a sample of
+    local atoms of one brick against the oracle (nlist rows, E_i)."""
+    import paper_2004_11658_b200 as pk
+    from oracle import Oracle
+    torch = _torch()
+    spec = MODELS["W24k"]
+    coord, types, box = gen.make_system("W24k")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    n = len(coord)
+    E, F, V = 0.0, np.zeros((n, 3)), np.zeros((3, 3))
+    first = None
+    for lo, hi in bricks(box, (2, 2, 1)):
+        loc, own, x, t, bounds = _domain(coord, types, box, lo, hi, spec.rcut)
+        got = _gpu_local(m, x, t, len(loc), bounds)
+        if first is None:
+            first = (loc, own, x, t, got)
+        E += got["energy"][0]
+        V += got["virial"]
+        np.add.at(F, np.concatenate([loc, own]), got["force"])
+    per = m.eval(torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda"), box)
+    torch.cuda.synchronize()
+    assert abs(E - per["energy"].item()) <= 1e-10 * abs(E)
+    assert np.abs(F - per["force"].cpu().numpy()).max() <= 2e-9
+    assert np.abs(V - per["virial"].cpu().numpy()).max() <= 1e-10 * max(1.0, np.abs(V).max())
+    loc, own, x, t, got = first
+    orc = Oracle.from_spec(spec, emb, fit)
+    rows = np.random.default_rng(5).choice(len(loc), size=48, replace=False).astype(np.int64)
+    big = np.diag([1e300] * 3).reshape(-1)                                    # the oracle's open-boundary box
+    nl = orc.build_nlist(x, t, big, rows=rows)
+    nl = nl[0] if isinstance(nl, tuple) else nl
+    assert np.array_equal(got["nlist"][rows], nl)
+    ar = orc.atom_rows(x, t, big, rows, nl)
+    assert np.abs(got["atom_energy"][rows] - ar["atom_energy"]).max() <= 1e-10 * np.abs(ar["atom_energy"]).max()
