@@ -183,3 +183,30 @@ def test_water24k_slab_identity():
     assert np.array_equal(got["nlist"][rows], nl)
     ar = orc.atom_rows(x, t, big, rows, nl)
     assert np.abs(got["atom_energy"][rows] - ar["atom_energy"]).max() <= 1e-10 * np.abs(ar["atom_energy"]).max()
+
+
+@pytest.mark.parametrize("name", ["W192", "W24k"])
+def test_decomposition_driver_on_one_gpu(name):
+    """paper_2004_11658_b200.dd with world size 1 on the device: the forward exchange makes the periodic images, the
+    reverse exchange folds their forces back, dpb_eval_local does the arithmetic; against dpb_eval on the same box.
+    (The multi-rank routes are covered over gloo in tests/test_dd_gloo.py.)"""
+    import paper_2004_11658_b200 as pk
+    from paper_2004_11658_b200.dd import BrickDecomposition
+    torch = _torch()
+    spec = MODELS[name]
+    coord, types, box = gen.make_system(name)
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda")
+    per = m.eval(dc, dt, box)
+    dd = BrickDecomposition(box, spec.rcut, grid=(1, 1, 1), rank=0, world=1)
+    mask, w = dd.owned_mask(dc)
+    assert bool(mask.all())
+    out = dd.evaluate(lambda x, t, nloc, bounds: m.eval_local(x, t, nloc, bounds), w.contiguous(), dt)
+    torch.cuda.synchronize()
+    assert out["nall"] > 2 * len(coord) or name != "W192"
+    assert abs(out["energy"].item() - per["energy"].item()) <= 1e-10 * abs(per["energy"].item())
+    assert (out["force"] - per["force"]).abs().max().item() <= 2e-9
+    assert (out["atom_energy"] - per["atom_energy"]).abs().max().item() <= 1e-10 * per["atom_energy"].abs().max().item()
+    assert (out["virial"] - per["virial"]).abs().max().item() <= 1e-10 * max(1.0, per["virial"].abs().max().item())
