@@ -215,6 +215,55 @@ def run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed):
     return out
 
 
+# ---- domain decomposition: weak scaling, one brick per rank ----------------------
+def run_dd(args, spec, name, coord, types, box, dev, model, world, rank):
+    """Every rank owns one copy of the workload's box as its brick of a px x py x pz times larger periodic box
+    (weak scaling).  One step = forward ghost exchange, dpb_eval_local, reverse force exchange, all-reduce
+    of E and the virial (paper_2004_11658_b200/dd.py).  With one rank the ghosts are the periodic images."""
+    import torch
+    import torch.distributed as dist
+    from paper_2004_11658_b200.dd import BrickDecomposition, choose_grid
+    grid = choose_grid(world, (1.0, 1.0, 1.0))
+    L = np.array([box[0], box[4], box[8]])
+    gbox = np.diag(L * np.array(grid)).reshape(-1)
+    dd = BrickDecomposition(gbox, spec.rcut, grid=grid, rank=rank, world=world)
+    w = coord - np.floor(coord / L) * L + dd.lo
+    w = np.minimum(w, np.nextafter(dd.hi, dd.lo))                    # x + lo can round onto the upper face
+    dc, dt = torch.tensor(w, device=dev), torch.tensor(types, device=dev)
+    ev_local = lambda x, t, nloc, bounds: model.eval_local(x, t, nloc, bounds, want_info=False)
+    steps, warm = max(3, min(args.steps, 20)), 3
+    for _ in range(warm):
+        out = dd.evaluate(ev_local, dc, dt)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    marks = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+    for k in range(steps):
+        marks[k][0].record()
+        x, t = dd.forward(dc, dt)
+        marks[k][1].record()
+        o = ev_local(x, t, dd.nloc, dd.bounds())
+        marks[k][2].record()
+        f = dd.reverse(o["force"])
+        red = torch.cat([o["energy"].reshape(1), o["virial"].reshape(9)])
+        if world > 1:
+            dist.all_reduce(red)
+        marks[k][3].record()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    seg = np.array([[m[i].elapsed_time(m[i + 1]) for i in range(3)] for m in marks]).sum(axis=0)
+    tot = torch.tensor([sum(m[0].elapsed_time(m[3]) for m in marks)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+    ms = float(tot[0]) / steps
+    return {"grid": list(grid), "atoms_per_rank": int(coord.shape[0]), "atoms_with_ghosts": int(x.shape[0]),
+            "steps": steps, "ms_per_step": ms, "atom_steps_per_s": world * coord.shape[0] / (ms * 1e-3),
+            "ms_forward_exchange": seg[0] / steps, "ms_eval_local": seg[1] / steps,
+            "ms_reverse_exchange_allreduce": seg[2] / steps, "energy_per_atom": float(red[0]) / (world * coord.shape[0]),
+            "note": "times of rank 0 for the three parts, max over ranks for the step"}
+
+
 # ---- the CUDA arm ---------------------------------------------------------------------------------------------
 def run_cuda(args):
     import torch
@@ -315,6 +364,9 @@ def run_cuda(args):
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
     dev_ms, e2e_ms = float(times[0]), float(times[1])
 
+    # optional extra leg, on every rank: the domain-decomposed step
+    dd_leg = run_dd(args, spec, name, coord, types, box, dev, model, world, rank) if args.dd else None
+
     if rank == 0:
         ms_per_step = dev_ms / args.steps
         value = world * n * args.steps / (dev_ms * 1e-3)
@@ -366,6 +418,8 @@ def run_cuda(args):
             line.pop("fp64_frac_of_peak", None)
         if args.md_steps > 0:
             line["md"] = run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed)
+        if dd_leg is not None:
+            line["dd"] = dd_leg
         if world == 1 and not args.no_cpu_baseline:
             step, k, desc, threads = oracle_step_sampler(name, gen.SEED_BASE, args.ref_sample)
             step()
@@ -397,6 +451,9 @@ def main():
     ap.add_argument("--md-steps", type=int, default=0,
                     help="also run this many velocity-Verlet steps (dpb_md_run; PAPER.md:298: 330 K, 0.5 / 1.0 fs, 2 A skin "
                          "rebuilt every 50 steps) and report steps/s and ns/day in an extra 'md' object")
+    ap.add_argument("--dd", action="store_true",
+                    help="also time the domain-decomposed step (one brick per rank, ghost exchange + dpb_eval_local + "
+                         "reverse force exchange + all-reduce) and report it in an extra 'dd' object")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
