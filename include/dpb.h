@@ -133,6 +133,21 @@ int dpb_eval_local(dpb_model *model, void *stream, int64_t nloc, int64_t nall, c
                    const int32_t *type, const double bounds[6], double *energy, double *atom_energy, double *force,
                    double *virial, int32_t *nlist, dpb_eval_info *info);
 
+/* Ghost exchange of the domain decomposition (the driver is paper_2004_11658_b200/dd.py).  All
+ * pointers DEVICE, all work asynchronous on `stream`; messages are rows of four fp64 (x, y, z, type).
+ * dpb_dd_pack: one stage of the forward exchange along dimension dim (0, 1, 2).  Atoms with coord[dim] < cut_minus go to
+ *   pack_minus (coord[dim] += shift_minus), atoms with coord[dim] >= cut_plus to pack_plus (+= shift_plus); an atom may
+ *   go both ways.  idx_* [cap] receives the atom index of each row (for the reverse exchange), counts[2] = rows wanted
+ *   for (minus, plus); rows beyond cap are counted but not written, so counts[d] > cap means: grow and call again.
+ *   Row order inside a message is arbitrary.
+ * dpb_dd_unpack: k received rows -> coord_out [k][3], type_out [k] (the tail of the atom arrays).
+ * dpb_dd_add_forces: reverse exchange, force[idx[i]][:] += fin[i][:] for i < k; idx must not repeat within one call. */
+int dpb_dd_pack(void *stream, int64_t n, const double *coord, const int32_t *type, int32_t dim, double cut_minus,
+                double cut_plus, double shift_minus, double shift_plus, int64_t cap, double *pack_minus,
+                int32_t *idx_minus, double *pack_plus, int32_t *idx_plus, int32_t *counts);
+int dpb_dd_unpack(void *stream, int64_t k, const double *pack, double *coord_out, int32_t *type_out);
+int dpb_dd_add_forces(void *stream, int64_t k, const int32_t *idx, const double *fin, double *force);
+
 /* Alg. 1 only (cell binning + neighbour search + format): nlist DEVICE int32 [N][Nm].  n_overflow HOST, may be
  * NULL (non-NULL synchronises). */
 int dpb_build_nlist(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,

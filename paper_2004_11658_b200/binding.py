@@ -85,6 +85,10 @@ def load_library():
     lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
     lib.dpb_md_run.argtypes = [vp, vp, i64, vp, vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                C.POINTER(_MDParams), vp, C.POINTER(_MDInfo)]
+    d = C.c_double
+    lib.dpb_dd_pack.argtypes = [vp, i64, vp, vp, i32, d, d, d, d, i64, vp, vp, vp, vp, vp]
+    lib.dpb_dd_unpack.argtypes = [vp, i64, vp, vp, vp]
+    lib.dpb_dd_add_forces.argtypes = [vp, i64, vp, vp, vp]
     lib.dpb_kernel_launches.restype = C.c_int64
     lib.dpb_last_error.restype = C.c_char_p
     lib.dpb_version.restype = C.c_char_p
@@ -285,3 +289,32 @@ class DPModel:
         self._chk(rc)
         return thermo, dict(n_thermo=info.n_thermo, n_rebuilds=info.n_rebuilds, skin_violated=bool(info.skin_violated),
                             max_displacement=info.max_displacement)
+
+
+# ---- ghost exchange kernels of the domain decomposition (dd.py); argument marshalling only ----------------------
+def _dd_chk(lib, rc):
+    if rc != 0:
+        raise DPBError(rc, lib.dpb_last_error().decode())
+
+
+def dd_pack(coord, types, n, dim, cut_minus, cut_plus, shift_minus, shift_plus, pack_minus, idx_minus, pack_plus,
+            idx_plus, counts):
+    """dpb_dd_pack on torch CUDA tensors: atoms [0, n) of coord / types; capacity = rows of the pack buffers."""
+    lib = load_library()
+    p = lambda t: C.c_void_p(t.data_ptr())
+    cap = int(pack_minus.shape[0])
+    assert int(pack_plus.shape[0]) == cap and int(idx_minus.shape[0]) >= cap and int(idx_plus.shape[0]) >= cap
+    _dd_chk(lib, lib.dpb_dd_pack(DPModel._stream(), n, p(coord), p(types), dim, cut_minus, cut_plus, shift_minus,
+                                 shift_plus, cap, p(pack_minus), p(idx_minus), p(pack_plus), p(idx_plus), p(counts)))
+
+
+def dd_unpack(pack, k, coord_out, type_out):
+    lib = load_library()
+    p = lambda t: C.c_void_p(t.data_ptr())
+    _dd_chk(lib, lib.dpb_dd_unpack(DPModel._stream(), k, p(pack), p(coord_out), p(type_out)))
+
+
+def dd_add_forces(idx, fin, k, force):
+    lib = load_library()
+    p = lambda t: C.c_void_p(t.data_ptr())
+    _dd_chk(lib, lib.dpb_dd_add_forces(DPModel._stream(), k, p(idx), p(fin), p(force)))

@@ -469,6 +469,33 @@ extern "C" int dpb_eval_local(dpb_model *m, void *stream, int64_t nloc, int64_t 
   return DPB_OK;
 }
 
+extern "C" int dpb_dd_pack(void *stream, int64_t n, const double *coord, const int32_t *type, int32_t dim,
+                           double cut_minus, double cut_plus, double shift_minus, double shift_plus, int64_t cap,
+                           double *pack_minus, int32_t *idx_minus, double *pack_plus, int32_t *idx_plus,
+                           int32_t *counts) {
+  if (n < 0 || n > 2000000000ll || cap < 0 || cap > 2000000000ll || dim < 0 || dim > 2)
+    return fail(DPB_EINVAL, "dpb_dd_pack: n / cap / dim out of range");
+  if (!counts || (n > 0 && (!coord || !type)) || (cap > 0 && (!pack_minus || !idx_minus || !pack_plus || !idx_plus)))
+    return fail(DPB_EINVAL, "dpb_dd_pack: null argument");
+  CU(launch_dd_pack(n, coord, type, dim, cut_minus, cut_plus, shift_minus, shift_plus, cap, pack_minus, idx_minus,
+                    pack_plus, idx_plus, counts, reinterpret_cast<cudaStream_t>(stream)), "dd pack");
+  return DPB_OK;
+}
+
+extern "C" int dpb_dd_unpack(void *stream, int64_t k, const double *pack, double *coord_out, int32_t *type_out) {
+  if (k < 0 || k > 2000000000ll) return fail(DPB_EINVAL, "dpb_dd_unpack: k out of range");
+  if (k > 0 && (!pack || !coord_out || !type_out)) return fail(DPB_EINVAL, "dpb_dd_unpack: null argument");
+  CU(launch_dd_unpack(k, pack, coord_out, type_out, reinterpret_cast<cudaStream_t>(stream)), "dd unpack");
+  return DPB_OK;
+}
+
+extern "C" int dpb_dd_add_forces(void *stream, int64_t k, const int32_t *idx, const double *fin, double *force) {
+  if (k < 0 || k > 2000000000ll) return fail(DPB_EINVAL, "dpb_dd_add_forces: k out of range");
+  if (k > 0 && (!idx || !fin || !force)) return fail(DPB_EINVAL, "dpb_dd_add_forces: null argument");
+  CU(launch_dd_add_forces(k, idx, fin, force, reinterpret_cast<cudaStream_t>(stream)), "dd add forces");
+  return DPB_OK;
+}
+
 extern "C" int dpb_build_nlist(dpb_model *m, void *stream, int64_t natoms, const double *coord, const int32_t *type,
                                const double box[9], int32_t *nlist, int64_t *n_overflow) {
   if (!m || !box || !nlist) return fail(DPB_EINVAL, "dpb_build_nlist: null argument");

@@ -65,6 +65,13 @@ struct ChunkView {
   double *fslot;           // deterministic mode: [n][nm][3] dE_i/dd_ik per slot (pass 2 stores instead of scattering)
 };
 
+// dd.cu: pack / unpack kernels of the domain decomposition's ghost exchange
+cudaError_t launch_dd_pack(int64_t n, const double *coord, const int *type, int dim, double cut_minus, double cut_plus,
+                           double shift_minus, double shift_plus, int64_t cap, double *pack_minus, int *idx_minus,
+                           double *pack_plus, int *idx_plus, int *counts, cudaStream_t st);
+cudaError_t launch_dd_unpack(int64_t k, const double *pack, double *coord_out, int *type_out, cudaStream_t st);
+cudaError_t launch_dd_add_forces(int64_t k, const int *idx, const double *fin, double *force, cudaStream_t st);
+
 // Process-wide count of kernels launched by this library (reported by dpb_kernel_launches()).
 extern unsigned long long g_dpb_launches;
 #define DPB_LAUNCHED(n) (g_dpb_launches += (unsigned long long)(n))

@@ -11,9 +11,11 @@ One process per GPU; each rank owns the atoms of one brick of an orthorhombic pe
                          and are ADDED there (PAPER.md:149: grad_{r_i} E_j != -grad_{r_j} E_i, so they cannot be dropped);
   4. all-reduce        — E and the nine virial components, ten doubles.
 
-Everything here is plumbing: index selection, packing and torch.distributed point-to-point calls on whatever device
-the tensors live on (NCCL over NVLink for CUDA tensors, gloo for the CPU tests).  All arithmetic of the model runs in
-the `evaluate` callable — DPModel.eval_local in production; there is no CPU fallback in this module.
+Everything here is plumbing.  For CUDA tensors the selection, packing (with the periodic shift) and the force fold-back
+are kernels of libdpb (csrc/dd.cu: dpb_dd_pack / dpb_dd_unpack / dpb_dd_add_forces) and the messages travel with
+torch.distributed point-to-point calls (NCCL over NVLink); one host synchronisation per stage (the message sizes).  For
+CPU tensors (the gloo tests of the routes) the same steps are torch indexing.  All arithmetic of the model runs in the
+`evaluate_local` callable — DPModel.eval_local in production; there is no CPU evaluation in this module.
 """
 from __future__ import annotations
 
@@ -88,6 +90,7 @@ class BrickDecomposition:
                 self.hi[c] = self.L[c]
         self.stages: List[_Stage] = []
         self.nloc = 0
+        self._bufs, self._x, self._t = {}, None, None               # device path: reused exchange buffers
         self._torch = torch
         self._dist = dist
 
@@ -178,6 +181,9 @@ class BrickDecomposition:
         torch = self._torch
         self.nloc = int(coord.shape[0])
         self.stages = []
+        if coord.is_cuda:
+            return self._forward_cuda(coord, types)
+        # CPU tensors (the gloo tests): the same selection, shifts and routes written with torch indexing
         x = coord
         t = types.to(torch.float64)
         for dim in range(3):
@@ -206,6 +212,8 @@ class BrickDecomposition:
     def reverse(self, force_all):
         """Reverse exchange: force_all [nall, 3] (local + ghost) -> force [nloc, 3] with every ghost increment added to
         its owner.  Stages in reverse order: what arrives may belong to a ghost of an earlier stage and travels on."""
+        if force_all.is_cuda:
+            return self._reverse_cuda(force_all)
         f = force_all.clone()
         for st in reversed(self.stages):
             (a0, a1), (b0, b1) = st.recv_range                    # a: came from the - neighbour, b: from the + neighbour
@@ -221,6 +229,85 @@ class BrickDecomposition:
                 f.index_add_(0, idx_minus, from_minus)
         assert f.shape[0] == self.nloc
         return f
+
+    # ---- device path: selection, packing and the force fold-back are kernels of libdpb (csrc/dd.cu) ------------------
+    def _buffers(self, dim: int, cap: int, dev):
+        torch = self._torch
+        b = self._bufs.get(dim)
+        if b is None or b["cap"] < cap:
+            b = {"cap": cap,
+                 "pack_minus": torch.empty((cap, 4), dtype=torch.float64, device=dev),
+                 "pack_plus": torch.empty((cap, 4), dtype=torch.float64, device=dev),
+                 "idx_minus": torch.empty(cap, dtype=torch.int32, device=dev),
+                 "idx_plus": torch.empty(cap, dtype=torch.int32, device=dev),
+                 "counts": torch.zeros(2, dtype=torch.int32, device=dev)}
+            self._bufs[dim] = b
+        return b
+
+    def _atoms(self, need: int, keep: int, dev):
+        """Atom arrays with room for `need` rows; the first `keep` rows survive a reallocation."""
+        torch = self._torch
+        if self._x is None or self._x.shape[0] < need or self._x.device != dev:
+            cap = int(need * 1.25) + 1024
+            x = torch.empty((cap, 3), dtype=torch.float64, device=dev)
+            t = torch.empty(cap, dtype=torch.int32, device=dev)
+            if keep:
+                x[:keep] = self._x[:keep]
+                t[:keep] = self._t[:keep]
+            self._x, self._t = x, t
+        return self._x, self._t
+
+    def _forward_cuda(self, coord, types):
+        from . import binding
+        torch = self._torch
+        dev = coord.device
+        n = self.nloc
+        width = self.hi - self.lo
+        grow = float(np.prod(1.0 + 2.0 * self.rcut / width))
+        x, t = self._atoms(int(n * grow * 1.1) + 1024, 0, dev)
+        x[:n] = coord
+        t[:n] = types
+        for dim in range(3):
+            lo, hi, L = float(self.lo[dim]), float(self.hi[dim]), float(self.L[dim])
+            shift_plus = -L if self.index[dim] == self.grid[dim] - 1 else 0.0
+            shift_minus = L if self.index[dim] == 0 else 0.0
+            cap = min(n, int(n * self.rcut / width[dim] * 1.3) + 256)
+            while True:
+                b = self._buffers(dim, cap, dev)
+                binding.dd_pack(x, t, n, dim, lo + self.rcut, hi - self.rcut, shift_minus, shift_plus, b["pack_minus"],
+                                b["idx_minus"], b["pack_plus"], b["idx_plus"], b["counts"])
+                km, kp = (int(v) for v in b["counts"].tolist())          # the one host synchronisation of the stage
+                if max(km, kp) <= b["cap"]:
+                    break
+                cap = max(km, kp)
+            to_plus, to_minus = b["pack_plus"][:kp], b["pack_minus"][:km]
+            if self.neighbour(dim, +1) == self.rank and self.neighbour(dim, -1) == self.rank:
+                from_minus, from_plus = to_plus, to_minus                 # the images of this brick's own atoms
+            else:
+                from_minus, from_plus = self._exchange(to_plus, to_minus, dim)
+            k0, k1 = int(from_minus.shape[0]), int(from_plus.shape[0])
+            x, t = self._atoms(n + k0 + k1, n, dev)
+            binding.dd_unpack(from_minus, k0, x[n:], t[n:])
+            binding.dd_unpack(from_plus, k1, x[n + k0:], t[n + k0:])
+            self.stages.append(_Stage(dim=dim, send_idx=[b["idx_plus"][:kp], b["idx_minus"][:km]],
+                                      recv_range=[(n, n + k0), (n + k0, n + k0 + k1)]))
+            n += k0 + k1
+        return x[:n], t[:n]
+
+    def _reverse_cuda(self, f):
+        """In place on the evaluator's force array (local + ghost rows); returns the view of the local rows."""
+        from . import binding
+        for st in reversed(self.stages):
+            (a0, a1), (b0, b1) = st.recv_range
+            idx_plus, idx_minus = st.send_idx
+            if self.neighbour(st.dim, +1) == self.rank and self.neighbour(st.dim, -1) == self.rank:
+                from_minus, from_plus = f[b0:b1], f[a0:a1]                # ghost rows lie behind every target row
+            else:
+                from_minus, from_plus = self._exchange_fixed(f[b0:b1], f[a0:a1], int(idx_minus.shape[0]),
+                                                             int(idx_plus.shape[0]), st.dim)
+            binding.dd_add_forces(idx_plus, from_plus, int(idx_plus.shape[0]), f)
+            binding.dd_add_forces(idx_minus, from_minus, int(idx_minus.shape[0]), f)
+        return f[:self.nloc]
 
     def evaluate(self, evaluate_local: Callable, coord, types):
         """One evaluation of the decomposed system.  `evaluate_local(coord_all, types_all, nloc, bounds)` must return a

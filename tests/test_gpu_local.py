@@ -210,3 +210,58 @@ def test_decomposition_driver_on_one_gpu(name):
     assert (out["force"] - per["force"]).abs().max().item() <= 2e-9
     assert (out["atom_energy"] - per["atom_energy"]).abs().max().item() <= 1e-10 * per["atom_energy"].abs().max().item()
     assert (out["virial"] - per["virial"]).abs().max().item() <= 1e-10 * max(1.0, per["virial"].abs().max().item())
+
+
+def test_exchange_kernels_against_numpy():
+    """dpb_dd_pack / dpb_dd_unpack / dpb_dd_add_forces (csrc/dd.cu) against the selection written in numpy: same rows
+    (as sets: the order inside a message is arbitrary), shifts applied by the sender, counts beyond the capacity reported
+    and nothing written past it, forces added at the packed indices."""
+    from paper_2004_11658_b200 import binding
+    torch = _torch()
+    rng = np.random.default_rng(12)
+    n = 5000
+    x = rng.uniform(0.0, 20.0, size=(n, 3))
+    t = rng.integers(0, 3, size=n).astype(np.int32)
+    dx, dt = torch.tensor(x, device="cuda"), torch.tensor(t, device="cuda")
+    for dim, (cm, cp, sm, sp) in enumerate([(4.0, 16.0, 20.0, -20.0), (3.0, 17.5, 0.0, 0.0), (12.0, 9.0, 20.0, 0.0)]):
+        want_m, want_p = np.nonzero(x[:, dim] < cm)[0], np.nonzero(x[:, dim] >= cp)[0]
+        cap = n
+        pm = torch.full((cap, 4), -7.0, dtype=torch.float64, device="cuda")
+        pp = torch.full((cap, 4), -7.0, dtype=torch.float64, device="cuda")
+        im = torch.full((cap,), -1, dtype=torch.int32, device="cuda")
+        ip = torch.full((cap,), -1, dtype=torch.int32, device="cuda")
+        cnt = torch.zeros(2, dtype=torch.int32, device="cuda")
+        binding.dd_pack(dx, dt, n, dim, cm, cp, sm, sp, pm, im, pp, ip, cnt)
+        km, kp = cnt.tolist()
+        assert (km, kp) == (len(want_m), len(want_p))
+        for pack, idx, k, want, shift in ((pm, im, km, want_m, sm), (pp, ip, kp, want_p, sp)):
+            got_idx = idx[:k].cpu().numpy()
+            assert np.array_equal(np.sort(got_idx), want)
+            rows = pack[:k].cpu().numpy()
+            exp = x[got_idx].copy()
+            exp[:, dim] += shift
+            assert np.array_equal(rows[:, :3], exp) and np.array_equal(rows[:, 3], t[got_idx].astype(np.float64))
+            assert (pack[k:] == -7.0).all() and (idx[k:] == -1).all()
+            # unpack and fold forces back
+            xo = torch.zeros((k, 3), dtype=torch.float64, device="cuda")
+            to = torch.zeros(k, dtype=torch.int32, device="cuda")
+            binding.dd_unpack(pack, k, xo, to)
+            assert np.array_equal(xo.cpu().numpy(), exp) and np.array_equal(to.cpu().numpy(), t[got_idx])
+            f = torch.tensor(rng.normal(size=(n, 3)), device="cuda")
+            f0 = f.cpu().numpy().copy()
+            fin = torch.tensor(rng.normal(size=(k, 3)), device="cuda")
+            binding.dd_add_forces(idx, fin, k, f)
+            f0[got_idx] += fin.cpu().numpy()
+            assert np.array_equal(f.cpu().numpy(), f0)
+        # capacity too small: counts still exact, nothing written beyond the capacity
+        small = 64
+        pm2 = torch.full((small + 8, 4), -7.0, dtype=torch.float64, device="cuda")
+        pp2 = torch.full((small + 8, 4), -7.0, dtype=torch.float64, device="cuda")
+        im2 = torch.full((small + 8,), -1, dtype=torch.int32, device="cuda")
+        ip2 = torch.full((small + 8,), -1, dtype=torch.int32, device="cuda")
+        binding.dd_pack(dx, dt, n, dim, cm, cp, sm, sp, pm2[:small], im2, pp2[:small], ip2, cnt)
+        assert cnt.tolist() == [len(want_m), len(want_p)] and len(want_m) > small
+        assert (pm2[small:] == -7.0).all() and (im2[small:] == -1).all() and (ip2[small:] == -1).all()
+    # empty input
+    binding.dd_pack(dx, dt, 0, 0, 1.0, 2.0, 0.0, 0.0, pm, im, pp, ip, cnt)
+    assert cnt.tolist() == [0, 0]
