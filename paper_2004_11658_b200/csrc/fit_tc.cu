@@ -278,43 +278,42 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
 // ---- S5: descriptor as the A image of G1 ---------------------------------------------------------------------------
 // D[b M^< + a] = sum_c T[b][c] T[a][c] (Eq. 4; reading R7), from the fp64 T rounded to fp32, written
 // straight into the hi / lo operand images (the descriptor never exists in another form).  Thread = atom (tile row).
-#define DESCR_BS 8
+#define DESCR_R 16                     // atoms per block
+// D = T (T^<)^T (Eq. 4) written directly as the A operand of G1 (hi / lo images).  A block stages the fp32 copy of its
+// atoms' T rows in shared memory (coalesced 16-byte loads of the contiguous fp64 rows), then walks (K panel, row, 16-byte
+// chunk) tasks with the chunk index fastest: eight lanes write one full 128-byte image row, a warp four adjacent rows =
+// 512 contiguous bytes per store (thread-per-row stores touched 32 separate lines, half a sector each).
 template <int MA>
-__global__ void __launch_bounds__(128) k_descr_tc(DevModel P, ChunkView C, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
-  const int tile = blockIdx.x, r = threadIdx.x, m = tile * 128 + r;
-  if (m >= C.n) return;
-  const double *T = C.T + (size_t)m * P.M * 4;
-  float ta[MA][4];
-#pragma unroll
-  for (int a = 0; a < MA; ++a) {
-    const double2 u = *reinterpret_cast<const double2 *>(T + 4 * a), v = *reinterpret_cast<const double2 *>(T + 4 * a + 2);
-    ta[a][0] = (float)u.x; ta[a][1] = (float)u.y; ta[a][2] = (float)v.x; ta[a][3] = (float)v.y;
-  }
-  // blockIdx.y splits the b range into slices of DESCR_BS rows (192 row tiles alone would leave most of the GPU idle);
-  // the slice's T rows are loaded up front: the image stores below may alias T as far as the compiler knows
-  const int b_lo = blockIdx.y * DESCR_BS;
-  float tb[DESCR_BS][4];
-#pragma unroll
-  for (int i = 0; i < DESCR_BS; ++i) {
-    const int b = min(b_lo + i, P.M - 1);
-    const double2 u = *reinterpret_cast<const double2 *>(T + 4 * b), v = *reinterpret_cast<const double2 *>(T + 4 * b + 2);
-    tb[i][0] = (float)u.x; tb[i][1] = (float)u.y; tb[i][2] = (float)v.x; tb[i][3] = (float)v.y;
-  }
-#pragma unroll
-  for (int i = 0; i < DESCR_BS; ++i) {
-    const int b = b_lo + i;
-    if (b >= P.M) break;
-#pragma unroll
-    for (int a = 0; a < MA; a += 4) {
-      float d[4];
-#pragma unroll
-      for (int k = 0; k < 4; ++k)
-        d[k] = fmaf(tb[i][0], ta[a + k][0], fmaf(tb[i][1], ta[a + k][1], fmaf(tb[i][2], ta[a + k][2], tb[i][3] * ta[a + k][3])));
-      img_store4(Dh, Dl, (size_t)tile, kpan, b * MA + a, r, d[0], d[1], d[2], d[3]);
+__global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
+  extern __shared__ float4 Ts[];                                   // [DESCR_R][M + 1]
+  const int row0 = blockIdx.x * DESCR_R, nrow = min(DESCR_R, C.n - row0), M = P.M, ld = M + 1;
+  {
+    const double2 *src = reinterpret_cast<const double2 *>(C.T + (size_t)row0 * M * 4);
+    float2 *dst = reinterpret_cast<float2 *>(Ts);
+    for (int k = threadIdx.x; k < nrow * M * 2; k += 256) {
+      const double2 v = src[k];
+      const int rl = k / (2 * M), w = k - rl * 2 * M;
+      dst[rl * 2 * ld + w] = make_float2((float)v.x, (float)v.y);
     }
   }
-  if (blockIdx.y == gridDim.y - 1)
-    for (int k = P.M * MA; k < kpan * FT_KP; k += 4) img_store4(Dh, Dl, (size_t)tile, kpan, k, r, 0.f, 0.f, 0.f, 0.f);
+  __syncthreads();
+  const int ntask = DESCR_R * kpan * 8, kreal = M * MA;
+  for (int q = threadIdx.x; q < ntask; q += 256) {
+    const int j = q & 7, rl = (q >> 3) & (DESCR_R - 1), pan = q / (8 * DESCR_R);
+    if (rl >= nrow) continue;
+    const int m = row0 + rl, k0 = pan * FT_KP + 4 * j;
+    float d[4] = {0.f, 0.f, 0.f, 0.f};                             // image columns between dim and the padded K are zero
+    if (k0 < kreal) {
+      const int b = k0 / MA, a0 = k0 - b * MA;
+      const float4 tb = Ts[rl * ld + b];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float4 ta = Ts[rl * ld + a0 + k];
+        d[k] = fmaf(tb.x, ta.x, fmaf(tb.y, ta.y, fmaf(tb.z, ta.z, tb.w * ta.w)));
+      }
+    }
+    img_store4(Dh, Dl, (size_t)(m >> 7), kpan, k0, m & 127, d[0], d[1], d[2], d[3]);
+  }
 }
 
 // ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c] (one of the S7 contractions: fp32
@@ -552,10 +551,14 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
   float *Z1 = p; p += rows * F->fwp;
   float *dZ1 = p; p += rows * F->fwp;
   float *dD = p;
-  switch (P.Ma) {
-    case 4: k_descr_tc<4><<<dim3((unsigned)tiles, (unsigned)((P.M + DESCR_BS - 1) / DESCR_BS)), 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
-    case 8: k_descr_tc<8><<<dim3((unsigned)tiles, (unsigned)((P.M + DESCR_BS - 1) / DESCR_BS)), 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
-    default: k_descr_tc<16><<<dim3((unsigned)tiles, (unsigned)((P.M + DESCR_BS - 1) / DESCR_BS)), 128, 0, st>>>(P, C, (int)kpd, Dh, Dl); break;
+  {
+    const unsigned nb = (unsigned)((C.n + DESCR_R - 1) / DESCR_R);
+    const size_t sm = (size_t)DESCR_R * (P.M + 1) * sizeof(float4);
+    switch (P.Ma) {
+      case 4: k_descr_tc<4><<<nb, 256, sm, st>>>(P, C, (int)kpd, Dh, Dl); break;
+      case 8: k_descr_tc<8><<<nb, 256, sm, st>>>(P, C, (int)kpd, Dh, Dl); break;
+      default: k_descr_tc<16><<<nb, 256, sm, st>>>(P, C, (int)kpd, Dh, Dl); break;
+    }
   }
   DPB_LAUNCHED(1);
   for (int ty = 0; ty < P.ntypes; ++ty) {
