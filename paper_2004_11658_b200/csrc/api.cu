@@ -24,6 +24,33 @@ static int fail(int code, const char *fmt, ...) {
 }
 
 unsigned long long g_dpb_launches = 0;
+
+cudaError_t dpb_fork_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]) {
+  static cudaStream_t aux[DPB_MAX_TYPES] = {};
+  static cudaEvent_t ev_fork = nullptr;
+  cudaError_t e;
+  s[0] = st;
+  if (ntypes <= 1) return cudaSuccess;
+  if (!ev_fork && (e = cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming)) != cudaSuccess) return e;
+  if ((e = cudaEventRecord(ev_fork, st)) != cudaSuccess) return e;
+  for (int ty = 1; ty < ntypes; ++ty) {
+    if (!aux[ty] && (e = cudaStreamCreateWithFlags(&aux[ty], cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(aux[ty], ev_fork, 0)) != cudaSuccess) return e;
+    s[ty] = aux[ty];
+  }
+  return cudaSuccess;
+}
+
+cudaError_t dpb_join_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]) {
+  static cudaEvent_t ev_join[DPB_MAX_TYPES] = {};
+  cudaError_t e;
+  for (int ty = 1; ty < ntypes; ++ty) {
+    if (!ev_join[ty] && (e = cudaEventCreateWithFlags(&ev_join[ty], cudaEventDisableTiming)) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(ev_join[ty], s[ty])) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(st, ev_join[ty], 0)) != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
 extern "C" int64_t dpb_kernel_launches(void) { return (int64_t)g_dpb_launches; }
 
 extern "C" const char *dpb_last_error(void) { return g_err; }

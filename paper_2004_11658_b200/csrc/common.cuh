@@ -65,6 +65,12 @@ struct ChunkView {
   double *fslot;           // deterministic mode: [n][nm][3] dE_i/dd_ik per slot (pass 2 stores instead of scattering)
 };
 
+// The per-type fitting chains are independent (disjoint rows) and one type's GEMM launch fills only as many SMs as that
+// type has row tiles; they run on forked streams so that the types share the GPU.  fork: s[0] = st, s[ty > 0] = auxiliary
+// streams that wait for everything enqueued on st so far; join: st waits for everything enqueued on them.
+cudaError_t dpb_fork_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]);
+cudaError_t dpb_join_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]);
+
 // dd.cu: pack / unpack kernels of the domain decomposition's ghost exchange
 cudaError_t launch_dd_pack(int64_t n, const double *coord, const int *type, int dim, double cut_minus, double cut_plus,
                            double shift_minus, double shift_plus, int64_t cap, double *pack_minus, int *idx_minus,

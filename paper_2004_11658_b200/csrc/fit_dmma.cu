@@ -352,30 +352,36 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
 
   k_descr_v1<<<C.n, 256, 0, st>>>(P, C, dimp, D);
   DPB_LAUNCHED(1);
-  for (int ty = 0; ty < P.ntypes; ++ty) {
+  // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint
+  cudaStream_t ts[DPB_MAX_TYPES];
+  if ((e = dpb_fork_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
+  for (int k = 0; k < P.ntypes; ++k) {
+    const int ty = P.ntypes - 1 - k;
+    cudaStream_t s = ts[k];
     const FitNet &N = F->nets[ty];
     GemmArgs g;
     // G1: Z0 = tanh(D W0 + b0)
     g = GemmArgs{D, dimp, N.W0, fwp, dimp, fwp, N.b0, nullptr, nullptr, fwp, Z0, nullptr, fwp};
-    if ((e = gemm<15, EPI_TANH>(C, ty, g, st)) != cudaSuccess) return e;
+    if ((e = gemm<15, EPI_TANH>(C, ty, g, s)) != cudaSuccess) return e;
     // G2: U1 = tanh(Z0 W1 + b1); Z1 = Z0 + U1
     g = GemmArgs{Z0, fwp, N.W1, fwp, fwp, fwp, N.b1, Z0, nullptr, fwp, U1, Z1, fwp};
-    if ((e = gemm<15, EPI_TANH_SKIP>(C, ty, g, st)) != cudaSuccess) return e;
+    if ((e = gemm<15, EPI_TANH_SKIP>(C, ty, g, s)) != cudaSuccess) return e;
     // G3: U2 = tanh(Z1 W2 + b2); Z2 = Z1 + U2; Q = w3 (1 - U2^2)
     g = GemmArgs{Z1, fwp, N.W2, fwp, fwp, fwp, N.b2, Z1, N.w3, fwp, Q, Z2, fwp};
-    if ((e = gemm<15, EPI_L3>(C, ty, g, st)) != cudaSuccess) return e;
-    k_rowdot_v1<<<(C.n + 7) / 8, 256, 0, st>>>(C, ty, fwp, Z2, N.w3, N.b3, atom_energy);
+    if ((e = gemm<15, EPI_L3>(C, ty, g, s)) != cudaSuccess) return e;
+    k_rowdot_v1<<<(C.n + 7) / 8, 256, 0, s>>>(C, ty, fwp, Z2, N.w3, N.b3, atom_energy);
     DPB_LAUNCHED(1);
     // G4: dZ1 = w3 + Q W2^T (-> Z1 buffer); Q' = dZ1 (1 - U1^2)
     g = GemmArgs{Q, fwp, N.W2T, fwp, fwp, fwp, N.w3, nullptr, U1, fwp, Z1, Q2, fwp};
-    if ((e = gemm<15, EPI_BWD>(C, ty, g, st)) != cudaSuccess) return e;
+    if ((e = gemm<15, EPI_BWD>(C, ty, g, s)) != cudaSuccess) return e;
     // G5: dZ0 = dZ1 + Q' W1^T; Q = dZ0 (1 - Z0^2)
     g = GemmArgs{Q2, fwp, N.W1T, fwp, fwp, fwp, nullptr, Z1, Z0, fwp, nullptr, Q, fwp};
-    if ((e = gemm<15, EPI_BWD>(C, ty, g, st)) != cudaSuccess) return e;
+    if ((e = gemm<15, EPI_BWD>(C, ty, g, s)) != cudaSuccess) return e;
     // G6: dD = Q W0^T
     g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
-    if ((e = gemm<8, EPI_STORE>(C, ty, g, st)) != cudaSuccess) return e;
+    if ((e = gemm<8, EPI_STORE>(C, ty, g, s)) != cudaSuccess) return e;
   }
+  if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
   const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
   static size_t configured = 0;
   if (sm > 48 * 1024 && sm > configured) {

@@ -562,26 +562,16 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
   }
   DPB_LAUNCHED(1);
   // The per-type GEMM chains are independent (disjoint rows; a tile on the type boundary is read by both and written
-  // row-wise by each) and G1-G5 of one type fill only as many SMs as that type has row tiles (W24k: 64 and 128 of 148).
-  // Run the chains on separate streams so that one type's CTAs take the SMs the other leaves idle; fork / join by events.
-  static cudaStream_t aux[DPB_MAX_TYPES] = {};
-  static cudaEvent_t ev_fork = nullptr, ev_join[DPB_MAX_TYPES] = {};
-  const bool fork = P.ntypes > 1;
-  if (fork) {
-    cudaError_t e;
-    if (!ev_fork && (e = cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming)) != cudaSuccess) return e;
-    for (int ty = 1; ty < P.ntypes; ++ty) {
-      if (!aux[ty] && (e = cudaStreamCreateWithFlags(&aux[ty], cudaStreamNonBlocking)) != cudaSuccess) return e;
-      if (!ev_join[ty] && (e = cudaEventCreateWithFlags(&ev_join[ty], cudaEventDisableTiming)) != cudaSuccess) return e;
-    }
-    if ((e = cudaEventRecord(ev_fork, st)) != cudaSuccess) return e;
-    for (int ty = 1; ty < P.ntypes; ++ty)
-      if ((e = cudaStreamWaitEvent(aux[ty], ev_fork, 0)) != cudaSuccess) return e;
+  // row-wise by each) and G1-G5 of one type fill only as many SMs as that type has row tiles (W24k: 64 and 128 of 148):
+  // forked streams let one type's CTAs take the SMs the other leaves idle.  Largest type (last) on the caller's stream.
+  cudaStream_t ts[DPB_MAX_TYPES];
+  {
+    cudaError_t e = dpb_fork_streams(P.ntypes, st, ts);
+    if (e != cudaSuccess) return e;
   }
-  // largest type first on the caller's stream
   for (int k = 0; k < P.ntypes; ++k) {
     const int ty = P.ntypes - 1 - k;
-    cudaStream_t s = (fork && ty > 0) ? aux[ty] : st;
+    cudaStream_t s = ts[k];
     cudaError_t e;
     switch (F->NT) {
       case 32: e = ft_run_type<32>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
@@ -591,13 +581,11 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
       default: e = ft_run_type<256>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
     }
     if (e != cudaSuccess) return e;
-    if (fork && ty > 0 && (e = cudaEventRecord(ev_join[ty], s)) != cudaSuccess) return e;
   }
-  if (fork)
-    for (int ty = 1; ty < P.ntypes; ++ty) {
-      cudaError_t e = cudaStreamWaitEvent(st, ev_join[ty], 0);
-      if (e != cudaSuccess) return e;
-    }
+  {
+    cudaError_t e = dpb_join_streams(P.ntypes, st, ts);
+    if (e != cudaSuccess) return e;
+  }
   const int log2ma = P.Ma == 4 ? 2 : (P.Ma == 8 ? 3 : 4);
   const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma + ((size_t)P.M * (P.Ma + 1) + 3) / 4);
   static size_t configured = 0;

@@ -121,7 +121,6 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
 // Cells are numbered z-fastest, so the three z-neighbours of a stencil column are one contiguous run of sorted
 // positions (two runs when the column wraps around the box): 9 x 2 entries per type instead of 27.
 #define NL_THREADS 128
-#define NL_ENTRIES (2 * 18 * DPB_MAX_TYPES)       // x 2: local and ghost groups of the sub-region mode
 #define NL_BUCKETS 32           // distance buckets per type, uniform in r^3: the ranking only compares inside a bucket
 
 struct __align__(16) NlHit { double r; int j; int t; };
@@ -131,7 +130,7 @@ struct __align__(16) NlHit { double r; int j; int t; };
 // candidate within r_c + skin is also appended to the atom's raw list (the paper's LAMMPS skin list, PAPER.md:193,
 // :298).  MODE 2 (MD, reuse step): candidates are the raw list — Alg. 1 proper: format a raw list.
 template <int MODE>
-__global__ void __launch_bounds__(NL_THREADS)
+__global__ void __launch_bounds__(NL_THREADS, MODE == 0 ? 10 : 1)   // 48 registers: 10 blocks per SM (64 gave 8: +11 %)
 k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, const int *__restrict__ start, int cap,
         int *__restrict__ nlist_out, DevStats *stats, NlRaw R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -139,7 +138,8 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
   int *hp = reinterpret_cast<int *>(hit + cap);                   // [cap] sorted position of j
   int *order = hp + cap;                                          // [cap] hits grouped by (type, distance bucket)
   __shared__ int bcnt[DPB_MAX_TYPES * NL_BUCKETS], bstart[DPB_MAX_TYPES * NL_BUCKETS + 1];
-  __shared__ int r_start[NL_ENTRIES], r_pref[NL_ENTRIES + 1], r_type[NL_ENTRIES];
+  const int nent_all = 18 * P.ntypes * G.ngrp;                    // stencil ranges: sized by the launcher
+  int *r_start = order + cap, *r_pref = r_start + nent_all, *r_type = r_pref + nent_all + 1;
   __shared__ int n_ranges, n_hit, n_raw, cnt[DPB_MAX_TYPES];
 
   const int tid = threadIdx.x, lane = tid & 31;
@@ -170,7 +170,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
     else if (lo[2] < 0) { z0 = 0; len0 = 2; z1 = G.nc[2] - 1; len1 = 1; }
     else if (lo[2] + 2 >= G.nc[2]) { z0 = lo[2]; len0 = 2; z1 = 0; len1 = 1; }
     else { z0 = lo[2]; len0 = 3; }
-    const int nent = 18 * P.ntypes * G.ngrp;
+    const int nent = nent_all;
     int nr = 0, run = 0;
     for (int base = 0; base < nent; base += 32) {
       const int ent = base + lane;
@@ -338,7 +338,7 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
                          const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode,
                          const NlRaw *raw) {
   if (C.n <= 0) return cudaSuccess;
-  const size_t smem = (size_t)cap * (sizeof(NlHit) + 2 * sizeof(int));
+  const size_t smem = (size_t)cap * (sizeof(NlHit) + 2 * sizeof(int)) + sizeof(int) * (3 * 18 * (size_t)P.ntypes * G.ngrp + 1);
   static size_t configured = 0;
   if (smem > 48 * 1024 && smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_nlist<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
