@@ -479,12 +479,18 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
     configured = true;
   }
   const int grid = min(g_sm_count, (C.n + P1_WARPS - 1) / P1_WARPS);
+  // nets of one centre type a accumulate into the same T rows (t = 0 stores, t > 0 adds): one stream per a, so that the
+  // tail of one launch overlaps the start of another centre type's
+  cudaStream_t ts[DPB_MAX_TYPES];
+  cudaError_t e = dpb_fork_streams(P.ntypes, st, ts);
+  if (e != cudaSuccess) return e;
   for (int a = 0; a < P.ntypes; ++a)
     for (int t = 0; t < P.ntypes; ++t) {
-      k_pass1_dmma<SP, 1><<<grid, (32 * P1_WARPS), smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
-                                                        t > 0);
+      k_pass1_dmma<SP, 1><<<grid, (32 * P1_WARPS), smem, ts[P.ntypes - 1 - a]>>>(
+          P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t, t > 0);
       DPB_LAUNCHED(1);
     }
+  if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
   return cudaGetLastError();
 }
 
@@ -500,12 +506,20 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     configured = true;
   }
   const int grid = min(g_sm_count, (C.n + P2_WARPS - 1) / P2_WARPS);
-  for (int a = 0; a < P.ntypes; ++a)
-    for (int t = 0; t < P.ntypes; ++t) {
-      k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, st>>>(P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t,
-                                                        force, virial);
+  // the nets are independent here (forces and virial are atomic sums, slot stores are disjoint): a stream per net, so
+  // that the tail of every launch is filled by the others
+  cudaStream_t ts[DPB_MAX_TYPES];
+  const int ns = min(P.ntypes * P.ntypes, DPB_MAX_TYPES);
+  cudaError_t e = dpb_fork_streams(ns, st, ts);
+  if (e != cudaSuccess) return e;
+  for (int a = P.ntypes - 1; a >= 0; --a)
+    for (int t = P.ntypes - 1; t >= 0; --t) {
+      const int net = a * P.ntypes + t;
+      k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, ts[(P.ntypes * P.ntypes - 1 - net) % ns]>>>(
+          P, C, W.emb + (size_t)net * W.net_stride, a, t, force, virial);
       DPB_LAUNCHED(1);
     }
+  if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;
   return cudaGetLastError();
 }
 
