@@ -407,36 +407,52 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       const float4 *et = reinterpret_cast<const float4 *>(envt);       // [4][32]: component c, rows 4 k .. 4 k + 3
       const int sw = b & 7;
       int row = 0;
+      float2 s01 = make_float2(0.f, 0.f), s23 = s01;
+      double a0, a1, a2, a3;
+      auto step = [&](int k, const float4 g4) {
+        const float4 e0 = et[k], e1 = et[32 + k], e2 = et[64 + k], e3 = et[96 + k];
+        s01 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e0.x, e1.x), s01);
+        s23 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e2.x, e3.x), s23);
+        s01 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e0.y, e1.y), s01);
+        s23 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e2.y, e3.y), s23);
+        s01 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e0.z, e1.z), s01);
+        s23 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e2.z, e3.z), s23);
+        s01 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e0.w, e1.w), s01);
+        s23 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e2.w, e3.w), s23);
+      };
+      auto flush = [&]() {
+        a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
+        s01 = make_float2(0.f, 0.f); s23 = s01;
+      };
+      auto masked_step = [&](int k, int lo_row, int hi_row) {   // a step cut by a segment boundary
+        float4 g4 = grow[k ^ sw];
+        const int r0 = 4 * k;
+        if (r0 < lo_row || r0 >= hi_row) g4.x = 0.f;
+        if (r0 + 1 < lo_row || r0 + 1 >= hi_row) g4.y = 0.f;
+        if (r0 + 2 < lo_row || r0 + 2 >= hi_row) g4.z = 0.f;
+        if (r0 + 3 < lo_row || r0 + 3 >= hi_row) g4.w = 0.f;
+        step(k, g4);
+        flush();
+      };
       while (row < nrows) {
         const int cur = ids[row];
         const int se = segs[row];                           // end row of this atom's segment; bit 8: whole section in the tile
         const int hi = se & 255;
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        float2 s01 = make_float2(0.f, 0.f), s23 = s01;
-        for (int k = row >> 2; 4 * k < hi; ++k) {
-          float4 g4 = grow[k ^ sw];
-          const int r0 = 4 * k;
-          if (r0 < row || r0 + 4 > hi) {                    // uniform over the warp: boundary step
-            if (r0 < row || r0 >= hi) g4.x = 0.f;
-            if (r0 + 1 < row || r0 + 1 >= hi) g4.y = 0.f;
-            if (r0 + 2 < row || r0 + 2 >= hi) g4.z = 0.f;
-            if (r0 + 3 < row || r0 + 3 >= hi) g4.w = 0.f;
-          }
-          const float4 e0 = et[k], e1 = et[32 + k], e2 = et[64 + k], e3 = et[96 + k];
-          s01 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e0.x, e1.x), s01);
-          s23 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e2.x, e3.x), s23);
-          s01 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e0.y, e1.y), s01);
-          s23 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e2.y, e3.y), s23);
-          s01 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e0.z, e1.z), s01);
-          s23 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e2.z, e3.z), s23);
-          s01 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e0.w, e1.w), s01);
-          s23 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e2.w, e3.w), s23);
-          if (k & 1) {
-            a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
-            s01 = make_float2(0.f, 0.f); s23 = s01;
-          }
+        a0 = 0.0; a1 = 0.0; a2 = 0.0; a3 = 0.0;
+        // whole steps [kb, ke) in a branch-free loop (two steps = 8 rows per fp64 flush); the at most two steps that a
+        // segment boundary cuts go through the masked path (uniform over the warp)
+        int kb = row >> 2;
+        const int ke = hi >> 2;
+        if (row & 3) { masked_step(kb, row, hi); ++kb; }
+        if ((hi & 3) && ke >= kb) masked_step(ke, row, hi);
+        int k = kb;
+        for (; k + 2 <= ke; k += 2) {
+          const float4 ga = grow[k ^ sw], gb = grow[(k + 1) ^ sw];
+          step(k, ga);
+          step(k + 1, gb);
+          flush();
         }
-        a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
+        if (k < ke) { step(k, grow[k ^ sw]); flush(); }
         double *dst = C.T + ((size_t)cur * P.M + b) * 4;
         if (P.ntypes == 1 && (se & 256)) {
           // one net only and the whole section of this atom lies inside the tile: nobody else writes T[cur][b][:]
