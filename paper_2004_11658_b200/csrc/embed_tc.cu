@@ -273,8 +273,8 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       segs[wt] = min(nrows, seg_hi) | ((seg_lo >= 0 && seg_hi <= 128) ? 256 : 0);
     }
     {
-      float *ef = reinterpret_cast<float *>(envt);            // transposed: [component][row]
-      ef[wt] = (float)e[0]; ef[128 + wt] = (float)e[1]; ef[256 + wt] = (float)e[2]; ef[384 + wt] = (float)e[3];
+      // [row][component]: one broadcast 16-byte load gives the accumulation (e0, e1) and (e2, e3) as register pairs
+      envt[wt] = make_float4((float)e[0], (float)e[1], (float)e[2], (float)e[3]);
     }
     const float x = (float)e[0];
     // layer 0 (Eq. 8): h0 = tanh(x W0 + b0)
@@ -398,27 +398,27 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       if (nx_valid) { nx_idx = pidx_t[pn]; nx_dv = C.dr[nx_idx]; }
     }
     // S5: T_i += sum_rows g (x) R~.  Thread b owns feature b; rows are grouped by centre atom (segments, from the pair
-    // offsets).  Four rows per step: one 16-byte load of gT, four broadcast loads of the transposed R~ tile, eight
+    // offsets).  Four rows per step: one 16-byte load of gT, four broadcast loads of R~ rows (e0..e3 adjacent), eight
     // packed FMAs (FFMA2); products and partial sums of up to 8 rows in fp32, accumulation across them in fp64
     // (DESIGN.md "Mixed precision"); steps cut by a segment boundary take the masked path.
     if (wt < 4 * S1) {
       const int b = wt;
       const float4 *grow = reinterpret_cast<const float4 *>(gt + b * 128);
-      const float4 *et = reinterpret_cast<const float4 *>(envt);       // [4][32]: component c, rows 4 k .. 4 k + 3
+      const float4 *et = reinterpret_cast<const float4 *>(envt);       // [128]: R~ row of tile row r
       const int sw = b & 7;
       int row = 0;
       float2 s01 = make_float2(0.f, 0.f), s23 = s01;
       double a0, a1, a2, a3;
       auto step = [&](int k, const float4 g4) {
-        const float4 e0 = et[k], e1 = et[32 + k], e2 = et[64 + k], e3 = et[96 + k];
-        s01 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e0.x, e1.x), s01);
-        s23 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(e2.x, e3.x), s23);
-        s01 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e0.y, e1.y), s01);
-        s23 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(e2.y, e3.y), s23);
-        s01 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e0.z, e1.z), s01);
-        s23 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(e2.z, e3.z), s23);
-        s01 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e0.w, e1.w), s01);
-        s23 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(e2.w, e3.w), s23);
+        const float4 r0 = et[4 * k], r1 = et[4 * k + 1], r2 = et[4 * k + 2], r3 = et[4 * k + 3];
+        s01 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(r0.x, r0.y), s01);
+        s23 = tc::ffma2(make_float2(g4.x, g4.x), make_float2(r0.z, r0.w), s23);
+        s01 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(r1.x, r1.y), s01);
+        s23 = tc::ffma2(make_float2(g4.y, g4.y), make_float2(r1.z, r1.w), s23);
+        s01 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(r2.x, r2.y), s01);
+        s23 = tc::ffma2(make_float2(g4.z, g4.z), make_float2(r2.z, r2.w), s23);
+        s01 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(r3.x, r3.y), s01);
+        s23 = tc::ffma2(make_float2(g4.w, g4.w), make_float2(r3.z, r3.w), s23);
       };
       auto flush = [&]() {
         a0 += (double)s01.x; a1 += (double)s01.y; a2 += (double)s23.x; a3 += (double)s23.y;
