@@ -113,6 +113,7 @@ class DPModel:
         self.ntypes = int(ntypes)
         self.sel = np.ascontiguousarray(sel, dtype=np.int32)
         self.nm = int(self.sel.sum())
+        self.rcut, self.rcut_smth = float(rcut), float(rcut_smth)
         self.s1, self.m_axis, self.fit_width = int(emb_s1), int(m_axis), int(fit_width)
         self.M = 4 * self.s1
         self.dim = self.M * self.m_axis

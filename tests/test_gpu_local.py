@@ -265,3 +265,47 @@ def test_exchange_kernels_against_numpy():
     # empty input
     binding.dd_pack(dx, dt, 0, 0, 1.0, 2.0, 0.0, 0.0, pm, im, pp, ip, cnt)
     assert cnt.tolist() == [0, 0]
+
+
+def test_triclinic_cell_through_explicit_images():
+    """paper_2004_11658_b200.cell.eval_cell: (1) a genuinely triclinic cell, thinner than 2 r_c
+    along c, against the oracle's dpo_eval_local on images built by brute force (tests/test_oracle_local.py);
+    (2) W192 described by the sheared cell (a1, a2 + a1, a3 + a2 - a1) against dpb_eval on the orthorhombic box."""
+    import paper_2004_11658_b200 as pk
+    from paper_2004_11658_b200.cell import eval_cell
+    from oracle import Oracle
+    from test_oracle_local import _brute_images
+    torch = _torch()
+    spec, emb, fit = small_model(ntypes=2, s1=8, m_axis=4, fit_width=16, sel=(40, 60), rcut=4.0, rcut_smth=1.0, seed=5,
+                                 fit_scale=0.05)
+    cell = np.array([[9.0, 0.0, 0.0], [2.5, 8.0, 0.0], [1.0, -1.5, 3.6]])
+    rng = np.random.default_rng(8)
+    x = rng.uniform(0, 1, size=(40, 3)) @ cell
+    t = rng.integers(0, 2, size=40).astype(np.int32)
+    orc = Oracle.from_spec(spec, emb, fit)
+    xi, own = _brute_images(x, cell, spec.rcut)
+    ref = orc.eval_local(xi, t[own], 40, want_nlist=False)
+    fref = np.zeros((40, 3))
+    np.add.at(fref, own, ref["force"])
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    got = eval_cell(m, torch.tensor(x, device="cuda"), torch.tensor(t, device="cuda"), cell)
+    torch.cuda.synchronize()
+    assert abs(got["energy"].item() - ref["energy"]) <= 1e-10 * abs(ref["energy"])
+    assert np.abs(got["atom_energy"].cpu().numpy() - ref["atom_energy"]).max() <= 1e-10 * np.abs(ref["atom_energy"]).max()
+    assert np.abs(got["force"].cpu().numpy() - fref).max() <= 1e-9
+    assert np.abs(got["virial"].cpu().numpy() - ref["virial"]).max() <= 1e-10 * max(1.0, np.abs(ref["virial"]).max())
+    m.close()
+    # (2)
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda")
+    per = m.eval(dc, dt, box)
+    a = np.asarray(box).reshape(3, 3)
+    got = eval_cell(m, dc, dt, np.array([a[0], a[1] + a[0], a[2] + a[1] - a[0]]))
+    torch.cuda.synchronize()
+    assert abs(got["energy"].item() - per["energy"].item()) <= 1e-10 * abs(per["energy"].item())
+    assert (got["force"] - per["force"]).abs().max().item() <= 2e-9
+    assert (got["virial"] - per["virial"]).abs().max().item() <= 1e-10 * max(1.0, per["virial"].abs().max().item())

@@ -150,3 +150,74 @@ def test_degenerate_cases():
     a, b = o.eval_local(coord, types, len(coord)), o.eval_local(x, t, len(coord))
     assert a["energy"] == b["energy"] and np.array_equal(a["force"], b["force"][:len(coord)])
     assert not b["force"][len(coord):].any()
+
+
+# ---- general periodic cells through explicit images (paper_2004_11658_b200/cell.py) ----------
+def _brute_images(coord, cell, rc, shells=2):
+    """Every lattice image (|n_c| <= shells) that has some atom of the cell within rc: O(N^2), independent of cell.py."""
+    a = np.asarray(cell).reshape(3, 3)
+    s = coord @ np.linalg.inv(a)
+    w = (s - np.floor(s)) @ a
+    xs, own = [w], [np.arange(len(w))]
+    for n in itertools.product(range(-shells, shells + 1), repeat=3):
+        if n == (0, 0, 0):
+            continue
+        x = w + np.array(n) @ a
+        d2 = ((x[:, None, :] - w[None, :, :]) ** 2).sum(-1).min(axis=1)
+        idx = np.nonzero(d2 <= rc * rc)[0]
+        xs.append(x[idx])
+        own.append(idx)
+    return np.concatenate(xs), np.concatenate(own)
+
+
+def _eval_cell_with_oracle(o, coord, types, cell, rc, images):
+    x, own = images(coord, cell, rc)
+    r = o.eval_local(x, types[own], len(coord), want_nlist=False)
+    f = np.zeros((len(coord), 3))
+    np.add.at(f, own, r["force"])
+    return r["energy"], r["atom_energy"], f, r["virial"], len(x)
+
+
+def _cellpy_images(coord, cell, rc):
+    import torch
+    from paper_2004_11658_b200.cell import periodic_images
+    x, own, (lo, hi) = periodic_images(torch.from_numpy(np.ascontiguousarray(coord)), cell, rc)
+    x = x.numpy()
+    assert (x >= lo).all() and (x <= hi).all()                       # the bounds handed to dpb_eval_local hold them all
+    return x, own.numpy()
+
+
+def test_sheared_description_of_an_orthorhombic_lattice():
+    """The cells (a1, a2, a3), (a1, a2 + a1, a3) and (a1, a2 + a1, a3 + a2 - a1) generate the same lattice, so E, E_i,
+    F and the virial from explicit images of the sheared (triclinic) cells must equal the orthorhombic periodic
+    evaluation; both image builders (brute force here, cell.py's fractional-coordinate margins) are checked."""
+    spec, emb, fit, coord, types, box = _setup()
+    o = Oracle.from_spec(spec, emb, fit)
+    ref = o.eval(coord, types, box)
+    a = np.asarray(box).reshape(3, 3)
+    cells = [a, np.array([a[0], a[1] + a[0], a[2]]), np.array([a[0], a[1] + a[0], a[2] + a[1] - a[0]])]
+    for cell in cells:
+        for images in (_brute_images, _cellpy_images):
+            E, Ei, F, V, nall = _eval_cell_with_oracle(o, coord, types, cell, spec.rcut, images)
+            assert abs(E - ref["energy"]) < 1e-12 * abs(ref["energy"])
+            assert np.abs(Ei - ref["atom_energy"]).max() < 1e-12 * np.abs(ref["atom_energy"]).max()
+            assert np.abs(F - ref["force"]).max() < 1e-11 * max(1.0, np.abs(ref["force"]).max())
+            assert np.abs(V - ref["virial"]).max() < 1e-10 * max(1.0, np.abs(ref["virial"]).max())
+
+
+def test_cell_images_thin_cell_and_heights():
+    """cell.py against the brute-force images on a genuinely triclinic cell thinner than 2 r_c in one direction
+    (two image shells there), and the perpendicular heights of a sheared cell."""
+    from paper_2004_11658_b200.cell import cell_heights
+    spec, emb, fit, coord, types, box = _setup(n=30, L=9.0, seed=6)
+    o = Oracle.from_spec(spec, emb, fit)
+    cell = np.array([[9.0, 0.0, 0.0], [2.5, 8.0, 0.0], [1.0, -1.5, 3.6]])     # height along c: 3.6 < r_c = 4
+    assert np.allclose(cell_heights(cell), [9.0 * 8.0 * 3.6 / np.linalg.norm(np.cross(cell[1], cell[2])),
+                                            9.0 * 8.0 * 3.6 / np.linalg.norm(np.cross(cell[2], cell[0])), 3.6])
+    rng = np.random.default_rng(8)
+    x = rng.uniform(0, 1, size=(30, 3)) @ cell
+    a = _eval_cell_with_oracle(o, x, types, cell, spec.rcut, _brute_images)
+    b = _eval_cell_with_oracle(o, x, types, cell, spec.rcut, _cellpy_images)
+    assert b[4] >= a[4]                                             # cell.py keeps a superset of the needed images
+    assert abs(a[0] - b[0]) < 1e-12 * abs(a[0]) and np.abs(a[2] - b[2]).max() < 1e-11 and np.abs(a[3] - b[3]).max() < 1e-10
+    assert np.abs(b[2].sum(axis=0)).max() < 1e-10                   # periodic system: total force vanishes
