@@ -415,7 +415,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       CU(tc_build_pairs(P, C, m->pairs.p, st), "pair list");
       CU(tc_pass1(P, C, m->tcw, m->pairs.p, st), "pass1 tf32");
       if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);
-      CU(tc_fit(P, C, m->tcw, m->tcfit.p, m->dT32.as<float>(), ei, st), "fit tf32");
+      CU(tc_fit(P, C, m->tcw, m->tcfit.p, m->dT32.as<float>(), ei, st, m->dbgdT != nullptr), "fit tf32");
       CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
       if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
       CU(tc_pass2(P, C, m->tcw, m->pairs.p, m->dT32.as<float>(), force, virial, st), "pass2 tf32");

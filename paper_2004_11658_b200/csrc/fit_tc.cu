@@ -318,21 +318,24 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int k
 
 // ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c] (one of the S7 contractions: fp32
 // products and sums like the GEMMs), written as fp64 (debug / ABI view) and as the fp32 copy pass 2 reads.
-// One WARP per atom, no block barrier: the atom's dD row (row stride M^< + 1: conflict-free column access) and an fp32
-// copy of T are staged in the warp's shared-memory slice.  First term: lane = b, all four c (one broadcast float4 of
-// T[a] per a).  Second term: lane = (a, half of the b' range), halves combined by one shuffle.  M^< in {4, 8, 16}.
+// One WARP per atom, no block barrier: the atom's dD row (row stride M^< + 4 floats: 16-byte stores and row loads, the
+// 16-byte row loads of consecutive lanes fall into distinct bank quads) and an fp32 copy of T are staged in the warp's
+// shared-memory slice.  First term: lane = b, all four c (one broadcast float4 of T[a] per a).  Second term: lane =
+// (a, part of the b' range, interleaved), parts combined by shuffles.  M^< in {4, 8, 16}.  `dT64` (the fp64 view the
+// debug hook reads) is written only when asked for.
 #define DT_WARPS 8
 __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C, int ldd, int log2ma,
-                                                         const float *__restrict__ dD, float *__restrict__ dT32) {
+                                                         const float *__restrict__ dD, float *__restrict__ dT32,
+                                                         double *__restrict__ dT64) {
   extern __shared__ float4 sm4[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = blockIdx.x * DT_WARPS + warp;
   if (q >= C.n) return;
-  const int M = P.M, Ma = 1 << log2ma, dim = P.dim, ldr = Ma + 1;
+  const int M = P.M, Ma = 1 << log2ma, dim = P.dim, ldr = Ma + 4;
   const int per4 = M + Ma + (M * ldr + 3) / 4;                  // float4 per warp slice
   float4 *Ts = sm4 + warp * per4;                               // [M]   T[b][0..3] in fp32
   float4 *t2 = Ts + M;                                          // [Ma]  second term
-  float *dd = reinterpret_cast<float *>(t2 + Ma);               // [M][Ma + 1]
+  float *dd = reinterpret_cast<float *>(t2 + Ma);               // [M][Ma + 4]
   const double2 *T = reinterpret_cast<const double2 *>(C.T + (size_t)q * M * 4);
   for (int k = lane; k < M; k += 32) {
     const double2 u = T[2 * k], v = T[2 * k + 1];
@@ -342,15 +345,14 @@ __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C
   for (int k4 = lane; k4 < dim / 4; k4 += 32) {
     const float4 v = src[k4];
     const int k = 4 * k4, o = (k >> log2ma) * ldr + (k & (Ma - 1));      // 4 | Ma: the four values stay in one row
-    dd[o] = v.x; dd[o + 1] = v.y; dd[o + 2] = v.z; dd[o + 3] = v.w;
+    *reinterpret_cast<float4 *>(dd + o) = v;
   }
   __syncwarp();
   // second term: lane = a + Ma * h (h < 32 / Ma parts of the b' range)
   {
     const int a = lane & (Ma - 1), h = lane >> log2ma, parts = 32 >> log2ma;
-    const int perp = (M + parts - 1) / parts, lo = h * perp, hi = min(M, lo + perp);
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-    for (int bp = lo; bp < hi; ++bp) {
+    for (int bp = h; bp < M; bp += parts) {
       const float d = dd[bp * ldr + a];
       const float4 tv = Ts[bp];
       s0 = fmaf(d, tv.x, s0); s1 = fmaf(d, tv.y, s1); s2 = fmaf(d, tv.z, s2); s3 = fmaf(d, tv.w, s3);
@@ -363,17 +365,22 @@ __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C
   }
   __syncwarp();
   for (int b = lane; b < M; b += 32) {
-    const float *row = dd + b * ldr;
+    const float4 *row = reinterpret_cast<const float4 *>(dd + b * ldr);
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-    for (int a = 0; a < Ma; ++a) {
-      const float d = row[a];
-      const float4 tv = Ts[a];
-      s0 = fmaf(d, tv.x, s0); s1 = fmaf(d, tv.y, s1); s2 = fmaf(d, tv.z, s2); s3 = fmaf(d, tv.w, s3);
+    for (int a4 = 0; a4 < Ma / 4; ++a4) {
+      const float4 d = row[a4];
+      const float4 u0 = Ts[4 * a4], u1 = Ts[4 * a4 + 1], u2 = Ts[4 * a4 + 2], u3 = Ts[4 * a4 + 3];
+      s0 = fmaf(d.x, u0.x, s0); s1 = fmaf(d.x, u0.y, s1); s2 = fmaf(d.x, u0.z, s2); s3 = fmaf(d.x, u0.w, s3);
+      s0 = fmaf(d.y, u1.x, s0); s1 = fmaf(d.y, u1.y, s1); s2 = fmaf(d.y, u1.z, s2); s3 = fmaf(d.y, u1.w, s3);
+      s0 = fmaf(d.z, u2.x, s0); s1 = fmaf(d.z, u2.y, s1); s2 = fmaf(d.z, u2.z, s2); s3 = fmaf(d.z, u2.w, s3);
+      s0 = fmaf(d.w, u3.x, s0); s1 = fmaf(d.w, u3.y, s1); s2 = fmaf(d.w, u3.z, s2); s3 = fmaf(d.w, u3.w, s3);
     }
     if (b < Ma) { const float4 u = t2[b]; s0 += u.x; s1 += u.y; s2 += u.z; s3 += u.w; }
-    double2 *o = reinterpret_cast<double2 *>(C.dT + ((size_t)q * M + b) * 4);
-    o[0] = make_double2((double)s0, (double)s1);
-    o[1] = make_double2((double)s2, (double)s3);
+    if (dT64) {
+      double2 *o = reinterpret_cast<double2 *>(dT64 + ((size_t)q * M + b) * 4);
+      o[0] = make_double2((double)s0, (double)s1);
+      o[1] = make_double2((double)s2, (double)s3);
+    }
     reinterpret_cast<float4 *>(dT32)[(size_t)q * M + b] = make_float4(s0, s1, s2, s3);
   }
 }
@@ -532,7 +539,7 @@ static cudaError_t ft_run_type(const DevModel &P, const ChunkView &C, const FitT
 }
 
 cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
-                   cudaStream_t st) {
+                   cudaStream_t st, bool want_dT64) {
   if (C.n <= 0) return cudaSuccess;
   const FitTC *F = reinterpret_cast<const FitTC *>(W.fit);
   if (!F) return cudaErrorNotSupported;
@@ -587,14 +594,14 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
     if (e != cudaSuccess) return e;
   }
   const int log2ma = P.Ma == 4 ? 2 : (P.Ma == 8 ? 3 : 4);
-  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma + ((size_t)P.M * (P.Ma + 1) + 3) / 4);
+  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma + ((size_t)P.M * (P.Ma + 4) + 3) / 4);
   static size_t configured = 0;
   if (sm > 48 * 1024 && sm > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_dT_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     configured = sm;
   }
-  k_dT_tc<<<(C.n + DT_WARPS - 1) / DT_WARPS, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, log2ma, dD, dT32);
+  k_dT_tc<<<(C.n + DT_WARPS - 1) / DT_WARPS, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, log2ma, dD, dT32, want_dT64 ? C.dT : nullptr);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }

@@ -27,4 +27,4 @@ cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W)
 void tc_release_fit(TCWeights &W);
 size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk);
 cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
-                   cudaStream_t st);
+                   cudaStream_t st, bool want_dT64);   // want_dT64: also write C.dT (fp64 view of dT for the debug hook)
