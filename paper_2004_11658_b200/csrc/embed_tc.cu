@@ -716,7 +716,8 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     }
     tc::bar_sync(1 + wg, 128);
     // epilogue: g = (h1, h1) + t2, g' = (h1', h1') + (1 - t2^2) (h1' W2); dots with the atom's dT rows
-    float pr0 = 0.f, pr1 = 0.f, pr2 = 0.f, pr3 = 0.f, dx = 0.f;
+    // packed FMAs: (pr0, pr1), (pr2, pr3) += g dT[o][:]; (q0, q1), (q2, q3) += g' dT[o][:], dotted with R~ at the end
+    float2 pr01 = make_float2(0.f, 0.f), pr23 = pr01, q01 = pr01, q23 = pr01;
     const bool staged = valid && qa - qa0 < nat;
     const float4 *dTrow = staged ? stage + (qa - qa0) * (4 * S1) : dT4 + (size_t)(valid ? qa : 0) * P.M;
     {
@@ -743,9 +744,10 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
             const float gv = h1v[o % (2 * S1)] + t2;
             const float gp = fmaf(d2, __uint_as_float(w[i]), h1t[o % (2 * S1)]);
             const float4 d4 = dTrow[o];
-            pr0 = fmaf(d4.x, gv, pr0); pr1 = fmaf(d4.y, gv, pr1); pr2 = fmaf(d4.z, gv, pr2); pr3 = fmaf(d4.w, gv, pr3);
-            const float dg = fmaf(d4.x, e0, fmaf(d4.y, e1, fmaf(d4.z, e2, d4.w * e3)));
-            dx = fmaf(dg, gp, dx);
+            pr01 = tc::ffma2(make_float2(gv, gv), make_float2(d4.x, d4.y), pr01);
+            pr23 = tc::ffma2(make_float2(gv, gv), make_float2(d4.z, d4.w), pr23);
+            q01 = tc::ffma2(make_float2(gp, gp), make_float2(d4.x, d4.y), q01);
+            q23 = tc::ffma2(make_float2(gp, gp), make_float2(d4.z, d4.w), q23);
           }
         }
       }
@@ -761,7 +763,8 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       const double s = w * ir, qq = s * ir;
       const double sp = dw * ir - w * ir * ir;
       const double qp = sp * ir - s * ir * ir;
-      const double dR0 = (double)pr0 + (double)dx, dR1 = (double)pr1, dR2 = (double)pr2, dR3 = (double)pr3;
+      const float dx = fmaf(q01.x, e0, fmaf(q01.y, e1, fmaf(q23.x, e2, q23.y * e3)));
+      const double dR0 = (double)pr01.x + (double)dx, dR1 = (double)pr01.y, dR2 = (double)pr23.x, dR3 = (double)pr23.y;
       const double dot = dR1 * dv.x + dR2 * dv.y + dR3 * dv.z;
       const double cm = (dR0 * sp + qp * dot) * ir;
       f0 = fma(cm, dv.x, qq * dR1); f1 = fma(cm, dv.y, qq * dR2); f2 = fma(cm, dv.z, qq * dR3);
