@@ -249,13 +249,20 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
   long long tp[11];
 #endif
 
-  int nx_idx = 0;
+  // the pair of the next tile, its centre atom and that atom's section bounds are fetched one tile ahead (a chain of
+  // three dependent global loads that would otherwise sit at the head of the tile)
+  int nx_qa = 0, nx_o0 = 0, nx_o1 = 0;
   double4 nx_dv = make_double4(0.0, 0.0, 0.0, 1.0);
   bool nx_valid = false;
   {
     const int t0 = blockIdx.x * 2 + wg, p0 = flat0 + t0 * 128 + wt;
     nx_valid = t0 < ntiles && p0 < flat1;
-    if (nx_valid) { nx_idx = pidx_t[p0]; nx_dv = C.dr[nx_idx]; }
+    if (nx_valid) {
+      const int idx = pidx_t[p0];
+      nx_dv = C.dr[idx];
+      nx_qa = idx / P.nm;
+      nx_o0 = off_t[nx_qa]; nx_o1 = off_t[nx_qa + 1];
+    }
   }
   for (int tile = blockIdx.x * 2 + wg; tile < ntiles; tile += gridDim.x * 2) {
     const bool valid = nx_valid;
@@ -264,12 +271,12 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     int qa = -1;
     TCP(0);
     if (valid) {
-      qa = nx_idx / P.nm;
+      qa = nx_qa;
       env_row4_tc(P, nx_dv, e);
     }
     ids[wt] = qa;
     if (valid) {
-      const int tile0 = flat0 + tile * 128, seg_lo = off_t[qa] - tile0, seg_hi = off_t[qa + 1] - tile0;
+      const int tile0 = flat0 + tile * 128, seg_lo = nx_o0 - tile0, seg_hi = nx_o1 - tile0;
       segs[wt] = min(nrows, seg_hi) | ((seg_lo >= 0 && seg_hi <= 128) ? 256 : 0);
     }
     {
@@ -395,7 +402,12 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     {
       const int tn = tile + gridDim.x * 2, pn = flat0 + tn * 128 + wt;
       nx_valid = tn < ntiles && pn < flat1;
-      if (nx_valid) { nx_idx = pidx_t[pn]; nx_dv = C.dr[nx_idx]; }
+      if (nx_valid) {
+        const int idx = pidx_t[pn];
+        nx_dv = C.dr[idx];
+        nx_qa = idx / P.nm;
+        nx_o0 = off_t[nx_qa]; nx_o1 = off_t[nx_qa + 1];
+      }
     }
     // S5: T_i += sum_rows g (x) R~.  Thread b owns feature b; rows are grouped by centre atom (segments, from the pair
     // offsets).  Four rows per step: one 16-byte load of gT, four broadcast loads of R~ rows (e0..e3 adjacent), eight
