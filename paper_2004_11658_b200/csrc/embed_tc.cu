@@ -716,6 +716,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     // The operand slot is free again (the tangent MMAs have completed): stage the dT rows of the tile's centre atoms in
     // it (coalesced), so that the epilogue reads them from shared memory — with 221 KB of shared memory in use the L1
     // holds almost nothing and the per-feature global loads were the largest phase of the tile.
+    const int jn = (valid && force) ? C.nl[idx] : 0;        // neighbour index for the force scatter: loaded ahead of its use
     const float4 *dT4 = reinterpret_cast<const float4 *>(dT32);
     float4 *stage = reinterpret_cast<float4 *>(slot);
     constexpr int CAP_AT = L::SLOT / (4 * S1 * 16);            // atoms whose rows fit the slot
@@ -781,7 +782,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       const double cm = (dR0 * sp + qp * dot) * ir;
       f0 = fma(cm, dv.x, qq * dR1); f1 = fma(cm, dv.y, qq * dR2); f2 = fma(cm, dv.z, qq * dR3);
       if (force) {
-        const int j = C.nl[idx];
+        const int j = jn;
         atomicAdd(&force[3 * (size_t)j + 0], -f0);
         atomicAdd(&force[3 * (size_t)j + 1], -f1);
         atomicAdd(&force[3 * (size_t)j + 2], -f2);
