@@ -336,7 +336,8 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
       const bool valid = row < n;
       double e[4] = {0.0, 0.0, 0.0, 0.0};
       double4 dv = make_double4(0.0, 0.0, 0.0, 1.0);
-      if (valid) { dv = dr[row]; env_row4(P, dv, e); }
+      int jn = 0;                                       // neighbour index for the scatter, loaded with the displacement
+      if (valid) { dv = dr[row]; jn = nl[row]; env_row4(P, dv, e); }
       // layer 0 and its tangent: h0' = (1 - t0^2) W0   (d tanh = 1 - tanh^2)
       double h0v[SP], h0t[SP];
 #pragma unroll
@@ -423,7 +424,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
           double *fs = C.fslot + ((size_t)qa * P.nm + P.sec_start[t] + row) * 3;
           fs[0] = f0; fs[1] = f1; fs[2] = f2;
         } else {
-        const int j = nl[row];
+        const int j = jn;
         if (force) {
           atomicAdd(&force[3 * (size_t)j + 0], -f0);
           atomicAdd(&force[3 * (size_t)j + 1], -f1);
