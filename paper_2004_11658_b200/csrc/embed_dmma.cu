@@ -50,6 +50,20 @@ struct EL {
   static constexpr int tile2 = 16 * SP * 4;              // pass 2, per warp: dT tile [16 SP][4]
 };
 
+// Row staging of the embedding passes: the (d, r) rows and neighbour indices of the next 32 slots are copied global ->
+// shared with cp.async (no registers in flight) while the current 32 are processed, so that no 8-row block starts with
+// a global-load round trip.  Per warp: 2 buffers x 32 rows x (32 B + 4 B).
+#define EMB_STG 288                                        // doubles per warp: 2 x 32 double4 + 2 x 32 int
+__device__ __forceinline__ void emb_cp16(void *smem_dst, const void *gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc));
+}
+__device__ __forceinline__ void emb_cp4(void *smem_dst, const void *gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc));
+}
+__device__ __forceinline__ void emb_cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void emb_cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
 static int sp_for(int s1) {
   if (s1 <= 8) return 2;
   if (s1 <= 16) return 4;
@@ -301,6 +315,8 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   double *W = smem;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
   double *dTt = smem + ((L::total + 1) & ~1) + warp * L::tile2;    // [16 SP][4], position 4 s + q
+  double4 *drs = reinterpret_cast<double4 *>(smem + ((L::total + 1) & ~1) + P2_WARPS * L::tile2 + warp * EMB_STG);
+  int *nls = reinterpret_cast<int *>(drs + 64);
   __shared__ double vred[P2_WARPS][9];
   for (int k = tid; k < L::total; k += (32 * P2_WARPS)) W[k] = netp[k];
   __syncthreads();
@@ -330,14 +346,30 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
     }
     __syncwarp();
     double fi[3] = {0.0, 0.0, 0.0};
+    auto stage_rows = [&](int base, int buf) {
+      const int r = base + lane;
+      if (r < n) {
+        emb_cp16(drs + buf * 32 + lane, dr + r);
+        emb_cp16(reinterpret_cast<double *>(drs + buf * 32 + lane) + 2, reinterpret_cast<const double *>(dr + r) + 2);
+        emb_cp4(nls + buf * 32 + lane, nl + r);
+      }
+      emb_cp_commit();
+    };
+    stage_rows(0, 0);
 
     for (int r0 = 0; r0 < n; r0 += 8) {
+      if ((r0 & 31) == 0) {
+        stage_rows(r0 + 32, ((r0 >> 5) + 1) & 1);        // next 32 rows in flight (possibly an empty group)
+        emb_cp_wait<1>();
+        __syncwarp();
+      }
       const int row = r0 + g;
       const bool valid = row < n;
+      const int sl = ((r0 >> 5) & 1) * 32 + (row & 31);
       double e[4] = {0.0, 0.0, 0.0, 0.0};
       double4 dv = make_double4(0.0, 0.0, 0.0, 1.0);
-      int jn = 0;                                       // neighbour index for the scatter, loaded with the displacement
-      if (valid) { dv = dr[row]; jn = nl[row]; env_row4(P, dv, e); }
+      int jn = 0;                                       // neighbour index for the scatter
+      if (valid) { dv = drs[sl]; jn = nls[sl]; env_row4(P, dv, e); }
       // layer 0 and its tangent: h0' = (1 - t0^2) W0   (d tanh = 1 - tanh^2)
       double h0v[SP], h0t[SP];
 #pragma unroll
@@ -499,7 +531,7 @@ template <int SP>
 static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weights &W, double *force, double *virial,
                              cudaStream_t st) {
   using L = EL<SP>;
-  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * L::tile2);
+  const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * (L::tile2 + EMB_STG));
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
