@@ -25,29 +25,49 @@ static int fail(int code, const char *fmt, ...) {
 
 unsigned long long g_dpb_launches = 0;
 
+// Auxiliary streams and events are per device (one process per GPU is the design, but a process that drives several
+// devices must not wait on another device's stream).
+#define DPB_MAX_DEVICES 32
+struct ForkState {
+  cudaStream_t aux[DPB_MAX_TYPES];
+  cudaEvent_t ev_fork, ev_join[DPB_MAX_TYPES];
+};
+static ForkState g_fork[DPB_MAX_DEVICES] = {};
+
+static cudaError_t fork_state(ForkState **out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= DPB_MAX_DEVICES) return cudaErrorInvalidDevice;
+  *out = &g_fork[dev];
+  return cudaSuccess;
+}
+
 cudaError_t dpb_fork_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]) {
-  static cudaStream_t aux[DPB_MAX_TYPES] = {};
-  static cudaEvent_t ev_fork = nullptr;
   cudaError_t e;
   s[0] = st;
   if (ntypes <= 1) return cudaSuccess;
-  if (!ev_fork && (e = cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming)) != cudaSuccess) return e;
-  if ((e = cudaEventRecord(ev_fork, st)) != cudaSuccess) return e;
+  ForkState *F;
+  if ((e = fork_state(&F)) != cudaSuccess) return e;
+  if (!F->ev_fork && (e = cudaEventCreateWithFlags(&F->ev_fork, cudaEventDisableTiming)) != cudaSuccess) return e;
+  if ((e = cudaEventRecord(F->ev_fork, st)) != cudaSuccess) return e;
   for (int ty = 1; ty < ntypes; ++ty) {
-    if (!aux[ty] && (e = cudaStreamCreateWithFlags(&aux[ty], cudaStreamNonBlocking)) != cudaSuccess) return e;
-    if ((e = cudaStreamWaitEvent(aux[ty], ev_fork, 0)) != cudaSuccess) return e;
-    s[ty] = aux[ty];
+    if (!F->aux[ty] && (e = cudaStreamCreateWithFlags(&F->aux[ty], cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(F->aux[ty], F->ev_fork, 0)) != cudaSuccess) return e;
+    s[ty] = F->aux[ty];
   }
   return cudaSuccess;
 }
 
 cudaError_t dpb_join_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]) {
-  static cudaEvent_t ev_join[DPB_MAX_TYPES] = {};
   cudaError_t e;
+  if (ntypes <= 1) return cudaSuccess;
+  ForkState *F;
+  if ((e = fork_state(&F)) != cudaSuccess) return e;
   for (int ty = 1; ty < ntypes; ++ty) {
-    if (!ev_join[ty] && (e = cudaEventCreateWithFlags(&ev_join[ty], cudaEventDisableTiming)) != cudaSuccess) return e;
-    if ((e = cudaEventRecord(ev_join[ty], s[ty])) != cudaSuccess) return e;
-    if ((e = cudaStreamWaitEvent(st, ev_join[ty], 0)) != cudaSuccess) return e;
+    if (!F->ev_join[ty] && (e = cudaEventCreateWithFlags(&F->ev_join[ty], cudaEventDisableTiming)) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(F->ev_join[ty], s[ty])) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(st, F->ev_join[ty], 0)) != cudaSuccess) return e;
   }
   return cudaSuccess;
 }
