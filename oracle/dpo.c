@@ -586,6 +586,43 @@ done:
   return rc;
 }
 
+/* ---- NEXT #3: per-atom virial ------------------------------------------------------------
+ * The paper names the virial only through the ProdVirial operator and gives no per-atom split.  Reading
+ * R14 defines Xi = -sum_i sum_k d_ik (x) dE_i/dd_ik; the split used here assigns every term to its CENTRE atom:
+ *     Xi_i[a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b],      sum_i Xi_i = Xi.
+ * Xi_i is then minus the (transposed) derivative of E_i alone under a homogeneous strain of the configuration, which is
+ * what tests/test_oracle_physics.py pins it to.  atom_virial is [N][9]. */
+int dpo_atom_virial(const dpo_model_desc *m, int64_t natoms, const double *coord, const int32_t *type,
+                    const double box[9], double *atom_virial) {
+  double L[3];
+  int rc = check_inputs(m, box, L);
+  if (rc != DPO_OK) return rc;
+  const int nm = dpo_nm(m);
+  const size_t nrow = (size_t)(natoms > 0 ? natoms : 1);
+  int32_t *nlist = (int32_t *)malloc(nrow * nm * sizeof(int32_t));
+  double *fslot = (double *)malloc(nrow * nm * 3 * sizeof(double));
+  double *ei = (double *)malloc(nrow * sizeof(double));
+  if (!nlist || !fslot || !ei) { rc = DPO_ENOMEM; goto done; }
+  rc = dpo_build_nlist_rows(m, natoms, coord, type, box, natoms, NULL, nlist, NULL);
+  if (rc != DPO_OK) goto done;
+  rc = dpo_atom_rows(m, natoms, coord, type, box, natoms, NULL, nlist, ei, fslot, NULL, NULL, NULL);
+  if (rc != DPO_OK) goto done;
+  memset(atom_virial, 0, (size_t)natoms * 9 * sizeof(double));
+  for (int64_t i = 0; i < natoms; ++i)
+    for (int k = 0; k < nm; ++k) {
+      int32_t j = nlist[i * nm + k];
+      if (j < 0) continue;
+      const double *f = fslot + ((size_t)i * nm + k) * 3;
+      double d[3], r;
+      dpo_displacement(coord + 3 * i, coord + 3 * (int64_t)j, L, d, &r);
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) atom_virial[9 * i + 3 * a + b] -= d[a] * f[b];
+    }
+done:
+  free(nlist); free(fslot); free(ei);
+  return rc;
+}
+
 /* ---- NEXT #2 / #3: evaluation of one sub-region with explicit ghost atoms ------------
  * The paper's parallel formulation: a sub-region owns its "local" atoms; the atoms of the
  * neighbouring sub-regions (and the periodic images) that lie within r_c of it are present as explicit "ghost" atoms.

@@ -81,6 +81,11 @@ int dpo_eval(const dpo_model_desc *m, int64_t natoms, const double *coord, const
              const double box[9], double *energy, double *atom_energy, double *force, double *virial,
              int32_t *nlist_out, int use_cells);
 
+/* NEXT #3: per-atom virial, centre-atom split of reading R14: atom_virial[i][a][b] =
+ * -sum_k d_ik[a] (dE_i/dd_ik)[b]; sums to the virial of dpo_eval.  atom_virial is [N][9]. */
+int dpo_atom_virial(const dpo_model_desc *m, int64_t natoms, const double *coord, const int32_t *type,
+                    const double box[9], double *atom_virial);
+
 /* NEXT #2 / #3: one sub-region with explicit ghost atoms, no box.  Atoms
  * 0..nloc-1 are local, nloc..nall-1 ghosts; energy[1] and atom_energy[nloc] cover the local atoms, force[nall][3] is
  * -dE/dr of that energy on local and ghost atoms, virial[9] the local atoms' part; nlist_out [nloc][Nm] or NULL. */

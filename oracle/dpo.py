@@ -166,6 +166,15 @@ class Oracle:
             out["nlist"] = nlist
         return out
 
+    def atom_virial(self, coord, types, box):
+        """Per-atom virial [N, 3, 3], centre-atom split (dpo_atom_virial)."""
+        coord, types, box = self._inputs(coord, types, box)
+        n = coord.shape[0]
+        out = np.empty((max(n, 1), 9))
+        rc = self.lib.dpo_atom_virial(C.byref(self.desc), C.c_int64(n), _d(coord), _i(types), _d(box), _d(out))
+        self._chk(rc, "dpo_atom_virial")
+        return out[:n].reshape(n, 3, 3)
+
     def eval_local(self, coord, types, nloc, want_nlist=True):
         """One sub-region with explicit ghost atoms, no box (dpo_eval_local): atoms [0, nloc) are
         local.  Returns dict(energy, atom_energy[nloc], force[nall], virial[, nlist[nloc]])."""

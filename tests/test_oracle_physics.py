@@ -223,3 +223,39 @@ def test_atom_rows_pieces_assemble_to_eval(water192_cond):
         f -= out["fslot"][q, hit[0]]
     assert np.abs(f - full["force"][i]).max() < 1e-12
     assert out["atom_energy"][0] == full["atom_energy"][i]
+
+
+def test_atom_virial_is_minus_the_strain_derivative_of_each_atom_energy(water192_cond):
+    """Per-atom virial, centre-atom split: Xi_i[a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b].  Under
+    x -> (1 + eps) x every displacement of atom i's environment is strained, so dE_i/d eps_ab = -Xi_i[b][a]: pinned by
+    central differences of E_i itself — diagonal strains of the periodic box, and all nine components (index order
+    included) on a cluster in a box far larger than it, where a shear of the coordinates needs no sheared box."""
+    cfg = water192_cond
+    o, coord, types, box = cfg["oracle"], cfg["coord"], cfg["types"], cfg["box"]
+    av = o.atom_virial(coord, types, box)
+    ref = o.eval(coord, types, box)
+    assert np.abs(av.sum(axis=0) - ref["virial"]).max() < 1e-11 * np.abs(ref["virial"]).max()
+    h = 1e-6
+    for a in range(3):
+        e = []
+        for sgn in (+1, -1):
+            F = np.eye(3)
+            F[a, a] += sgn * h
+            e.append(o.eval(coord @ F.T, types, (box.reshape(3, 3) @ F.T).reshape(9))["atom_energy"])
+        fd = -(e[0] - e[1]) / (2 * h)
+        assert np.abs(fd - av[:, a, a]).max() < 5e-7 * max(1.0, np.abs(fd).max())
+    # cluster: 40 atoms of the same configuration in a 60 A box
+    x = coord[:40] - coord[:40].mean(axis=0) + 30.0
+    t = types[:40]
+    big = np.diag([60.0, 60.0, 60.0]).reshape(9)
+    avc = o.atom_virial(x, t, big)
+    assert np.abs(avc).max() > 1e-3
+    for a in range(3):
+        for b in range(3):
+            e = []
+            for sgn in (+1, -1):
+                F = np.eye(3)
+                F[a, b] += sgn * h
+                e.append(o.eval((x - 30.0) @ F.T + 30.0, t, big)["atom_energy"])
+            fd = -(e[0] - e[1]) / (2 * h)                       # = -dE_i/d eps_ab = Xi_i[b][a]
+            assert np.abs(fd - avc[:, b, a]).max() < 5e-7 * max(1.0, np.abs(fd).max()), (a, b)
