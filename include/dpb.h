@@ -89,6 +89,14 @@ int dpb_model_set_variant(dpb_model *model, int variant);
  * by a full type section (info.n_overflow == 0).  Other precisions / variants: dpb_eval returns DPB_ENOTIMPL. */
 int dpb_model_set_deterministic(dpb_model *model, int on);
 
+/* Per-atom virial.  The paper gives no per-atom split (the virial is only named through the
+ * ProdVirial operator); this library assigns every term to its centre atom:
+ *     atom_virial[i][a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b],     sum_i atom_virial[i] = virial of dpb_eval.
+ * atom_virial: DEVICE fp64 [N][9] that the following dpb_eval calls fill (indexed by the input atom order), or NULL to
+ * switch the output off.  The caller owns the buffer and keeps it alive.  Produced by the gather of the deterministic
+ * reduction: dpb_eval returns DPB_ENOTIMPL while a buffer is set and dpb_model_set_deterministic is off. */
+int dpb_model_set_atom_virial(dpb_model *model, double *atom_virial);
+
 /* One evaluation (the paper's problem statement: coordinates, types and box in; E, E_i, F_i and the virial out).
  *   stream       cudaStream_t (as void*) on which all work is enqueued; NULL = the legacy default stream
  *   natoms       N >= 0

@@ -75,6 +75,7 @@ def load_library():
     lib.dpb_model_set_chunk.argtypes = [vp, i64]
     lib.dpb_model_set_variant.argtypes = [vp, i32]
     lib.dpb_model_set_deterministic.argtypes = [vp, i32]
+    lib.dpb_model_set_atom_virial.argtypes = [vp, vp]
     lib.dpb_model_set_timing.argtypes = [vp, i32]
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
     lib.dpb_set_debug_buffers.argtypes = [vp, vp, vp, vp]
@@ -153,6 +154,15 @@ class DPModel:
 
     def set_deterministic(self, on: bool):
         self._chk(self.lib.dpb_model_set_deterministic(self._h, int(bool(on))))
+
+    def set_atom_virial(self, buf=None):
+        """dpb_model_set_atom_virial: a CUDA float64 [N, 9] (or [N, 3, 3]) tensor that the following evaluations fill with
+        the per-atom virial (needs set_deterministic(True)); None switches it off.  The tensor is kept alive here."""
+        if buf is not None:
+            torch = _torch()
+            assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous()
+        self._atom_virial_keep = buf
+        self._chk(self.lib.dpb_model_set_atom_virial(self._h, None if buf is None else C.c_void_p(buf.data_ptr())))
 
     def set_timing(self, on: bool):
         self._chk(self.lib.dpb_model_set_timing(self._h, int(bool(on))))

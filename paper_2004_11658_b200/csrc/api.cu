@@ -95,6 +95,7 @@ struct Buf {
 struct dpb_model {
   DevModel P;
   int precision = 0, variant = 1, timing = 0, deterministic = 0;
+  double *atom_virial = nullptr;        // caller's [N][9] buffer (dpb_model_set_atom_virial)
   int64_t chunk = 32768;
   int device = 0;
   Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
@@ -206,6 +207,12 @@ extern "C" int dpb_model_set_chunk(dpb_model *m, int64_t chunk) {
 extern "C" int dpb_model_set_variant(dpb_model *m, int variant) {
   if (!m || variant < 0 || variant > 1) return fail(DPB_EINVAL, "dpb_model_set_variant: variant must be 0 or 1");
   m->variant = variant;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_atom_virial(dpb_model *m, double *atom_virial) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  m->atom_virial = atom_virial;
   return DPB_OK;
 }
 
@@ -342,6 +349,9 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   if (det && (m->precision != DPB_FP64 || m->variant != 1 || !m->v1.ready))
     return fail(DPB_ENOTIMPL, "the deterministic reduction is built for DPB_FP64, variant 1");
   if (det && nloc >= 0) return fail(DPB_ENOTIMPL, "the deterministic reduction is built for the periodic box");
+  if (m->atom_virial && !nlist_only && !det)
+    return fail(DPB_ENOTIMPL, "the per-atom virial comes from the deterministic reduction: switch it on "
+                              "(dpb_model_set_deterministic) or clear the buffer");
   if (det) {
     CU(m->pos_of.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
     CU(m->nl_all.reserve(sizeof(int) * (size_t)(N + 1) * P.nm), "workspace");
@@ -466,7 +476,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   if (det)
     CU(launch_force_gather(P, G, natoms, m->s_idx.as<int>(), m->pos_of.as<int>(), start + nkeys + 1,
                            m->s_xyz.as<double>(), m->nl_all.as<int>(), m->nreal_all.as<int>(), m->fslot.as<double>(),
-                           force, m->vpart.as<double>(), virial, st), "deterministic force gather");
+                           force, m->atom_virial ? m->atom_virial : m->vpart.as<double>(), virial, st),
+       "deterministic force gather");
   if (!nlist_only) {
     if (energy) CU(launch_reduce_energy(ncentre, ei, energy, st), "energy reduction");
     if (timing) cudaEventRecord(m->evs[2 + 4 * nchunks], st);

@@ -363,3 +363,38 @@ def test_deterministic_mode_is_refused_where_it_is_not_built():
         m.eval(torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda"), box)
     assert e.value.status == -6
     m.close()
+
+
+def test_atom_virial_against_the_oracle():
+    """Per-atom virial (centre-atom split, include/dpb.h) from the deterministic gather: every
+    component of every atom against dpo_atom_virial on W192 and on a 3-species box; its sum equals the virial output;
+    without the deterministic reduction the request is refused."""
+    torch = _torch()
+    from paper_2004_11658_b200 import DPBError
+    cases = []
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    cases.append((spec, emb, gen.condition_fit_w0(spec, fit), coord, types, box))
+    spec3, emb3, fit3 = small_model(ntypes=3, s1=5, m_axis=3, fit_width=9, sel=(24, 30, 30), rcut=3.5, rcut_smth=0.8, seed=11)
+    c3, t3, b3 = random_box(150, 9.0, 3, seed=5, min_dist=0.9)
+    cases.append((spec3, emb3, fit3, c3, t3, b3))
+    for spec, emb, fit, coord, types, box in cases:
+        orc, m = _models(spec, emb, fit, 1)
+        ref = orc.atom_virial(coord, types, box)
+        dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda")
+        av = torch.full((len(coord), 9), float("nan"), dtype=torch.float64, device="cuda")
+        m.set_atom_virial(av)
+        with pytest.raises(DPBError):
+            m.eval(dc, dt, box)
+        m.set_deterministic(True)
+        out = m.eval(dc, dt, box, want_info=True)
+        torch.cuda.synchronize()
+        assert out["info"].n_overflow == 0
+        got = av.cpu().numpy().reshape(-1, 3, 3)
+        assert np.abs(got - ref).max() <= 1e-10 * max(1.0, np.abs(ref).max())
+        assert np.abs(got.sum(axis=0) - out["virial"].cpu().numpy()).max() <= 1e-10 * max(1.0, np.abs(ref.sum(axis=0)).max())
+        m.set_atom_virial(None)
+        m.set_deterministic(False)
+        m.eval(dc, dt, box)
+        m.close()

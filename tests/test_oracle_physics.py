@@ -228,13 +228,15 @@ def test_atom_rows_pieces_assemble_to_eval(water192_cond):
 def test_atom_virial_is_minus_the_strain_derivative_of_each_atom_energy(water192_cond):
     """Per-atom virial, centre-atom split: Xi_i[a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b].  Under
     x -> (1 + eps) x every displacement of atom i's environment is strained, so dE_i/d eps_ab = -Xi_i[b][a]: pinned by
-    central differences of E_i itself — diagonal strains of the periodic box, and all nine components (index order
-    included) on a cluster in a box far larger than it, where a shear of the coordinates needs no sheared box."""
+    central differences of E_i itself — diagonal strains of the periodic box, and all nine components on a cluster in a
+    box far larger than it, where a shear of the coordinates needs no sheared box.  E_i is invariant under rotations of
+    its environment, so every Xi_i is symmetric (checked): the index order cannot and need not be told apart."""
     cfg = water192_cond
     o, coord, types, box = cfg["oracle"], cfg["coord"], cfg["types"], cfg["box"]
     av = o.atom_virial(coord, types, box)
     ref = o.eval(coord, types, box)
     assert np.abs(av.sum(axis=0) - ref["virial"]).max() < 1e-11 * np.abs(ref["virial"]).max()
+    assert np.abs(av - av.transpose(0, 2, 1)).max() < 1e-12 * np.abs(av).max()
     h = 1e-6
     for a in range(3):
         e = []
