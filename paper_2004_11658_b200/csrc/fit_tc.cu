@@ -317,12 +317,11 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int k
 }
 
 // ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c] (one of the S7 contractions: fp32
-// products and sums like the GEMMs), written as fp64 (debug / ABI view) and as the fp32 copy pass 2 reads.
-// One WARP per atom, no block barrier: the atom's dD row (row stride M^< + 4 floats: 16-byte stores and row loads, the
-// 16-byte row loads of consecutive lanes fall into distinct bank quads) and an fp32 copy of T are staged in the warp's
-// shared-memory slice.  First term: lane = b, all four c (one broadcast float4 of T[a] per a).  Second term: lane =
-// (a, part of the b' range, interleaved), parts combined by shuffles.  M^< in {4, 8, 16}.  `dT64` (the fp64 view the
-// debug hook reads) is written only when asked for.
+// products and sums like the GEMMs), written as the fp32 copy pass 2 reads and, for the debug hook only, as fp64.
+// One WARP per atom, no block barrier.  Only the fp32 copy of T (and the M^< second-term rows) lives in the warp's
+// shared-memory slice; the atom's dD row is read straight from global memory, every access a run of 64 contiguous
+// bytes per row: first term lane = b (four 16-byte loads of its row, all four c at once), second term lane = (a, part
+// of the b' range, interleaved), parts combined by shuffles.  M^< in {4, 8, 16}.
 #define DT_WARPS 8
 __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C, int ldd, int log2ma,
                                                          const float *__restrict__ dD, float *__restrict__ dT32,
@@ -331,29 +330,32 @@ __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = blockIdx.x * DT_WARPS + warp;
   if (q >= C.n) return;
-  const int M = P.M, Ma = 1 << log2ma, dim = P.dim, ldr = Ma + 4;
-  const int per4 = M + Ma + (M * ldr + 3) / 4;                  // float4 per warp slice
-  float4 *Ts = sm4 + warp * per4;                               // [M]   T[b][0..3] in fp32
+  const int M = P.M, Ma = 1 << log2ma;
+  float4 *Ts = sm4 + warp * (M + Ma);                           // [M]   T[b][0..3] in fp32
   float4 *t2 = Ts + M;                                          // [Ma]  second term
-  float *dd = reinterpret_cast<float *>(t2 + Ma);               // [M][Ma + 4]
   const double2 *T = reinterpret_cast<const double2 *>(C.T + (size_t)q * M * 4);
   for (int k = lane; k < M; k += 32) {
     const double2 u = T[2 * k], v = T[2 * k + 1];
     Ts[k] = make_float4((float)u.x, (float)u.y, (float)v.x, (float)v.y);
   }
-  const float4 *src = reinterpret_cast<const float4 *>(dD + (size_t)q * ldd);
-  for (int k4 = lane; k4 < dim / 4; k4 += 32) {
-    const float4 v = src[k4];
-    const int k = 4 * k4, o = (k >> log2ma) * ldr + (k & (Ma - 1));      // 4 | Ma: the four values stay in one row
-    *reinterpret_cast<float4 *>(dd + o) = v;
-  }
+  const float *row0 = dD + (size_t)q * ldd;                     // dD[b][a] at row0[b * Ma + a]
   __syncwarp();
   // second term: lane = a + Ma * h (h < 32 / Ma parts of the b' range)
   {
     const int a = lane & (Ma - 1), h = lane >> log2ma, parts = 32 >> log2ma;
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-    for (int bp = h; bp < M; bp += parts) {
-      const float d = dd[bp * ldr + a];
+    int bp = h;
+    for (; bp + 3 * parts < M; bp += 4 * parts) {               // four loads in flight
+      const float d0 = row0[bp * Ma + a], d1 = row0[(bp + parts) * Ma + a], d2 = row0[(bp + 2 * parts) * Ma + a],
+                  d3 = row0[(bp + 3 * parts) * Ma + a];
+      const float4 u0 = Ts[bp], u1 = Ts[bp + parts], u2 = Ts[bp + 2 * parts], u3 = Ts[bp + 3 * parts];
+      s0 = fmaf(d0, u0.x, s0); s1 = fmaf(d0, u0.y, s1); s2 = fmaf(d0, u0.z, s2); s3 = fmaf(d0, u0.w, s3);
+      s0 = fmaf(d1, u1.x, s0); s1 = fmaf(d1, u1.y, s1); s2 = fmaf(d1, u1.z, s2); s3 = fmaf(d1, u1.w, s3);
+      s0 = fmaf(d2, u2.x, s0); s1 = fmaf(d2, u2.y, s1); s2 = fmaf(d2, u2.z, s2); s3 = fmaf(d2, u2.w, s3);
+      s0 = fmaf(d3, u3.x, s0); s1 = fmaf(d3, u3.y, s1); s2 = fmaf(d3, u3.z, s2); s3 = fmaf(d3, u3.w, s3);
+    }
+    for (; bp < M; bp += parts) {
+      const float d = row0[bp * Ma + a];
       const float4 tv = Ts[bp];
       s0 = fmaf(d, tv.x, s0); s1 = fmaf(d, tv.y, s1); s2 = fmaf(d, tv.z, s2); s3 = fmaf(d, tv.w, s3);
     }
@@ -365,7 +367,7 @@ __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C
   }
   __syncwarp();
   for (int b = lane; b < M; b += 32) {
-    const float4 *row = reinterpret_cast<const float4 *>(dd + b * ldr);
+    const float4 *row = reinterpret_cast<const float4 *>(row0 + b * Ma);
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
     for (int a4 = 0; a4 < Ma / 4; ++a4) {
       const float4 d = row[a4];
@@ -594,7 +596,7 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
     if (e != cudaSuccess) return e;
   }
   const int log2ma = P.Ma == 4 ? 2 : (P.Ma == 8 ? 3 : 4);
-  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma + ((size_t)P.M * (P.Ma + 4) + 3) / 4);
+  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma);
   static size_t configured = 0;
   if (sm > 48 * 1024 && sm > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_dT_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
