@@ -318,72 +318,101 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int k
 
 // ---- S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c] (one of the S7 contractions: fp32
 // products and sums like the GEMMs), written as the fp32 copy pass 2 reads and, for the debug hook only, as fp64.
-// One WARP per atom, no block barrier.  Only the fp32 copy of T (and the M^< second-term rows) lives in the warp's
-// shared-memory slice; the atom's dD row is read straight from global memory, every access a run of 64 contiguous
-// bytes per row: first term lane = b (four 16-byte loads of its row, all four c at once), second term lane = (a, part
-// of the b' range, interleaved), parts combined by shuffles.  M^< in {4, 8, 16}.
+// One WARP per atom, no block barrier, ONE coalesced pass over the atom's dD row (M M^< floats): a warp instruction loads
+// 512 contiguous bytes, lane l holds dD[b][a0 .. a0 + 3] with b = 32 / LPR * i + l / LPR, a0 = 4 (l mod LPR), LPR = M^< / 4
+// lanes per row.  From that one load: the first term's partial sum over the lane's four a (T[a0 ..] kept in registers),
+// completed across the LPR lanes of the row by shuffles; and the second term's 4 x 4 accumulators (a = a0 + k, c), summed
+// over the lane's rows and at the end across the lanes that share a0.  Only the fp32 copy of T is in shared memory.
 #define DT_WARPS 8
-__global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C, int ldd, int log2ma,
-                                                         const float *__restrict__ dD, float *__restrict__ dT32,
-                                                         double *__restrict__ dT64) {
+template <int LPR>
+__global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C, int ldd, const float *__restrict__ dD,
+                                                         float *__restrict__ dT32, double *__restrict__ dT64) {
   extern __shared__ float4 sm4[];
+  constexpr int Ma = 4 * LPR, RPI = 32 / LPR;                   // rows per warp instruction
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = blockIdx.x * DT_WARPS + warp;
   if (q >= C.n) return;
-  const int M = P.M, Ma = 1 << log2ma;
-  float4 *Ts = sm4 + warp * (M + Ma);                           // [M]   T[b][0..3] in fp32
-  float4 *t2 = Ts + M;                                          // [Ma]  second term
+  const int M = P.M;
+  float4 *Ts = sm4 + warp * (M + 2 * Ma);                       // [M]   T[b][0..3] in fp32
+  float4 *f1 = Ts + M, *t2 = f1 + Ma;                           // [Ma] first term of rows b < M^<; [Ma] second term
   const double2 *T = reinterpret_cast<const double2 *>(C.T + (size_t)q * M * 4);
   for (int k = lane; k < M; k += 32) {
     const double2 u = T[2 * k], v = T[2 * k + 1];
     Ts[k] = make_float4((float)u.x, (float)u.y, (float)v.x, (float)v.y);
   }
-  const float *row0 = dD + (size_t)q * ldd;                     // dD[b][a] at row0[b * Ma + a]
   __syncwarp();
-  // second term: lane = a + Ma * h (h < 32 / Ma parts of the b' range)
-  {
-    const int a = lane & (Ma - 1), h = lane >> log2ma, parts = 32 >> log2ma;
-    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-    int bp = h;
-    for (; bp + 3 * parts < M; bp += 4 * parts) {               // four loads in flight
-      const float d0 = row0[bp * Ma + a], d1 = row0[(bp + parts) * Ma + a], d2 = row0[(bp + 2 * parts) * Ma + a],
-                  d3 = row0[(bp + 3 * parts) * Ma + a];
-      const float4 u0 = Ts[bp], u1 = Ts[bp + parts], u2 = Ts[bp + 2 * parts], u3 = Ts[bp + 3 * parts];
-      s0 = fmaf(d0, u0.x, s0); s1 = fmaf(d0, u0.y, s1); s2 = fmaf(d0, u0.z, s2); s3 = fmaf(d0, u0.w, s3);
-      s0 = fmaf(d1, u1.x, s0); s1 = fmaf(d1, u1.y, s1); s2 = fmaf(d1, u1.z, s2); s3 = fmaf(d1, u1.w, s3);
-      s0 = fmaf(d2, u2.x, s0); s1 = fmaf(d2, u2.y, s1); s2 = fmaf(d2, u2.z, s2); s3 = fmaf(d2, u2.w, s3);
-      s0 = fmaf(d3, u3.x, s0); s1 = fmaf(d3, u3.y, s1); s2 = fmaf(d3, u3.z, s2); s3 = fmaf(d3, u3.w, s3);
-    }
-    for (; bp < M; bp += parts) {
-      const float d = row0[bp * Ma + a];
-      const float4 tv = Ts[bp];
-      s0 = fmaf(d, tv.x, s0); s1 = fmaf(d, tv.y, s1); s2 = fmaf(d, tv.z, s2); s3 = fmaf(d, tv.w, s3);
-    }
-    for (int off = Ma; off < 32; off <<= 1) {
+  const int a0 = 4 * (lane % LPR), rl = lane / LPR;
+  const float4 ta0 = Ts[a0], ta1 = Ts[a0 + 1], ta2 = Ts[a0 + 2], ta3 = Ts[a0 + 3];
+  const float4 *row4 = reinterpret_cast<const float4 *>(dD + (size_t)q * ldd) + lane;
+  float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0, c2 = c0, c3 = c0;      // second term, a = a0 + k
+  auto one = [&](int b, const float4 d) {
+    // first term, partial over a0 .. a0 + 3
+    float s0 = fmaf(d.x, ta0.x, fmaf(d.y, ta1.x, fmaf(d.z, ta2.x, d.w * ta3.x)));
+    float s1 = fmaf(d.x, ta0.y, fmaf(d.y, ta1.y, fmaf(d.z, ta2.y, d.w * ta3.y)));
+    float s2 = fmaf(d.x, ta0.z, fmaf(d.y, ta1.z, fmaf(d.z, ta2.z, d.w * ta3.z)));
+    float s3 = fmaf(d.x, ta0.w, fmaf(d.y, ta1.w, fmaf(d.z, ta2.w, d.w * ta3.w)));
+#pragma unroll
+    for (int off = 1; off < LPR; off <<= 1) {
       s0 += __shfl_xor_sync(0xffffffffu, s0, off); s1 += __shfl_xor_sync(0xffffffffu, s1, off);
       s2 += __shfl_xor_sync(0xffffffffu, s2, off); s3 += __shfl_xor_sync(0xffffffffu, s3, off);
     }
-    if (lane < Ma) t2[a] = make_float4(s0, s1, s2, s3);
-  }
-  __syncwarp();
-  for (int b = lane; b < M; b += 32) {
-    const float4 *row = reinterpret_cast<const float4 *>(row0 + b * Ma);
-    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-    for (int a4 = 0; a4 < Ma / 4; ++a4) {
-      const float4 d = row[a4];
-      const float4 u0 = Ts[4 * a4], u1 = Ts[4 * a4 + 1], u2 = Ts[4 * a4 + 2], u3 = Ts[4 * a4 + 3];
-      s0 = fmaf(d.x, u0.x, s0); s1 = fmaf(d.x, u0.y, s1); s2 = fmaf(d.x, u0.z, s2); s3 = fmaf(d.x, u0.w, s3);
-      s0 = fmaf(d.y, u1.x, s0); s1 = fmaf(d.y, u1.y, s1); s2 = fmaf(d.y, u1.z, s2); s3 = fmaf(d.y, u1.w, s3);
-      s0 = fmaf(d.z, u2.x, s0); s1 = fmaf(d.z, u2.y, s1); s2 = fmaf(d.z, u2.z, s2); s3 = fmaf(d.z, u2.w, s3);
-      s0 = fmaf(d.w, u3.x, s0); s1 = fmaf(d.w, u3.y, s1); s2 = fmaf(d.w, u3.z, s2); s3 = fmaf(d.w, u3.w, s3);
+    if (b < M) {
+      const float4 tb = Ts[b];
+      c0.x = fmaf(d.x, tb.x, c0.x); c0.y = fmaf(d.x, tb.y, c0.y); c0.z = fmaf(d.x, tb.z, c0.z); c0.w = fmaf(d.x, tb.w, c0.w);
+      c1.x = fmaf(d.y, tb.x, c1.x); c1.y = fmaf(d.y, tb.y, c1.y); c1.z = fmaf(d.y, tb.z, c1.z); c1.w = fmaf(d.y, tb.w, c1.w);
+      c2.x = fmaf(d.z, tb.x, c2.x); c2.y = fmaf(d.z, tb.y, c2.y); c2.z = fmaf(d.z, tb.z, c2.z); c2.w = fmaf(d.z, tb.w, c2.w);
+      c3.x = fmaf(d.w, tb.x, c3.x); c3.y = fmaf(d.w, tb.y, c3.y); c3.z = fmaf(d.w, tb.z, c3.z); c3.w = fmaf(d.w, tb.w, c3.w);
+      if (lane % LPR == 0) {
+        const float4 o4 = make_float4(s0, s1, s2, s3);
+        if (b < Ma) f1[b] = o4;                                  // completed below with the second term
+        else {
+          reinterpret_cast<float4 *>(dT32)[(size_t)q * M + b] = o4;
+          if (dT64) {
+            double2 *o = reinterpret_cast<double2 *>(dT64 + ((size_t)q * M + b) * 4);
+            o[0] = make_double2((double)s0, (double)s1);
+            o[1] = make_double2((double)s2, (double)s3);
+          }
+        }
+      }
     }
-    if (b < Ma) { const float4 u = t2[b]; s0 += u.x; s1 += u.y; s2 += u.z; s3 += u.w; }
+  };
+  const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  const int NI = (M + RPI - 1) / RPI;                           // the same trip count for every lane: the shuffles are warp-wide
+  int i = 0;
+  for (; i + 2 <= NI; i += 2) {                                 // two loads in flight
+    const int b0 = i * RPI + rl, b1 = b0 + RPI;
+    const float4 d0 = b0 < M ? row4[(size_t)i * 32] : z4;
+    const float4 d1 = b1 < M ? row4[(size_t)(i + 1) * 32] : z4;
+    one(b0, d0);
+    one(b1, d1);
+  }
+  if (i < NI) {
+    const int b0 = i * RPI + rl;
+    one(b0, b0 < M ? row4[(size_t)i * 32] : z4);
+  }
+  // second term: sum over the lanes that share a0
+#pragma unroll
+  for (int off = LPR; off < 32; off <<= 1) {
+    c0.x += __shfl_xor_sync(0xffffffffu, c0.x, off); c0.y += __shfl_xor_sync(0xffffffffu, c0.y, off);
+    c0.z += __shfl_xor_sync(0xffffffffu, c0.z, off); c0.w += __shfl_xor_sync(0xffffffffu, c0.w, off);
+    c1.x += __shfl_xor_sync(0xffffffffu, c1.x, off); c1.y += __shfl_xor_sync(0xffffffffu, c1.y, off);
+    c1.z += __shfl_xor_sync(0xffffffffu, c1.z, off); c1.w += __shfl_xor_sync(0xffffffffu, c1.w, off);
+    c2.x += __shfl_xor_sync(0xffffffffu, c2.x, off); c2.y += __shfl_xor_sync(0xffffffffu, c2.y, off);
+    c2.z += __shfl_xor_sync(0xffffffffu, c2.z, off); c2.w += __shfl_xor_sync(0xffffffffu, c2.w, off);
+    c3.x += __shfl_xor_sync(0xffffffffu, c3.x, off); c3.y += __shfl_xor_sync(0xffffffffu, c3.y, off);
+    c3.z += __shfl_xor_sync(0xffffffffu, c3.z, off); c3.w += __shfl_xor_sync(0xffffffffu, c3.w, off);
+  }
+  if (lane < LPR) { t2[a0] = c0; t2[a0 + 1] = c1; t2[a0 + 2] = c2; t2[a0 + 3] = c3; }
+  __syncwarp();
+  if (lane < Ma && lane < M) {
+    const float4 u = f1[lane], v = t2[lane];
+    const float s0 = u.x + v.x, s1 = u.y + v.y, s2 = u.z + v.z, s3 = u.w + v.w;
+    reinterpret_cast<float4 *>(dT32)[(size_t)q * M + lane] = make_float4(s0, s1, s2, s3);
     if (dT64) {
-      double2 *o = reinterpret_cast<double2 *>(dT64 + ((size_t)q * M + b) * 4);
+      double2 *o = reinterpret_cast<double2 *>(dT64 + ((size_t)q * M + lane) * 4);
       o[0] = make_double2((double)s0, (double)s1);
       o[1] = make_double2((double)s2, (double)s3);
     }
-    reinterpret_cast<float4 *>(dT32)[(size_t)q * M + b] = make_float4(s0, s1, s2, s3);
   }
 }
 
@@ -595,15 +624,15 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
     cudaError_t e = dpb_join_streams(P.ntypes, st, ts);
     if (e != cudaSuccess) return e;
   }
-  const int log2ma = P.Ma == 4 ? 2 : (P.Ma == 8 ? 3 : 4);
-  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + P.Ma);
-  static size_t configured = 0;
-  if (sm > 48 * 1024 && sm > configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_dT_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return e;
-    configured = sm;
+  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + 2 * P.Ma);
+  const unsigned nbt = (unsigned)((C.n + DT_WARPS - 1) / DT_WARPS);
+  double *dT64 = want_dT64 ? C.dT : nullptr;
+  if (sm > 48 * 1024) return cudaErrorInvalidValue;             // M <= 256 is checked at model creation
+  switch (P.Ma) {
+    case 4: k_dT_tc<1><<<nbt, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, dD, dT32, dT64); break;
+    case 8: k_dT_tc<2><<<nbt, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, dD, dT32, dT64); break;
+    default: k_dT_tc<4><<<nbt, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, dD, dT32, dT64); break;
   }
-  k_dT_tc<<<(C.n + DT_WARPS - 1) / DT_WARPS, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, log2ma, dD, dT32, want_dT64 ? C.dT : nullptr);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
