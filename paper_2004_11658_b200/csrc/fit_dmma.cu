@@ -237,6 +237,88 @@ __global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restr
   }
 }
 
+// S7 again, the kernel the launcher prefers (M^< in {4, 8, 16}): one WARP per atom, no block barrier, ONE coalesced pass
+// over the atom's dD row.  A warp instruction loads 512 contiguous bytes; lane l holds dD[b][a0], dD[b][a0 + 1] with
+// b = 32 / LPR * i + l / LPR, a0 = 2 (l mod LPR), LPR = M^< / 2 lanes per row.  First term: partial sum over the lane's
+// two a (T[a0], T[a0 + 1] in registers), completed across the row's lanes by shuffles.  Second term: 2 x 4 accumulators
+// (a, c) summed over the lane's rows, at the end across the lanes that share a0.  Only T is staged in shared memory.
+#define DTV_WARPS 8
+template <int LPR>
+__global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView C, int dimp, const double *__restrict__ dD) {
+  extern __shared__ double sm2[];
+  constexpr int Ma = 2 * LPR, RPI = 32 / LPR;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int q = blockIdx.x * DTV_WARPS + warp;
+  if (q >= C.n) return;
+  const int M = P.M;
+  double *Ts = sm2 + (size_t)warp * (M + 2 * Ma) * 4;      // [M][4]
+  double *f1 = Ts + 4 * M, *t2 = f1 + 4 * Ma;              // [Ma][4] first term of rows b < M^<; [Ma][4] second term
+  const double2 *T = reinterpret_cast<const double2 *>(C.T + (size_t)q * M * 4);
+  for (int k = lane; k < 2 * M; k += 32) reinterpret_cast<double2 *>(Ts)[k] = T[k];
+  __syncwarp();
+  const int a0 = 2 * (lane % LPR), rl = lane / LPR;
+  double ta[2][4], c2[2][4];
+#pragma unroll
+  for (int k = 0; k < 2; ++k)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { ta[k][c] = Ts[4 * (a0 + k) + c]; c2[k][c] = 0.0; }
+  const double2 *row2 = reinterpret_cast<const double2 *>(dD + (size_t)q * dimp) + lane;
+  auto one = [&](int b, const double2 d) {
+    double s[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) s[c] = fma(d.x, ta[0][c], d.y * ta[1][c]);
+#pragma unroll
+    for (int off = 1; off < LPR; off <<= 1)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) s[c] += __shfl_xor_sync(0xffffffffu, s[c], off);
+    if (b < M) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const double tb = Ts[4 * b + c];
+        c2[0][c] = fma(d.x, tb, c2[0][c]);
+        c2[1][c] = fma(d.y, tb, c2[1][c]);
+      }
+      if (lane % LPR == 0) {
+        double2 *o = reinterpret_cast<double2 *>(b < Ma ? f1 + 4 * b : C.dT + ((size_t)q * M + b) * 4);
+        o[0] = make_double2(s[0], s[1]);
+        o[1] = make_double2(s[2], s[3]);
+      }
+    }
+  };
+  const double2 z2 = make_double2(0.0, 0.0);
+  const int NI = (M + RPI - 1) / RPI;                      // the same trip count for every lane: the shuffles are warp-wide
+  int i = 0;
+  for (; i + 2 <= NI; i += 2) {                            // two loads in flight
+    const int b0 = i * RPI + rl, b1 = b0 + RPI;
+    const double2 d0 = b0 < M ? row2[(size_t)i * 32] : z2;
+    const double2 d1 = b1 < M ? row2[(size_t)(i + 1) * 32] : z2;
+    one(b0, d0);
+    one(b1, d1);
+  }
+  if (i < NI) {
+    const int b0 = i * RPI + rl;
+    one(b0, b0 < M ? row2[(size_t)i * 32] : z2);
+  }
+#pragma unroll
+  for (int off = LPR; off < 32; off <<= 1)
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) c2[k][c] += __shfl_xor_sync(0xffffffffu, c2[k][c], off);
+  if (lane < LPR) {
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) t2[4 * (a0 + k) + c] = c2[k][c];
+  }
+  __syncwarp();
+  if (lane < Ma && lane < M) {
+    double2 *o = reinterpret_cast<double2 *>(C.dT + ((size_t)q * M + lane) * 4);
+    o[0] = make_double2(f1[4 * lane] + t2[4 * lane], f1[4 * lane + 1] + t2[4 * lane + 1]);
+    o[1] = make_double2(f1[4 * lane + 2] + t2[4 * lane + 2], f1[4 * lane + 3] + t2[4 * lane + 3]);
+  }
+}
+
 // E_i = Z2 . w3 + b3 (output layer, reading R4): one warp per atom.
 __global__ void k_rowdot_v1(ChunkView C, int ty, int fwp, const double *__restrict__ Z2, const double *__restrict__ w3,
                             double b3, double *__restrict__ atom_energy) {
@@ -389,7 +471,12 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     if (e != cudaSuccess) return e;
     configured = sm;
   }
-  k_dT_v1<<<C.n, 256, sm, st>>>(P, C, dimp, dD);
+  const size_t sms = sizeof(double) * DTV_WARPS * 4 * ((size_t)P.M + 2 * P.Ma);
+  const unsigned nbs = (unsigned)((C.n + DTV_WARPS - 1) / DTV_WARPS);
+  if (P.Ma == 16 && sms <= 48 * 1024) k_dT_v1s<8><<<nbs, 32 * DTV_WARPS, sms, st>>>(P, C, dimp, dD);
+  else if (P.Ma == 8 && sms <= 48 * 1024) k_dT_v1s<4><<<nbs, 32 * DTV_WARPS, sms, st>>>(P, C, dimp, dD);
+  else if (P.Ma == 4 && sms <= 48 * 1024) k_dT_v1s<2><<<nbs, 32 * DTV_WARPS, sms, st>>>(P, C, dimp, dD);
+  else k_dT_v1<<<C.n, 256, sm, st>>>(P, C, dimp, dD);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
