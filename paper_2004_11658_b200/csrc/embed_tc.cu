@@ -106,23 +106,51 @@ void tc_release_weights(TCWeights &W) {
 // ---- pair list -----------------------------------------------------------------------------------------------
 // off[t][q] = number of real slots of section t over the chunk's atoms before sorted position q (q in [0, n]).
 __global__ void __launch_bounds__(1024) k_pair_scan(int n, int ntypes, const int *__restrict__ nreal, int *__restrict__ off) {
-  const int t = blockIdx.x, tid = threadIdx.x;
-  __shared__ int part[1024];
-  const int per = (n + 1023) / 1024, lo = min(n, tid * per), hi = min(n, lo + per);
-  int s = 0;
-  for (int q = lo; q < hi; ++q) s += nreal[(size_t)q * ntypes + t];
-  part[tid] = s;
-  __syncthreads();
-  for (int d = 1; d < 1024; d <<= 1) {
-    const int v = tid >= d ? part[tid - d] : 0;
-    __syncthreads();
-    part[tid] += v;
-    __syncthreads();
-  }
-  int run = part[tid] - s;
+  const int t = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  __shared__ int wsum[32];
+  __shared__ int carry_s;
   int *o = off + (size_t)t * (n + 1);
-  for (int q = lo; q < hi; ++q) { o[q] = run; run += nreal[(size_t)q * ntypes + t]; }
-  if (tid == 1023) o[n] = part[1023];
+  int carry = 0;
+  // 1024 consecutive atoms per round (coalesced): warp scan, scan of the 32 warp totals, running carry
+  for (int sb = 0; sb < n; sb += 32 * 1024) {
+  int vals[32];                                              // 32 rounds' loads in flight before the first barrier
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    const int q = sb + r * 1024 + tid;
+    vals[r] = q < n ? nreal[(size_t)q * ntypes + t] : 0;
+  }
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    const int base = sb + r * 1024;
+    if (base >= n) break;
+    const int q = base + tid;
+    const int v = vals[r];
+    int incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl += u;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+      const int w = wsum[lane];
+      int wi = w;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, wi, d);
+        if (lane >= d) wi += u;
+      }
+      wsum[lane] = wi - w;                                   // exclusive prefix of the warp totals
+      if (lane == 31) carry_s = wi;                          // total of this round
+    }
+    __syncthreads();
+    if (q < n) o[q] = carry + wsum[warp] + incl - v;
+    carry += carry_s;
+    __syncthreads();                                         // wsum / carry_s are rewritten in the next round
+  }
+  }
+  if (tid == 0) o[n] = carry;
 }
 
 // pidx[n sec_start[t] + off[t][q] + k] = q Nm + sec_start[t] + k  for every real slot k of section t of atom q.
