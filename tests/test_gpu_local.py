@@ -309,3 +309,25 @@ def test_triclinic_cell_through_explicit_images():
     assert abs(got["energy"].item() - per["energy"].item()) <= 1e-10 * abs(per["energy"].item())
     assert (got["force"] - per["force"]).abs().max().item() <= 2e-9
     assert (got["virial"] - per["virial"]).abs().max().item() <= 1e-10 * max(1.0, per["virial"].abs().max().item())
+
+
+def test_subregion_in_several_chunks():
+    """dpb_eval_local with a chunk smaller than the number of local atoms (the centres are processed in several chunks,
+    the ghosts in none): same result as in one chunk, and parity with the oracle."""
+    import paper_2004_11658_b200 as pk
+    from oracle import Oracle
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc = Oracle.from_spec(spec, emb, fit)
+    lo, hi = next(iter(bricks(box, (2, 1, 1))))
+    loc, own, x, t, bounds = _domain(coord, types, box, lo, hi, spec.rcut)
+    ref = orc.eval_local(x, t, len(loc))
+    for precision in (0, 1):
+        m = pk.DPModel.from_spec(spec, emb, fit, precision=precision)
+        m.set_chunk(37)
+        got = _gpu_local(m, x, t, len(loc), bounds)
+        assert got["info"].n_chunks == (len(loc) + 36) // 37 and got["info"].n_chunks > 2
+        _check(ref, got, precision)
+        m.close()
