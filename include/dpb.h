@@ -141,6 +141,22 @@ int dpb_eval_local(dpb_model *model, void *stream, int64_t nloc, int64_t nall, c
                    const int32_t *type, const double bounds[6], double *energy, double *atom_energy, double *force,
                    double *virial, int32_t *nlist, dpb_eval_info *info);
 
+/* Velocity-Verlet pieces for a driver that owns the time loop — the decomposition's MD driver in
+ * paper_2004_11658_b200/dd.py, where an evaluation is ghost exchange + dpb_eval_local + reverse exchange.
+ * dpb_md_coefficients (HOST -> HOST): coeff_h[t] = (dt/2) / (m_t u) and coeff_h[ntypes + t] = m_t u with
+ *   u = 103.6426965268 eV fs^2 / (amu A^2); the caller copies the 2 ntypes doubles to the device.
+ * dpb_md_kick_drift: v <- v + coeff[type] F;  x <- x + dt v     (n atoms; all pointers DEVICE, coeff = first half)
+ * dpb_md_kick:       v <- v + coeff[type] F
+ * dpb_md_kinetic_energy: ekin[0] = sum_i 1/2 mass_ev[type_i] v_i^2 in eV (mass_ev = second half of the coefficients),
+ *   fixed summation order; the sum over sub-regions is the caller's all-reduce.
+ * Asynchronous on `stream`; the caller owns every buffer. */
+int dpb_md_coefficients(const double *mass_h, int32_t ntypes, double dt_fs, double *coeff_h);
+int dpb_md_kick_drift(void *stream, int64_t n, double *coord, double *vel, const double *force, const int32_t *type,
+                      const double *coeff, double dt_fs);
+int dpb_md_kick(void *stream, int64_t n, double *vel, const double *force, const int32_t *type, const double *coeff);
+int dpb_md_kinetic_energy(void *stream, int64_t n, const double *vel, const int32_t *type, const double *mass_ev,
+                          double *ekin);
+
 /* Ghost exchange of the domain decomposition (the driver is paper_2004_11658_b200/dd.py).  All
  * pointers DEVICE, all work asynchronous on `stream`; messages are rows of four fp64 (x, y, z, type).
  * dpb_dd_pack: one stage of the forward exchange along dimension dim (0, 1, 2).  Atoms with coord[dim] < cut_minus go to

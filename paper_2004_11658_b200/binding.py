@@ -89,6 +89,10 @@ def load_library():
     d = C.c_double
     lib.dpb_dd_pack.argtypes = [vp, i64, vp, vp, i32, d, d, d, d, i64, vp, vp, vp, vp, vp]
     lib.dpb_dd_unpack.argtypes = [vp, i64, vp, vp, vp]
+    lib.dpb_md_coefficients.argtypes = [C.POINTER(C.c_double), i32, d, C.POINTER(C.c_double)]
+    lib.dpb_md_kick_drift.argtypes = [vp, i64, vp, vp, vp, vp, vp, d]
+    lib.dpb_md_kick.argtypes = [vp, i64, vp, vp, vp, vp]
+    lib.dpb_md_kinetic_energy.argtypes = [vp, i64, vp, vp, vp, vp]
     lib.dpb_dd_add_forces.argtypes = [vp, i64, vp, vp, vp]
     lib.dpb_kernel_launches.restype = C.c_int64
     lib.dpb_last_error.restype = C.c_char_p
@@ -329,3 +333,37 @@ def dd_add_forces(idx, fin, k, force):
     lib = load_library()
     p = lambda t: C.c_void_p(t.data_ptr())
     _dd_chk(lib, lib.dpb_dd_add_forces(DPModel._stream(), k, p(idx), p(fin), p(force)))
+
+
+# ---- velocity-Verlet pieces (dpb_md_*): the integrator of the decomposition's MD driver -----------------------------
+class CudaIntegrator:
+    """Kick / drift / kinetic energy on CUDA tensors through libdpb's kernels (csrc/md.cu)."""
+
+    def __init__(self, masses, dt_fs: float, device):
+        torch = _torch()
+        self.lib = load_library()
+        m = np.ascontiguousarray(masses, dtype=np.float64)
+        self.ntypes, self.dt = int(m.size), float(dt_fs)
+        co = np.zeros(2 * self.ntypes)
+        _dd_chk(self.lib, self.lib.dpb_md_coefficients(m.ctypes.data_as(C.POINTER(C.c_double)), self.ntypes, self.dt,
+                                                      co.ctypes.data_as(C.POINTER(C.c_double))))
+        self.coeff = torch.tensor(co, device=device)
+        self._ek = torch.zeros(1, dtype=torch.float64, device=device)
+
+    def kick_drift(self, coord, vel, force, types):
+        p = lambda t: C.c_void_p(t.data_ptr())
+        assert coord.is_contiguous() and vel.is_contiguous() and force.is_contiguous()
+        _dd_chk(self.lib, self.lib.dpb_md_kick_drift(DPModel._stream(), int(coord.shape[0]), p(coord), p(vel), p(force),
+                                                    p(types), p(self.coeff), self.dt))
+
+    def kick(self, vel, force, types):
+        p = lambda t: C.c_void_p(t.data_ptr())
+        assert vel.is_contiguous() and force.is_contiguous()
+        _dd_chk(self.lib, self.lib.dpb_md_kick(DPModel._stream(), int(vel.shape[0]), p(vel), p(force), p(types),
+                                              p(self.coeff)))
+
+    def kinetic_energy(self, vel, types):
+        p = lambda t: C.c_void_p(t.data_ptr())
+        _dd_chk(self.lib, self.lib.dpb_md_kinetic_energy(DPModel._stream(), int(vel.shape[0]), p(vel), p(types),
+                                                        C.c_void_p(self.coeff.data_ptr() + 8 * self.ntypes), p(self._ek)))
+        return self._ek.clone()

@@ -527,6 +527,43 @@ extern "C" int dpb_eval_local(dpb_model *m, void *stream, int64_t nloc, int64_t 
   return DPB_OK;
 }
 
+// ---- velocity-Verlet pieces for drivers that own the time loop (the decomposition's MD driver, dd.py) -----------------
+extern "C" int dpb_md_coefficients(const double *mass_h, int32_t ntypes, double dt_fs, double *coeff_h) {
+  if (!mass_h || !coeff_h || ntypes < 1 || ntypes > DPB_MAX_TYPES || !(dt_fs > 0.0))
+    return fail(DPB_EINVAL, "dpb_md_coefficients: bad argument");
+  const double AMU = 103.6426965268;                           // 1 amu A^2/fs^2 in eV (CODATA 2018)
+  for (int t = 0; t < ntypes; ++t) {
+    if (!(mass_h[t] > 0.0)) return fail(DPB_EINVAL, "dpb_md_coefficients: mass[%d] <= 0", t);
+    coeff_h[t] = 0.5 * dt_fs / (mass_h[t] * AMU);
+    coeff_h[ntypes + t] = mass_h[t] * AMU;
+  }
+  return DPB_OK;
+}
+
+extern "C" int dpb_md_kick_drift(void *stream, int64_t n, double *coord, double *vel, const double *force,
+                                 const int32_t *type, const double *coeff, double dt_fs) {
+  if (n < 0 || n > 2000000000ll) return fail(DPB_EINVAL, "dpb_md_kick_drift: n out of range");
+  if (n > 0 && (!coord || !vel || !force || !type || !coeff)) return fail(DPB_EINVAL, "dpb_md_kick_drift: null argument");
+  CU(launch_md_kick_drift(n, coord, vel, force, type, coeff, dt_fs, reinterpret_cast<cudaStream_t>(stream)), "kick + drift");
+  return DPB_OK;
+}
+
+extern "C" int dpb_md_kick(void *stream, int64_t n, double *vel, const double *force, const int32_t *type,
+                           const double *coeff) {
+  if (n < 0 || n > 2000000000ll) return fail(DPB_EINVAL, "dpb_md_kick: n out of range");
+  if (n > 0 && (!vel || !force || !type || !coeff)) return fail(DPB_EINVAL, "dpb_md_kick: null argument");
+  CU(launch_md_kick(n, vel, force, type, coeff, reinterpret_cast<cudaStream_t>(stream)), "kick");
+  return DPB_OK;
+}
+
+extern "C" int dpb_md_kinetic_energy(void *stream, int64_t n, const double *vel, const int32_t *type,
+                                     const double *mass_ev, double *ekin) {
+  if (n < 0 || n > 2000000000ll || !ekin) return fail(DPB_EINVAL, "dpb_md_kinetic_energy: bad argument");
+  if (n > 0 && (!vel || !type || !mass_ev)) return fail(DPB_EINVAL, "dpb_md_kinetic_energy: null argument");
+  CU(launch_md_ekin(n, vel, type, mass_ev, ekin, reinterpret_cast<cudaStream_t>(stream)), "kinetic energy");
+  return DPB_OK;
+}
+
 extern "C" int dpb_dd_pack(void *stream, int64_t n, const double *coord, const int32_t *type, int32_t dim,
                            double cut_minus, double cut_plus, double shift_minus, double shift_plus, int64_t cap,
                            double *pack_minus, int32_t *idx_minus, double *pack_plus, int32_t *idx_plus,

@@ -116,6 +116,8 @@ cudaError_t launch_md_kick_drift(int64_t n, double *coord, double *vel, const do
                                  const double *hm, double dt, cudaStream_t st);
 cudaError_t launch_md_kick(int64_t n, double *vel, const double *force, const int *type, const double *hm,
                            cudaStream_t st);
+cudaError_t launch_md_ekin(int64_t n, const double *vel, const int *type, const double *mass_ev, double *ekin,
+                           cudaStream_t st);
 cudaError_t launch_md_thermo(int64_t n, const double *vel, const int *type, const double *mass_ev, const double *epot,
                              const double *virial, double volume, double *thermo, int slot, cudaStream_t st);
 

@@ -68,3 +68,29 @@ cudaError_t launch_md_thermo(int64_t n, const double *vel, const int *type, cons
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
+
+// E_kin = sum_i 1/2 m_i v_i^2 of n atoms (eV), fixed-order reduction by one block: the local part of a sub-region, summed
+// over the ranks by the decomposition driver (dd.py).
+__global__ void k_md_ekin(int n, const double *__restrict__ vel, const int *__restrict__ type,
+                          const double *__restrict__ mass_ev, double *__restrict__ ekin) {
+  __shared__ double part[1024];
+  double s = 0.0;
+  for (int i = threadIdx.x; i < n; i += 1024) {
+    const double vx = vel[3 * (size_t)i], vy = vel[3 * (size_t)i + 1], vz = vel[3 * (size_t)i + 2];
+    s += 0.5 * mass_ev[type[i]] * (vx * vx + vy * vy + vz * vz);
+  }
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int off = 512; off > 0; off >>= 1) {
+    if ((int)threadIdx.x < off) part[threadIdx.x] += part[threadIdx.x + off];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *ekin = part[0];
+}
+
+cudaError_t launch_md_ekin(int64_t n, const double *vel, const int *type, const double *mass_ev, double *ekin,
+                           cudaStream_t st) {
+  k_md_ekin<<<1, 1024, 0, st>>>((int)n, vel, type, mass_ev, ekin);
+  DPB_LAUNCHED(1);
+  return cudaGetLastError();
+}

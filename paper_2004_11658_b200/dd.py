@@ -322,3 +322,59 @@ class BrickDecomposition:
             dist.all_reduce(red, op=dist.ReduceOp.SUM, group=self.group)
         return {"energy": red[0:1], "virial": red[1:].reshape(3, 3), "force": force,
                 "atom_energy": out["atom_energy"], "nall": int(x.shape[0])}
+
+    # ---- molecular dynamics on the decomposition: atom migration and the time loop -----------------------------------
+    def migrate(self, coord, vel, types, tags=None):
+        """Atoms that left the brick move to the neighbour that now owns them (three stages, as the ghost exchange; an
+        atom may move less than one brick width per call).  Rows of (x, v, type, tag) travel together; the periodic shift
+        is applied by the sender, so local coordinates always lie inside [lo, hi).  `tags` (optional, one number per atom,
+        e.g. a global index below 2^53) travels with its atom.  Returns the new (coord, vel, types, tags)."""
+        torch = self._torch
+        x, v, t = coord, vel, types.to(torch.float64)
+        g = (tags if tags is not None else torch.zeros(x.shape[0], device=x.device)).to(torch.float64)
+        for dim in range(3):
+            lo, hi, L = float(self.lo[dim]), float(self.hi[dim]), float(self.L[dim])
+            up, dn = x[:, dim] >= hi, x[:, dim] < lo
+            iu, idn = torch.nonzero(up).flatten(), torch.nonzero(dn).flatten()
+            pack_up = torch.cat([x[iu], v[iu], t[iu, None], g[iu, None]], dim=1)
+            pack_dn = torch.cat([x[idn], v[idn], t[idn, None], g[idn, None]], dim=1)
+            if self.index[dim] == self.grid[dim] - 1:
+                pack_up[:, dim] -= L
+            if self.index[dim] == 0:
+                pack_dn[:, dim] += L
+            from_minus, from_plus = self._exchange(pack_up, pack_dn, dim)
+            keep = torch.nonzero(~(up | dn)).flatten()
+            x = torch.cat([x[keep], from_minus[:, 0:3], from_plus[:, 0:3]], dim=0)
+            v = torch.cat([v[keep], from_minus[:, 3:6], from_plus[:, 3:6]], dim=0)
+            t = torch.cat([t[keep], from_minus[:, 6], from_plus[:, 6]], dim=0)
+            g = torch.cat([g[keep], from_minus[:, 7], from_plus[:, 7]], dim=0)
+        return x.contiguous(), v.contiguous(), t.to(torch.int32).contiguous(), (g if tags is not None else None)
+
+    def md_run(self, evaluate_local: Callable, integrator, coord, vel, types, nsteps: int, thermo_every: int = 1,
+               tags=None):
+        """Velocity-Verlet NVE on the decomposed system: per step kick + drift, migration, ghost exchange,
+        dpb_eval_local, reverse exchange, kick.  `integrator` supplies kick_drift / kick / kinetic_energy
+        (binding.CudaIntegrator: libdpb's kernels).  Returns (coord, vel, types, tags) of this rank's atoms after the
+        run and thermo [k][2] = global (E_pot, E_kin) at steps 0, thermo_every, ..."""
+        torch, dist = self._torch, self._dist
+        thermo = []
+
+        def record(out):
+            ek = integrator.kinetic_energy(vel, types).reshape(1).to(torch.float64)
+            if self.world > 1:
+                dist.all_reduce(ek, op=dist.ReduceOp.SUM, group=self.group)
+            thermo.append(torch.cat([out["energy"].reshape(1), ek]))
+
+        coord, vel, types, tags = self.migrate(coord, vel, types, tags)
+        out = self.evaluate(evaluate_local, coord, types)
+        force = out["force"].contiguous()
+        record(out)
+        for step in range(1, nsteps + 1):
+            integrator.kick_drift(coord, vel, force, types)
+            coord, vel, types, tags = self.migrate(coord, vel, types, tags)
+            out = self.evaluate(evaluate_local, coord, types)
+            force = out["force"].contiguous()
+            integrator.kick(vel, force, types)
+            if step % thermo_every == 0:
+                record(out)
+        return coord, vel, types, tags, torch.stack(thermo)

@@ -129,3 +129,101 @@ def test_grid_choice_and_refusals():
     d = BrickDecomposition(box, 3.0, grid=(1, 2, 3), rank=5, world=6)
     assert d.index == (0, 1, 2) and d.neighbour(2, +1) == d.rank_of((0, 1, 0)) == 3 and d.neighbour(1, -1) == 2
     assert np.allclose(d.bounds(), [-3.0, 1.0, 9.5 * 2 / 3 - 3.0, 10.0, 11.0, 12.5])
+
+
+# ---- molecular dynamics on the decomposition: migration + time loop against the oracle's single-box MD --------------
+MASS2 = (15.999, 1.008)
+AMU = 1.66053906660e-27 * 1e10 / 1.602176634e-19           # 1 amu A^2/fs^2 in eV, straight from CODATA 2018
+
+
+class _TorchIntegrator:
+    """Test-side velocity-Verlet pieces on CPU tensors (the product's are libdpb kernels, binding.CudaIntegrator)."""
+
+    def __init__(self, masses, dt):
+        self.m = torch.tensor(masses, dtype=torch.float64) * AMU
+        self.dt = dt
+
+    def kick_drift(self, coord, vel, force, types):
+        vel += (0.5 * self.dt / self.m[types.long()])[:, None] * force
+        coord += self.dt * vel
+
+    def kick(self, vel, force, types):
+        vel += (0.5 * self.dt / self.m[types.long()])[:, None] * force
+
+    def kinetic_energy(self, vel, types):
+        return (0.5 * self.m[types.long()] * (vel ** 2).sum(dim=1)).sum().reshape(1)
+
+
+def _md_inputs():
+    import gen
+    spec, emb, fit, coord, types, box = _system()
+    vel = gen.maxwell_boltzmann(types, MASS2, 330.0, seed=21) * 12.0          # fast: atoms cross brick faces in 12 steps
+    return spec, emb, fit, coord, types, box, vel
+
+
+def _md_rank(rank, world, grid, nsteps, dt):
+    from oracle import Oracle
+    from paper_2004_11658_b200.dd import BrickDecomposition
+    spec, emb, fit, coord, types, box, vel = _md_inputs()
+    orc = Oracle.from_spec(spec, emb, fit)
+    dd = BrickDecomposition(box, spec.rcut, grid=grid, rank=rank, world=world)
+    mask, w = dd.owned_mask(torch.from_numpy(coord))
+    ids = torch.nonzero(mask).flatten()
+    x, v, t, tags, thermo = dd.md_run(_oracle_evaluator(orc), _TorchIntegrator(MASS2, dt), w[ids].contiguous().clone(),
+                                      torch.from_numpy(vel)[ids].contiguous().clone(),
+                                      torch.from_numpy(types.astype(np.int32))[ids], nsteps, thermo_every=4,
+                                      tags=ids.to(torch.float64))
+    return tags.numpy().astype(np.int64), x.numpy(), v.numpy(), t.numpy(), thermo.numpy(), ids.numpy()
+
+
+def _md_worker(rank, world, port, grid, nsteps, dt, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        q.put((rank,) + _md_rank(rank, world, grid, nsteps, dt))
+    finally:
+        dist.destroy_process_group()
+
+
+def _md_check(results, nsteps, dt):
+    from oracle import Oracle
+    spec, emb, fit, coord, types, box, vel = _md_inputs()
+    xr, vr, th = Oracle.from_spec(spec, emb, fit).md_run(coord, vel, types, MASS2, box, dt, nsteps, thermo_every=4)
+    L = np.array([box[0], box[4], box[8]])
+    n = len(coord)
+    seen, moved = np.zeros(n, int), 0
+    for rank, tags, x, v, t, thermo, n0 in results:
+        seen[tags] += 1
+        d = x - xr[tags]
+        d -= np.round(d / L) * L                                  # the decomposition keeps atoms wrapped, the oracle does not
+        assert np.abs(d).max() < 1e-9
+        assert np.abs(v - vr[tags]).max() < 1e-10
+        assert np.array_equal(t, types[tags])
+        assert np.abs(thermo[:, 0] - th[:, 0]).max() < 1e-10 * np.abs(th[:, 0]).max()      # E_pot, on every rank
+        assert np.abs(thermo[:, 1] - th[:, 1]).max() < 1e-10 * np.abs(th[:, 1]).max()      # E_kin
+        moved += len(set(tags.tolist()) - set(n0.tolist()))       # atoms this rank received during the run
+    assert (seen == 1).all()
+    return moved
+
+
+def test_md_single_rank_against_the_oracle():
+    res = (0,) + _md_rank(0, 1, (1, 1, 1), 12, 1.0)
+    _md_check([res], 12, 1.0)
+
+
+@pytest.mark.parametrize("world,grid", [(2, (1, 1, 2)), (4, (2, 2, 1))])
+def test_md_with_migration_over_gloo(world, grid):
+    """Atoms cross brick faces and the periodic boundary during the run: positions (mod L), velocities, types and the
+    global E_pot / E_kin of every rank against the oracle's single-box velocity-Verlet, atom by atom through the tags."""
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_md_worker, args=(r, world, port, grid, 12, 1.0, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    results = [q.get(timeout=400) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    moved = _md_check(sorted(results, key=lambda r: r[0]), 12, 1.0)
+    assert moved > 0                                             # the run did exercise the migration

@@ -115,3 +115,55 @@ def test_md_argument_errors():
     with pytest.raises(DPBError) as e:
         _gpu_md(spec, emb, fit, coord, vel, types, box, mass, dt_fs=-1.0, nsteps=2)
     assert e.value.status == -1
+
+
+def test_decomposition_md_on_one_gpu_against_dpb_md_run():
+    """dd.md_run with world size 1 on the device — libdpb's kick / drift / kinetic-energy kernels
+    (binding.CudaIntegrator), migration across the periodic boundary, ghost images, dpb_eval_local, force fold-back —
+    against dpb_md_run on the same box: positions (mod L), velocities, E_pot and E_kin after 20 steps.  Also the three
+    integrator kernels against the formulas written in numpy."""
+    import torch
+    import paper_2004_11658_b200 as pk
+    from paper_2004_11658_b200.binding import CudaIntegrator
+    from paper_2004_11658_b200.dd import BrickDecomposition
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    masses = gen.MASSES["W192"]
+    vel = gen.maxwell_boltzmann(types, masses, 330.0, seed=5) * 8.0
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    dc, dv = torch.tensor(coord, device="cuda"), torch.tensor(vel, device="cuda")
+    dt = torch.tensor(types, device="cuda")
+    # integrator kernels against numpy
+    integ = CudaIntegrator(masses, 0.5, dc.device)
+    amu = 1.66053906660e-27 * 1e10 / 1.602176634e-19
+    f = torch.tensor(np.random.default_rng(1).normal(size=coord.shape), device="cuda")
+    x1, v1 = dc.clone(), dv.clone()
+    integ.kick_drift(x1, v1, f, dt)
+    mm = np.asarray(masses)[types] * amu
+    v_ref = vel + (0.25 / mm)[:, None] * f.cpu().numpy()
+    assert np.abs(v1.cpu().numpy() - v_ref).max() < 1e-14 and np.abs(x1.cpu().numpy() - (coord + 0.5 * v_ref)).max() < 1e-12
+    integ.kick(v1, f, dt)
+    assert np.abs(v1.cpu().numpy() - (v_ref + (0.25 / mm)[:, None] * f.cpu().numpy())).max() < 1e-14
+    ek = integ.kinetic_energy(dv, dt).item()
+    assert abs(ek - (0.5 * mm * (vel ** 2).sum(axis=1)).sum()) < 1e-12 * ek
+    # the run
+    xa, va = dc.clone(), dv.clone()
+    thermo, info = m.md_run(xa, va, dt, masses, box, 0.5, 20, thermo_every=5)
+    dd = BrickDecomposition(box, spec.rcut, grid=(1, 1, 1), rank=0, world=1)
+    mask, w = dd.owned_mask(dc)
+    tags = torch.arange(len(coord), device="cuda", dtype=torch.float64)
+    xb, vb, tb, gb, th = dd.md_run(lambda x, t, nloc, bounds: m.eval_local(x, t, nloc, bounds, want_info=False), integ,
+                                   w.contiguous().clone(), dv.clone(), dt, 20, thermo_every=5, tags=tags)
+    torch.cuda.synchronize()
+    order = gb.long()
+    L = torch.tensor([box[0], box[4], box[8]], device="cuda")
+    d = xb - xa[order]
+    d -= torch.round(d / L) * L
+    assert d.abs().max().item() < 1e-9 and (vb - va[order]).abs().max().item() < 1e-10
+    assert torch.equal(tb, dt[order])
+    th = th.cpu().numpy()
+    assert np.abs(th[:, 0] - thermo[:, 0]).max() < 1e-10 * np.abs(thermo[:, 0]).max()
+    assert np.abs(th[:, 1] - thermo[:, 1]).max() < 1e-10 * np.abs(thermo[:, 1]).max()
+    m.close()
