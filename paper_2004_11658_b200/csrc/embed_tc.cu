@@ -738,6 +738,20 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       nx_valid = tn < ntiles && pn < flat1;
       if (nx_valid) { nx_idx = pidx_t[pn]; nx_dv = C.dr[nx_idx]; }
     }
+    // ... and the first dT rows of this tile's centre atoms (staged in the operand slot once the MMAs are done)
+    const float4 *dT4 = reinterpret_cast<const float4 *>(dT32);
+    constexpr int CAP_AT = L::SLOT / (4 * S1 * 16);            // atoms whose rows fit the slot
+    constexpr int DT_PF = 3;                                   // float4 per thread in flight over the MMA wait
+    const int nrows_t = min(128, flat1 - (flat0 + tile * 128));
+    const int qa0 = ids[0];
+    const int nat = min(ids[nrows_t - 1] - qa0 + 1, CAP_AT);
+    const float4 *dsrc = dT4 + (size_t)qa0 * P.M;
+    float4 pf[DT_PF];
+#pragma unroll
+    for (int u = 0; u < DT_PF; ++u) {
+      const int k = wt + 128 * u;
+      pf[u] = k < nat * 4 * S1 ? dsrc[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     tc::mbar_wait(mbar, phase);
     phase ^= 1;
     tc::fence_after_sync();
@@ -745,15 +759,14 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     // it (coalesced), so that the epilogue reads them from shared memory — with 221 KB of shared memory in use the L1
     // holds almost nothing and the per-feature global loads were the largest phase of the tile.
     const int jn = (valid && force) ? C.nl[idx] : 0;        // neighbour index for the force scatter: loaded ahead of its use
-    const float4 *dT4 = reinterpret_cast<const float4 *>(dT32);
     float4 *stage = reinterpret_cast<float4 *>(slot);
-    constexpr int CAP_AT = L::SLOT / (4 * S1 * 16);            // atoms whose rows fit the slot
-    const int nrows_t = min(128, flat1 - (flat0 + tile * 128));
-    const int qa0 = ids[0];
-    const int nat = min(ids[nrows_t - 1] - qa0 + 1, CAP_AT);
     {
-      const float4 *src = dT4 + (size_t)qa0 * P.M;
-      for (int k = wt; k < nat * 4 * S1; k += 128) stage[k] = src[k];
+#pragma unroll
+      for (int u = 0; u < DT_PF; ++u) {
+        const int k = wt + 128 * u;
+        if (k < nat * 4 * S1) stage[k] = pf[u];
+      }
+      for (int k = wt + 128 * DT_PF; k < nat * 4 * S1; k += 128) stage[k] = dsrc[k];
     }
     tc::bar_sync(1 + wg, 128);
     // epilogue: g = (h1, h1) + t2, g' = (h1', h1') + (1 - t2^2) (h1' W2); dots with the atom's dT rows
