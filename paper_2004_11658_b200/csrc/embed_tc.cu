@@ -759,6 +759,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
     // it (coalesced), so that the epilogue reads them from shared memory — with 221 KB of shared memory in use the L1
     // holds almost nothing and the per-feature global loads were the largest phase of the tile.
     const int jn = (valid && force) ? C.nl[idx] : 0;        // neighbour index for the force scatter: loaded ahead of its use
+    const int in_ = (valid && force) ? C.s_idx[C.p0 + qa] : 0;   // ... and the centre atom's own index
     float4 *stage = reinterpret_cast<float4 *>(slot);
     {
 #pragma unroll
@@ -843,7 +844,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       }
       const int qprev = __shfl_up_sync(0xffffffffu, qa, 1);
       if (valid && (lane == 0 || qprev != qa)) {
-        const size_t i = (size_t)C.s_idx[C.p0 + qa];
+        const size_t i = (size_t)in_;
         atomicAdd(&force[3 * i + 0], f0); atomicAdd(&force[3 * i + 1], f1); atomicAdd(&force[3 * i + 2], f2);
       }
     }
