@@ -592,6 +592,7 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
   tc::fence_after_sync();
   const uint32_t tmem = *tmem_slot;
   const uint32_t tD1v = tmem + wg * 256, tD1t = tD1v + 64, tD2v = tD1v, tD2t = tD1v + 128;
+  const uint32_t tA1 = tD1v + 128;                           // layer-1 A operands: v hi, v lo, t hi, t lo, 32 columns each
   const uint32_t lane_sel = (uint32_t)(32 * (warp & 3)) << 16;
   const uint32_t slot_a = tc::smem_u32(slot), img_a = tc::smem_u32(smem);
   const uint32_t rowbase = (uint32_t)(wt >> 3) * 1024u + (uint32_t)(wt & 7) * 128u, r7 = wt & 7;
@@ -649,12 +650,22 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
         h0v[s] = 0.0f; h0t[s] = 0.0f;
       }
     }
+    // layer-1 A operands (value and tangent, hi and lo) go to tensor memory, columns [128, 256) of the warpgroup — the
+    // tangent accumulator of layer 2 lives there later — and the MMAs read them from there (TS form, as in pass 1)
+    {
+      uint32_t w[32];
 #pragma unroll
-    for (int j = 0; j < 2 * L::KS1; ++j) {
-      store_split4(slot, slot + 16384, rowbase, r7, j, h0v[4 * j], h0v[4 * j + 1], h0v[4 * j + 2], h0v[4 * j + 3]);
-      store_split4(slot + 32768, slot + 49152, rowbase, r7, j, h0t[4 * j], h0t[4 * j + 1], h0t[4 * j + 2], h0t[4 * j + 3]);
+      for (int part = 0; part < 4; ++part) {
+#pragma unroll
+        for (int s = 0; s < 32; ++s) {
+          float fh, fl;
+          tc::split_tf32(part < 2 ? h0v[s] : h0t[s], fh, fl);
+          w[s] = __float_as_uint((part & 1) ? fl : fh);
+        }
+        tc::tmem_st32_nowait(tA1 + 32 * part + lane_sel, w);
+      }
+      tc::tmem_wait_st();
     }
-    tc::fence_proxy_async();
     tc::fence_before_sync();
     tc::bar_sync(1 + wg, 128);
     if (wt == 0) {
@@ -662,10 +673,13 @@ k_pass2_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
       constexpr uint32_t idesc = tc::make_idesc_tf32(128, L::N1);
 #pragma unroll
       for (int ks = 0; ks < L::KS1; ++ks) {
-        mma3(tD1v, slot_a + ks * 32, slot_a + 16384 + ks * 32, img_a + L::oW1h + ks * 32, img_a + L::oW1l + ks * 32, idesc,
-             ks == 0);
-        mma3(tD1t, slot_a + 32768 + ks * 32, slot_a + 49152 + ks * 32, img_a + L::oW1h + ks * 32, img_a + L::oW1l + ks * 32,
-             idesc, ks == 0);
+        const uint64_t dbh = tc::make_desc_sw128(img_a + L::oW1h + ks * 32), dbl = tc::make_desc_sw128(img_a + L::oW1l + ks * 32);
+        tc::mma_tf32_ts(tD1v, tA1 + 32 + 8 * ks, dbh, idesc, ks == 0 ? 0u : 1u);      // lo hi + hi lo + hi hi
+        tc::mma_tf32_ts(tD1v, tA1 + 8 * ks, dbl, idesc, 1u);
+        tc::mma_tf32_ts(tD1v, tA1 + 8 * ks, dbh, idesc, 1u);
+        tc::mma_tf32_ts(tD1t, tA1 + 96 + 8 * ks, dbh, idesc, ks == 0 ? 0u : 1u);
+        tc::mma_tf32_ts(tD1t, tA1 + 64 + 8 * ks, dbl, idesc, 1u);
+        tc::mma_tf32_ts(tD1t, tA1 + 64 + 8 * ks, dbh, idesc, 1u);
       }
       tc::mma_commit(mbar);
     }
