@@ -154,16 +154,17 @@ __global__ void __launch_bounds__(1024) k_pair_scan(int n, int ntypes, const int
 }
 
 // pidx[n sec_start[t] + off[t][q] + k] = q Nm + sec_start[t] + k  for every real slot k of section t of atom q.
-__global__ void k_pair_expand(DevModel P, int n, const int *__restrict__ nreal, const int *__restrict__ off,
-                              int *__restrict__ pidx) {
-  const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (g >= (long long)n * P.nm) return;
-  const int q = (int)(g / P.nm), slot = (int)(g - (long long)q * P.nm);
-  int t = 0;
-  while (t + 1 < P.ntypes && slot >= P.sec_start[t + 1]) ++t;
-  const int k = slot - P.sec_start[t];
-  if (k < nreal[(size_t)q * P.ntypes + t])
-    pidx[(size_t)n * P.sec_start[t] + off[(size_t)t * (n + 1) + q] + k] = (int)g;
+// One warp per atom: only the real slots are visited (copper at sel = 512 is 65 % padding), stores are contiguous.
+__global__ void __launch_bounds__(256) k_pair_expand(DevModel P, int n, const int *__restrict__ nreal,
+                                                     const int *__restrict__ off, int *__restrict__ pidx) {
+  const int q = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (q >= n) return;
+  for (int t = 0; t < P.ntypes; ++t) {
+    const int nr = nreal[(size_t)q * P.ntypes + t];
+    int *dst = pidx + (size_t)n * P.sec_start[t] + off[(size_t)t * (n + 1) + q];
+    const int base = q * P.nm + P.sec_start[t];
+    for (int k = lane; k < nr; k += 32) dst[k] = base + k;
+  }
 }
 
 size_t tc_pair_workspace_bytes(const DevModel &P, int64_t chunk) {
@@ -175,8 +176,7 @@ cudaError_t tc_build_pairs(const DevModel &P, const ChunkView &C, void *ws, cuda
   int *off = reinterpret_cast<int *>(ws);
   int *pidx = off + (size_t)P.ntypes * (C.n + 1);
   k_pair_scan<<<P.ntypes, 1024, 0, st>>>(C.n, P.ntypes, C.nreal, off);
-  const long long tot = (long long)C.n * P.nm;
-  k_pair_expand<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(P, C.n, C.nreal, off, pidx);
+  k_pair_expand<<<(unsigned)((C.n + 7) / 8), 256, 0, st>>>(P, C.n, C.nreal, off, pidx);
   DPB_LAUNCHED(2);
   return cudaGetLastError();
 }
