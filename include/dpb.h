@@ -13,6 +13,11 @@
  * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  All calls return 0 on success or a
  * negative dpb_status; on error the outputs are undefined and dpb_last_error() describes the failure.
  * Nothing here throws or aborts.  Units: Angstrom, eV, eV/Angstrom.  All matrices row-major.
+ *
+ * Concurrency: one host thread per process and GPU drives the library (the design is one process per GPU); calls are not
+ * thread-safe.  Work is enqueued on the caller's stream; internally independent launches (the nets of a pass, the
+ * species' fitting chains) are forked onto library-owned streams and joined by events before the call's last kernel, so
+ * for the caller everything is ordered as if it ran on `stream` alone.
  */
 #ifndef DPB_H
 #define DPB_H
