@@ -284,9 +284,12 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
 // chunk) tasks with the chunk index fastest: eight lanes write one full 128-byte image row, a warp four adjacent rows =
 // 512 contiguous bytes per store (thread-per-row stores touched 32 separate lines, half a sector each).
 template <int MA>
-__global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
+__global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int ty, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
   extern __shared__ float4 Ts[];                                   // [DESCR_R][M + 1]
+  // one launch per species, on that species' stream: blocks outside its row range leave at once
+  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
   const int row0 = blockIdx.x * DESCR_R, nrow = min(DESCR_R, C.n - row0), M = P.M, ld = M + 1;
+  if (row0 >= row_hi || row0 + DESCR_R <= row_lo) return;
   {
     const double2 *src = reinterpret_cast<const double2 *>(C.T + (size_t)row0 * M * 4);
     float2 *dst = reinterpret_cast<float2 *>(Ts);
@@ -300,8 +303,8 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int k
   const int ntask = DESCR_R * kpan * 8, kreal = M * MA;
   for (int q = threadIdx.x; q < ntask; q += 256) {
     const int j = q & 7, rl = (q >> 3) & (DESCR_R - 1), pan = q / (8 * DESCR_R);
-    if (rl >= nrow) continue;
     const int m = row0 + rl, k0 = pan * FT_KP + 4 * j;
+    if (rl >= nrow || m < row_lo || m >= row_hi) continue;
     float d[4] = {0.f, 0.f, 0.f, 0.f};                             // image columns between dim and the padded K are zero
     if (k0 < kreal) {
       const int b = k0 / MA, a0 = k0 - b * MA;
@@ -326,12 +329,14 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int k
 #define DT_WARPS 8
 template <int LPR>
 __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C, int ldd, const float *__restrict__ dD,
-                                                         float *__restrict__ dT32, double *__restrict__ dT64) {
+                                                         float *__restrict__ dT32, double *__restrict__ dT64, int ty) {
   extern __shared__ float4 sm4[];
   constexpr int Ma = 4 * LPR, RPI = 32 / LPR;                   // rows per warp instruction
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = blockIdx.x * DT_WARPS + warp;
-  if (q >= C.n) return;
+  // one launch per species, at the tail of that species' chain
+  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  if (q >= C.n || q < row_lo || q >= row_hi) return;
   const int M = P.M;
   float4 *Ts = sm4 + warp * (M + 2 * Ma);                       // [M]   T[b][0..3] in fp32
   float4 *f1 = Ts + M, *t2 = f1 + Ma;                           // [Ma] first term of rows b < M^<; [Ma] second term
@@ -589,19 +594,15 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
   float *Z1 = p; p += rows * F->fwp;
   float *dZ1 = p; p += rows * F->fwp;
   float *dD = p;
-  {
-    const unsigned nb = (unsigned)((C.n + DESCR_R - 1) / DESCR_R);
-    const size_t sm = (size_t)DESCR_R * (P.M + 1) * sizeof(float4);
-    switch (P.Ma) {
-      case 4: k_descr_tc<4><<<nb, 256, sm, st>>>(P, C, (int)kpd, Dh, Dl); break;
-      case 8: k_descr_tc<8><<<nb, 256, sm, st>>>(P, C, (int)kpd, Dh, Dl); break;
-      default: k_descr_tc<16><<<nb, 256, sm, st>>>(P, C, (int)kpd, Dh, Dl); break;
-    }
-  }
-  DPB_LAUNCHED(1);
-  // The per-type GEMM chains are independent (disjoint rows; a tile on the type boundary is read by both and written
-  // row-wise by each) and G1-G5 of one type fill only as many SMs as that type has row tiles (W24k: 64 and 128 of 148):
-  // forked streams let one type's CTAs take the SMs the other leaves idle.  Largest type (last) on the caller's stream.
+  // The per-type chains (descriptor rows, six GEMMs, dT contraction) are independent: disjoint rows; a tile on the type
+  // boundary is read by both and written row-wise by each.  G1-G5 of one type fill only as many SMs as that type has row
+  // tiles (W24k: 64 and 128 of 148), and the descriptor / dT kernels are memory-bound while the GEMMs are not: forked
+  // streams let one type's work take what the other leaves idle.  Largest type (last) on the caller's stream.
+  const unsigned nbd = (unsigned)((C.n + DESCR_R - 1) / DESCR_R), nbt = (unsigned)((C.n + DT_WARPS - 1) / DT_WARPS);
+  const size_t smd = (size_t)DESCR_R * (P.M + 1) * sizeof(float4);
+  const size_t smt = sizeof(float4) * DT_WARPS * ((size_t)P.M + 2 * P.Ma);
+  if (smt > 48 * 1024 || smd > 48 * 1024) return cudaErrorInvalidValue;   // M <= 256 is checked at model creation
+  double *dT64 = want_dT64 ? C.dT : nullptr;
   cudaStream_t ts[DPB_MAX_TYPES];
   {
     cudaError_t e = dpb_fork_streams(P.ntypes, st, ts);
@@ -610,6 +611,12 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
   for (int k = 0; k < P.ntypes; ++k) {
     const int ty = P.ntypes - 1 - k;
     cudaStream_t s = ts[k];
+    switch (P.Ma) {
+      case 4: k_descr_tc<4><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, Dh, Dl); break;
+      case 8: k_descr_tc<8><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, Dh, Dl); break;
+      default: k_descr_tc<16><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, Dh, Dl); break;
+    }
+    DPB_LAUNCHED(1);
     cudaError_t e;
     switch (F->NT) {
       case 32: e = ft_run_type<32>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
@@ -619,20 +626,16 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
       default: e = ft_run_type<256>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
     }
     if (e != cudaSuccess) return e;
+    switch (P.Ma) {
+      case 4: k_dT_tc<1><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, dD, dT32, dT64, ty); break;
+      case 8: k_dT_tc<2><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, dD, dT32, dT64, ty); break;
+      default: k_dT_tc<4><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, dD, dT32, dT64, ty); break;
+    }
+    DPB_LAUNCHED(1);
   }
   {
     cudaError_t e = dpb_join_streams(P.ntypes, st, ts);
     if (e != cudaSuccess) return e;
   }
-  const size_t sm = sizeof(float4) * DT_WARPS * ((size_t)P.M + 2 * P.Ma);
-  const unsigned nbt = (unsigned)((C.n + DT_WARPS - 1) / DT_WARPS);
-  double *dT64 = want_dT64 ? C.dT : nullptr;
-  if (sm > 48 * 1024) return cudaErrorInvalidValue;             // M <= 256 is checked at model creation
-  switch (P.Ma) {
-    case 4: k_dT_tc<1><<<nbt, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, dD, dT32, dT64); break;
-    case 8: k_dT_tc<2><<<nbt, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, dD, dT32, dT64); break;
-    default: k_dT_tc<4><<<nbt, 32 * DT_WARPS, sm, st>>>(P, C, F->dimp, dD, dT32, dT64); break;
-  }
-  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
