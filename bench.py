@@ -398,8 +398,10 @@ def run_cuda(args):
                          "traffic": traffic,
                          "note": "fp64 pipe (DFMA/DMMA share one pipe, measured 37.0 TF/s; peak derived from 148 SM x 64 "
                                  "FMA/clk x 1.965 GHz); algorithmic flops of the stage / its CUDA-event time; the "
-                                 "stage executes ~1.45x its algorithmic flops (forward-mode tangent rows, tanh) and "
-                                 "keeps the fp64 pipe 76.5 % busy (ncu, profiles/r1_ncu_full_w24k.md)"},
+                                 "embedding passes execute 2.4-2.8x their algorithmic flops (pass 2 recomputes the "
+                                 "forward chain and carries a tangent chain instead of reading stored activations; "
+                                 "tanh; 25 -> 28 padding on water) and keep the fp64 pipe 74-81 % busy (ncu: "
+                                 "profiles/r1_ncu_full_w24k.md, profiles/r1_ncu_full_cu32k.md)"},
             "e2e": {"value": world * n * e2e_steps / (e2e_ms * 1e-3), "unit": "atom-steps/s",
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": int(launches),
