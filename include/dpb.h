@@ -94,6 +94,20 @@ int dpb_model_set_variant(dpb_model *model, int variant);
  * by a full type section (info.n_overflow == 0).  Other precisions / variants: dpb_eval returns DPB_ENOTIMPL. */
 int dpb_model_set_deterministic(dpb_model *model, int on);
 
+/* Same-species pair reuse in pass 1 (DPB_FP64, variant 1; on by default, off while the deterministic reduction is on).
+ * The embedding net of a pair depends on s(r_ij) = s(r_ji) only (Eq. 5 and 8-9), so for the nets
+ * G^{a,a} one evaluation serves both directions: the atom with the lower sorted position adds g (x) R~_ik to its own
+ * T_i (Eq. 4's G^T R~) and g (x) R~_ki to T_k with fp64 reductions.  Only pairs whose two atoms are centres of the same
+ * chunk are shared; it is switched off on the device for an evaluation in which a neighbour was dropped by a full type
+ * section (n_overflow > 0), because the two lists are then not symmetric.  T is summed in a different (and, with the
+ * reductions, run-to-run varying) order: results move at the 1e-15 relative level.  Other precisions ignore it.
+ *   on = 0  off
+ *   on = 1  (default) evaluations that run as a single chunk (dpb_model_set_chunk): with several chunks only the pairs
+ *           inside a chunk can be shared and the bookkeeping costs more than it saves (measured on the 864,000-atom box)
+ *   on = 2  always (pairs across a chunk boundary are evaluated in both directions)
+ * Returns DPB_EINVAL for any other value. */
+int dpb_model_set_pair_reuse(dpb_model *model, int on);
+
 /* Per-atom virial.  The paper gives no per-atom split (the virial is only named through the
  * ProdVirial operator); this library assigns every term to its centre atom:
  *     atom_virial[i][a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b],     sum_i atom_virial[i] = virial of dpb_eval.

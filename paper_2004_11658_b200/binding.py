@@ -75,6 +75,7 @@ def load_library():
     lib.dpb_model_set_chunk.argtypes = [vp, i64]
     lib.dpb_model_set_variant.argtypes = [vp, i32]
     lib.dpb_model_set_deterministic.argtypes = [vp, i32]
+    lib.dpb_model_set_pair_reuse.argtypes = [vp, i32]
     lib.dpb_model_set_atom_virial.argtypes = [vp, vp]
     lib.dpb_model_set_timing.argtypes = [vp, i32]
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
@@ -158,6 +159,10 @@ class DPModel:
 
     def set_deterministic(self, on: bool):
         self._chk(self.lib.dpb_model_set_deterministic(self._h, int(bool(on))))
+
+    def set_pair_reuse(self, on: int):
+        """dpb_model_set_pair_reuse: 0 off, 1 single-chunk evaluations (default), 2 always."""
+        self._chk(self.lib.dpb_model_set_pair_reuse(self._h, int(on)))
 
     def set_atom_virial(self, buf=None):
         """dpb_model_set_atom_virial: a CUDA float64 [N, 9] (or [N, 3, 3]) tensor that the following evaluations fill with

@@ -94,7 +94,7 @@ struct Buf {
 
 struct dpb_model {
   DevModel P;
-  int precision = 0, variant = 1, timing = 0, deterministic = 0;
+  int precision = 0, variant = 1, timing = 0, deterministic = 0, pair_reuse = 1;
   double *atom_virial = nullptr;        // caller's [N][9] buffer (dpb_model_set_atom_virial)
   int64_t chunk = 32768;
   int device = 0;
@@ -219,6 +219,13 @@ extern "C" int dpb_model_set_atom_virial(dpb_model *m, double *atom_virial) {
 extern "C" int dpb_model_set_deterministic(dpb_model *m, int on) {
   if (!m) return fail(DPB_EINVAL, "null model");
   m->deterministic = on ? 1 : 0;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_pair_reuse(dpb_model *m, int on) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  if (on < 0 || on > 2) return fail(DPB_EINVAL, "pair reuse: 0 (off), 1 (single-chunk evaluations) or 2 (always)");
+  m->pair_reuse = on;
   return DPB_OK;
 }
 
@@ -352,8 +359,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   if (m->atom_virial && !nlist_only && !det)
     return fail(DPB_ENOTIMPL, "the per-atom virial comes from the deterministic reduction: switch it on "
                               "(dpb_model_set_deterministic) or clear the buffer");
+  CU(m->pos_of.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
   if (det) {
-    CU(m->pos_of.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
     CU(m->nl_all.reserve(sizeof(int) * (size_t)(N + 1) * P.nm), "workspace");
     CU(m->nreal_all.reserve(sizeof(int) * (size_t)(N + 1) * P.ntypes), "workspace");
     CU(m->fslot.reserve(sizeof(double) * 3 * (size_t)(N + 1) * P.nm), "workspace");
@@ -405,7 +412,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
                             st), "gather");
   } else {
     CU(launch_cell_sort(P, G, natoms, coord, type, m->key.as<int>(), m->count.as<int>(), start, m->cursor.as<int>(),
-                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st, det ? m->pos_of.as<int>() : nullptr),
+                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st, m->pos_of.as<int>()),
        "cell sort");
     if (nl_mode == 1 && natoms > 0)
       CU(cudaMemcpyAsync(m->md_xyz0.p, m->s_xyz.p, sizeof(double) * 3 * (size_t)natoms, cudaMemcpyDeviceToDevice, st),
@@ -432,6 +439,9 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.T = m->T.as<double>();
     C.dT = m->dT.as<double>();
     C.fslot = nullptr;
+    C.pos_of = m->pos_of.as<int>();
+    C.stats = stats;
+    C.reuse = (!det && (m->pair_reuse == 2 || (m->pair_reuse == 1 && nchunks == 1))) ? 1 : 0;
     if (det) {                                           // full-size lists: the gather needs every atom's row
       C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
       C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;

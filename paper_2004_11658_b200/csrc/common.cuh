@@ -62,7 +62,11 @@ struct ChunkView {
   int *nreal;              // [n][ntypes] real (non-padded) slots per section
   double *T;               // [n][M][4]
   double *dT;              // [n][M][4]
-  double *fslot;           // deterministic mode: [n][nm][3] dE_i/dd_ik per slot (pass 2 stores instead of scattering)
+  double *fslot;           // deterministic mode: [n][nm][3] dE_i/dd_ik per slot (pass 2 stores instead of scattering)  // same-species pair reuse in pass 1 (fp64 variant 1): g(s(r_ij)) = g(s(r_ji)) for a net (a, a), so
+  // the atom with the lower sorted position evaluates the pair once and adds g (x) R~_ji to T_j with red.global.add.f64
+  const int *pos_of;       // [N] sorted position of original atom index (nullptr: no reuse)
+  const DevStats *stats;   // reuse is taken only while stats->n_overflow == 0 (a dropped neighbour breaks the symmetry)
+  int reuse;
 };
 
 // The per-type fitting chains are independent (disjoint rows) and one type's GEMM launch fills only as many SMs as that

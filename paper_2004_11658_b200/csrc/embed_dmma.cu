@@ -167,7 +167,12 @@ __device__ __forceinline__ void env_row4(const DevModel &P, const double4 v, dou
 // takes atoms of type a round-robin and walks the real slots of section t in blocks of 8 * RB rows (RB m-blocks that
 // share every B fragment).  T_i is accumulated in registers (lane-owned features) through a per-warp g tile.
 // RB = 1 keeps the fully unrolled loop body inside the instruction cache (RB = 2 measured 49 % stall_no_inst).
-template <int SP, int RB>
+// RU (launched for the nets (a, a) when C.reuse): same-species pair reuse.  g depends on s(r_ij) = s(r_ji) only, so of
+// the two directions of a pair whose atoms are both centres of this chunk only the atom with the lower row evaluates
+// the embedding net; it adds g (x) R~_ik to its own T_i and g (x) R~_ki = g (x) (s, -s d/r) to T_k with warp-coalesced
+// red.global.add.f64 (580 G/s measured, profiles/r1_fp64_peaks.md).  T rows are zeroed by the launcher and every
+// accumulation of this launch into T is a reduction.  Taken only while no neighbour was dropped (n_overflow == 0).
+template <int SP, int RB, bool RU>
 __global__ void __launch_bounds__((32 * P1_WARPS), 1)
 k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate) {
   using L = EL<SP>;
@@ -176,6 +181,23 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
   double *gt = smem + ((L::total + 1) & ~1) + warp * (RB == 1 ? L::tile1s : L::tile1);     // [8 RB][LDG]
   double *envt = gt + 8 * RB * L::LDG;                             // [8 RB][4]
+  // RU: per warp, the kept slots of the atom (slot index, row of the neighbour inside the chunk or -1)
+  int *ksl = reinterpret_cast<int *>(smem + ((L::total + 1) & ~1) + P1_WARPS * (RB == 1 ? L::tile1s : L::tile1)) +
+             warp * 2 * P.nm;
+  int *krow = ksl + P.nm;
+  const bool ru = RU && C.stats->n_overflow == 0ull;
+  // RU: offset inside a T tile of the element this lane adds in step k of N chunk ch (position p = lane / 4 + 8 k of
+  // the g tile, component lane % 4), or -1 for a pad
+  int toff[RU ? 2 : 1][RU ? SP : 1];
+  if (RU) {
+#pragma unroll
+    for (int ch = 0; ch < 2; ++ch)
+#pragma unroll
+      for (int k = 0; k < SP; ++k) {
+        const int p = (lane >> 2) + 8 * k, sg = ch * 2 * SP + (p >> 2), c = sg / SP, r = (sg % SP) * 4 + (p & 3);
+        toff[ch][k] = r < P.s1 ? (c * P.s1 + r) * 4 + (lane & 3) : -1;
+      }
+  }
   for (int k = tid; k < L::total; k += (32 * P1_WARPS)) W[k] = netp[k];
   __syncthreads();
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
@@ -184,8 +206,31 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   const int s1 = P.s1, M = P.M;
 
   for (int qa = row_lo + blockIdx.x * P1_WARPS + warp; qa < row_hi; qa += gridDim.x * P1_WARPS) {
-    const int n = C.nreal[(size_t)qa * P.ntypes + t];
+    int n = C.nreal[(size_t)qa * P.ntypes + t];
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
+    if (RU && ru) {                                      // keep the slots whose pair this atom evaluates
+      const int *nlr = C.nl + (size_t)qa * P.nm + P.sec_start[t];
+      int nk = 0;
+      __syncwarp();
+      for (int base = 0; base < n; base += 32) {
+        const int slot = base + lane;
+        bool keep = false;
+        int qj = -1;
+        if (slot < n) {
+          qj = C.pos_of[nlr[slot]] - C.p0;
+          if (qj < 0 || qj >= C.n) qj = -1;              // not a centre of this chunk (other chunk, ghost): one direction
+          keep = qj < 0 || qj > qa;
+        }
+        const unsigned mk = __ballot_sync(0xffffffffu, keep);
+        if (keep) {
+          const int pos = nk + __popc(mk & ((1u << lane) - 1u));
+          ksl[pos] = slot; krow[pos] = qj;
+        }
+        nk += __popc(mk);
+      }
+      n = nk;
+      __syncwarp();
+    }
     double Tacc[2][2][4];
 #pragma unroll
     for (int ch = 0; ch < 2; ++ch)
@@ -200,7 +245,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
       for (int rb = 0; rb < RB; ++rb) {
         const int row = r0 + g + 8 * rb;
         double e[4] = {0.0, 0.0, 0.0, 0.0};
-        if (row < n) env_row4(P, dr[row], e);
+        if (row < n) env_row4(P, dr[(RU && ru) ? ksl[row] : row], e);
         x[rb] = e[0];
         if (q == 0) {
           double *dst = envt + (g + 8 * rb) * 4;
@@ -277,6 +322,23 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
             }
           }
         }
+        if (RU && ru) {                                  // T_k += g (x) R~_ki, 8 positions x 4 components per instruction
+          const int comp = lane & 3;
+#pragma unroll 1
+          for (int row = 0; row < 8 * RB; ++row) {
+            if (r0 + row >= n) break;
+            const int qj = krow[r0 + row];
+            if (qj < 0) continue;
+            const double ev = comp == 0 ? envt[row * 4] : -envt[row * 4 + comp];
+            double *Tj = C.T + (size_t)qj * M * 4;
+            const double *gr = gt + row * L::LDG + (lane >> 2);
+#pragma unroll
+            for (int k = 0; k < SP; ++k) {
+              const int o = toff[ch][k];
+              if (o >= 0) atomicAdd(Tj + o, gr[8 * k] * ev);
+            }
+          }
+        }
       }
       __syncwarp();                                      // envt / gt are rewritten by the next row block
     }
@@ -291,7 +353,10 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
           const int c = s / SP, r = (s % SP) * 4 + qq;
           if (r < s1) {
             double *dst = C.T + ((size_t)qa * M + c * s1 + r) * 4;
-            if (accumulate) {
+            if (RU && ru) {
+              atomicAdd(dst + 0, Tacc[ch][u][0]); atomicAdd(dst + 1, Tacc[ch][u][1]);
+              atomicAdd(dst + 2, Tacc[ch][u][2]); atomicAdd(dst + 3, Tacc[ch][u][3]);
+            } else if (accumulate) {
               dst[0] += Tacc[ch][u][0]; dst[1] += Tacc[ch][u][1]; dst[2] += Tacc[ch][u][2]; dst[3] += Tacc[ch][u][3];
             } else {
               dst[0] = Tacc[ch][u][0]; dst[1] = Tacc[ch][u][1]; dst[2] = Tacc[ch][u][2]; dst[3] = Tacc[ch][u][3];
@@ -505,11 +570,23 @@ template <int SP>
 static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weights &W, cudaStream_t st) {
   using L = EL<SP>;
   const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P1_WARPS * L::tile1s);
+  const size_t smem_ru = smem + sizeof(int) * 2 * (size_t)P.nm * P1_WARPS;
+  const bool reuse = C.reuse && C.pos_of && smem_ru <= 227 * 1024;
   static bool configured = false;
+  static size_t configured_ru = 0;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
+  }
+  if (reuse && smem_ru > configured_ru) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ru);
+    if (e != cudaSuccess) return e;
+    configured_ru = smem_ru;
+  }
+  if (reuse) {                                           // every accumulation into T is then an addition
+    cudaError_t e = cudaMemsetAsync(C.T, 0, sizeof(double) * (size_t)C.n * P.M * 4, st);
+    if (e != cudaSuccess) return e;
   }
   const int grid = min(g_sm_count, (C.n + P1_WARPS - 1) / P1_WARPS);
   // nets of one centre type a accumulate into the same T rows (t = 0 stores, t > 0 adds): one stream per a, so that the
@@ -519,8 +596,12 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
   if (e != cudaSuccess) return e;
   for (int a = 0; a < P.ntypes; ++a)
     for (int t = 0; t < P.ntypes; ++t) {
-      k_pass1_dmma<SP, 1><<<grid, (32 * P1_WARPS), smem, ts[P.ntypes - 1 - a]>>>(
-          P, C, W.emb + (size_t)(a * P.ntypes + t) * W.net_stride, a, t, t > 0);
+      const double *net = W.emb + (size_t)(a * P.ntypes + t) * W.net_stride;
+      if (reuse && a == t)
+        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, ts[P.ntypes - 1 - a]>>>(P, C, net, a, t, 1);
+      else
+        k_pass1_dmma<SP, 1, false><<<grid, (32 * P1_WARPS), smem, ts[P.ntypes - 1 - a]>>>(P, C, net, a, t,
+                                                                                        reuse ? 1 : t > 0);
       DPB_LAUNCHED(1);
     }
   if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;

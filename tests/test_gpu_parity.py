@@ -398,3 +398,30 @@ def test_atom_virial_against_the_oracle():
         m.set_deterministic(False)
         m.eval(dc, dt, box)
         m.close()
+
+
+@pytest.mark.parametrize("name,chunk", [("W192", 100000), ("W192", 50), ("Cu-small", 100000)])
+def test_pair_reuse_matches_oracle_and_the_plain_pass(name, chunk):
+    """Same-species pair reuse in pass 1 (dpb_model_set_pair_reuse, on by default): T (Eq. 4's G^T R~, checked through the
+    debug buffer), E, F and the virial against the oracle with the reuse on, and against the pass without it; with
+    chunks the pairs that straddle a chunk boundary are evaluated in both directions."""
+    if name == "W192":
+        spec = MODELS["W192"]
+        coord, types, box = gen.make_system("W192")
+    else:
+        spec = MODELS["Cu32k"]
+        coord, types, box = gen.copper_box(6, 0.05, seed=gen.SEED_BASE + 2)
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, 1)
+    m.set_chunk(chunk)
+    ref = orc.eval(coord, types, box)
+    res = {}
+    for on in (True, False):
+        m.set_pair_reuse(2 if on else 0)                # 2: also when the evaluation runs in several chunks
+        res[on] = _gpu_eval(m, coord, types, box, debug=True, spec=spec)
+        _check_full(ref, res[on])
+    scale = np.abs(res[False]["T"]).max()
+    assert np.abs(res[True]["T"] - res[False]["T"]).max() <= 1e-13 * scale
+    assert np.abs(res[True]["force"] - res[False]["force"]).max() <= 1e-11
+    m.close()
