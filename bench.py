@@ -174,7 +174,8 @@ def workload_config(name, args):
             "perturbation_sigma_A": 0.01, "neighbour_build": "every step",
             "parallelism": "replicas only (1 GPU per replica, no collectives)",
             "l2": "flushed between timed steps (256 MiB write)", "variant": getattr(args, "variant", 1),
-            "precision": getattr(args, "precision", "fp64")}
+            "precision": getattr(args, "precision", "fp64"),
+            "pair_reuse": "pass 1, nets (a,a), single-chunk evaluations (library default; fp64 variant 1 only)"}
 
 
 # ---- molecular dynamics: the paper's own unit, steps/s and ns/day ----------------------
