@@ -134,6 +134,16 @@ int dpb_eval(dpb_model *model, void *stream, int64_t natoms, const double *coord
              const double box[9], double *energy, double *atom_energy, double *force, double *virial,
              int32_t *nlist, dpb_eval_info *info);
 
+/* Deferred input errors.  Three conditions are detected on the device and therefore only reported by a call that
+ * synchronises (dpb_eval / dpb_eval_local / dpb_eval_host with info != NULL, dpb_build_nlist with n_overflow != NULL,
+ * dpb_md_run) — with info == NULL the call returns DPB_OK and its outputs are undefined:
+ *   DPB_EINVAL  an atom's type index lies outside [0, ntypes) (it is evaluated as type 0)
+ *   DPB_ECAP    an atom has more in-range candidates than the staging capacity max(256, 2 Nm) (its row is written empty)
+ *   DPB_EBOX    dpb_eval_local: an atom lies outside `bounds`
+ * dpb_model_status synchronises `stream` and returns the status of the LAST evaluation enqueued for this model
+ * (DPB_OK, or one of the three above with dpb_last_error set), for callers that run with info == NULL. */
+int dpb_model_status(dpb_model *model, void *stream);
+
 /* Same call with HOST buffers for coord/type and for every output (end-to-end entry: host->device copies of the
  * inputs, the evaluation, and device->host copies of the requested outputs, all on `stream`, then a stream
  * synchronise).  Pinned host memory makes the copies asynchronous, pageable memory is accepted. */
@@ -203,6 +213,12 @@ int dpb_build_nlist(dpb_model *model, void *stream, int64_t natoms, const double
  *   dT [N][M][4]   = dE_i/dT_i
  * Pass all NULL to switch it off. */
 int dpb_set_debug_buffers(dpb_model *model, double *T, double *D, double *dT);
+
+/* Test hook, not part of the contract: order DEVICE int32 [natoms] receives, for every sorted position p of the LAST
+ * evaluation of this model (atoms are processed in the order (ghost?, type, cell); chunk c covers the positions
+ * [c * chunk_atoms, (c + 1) * chunk_atoms)), the input index of the atom at p.  Lets a test pick atoms on both sides of
+ * a chunk boundary.  Asynchronous on `stream`; DPB_EINVAL before the first evaluation or if natoms differs from it. */
+int dpb_debug_sorted_order(dpb_model *model, void *stream, int64_t natoms, int32_t *order);
 
 /* Per-stage device time of the last dpb_eval issued after dpb_model_set_timing(model, 1), in microseconds (CUDA
  * events recorded on the caller's stream between the stages; the caller must have synchronised that stream):

@@ -80,6 +80,8 @@ def load_library():
     lib.dpb_model_set_timing.argtypes = [vp, i32]
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
     lib.dpb_set_debug_buffers.argtypes = [vp, vp, vp, vp]
+    lib.dpb_debug_sorted_order.argtypes = [vp, vp, i64, vp]
+    lib.dpb_model_status.argtypes = [vp, vp]
     lib.dpb_eval.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp, C.POINTER(_Info)]
     lib.dpb_eval_local.argtypes = [vp, vp, i64, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp,
                                    C.POINTER(_Info)]
@@ -188,6 +190,17 @@ class DPModel:
         p = [None if t is None else C.c_void_p(t.data_ptr()) for t in (T, D, dT)]
         self._debug_keep = (T, D, dT)
         self._chk(self.lib.dpb_set_debug_buffers(self._h, *p))
+
+    def status(self):
+        """dpb_model_status: synchronise and raise DPBError if the last evaluation hit a deferred input error."""
+        self._chk(self.lib.dpb_model_status(self._h, self._stream()))
+
+    def sorted_order(self, natoms: int):
+        """dpb_debug_sorted_order: CUDA int32 [natoms], input index of the atom at every sorted position of the last call."""
+        torch = _torch()
+        order = torch.empty(int(natoms), dtype=torch.int32, device="cuda")
+        self._chk(self.lib.dpb_debug_sorted_order(self._h, self._stream(), int(natoms), C.c_void_p(order.data_ptr())))
+        return order
 
     @staticmethod
     def _box(box):

@@ -79,13 +79,14 @@ extern "C" const char *dpb_version(void) { return "dpb 1 sm_100a"; }
 struct Buf {
   void *p = nullptr;
   size_t cap = 0;
-  cudaError_t reserve(size_t bytes) {
+  cudaError_t reserve(size_t bytes, bool zero = false) {
     if (bytes <= cap) return cudaSuccess;
     if (p) cudaFree(p);
     p = nullptr; cap = 0;
     size_t want = bytes + bytes / 8 + 256;
     cudaError_t e = cudaMalloc(&p, want);
     if (e == cudaSuccess) cap = want;
+    if (e == cudaSuccess && zero) e = cudaMemset(p, 0, want);      // (re)allocation only: synchronous, rare
     return e;
   }
   void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
@@ -103,7 +104,8 @@ struct dpb_model {
   TCWeights tcw;                // mixed precision: TF32 hi / lo operand images (embed_tc.cu)
   // workspace
   Buf key, count, start, cursor, s_idx, s_xyz, stats, ei;
-  Buf nl, dr, nreal, T, dT;
+  Buf nl, nlp, dr, nreal, T, dT;
+  int dt_pad_alloc = -1;          // layout the dT buffer was last used with (pad rows must be zero: cleared on a change)
   Buf v0[9];
   Buf v1ws;
   Buf tcfit;                    // mixed precision: operand images and activations of the fitting stage
@@ -120,6 +122,7 @@ struct dpb_model {
   double *dbgT = nullptr, *dbgD = nullptr, *dbgdT = nullptr;
   std::vector<cudaEvent_t> evs;   // stage timers: [0] start, [1] after S1, then 4 per chunk, then the end
   int ev_chunks = 0;              // chunks of the last timed evaluation
+  int64_t last_natoms = -1;       // atoms of the last evaluation (dpb_debug_sorted_order)
 };
 
 static int nm_of(const DevModel &P) { return P.nm; }
@@ -186,7 +189,7 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
+                &m->nl, &m->nlp, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
                 &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
                 &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass};
   for (Buf *b : all) b->release();
@@ -232,6 +235,17 @@ extern "C" int dpb_model_set_pair_reuse(dpb_model *m, int on) {
 extern "C" int dpb_set_debug_buffers(dpb_model *m, double *T, double *D, double *dT) {
   if (!m) return fail(DPB_EINVAL, "null model");
   m->dbgT = T; m->dbgD = D; m->dbgdT = dT;
+  return DPB_OK;
+}
+
+extern "C" int dpb_debug_sorted_order(dpb_model *m, void *stream, int64_t natoms, int32_t *order) {
+  if (!m || !order) return fail(DPB_EINVAL, "dpb_debug_sorted_order: null argument");
+  if (m->last_natoms < 0 || natoms != m->last_natoms)
+    return fail(DPB_EINVAL, "dpb_debug_sorted_order: natoms differs from the last evaluation (%lld)", (long long)m->last_natoms);
+  if (natoms == 0) return DPB_OK;
+  cudaError_t e = cudaMemcpyAsync(order, m->s_idx.p, sizeof(int) * (size_t)natoms, cudaMemcpyDeviceToDevice,
+                                  reinterpret_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return fail(DPB_ECUDA, "dpb_debug_sorted_order: %s", cudaGetErrorString(e));
   return DPB_OK;
 }
 
@@ -366,12 +380,18 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     CU(m->fslot.reserve(sizeof(double) * 3 * (size_t)(N + 1) * P.nm), "workspace");
     CU(m->vpart.reserve(sizeof(double) * 9 * (size_t)(N + 1)), "workspace");
   }
+  int dt_pad = 0;
   CU(m->nl.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
+  CU(m->nlp.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
   CU(m->dr.reserve(sizeof(double4) * (size_t)chunk * P.nm), "workspace");
   CU(m->nreal.reserve(sizeof(int) * (size_t)chunk * P.ntypes), "workspace");
   if (!nlist_only) {
     CU(m->T.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
-    CU(m->dT.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
+    // fp64 variant 1 keeps dT in the padded lane order of the DMMA kernels (ChunkView::dt_pad); the pad rows are zero
+    dt_pad = (m->precision == DPB_FP64 && m->variant == 1 && m->v1.ready) ? 4 * m->v1.SP : 0;
+    const size_t dt_bytes = sizeof(double) * (size_t)chunk * (dt_pad ? 4 * dt_pad : P.M) * 4;
+    if (dt_pad != m->dt_pad_alloc) { m->dT.release(); m->dt_pad_alloc = dt_pad; }
+    CU(m->dT.reserve(dt_bytes, true), "workspace");
     if (m->precision == DPB_FP64 && (m->variant == 0 || !m->v1.ready)) {
       CU(m->v0[0].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
       CU(m->v0[1].reserve(sizeof(double) * (size_t)chunk * P.dim), "workspace");
@@ -406,6 +426,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     cudaEventRecord(m->evs[0], st);
   }
 
+  m->last_natoms = natoms;
   int *start = m->start.as<int>();
   if (nl_mode == 2) {
     CU(launch_gather_sorted(natoms, coord, m->s_idx.as<int>(), m->s_xyz.as<double>(), m->md_xyz0.as<double>(), stats,
@@ -438,10 +459,14 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.nreal = m->nreal.as<int>();
     C.T = m->T.as<double>();
     C.dT = m->dT.as<double>();
+    C.dt_pad = dt_pad;
+    C.dt_rows = dt_pad ? 4 * dt_pad : P.M;
+    C.nlp = m->nlp.as<int>();
     C.fslot = nullptr;
     C.pos_of = m->pos_of.as<int>();
     C.stats = stats;
     C.reuse = (!det && (m->pair_reuse == 2 || (m->pair_reuse == 1 && nchunks == 1))) ? 1 : 0;
+    C.reuse2 = (!det && m->pair_reuse >= 1) ? 1 : 0;     // pass 2 only reads dT_j: no bookkeeping, any chunking
     if (det) {                                           // full-size lists: the gather needs every atom's row
       C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
       C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;
@@ -512,6 +537,11 @@ static int finish_info(dpb_model *m, cudaStream_t st, int64_t natoms, dpb_eval_i
     info->n_chunks = (int32_t)((natoms + chunk - 1) / chunk);
   }
   return DPB_OK;
+}
+
+extern "C" int dpb_model_status(dpb_model *m, void *stream) {
+  if (!m) return fail(DPB_EINVAL, "dpb_model_status: null model");
+  return finish_info(m, reinterpret_cast<cudaStream_t>(stream), 0, nullptr);
 }
 
 extern "C" int dpb_eval(dpb_model *m, void *stream, int64_t natoms, const double *coord, const int32_t *type,

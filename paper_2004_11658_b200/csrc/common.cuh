@@ -61,12 +61,20 @@ struct ChunkView {
   double4 *dr;             // [n][nm] (dx, dy, dz, r) of real slots
   int *nreal;              // [n][ntypes] real (non-padded) slots per section
   double *T;               // [n][M][4]
-  double *dT;              // [n][M][4]
+  double *dT;              // [n][dt_rows][4]: dE_i/dT_i, row of feature b given by dt_offset() below
+  // Layout of dT.  dt_pad == 0: plain, row = b, dt_rows = M.  dt_pad = 4 SP > 0 (fp64 variant 1): every copy of s1
+  // features is padded to 4 SP rows, row = (b / s1) * dt_pad + b % s1, dt_rows = 4 dt_pad — the order in which the lanes
+  // of the DMMA embedding kernels hold the features (embed_dmma.cu), so that any run of feature slots is one contiguous
+  // piece of the tile (bulk-copied as such by pass 2).  Pad rows are zero (the buffer is cleared when it is allocated
+  // and no kernel writes them).
+  int dt_pad, dt_rows;
+  const int *nlp;          // [n][nm] sorted position of the neighbour in each real slot (nl holds its input index)
   double *fslot;           // deterministic mode: [n][nm][3] dE_i/dd_ik per slot (pass 2 stores instead of scattering)  // same-species pair reuse in pass 1 (fp64 variant 1): g(s(r_ij)) = g(s(r_ji)) for a net (a, a), so
   // the atom with the lower sorted position evaluates the pair once and adds g (x) R~_ji to T_j with red.global.add.f64
   const int *pos_of;       // [N] sorted position of original atom index (nullptr: no reuse)
   const DevStats *stats;   // reuse is taken only while stats->n_overflow == 0 (a dropped neighbour breaks the symmetry)
-  int reuse;
+  int reuse;               // pass 1
+  int reuse2;              // pass 2 (k_pass2_dmma_ru): both directions of a same-species pair from one evaluation
 };
 
 // The per-type fitting chains are independent (disjoint rows) and one type's GEMM launch fills only as many SMs as that
@@ -140,6 +148,12 @@ __device__ __forceinline__ void dp_displacement(const double xi[3], const double
   }
   double r2 = __fma_rn(d[2], d[2], __fma_rn(d[1], d[1], __dmul_rn(d[0], d[0])));
   r = __dsqrt_rn(r2);
+}
+
+// Offset (in doubles) of dT[q][b][0] in the chunk's dT buffer (layouts: ChunkView::dt_pad).
+__device__ __forceinline__ size_t dt_offset(const DevModel &P, const ChunkView &C, int q, int b) {
+  const int row = C.dt_pad ? (b / P.s1) * C.dt_pad + (b % P.s1) : b;
+  return ((size_t)q * C.dt_rows + row) * 4;
 }
 
 // Gate w(r) of Eq. 5, reading R1: quintic between r_cs and r_c.

@@ -17,6 +17,7 @@
 // h' = dh/dx runs through the same GEMM chain as the value row (second m-block, same B fragments), and
 //   dE/dx = sum_o (dT R~)[o] g'[o],   dE/dR~[c] = sum_o dT[o][c] g[o]          (O9 of DESIGN.md / SURVEY.md §8(c)).
 #include "v1_kernels.cuh"
+#include "tc_common.cuh"
 
 #include <vector>
 
@@ -388,7 +389,6 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
-  const int s1 = P.s1, M = P.M;
   double vir[9];
 #pragma unroll
   for (int k = 0; k < 9; ++k) vir[k] = 0.0;
@@ -399,15 +399,9 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
     const int *nl = C.nl + (size_t)qa * P.nm + P.sec_start[t];
     __syncwarp();
-    for (int p = lane; p < 16 * SP; p += 32) {
-      const int s = p >> 2, qq = p & 3;
-      const int c = s / SP, r = (s % SP) * 4 + qq;
-      double4 v = make_double4(0.0, 0.0, 0.0, 0.0);
-      if (r < s1) {
-        const double *src = C.dT + ((size_t)qa * M + c * s1 + r) * 4;
-        v = make_double4(src[0], src[1], src[2], src[3]);
-      }
-      *reinterpret_cast<double4 *>(dTt + 4 * p) = v;
+    {                                                    // dT is stored in lane order (ChunkView::dt_pad): a plain copy
+      const double4 *src = reinterpret_cast<const double4 *>(C.dT + (size_t)qa * C.dt_rows * 4);
+      for (int p = lane; p < 16 * SP; p += 32) *reinterpret_cast<double4 *>(dTt + 4 * p) = src[p];
     }
     __syncwarp();
     double fi[3] = {0.0, 0.0, 0.0};
@@ -563,6 +557,304 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// Pass 2 with same-species pair reuse (nets (a, a); dpb_model_set_pair_reuse).  The embedding net
+// depends on s(r_ij) = s(r_ji) only (Eq. 5, 8-9): of the two directions of a pair whose atoms are both
+// centres of this chunk, ONE atom (the lower row when the row sum is even, the higher one otherwise: every atom keeps
+// about half of its pairs) runs the value and tangent chains and applies the epilogue twice — with its own dT tile and
+// R~_ij, and with dT_j and R~_ji = (s, -s d/r).  The dT_j slices of the 8 rows of a block are fetched from L2 by the
+// TMA engine (cp.async.bulk, one 1 KB piece per row and N chunk, completion on a per-warp mbarrier) while the DMMAs of
+// that chunk run; the force on the pair is f_ij - f_ji (F_i += f, F_j -= f, Xi -= d_ij (x) f).  Pairs whose neighbour
+// is not a centre of this chunk (another chunk, a ghost) are evaluated in one direction as before.  Layer 2 runs as a
+// two-trip loop over halves of N (two N chunks each), which also keeps the unrolled body inside the instruction cache.
+template <int SP>
+struct P2R {
+  static constexpr int NBA = (SP + 1) / 2, NBB = SP - NBA;   // n-blocks of the two N chunks of a half (SP n-blocks)
+  static constexpr int SLICE = 32 * NBA + 16;                // doubles per staged row slice (+128 B: rows on distinct banks)
+  static constexpr int RING = 64;                            // kept rows in flight per warp
+  // per warp: own dT tile [16 SP][4] | dT_j slices [8][SLICE] | ring (d, r) [RING] | ring j [RING] | ring row of j | mbarrier
+  static constexpr int per_warp = 64 * SP + 8 * SLICE + 4 * RING + RING / 2 + RING / 2 + 2;
+};
+
+// value and tangent MMAs of NB n-blocks (starting at n-block NB0 of the half), then the epilogue over their 2 NB slots
+template <int SP, int NB, int NB0>
+__device__ __forceinline__ void p2r_chunk(const double *__restrict__ W2h, const double *__restrict__ b2h,
+                                          const double *__restrict__ dTh, const double *__restrict__ jrow,
+                                          const bool anyboth, uint64_t *mbar, unsigned &parity,
+                                          const double (&h1v)[2 * SP], const double (&h1t)[2 * SP],
+                                          const double (&e)[4], const int g, const int q, double (&pr)[5],
+                                          double (&pj)[5]) {
+  using L = EL<SP>;
+  double av[2 * NB], at[2 * NB];
+#pragma unroll
+  for (int nb = 0; nb < NB; ++nb) {
+    const double2 bb = *reinterpret_cast<const double2 *>(b2h + 8 * (NB0 + nb) + 2 * q);
+    av[2 * nb] = bb.x; av[2 * nb + 1] = bb.y;
+    at[2 * nb] = 0.0; at[2 * nb + 1] = 0.0;
+  }
+#pragma unroll
+  for (int ks = 0; ks < 2 * SP; ++ks) {
+#pragma unroll
+    for (int nb = 0; nb < NB; ++nb) {
+      const double b = W2h[(4 * ks + q) * L::LD2 + 8 * (NB0 + nb) + g];
+      dmma884(av[2 * nb], av[2 * nb + 1], h1v[ks], b);
+      dmma884(at[2 * nb], at[2 * nb + 1], h1t[ks], b);
+    }
+  }
+  // g and g' of the chunk's slots (left in av / at), and the direction i -> j against the atom's own dT tile
+#pragma unroll
+  for (int s = 0; s < 2 * NB; ++s) {
+    const int sl = 2 * NB0 + s;                             // slot inside the half: the skip comes from slot sl of layer 1
+    const double t2 = dp_tanh(av[s]);
+    const double gv = h1v[sl] + t2;
+    const double gp = fma(fma(-t2, t2, 1.0), at[s], h1t[sl]);
+    av[s] = gv; at[s] = gp;
+    const double4 d4 = *reinterpret_cast<const double4 *>(dTh + 4 * (4 * sl + q));
+    pr[0] = fma(d4.x, gv, pr[0]);
+    pr[1] = fma(d4.y, gv, pr[1]);
+    pr[2] = fma(d4.z, gv, pr[2]);
+    pr[3] = fma(d4.w, gv, pr[3]);
+    const double dg = fma(d4.x, e[0], fma(d4.y, e[1], fma(d4.z, e[2], d4.w * e[3])));
+    pr[4] = fma(dg, gp, pr[4]);
+  }
+  if (anyboth) {                                            // direction j -> i: dT_j (staged slice), R~_ji = (s, -s d/r)
+    tc::mbar_wait(mbar, parity);
+    parity ^= 1u;
+#pragma unroll
+    for (int s = 0; s < 2 * NB; ++s) {
+      const double4 d4 = *reinterpret_cast<const double4 *>(jrow + 4 * (4 * s + q));
+      pj[0] = fma(d4.x, av[s], pj[0]);
+      pj[1] = fma(d4.y, av[s], pj[1]);
+      pj[2] = fma(d4.z, av[s], pj[2]);
+      pj[3] = fma(d4.w, av[s], pj[3]);
+      const double dg = fma(d4.x, e[0], -fma(d4.y, e[1], fma(d4.z, e[2], d4.w * e[3])));
+      pj[4] = fma(dg, at[s], pj[4]);
+    }
+  }
+}
+
+template <int SP>
+__global__ void __launch_bounds__((32 * P2_WARPS), 1)
+k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a, double *__restrict__ force,
+                double *__restrict__ virial) {
+  using L = EL<SP>;
+  using R = P2R<SP>;
+  extern __shared__ __align__(16) double smem[];
+  double *W = smem;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
+  double *dTt = smem + ((L::total + 1) & ~1) + warp * R::per_warp;      // [16 SP][4], position 4 s + q
+  double *jbuf = dTt + 64 * SP;                                         // [8][SLICE]
+  double4 *rdv = reinterpret_cast<double4 *>(jbuf + 8 * R::SLICE);      // ring of kept rows: (d, r)
+  int *rjn = reinterpret_cast<int *>(rdv + R::RING);                    //   input index of the neighbour (force scatter)
+  int *rqj = rjn + R::RING;                                             //   its row in this chunk when both directions run, else -1
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(rqj + R::RING);
+  __shared__ double vred[P2_WARPS][9];
+  for (int k = tid; k < L::total; k += (32 * P2_WARPS)) W[k] = netp[k];
+  if (lane == 0) tc::mbar_init(mbar, 1);
+  tc::fence_mbar_init();
+  __syncthreads();
+  const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
+               *b2p = W + L::ob2;
+  const int t = a;
+  const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
+  const bool ru = C.stats->n_overflow == 0ull;           // a dropped neighbour breaks the symmetry of the lists
+  const size_t dt_tile = (size_t)C.dt_rows * 4;          // doubles per dT tile (= 64 SP)
+  unsigned parity = 0;
+  double vir[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+
+  for (int qa = row_lo + blockIdx.x * P2_WARPS + warp; qa < row_hi; qa += gridDim.x * P2_WARPS) {
+    const int n = C.nreal[(size_t)qa * P.ntypes + t];
+    if (n == 0) continue;
+    const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
+    const int *nl = C.nl + (size_t)qa * P.nm + P.sec_start[t];
+    const int *nlp = C.nlp + (size_t)qa * P.nm + P.sec_start[t];
+    __syncwarp();
+    {
+      const double4 *src = reinterpret_cast<const double4 *>(C.dT + (size_t)qa * dt_tile);
+      for (int p = lane; p < 16 * SP; p += 32) *reinterpret_cast<double4 *>(dTt + 4 * p) = src[p];
+    }
+    // kept rows: sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs
+    int head = 0, cnt = 0, rawpos = 0, sweep = ru ? 0 : 1;
+    bool done = false;
+    auto refill = [&]() {
+      const int slot = rawpos + lane;
+      bool keep = false;
+      int qj = -1;
+      if (slot < n) {
+        if (ru) {
+          const int pj = nlp[slot] - C.p0;
+          const bool inchunk = pj >= 0 && pj < C.n;
+          if (sweep == 0) { keep = inchunk && ((((qa + pj) & 1) == 0) == (qa < pj)); qj = pj; }
+          else keep = !inchunk;
+        } else {
+          keep = true;
+        }
+      }
+      const unsigned mk = __ballot_sync(0xffffffffu, keep);
+      if (keep) {
+        const int pos = (head + cnt + __popc(mk & ((1u << lane) - 1u))) & (R::RING - 1);
+        rdv[pos] = dr[slot]; rjn[pos] = nl[slot]; rqj[pos] = qj;
+      }
+      cnt += __popc(mk);
+      rawpos += 32;
+      if (rawpos >= n) {
+        if (ru && sweep == 0) { sweep = 1; rawpos = 0; } else done = true;
+      }
+    };
+    // both-direction rows of the block at the ring head, and (lanes 0..7) the row of neighbour j of ring row `lane`
+    int myqj = -1;
+    auto block_mask = [&]() -> unsigned {
+      myqj = (lane < 8 && lane < cnt) ? rqj[(head + lane) & (R::RING - 1)] : -1;
+      return __ballot_sync(0xffffffffu, myqj >= 0);
+    };
+    // TMA: the dT_j slices of N chunk k (0..3) of the block at the ring head -> jbuf rows
+    auto issue = [&](const unsigned bm, const int k) {
+      if (bm == 0u) return;
+      const int slot0 = (k >> 1) * 2 * SP + ((k & 1) ? 2 * R::NBA : 0);
+      const unsigned bytes = ((k & 1) ? R::NBB : R::NBA) * 256u;
+      if (lane == 0) tc::mbar_arrive_expect_tx(mbar, (unsigned)__popc(bm) * bytes);
+      __syncwarp();
+      if (myqj >= 0) tc::bulk_g2s(jbuf + lane * R::SLICE, C.dT + (size_t)myqj * dt_tile + 16 * slot0, bytes, mbar);
+    };
+    while (cnt < 16 && !done) refill();
+    __syncwarp();
+    unsigned bmask = block_mask();
+    issue(bmask, 0);
+    double fi[3] = {0.0, 0.0, 0.0};
+
+    while (cnt > 0) {
+      const int nrows = min(cnt, 8);
+      const bool valid = g < nrows;
+      const bool both = (bmask >> g) & 1u;
+      const bool anyboth = bmask != 0u;
+      double e[4] = {0.0, 0.0, 0.0, 0.0};
+      double4 dv = make_double4(0.0, 0.0, 0.0, 1.0);
+      int jn = 0;
+      if (valid) {
+        const int ri = (head + g) & (R::RING - 1);
+        dv = rdv[ri]; jn = rjn[ri];
+        env_row4(P, dv, e);
+      }
+      // layer 0 and its tangent: h0' = (1 - t0^2) W0   (d tanh = 1 - tanh^2)
+      double h0v[SP], h0t[SP];
+#pragma unroll
+      for (int s = 0; s < SP; ++s) {
+        const double w0 = W0p[4 * s + q], bb = b0p[4 * s + q];
+        const double t0 = dp_tanh(fma(e[0], w0, bb));
+        h0v[s] = t0;
+        h0t[s] = fma(-t0, t0, 1.0) * w0;
+      }
+      double h1v[2 * SP], h1t[2 * SP];
+#pragma unroll
+      for (int nb = 0; nb < L::NB1; ++nb) {
+        const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
+        h1v[2 * nb] = bb.x; h1v[2 * nb + 1] = bb.y;
+        h1t[2 * nb] = 0.0; h1t[2 * nb + 1] = 0.0;
+      }
+#pragma unroll
+      for (int ks = 0; ks < SP; ++ks) {
+#pragma unroll
+        for (int nb = 0; nb < L::NB1; ++nb) {
+          const double b = W1p[(4 * ks + q) * L::LD1 + 8 * nb + g];
+          dmma884(h1v[2 * nb], h1v[2 * nb + 1], h0v[ks], b);
+          dmma884(h1t[2 * nb], h1t[2 * nb + 1], h0t[ks], b);
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < 2 * SP; ++s) {
+        const double t1 = dp_tanh(h1v[s]);
+        h1v[s] = h0v[s % SP] + t1;
+        h1t[s] = fma(fma(-t1, t1, 1.0), h1t[s], h0t[s % SP]);
+      }
+      double pr[5] = {0.0, 0.0, 0.0, 0.0, 0.0};         // partial dR~_ij[0..3], dx over this thread's features
+      double pj[5] = {0.0, 0.0, 0.0, 0.0, 0.0};         // the same for the direction j -> i
+      const double *jrow = jbuf + g * R::SLICE;
+#pragma unroll 1
+      for (int half = 0; half < 2; ++half) {
+        const double *W2h = W2p + 8 * half * SP, *b2h = b2p + 8 * half * SP, *dTh = dTt + 32 * half * SP;
+        p2r_chunk<SP, R::NBA, 0>(W2h, b2h, dTh, jrow, anyboth, mbar, parity, h1v, h1t, e, g, q, pr, pj);
+        __syncwarp();                                    // every lane has read its slice: the next one may land
+        issue(bmask, 2 * half + 1);
+        if (R::NBB > 0) p2r_chunk<SP, R::NBB, R::NBA>(W2h, b2h, dTh, jrow, anyboth, mbar, parity, h1v, h1t, e, g, q, pr, pj);
+        __syncwarp();
+        if (half == 0) issue(bmask, 2);
+      }
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        pr[k] += __shfl_xor_sync(0xffffffffu, pr[k], 1);
+        pr[k] += __shfl_xor_sync(0xffffffffu, pr[k], 2);
+      }
+      if (anyboth) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+          pj[k] += __shfl_xor_sync(0xffffffffu, pj[k], 1);
+          pj[k] += __shfl_xor_sync(0xffffffffu, pj[k], 2);
+        }
+      }
+      // advance the ring and start the next block's first slices before the scalar tail of this one
+      head = (head + nrows) & (R::RING - 1);
+      cnt -= nrows;
+      while (cnt < 16 && !done) refill();
+      __syncwarp();
+      bmask = block_mask();
+      issue(bmask, 0);
+      if (valid && q == 0) {
+        // O10: derivative of R~ with respect to the displacement; f_ik[c] = sum_m dR~[m] dR~_m / dd_c
+        const double r = dv.w, ir = 1.0 / r;
+        double w, dw;
+        dp_switch(r, P.rcs, P.rc, w, dw);
+        const double s = w * ir, qq = s * ir;
+        const double sp = dw * ir - w * ir * ir;
+        const double qp = sp * ir - s * ir * ir;
+        const double dot = pr[1] * dv.x + pr[2] * dv.y + pr[3] * dv.z;
+        const double cm = ((pr[0] + pr[4]) * sp + qp * dot) * ir;
+        double f0 = fma(cm, dv.x, qq * pr[1]), f1 = fma(cm, dv.y, qq * pr[2]), f2 = fma(cm, dv.z, qq * pr[3]);
+        if (both) {                                      // f_ji = dE_j/dd_ji with d_ji = -d_ij; the pair force is f_ij - f_ji
+          const double dotj = -(pj[1] * dv.x + pj[2] * dv.y + pj[3] * dv.z);
+          const double cmj = ((pj[0] + pj[4]) * sp + qp * dotj) * ir;
+          f0 -= fma(-cmj, dv.x, qq * pj[1]);
+          f1 -= fma(-cmj, dv.y, qq * pj[2]);
+          f2 -= fma(-cmj, dv.z, qq * pj[3]);
+        }
+        if (force) {
+          atomicAdd(&force[3 * (size_t)jn + 0], -f0);
+          atomicAdd(&force[3 * (size_t)jn + 1], -f1);
+          atomicAdd(&force[3 * (size_t)jn + 2], -f2);
+        }
+        fi[0] += f0; fi[1] += f1; fi[2] += f2;
+        vir[0] -= dv.x * f0; vir[1] -= dv.x * f1; vir[2] -= dv.x * f2;
+        vir[3] -= dv.y * f0; vir[4] -= dv.y * f1; vir[5] -= dv.y * f2;
+        vir[6] -= dv.z * f0; vir[7] -= dv.z * f1; vir[8] -= dv.z * f2;
+      }
+    }
+    // F_i += sum_k f_ik (ProdForce)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      double v = fi[k];                                 // only the q == 0 lanes hold contributions; every lane gets the sum
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+      fi[k] = v;
+    }
+    if (lane < 3 && force) atomicAdd(&force[3 * (size_t)C.s_idx[C.p0 + qa] + lane], lane == 0 ? fi[0] : (lane == 1 ? fi[1] : fi[2]));
+  }
+#pragma unroll
+  for (int k = 0; k < 9; ++k) {
+    double v = vir[k];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if (lane == 0) vred[warp][k] = v;
+  }
+  __syncthreads();
+  if (tid < 9 && virial) {
+    double v = 0.0;
+    for (int w = 0; w < P2_WARPS; ++w) v += vred[w][tid];
+    atomicAdd(&virial[tid], v);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 static int g_sm_count = 0;
 
@@ -619,6 +911,15 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     if (e != cudaSuccess) return e;
     configured = true;
   }
+  using R = P2R<SP>;
+  const size_t smem_ru = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * R::per_warp);
+  const bool reuse = C.reuse2 && !C.fslot && C.nlp && C.dt_pad == 4 * SP && smem_ru <= 227 * 1024;
+  static bool configured_ru = false;
+  if (reuse && !configured_ru) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_ru<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ru);
+    if (e != cudaSuccess) return e;
+    configured_ru = true;
+  }
   const int grid = min(g_sm_count, (C.n + P2_WARPS - 1) / P2_WARPS);
   // the nets are independent here (forces and virial are atomic sums, slot stores are disjoint): a stream per net, so
   // that the tail of every launch is filled by the others
@@ -629,8 +930,13 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
   for (int a = P.ntypes - 1; a >= 0; --a)
     for (int t = P.ntypes - 1; t >= 0; --t) {
       const int net = a * P.ntypes + t;
-      k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, ts[(P.ntypes * P.ntypes - 1 - net) % ns]>>>(
-          P, C, W.emb + (size_t)net * W.net_stride, a, t, force, virial);
+      cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
+      if (reuse && a == t)
+        k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, force,
+                                                                     virial);
+      else
+        k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
+                                                              virial);
       DPB_LAUNCHED(1);
     }
   if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;

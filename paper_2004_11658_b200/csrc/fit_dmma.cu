@@ -233,7 +233,7 @@ __global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restr
     for (int a = 0; a < P.Ma; ++a) acc += dd[b * ldr + a] * Ts[a * 4 + c];
     if (b < P.Ma)
       for (int pt = 0; pt < nparts; ++pt) acc += part[pt * nout2 + e];
-    C.dT[(size_t)q * P.M * 4 + e] = acc;
+    C.dT[dt_offset(P, C, q, b) + c] = acc;
   }
 }
 
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView
         c2[1][c] = fma(d.y, tb, c2[1][c]);
       }
       if (lane % LPR == 0) {
-        double2 *o = reinterpret_cast<double2 *>(b < Ma ? f1 + 4 * b : C.dT + ((size_t)q * M + b) * 4);
+        double2 *o = reinterpret_cast<double2 *>(b < Ma ? f1 + 4 * b : C.dT + dt_offset(P, C, q, b));
         o[0] = make_double2(s[0], s[1]);
         o[1] = make_double2(s[2], s[3]);
       }
@@ -313,7 +313,7 @@ __global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView
   }
   __syncwarp();
   if (lane < Ma && lane < M) {
-    double2 *o = reinterpret_cast<double2 *>(C.dT + ((size_t)q * M + lane) * 4);
+    double2 *o = reinterpret_cast<double2 *>(C.dT + dt_offset(P, C, q, lane));
     o[0] = make_double2(f1[4 * lane] + t2[4 * lane], f1[4 * lane + 1] + t2[4 * lane + 1]);
     o[1] = make_double2(f1[4 * lane + 2] + t2[4 * lane + 2], f1[4 * lane + 3] + t2[4 * lane + 3]);
   }

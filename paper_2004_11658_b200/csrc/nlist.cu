@@ -259,14 +259,20 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
 
   int nh = n_hit;
   if (nh > cap) {
+    // More in-range candidates than staging slots (DPB_ECAP): cnt[] counted every hit but only `cap` were staged, so
+    // the ranks below could not fill the slots that nreal would promise.  The row is written as EMPTY (all -1,
+    // nreal = 0): the passes that are enqueued behind this kernel never touch an unwritten slot; the evaluation is
+    // reported as failed through err_cap.
     if (tid == 0) atomicExch(&stats->err_cap, 1);
-    nh = cap;
+    if (tid < DPB_MAX_TYPES) cnt[tid] = 0;
+    nh = 0;
   }
   if (MODE == 1 && tid == 0) {
     R.nraw[p] = n_raw;
     if (n_raw > R.cap) atomicExch(&stats->err_cap, 1);
   }
   int *nl_row = C.nl + (size_t)q * P.nm;
+  int *nlp_row = C.nlp ? const_cast<int *>(C.nlp) + (size_t)q * P.nm : nullptr;
   double4 *dr_row = C.dr + (size_t)q * P.nm;
   int *out_row = nlist_out ? nlist_out + (size_t)i * P.nm : nullptr;
 
@@ -310,6 +316,7 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
       nl_row[slot] = me.j;
       if (out_row) out_row[slot] = me.j;
       const int pj = hp[h];
+      if (nlp_row) nlp_row[slot] = pj;
       const double xj[3] = {s_xyz[3 * (size_t)pj], s_xyz[3 * (size_t)pj + 1], s_xyz[3 * (size_t)pj + 2]};
       double d[3], rr;
       dp_displacement(xi, xj, G.L, d, rr);
@@ -418,7 +425,7 @@ __global__ void k_scatter_debug(DevModel P, ChunkView C, double *dbgT, double *d
   const int n = P.M * 4;
   for (int k = threadIdx.x; k < n; k += blockDim.x) {
     if (dbgT) dbgT[(size_t)i * n + k] = C.T[(size_t)q * n + k];
-    if (dbgdT) dbgdT[(size_t)i * n + k] = C.dT[(size_t)q * n + k];
+    if (dbgdT) dbgdT[(size_t)i * n + k] = C.dT[dt_offset(P, C, q, k >> 2) + (k & 3)];
   }
 }
 

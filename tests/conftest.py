@@ -67,3 +67,53 @@ def random_box(n, L, ntypes, seed, min_dist=0.7):
     coord = np.array(pts)
     types = rng.integers(0, ntypes, n).astype(np.int32)
     return coord, types, np.diag([L, L, L]).reshape(9).astype(np.float64)
+
+
+_ORACLE_FULL = {}
+
+
+def oracle_full(name, conditioned):
+    """The CPU oracle's complete evaluation (dpo_eval over its own cell list, itself pinned against its brute-force search
+    in tests/test_oracle_nlist.py) of a BASELINE.json workload at full size, cached for the session: the reference of
+    every element-by-element parity test at the sizes bench.py times.  Returns (spec, emb, fit, coord, types, box, ref)."""
+    key = (name, bool(conditioned))
+    if key not in _ORACLE_FULL:
+        import gen
+        from gen.weights import MODELS
+        from oracle import Oracle
+        spec = MODELS[name]
+        coord, types, box = gen.make_system(name)
+        emb, fit = gen.make_weights(spec)
+        if conditioned:
+            fit = gen.condition_fit_w0(spec, fit)
+        ref = Oracle.from_spec(spec, emb, fit).eval(coord, types, box, cells=True)
+        _ORACLE_FULL[key] = (spec, emb, fit, coord, types, box, ref)
+    return _ORACLE_FULL[key]
+
+
+def oracle_forces_of(orc, coord, types, box, atoms):
+    """Forces of the listed atoms from the oracle's per-row pieces, for boxes too large for a whole oracle evaluation:
+    F_i = sum_k f_ik - sum_{j : i in L(j)} f_{j, slot of i}   (Eq. 10 with ProdForce; the
+    assembly is pinned by tests/test_oracle_physics.py::test_atom_rows_pieces_assemble_to_eval).  Needs no neighbour
+    overflow (then i in L(j) <=> j in L(i)).  Returns (F [len(atoms)][3], E_i [len(atoms)], nlist rows of the atoms)."""
+    atoms = np.asarray(atoms, dtype=np.int64)
+    nl_i, ovf = orc.build_nlist(coord, types, box, rows=atoms)
+    assert ovf == 0
+    nbrs = np.unique(nl_i[nl_i >= 0]).astype(np.int64)
+    rows = np.unique(np.concatenate([atoms, nbrs]))
+    nl, ovf = orc.build_nlist(coord, types, box, rows=rows)
+    assert ovf == 0
+    out = orc.atom_rows(coord, types, box, rows, nl)
+    where = {int(r): k for k, r in enumerate(rows)}
+    F = np.zeros((len(atoms), 3))
+    E = np.zeros(len(atoms))
+    for a, i in enumerate(atoms):
+        qi = where[int(i)]
+        F[a] = out["fslot"][qi][nl[qi] >= 0].sum(0)
+        E[a] = out["atom_energy"][qi]
+        for j in nl[qi][nl[qi] >= 0]:
+            qj = where[int(j)]
+            hit = np.where(nl[qj] == i)[0]
+            assert len(hit) == 1
+            F[a] -= out["fslot"][qj, hit[0]]
+    return F, E, nl_i

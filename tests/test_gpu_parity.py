@@ -212,37 +212,34 @@ def test_errors_are_reported_not_thrown_from_c():
     m.close()
 
 
+@pytest.mark.parametrize("conditioned", [False, True])
 @pytest.mark.parametrize("name", ["W24k", "Cu32k"])
-def test_full_size_sampled_parity(name):
-    """BASELINE configs 1 and 2 at full size, in the launch configuration bench.py times (variant 1, default chunk):
-    sampled atoms against the oracle (nlist rows bit-exact, E_i, T, dT), plus whole-system properties that hold at
-    any size: sum F = 0, symmetric virial, force parity between the two kernel generations."""
+def test_full_size_parity_every_element(name, conditioned):
+    """BASELINE configs 1 and 2 at full size, in the launch configuration bench.py times (variant 1, default chunk,
+    default pair reuse) and on the weight set it times (literal) as well as the conditioned one: EVERY output element
+    against the oracle's whole evaluation — nlist bit-exact on all rows, E, E_i, every force component, the virial
+    (Eq. 10; ProdForce / ProdVirial :240), T and dT through the debug buffers on sampled rows.
+    The pair reuse is also switched off and on again; the two kernel generations are compared as an extra."""
+    from conftest import oracle_full
     torch = _torch()
-    spec = MODELS[name]
-    coord, types, box = gen.make_system(name)
-    emb, fit = gen.make_weights(spec)
-    fit = gen.condition_fit_w0(spec, fit)
+    spec, emb, fit, coord, types, box, ref = oracle_full(name, conditioned)
     orc, m = _models(spec, emb, fit, 1)
     got = _gpu_eval(m, coord, types, box, debug=True, spec=spec)
-    n = coord.shape[0]
-    rows = np.random.default_rng(1).choice(n, 48, replace=False).astype(np.int64)
-    nl_ref, _ = orc.build_nlist(coord, types, box, rows=rows)
-    assert np.array_equal(got["nlist"][rows], nl_ref)
-    ar = orc.atom_rows(coord, types, box, rows, nl_ref, want_T=True)
-    assert np.abs(got["atom_energy"][rows] - ar["atom_energy"]).max() <= E_REL * np.abs(ar["atom_energy"]).max()
+    _check_full(ref, got)
+    assert got["info"].n_real_pairs == int((ref["nlist"] >= 0).sum())
+    rows = np.random.default_rng(1).choice(coord.shape[0], 48, replace=False).astype(np.int64)
+    ar = orc.atom_rows(coord, types, box, rows, ref["nlist"][rows], want_T=True)
     assert np.abs(got["T"][rows] - ar["T"]).max() <= 1e-12 * np.abs(ar["T"]).max()
     assert np.abs(got["dT"][rows] - ar["dT"]).max() <= 1e-11 * np.abs(ar["dT"]).max()
-    # forces of the sampled atoms' own slots: F_i gets contributions from neighbours' lists too, so compare the two
-    # independent kernel generations on every atom instead, and check the conservation laws
-    assert np.abs(got["force"].sum(0)).max() <= 1e-9
-    assert np.abs(got["virial"] - got["virial"].T).max() <= 1e-9 * np.abs(got["virial"]).max()
     assert abs(got["energy"][0] - got["atom_energy"].sum()) <= 1e-12 * np.abs(got["atom_energy"]).sum()
-    m0 = _models(spec, emb, fit, 0)[1]
-    got0 = _gpu_eval(m0, coord, types, box)
-    assert np.array_equal(got0["nlist"], got["nlist"])
-    assert np.abs(got0["force"] - got["force"]).max() <= F_ABS
-    assert abs(got0["energy"][0] - got["energy"][0]) <= E_REL * abs(got0["energy"][0])
-    m.close(); m0.close()
+    for reuse in (0, 2):
+        m.set_pair_reuse(reuse)
+        _check_full(ref, _gpu_eval(m, coord, types, box))
+    m.close()
+    if not conditioned:
+        m0 = _models(spec, emb, fit, 0)[1]
+        _check_full(ref, _gpu_eval(m0, coord, types, box))
+        m0.close()
 
 
 def test_eval_host_matches_device_entry():
@@ -260,15 +257,21 @@ def test_eval_host_matches_device_entry():
     m.close()
 
 
-def test_config5_copper_864k_sampled():
-    """BASELINE configs[4]: 864,000-atom copper box (27 chunks of 32,768 atoms).  Sampled rows against the oracle
-    (nlist bit-exact, E_i), conservation laws, and extensivity: the box is NOT a replica of config 2 (independent
-    jitter), so extensivity is checked on E / N against the 32,000-atom box only loosely (same lattice, same model)."""
+@pytest.mark.parametrize("conditioned", [False, True])
+def test_config5_copper_864k_sampled(conditioned):
+    """BASELINE configs[4]: 864,000-atom copper box (27 chunks of 32,768 atoms), too large for a whole oracle evaluation
+    inside the test budget.  Against the oracle, element by element, on sampled atoms — 16 random ones plus the two
+    atoms on either side of four chunk boundaries (sorted order through dpb_debug_sorted_order): nlist rows bit-exact,
+    E_i, and the FORCE, assembled from the oracle's per-row pieces F_i = sum_k f_ik - sum_{j: i in L(j)} f_{j,slot(i)}
+    over the atom and all of its neighbours (conftest.oracle_forces_of).  Whole-box properties: sum F = 0, symmetric
+    virial, E = sum E_i.  The box is not a replica of config 2 (independent jitter), so no extensivity check."""
+    from conftest import oracle_forces_of
     torch = _torch()
     spec = MODELS["Cu864k"]
     coord, types, box = gen.make_system("Cu864k")
     emb, fit = gen.make_weights(spec)
-    fit = gen.condition_fit_w0(spec, fit)
+    if conditioned:
+        fit = gen.condition_fit_w0(spec, fit)
     orc, m = _models(spec, emb, fit, 1)
     dc = torch.tensor(coord, device="cuda")
     dt = torch.tensor(types, device="cuda")
@@ -276,14 +279,17 @@ def test_config5_copper_864k_sampled():
     torch.cuda.synchronize()
     info = out["info"]
     assert info.n_overflow == 0 and info.n_chunks == 27
-    rows = np.random.default_rng(2).choice(coord.shape[0], 12, replace=False).astype(np.int64)
-    nl_ref, _ = orc.build_nlist(coord, types, box, rows=rows)
-    nl = out["nlist"][torch.tensor(rows, device="cuda")].cpu().numpy()
-    assert np.array_equal(nl, nl_ref)
-    ar = orc.atom_rows(coord, types, box, rows, nl_ref)
+    order = m.sorted_order(coord.shape[0]).cpu().numpy().astype(np.int64)
+    assert np.array_equal(np.sort(order), np.arange(coord.shape[0]))
+    edge = [order[c * 32768 + d] for c in (1, 9, 17, 26) for d in (-1, 0)]
+    atoms = np.unique(np.concatenate([np.random.default_rng(2).choice(coord.shape[0], 16, replace=False), edge]))
+    F_ref, E_ref, nl_ref = oracle_forces_of(orc, coord, types, box, atoms)
+    sel = torch.tensor(atoms, device="cuda")
+    assert np.array_equal(out["nlist"][sel].cpu().numpy(), nl_ref)
     ei = out["atom_energy"].cpu().numpy()
-    assert np.abs(ei[rows] - ar["atom_energy"]).max() <= E_REL * np.abs(ar["atom_energy"]).max()
+    assert np.abs(ei[atoms] - E_ref).max() <= E_REL * np.abs(E_ref).max()
     f = out["force"].cpu().numpy()
+    assert np.abs(f[atoms] - F_ref).max() <= F_ABS
     assert np.abs(f.sum(0)).max() <= 1e-9
     v = out["virial"].cpu().numpy()
     assert np.abs(v - v.T).max() <= 1e-9 * np.abs(v).max()
@@ -424,4 +430,38 @@ def test_pair_reuse_matches_oracle_and_the_plain_pass(name, chunk):
     scale = np.abs(res[False]["T"]).max()
     assert np.abs(res[True]["T"] - res[False]["T"]).max() <= 1e-13 * scale
     assert np.abs(res[True]["force"] - res[False]["force"]).max() <= 1e-11
+    m.close()
+
+
+def test_staging_capacity_overflow_is_reported_and_touches_no_unwritten_slot():
+    """More in-range candidates than the staging capacity max(256, 2 Nm) (a mis-scaled, far too dense input): the call
+    with info reports DPB_ECAP; the overflowing rows are written empty (all -1), so the passes enqueued behind the
+    neighbour kernel read no stale slot — the call without info runs through, outputs are finite, dpb_model_status
+    then reports the error, and the model still evaluates a sane input correctly afterwards."""
+    from paper_2004_11658_b200 import DPBError
+    torch = _torch()
+    spec, emb, fit = small_model(ntypes=1, s1=4, m_axis=3, fit_width=8, sel=(20,), rcut=4.0, rcut_smth=1.0, seed=5)
+    orc, m = _models(spec, emb, fit, 1)
+    rng = np.random.default_rng(12)
+    n = 2000                                             # 2000 atoms in a 9 A box: ~730 atoms inside r_c = 4 > cap = 256
+    coord = rng.uniform(0, 9.0, (n, 3))
+    types = np.zeros(n, dtype=np.int32)
+    box = np.diag([9.0] * 3).reshape(9)
+    dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types, device="cuda")
+    with pytest.raises(DPBError) as e:
+        m.eval(dc, dt, box, want_info=True)
+    assert e.value.status == -5
+    out = m.eval(dc, dt, box, want_nlist=True)           # no info: DPB_OK now, the error is deferred
+    torch.cuda.synchronize()
+    assert bool((out["nlist"] == -1).all())
+    assert bool(torch.isfinite(out["force"]).all()) and bool(torch.isfinite(out["atom_energy"]).all())
+    with pytest.raises(DPBError) as e:
+        m.status()
+    assert e.value.status == -5
+    coord2, types2, box2 = random_box(60, 10.0, 1, seed=2, min_dist=1.0)
+    ref = orc.eval(coord2, types2, box2)
+    got = _gpu_eval(m, coord2, types2, box2)
+    assert np.array_equal(got["nlist"], ref["nlist"])
+    assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
+    m.status()
     m.close()

@@ -261,3 +261,23 @@ def test_atom_virial_is_minus_the_strain_derivative_of_each_atom_energy(water192
                 e.append(o.eval((x - 30.0) @ F.T + 30.0, t, big)["atom_energy"])
             fd = -(e[0] - e[1]) / (2 * h)                       # = -dE_i/d eps_ab = Xi_i[b][a]
             assert np.abs(fd - avc[:, b, a]).max() < 5e-7 * max(1.0, np.abs(fd).max()), (a, b)
+
+
+def test_sampled_force_assembly_helper_matches_the_whole_evaluation():
+    """conftest.oracle_forces_of (the reference of the 864,000-atom GPU parity tests) against dpo_eval on a small copper
+    box: the forces and E_i of sampled atoms, assembled from per-row pieces, equal the whole evaluation's."""
+    import gen
+    from gen.weights import MODELS
+    from oracle import Oracle
+    from conftest import oracle_forces_of
+    spec = MODELS["Cu32k"]
+    coord, types, box = gen.copper_box(5, 0.05, seed=3)
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc = Oracle.from_spec(spec, emb, fit)
+    full = orc.eval(coord, types, box)
+    atoms = np.array([0, 17, 250, 499])
+    F, E, nl = oracle_forces_of(orc, coord, types, box, atoms)
+    assert np.array_equal(nl, full["nlist"][atoms])
+    assert np.abs(F - full["force"][atoms]).max() < 1e-13
+    assert np.array_equal(E, full["atom_energy"][atoms])
