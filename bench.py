@@ -34,7 +34,13 @@ import gen  # noqa: E402
 from gen.weights import MODELS  # noqa: E402
 
 METRIC = "atom-steps/s"
-FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; measured 37.0
+FP64_FMA_PER_CLK = 148 * 64   # 148 SMs x 64 DFMA lanes per clock (measured 37.0 TF/s at 1965 MHz)
+
+
+def fp64_peak_tflops(sm_mhz):
+    """fp64 pipe peak at the SM clock sampled during the timed region (DFMA and DMMA share this pipe):
+    148 x 64 FMA/clk x 2 flop x clock; 37.2 TFLOP/s at the 1965 MHz the B200 holds in these runs."""
+    return FP64_FMA_PER_CLK * 2 * float(sm_mhz or 1965.0) * 1e6 / 1e12
 
 
 def tf32_peak_tflops():
@@ -51,7 +57,9 @@ def algorithmic_flops(spec, n_atoms, n_pairs):
     s1, M, Ma, w, D = spec.emb_s1, spec.m, spec.m_axis, spec.fit_width, spec.dim_descrpt
     gemm = 2 * (s1 + 2 * s1 * s1 + 8 * s1 * s1)                 # one direction, per neighbour
     emb_fwd = gemm + (s1 + 2 * s1 + 4 * s1) + (2 * s1 + 4 * s1) + 2 * 4 * M     # + bias, skip adds, T update
-    emb_bwd = gemm + 2 * 4 * M + 2 * 4 * M + 2 * (7 * s1) + (2 * s1 + 4 * s1) + 60   # dg, dR~, (1-t^2), folds, chain
+    # dg = dT R~ and dR~ = dT^T g (2 x 2*4*M), 1 - t^2 and its product (3 x 7 s1), the two concat folds
+    # (2 s1 + 4 s1), the chain to the displacement (36): 14,861 flop per neighbour for water, 23,492 for copper
+    emb_bwd = gemm + 2 * (2 * 4 * M) + 3 * (7 * s1) + (2 * s1 + 4 * s1) + 36
     fit = 2 * (D * w + 2 * w * w + w)                            # forward = backward, per atom
     contr = 3 * (2 * 4 * M * Ma)                                 # D, and the two dT terms
     return {
@@ -175,7 +183,7 @@ def workload_config(name, args):
             "parallelism": "replicas only (1 GPU per replica, no collectives)",
             "l2": "flushed between timed steps (256 MiB write)", "variant": getattr(args, "variant", 1),
             "precision": getattr(args, "precision", "fp64"),
-            "pair_reuse": "pass 1, nets (a,a), single-chunk evaluations (library default; fp64 variant 1 only)"}
+            "pair_reuse": "nets (a,a): pass 2 always, pass 1 in single-chunk evaluations (library default; fp64 variant 1)"}
 
 
 # ---- molecular dynamics: the paper's own unit, steps/s and ns/day ----------------------
@@ -185,7 +193,7 @@ def run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed):
     DESIGN.md section 3: forces ~0.2 eV/A rms); the kernels and their cost are the same."""
     import torch
     from paper_2004_11658_b200 import DPModel
-    model = DPModel.from_spec(spec, emb, gen.condition_fit_w0(spec, fit), precision=1 if mixed else 0)
+    model = DPModel.from_spec(spec, emb, gen.condition_fit_w0(spec, fit), precision={"fp64": 0, "tf32": 1, "bf16": 2}[args.precision])
     masses = gen.MASSES[name]
     dt_fs = 0.5 if spec.ntypes == 2 else 1.0                     # PAPER.md:298: 0.5 fs water, 1.0 fs copper
     vel = gen.maxwell_boltzmann(types, masses, 330.0, seed=gen.SEED_BASE + 500)
@@ -266,10 +274,153 @@ def run_dd(args, spec, name, coord, types, box, dev, model, world, rank):
 
 
 # ---- the CUDA arm ---------------------------------------------------------------------------------------------
-def run_cuda(args):
+STAGES = ["cell_sort", "nlist", "pass1_env_embed_T", "fit_fwd_bwd", "pass2_embed_bwd_force", "reduce"]
+
+
+def measure(name, precision, variant, steps, warmup, dev, rank=0, world=1, stage_every=10, want_e2e=False):
+    """Time `steps` evaluations of workload `name` (each on a freshly perturbed copy of its box, L2 flushed in between,
+    CUDA events on the launching stream, W untimed warm-up calls).  Returns a dict; times are this rank's."""
     import torch
     import torch.distributed as dist
     from paper_2004_11658_b200 import DPModel
+
+    spec = MODELS[name]
+    coord, types, box = gen.make_system(name, seed=gen.SEED_BASE + gen.CONFIGS[name].config_id + 7919 * rank)
+    emb, fit = gen.make_weights(spec)
+    n = coord.shape[0]
+    mixed = precision != "fp64"
+    model = DPModel.from_spec(spec, emb, fit, precision={"fp64": 0, "tf32": 1, "bf16": 2}[precision])
+    model.set_variant(variant)
+
+    # pool of freshly perturbed copies (reading R24: fresh perturbation of the base positions per call)
+    pool = min(steps + warmup, 16 if n < 200000 else 3)
+    host_coords = [gen.perturbed(coord, box, 0.01, gen.SEED_BASE + 1000 * (rank + 1) + k) for k in range(pool)]
+    dcoords = [torch.tensor(c, device=dev) for c in host_coords]
+    dtypes = torch.tensor(types, device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    out = model.eval(dcoords[0], dtypes, box, want_info=True)        # correctness guard + pair count (not timed)
+    info = out.pop("info")
+    assert info.n_overflow == 0, "neighbour overflow in the benchmark workload"
+    torch.cuda.synchronize()
+    torch.cuda.reset_peak_memory_stats(dev)
+    flops = algorithmic_flops(spec, n, info.n_real_pairs)
+    for k in range(warmup):
+        model.eval(dcoords[k % pool], dtypes, box, out=out)
+    barrier()
+
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    launches0 = model.kernel_launches()
+    wall0 = time.perf_counter()
+    for k in range(steps):
+        flush.zero_()                                            # L2 flush, outside the timed events
+        ev[k][0].record()
+        model.eval(dcoords[(warmup + k) % pool], dtypes, box, out=out)
+        ev[k][1].record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    launches = model.kernel_launches() - launches0
+    clocks = sampler.stop() if rank == 0 else {}
+    per_step = sorted(a.elapsed_time(b) for a, b in ev)
+    dev_ms = float(sum(per_step))
+    # per-stage device times from a few EXTRA steps with the library's stage timers on (events between the stages; they
+    # switch the CUDA-graph replay off, so they are kept out of the timed region)
+    stage_sum, n_stage = np.zeros(8), 0
+    if stage_every:
+        model.set_timing(True)
+        for k in range(max(1, min(steps, 5))):
+            flush.zero_()
+            model.eval(dcoords[k % pool], dtypes, box, out=out)
+            torch.cuda.synchronize()
+            stage_sum += np.array(model.stage_us())
+            n_stage += 1
+        model.set_timing(False)
+    stage_us = (stage_sum / max(1, n_stage)).tolist()
+    res = {"name": name, "precision": precision, "variant": variant, "spec": spec, "n": n, "info": info, "flops": flops,
+           "dev_ms": dev_ms, "ms_median": per_step[len(per_step) // 2], "ms_min": per_step[0], "wall": wall,
+           "launches": int(launches), "clocks": clocks, "stage_us": stage_us,
+           "coord": coord, "types": types, "box": box, "emb": emb, "fit": fit, "model": model}
+
+    if want_e2e:
+        # end to end through the host entry point (pinned host buffers, copies inside the timed region)
+        pc = [torch.tensor(c).pin_memory() for c in host_coords[:4]]
+        pt = torch.tensor(types).pin_memory()
+        hout = {"energy": torch.empty(1, dtype=torch.float64).pin_memory(),
+                "atom_energy": torch.empty(n, dtype=torch.float64).pin_memory(),
+                "force": torch.empty((n, 3), dtype=torch.float64).pin_memory(),
+                "virial": torch.empty((3, 3), dtype=torch.float64).pin_memory()}
+        e2e_steps = max(3, min(steps, 20))
+        for k in range(2):
+            model.eval_host(pc[k % len(pc)], pt, box, out=hout)
+        barrier()
+        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(e2e_steps):
+            model.eval_host(pc[k % len(pc)], pt, box, out=hout)
+        e1.record()
+        barrier()
+        e2e_wall = time.perf_counter() - t0
+        res.update(e2e_ms=max(e0.elapsed_time(e1), e2e_wall * 1e3), e2e_steps=e2e_steps,
+                   h2d=n * 3 * 8 + n * 4, d2h=8 + n * 8 + n * 24 + 72)
+    return res
+
+
+def stage_roofline(res, sm_mhz):
+    """Algorithmic roofline fraction of every fp64-pipe (or, in mixed precision, tensor-pipe) stage and of the whole step."""
+    mixed = res["precision"] != "fp64"
+    if mixed:
+        peak, how = tf32_peak_tflops()
+        if res["precision"] == "bf16":
+            peak, how = peak * 2.0, how.replace("x 1/2", "x 1")
+    else:
+        peak, how = fp64_peak_tflops(sm_mhz), f"148 SM x 64 FMA/clk x 2 x {sm_mhz or 1965.0:.0f} MHz (sampled)"
+    idx = {"pass1": 2, "fit": 3, "pass2": 4}
+    frac = {}
+    for k, i in idx.items():
+        t = res["stage_us"][i] * 1e-6
+        frac[k] = (res["flops"][k] / t / 1e12 / peak) if t > 0 else None
+    dom = max(idx, key=lambda k: res["stage_us"][idx[k]])
+    return peak, how, frac, dom
+
+
+def config_summary(res):
+    """One entry of the `configs` object: a BASELINE.json config in the launch configuration of the headline run."""
+    sm = res["clocks"].get("sm_mhz")
+    peak, how, frac, dom = stage_roofline(res, sm)
+    ms = res["ms_median"]
+    total = sum(res["flops"].values())
+    out = {"workload": f"{res['name']} (BASELINE.json configs[{gen.CONFIGS[res['name']].config_id}])",
+           "precision": res["precision"], "natoms": res["n"], "real_pairs": res["info"].n_real_pairs,
+           "n_overflow": res["info"].n_overflow, "n_chunks": res["info"].n_chunks,
+           "ms_per_step": ms, "ms_min": res["ms_min"], "us_per_eval": ms * 1e3,
+           "atom_steps_per_s": res["n"] / (ms * 1e-3),
+           "stage_us": {nm: res["stage_us"][i] for i, nm in enumerate(STAGES)},
+           "algorithmic_tflops": total / (ms * 1e-3) / 1e12,
+           "frac_of_peak": total / (ms * 1e-3) / 1e12 / peak,
+           "stage_frac_of_peak": frac, "dominant_stage": dom, "dominant_frac": frac[dom],
+           "peak_tflops": peak, "peak_how": how, "sm_mhz": sm, "reasons": res["clocks"].get("reasons", []),
+           "gpu_launches_per_step": res["launches"] / max(1, res["steps"])}
+    return out
+
+
+EXTRA_CONFIGS = [  # (workload, precision, steps, warmup): every BASELINE.json config beside the headline (W24k fp64)
+    ("W192", "fp64", 200, 10), ("Cu32k", "fp64", 5, 3), ("W24k", "tf32", 20, 5), ("W24k", "bf16", 20, 5),
+    ("Cu864k", "fp64", 3, 3),
+]
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -282,85 +433,14 @@ def run_cuda(args):
         dist.init_process_group("nccl", device_id=dev)
 
     name = args.workload
-    spec = MODELS[name]
-    coord, types, box = gen.make_system(name, seed=gen.SEED_BASE + gen.CONFIGS[name].config_id + 7919 * rank)
-    emb, fit = gen.make_weights(spec)
-    n = coord.shape[0]
-    mixed = args.precision == "tf32"
-    model = DPModel.from_spec(spec, emb, fit, precision=1 if mixed else 0)
-    model.set_variant(args.variant)
-    model.set_timing(True)
+    mixed = args.precision != "fp64"
+    res = measure(name, args.precision, args.variant, args.steps, args.warmup, dev, rank, world, args.stage_every,
+                  want_e2e=True)
+    res["steps"] = args.steps
+    spec, n, info, flops, model = res["spec"], res["n"], res["info"], res["flops"], res["model"]
+    coord, types, box, emb, fit = res["coord"], res["types"], res["box"], res["emb"], res["fit"]
 
-    # pool of freshly perturbed copies (reading R24: fresh perturbation of the base positions per call)
-    pool = min(args.steps + args.warmup, 16)
-    host_coords = [gen.perturbed(coord, box, 0.01, gen.SEED_BASE + 1000 * (rank + 1) + k) for k in range(pool)]
-    dcoords = [torch.tensor(c, device=dev) for c in host_coords]
-    dtypes = torch.tensor(types, device=dev)
-    out = None
-    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # correctness guard + pair count (not timed)
-    out = model.eval(dcoords[0], dtypes, box, want_info=True)
-    info = out.pop("info")
-    assert info.n_overflow == 0, "neighbour overflow in the benchmark workload"
-    torch.cuda.synchronize()
-    flops = algorithmic_flops(spec, n, info.n_real_pairs)
-
-    for k in range(args.warmup):
-        model.eval(dcoords[k % pool], dtypes, box, out=out)
-    barrier()
-
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    stage_sum = np.zeros(8)
-    launches0 = model.kernel_launches()
-    wall0 = time.perf_counter()
-    for k in range(args.steps):
-        flush.zero_()                                            # L2 flush, outside the timed events
-        ev[k][0].record()
-        model.eval(dcoords[(args.warmup + k) % pool], dtypes, box, out=out)
-        ev[k][1].record()
-        if args.stage_every and k % args.stage_every == 0:
-            torch.cuda.synchronize()
-            stage_sum += np.array(model.stage_us())
-    barrier()
-    wall = time.perf_counter() - wall0
-    launches = model.kernel_launches() - launches0
-    clocks = sampler.stop() if rank == 0 else {}
-    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
-    n_stage = len(range(0, args.steps, args.stage_every)) if args.stage_every else 0
-
-    # end to end through the host entry point (pinned host buffers, copies inside the timed region)
-    pc = [torch.tensor(c).pin_memory() for c in host_coords[:4]]
-    pt = torch.tensor(types).pin_memory()
-    hout = {"energy": torch.empty(1, dtype=torch.float64).pin_memory(),
-            "atom_energy": torch.empty(n, dtype=torch.float64).pin_memory(),
-            "force": torch.empty((n, 3), dtype=torch.float64).pin_memory(),
-            "virial": torch.empty((3, 3), dtype=torch.float64).pin_memory()}
-    e2e_steps = max(3, min(args.steps, 20))
-    for k in range(2):
-        model.eval_host(pc[k % 4], pt, box, out=hout)
-    barrier()
-    t0 = time.perf_counter()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for k in range(e2e_steps):
-        model.eval_host(pc[k % 4], pt, box, out=hout)
-    e1.record()
-    barrier()
-    e2e_wall = time.perf_counter() - t0
-    e2e_ms = max(e0.elapsed_time(e1), e2e_wall * 1e3)
-    h2d = n * 3 * 8 + n * 4
-    d2h = 8 + n * 8 + n * 24 + 72
-
-    times = torch.tensor([dev_ms, e2e_ms], dtype=torch.float64, device=dev)
+    times = torch.tensor([res["dev_ms"], res["e2e_ms"]], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
     dev_ms, e2e_ms = float(times[0]), float(times[1])
@@ -369,60 +449,88 @@ def run_cuda(args):
     dd_leg = run_dd(args, spec, name, coord, types, box, dev, model, world, rank) if args.dd else None
 
     if rank == 0:
+        clocks = res["clocks"]
         ms_per_step = dev_ms / args.steps
         value = world * n * args.steps / (dev_ms * 1e-3)
-        stage_us = (stage_sum / max(1, n_stage)).tolist()
-        names = ["cell_sort", "nlist", "pass1_env_embed_T", "fit_fwd_bwd", "pass2_embed_bwd_force", "reduce"]
-        stages = {nm: stage_us[i] for i, nm in enumerate(names)}
-        dom = max(("pass1", 2), ("fit", 3), ("pass2", 4), key=lambda kv: stage_us[kv[1]])
-        dom_t = stage_us[dom[1]] * 1e-6
-        achieved = flops[dom[0]] / dom_t / 1e12 if dom_t > 0 else None
+        stage_us = res["stage_us"]
+        stages = {nm: stage_us[i] for i, nm in enumerate(STAGES)}
+        peak, how, frac, dom = stage_roofline(res, clocks.get("sm_mhz"))
+        idx = {"pass1": 2, "fit": 3, "pass2": 4}
+        dom_t = stage_us[idx[dom]] * 1e-6
+        achieved = flops[dom] / dom_t / 1e12 if dom_t > 0 else None
         total_flops = sum(flops.values())
-        traffic = None
+        traffic, traffic_src = None, None
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get(f"{name}:{'tf32' if mixed else 'v' + str(args.variant)}:{dom[0]}")
+                tj = json.load(open(tpath))
+                traffic = tj.get(f"{name}:{args.precision if mixed else 'v' + str(args.variant)}:{dom}")
+                traffic_src = tj.get("source")
             except Exception:
                 traffic = None
         line = {
             "metric": METRIC, "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "tf32x3+f32acc (env/force/accumulations f64)" if mixed else "f64",
+            "vs_baseline": None,
+            "dtype": {"fp64": "f64", "tf32": "tf32x3+f32acc (env/force/accumulations f64)",
+                      "bf16": "bf16x6+f32acc (env/force/accumulations f64)"}[args.precision],
             "data": "synthetic", "config": workload_config(name, args),
-            "natoms_per_gpu": n, "real_pairs": info.n_real_pairs, "wall_s": wall,
+            "natoms_per_gpu": n, "real_pairs": info.n_real_pairs, "wall_s": res["wall"],
             "algorithmic_tflops": total_flops / (ms_per_step * 1e-3) / 1e12,
-            "fp64_frac_of_peak": total_flops / (ms_per_step * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
-            "stage_us": stages,
-            "roofline": {"bound": "alu", "kernel": dom[0], "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
-                         "unit": "TFLOP/s", "frac": (achieved / FP64_PEAK_TFLOPS) if achieved else None,
-                         "traffic": traffic,
-                         "note": "fp64 pipe (DFMA/DMMA share one pipe, measured 37.0 TF/s; peak derived from 148 SM x 64 "
-                                 "FMA/clk x 1.965 GHz); algorithmic flops of the stage / its CUDA-event time; the "
-                                 "embedding passes execute 2.4-2.8x their algorithmic flops (pass 2 recomputes the "
-                                 "forward chain and carries a tangent chain instead of reading stored activations; "
-                                 "tanh; 25 -> 28 padding on water) and keep the fp64 pipe 74-81 % busy (ncu: "
-                                 "profiles/r1_ncu_full_w24k.md, profiles/r1_ncu_full_cu32k.md)"},
-            "e2e": {"value": world * n * e2e_steps / (e2e_ms * 1e-3), "unit": "atom-steps/s",
-                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
-            "gpu_launches": int(launches),
+            "stage_us": stages, "stage_frac_of_peak": frac,
+            "roofline": {"bound": "tensor" if mixed else "alu", "kernel": dom, "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                         "traffic_note": ("DRAM bytes summed over ALL launches of this stage in one evaluation (ncu --set "
+                                          f"full, cold cache): {traffic_src}") if traffic else None,
+                         "peak_how": how},
+            "e2e": {"value": world * n * res["e2e_steps"] / (e2e_ms * 1e-3), "unit": "atom-steps/s",
+                    "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"], "steps": res["e2e_steps"]},
+            "gpu_launches": res["launches"],
             "clocks": {"sm_mhz": clocks.get("sm_mhz"), "sm_max_mhz": clocks.get("sm_max_mhz"),
                        "reasons": clocks.get("reasons", []), "samples": clocks.get("samples", 0),
                        "power_w_max": clocks.get("power_w_max")},
         }
-        if mixed:
-            # the GEMMs run on the tensor pipe: 3 TF32 MMAs per algorithmic product (3xTF32 split)
-            peak, how = tf32_peak_tflops()
-            line["roofline"] = {"bound": "tensor", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
-                                "note": f"algorithmic flops of the stage / its CUDA-event time against the dense TF32 peak "
-                                        f"({how}); the tensor pipe executes 3x these flops (3xTF32 split); the stage is bound "
-                                        f"by MUFU (fp32 tanh) and instruction issue, not by the tensor pipe (DESIGN.md)"}
-            line.pop("fp64_frac_of_peak", None)
+        if not mixed:
+            line["fp64_frac_of_peak"] = total_flops / (ms_per_step * 1e-3) / 1e12 / peak
+            line["roofline"]["note"] = (
+                "fp64 pipe: DFMA and DMMA share one pipe (measured 37.0 TF/s at 1965 MHz, profiles/r1_fp64_peaks.md); "
+                "`achieved` = ALGORITHMIC flops of the stage (SURVEY.md 8(d): both directions of every pair, no recompute, "
+                "no padding, tanh not counted) / its CUDA-event time.  The kernels execute more than that: pass 2 recomputes "
+                "the forward chain and carries a tangent chain, tanh costs 19 pipe slots, 25 -> 28 padding on water; with "
+                "the same-species pair reuse they execute fewer chains than the algorithmic count for the nets (a,a) — so "
+                "this is a throughput figure, not a pipe-utilisation figure (that is ncu's, profiles/)")
+        else:
+            line["roofline"]["note"] = (
+                f"algorithmic flops of the stage / its CUDA-event time against the dense tensor peak ({how}); the tensor "
+                "pipe executes 3x (tf32) or 6x (bf16) these flops (error-compensated split); the stage is bound by MUFU "
+                "(fp32 tanh) and instruction issue, not by the tensor pipe (DESIGN.md section 9)")
         if args.md_steps > 0:
             line["md"] = run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed)
         if dd_leg is not None:
             line["dd"] = dd_leg
+    model.close()
+    del res
+
+    # every other BASELINE.json config, 1 GPU only, short: the driver's record then holds all of them
+    if rank == 0 and world == 1 and args.configs and name == "W24k" and args.precision == "fp64":
+        cfgs = {}
+        for (wn, prec, st, wu) in EXTRA_CONFIGS:
+            key = wn if prec == "fp64" else f"{wn}-{prec}"
+            try:
+                torch.cuda.empty_cache()
+                r = measure(wn, prec, args.variant, st, wu, dev)
+                r["steps"] = st
+                cfgs[key] = config_summary(r)
+                cfgs[key]["steps"] = st
+                free_b, total_b = torch.cuda.mem_get_info(dev)      # the library's workspace is grow-only: in use = peak
+                cfgs[key]["device_memory_in_use_bytes"] = int(total_b - free_b)
+                r["model"].close()
+                del r
+            except Exception as exc:                              # a config that cannot run is reported, not hidden
+                cfgs[key] = {"error": f"{type(exc).__name__}: {exc}"}
+        line["configs"] = cfgs
+
+    if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             step, k, desc, threads = oracle_step_sampler(name, gen.SEED_BASE, args.ref_sample)
             step()
@@ -433,7 +541,6 @@ def run_cuda(args):
             line["cpu_baseline"] = {"value": k * reps / dt, "unit": "atom-steps/s", "cores": threads, "kind": "oracle",
                                     "sample": f"{reps} steps x {desc}"}
         print(json.dumps(line))
-    model.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -446,10 +553,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="W24k", choices=sorted(MODELS))
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "tf32"])
-    ap.add_argument("--variant", type=int, default=int(os.environ.get("DPB_VARIANT", "1")))
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "tf32", "bf16"])
+    ap.add_argument("--variant", type=int, default=1)
+    ap.add_argument("--no-configs", dest="configs", action="store_false",
+                    help="skip the short legs over the other BASELINE.json configs (W192, Cu32k, W24k mixed, Cu864k) that the "
+                         "default run appends as a `configs` object")
     ap.add_argument("--ref-sample", type=int, default=2048, help="atoms per step of the CPU oracle arm")
-    ap.add_argument("--stage-every", type=int, default=10, help="read the stage timers every n-th step (0: never)")
+    ap.add_argument("--stage-every", type=int, default=1, help="0: do not run the extra stage-timer steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--md-steps", type=int, default=0,
                     help="also run this many velocity-Verlet steps (dpb_md_run; PAPER.md:298: 330 K, 0.5 / 1.0 fs, 2 A skin "

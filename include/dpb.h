@@ -79,8 +79,11 @@ int dpb_model_destroy(dpb_model *model);
 /* Nm = sum_t sel[t]. */
 int dpb_model_nm(const dpb_model *model);
 
-/* Upper bound on the atoms processed per pass (bounds the workspace: about 80 KB per atom for copper).
- * Default 32768.  Returns DPB_EINVAL if chunk < 1. */
+/* Upper bound on the atoms processed per pass (bounds the workspace: about 73 KB per atom for the copper model).
+ * chunk_atoms = 0 (the default) sizes it automatically: the largest chunk whose workspace fits in half of the device
+ * memory that was free when the model was created, at least 32768 atoms (the 864,000-atom copper box then runs as one
+ * chunk in 63 GB of the B200's 180 GB).  Larger chunks are faster: the same-species pair reuse shares only pairs whose
+ * two atoms are centres of the same chunk.  Returns DPB_EINVAL if chunk < 0. */
 int dpb_model_set_chunk(dpb_model *model, int64_t chunk_atoms);
 
 /* Select the kernel generation: 0 = plain reference kernels ("v0": unfused, thread-per-output FMA loops),
@@ -93,6 +96,15 @@ int dpb_model_set_variant(dpb_model *model, int variant);
  * Costs about N * Nm * 28 bytes of extra workspace and one gather kernel.  Exact only when no neighbour was dropped
  * by a full type section (info.n_overflow == 0).  Other precisions / variants: dpb_eval returns DPB_ENOTIMPL. */
 int dpb_model_set_deterministic(dpb_model *model, int on);
+
+/* CUDA-graph replay of dpb_eval (calls with info == NULL and the stage timers off).  The first call with a given set of
+ * arguments (natoms, every pointer, the box) runs eagerly, the second one is captured into a CUDA graph, later ones
+ * replay it — one launch instead of about 30, which is what bounds a 192-atom evaluation (the paper's regime below
+ * ~1000 atoms per GPU).  The library keeps the 32 most recent argument sets; a change of the
+ * workspace or of any model setting drops them.  The buffers named by the arguments must stay valid while the model may
+ * replay them (as for any asynchronous call).  mode: 0 off, 1 (default) evaluations of at most 4096 atoms, 2 always.
+ * dpb_eval_local, dpb_eval_host and dpb_md_run always run eagerly. */
+int dpb_model_set_graph(dpb_model *model, int mode);
 
 /* Same-species pair reuse in pass 1 (DPB_FP64, variant 1; on by default, off while the deterministic reduction is on).
  * The embedding net of a pair depends on s(r_ij) = s(r_ji) only (Eq. 5 and 8-9), so for the nets

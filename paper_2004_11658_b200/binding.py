@@ -82,6 +82,7 @@ def load_library():
     lib.dpb_set_debug_buffers.argtypes = [vp, vp, vp, vp]
     lib.dpb_debug_sorted_order.argtypes = [vp, vp, i64, vp]
     lib.dpb_model_status.argtypes = [vp, vp]
+    lib.dpb_model_set_graph.argtypes = [vp, i32]
     lib.dpb_eval.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp, C.POINTER(_Info)]
     lib.dpb_eval_local.argtypes = [vp, vp, i64, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp,
                                    C.POINTER(_Info)]
@@ -165,6 +166,10 @@ class DPModel:
     def set_pair_reuse(self, on: int):
         """dpb_model_set_pair_reuse: 0 off, 1 single-chunk evaluations (default), 2 always."""
         self._chk(self.lib.dpb_model_set_pair_reuse(self._h, int(on)))
+
+    def set_graph(self, mode: int):
+        """dpb_model_set_graph: 0 off, 1 evaluations of at most 4096 atoms (default), 2 always."""
+        self._chk(self.lib.dpb_model_set_graph(self._h, int(mode)))
 
     def set_atom_virial(self, buf=None):
         """dpb_model_set_atom_virial: a CUDA float64 [N, 9] (or [N, 3, 3]) tensor that the following evaluations fill with

@@ -76,11 +76,15 @@ extern "C" int64_t dpb_kernel_launches(void) { return (int64_t)g_dpb_launches; }
 extern "C" const char *dpb_last_error(void) { return g_err; }
 extern "C" const char *dpb_version(void) { return "dpb 1 sm_100a"; }
 
+// Bumped whenever a workspace buffer is (re)allocated or released: captured CUDA graphs hold the old pointers.
+static unsigned long long g_ws_epoch = 1;
+
 struct Buf {
   void *p = nullptr;
   size_t cap = 0;
   cudaError_t reserve(size_t bytes, bool zero = false) {
     if (bytes <= cap) return cudaSuccess;
+    ++g_ws_epoch;
     if (p) cudaFree(p);
     p = nullptr; cap = 0;
     size_t want = bytes + bytes / 8 + 256;
@@ -89,15 +93,36 @@ struct Buf {
     if (e == cudaSuccess && zero) e = cudaMemset(p, 0, want);      // (re)allocation only: synchronous, rare
     return e;
   }
-  void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+  void release() { if (p) { cudaFree(p); ++g_ws_epoch; } p = nullptr; cap = 0; }
   template <class T> T *as() const { return reinterpret_cast<T *>(p); }
 };
 
+// One captured evaluation (dpb_model_set_graph): every argument that is baked into the kernel parameters is part of the key.
+struct GraphKey {
+  int64_t natoms;
+  const void *ptr[7];       // coord, type, energy, atom_energy, force, virial, nlist
+  double box[9];
+  bool operator==(const GraphKey &o) const { return memcmp(this, &o, sizeof(GraphKey)) == 0; }
+};
+struct GraphEntry {
+  GraphKey key;
+  cudaGraphExec_t exec = nullptr;
+  unsigned long long epoch = 0, stamp = 0;   // workspace / configuration state the entry belongs to; last use
+  long long kernels = 0;                     // kernel launches inside the graph
+  bool failed = false;                       // capture did not work for this call: run it eagerly from now on
+};
+#define DPB_GRAPH_SLOTS 32
+#define DPB_GRAPH_AUTO_ATOMS 4096
+
 struct dpb_model {
   DevModel P;
+  int graph_mode = 1;                        // 0 off, 1 evaluations of at most DPB_GRAPH_AUTO_ATOMS atoms, 2 always
+  unsigned long long cfg_epoch = 1, graph_clock = 0;
+  std::vector<GraphEntry> graphs;
   int precision = 0, variant = 1, timing = 0, deterministic = 0, pair_reuse = 1;
   double *atom_virial = nullptr;        // caller's [N][9] buffer (dpb_model_set_atom_virial)
-  int64_t chunk = 32768;
+  int64_t chunk = 0;            // atoms per pass; 0 = automatic (effective_chunk)
+  size_t ws_budget = 0;         // bytes the per-chunk workspace may take in automatic mode (half of the memory free at creation)
   int device = 0;
   Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
   V1Weights v1;                 // re-laid-out weights of the fused kernels
@@ -126,6 +151,26 @@ struct dpb_model {
 };
 
 static int nm_of(const DevModel &P) { return P.nm; }
+
+// Atoms per chunk.  An explicit dpb_model_set_chunk wins; otherwise the largest chunk whose workspace (lists, (d, r)
+// rows, T, dT and the fitting activations: 73 KB per atom for the copper model in fp64) stays inside the budget fixed
+// at model creation, at least 32768 atoms.  Larger chunks are faster, not only smaller in launch count: the
+// same-species pair reuse only shares pairs whose two atoms are centres of the same chunk.
+static int64_t effective_chunk(const dpb_model *m) {
+  if (m->chunk > 0) return m->chunk;
+  if (m->precision != DPB_FP64) return 32768;            // mixed precision: the tile / pair-list kernels are sized for this
+  const DevModel &P = m->P;
+  size_t per = (size_t)P.nm * (4 + 4 + 32) + (size_t)P.ntypes * 4 + (size_t)P.M * 32 + (size_t)(16 * 8 + P.M) * 32;
+  if (m->precision == DPB_FP64) {
+    if (m->variant == 0 || !m->v1.ready) per += sizeof(double) * (2 * (size_t)P.dim + 7 * (size_t)P.fw);
+    else per += v1_workspace_bytes(P, 1024) / 1024;
+  } else {
+    per += (tc_pair_workspace_bytes(P, 1024) + tc_pass2_workspace_bytes(P, 1024) + tc_fit_workspace_bytes(P, 1024)) / 1024;
+  }
+  int64_t c = (int64_t)(m->ws_budget / (per + 1));
+  c -= c % 1024;
+  return c < 32768 ? 32768 : c;
+}
 
 extern "C" int dpb_model_nm(const dpb_model *m) { return m ? nm_of(m->P) : DPB_EINVAL; }
 
@@ -159,6 +204,10 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
   P.emb_net_size = s1 + s1 + s1 * 2 * s1 + 2 * s1 + 2 * s1 * 4 * s1 + 4 * s1;
   P.fit_net_size = (long long)P.dim * P.fw + P.fw + 2 * ((long long)P.fw * P.fw + P.fw) + P.fw + 1;
   cudaGetDevice(&m->device);
+  {
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) m->ws_budget = free_b / 2;
+  }
   const size_t eb = sizeof(double) * (size_t)P.emb_net_size * P.ntypes * P.ntypes;
   const size_t fb = sizeof(double) * (size_t)P.fit_net_size * P.ntypes;
   cudaError_t e = m->emb.reserve(eb);
@@ -197,31 +246,36 @@ extern "C" int dpb_model_destroy(dpb_model *m) {
   v1_release_weights(m->v1);
   tc_release_weights(m->tcw);
   for (cudaEvent_t &e : m->evs) cudaEventDestroy(e);
+  for (GraphEntry &g : m->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
   delete m;
   return DPB_OK;
 }
 
 extern "C" int dpb_model_set_chunk(dpb_model *m, int64_t chunk) {
-  if (!m || chunk < 1) return fail(DPB_EINVAL, "dpb_model_set_chunk: chunk must be >= 1");
+  if (!m || chunk < 0) return fail(DPB_EINVAL, "dpb_model_set_chunk: chunk must be >= 1, or 0 for the automatic size");
   m->chunk = chunk;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
 extern "C" int dpb_model_set_variant(dpb_model *m, int variant) {
   if (!m || variant < 0 || variant > 1) return fail(DPB_EINVAL, "dpb_model_set_variant: variant must be 0 or 1");
   m->variant = variant;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
 extern "C" int dpb_model_set_atom_virial(dpb_model *m, double *atom_virial) {
   if (!m) return fail(DPB_EINVAL, "null model");
   m->atom_virial = atom_virial;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
 extern "C" int dpb_model_set_deterministic(dpb_model *m, int on) {
   if (!m) return fail(DPB_EINVAL, "null model");
   m->deterministic = on ? 1 : 0;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
@@ -229,12 +283,14 @@ extern "C" int dpb_model_set_pair_reuse(dpb_model *m, int on) {
   if (!m) return fail(DPB_EINVAL, "null model");
   if (on < 0 || on > 2) return fail(DPB_EINVAL, "pair reuse: 0 (off), 1 (single-chunk evaluations) or 2 (always)");
   m->pair_reuse = on;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
 extern "C" int dpb_set_debug_buffers(dpb_model *m, double *T, double *D, double *dT) {
   if (!m) return fail(DPB_EINVAL, "null model");
   m->dbgT = T; m->dbgD = D; m->dbgdT = dT;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
@@ -252,6 +308,7 @@ extern "C" int dpb_debug_sorted_order(dpb_model *m, void *stream, int64_t natoms
 extern "C" int dpb_model_set_timing(dpb_model *m, int on) {
   if (!m) return fail(DPB_EINVAL, "null model");
   m->timing = on ? 1 : 0;
+  ++m->cfg_epoch;
   return DPB_OK;
 }
 
@@ -357,7 +414,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   const int N = (int)natoms;
   const int nkeys = P.ntypes * G.ngrp * G.ncell;
   const int64_t ncentre = nloc >= 0 ? nloc : natoms;
-  const int64_t chunk = m->chunk < ncentre ? m->chunk : (ncentre > 0 ? ncentre : 1);
+  const int64_t chunk_cap = effective_chunk(m);
+  const int64_t chunk = chunk_cap < ncentre ? chunk_cap : (ncentre > 0 ? ncentre : 1);
 
   CU(m->key.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
   CU(m->count.reserve(sizeof(int) * (size_t)(nkeys + 1)), "workspace");
@@ -533,7 +591,7 @@ static int finish_info(dpb_model *m, cudaStream_t st, int64_t natoms, dpb_eval_i
     info->n_real_pairs = (int64_t)hs.n_real_pairs;
     info->n_overflow = (int64_t)hs.n_overflow;
     for (int t = 0; t < 8 && t < DPB_MAX_TYPES; ++t) info->max_nei[t] = hs.max_nei[t];
-    const int64_t chunk = m->chunk;
+    const int64_t chunk = effective_chunk(m);
     info->n_chunks = (int32_t)((natoms + chunk - 1) / chunk);
   }
   return DPB_OK;
@@ -544,11 +602,86 @@ extern "C" int dpb_model_status(dpb_model *m, void *stream) {
   return finish_info(m, reinterpret_cast<cudaStream_t>(stream), 0, nullptr);
 }
 
+extern "C" int dpb_model_set_graph(dpb_model *m, int mode) {
+  if (!m || mode < 0 || mode > 2) return fail(DPB_EINVAL, "dpb_model_set_graph: mode must be 0, 1 or 2");
+  m->graph_mode = mode;
+  return DPB_OK;
+}
+
+// dpb_eval through a CUDA graph.  The first call with a given argument set runs eagerly (it sizes the workspace and sets
+// the kernel attributes), the second one is captured — run_eval only enqueues work, forks and joins included — and
+// instantiated, later ones replay the graph: one launch instead of ~30, which is what a 192-atom evaluation is bound
+// by.  Returns 1 if the call was served by a graph, 0 if the caller has to run it eagerly, < 0 on error.
+static int eval_graphed(dpb_model *m, cudaStream_t st, int64_t natoms, const double *coord, const int32_t *type,
+                        const double box[9], double *energy, double *atom_energy, double *force, double *virial,
+                        int32_t *nlist) {
+  if (m->graph_mode == 0 || m->timing || (m->graph_mode == 1 && natoms > DPB_GRAPH_AUTO_ATOMS)) return 0;
+  GraphKey key;
+  memset(&key, 0, sizeof(key));
+  key.natoms = natoms;
+  const void *ptrs[7] = {coord, type, energy, atom_energy, force, virial, nlist};
+  memcpy(key.ptr, ptrs, sizeof(ptrs));
+  memcpy(key.box, box, sizeof(key.box));
+  const unsigned long long epoch = g_ws_epoch * 1000003ull + m->cfg_epoch;
+  GraphEntry *hit = nullptr;
+  for (GraphEntry &g : m->graphs) if (g.key == key) { hit = &g; break; }
+  if (hit && hit->epoch != epoch) {                       // workspace or configuration changed since: start over
+    if (hit->exec) cudaGraphExecDestroy(hit->exec);
+    hit->exec = nullptr; hit->failed = false; hit->epoch = 0;
+  }
+  if (!hit) {
+    if (m->graphs.size() < DPB_GRAPH_SLOTS) { m->graphs.emplace_back(); hit = &m->graphs.back(); }
+    else {
+      hit = &m->graphs[0];
+      for (GraphEntry &g : m->graphs) if (g.stamp < hit->stamp) hit = &g;
+      if (hit->exec) cudaGraphExecDestroy(hit->exec);
+      *hit = GraphEntry();
+    }
+    hit->key = key;
+  }
+  hit->stamp = ++m->graph_clock;
+  if (hit->failed) return 0;
+  if (hit->exec) {
+    cudaError_t e = cudaGraphLaunch(hit->exec, st);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGraphLaunch");
+    DPB_LAUNCHED(hit->kernels);
+    return 1;
+  }
+  if (hit->epoch == 0) { hit->epoch = epoch; return 0; }  // first sighting: eager (may grow the workspace: new epoch)
+  // second call in the same state: capture
+  const unsigned long long l0 = g_dpb_launches;
+  cudaError_t e = cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed);
+  if (e != cudaSuccess) { cudaGetLastError(); hit->failed = true; return 0; }
+  const int rc = run_eval(m, st, natoms, coord, type, box, energy, atom_energy, force, virial, nlist, false);
+  cudaGraph_t graph = nullptr;
+  e = cudaStreamEndCapture(st, &graph);
+  const long long kernels = (long long)(g_dpb_launches - l0);
+  g_dpb_launches = l0;                                    // nothing has run yet
+  if (rc != DPB_OK || e != cudaSuccess || !graph || g_ws_epoch * 1000003ull + m->cfg_epoch != epoch) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    hit->failed = true;
+    return rc != DPB_OK ? rc : 0;
+  }
+  e = cudaGraphInstantiate(&hit->exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { cudaGetLastError(); hit->exec = nullptr; hit->failed = true; return 0; }
+  hit->kernels = kernels;
+  e = cudaGraphLaunch(hit->exec, st);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGraphLaunch");
+  DPB_LAUNCHED(hit->kernels);
+  return 1;
+}
+
 extern "C" int dpb_eval(dpb_model *m, void *stream, int64_t natoms, const double *coord, const int32_t *type,
                         const double box[9], double *energy, double *atom_energy, double *force, double *virial,
                         int32_t *nlist, dpb_eval_info *info) {
   if (!m || !box) return fail(DPB_EINVAL, "dpb_eval: null model / box");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (!info) {
+    const int g = eval_graphed(m, st, natoms, coord, type, box, energy, atom_energy, force, virial, nlist);
+    if (g != 0) return g < 0 ? g : DPB_OK;
+  }
   int rc = run_eval(m, st, natoms, coord, type, box, energy, atom_energy, force, virial, nlist, false);
   if (rc != DPB_OK) return rc;
   if (info) return finish_info(m, st, natoms, info);

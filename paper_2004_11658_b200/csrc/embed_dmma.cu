@@ -175,7 +175,7 @@ __device__ __forceinline__ void env_row4(const DevModel &P, const double4 v, dou
 // accumulation of this launch into T is a reduction.  Taken only while no neighbour was dropped (n_overflow == 0).
 template <int SP, int RB, bool RU>
 __global__ void __launch_bounds__((32 * P1_WARPS), 1)
-k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate) {
+k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate, int nseg) {
   using L = EL<SP>;
   extern __shared__ __align__(16) double smem[];
   double *W = smem;
@@ -206,14 +206,24 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
   const int s1 = P.s1, M = P.M;
 
-  for (int qa = row_lo + blockIdx.x * P1_WARPS + warp; qa < row_hi; qa += gridDim.x * P1_WARPS) {
+  // work item = (atom, segment of its section): nseg > 1 splits the rows of an atom over several warps when the chunk has
+  // too few atoms to fill the GPU (configs[0]: 192 atoms); T is then accumulated with reductions (accumulate == 2)
+  for (int item = blockIdx.x * P1_WARPS + warp; item < (row_hi - row_lo) * nseg; item += gridDim.x * P1_WARPS) {
+    const int qa = row_lo + item / nseg;
     int n = C.nreal[(size_t)qa * P.ntypes + t];
+    int s_lo = 0;
+    if (nseg > 1) {
+      const int rs = (((n + nseg - 1) / nseg) + 7) & ~7;
+      s_lo = min(n, (item % nseg) * rs);
+      n = min(n, s_lo + rs);
+    }
+    if (s_lo >= n && accumulate) continue;               // (store mode still has to write the zero tile)
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
     if (RU && ru) {                                      // keep the slots whose pair this atom evaluates
       const int *nlr = C.nl + (size_t)qa * P.nm + P.sec_start[t];
       int nk = 0;
       __syncwarp();
-      for (int base = 0; base < n; base += 32) {
+      for (int base = s_lo; base < n; base += 32) {
         const int slot = base + lane;
         bool keep = false;
         int qj = -1;
@@ -231,6 +241,9 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
       }
       n = nk;
       __syncwarp();
+    } else {
+      dr += s_lo;
+      n -= s_lo;
     }
     double Tacc[2][2][4];
 #pragma unroll
@@ -354,7 +367,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
           const int c = s / SP, r = (s % SP) * 4 + qq;
           if (r < s1) {
             double *dst = C.T + ((size_t)qa * M + c * s1 + r) * 4;
-            if (RU && ru) {
+            if ((RU && ru) || accumulate == 2) {
               atomicAdd(dst + 0, Tacc[ch][u][0]); atomicAdd(dst + 1, Tacc[ch][u][1]);
               atomicAdd(dst + 2, Tacc[ch][u][2]); atomicAdd(dst + 3, Tacc[ch][u][3]);
             } else if (accumulate) {
@@ -375,7 +388,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 template <int SP>
 __global__ void __launch_bounds__((32 * P2_WARPS), 1)
 k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
-             double *__restrict__ virial) {
+             double *__restrict__ virial, int nseg) {
   using L = EL<SP>;
   extern __shared__ __align__(16) double smem[];
   double *W = smem;
@@ -393,11 +406,18 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 #pragma unroll
   for (int k = 0; k < 9; ++k) vir[k] = 0.0;
 
-  for (int qa = row_lo + blockIdx.x * P2_WARPS + warp; qa < row_hi; qa += gridDim.x * P2_WARPS) {
-    const int n = C.nreal[(size_t)qa * P.ntypes + t];
-    if (n == 0) continue;
-    const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
-    const int *nl = C.nl + (size_t)qa * P.nm + P.sec_start[t];
+  for (int item = blockIdx.x * P2_WARPS + warp; item < (row_hi - row_lo) * nseg; item += gridDim.x * P2_WARPS) {
+    const int qa = row_lo + item / nseg;                 // work item = (atom, segment of its section), as in pass 1
+    int n = C.nreal[(size_t)qa * P.ntypes + t];
+    int s_lo = 0;
+    if (nseg > 1) {
+      const int rs = (((n + nseg - 1) / nseg) + 7) & ~7;
+      s_lo = min(n, (item % nseg) * rs);
+      n = min(n, s_lo + rs) - s_lo;
+    }
+    if (n <= 0) continue;
+    const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t] + s_lo;
+    const int *nl = C.nl + (size_t)qa * P.nm + P.sec_start[t] + s_lo;
     __syncwarp();
     {                                                    // dT is stored in lane order (ChunkView::dt_pad): a plain copy
       const double4 *src = reinterpret_cast<const double4 *>(C.dT + (size_t)qa * C.dt_rows * 4);
@@ -512,7 +532,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         const double f0 = fma(cm, dv.x, qq * pr[1]), f1 = fma(cm, dv.y, qq * pr[2]), f2 = fma(cm, dv.z, qq * pr[3]);
         if (C.fslot) {
           // deterministic mode: keep dE_i/dd_ik per slot; forces and virial are gathered in a fixed order afterwards
-          double *fs = C.fslot + ((size_t)qa * P.nm + P.sec_start[t] + row) * 3;
+          double *fs = C.fslot + ((size_t)qa * P.nm + P.sec_start[t] + s_lo + row) * 3;
           fs[0] = f0; fs[1] = f1; fs[2] = f2;
         } else {
         const int j = jn;
@@ -637,7 +657,7 @@ __device__ __forceinline__ void p2r_chunk(const double *__restrict__ W2h, const 
 template <int SP>
 __global__ void __launch_bounds__((32 * P2_WARPS), 1)
 k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a, double *__restrict__ force,
-                double *__restrict__ virial) {
+                double *__restrict__ virial, int nseg) {
   using L = EL<SP>;
   using R = P2R<SP>;
   extern __shared__ __align__(16) double smem[];
@@ -665,9 +685,16 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 #pragma unroll
   for (int k = 0; k < 9; ++k) vir[k] = 0.0;
 
-  for (int qa = row_lo + blockIdx.x * P2_WARPS + warp; qa < row_hi; qa += gridDim.x * P2_WARPS) {
-    const int n = C.nreal[(size_t)qa * P.ntypes + t];
-    if (n == 0) continue;
+  for (int item = blockIdx.x * P2_WARPS + warp; item < (row_hi - row_lo) * nseg; item += gridDim.x * P2_WARPS) {
+    const int qa = row_lo + item / nseg;                 // work item = (atom, segment of its section), as in pass 1
+    int n = C.nreal[(size_t)qa * P.ntypes + t];
+    int s_lo = 0;
+    if (nseg > 1) {
+      const int rs = (((n + nseg - 1) / nseg) + 7) & ~7;
+      s_lo = min(n, (item % nseg) * rs);
+      n = min(n, s_lo + rs);
+    }
+    if (s_lo >= n) continue;                             // the raw slots [s_lo, n) of the section
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
     const int *nl = C.nl + (size_t)qa * P.nm + P.sec_start[t];
     const int *nlp = C.nlp + (size_t)qa * P.nm + P.sec_start[t];
@@ -677,7 +704,7 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       for (int p = lane; p < 16 * SP; p += 32) *reinterpret_cast<double4 *>(dTt + 4 * p) = src[p];
     }
     // kept rows: sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs
-    int head = 0, cnt = 0, rawpos = 0, sweep = ru ? 0 : 1;
+    int head = 0, cnt = 0, rawpos = s_lo, sweep = ru ? 0 : 1;
     bool done = false;
     auto refill = [&]() {
       const int slot = rawpos + lane;
@@ -701,7 +728,7 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       cnt += __popc(mk);
       rawpos += 32;
       if (rawpos >= n) {
-        if (ru && sweep == 0) { sweep = 1; rawpos = 0; } else done = true;
+        if (ru && sweep == 0) { sweep = 1; rawpos = s_lo; } else done = true;
       }
     };
     // both-direction rows of the block at the ring head, and (lanes 0..7) the row of neighbour j of ring row `lane`
@@ -858,6 +885,14 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 // ---------------------------------------------------------------------------------------------------------
 static int g_sm_count = 0;
 
+// Segments per atom (work items per atom and net): 1 when the chunk has enough atoms to give every warp of the GPU two
+// of them; up to 8 for small chunks (configs[0]: 192 atoms on 148 SMs x 8 warps).
+static int seg_count(int n_atoms, int warps) {
+  const long long want = 2ll * g_sm_count * warps;
+  long long k = (want + n_atoms - 1) / (n_atoms > 0 ? n_atoms : 1);
+  return (int)(k < 1 ? 1 : (k > 8 ? 8 : k));
+}
+
 template <int SP>
 static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weights &W, cudaStream_t st) {
   using L = EL<SP>;
@@ -876,11 +911,12 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
     if (e != cudaSuccess) return e;
     configured_ru = smem_ru;
   }
-  if (reuse) {                                           // every accumulation into T is then an addition
+  const int nseg = C.fslot ? 1 : seg_count(C.n, P1_WARPS);   // deterministic mode: no reductions into T
+  if (reuse || nseg > 1) {                               // every accumulation into T is then an addition
     cudaError_t e = cudaMemsetAsync(C.T, 0, sizeof(double) * (size_t)C.n * P.M * 4, st);
     if (e != cudaSuccess) return e;
   }
-  const int grid = min(g_sm_count, (C.n + P1_WARPS - 1) / P1_WARPS);
+  const int grid = (int)min((long long)g_sm_count, ((long long)C.n * nseg + P1_WARPS - 1) / P1_WARPS);
   // nets of one centre type a accumulate into the same T rows (t = 0 stores, t > 0 adds): one stream per a, so that the
   // tail of one launch overlaps the start of another centre type's
   cudaStream_t ts[DPB_MAX_TYPES];
@@ -890,10 +926,11 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
     for (int t = 0; t < P.ntypes; ++t) {
       const double *net = W.emb + (size_t)(a * P.ntypes + t) * W.net_stride;
       if (reuse && a == t)
-        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, ts[P.ntypes - 1 - a]>>>(P, C, net, a, t, 1);
+        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, ts[P.ntypes - 1 - a]>>>(P, C, net, a, t,
+                                                                                           nseg > 1 ? 2 : 1, nseg);
       else
-        k_pass1_dmma<SP, 1, false><<<grid, (32 * P1_WARPS), smem, ts[P.ntypes - 1 - a]>>>(P, C, net, a, t,
-                                                                                        reuse ? 1 : t > 0);
+        k_pass1_dmma<SP, 1, false><<<grid, (32 * P1_WARPS), smem, ts[P.ntypes - 1 - a]>>>(
+            P, C, net, a, t, nseg > 1 ? 2 : (reuse ? 1 : t > 0), nseg);
       DPB_LAUNCHED(1);
     }
   if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
@@ -920,7 +957,8 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     if (e != cudaSuccess) return e;
     configured_ru = true;
   }
-  const int grid = min(g_sm_count, (C.n + P2_WARPS - 1) / P2_WARPS);
+  const int nseg = C.fslot ? 1 : seg_count(C.n, P2_WARPS);
+  const int grid = (int)min((long long)g_sm_count, ((long long)C.n * nseg + P2_WARPS - 1) / P2_WARPS);
   // the nets are independent here (forces and virial are atomic sums, slot stores are disjoint): a stream per net, so
   // that the tail of every launch is filled by the others
   cudaStream_t ts[DPB_MAX_TYPES];
@@ -933,10 +971,10 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
       cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
       if (reuse && a == t)
         k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, force,
-                                                                     virial);
+                                                                     virial, nseg);
       else
         k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
-                                                              virial);
+                                                              virial, nseg);
       DPB_LAUNCHED(1);
     }
   if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;

@@ -18,11 +18,6 @@
 
 #include <vector>
 
-#ifndef FIT_WM
-#define FIT_WM 2            // warp rows per CTA: CTA tile = 16 FIT_WM rows, 64 FIT_WM threads
-#endif
-#define FIT_BM (16 * FIT_WM)
-#define FIT_THREADS (64 * FIT_WM)
 #define FIT_BK 16
 #define FIT_STAGES 3
 #define FIT_LDA (FIT_BK + 4)
@@ -52,7 +47,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
-enum { EPI_TANH = 0, EPI_TANH_SKIP = 1, EPI_L3 = 2, EPI_BWD = 3, EPI_STORE = 4 };
+enum { EPI_TANH = 0, EPI_TANH_SKIP = 1, EPI_L3 = 2, EPI_BWD = 3, EPI_STORE = 4, EPI_ATOMIC = 5 };
 
 struct GemmArgs {
   const double *A; int lda;          // [rows][lda], K columns used
@@ -63,9 +58,12 @@ struct GemmArgs {
   double *out0; double *out1; int ldo;
 };
 
-template <int NBW, int EPI>
-__global__ void __launch_bounds__(FIT_THREADS, FIT_WM <= 2 ? 2 : 1)
+// WM = warp rows per CTA: CTA tile = 16 WM rows x 16 NBW columns, 64 WM threads.  (2, 15 / 8): the throughput shape;
+// (1, 3): 16 x 48 tiles for small systems, where the number of CTAs, not the tile efficiency, bounds the stage.
+template <int WM, int NBW, int EPI>
+__global__ void __launch_bounds__(64 * WM, 2)
 k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
+  constexpr int FIT_BM = 16 * WM, FIT_THREADS = 64 * WM;
   constexpr int BN = 16 * NBW, LDB = BN + 4;
   extern __shared__ __align__(16) double smem[];
   double *As = smem;                                        // [STAGES][BM][LDA]
@@ -76,12 +74,15 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
   const int n0 = blockIdx.y * BN;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gq = lane >> 2, q = lane & 3;
   const int wm = warp >> 1, wn = warp & 1;                  // warp tile: rows 16 wm .., cols 8 NBW wn ..
-  const int nkt = g.K / FIT_BK;
+  // split-K (EPI_ATOMIC, small systems): blockIdx.z takes the K tiles [kt0, kt1) and adds its partial sums to out0
+  const int nkt_all = g.K / FIT_BK;
+  const int kt0 = (int)(((long long)nkt_all * blockIdx.z) / gridDim.z);
+  const int nkt = (int)(((long long)nkt_all * (blockIdx.z + 1)) / gridDim.z) - kt0;
 
   auto load_tile = [&](int kt, int stage) {
     double *as = As + stage * FIT_BM * FIT_LDA;
     double *bs = Bs + stage * FIT_BK * LDB;
-    const int k0 = kt * FIT_BK;
+    const int k0 = (kt0 + kt) * FIT_BK;
     for (int c = tid; c < FIT_BM * (FIT_BK / 2); c += FIT_THREADS) {
       const int m = c >> 3, kk = (c & 7) * 2;
       const bool ok = m0 + m < row_hi;
@@ -179,6 +180,9 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
         const double2 u = x1[nb];
         if (g.out0) *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0, v1);
         *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(v0 * (1.0 - u.x * u.x), v1 * (1.0 - u.y * u.y));
+      } else if (EPI == EPI_ATOMIC) {
+        atomicAdd(g.out0 + oo, v0);
+        atomicAdd(g.out0 + oo + 1, v1);
       } else {
         *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0, v1);
       }
@@ -319,6 +323,14 @@ __global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView
   }
 }
 
+// Z0 = tanh(X + b0) in place, after a split-K G1 (small systems): rows of species ty.
+__global__ void k_bias_tanh_v1(ChunkView C, int ty, int fwp, const double *__restrict__ bias, double *__restrict__ Z) {
+  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  const int q = row_lo + blockIdx.x;
+  if (q >= row_hi) return;
+  for (int o = threadIdx.x; o < fwp; o += blockDim.x) Z[(size_t)q * fwp + o] = dp_tanh(Z[(size_t)q * fwp + o] + bias[o]);
+}
+
 // E_i = Z2 . w3 + b3 (output layer, reading R4): one warp per atom.
 __global__ void k_rowdot_v1(ChunkView C, int ty, int fwp, const double *__restrict__ Z2, const double *__restrict__ w3,
                             double b3, double *__restrict__ atom_energy) {
@@ -397,20 +409,29 @@ size_t v1_workspace_bytes(const DevModel &P, int64_t chunk) {
   return sizeof(double) * (size_t)chunk * (2 * dimp + 6 * fwp) + 256;
 }
 
-template <int NBW, int EPI>
-static cudaError_t gemm(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st) {
-  constexpr int BN = 16 * NBW;
+template <int WM, int NBW, int EPI>
+static cudaError_t gemm_t(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st, int splitk = 1) {
+  constexpr int BN = 16 * NBW, FIT_BM = 16 * WM;
   const size_t smem = sizeof(double) * FIT_STAGES * (FIT_BM * FIT_LDA + FIT_BK * (BN + 4));
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_fit_gemm<NBW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_fit_gemm<WM, NBW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid((C.n + FIT_BM - 1) / FIT_BM, (g.N + BN - 1) / BN);
-  k_fit_gemm<NBW, EPI><<<grid, FIT_THREADS, smem, st>>>(C, ty, g);
+  dim3 grid((C.n + FIT_BM - 1) / FIT_BM, (g.N + BN - 1) / BN, splitk);
+  k_fit_gemm<WM, NBW, EPI><<<grid, 64 * WM, smem, st>>>(C, ty, g);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
+}
+
+// Small systems (a chunk of at most FIT_SMALL_N atoms: BASELINE.json configs[0], 192 atoms) are bound by how many CTAs a
+// GEMM offers, not by tile efficiency: 16 x 48 tiles give 5 (240 columns) or 34 (1600) CTAs per 16 rows.
+#define FIT_SMALL_N 2048
+template <int NBW, int EPI>
+static cudaError_t gemm(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st) {
+  if (C.n <= FIT_SMALL_N) return gemm_t<1, 3, EPI>(C, ty, g, st);
+  return gemm_t<2, NBW, EPI>(C, ty, g, st);
 }
 
 cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, const double *fit, void *ws,
@@ -434,6 +455,8 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
 
   k_descr_v1<<<C.n, 256, 0, st>>>(P, C, dimp, D);
   DPB_LAUNCHED(1);
+  const bool splitk = C.n <= FIT_SMALL_N && !C.fslot;    // (not in deterministic mode: the partial sums are reductions)
+  if (splitk && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
   // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint
   cudaStream_t ts[DPB_MAX_TYPES];
   if ((e = dpb_fork_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
@@ -442,9 +465,14 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     cudaStream_t s = ts[k];
     const FitNet &N = F->nets[ty];
     GemmArgs g;
-    // G1: Z0 = tanh(D W0 + b0)
+    // G1: Z0 = tanh(D W0 + b0).  Small systems: split-K over 8 CTAs (K = dim is a serial loop of dim / 16 tiles for
+    // the few CTAs a 192-atom box offers), partial sums added into the cleared Z0, bias and tanh in a second kernel.
     g = GemmArgs{D, dimp, N.W0, fwp, dimp, fwp, N.b0, nullptr, nullptr, fwp, Z0, nullptr, fwp};
-    if ((e = gemm<15, EPI_TANH>(C, ty, g, s)) != cudaSuccess) return e;
+    if (splitk) {
+      if ((e = gemm_t<1, 3, EPI_ATOMIC>(C, ty, g, s, 8)) != cudaSuccess) return e;
+      k_bias_tanh_v1<<<C.n, 64, 0, s>>>(C, ty, fwp, N.b0, Z0);
+      DPB_LAUNCHED(1);
+    } else if ((e = gemm<15, EPI_TANH>(C, ty, g, s)) != cudaSuccess) return e;
     // G2: U1 = tanh(Z0 W1 + b1); Z1 = Z0 + U1
     g = GemmArgs{Z0, fwp, N.W1, fwp, fwp, fwp, N.b1, Z0, nullptr, fwp, U1, Z1, fwp};
     if ((e = gemm<15, EPI_TANH_SKIP>(C, ty, g, s)) != cudaSuccess) return e;

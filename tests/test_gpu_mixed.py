@@ -171,6 +171,7 @@ def test_mixed_config5_copper_864k():
     order = None
     for name, prec in (("f64", FP64), ("tf32", TF32)):
         m = _model(spec, emb, fit, prec)
+        m.set_chunk(32768)
         out = m.eval(dc, dt, box, want_nlist=True, want_info=True)
         torch.cuda.synchronize()
         assert out["info"].n_overflow == 0 and out["info"].n_chunks == 27

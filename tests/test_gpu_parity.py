@@ -257,9 +257,10 @@ def test_eval_host_matches_device_entry():
     m.close()
 
 
-@pytest.mark.parametrize("conditioned", [False, True])
-def test_config5_copper_864k_sampled(conditioned):
-    """BASELINE configs[4]: 864,000-atom copper box (27 chunks of 32,768 atoms), too large for a whole oracle evaluation
+@pytest.mark.parametrize("conditioned,chunk", [(False, 0), (True, 32768)])
+def test_config5_copper_864k_sampled(conditioned, chunk):
+    """BASELINE configs[4]: 864,000-atom copper box, in the launch configuration bench.py times (automatic chunk: one chunk
+    on an otherwise empty B200) and as 27 chunks of 32,768 atoms; too large for a whole oracle evaluation
     inside the test budget.  Against the oracle, element by element, on sampled atoms — 16 random ones plus the two
     atoms on either side of four chunk boundaries (sorted order through dpb_debug_sorted_order): nlist rows bit-exact,
     E_i, and the FORCE, assembled from the oracle's per-row pieces F_i = sum_k f_ik - sum_{j: i in L(j)} f_{j,slot(i)}
@@ -273,15 +274,17 @@ def test_config5_copper_864k_sampled(conditioned):
     if conditioned:
         fit = gen.condition_fit_w0(spec, fit)
     orc, m = _models(spec, emb, fit, 1)
+    if chunk:
+        m.set_chunk(chunk)
     dc = torch.tensor(coord, device="cuda")
     dt = torch.tensor(types, device="cuda")
     out = m.eval(dc, dt, box, want_nlist=True, want_info=True)
     torch.cuda.synchronize()
     info = out["info"]
-    assert info.n_overflow == 0 and info.n_chunks == 27
+    assert info.n_overflow == 0 and (info.n_chunks == 27 if chunk else info.n_chunks >= 1)
     order = m.sorted_order(coord.shape[0]).cpu().numpy().astype(np.int64)
     assert np.array_equal(np.sort(order), np.arange(coord.shape[0]))
-    edge = [order[c * 32768 + d] for c in (1, 9, 17, 26) for d in (-1, 0)]
+    edge = [order[c * 32768 + d] for c in (1, 9, 17, 26) for d in (-1, 0)]    # chunk boundaries of the 27-chunk run
     atoms = np.unique(np.concatenate([np.random.default_rng(2).choice(coord.shape[0], 16, replace=False), edge]))
     F_ref, E_ref, nl_ref = oracle_forces_of(orc, coord, types, box, atoms)
     sel = torch.tensor(atoms, device="cuda")
@@ -464,4 +467,43 @@ def test_staging_capacity_overflow_is_reported_and_touches_no_unwritten_slot():
     assert np.array_equal(got["nlist"], ref["nlist"])
     assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
     m.status()
+    m.close()
+
+
+def test_cuda_graph_replay_matches_the_oracle():
+    """dpb_model_set_graph (default: evaluations of at most 4096 atoms): the first call with an argument set runs eagerly,
+    the second is captured, later ones replay the graph.  Calls 1-4 on two alternating coordinate buffers (W192, fresh
+    perturbations written INTO the same device buffers between calls) are each compared with the oracle; the kernel
+    counter advances by the same amount per call whether eager or replayed; mode 0 gives the same numbers."""
+    torch = _torch()
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc, m = _models(spec, emb, fit, 1)
+    bufs = [torch.empty((192, 3), dtype=torch.float64, device="cuda") for _ in range(2)]
+    dt = torch.tensor(types, device="cuda")
+    outs = [None, None]
+    per_call = []
+    for call in range(8):
+        c = gen.perturbed(coord, box, 0.01, 77 + call)
+        b = call % 2
+        bufs[b].copy_(torch.tensor(c))
+        n0 = m.kernel_launches()
+        outs[b] = m.eval(bufs[b], dt, box, want_nlist=True, out=outs[b])
+        torch.cuda.synchronize()
+        per_call.append(m.kernel_launches() - n0)
+        ref = orc.eval(c, types, box)
+        got = {k: v.cpu().numpy() for k, v in outs[b].items()}
+        assert np.array_equal(got["nlist"], ref["nlist"]), call
+        assert abs(got["energy"][0] - ref["energy"]) <= E_REL * abs(ref["energy"]), call
+        assert np.abs(got["force"] - ref["force"]).max() <= F_ABS, call
+        assert np.abs(got["virial"] - ref["virial"]).max() <= 1e-10 * max(1.0, np.abs(ref["virial"]).max()), call
+    assert len(set(per_call)) == 1 and per_call[0] > 0, per_call
+    m.set_graph(0)
+    n0 = m.kernel_launches()
+    eager = m.eval(bufs[1], dt, box)
+    torch.cuda.synchronize()
+    assert m.kernel_launches() - n0 == per_call[0]
+    assert np.abs(eager["force"].cpu().numpy() - outs[1]["force"].cpu().numpy()).max() <= 1e-12
     m.close()
