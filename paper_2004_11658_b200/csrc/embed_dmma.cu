@@ -65,6 +65,21 @@ __device__ __forceinline__ void emb_cp_commit() { asm volatile("cp.async.commit_
 template <int N>
 __device__ __forceinline__ void emb_cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
+
+// The net's padded weights (EL<SP>::total doubles: 67 KB for 25-50-100, 87 KB for 32-64-128) go global -> shared as ONE
+// bulk copy of the TMA engine (cp.async.bulk, completion on an mbarrier): one memory round trip per CTA instead of a
+// loop of dependent loads — what a 192-atom evaluation with a cold L2 waits for.
+__device__ __forceinline__ void stage_net(double *W, const double *__restrict__ netp, int total, uint64_t *mbar) {
+  if (threadIdx.x == 0) {
+    tc::mbar_init(mbar, 1);
+    tc::fence_mbar_init();
+    tc::mbar_arrive_expect_tx(mbar, (unsigned)total * 8u);
+    tc::bulk_g2s(W, netp, (unsigned)total * 8u, mbar);
+  }
+  __syncthreads();                                       // the initialised barrier is visible to every waiter
+  tc::mbar_wait(mbar, 0);
+}
+
 static int sp_for(int s1) {
   if (s1 <= 8) return 2;
   if (s1 <= 16) return 4;
@@ -199,8 +214,8 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         toff[ch][k] = r < P.s1 ? (c * P.s1 + r) * 4 + (lane & 3) : -1;
       }
   }
-  for (int k = tid; k < L::total; k += (32 * P1_WARPS)) W[k] = netp[k];
-  __syncthreads();
+  __shared__ uint64_t wbar;
+  stage_net(W, netp, L::total, &wbar);
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
@@ -397,8 +412,8 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
   double4 *drs = reinterpret_cast<double4 *>(smem + ((L::total + 1) & ~1) + P2_WARPS * L::tile2 + warp * EMB_STG);
   int *nls = reinterpret_cast<int *>(drs + 64);
   __shared__ double vred[P2_WARPS][9];
-  for (int k = tid; k < L::total; k += (32 * P2_WARPS)) W[k] = netp[k];
-  __syncthreads();
+  __shared__ uint64_t wbar;
+  stage_net(W, netp, L::total, &wbar);
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
@@ -670,10 +685,10 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   int *rqj = rjn + R::RING;                                             //   its row in this chunk when both directions run, else -1
   uint64_t *mbar = reinterpret_cast<uint64_t *>(rqj + R::RING);
   __shared__ double vred[P2_WARPS][9];
-  for (int k = tid; k < L::total; k += (32 * P2_WARPS)) W[k] = netp[k];
+  __shared__ uint64_t wbar;
   if (lane == 0) tc::mbar_init(mbar, 1);
   tc::fence_mbar_init();
-  __syncthreads();
+  stage_net(W, netp, L::total, &wbar);
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
   const int t = a;
@@ -886,9 +901,9 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 static int g_sm_count = 0;
 
 // Segments per atom (work items per atom and net): 1 when the chunk has enough atoms to give every warp of the GPU two
-// of them; up to 8 for small chunks (configs[0]: 192 atoms on 148 SMs x 8 warps).
-static int seg_count(int n_atoms, int warps) {
-  const long long want = 2ll * g_sm_count * warps;
+// of them (counting all nets); up to 8 for small chunks (configs[0]: 192 atoms on 148 SMs x 8 warps).
+static int seg_count(int n_atoms, int warps, int nets) {
+  const long long want = 2ll * g_sm_count * warps / (nets > 0 ? nets : 1);   // the nets' launches run side by side
   long long k = (want + n_atoms - 1) / (n_atoms > 0 ? n_atoms : 1);
   return (int)(k < 1 ? 1 : (k > 8 ? 8 : k));
 }
@@ -911,7 +926,7 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
     if (e != cudaSuccess) return e;
     configured_ru = smem_ru;
   }
-  const int nseg = C.fslot ? 1 : seg_count(C.n, P1_WARPS);   // deterministic mode: no reductions into T
+  const int nseg = C.fslot ? 1 : seg_count(C.n, P1_WARPS, P.ntypes * P.ntypes);   // deterministic mode: no reductions into T
   if (reuse || nseg > 1) {                               // every accumulation into T is then an addition
     cudaError_t e = cudaMemsetAsync(C.T, 0, sizeof(double) * (size_t)C.n * P.M * 4, st);
     if (e != cudaSuccess) return e;
@@ -919,21 +934,23 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
   const int grid = (int)min((long long)g_sm_count, ((long long)C.n * nseg + P1_WARPS - 1) / P1_WARPS);
   // nets of one centre type a accumulate into the same T rows (t = 0 stores, t > 0 adds): one stream per a, so that the
   // tail of one launch overlaps the start of another centre type's
+  // (with row segments every accumulation is a reduction: then every net gets its own stream)
   cudaStream_t ts[DPB_MAX_TYPES];
-  cudaError_t e = dpb_fork_streams(P.ntypes, st, ts);
+  const int ns = nseg > 1 ? min(P.ntypes * P.ntypes, DPB_MAX_TYPES) : P.ntypes;
+  cudaError_t e = dpb_fork_streams(ns, st, ts);
   if (e != cudaSuccess) return e;
   for (int a = 0; a < P.ntypes; ++a)
     for (int t = 0; t < P.ntypes; ++t) {
       const double *net = W.emb + (size_t)(a * P.ntypes + t) * W.net_stride;
+      cudaStream_t s = nseg > 1 ? ts[(a * P.ntypes + t) % ns] : ts[P.ntypes - 1 - a];
       if (reuse && a == t)
-        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, ts[P.ntypes - 1 - a]>>>(P, C, net, a, t,
-                                                                                           nseg > 1 ? 2 : 1, nseg);
+        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, s>>>(P, C, net, a, t, nseg > 1 ? 2 : 1, nseg);
       else
-        k_pass1_dmma<SP, 1, false><<<grid, (32 * P1_WARPS), smem, ts[P.ntypes - 1 - a]>>>(
-            P, C, net, a, t, nseg > 1 ? 2 : (reuse ? 1 : t > 0), nseg);
+        k_pass1_dmma<SP, 1, false><<<grid, (32 * P1_WARPS), smem, s>>>(P, C, net, a, t,
+                                                                      nseg > 1 ? 2 : (reuse ? 1 : t > 0), nseg);
       DPB_LAUNCHED(1);
     }
-  if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
+  if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;
   return cudaGetLastError();
 }
 
@@ -957,7 +974,7 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     if (e != cudaSuccess) return e;
     configured_ru = true;
   }
-  const int nseg = C.fslot ? 1 : seg_count(C.n, P2_WARPS);
+  const int nseg = C.fslot ? 1 : seg_count(C.n, P2_WARPS, P.ntypes * P.ntypes);
   const int grid = (int)min((long long)g_sm_count, ((long long)C.n * nseg + P2_WARPS - 1) / P2_WARPS);
   // the nets are independent here (forces and virial are atomic sums, slot stores are disjoint): a stream per net, so
   // that the tail of every launch is filled by the others

@@ -18,9 +18,7 @@
 
 #include <vector>
 
-#define FIT_BK 16
 #define FIT_STAGES 3
-#define FIT_LDA (FIT_BK + 4)
 
 struct FitNet {            // device pointers into the padded fitting weights of one species
   const double *W0, *b0, *W1, *b1, *W2, *b2, *w3, *W0T, *W1T, *W2T;
@@ -60,10 +58,12 @@ struct GemmArgs {
 
 // WM = warp rows per CTA: CTA tile = 16 WM rows x 16 NBW columns, 64 WM threads.  (2, 15 / 8): the throughput shape;
 // (1, 3): 16 x 48 tiles for small systems, where the number of CTAs, not the tile efficiency, bounds the stage.
-template <int WM, int NBW, int EPI>
-__global__ void __launch_bounds__(64 * WM, 2)
+// FIT_BK = K tile: 16 for the throughput shape; 80 for small systems, where a K = 240 GEMM is then three tiles that are
+// all in flight at once (one memory latency instead of fifteen; a ragged last tile is zero-filled).
+template <int WM, int NBW, int EPI, int FIT_BK>
+__global__ void __launch_bounds__(64 * WM, FIT_BK == 16 ? 2 : 1)
 k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
-  constexpr int FIT_BM = 16 * WM, FIT_THREADS = 64 * WM;
+  constexpr int FIT_BM = 16 * WM, FIT_THREADS = 64 * WM, FIT_LDA = FIT_BK + 4;
   constexpr int BN = 16 * NBW, LDB = BN + 4;
   extern __shared__ __align__(16) double smem[];
   double *As = smem;                                        // [STAGES][BM][LDA]
@@ -75,7 +75,7 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gq = lane >> 2, q = lane & 3;
   const int wm = warp >> 1, wn = warp & 1;                  // warp tile: rows 16 wm .., cols 8 NBW wn ..
   // split-K (EPI_ATOMIC, small systems): blockIdx.z takes the K tiles [kt0, kt1) and adds its partial sums to out0
-  const int nkt_all = g.K / FIT_BK;
+  const int nkt_all = (g.K + FIT_BK - 1) / FIT_BK;
   const int kt0 = (int)(((long long)nkt_all * blockIdx.z) / gridDim.z);
   const int nkt = (int)(((long long)nkt_all * (blockIdx.z + 1)) / gridDim.z) - kt0;
 
@@ -84,14 +84,14 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
     double *bs = Bs + stage * FIT_BK * LDB;
     const int k0 = (kt0 + kt) * FIT_BK;
     for (int c = tid; c < FIT_BM * (FIT_BK / 2); c += FIT_THREADS) {
-      const int m = c >> 3, kk = (c & 7) * 2;
-      const bool ok = m0 + m < row_hi;
-      cp_async16(as + m * FIT_LDA + kk, g.A + (size_t)(ok ? m0 + m : m0) * g.lda + k0 + kk, ok);
+      const int m = c / (FIT_BK / 2), kk = (c - m * (FIT_BK / 2)) * 2;
+      const bool ok = m0 + m < row_hi && k0 + kk < g.K;
+      cp_async16(as + m * FIT_LDA + kk, g.A + (size_t)(m0 + m < row_hi ? m0 + m : m0) * g.lda + (ok ? k0 + kk : 0), ok);
     }
     for (int c = tid; c < FIT_BK * (BN / 2); c += FIT_THREADS) {
       const int k = c / (BN / 2), nn = (c - k * (BN / 2)) * 2;
-      const bool ok = n0 + nn < g.N;
-      cp_async16(bs + k * LDB + nn, g.B + (size_t)(k0 + k) * g.ldb + (ok ? n0 + nn : 0), ok);
+      const bool ok = n0 + nn < g.N && k0 + k < g.K;
+      cp_async16(bs + k * LDB + nn, g.B + (size_t)(ok ? k0 + k : 0) * g.ldb + (ok ? n0 + nn : 0), ok);
     }
   };
 
@@ -409,18 +409,19 @@ size_t v1_workspace_bytes(const DevModel &P, int64_t chunk) {
   return sizeof(double) * (size_t)chunk * (2 * dimp + 6 * fwp) + 256;
 }
 
-template <int WM, int NBW, int EPI>
+template <int WM, int NBW, int EPI, int FIT_BK = 16>
 static cudaError_t gemm_t(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st, int splitk = 1) {
   constexpr int BN = 16 * NBW, FIT_BM = 16 * WM;
-  const size_t smem = sizeof(double) * FIT_STAGES * (FIT_BM * FIT_LDA + FIT_BK * (BN + 4));
+  const size_t smem = sizeof(double) * FIT_STAGES * (FIT_BM * (FIT_BK + 4) + FIT_BK * (BN + 4));
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_fit_gemm<WM, NBW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_fit_gemm<WM, NBW, EPI, FIT_BK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
   dim3 grid((C.n + FIT_BM - 1) / FIT_BM, (g.N + BN - 1) / BN, splitk);
-  k_fit_gemm<WM, NBW, EPI><<<grid, 64 * WM, smem, st>>>(C, ty, g);
+  k_fit_gemm<WM, NBW, EPI, FIT_BK><<<grid, 64 * WM, smem, st>>>(C, ty, g);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
@@ -430,7 +431,7 @@ static cudaError_t gemm_t(const ChunkView &C, int ty, const GemmArgs &g, cudaStr
 #define FIT_SMALL_N 2048
 template <int NBW, int EPI>
 static cudaError_t gemm(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st) {
-  if (C.n <= FIT_SMALL_N) return gemm_t<1, 3, EPI>(C, ty, g, st);
+  if (C.n <= FIT_SMALL_N) return gemm_t<1, 3, EPI, 80>(C, ty, g, st);
   return gemm_t<2, NBW, EPI>(C, ty, g, st);
 }
 
@@ -469,7 +470,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     // the few CTAs a 192-atom box offers), partial sums added into the cleared Z0, bias and tanh in a second kernel.
     g = GemmArgs{D, dimp, N.W0, fwp, dimp, fwp, N.b0, nullptr, nullptr, fwp, Z0, nullptr, fwp};
     if (splitk) {
-      if ((e = gemm_t<1, 3, EPI_ATOMIC>(C, ty, g, s, 8)) != cudaSuccess) return e;
+      if ((e = gemm_t<1, 3, EPI_ATOMIC, 80>(C, ty, g, s, 8)) != cudaSuccess) return e;
       k_bias_tanh_v1<<<C.n, 64, 0, s>>>(C, ty, fwp, N.b0, Z0);
       DPB_LAUNCHED(1);
     } else if ((e = gemm<15, EPI_TANH>(C, ty, g, s)) != cudaSuccess) return e;
