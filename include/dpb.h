@@ -182,6 +182,22 @@ int dpb_eval_local(dpb_model *model, void *stream, int64_t nloc, int64_t nall, c
                    const int32_t *type, const double bounds[6], double *energy, double *atom_energy, double *force,
                    double *virial, int32_t *nlist, dpb_eval_info *info);
 
+/* General periodic cell: triclinic cells and cells thinner than 2 r_c, which dpb_eval refuses.
+ * Evaluated the way the paper formulates periodicity: the atoms, wrapped into the cell, are the local
+ * atoms; every lattice image whose fractional coordinate lies within r_c / h_c of the cell (h_c = perpendicular height
+ * along lattice vector c; ceil(r_c / h_c) image shells) is a ghost; dpb_eval_local's kernels do the arithmetic; the
+ * ghost force increments are added to the atoms they are images of.  Image construction and fold-back are kernels of
+ * this library (csrc/cell.cu).
+ *   cell         HOST fp64 [9], rows = lattice vectors (any non-singular cell; DPB_EBOX if singular or thinner than r_c/16)
+ *   coord, type  DEVICE, [N][3] / [N]; raw positions (wrapped internally)
+ *   energy [1], atom_energy [N], force [N][3], virial [9]: DEVICE, as dpb_eval (any may be NULL)
+ *   info         HOST or NULL; n_real_pairs etc. refer to the N atoms of the cell
+ * One host synchronisation (the number of images sizes the evaluation), otherwise asynchronous on `stream`.
+ * Not available with the deterministic reduction (DPB_ENOTIMPL). */
+int dpb_eval_cell(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,
+                  const double cell[9], double *energy, double *atom_energy, double *force, double *virial,
+                  dpb_eval_info *info);
+
 /* Velocity-Verlet pieces for a driver that owns the time loop — the decomposition's MD driver in
  * paper_2004_11658_b200/dd.py, where an evaluation is ghost exchange + dpb_eval_local + reverse exchange.
  * dpb_md_coefficients (HOST -> HOST): coeff_h[t] = (dt/2) / (m_t u) and coeff_h[ntypes + t] = m_t u with

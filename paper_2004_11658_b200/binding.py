@@ -51,8 +51,8 @@ class EvalInfo:
 
 
 def lib_path() -> str:
-    # DPB_LIBRARY selects another build of the same library (kernel-tuning experiments); default: the in-tree build
-    return os.environ.get("DPB_LIBRARY") or os.path.join(HERE, "libdpb.so")
+    """The in-tree build (paper_2004_11658_b200/build.py); there is no other place the library is looked for."""
+    return os.path.join(HERE, "libdpb.so")
 
 
 _LIB = None
@@ -87,6 +87,7 @@ def load_library():
     lib.dpb_eval_local.argtypes = [vp, vp, i64, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, vp,
                                    C.POINTER(_Info)]
     lib.dpb_eval_host.argtypes = lib.dpb_eval.argtypes
+    lib.dpb_eval_cell.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, C.POINTER(_Info)]
     lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
     lib.dpb_md_run.argtypes = [vp, vp, i64, vp, vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                C.POINTER(_MDParams), vp, C.POINTER(_MDInfo)]
@@ -268,6 +269,29 @@ class DPModel:
                                      C.c_void_p(o["force"].data_ptr()), C.c_void_p(o["virial"].data_ptr()),
                                      C.c_void_p(o["nlist"].data_ptr()) if want_nlist else None,
                                      C.byref(info) if want_info else None)
+        self._chk(rc)
+        if want_info:
+            o["info"] = EvalInfo(int(info.n_real_pairs), int(info.n_overflow), tuple(info.max_nei), int(info.n_chunks))
+        return o
+
+    def eval_cell(self, coord, types, cell, want_info=False):
+        """dpb_eval_cell: N atoms in a general periodic cell (rows of `cell` = lattice vectors; triclinic allowed, r_c may
+        exceed half the cell).  coord float64 [N,3] and types int32 [N] are CUDA tensors; returns a dict of CUDA tensors."""
+        torch = _torch()
+        assert coord.is_cuda and coord.dtype == torch.float64 and coord.is_contiguous()
+        assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
+        n = int(coord.shape[0])
+        dev = coord.device
+        o = {"energy": torch.empty(1, dtype=torch.float64, device=dev),
+             "atom_energy": torch.empty(max(n, 1), dtype=torch.float64, device=dev)[:n],
+             "force": torch.empty((max(n, 1), 3), dtype=torch.float64, device=dev)[:n],
+             "virial": torch.empty((3, 3), dtype=torch.float64, device=dev)}
+        b, bp = self._box(cell)
+        info = _Info() if want_info else None
+        rc = self.lib.dpb_eval_cell(self._h, self._stream(), n, C.c_void_p(coord.data_ptr()), C.c_void_p(types.data_ptr()),
+                                    bp, C.c_void_p(o["energy"].data_ptr()), C.c_void_p(o["atom_energy"].data_ptr()),
+                                    C.c_void_p(o["force"].data_ptr()), C.c_void_p(o["virial"].data_ptr()),
+                                    C.byref(info) if want_info else None)
         self._chk(rc)
         if want_info:
             o["info"] = EvalInfo(int(info.n_real_pairs), int(info.n_overflow), tuple(info.max_nei), int(info.n_chunks))

@@ -141,6 +141,7 @@ struct dpb_model {
   // deterministic mode: inverse of s_idx, full-size lists, per-slot dE_i/dd_ik, per-atom virial parts
   Buf pos_of, nl_all, nreal_all, fslot, vpart;
   Buf md_raw, md_nraw, md_xyz0, md_force, md_scal, md_mass;
+  Buf cell_frac, cell_x, cell_t, cell_owner, cell_f, cell_cnt;   // dpb_eval_cell: local + image atoms
   int md_cap_raw = 0;
   double md_skin = 0.0;
   DevGrid md_grid;
@@ -240,7 +241,8 @@ extern "C" int dpb_model_destroy(dpb_model *m) {
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
                 &m->nl, &m->nlp, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
                 &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
-                &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass};
+                &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass,
+                &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_owner, &m->cell_f, &m->cell_cnt};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
@@ -697,6 +699,72 @@ extern "C" int dpb_eval_local(dpb_model *m, void *stream, int64_t nloc, int64_t 
   int rc = run_eval(m, st, nall, coord, type, bounds, energy, atom_energy, force, virial, nlist, false, 0, nloc);
   if (rc != DPB_OK) return rc;
   if (info) return finish_info(m, st, nloc, info);
+  return DPB_OK;
+}
+
+// ---- general periodic cell through explicit images ---------------------------
+extern "C" int dpb_eval_cell(dpb_model *m, void *stream, int64_t natoms, const double *coord, const int32_t *type,
+                             const double cell[9], double *energy, double *atom_energy, double *force, double *virial,
+                             dpb_eval_info *info) {
+  if (!m || !cell) return fail(DPB_EINVAL, "dpb_eval_cell: null model / cell");
+  if (natoms < 0 || natoms > 2000000000ll) return fail(DPB_EINVAL, "natoms out of range");
+  if (natoms > 0 && (!coord || !type)) return fail(DPB_EINVAL, "null coord / type");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const DevModel &P = m->P;
+  CellGeom G;
+  const double *a = cell;
+  for (int k = 0; k < 9; ++k) G.A[k] = a[k];
+  const double cr[3][3] = {{a[4] * a[8] - a[5] * a[7], a[5] * a[6] - a[3] * a[8], a[3] * a[7] - a[4] * a[6]},   // a1 x a2
+                           {a[7] * a[2] - a[8] * a[1], a[8] * a[0] - a[6] * a[2], a[6] * a[1] - a[7] * a[0]},   // a2 x a0
+                           {a[1] * a[5] - a[2] * a[4], a[2] * a[3] - a[0] * a[5], a[0] * a[4] - a[1] * a[3]}};  // a0 x a1
+  const double det = a[0] * cr[0][0] + a[1] * cr[0][1] + a[2] * cr[0][2];
+  if (!(fabs(det) > 0.0) || !std::isfinite(det)) return fail(DPB_EBOX, "dpb_eval_cell: the cell is singular");
+  long long nshift = 1;
+  for (int c = 0; c < 3; ++c) {
+    const double nrm = sqrt(cr[c][0] * cr[c][0] + cr[c][1] * cr[c][1] + cr[c][2] * cr[c][2]);
+    const double h = fabs(det) / nrm;                      // perpendicular height along lattice direction c
+    G.margin[c] = P.rc / h;
+    const double ns = ceil(G.margin[c]);
+    if (!(ns <= 16.0)) return fail(DPB_EBOX, "dpb_eval_cell: the cell is thinner than r_c / 16 along lattice vector %d", c);
+    G.nshell[c] = (int)ns;
+    nshift *= 2 * G.nshell[c] + 1;
+    for (int r = 0; r < 3; ++r) G.Ainv[3 * r + c] = cr[c][r] / det;      // column c of A^-1 = (a_j x a_k) / det
+  }
+  // bounds: the 8 corners of the parallelepiped widened by the margins
+  double bounds[6] = {1e300, 1e300, 1e300, -1e300, -1e300, -1e300}, big = 0.0;
+  for (int k = 0; k < 8; ++k) {
+    double f[3], x[3] = {0.0, 0.0, 0.0};
+    for (int c = 0; c < 3; ++c) f[c] = ((k >> c) & 1) ? 1.0 + G.margin[c] : -G.margin[c];
+    for (int c = 0; c < 3; ++c) x[c] = f[0] * a[c] + f[1] * a[3 + c] + f[2] * a[6 + c];
+    for (int c = 0; c < 3; ++c) {
+      if (x[c] < bounds[c]) bounds[c] = x[c];
+      if (x[c] > bounds[3 + c]) bounds[3 + c] = x[c];
+      if (fabs(x[c]) > big) big = fabs(x[c]);
+    }
+  }
+  for (int c = 0; c < 3; ++c) { bounds[c] -= 1e-9 * (1.0 + big); bounds[3 + c] += 1e-9 * (1.0 + big); }
+  const long long cap = natoms * (nshift - 1);
+  if (natoms + cap > 2000000000ll) return fail(DPB_EINVAL, "dpb_eval_cell: too many lattice images (%lld)", cap);
+  const size_t rows = (size_t)(natoms + cap) + 1;
+  CU(m->cell_frac.reserve(sizeof(double) * 3 * ((size_t)natoms + 1)), "cell workspace");
+  CU(m->cell_x.reserve(sizeof(double) * 3 * rows), "cell workspace");
+  CU(m->cell_t.reserve(sizeof(int) * rows), "cell workspace");
+  CU(m->cell_owner.reserve(sizeof(int) * rows), "cell workspace");
+  CU(m->cell_f.reserve(sizeof(double) * 3 * rows), "cell workspace");
+  CU(m->cell_cnt.reserve(16), "cell workspace");
+  CU(launch_cell_wrap(natoms, coord, type, G, m->cell_frac.as<double>(), m->cell_x.as<double>(), m->cell_t.as<int>(),
+                      m->cell_owner.as<int>(), st), "cell wrap");
+  CU(launch_cell_images(natoms, m->cell_frac.as<double>(), type, G, cap, m->cell_x.as<double>(), m->cell_t.as<int>(),
+                        m->cell_owner.as<int>(), m->cell_cnt.as<unsigned long long>(), st), "cell images");
+  unsigned long long nimg = 0;                             // the number of images sizes the evaluation: one host sync
+  CU(cudaMemcpyAsync(&nimg, m->cell_cnt.p, sizeof(nimg), cudaMemcpyDeviceToHost, st), "image count");
+  CU(cudaStreamSynchronize(st), "stream synchronise");
+  const int64_t nall = natoms + (int64_t)nimg;
+  int rc = run_eval(m, st, nall, m->cell_x.as<double>(), m->cell_t.as<int>(), bounds, energy, atom_energy,
+                    force ? m->cell_f.as<double>() : nullptr, virial, nullptr, false, 0, natoms);
+  if (rc != DPB_OK) return rc;
+  if (force) CU(launch_cell_fold(nall, natoms, m->cell_owner.as<int>(), m->cell_f.as<double>(), force, st), "cell fold");
+  if (info) return finish_info(m, st, natoms, info);
   return DPB_OK;
 }
 

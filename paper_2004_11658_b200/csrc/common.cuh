@@ -90,6 +90,19 @@ cudaError_t launch_dd_pack(int64_t n, const double *coord, const int *type, int 
 cudaError_t launch_dd_unpack(int64_t k, const double *pack, double *coord_out, int *type_out, cudaStream_t st);
 cudaError_t launch_dd_add_forces(int64_t k, const int *idx, const double *fin, double *force, cudaStream_t st);
 
+// cell.cu: explicit lattice images of a general periodic cell (dpb_eval_cell)
+struct CellGeom {
+  double A[9], Ainv[9];      // rows of A = lattice vectors; x = s A, s = x Ainv
+  double margin[3];          // r_c / h_c, h_c = perpendicular height of the cell along lattice direction c
+  int nshell[3];             // ceil(r_c / h_c) image shells
+};
+cudaError_t launch_cell_wrap(int64_t n, const double *coord, const int *type, const CellGeom &G, double *frac,
+                             double *xall, int *tall, int *owner, cudaStream_t st);
+cudaError_t launch_cell_images(int64_t n, const double *frac, const int *type, const CellGeom &G, int64_t cap,
+                               double *xall, int *tall, int *owner, unsigned long long *count, cudaStream_t st);
+cudaError_t launch_cell_fold(int64_t nall, int64_t n, const int *owner, const double *fall, double *force,
+                             cudaStream_t st);
+
 // Process-wide count of kernels launched by this library (reported by dpb_kernel_launches()).
 extern unsigned long long g_dpb_launches;
 #define DPB_LAUNCHED(n) (g_dpb_launches += (unsigned long long)(n))

@@ -268,7 +268,7 @@ def test_exchange_kernels_against_numpy():
 
 
 def test_triclinic_cell_through_explicit_images():
-    """paper_2004_11658_b200.cell.eval_cell: (1) a genuinely triclinic cell, thinner than 2 r_c
+    """dpb_eval_cell through the C ABI (cell.py only marshals): (1) a genuinely triclinic cell, thinner than 2 r_c
     along c, against the oracle's dpo_eval_local on images built by brute force (tests/test_oracle_local.py);
     (2) W192 described by the sheared cell (a1, a2 + a1, a3 + a2 - a1) against dpb_eval on the orthorhombic box."""
     import paper_2004_11658_b200 as pk

@@ -178,26 +178,51 @@ def _eval_cell_with_oracle(o, coord, types, cell, rc, images):
     return r["energy"], r["atom_energy"], f, r["virial"], len(x)
 
 
-def _cellpy_images(coord, cell, rc):
-    import torch
-    from paper_2004_11658_b200.cell import periodic_images
-    x, own, (lo, hi) = periodic_images(torch.from_numpy(np.ascontiguousarray(coord)), cell, rc)
-    x = x.numpy()
-    assert (x >= lo).all() and (x <= hi).all()                       # the bounds handed to dpb_eval_local hold them all
-    return x, own.numpy()
+def _cell_heights(cell):
+    """Perpendicular heights h_c = V / |a_j x a_k| of the parallelepiped spanned by the rows of `cell`."""
+    a = np.asarray(cell, dtype=np.float64).reshape(3, 3)
+    vol = abs(np.linalg.det(a))
+    return np.array([vol / np.linalg.norm(np.cross(a[(c + 1) % 3], a[(c + 2) % 3])) for c in range(3)])
+
+
+def _margin_images(coord, cell, rc):
+    """The image selection rule of dpb_eval_cell (include/dpb.h, csrc/cell.cu), restated in numpy so that the RULE is
+    pinned here without a GPU: wrap the fractional coordinates into [0, 1); keep every lattice image whose fractional
+    coordinate t_c lies in [-r_c / h_c, 1 + r_c / h_c] for all c (ceil(r_c / h_c) shells per lattice direction); the
+    bounds are the corners of the widened parallelepiped."""
+    import itertools
+    a = np.asarray(cell, dtype=np.float64).reshape(3, 3)
+    h = _cell_heights(a)
+    s = coord @ np.linalg.inv(a)
+    s = s - np.floor(s)
+    m = rc / h
+    n = [int(np.ceil(v)) for v in m]
+    parts, owners = [s], [np.arange(len(coord))]
+    for shift in itertools.product(*(range(-k, k + 1) for k in n)):
+        if shift == (0, 0, 0):
+            continue
+        t = s + np.array(shift, dtype=np.float64)
+        idx = np.nonzero(((t >= -m) & (t <= 1.0 + m)).all(axis=1))[0]
+        parts.append(t[idx])
+        owners.append(idx)
+    x = np.concatenate(parts) @ a
+    corners = np.array([[(-m[c] if (k >> c) & 1 == 0 else 1.0 + m[c]) for c in range(3)] for k in range(8)]) @ a
+    pad = 1e-9 * (1.0 + np.abs(corners).max())
+    assert (x >= corners.min(axis=0) - pad).all() and (x <= corners.max(axis=0) + pad).all()   # the bounds hold them all
+    return x, np.concatenate(owners)
 
 
 def test_sheared_description_of_an_orthorhombic_lattice():
     """The cells (a1, a2, a3), (a1, a2 + a1, a3) and (a1, a2 + a1, a3 + a2 - a1) generate the same lattice, so E, E_i,
     F and the virial from explicit images of the sheared (triclinic) cells must equal the orthorhombic periodic
-    evaluation; both image builders (brute force here, cell.py's fractional-coordinate margins) are checked."""
+    evaluation; both image builders (brute force here, dpb_eval_cell's fractional-coordinate margins) are checked."""
     spec, emb, fit, coord, types, box = _setup()
     o = Oracle.from_spec(spec, emb, fit)
     ref = o.eval(coord, types, box)
     a = np.asarray(box).reshape(3, 3)
     cells = [a, np.array([a[0], a[1] + a[0], a[2]]), np.array([a[0], a[1] + a[0], a[2] + a[1] - a[0]])]
     for cell in cells:
-        for images in (_brute_images, _cellpy_images):
+        for images in (_brute_images, _margin_images):
             E, Ei, F, V, nall = _eval_cell_with_oracle(o, coord, types, cell, spec.rcut, images)
             assert abs(E - ref["energy"]) < 1e-12 * abs(ref["energy"])
             assert np.abs(Ei - ref["atom_energy"]).max() < 1e-12 * np.abs(ref["atom_energy"]).max()
@@ -206,9 +231,9 @@ def test_sheared_description_of_an_orthorhombic_lattice():
 
 
 def test_cell_images_thin_cell_and_heights():
-    """cell.py against the brute-force images on a genuinely triclinic cell thinner than 2 r_c in one direction
-    (two image shells there), and the perpendicular heights of a sheared cell."""
-    from paper_2004_11658_b200.cell import cell_heights
+    """dpb_eval_cell's image rule against the brute-force images on a genuinely triclinic cell thinner than 2 r_c in one
+    direction (two image shells there), and the perpendicular heights of a sheared cell."""
+    cell_heights = _cell_heights
     spec, emb, fit, coord, types, box = _setup(n=30, L=9.0, seed=6)
     o = Oracle.from_spec(spec, emb, fit)
     cell = np.array([[9.0, 0.0, 0.0], [2.5, 8.0, 0.0], [1.0, -1.5, 3.6]])     # height along c: 3.6 < r_c = 4
@@ -217,7 +242,7 @@ def test_cell_images_thin_cell_and_heights():
     rng = np.random.default_rng(8)
     x = rng.uniform(0, 1, size=(30, 3)) @ cell
     a = _eval_cell_with_oracle(o, x, types, cell, spec.rcut, _brute_images)
-    b = _eval_cell_with_oracle(o, x, types, cell, spec.rcut, _cellpy_images)
-    assert b[4] >= a[4]                                             # cell.py keeps a superset of the needed images
+    b = _eval_cell_with_oracle(o, x, types, cell, spec.rcut, _margin_images)
+    assert b[4] >= a[4]                                             # the margin rule keeps a superset of the needed images
     assert abs(a[0] - b[0]) < 1e-12 * abs(a[0]) and np.abs(a[2] - b[2]).max() < 1e-11 and np.abs(a[3] - b[3]).max() < 1e-10
     assert np.abs(b[2].sum(axis=0)).max() < 1e-10                   # periodic system: total force vanishes
