@@ -504,6 +504,21 @@ def run_cuda(args):
                 f"algorithmic flops of the stage / its CUDA-event time against the dense tensor peak ({how}); the tensor "
                 "pipe executes 3x (tf32) or 6x (bf16) these flops (error-compensated split); the stage is bound by MUFU "
                 "(fp32 tanh) and instruction issue, not by the tensor pipe (DESIGN.md section 9)")
+        if args.variant == 2 and not mixed:
+            # what fusion and padding-skip buy = this run (the paper's pipeline) against variant 1
+            free_b, total_b = torch.cuda.mem_get_info(dev)
+            model.close()
+            r1 = measure(name, "fp64", 1, max(3, min(args.steps, 10)), 3, dev, rank, world, args.stage_every)
+            r1["model"].close()
+            nm = sum(spec.sel)
+            line["strawman"] = {
+                "what": "variant 2 = PAPER.md section 3.2.3 on B200: GEMMs over all padded slots, bias and concat as GEMMs, "
+                        "separate tanh / tanh-grad kernels, G and activations materialised, reverse-mode backward",
+                "padded_slots": int(n * nm), "real_pairs": int(info.n_real_pairs),
+                "device_memory_in_use_bytes": int(total_b - free_b),
+                "variant1_ms_per_step": r1["ms_median"], "variant1_stage_us": {nm_: r1["stage_us"][i] for i, nm_ in enumerate(STAGES)},
+                "ratio_variant2_over_variant1": ms_per_step / r1["ms_median"],
+                "ratio_embedding_stages": (stage_us[2] + stage_us[4]) / max(1e-9, r1["stage_us"][2] + r1["stage_us"][4])}
         if args.md_steps > 0:
             line["md"] = run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed)
         if dd_leg is not None:

@@ -87,7 +87,11 @@ int dpb_model_nm(const dpb_model *model);
 int dpb_model_set_chunk(dpb_model *model, int64_t chunk_atoms);
 
 /* Select the kernel generation: 0 = plain reference kernels ("v0": unfused, thread-per-output FMA loops),
- * 1 = fused DMMA kernels (default).  Both compute the same path; tests compare each with the oracle. */
+ * 1 = fused DMMA kernels (default), 2 = the paper's own embedding pipeline as a measured strawman (
+ * PAPER.md:250-290): GEMMs over ALL padded slots of every (centre type, neighbour type) batch with the bias folded in,
+ * the concat skip as a GEMM with (I, I) (Eq. 12), separate tanh / tanh-grad kernels, G and every activation materialised
+ * in HBM (Eq. 13: about 4.8 KB per padded slot for the water model) and a reverse-mode backward; DPB_FP64 only, one host
+ * synchronisation per evaluation (the batch sizes).  All compute the same path; tests compare each with the oracle. */
 int dpb_model_set_variant(dpb_model *model, int variant);
 
 /* Deterministic reduction (DPB_FP64, variant 1): forces and virial are summed in a fixed order instead of with fp64

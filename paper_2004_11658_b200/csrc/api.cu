@@ -127,6 +127,8 @@ struct dpb_model {
   Buf emb, fit;                 // raw weights (layout of dpb_model_desc)
   V1Weights v1;                 // re-laid-out weights of the fused kernels
   TCWeights tcw;                // mixed precision: TF32 hi / lo operand images (embed_tc.cu)
+  V2Weights v2;                 // variant 2 (strawman.cu): padded matrices of the paper's pipeline, built on first use
+  Buf v2ws;
   // workspace
   Buf key, count, start, cursor, s_idx, s_xyz, stats, ei;
   Buf nl, nlp, dr, nreal, T, dT;
@@ -165,6 +167,7 @@ static int64_t effective_chunk(const dpb_model *m) {
   if (m->precision == DPB_FP64) {
     if (m->variant == 0 || !m->v1.ready) per += sizeof(double) * (2 * (size_t)P.dim + 7 * (size_t)P.fw);
     else per += v1_workspace_bytes(P, 1024) / 1024;
+    if (m->variant == 2) per += (size_t)P.nm * v2_slot_bytes(m->v2);       // Eq. 13's tensors: every padded slot
   } else {
     per += (tc_pair_workspace_bytes(P, 1024) + tc_pass2_workspace_bytes(P, 1024) + tc_fit_workspace_bytes(P, 1024)) / 1024;
   }
@@ -239,13 +242,14 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->nlp, &m->dr, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
+                &m->nl, &m->nlp, &m->dr, &m->v2ws, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
                 &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
                 &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass,
                 &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_owner, &m->cell_f, &m->cell_cnt};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
+  v2_release_weights(m->v2);
   tc_release_weights(m->tcw);
   for (cudaEvent_t &e : m->evs) cudaEventDestroy(e);
   for (GraphEntry &g : m->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
@@ -261,7 +265,18 @@ extern "C" int dpb_model_set_chunk(dpb_model *m, int64_t chunk) {
 }
 
 extern "C" int dpb_model_set_variant(dpb_model *m, int variant) {
-  if (!m || variant < 0 || variant > 1) return fail(DPB_EINVAL, "dpb_model_set_variant: variant must be 0 or 1");
+  if (!m || variant < 0 || variant > 2) return fail(DPB_EINVAL, "dpb_model_set_variant: variant must be 0, 1 or 2");
+  if (variant == 2) {
+    if (m->precision != DPB_FP64 || !m->v1.ready)
+      return fail(DPB_ENOTIMPL, "variant 2 (the paper's padded-dense pipeline) is built for DPB_FP64 and emb_s1 <= 32");
+    if (!m->v2.ready) {                                    // the raw weights live on the device: fetch them once
+      const DevModel &P = m->P;
+      std::vector<double> h((size_t)P.emb_net_size * P.ntypes * P.ntypes);
+      cudaError_t e = cudaMemcpy(h.data(), m->emb.p, sizeof(double) * h.size(), cudaMemcpyDeviceToHost);
+      if (e == cudaSuccess) e = v2_prepare_weights(P, h.data(), m->v2);
+      if (e != cudaSuccess) return fail(DPB_ECUDA, "variant 2 weights: %s", cudaGetErrorString(e));
+    }
+  }
   m->variant = variant;
   ++m->cfg_epoch;
   return DPB_OK;
@@ -459,6 +474,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     } else {
       CU(m->v1ws.reserve(v1_workspace_bytes(P, chunk)), "workspace");
     }
+    if (m->precision == DPB_FP64 && m->variant == 2)
+      CU(m->v2ws.reserve((size_t)chunk * P.nm * v2_slot_bytes(m->v2)), "workspace of the paper pipeline");
     if (m->precision == DPB_TF32) {
       CU(m->pairs.reserve(tc_pair_workspace_bytes(P, chunk)), "workspace");
       CU(m->dT32.reserve(tc_pass2_workspace_bytes(P, chunk)), "workspace");
@@ -500,6 +517,11 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
          "copy of the rebuild coordinates");
   }
   if (timing) cudaEventRecord(m->evs[1], st);
+  int ts_h[DPB_MAX_TYPES + 1] = {0};
+  if (m->precision == DPB_FP64 && m->variant == 2 && !nlist_only) {      // batch sizes of the padded GEMMs: one host sync
+    CU(cudaMemcpyAsync(ts_h, start + nkeys + 1, sizeof(int) * (P.ntypes + 1), cudaMemcpyDeviceToHost, st), "type counts");
+    CU(cudaStreamSynchronize(st), "stream synchronise");
+  }
 
   double *ei = atom_energy ? atom_energy : m->ei.as<double>();
   if (!nlist_only) {
@@ -544,6 +566,14 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
       if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
       CU(tc_pass2(P, C, m->tcw, m->pairs.p, m->dT32.as<float>(), force, virial, st), "pass2 tf32");
+      if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
+    } else if (m->variant == 2) {
+      CU(v2_pass1(P, C, m->v2, ts_h, m->v2ws.p, st), "pass1 v2");
+      if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);
+      CU(v1_fit(P, C, m->v1, m->fit.as<double>(), m->v1ws.p, ei, st), "fit");
+      CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
+      if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
+      CU(v2_pass2(P, C, m->v2, ts_h, m->v2ws.p, force, virial, st), "pass2 v2");
       if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
     } else if (m->variant == 0 || !m->v1.ready) {
       V0Scratch S;
@@ -617,7 +647,7 @@ extern "C" int dpb_model_set_graph(dpb_model *m, int mode) {
 static int eval_graphed(dpb_model *m, cudaStream_t st, int64_t natoms, const double *coord, const int32_t *type,
                         const double box[9], double *energy, double *atom_energy, double *force, double *virial,
                         int32_t *nlist) {
-  if (m->graph_mode == 0 || m->timing || (m->graph_mode == 1 && natoms > DPB_GRAPH_AUTO_ATOMS)) return 0;
+  if (m->graph_mode == 0 || m->timing || m->variant == 2 || (m->graph_mode == 1 && natoms > DPB_GRAPH_AUTO_ATOMS)) return 0;
   GraphKey key;
   memset(&key, 0, sizeof(key));
   key.natoms = natoms;

@@ -45,7 +45,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
-enum { EPI_TANH = 0, EPI_TANH_SKIP = 1, EPI_L3 = 2, EPI_BWD = 3, EPI_STORE = 4, EPI_ATOMIC = 5 };
+enum { EPI_TANH = 0, EPI_TANH_SKIP = 1, EPI_L3 = 2, EPI_BWD = 3, EPI_STORE = 4, EPI_ATOMIC = 5, EPI_ADD = 6 };
 
 struct GemmArgs {
   const double *A; int lda;          // [rows][lda], K columns used
@@ -145,7 +145,7 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
       const size_t oi = (size_t)m * g.ldi + n;
       x0[nb] = zero2; x1[nb] = zero2;
       if (n < g.N) {
-        if (EPI == EPI_TANH_SKIP || EPI == EPI_L3) x0[nb] = *reinterpret_cast<const double2 *>(g.in0 + oi);
+        if (EPI == EPI_TANH_SKIP || EPI == EPI_L3 || EPI == EPI_ADD) x0[nb] = *reinterpret_cast<const double2 *>(g.in0 + oi);
         if (EPI == EPI_BWD) {
           if (g.in0) x0[nb] = *reinterpret_cast<const double2 *>(g.in0 + oi);
           x1[nb] = *reinterpret_cast<const double2 *>(g.in1 + oi);
@@ -180,6 +180,8 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
         const double2 u = x1[nb];
         if (g.out0) *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0, v1);
         *reinterpret_cast<double2 *>(g.out1 + oo) = make_double2(v0 * (1.0 - u.x * u.x), v1 * (1.0 - u.y * u.y));
+      } else if (EPI == EPI_ADD) {
+        *reinterpret_cast<double2 *>(g.out0 + oo) = make_double2(v0 + x0[nb].x, v1 + x0[nb].y);
       } else if (EPI == EPI_ATOMIC) {
         atomicAdd(g.out0 + oo, v0);
         atomicAdd(g.out0 + oo + 1, v1);
@@ -433,6 +435,20 @@ template <int NBW, int EPI>
 static cudaError_t gemm(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st) {
   if (C.n <= FIT_SMALL_N) return gemm_t<1, 3, EPI, 80>(C, ty, g, st);
   return gemm_t<2, NBW, EPI>(C, ty, g, st);
+}
+
+// Plain GEMM on the same tiles for the strawman pipeline (strawman.cu): C[rows x N] = A[rows x K] B[K x N] (+ Cin).
+// K and N even, lda / ldb / ldc even (16-byte rows); `range` = device int[2] {0, INT_MAX} (the kernel's row-range hook).
+cudaError_t v1_plain_gemm(int64_t rows, const double *A, int lda, const double *B, int ldb, int K, int N,
+                          const double *Cin, double *Cout, int ldc, const int *range, cudaStream_t st) {
+  if (rows <= 0) return cudaSuccess;
+  ChunkView C{};
+  C.p0 = 0; C.n = (int)rows; C.type_start = range;
+  GemmArgs g{A, lda, B, ldb, K, N, nullptr, Cin, nullptr, ldc, Cout, nullptr, ldc};
+  if (N <= 32) return Cin ? gemm_t<2, 2, EPI_ADD>(C, 0, g, st) : gemm_t<2, 2, EPI_STORE>(C, 0, g, st);
+  if (N <= 64) return Cin ? gemm_t<2, 4, EPI_ADD>(C, 0, g, st) : gemm_t<2, 4, EPI_STORE>(C, 0, g, st);
+  if (N <= 112) return Cin ? gemm_t<2, 7, EPI_ADD>(C, 0, g, st) : gemm_t<2, 7, EPI_STORE>(C, 0, g, st);
+  return Cin ? gemm_t<2, 8, EPI_ADD>(C, 0, g, st) : gemm_t<2, 8, EPI_STORE>(C, 0, g, st);
 }
 
 cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, const double *fit, void *ws,

@@ -23,6 +23,27 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
 cudaError_t v1_pass2(const DevModel &P, const ChunkView &C, const V1Weights &W, double *force, double *virial,
                      cudaStream_t st);
 
+cudaError_t v1_plain_gemm(int64_t rows, const double *A, int lda, const double *B, int ldb, int K, int N,
+                          const double *Cin, double *Cout, int ldc, const int *range, cudaStream_t st);
+
+// Variant 2 ("paper pipeline", strawman.cu): padded-dense, unfused embedding stage of PAPER.md
+// section 3.2.3 — GEMMs over all padded slots with the bias folded in, concat as a GEMM with (I, I), separate tanh /
+// tanh-grad kernels, G and every activation materialised.
+struct V2Weights {
+  double *buf = nullptr;      // per net: B0 B1 II1 B2 II2 B2T II2T B1T II1T B0T (padded, see strawman.cu)
+  int *range = nullptr;       // device {0, INT_MAX}
+  int LD0 = 0, LD1 = 0, LD2 = 0;
+  long long net_stride = 0;
+  bool ready = false;
+};
+cudaError_t v2_prepare_weights(const DevModel &P, const double *emb_h, V2Weights &W);
+void v2_release_weights(V2Weights &W);
+size_t v2_slot_bytes(const V2Weights &W);                         // workspace per padded slot of a net batch
+cudaError_t v2_pass1(const DevModel &P, const ChunkView &C, const V2Weights &W, const int *type_start_h, void *ws,
+                     cudaStream_t st);
+cudaError_t v2_pass2(const DevModel &P, const ChunkView &C, const V2Weights &W, const int *type_start_h, void *ws,
+                     double *force, double *virial, cudaStream_t st);
+
 #ifdef __CUDACC__
 // tanh(x) = 1 - 2 / (exp(2x) + 1) with exp(2x) = 2^n 2^f: n = rint(2x log2 e) by the 1.5 * 2^52 trick, 2^f by a
 // degree-10 polynomial on [-0.5, 0.5] (relative error 2.9e-16), the reciprocal from MUFU.RCP64H refined by one cubic

@@ -2,7 +2,8 @@
 seeded inputs.  Bars (BASELINE.json north_star): nlist bit-exact including order and padding; fp64: relative error
 <= 1e-10 on E, absolute error <= 1e-9 eV/A on F.  We also bound E_i, the virial, T and dT.
 
-Both kernel generations are checked: variant 0 (plain unfused kernels) and variant 1 (fused DMMA kernels)."""
+All kernel generations are checked: variant 0 (plain unfused kernels), variant 1 (fused DMMA kernels) and variant 2
+(the paper's padded-dense, unfused GEMM pipeline as a strawman)."""
 import numpy as np
 import pytest
 
@@ -64,7 +65,7 @@ def _check_full(ref, got, n_overflow=0):
     assert np.abs(got["virial"] - ref["virial"]).max() <= 1e-10 * max(1.0, np.abs(ref["virial"]).max())
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("conditioned", [False, True])
 def test_water192_full_parity(variant, conditioned):
     """BASELINE config 0 (W192), literal and conditioned weight sets: every output element against the oracle."""
@@ -84,7 +85,7 @@ def test_water192_full_parity(variant, conditioned):
     m.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_copper_small_full_parity(variant):
     """Copper model (sel 512, 32-64-128) on a 6x6x6-cell FCC box (864 atoms, several row tiles + ragged tail)."""
     spec = MODELS["Cu32k"]
@@ -99,7 +100,7 @@ def test_copper_small_full_parity(variant):
     m.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("chunk", [1, 7, 100000])
 def test_chunking_does_not_change_results(variant, chunk):
     """Atom chunking (the memory bound for the 864k-atom config) must give the same result for any chunk size,
@@ -116,7 +117,7 @@ def test_chunking_does_not_change_results(variant, chunk):
     m.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_tiny_model_three_types_random_box(variant):
     """A small 3-species model with odd widths (s1 = 5, M^< = 3, width 9) on a random box with unsorted types:
     exercises padding of every tile dimension and ntypes^2 = 9 embedding nets (Remark 1)."""
@@ -133,7 +134,7 @@ def test_tiny_model_three_types_random_box(variant):
     m.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_neighbour_overflow_keeps_nearest(variant):
     """Reading R8: more neighbours than sel[t] -> the nearest sel[t] are kept and the drops are counted."""
     spec, emb, fit = small_model(ntypes=2, s1=4, m_axis=3, fit_width=8, sel=(3, 4), rcut=4.0, rcut_smth=1.0, seed=3)
