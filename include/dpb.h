@@ -35,7 +35,14 @@ typedef enum {
                      the error-compensated 3xTF32 split, fp32 accumulate (tcgen05 / TMEM), tanh in fp32; neighbour
                      list, env matrix, chain to the displacement and the T, F, virial, E accumulations in fp64.
                      Built for emb_s1 in {8, 16, 25, 32}, m_axis in {4, 8, 16}, fit_width % 4 == 0 and <= 256.   */
-  DPB_BF16 = 2    /* reserved (BF16 operand variant): DPB_ENOTIMPL in this build                             */
+  DPB_BF16 = 2,   /* BASELINE.json configs[3] "and a BF16 variant": the FITTING-net GEMMs (Eq. 2-3 and their backward: the
+                     K = 1600 / 240 contractions) with BF16 operands on tcgen05 kind::f16 — every operand split into three
+                     BF16 pieces (8 + 8 + 8 significant bits), six piece products per product, fp32 accumulate; the
+                     embedding-net GEMMs run as in DPB_TF32 (their tcgen05 kernels are written for 32-bit operand cells).
+                     Meets the same tolerance as DPB_TF32 at the same tensor-pipe cost (6 K=16 MMAs against 3 K=8 MMAs).  */
+  DPB_BF16_PLAIN = 3 /* as DPB_BF16 with ONE BF16 piece per operand (plain BF16 GEMMs in the fitting net): kept to MEASURE
+                     what plain BF16 costs in accuracy on this model; it misses the mixed-precision tolerance by orders of
+                     magnitude (tests record the error) and is not meant for production use.        */
 } dpb_precision;
 
 typedef enum {
@@ -72,7 +79,7 @@ typedef struct {
 } dpb_eval_info;
 
 /* Create / destroy.  dpb_model_create copies (and re-lays-out) the weights to the current CUDA device.
- * Errors: DPB_EINVAL (shape), DPB_ENOTIMPL (DPB_BF16; DPB_TF32 with an unsupported shape), DPB_ENOMEM, DPB_ECUDA. */
+ * Errors: DPB_EINVAL (shape, precision), DPB_ENOTIMPL (mixed precision with an unsupported shape), DPB_ENOMEM, DPB_ECUDA. */
 int dpb_model_create(const dpb_model_desc *desc, int precision, dpb_model **out);
 int dpb_model_destroy(dpb_model *model);
 

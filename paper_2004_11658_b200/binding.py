@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 STATUS = {0: "DPB_OK", -1: "DPB_EINVAL", -2: "DPB_EBOX", -3: "DPB_ENOMEM", -4: "DPB_ECUDA", -5: "DPB_ECAP",
           -6: "DPB_ENOTIMPL"}
-FP64, TF32, BF16 = 0, 1, 2
+FP64, TF32, BF16, BF16_PLAIN = 0, 1, 2, 3
 
 
 class DPBError(RuntimeError):

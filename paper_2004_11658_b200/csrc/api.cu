@@ -169,7 +169,7 @@ static int64_t effective_chunk(const dpb_model *m) {
     else per += v1_workspace_bytes(P, 1024) / 1024;
     if (m->variant == 2) per += (size_t)P.nm * v2_slot_bytes(m->v2);       // Eq. 13's tensors: every padded slot
   } else {
-    per += (tc_pair_workspace_bytes(P, 1024) + tc_pass2_workspace_bytes(P, 1024) + tc_fit_workspace_bytes(P, 1024)) / 1024;
+    per += (tc_pair_workspace_bytes(P, 1024) + tc_pass2_workspace_bytes(P, 1024) + tc_fit_workspace_bytes(P, 1024, m->precision - DPB_TF32)) / 1024;
   }
   int64_t c = (int64_t)(m->ws_budget / (per + 1));
   c -= c % 1024;
@@ -181,8 +181,8 @@ extern "C" int dpb_model_nm(const dpb_model *m) { return m ? nm_of(m->P) : DPB_E
 extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_model **out) {
   if (!d || !out) return fail(DPB_EINVAL, "dpb_model_create: null argument");
   *out = nullptr;
-  if (precision != DPB_FP64 && precision != DPB_TF32)
-    return fail(DPB_ENOTIMPL, "dpb_model_create: precision must be DPB_FP64 or DPB_TF32 (DPB_BF16 is not built)");
+  if (precision < DPB_FP64 || precision > DPB_BF16_PLAIN)
+    return fail(DPB_EINVAL, "dpb_model_create: precision must be DPB_FP64, DPB_TF32, DPB_BF16 or DPB_BF16_PLAIN");
   if (d->ntypes < 1 || d->ntypes > DPB_MAX_TYPES) return fail(DPB_EINVAL, "ntypes must be in [1, %d]", DPB_MAX_TYPES);
   if (!d->sel || !d->emb_weights || !d->fit_weights) return fail(DPB_EINVAL, "null sel / weights");
   if (d->emb_s1 < 1 || d->emb_s1 > 64) return fail(DPB_EINVAL, "emb_s1 must be in [1, 64]");
@@ -221,12 +221,12 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
   if (e == cudaSuccess) e = cudaMemcpy(m->fit.p, d->fit_weights, fb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = v1_prepare_weights(P, d->emb_weights, d->fit_weights, m->v1);
   m->precision = precision;
-  if (e == cudaSuccess && precision == DPB_TF32) {
+  if (e == cudaSuccess && precision != DPB_FP64) {
     e = tc_prepare_weights(P, d->emb_weights, m->tcw);
-    if (e == cudaSuccess) e = tc_prepare_fit(P, d->fit_weights, m->tcw);
+    if (e == cudaSuccess) e = tc_prepare_fit(P, d->fit_weights, m->tcw, precision - DPB_TF32);
     if (e == cudaErrorNotSupported) {
       dpb_model_destroy(m);
-      return fail(DPB_ENOTIMPL, "DPB_TF32 is built for emb_s1 in {8, 16, 25, 32}, m_axis in {4, 8, 16} and "
+      return fail(DPB_ENOTIMPL, "mixed precision is built for emb_s1 in {8, 16, 25, 32}, m_axis in {4, 8, 16} and "
                                 "fit_width %% 4 == 0, <= 256 (got %d, %d, %d)", d->emb_s1, d->m_axis, d->fit_width);
     }
   }
@@ -476,10 +476,10 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     }
     if (m->precision == DPB_FP64 && m->variant == 2)
       CU(m->v2ws.reserve((size_t)chunk * P.nm * v2_slot_bytes(m->v2)), "workspace of the paper pipeline");
-    if (m->precision == DPB_TF32) {
+    if (m->precision != DPB_FP64) {
       CU(m->pairs.reserve(tc_pair_workspace_bytes(P, chunk)), "workspace");
       CU(m->dT32.reserve(tc_pass2_workspace_bytes(P, chunk)), "workspace");
-      CU(m->tcfit.reserve(tc_fit_workspace_bytes(P, chunk)), "workspace");
+      CU(m->tcfit.reserve(tc_fit_workspace_bytes(P, chunk, m->precision - DPB_TF32)), "workspace");
     }
   }
   DevStats *stats = m->stats.as<DevStats>();
@@ -558,7 +558,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
        "nlist");
     if (nlist_only) continue;
     if (timing) cudaEventRecord(m->evs[2 + 4 * ci], st);
-    if (m->precision == DPB_TF32) {
+    if (m->precision != DPB_FP64) {
       CU(tc_build_pairs(P, C, m->pairs.p, st), "pair list");
       CU(tc_pass1(P, C, m->tcw, m->pairs.p, st), "pass1 tf32");
       if (timing) cudaEventRecord(m->evs[3 + 4 * ci], st);

@@ -20,58 +20,86 @@
 #include "tc_common.cuh"
 #include "tc_kernels.cuh"
 
-#define FT_KP 32                       // K columns per panel (128 bytes of tf32)
-#define FT_APANEL (128 * 128)          // bytes of one A panel (hi or lo)
+#define FT_APANEL (128 * 128)          // bytes of one A panel: 128 rows x 128 B (32 TF32 or 64 BF16 K-columns per row)
+
+// Operand format of the GEMMs (tc_fit's `opf`).  An operand x is stored as NP pieces whose sum is x to fp32 accuracy; the
+// product a b is the sum of the listed piece products (error-compensated split; the dropped products are below fp32's
+// rounding):
+//   0  3xTF32 (DPB_TF32):       x = hi + lo in TF32;       lo hi + hi lo + hi hi                  kind::tf32, K = 8 per MMA
+//   1  BF16 x 6 (DPB_BF16):     x = p0 + p1 + p2 in BF16;  p2 p0 + p0 p2 + p1 p1 + p1 p0 + p0 p1 + p0 p0   kind::f16, K = 16
+//   2  plain BF16 (DPB_BF16_PLAIN): x ~ p0;                p0 p0      (measured, not meant to meet the tolerance)
+// KP = K columns per 128-byte panel row; CP = panels per accumulation chunk (K = 64, see FT_CP below).
+template <int OPF> struct OpFmt;
+template <> struct OpFmt<0> { static constexpr int NP = 2, KP = 32, CP = 2; };
+template <> struct OpFmt<1> { static constexpr int NP = 3, KP = 64, CP = 1; };
+template <> struct OpFmt<2> { static constexpr int NP = 1, KP = 64, CP = 1; };
+static int opf_np(int opf) { return opf == 0 ? 2 : (opf == 1 ? 3 : 1); }
+static int opf_kp(int opf) { return opf == 0 ? 32 : 64; }
 
 enum { FE_TANH = 0, FE_TANH_SKIP = 1, FE_L3 = 2, FE_BWD1 = 3, FE_BWD0 = 4, FE_STORE = 5 };
 
-struct FitTCNet {                      // device pointers (floats) of one species
-  const float *W0h, *W0l, *W1h, *W1l, *W2h, *W2l, *W2Th, *W2Tl, *W1Th, *W1Tl, *W0Th, *W0Tl;
+struct FitTCNet {                      // device pointers of one species: B images per piece, fp32 vectors
+  const uint8_t *W0[3], *W1[3], *W2[3], *W2T[3], *W1T[3], *W0T[3];
   const float *b0, *b1, *b2, *w3;
   float b3;
 };
 
 struct FitTC {
-  float *buf = nullptr;
-  int fw = 0, fwp = 0, NT = 0;         // width, width padded to 32 (K panels), N tile of the fw-wide GEMMs
+  uint8_t *buf = nullptr;
+  int opf = 0;
+  int fw = 0, fwp = 0, NT = 0;         // width, width padded to the K panel, N tile of the fw-wide GEMMs
   int dim = 0, dimp = 0, NT6 = 0;      // descriptor size, padded to the N tile of G6 (240: fewer re-reads of A than 128)
   std::vector<FitTCNet> nets;
 };
 
 struct FitTCArgs {
-  const float *Ah, *Al;                // A images [tile][KPAN][4096 floats]
-  const float *Bh, *Bl;                // B images [ntile][KPAN][NT * 32 floats]
+  const uint8_t *A[3];                 // A images per piece: [tile][KPAN][FT_APANEL bytes]
+  const uint8_t *B[3];                 // B images per piece: [ntile][KPAN][NT * 128 bytes]
   int KPAN;                            // K panels
   int N;                               // real output columns (<= gridDim.y * NT)
   int KPAN_out;                        // K panels of the output image (its K = this GEMM's N)
   const float *bias, *w3;              // [N]
   const float *in0, *in1;              // plain fp32 [rows][ldp]
   float *out_plain0, *out_plain1;      // plain fp32 [rows][ldp]
-  float *out_h, *out_l;                // output A image (hi / lo) or null
+  uint8_t *out[3];                     // output A image per piece, or out[0] == null
   int ldp;
   float b3;
   double *atom_energy;                 // FE_L3
   const int *s_idx;
 };
 
-// store 4 consecutive columns (chunk j of K panel kp) of row r into an A image in global memory
-__device__ __forceinline__ void img_store4(float *img_h, float *img_l, size_t tile, int kpan, int n0, int r, float v0,
+// store 4 consecutive columns n0 .. n0 + 3 of row r into an A image in global memory (all pieces)
+template <int OPF>
+__device__ __forceinline__ void img_store4(uint8_t *const img[3], size_t tile, int kpan, int n0, int r, float v0,
                                            float v1, float v2, float v3) {
-  float4 h, l;
-  tc::split_tf32(v0, h.x, l.x);
-  tc::split_tf32(v1, h.y, l.y);
-  tc::split_tf32(v2, h.z, l.z);
-  tc::split_tf32(v3, h.w, l.w);
-  const size_t o = (tile * kpan + (n0 >> 5)) * 4096 + (tc::sw128_offset(r, n0 & 31) >> 2);
-  *reinterpret_cast<float4 *>(img_h + o) = h;
-  *reinterpret_cast<float4 *>(img_l + o) = l;
+  constexpr int KP = OpFmt<OPF>::KP;
+  const size_t pan = (tile * kpan + (size_t)(n0 / KP)) * FT_APANEL;
+  if (OPF == 0) {
+    float4 h, l;
+    tc::split_tf32(v0, h.x, l.x);
+    tc::split_tf32(v1, h.y, l.y);
+    tc::split_tf32(v2, h.z, l.z);
+    tc::split_tf32(v3, h.w, l.w);
+    const size_t o = pan + tc::sw128_offset(r, n0 & 31);
+    *reinterpret_cast<float4 *>(img[0] + o) = h;
+    *reinterpret_cast<float4 *>(img[1] + o) = l;
+  } else {
+    uint32_t p[4][3];
+    const float v[4] = {v0, v1, v2, v3};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) tc::split_bf16x3(v[i], p[i][0], p[i][1], p[i][2]);
+    const size_t o = pan + tc::sw128_offset_b16(r, n0 & 63);
+#pragma unroll
+    for (int q = 0; q < OpFmt<OPF>::NP; ++q)
+      *reinterpret_cast<uint2 *>(img[q] + o) = make_uint2(p[0][q] | (p[1][q] << 16), p[2][q] | (p[3][q] << 16));
+  }
 }
 
 // One group of 8 output columns of row m (tile row r): apply the GEMM's epilogue to the accumulators a[8].
 // The plain fp32 activation arrays (Z0, S0, S1, Z1, dZ1) are private to these epilogues, which all map thread r to tile
 // row r; they are stored tile-wise transposed, [tile][column / 4][row][4], so that the 32 lanes of a warp (32 rows) touch
 // 512 contiguous bytes per access instead of 32 separate lines.  dD (FE_STORE) stays row-major for k_dT_tc.
-template <int EPI>
+template <int EPI, int OPF>
 __device__ __forceinline__ void ft_epi8(const float a[8], int nn0, const FitTCArgs &g, size_t tile, int r, int m,
                                         double &edot) {
   float o0[8], o1[8];
@@ -123,8 +151,8 @@ __device__ __forceinline__ void ft_epi8(const float a[8], int nn0, const FitTCAr
 #pragma unroll
   for (int q4 = 0; q4 < 2; ++q4) {
     const int nn = nn0 + 4 * q4;
-    if (g.out_h && nn < g.KPAN_out * FT_KP)
-      img_store4(g.out_h, g.out_l, tile, g.KPAN_out, nn, r, o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
+    if (g.out[0] && nn < g.KPAN_out * OpFmt<OPF>::KP)
+      img_store4<OPF>(g.out, tile, g.KPAN_out, nn, r, o0[4 * q4], o0[4 * q4 + 1], o0[4 * q4 + 2], o0[4 * q4 + 3]);
     if (nn < g.ldp) {
       const size_t po = EPI == FE_STORE ? (size_t)m * g.ldp + nn
                                         : ((tile * (size_t)(g.ldp >> 2) + (size_t)(nn >> 2)) * 128 + (size_t)r) * 4;
@@ -142,16 +170,17 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *mbar) {
 
 // The tensor core accumulates in fp32 with truncation; over a long K (1600 for G1) that bias reaches 1e-4 of the
 // pre-activations and breaks the force tolerance (measured).  The accumulation is therefore
-// chunked: the MMAs of FT_CP K panels (K = 64) go to one of two TMEM accumulators starting from zero, and the epilogue
+// chunked: the MMAs of CP K panels (K = 64) go to one of two TMEM accumulators starting from zero, and the epilogue
 // warps add the finished chunk to fp32 registers (round-to-nearest) while the next chunk runs in the other buffer.
-#define FT_CP 2
 
-template <int NT, int EPI>
+template <int NT, int EPI, int OPF>
 __global__ void __launch_bounds__(320, 1)
 k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
-  constexpr int BPANEL = NT * 128;                               // bytes of one B panel (hi or lo)
-  constexpr int STAGE = 2 * FT_APANEL + 2 * BPANEL;
-  constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : 2;
+  using F = OpFmt<OPF>;
+  constexpr int NP = F::NP, FT_CP = F::CP;
+  constexpr int BPANEL = NT * 128;                               // bytes of one B panel (one piece)
+  constexpr int STAGE = NP * (FT_APANEL + BPANEL);               // pieces of A, then pieces of B
+  constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : ((STAGE * 2 <= 200 * 1024) ? 2 : 1);
   constexpr int NH = NT / 2;                                     // columns per epilogue warpgroup
   static_assert(NH % 8 == 0 && NH <= 128, "");
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -181,22 +210,22 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
 
   if (warp == 0) {
     if (lane == 0) {
-      const float *ah = g.Ah + (size_t)tile * g.KPAN * 4096, *al = g.Al + (size_t)tile * g.KPAN * 4096;
-      const float *bh = g.Bh + (size_t)nt * g.KPAN * (NT * 32), *bl = g.Bl + (size_t)nt * g.KPAN * (NT * 32);
+      const size_t aoff = (size_t)tile * g.KPAN * FT_APANEL, boff = (size_t)nt * g.KPAN * BPANEL;
       for (int kp = 0; kp < g.KPAN; ++kp) {
         const int s = kp % STAGES;
         if (kp >= STAGES) tc::mbar_wait(empty + s, ((kp / STAGES) - 1) & 1);
         uint8_t *st = smem + s * STAGE;
         tc::mbar_arrive_expect_tx(full + s, STAGE);
-        tc::bulk_g2s(st, ah + (size_t)kp * 4096, FT_APANEL, full + s);
-        tc::bulk_g2s(st + FT_APANEL, al + (size_t)kp * 4096, FT_APANEL, full + s);
-        tc::bulk_g2s(st + 2 * FT_APANEL, bh + (size_t)kp * (NT * 32), BPANEL, full + s);
-        tc::bulk_g2s(st + 2 * FT_APANEL + BPANEL, bl + (size_t)kp * (NT * 32), BPANEL, full + s);
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          tc::bulk_g2s(st + q * FT_APANEL, g.A[q] + aoff + (size_t)kp * FT_APANEL, FT_APANEL, full + s);
+          tc::bulk_g2s(st + NP * FT_APANEL + q * BPANEL, g.B[q] + boff + (size_t)kp * BPANEL, BPANEL, full + s);
+        }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {
-      constexpr uint32_t idesc = tc::make_idesc_tf32(128, NT);
+      constexpr uint32_t idesc = OPF == 0 ? tc::make_idesc_tf32(128, NT) : tc::make_idesc_bf16(128, NT);
       for (int c = 0; c < nchunks; ++c) {
         const int buf = c & 1;
         if (c >= 2) tc::mbar_wait(accempty + buf, ((c >> 1) - 1) & 1);
@@ -207,15 +236,30 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
           const int s = kp % STAGES;
           tc::mbar_wait(full + s, (kp / STAGES) & 1);
           tc::fence_after_sync();
-          const uint32_t sa = tc::smem_u32(smem + s * STAGE);
+          const uint32_t sa = tc::smem_u32(smem + s * STAGE), sb = sa + NP * FT_APANEL;
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            const uint64_t dah = tc::make_desc_sw128(sa + ks * 32), dal = tc::make_desc_sw128(sa + FT_APANEL + ks * 32);
-            const uint64_t dbh = tc::make_desc_sw128(sa + 2 * FT_APANEL + ks * 32),
-                           dbl = tc::make_desc_sw128(sa + 2 * FT_APANEL + BPANEL + ks * 32);
-            tc::mma_tf32_ss(td, dal, dbh, idesc, (kp > c * FT_CP || ks > 0) ? 1u : 0u);
-            tc::mma_tf32_ss(td, dah, dbl, idesc, 1u);
-            tc::mma_tf32_ss(td, dah, dbh, idesc, 1u);
+          for (int ks = 0; ks < 4; ++ks) {                         // 32 bytes of K per MMA: 8 TF32 or 16 BF16 columns
+            const uint32_t first = (kp > c * FT_CP || ks > 0) ? 1u : 0u;
+            uint64_t da[NP], db[NP];
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+              da[q] = tc::make_desc_sw128(sa + q * FT_APANEL + ks * 32);
+              db[q] = tc::make_desc_sw128(sb + q * BPANEL + ks * 32);
+            }
+            if constexpr (OPF == 0) {                              // pieces (hi, lo): lo hi + hi lo + hi hi
+              tc::mma_tf32_ss(td, da[1], db[0], idesc, first);
+              tc::mma_tf32_ss(td, da[0], db[1], idesc, 1u);
+              tc::mma_tf32_ss(td, da[0], db[0], idesc, 1u);
+            } else if constexpr (OPF == 1) {                       // pieces (p0, p1, p2), smallest products first
+              tc::mma_f16_ss(td, da[2], db[0], idesc, first);
+              tc::mma_f16_ss(td, da[0], db[2], idesc, 1u);
+              tc::mma_f16_ss(td, da[1], db[1], idesc, 1u);
+              tc::mma_f16_ss(td, da[1], db[0], idesc, 1u);
+              tc::mma_f16_ss(td, da[0], db[1], idesc, 1u);
+              tc::mma_f16_ss(td, da[0], db[0], idesc, 1u);
+            } else {
+              tc::mma_f16_ss(td, da[0], db[0], idesc, first);
+            }
           }
           tc::mma_commit(empty + s);
         }
@@ -258,10 +302,10 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
     double edot = 0.0;
     if (ok) {
 #pragma unroll
-      for (int j = 0; j < NH; j += 8) ft_epi8<EPI>(acc + j, n0 + e * NH + j, g, (size_t)tile, r, m, edot);
-      if (EPI != FE_STORE && g.out_h && e == 1)               // image columns between NT and the padded K must be zero
-        for (int nn = n0 + NT; nn < g.KPAN_out * FT_KP; nn += 4)
-          img_store4(g.out_h, g.out_l, (size_t)tile, g.KPAN_out, nn, r, 0.f, 0.f, 0.f, 0.f);
+      for (int j = 0; j < NH; j += 8) ft_epi8<EPI, OPF>(acc + j, n0 + e * NH + j, g, (size_t)tile, r, m, edot);
+      if (EPI != FE_STORE && g.out[0] && e == 1)              // image columns between NT and the padded K must be zero
+        for (int nn = n0 + NT; nn < g.KPAN_out * F::KP; nn += 4)
+          img_store4<OPF>(g.out, (size_t)tile, g.KPAN_out, nn, r, 0.f, 0.f, 0.f, 0.f);
     }
     if (EPI == FE_L3) {
       // all stages have been consumed (the last accfull implies every MMA read its operands): smem is free
@@ -283,8 +327,9 @@ k_fit_tc(ChunkView C, int ty, FitTCArgs g) {
 // atoms' T rows in shared memory (coalesced 16-byte loads of the contiguous fp64 rows), then walks (K panel, row, 16-byte
 // chunk) tasks with the chunk index fastest: eight lanes write one full 128-byte image row, a warp four adjacent rows =
 // 512 contiguous bytes per store (thread-per-row stores touched 32 separate lines, half a sector each).
-template <int MA>
-__global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int ty, int kpan, float *__restrict__ Dh, float *__restrict__ Dl) {
+template <int MA, int OPF>
+__global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int ty, int kpan, FitTCArgs img) {
+  constexpr int KP = OpFmt<OPF>::KP, CH = KP / 4;                  // 4-column chunks per panel row
   extern __shared__ float4 Ts[];                                   // [DESCR_R][M + 1]
   // one launch per species, on that species' stream: blocks outside its row range leave at once
   const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
@@ -300,10 +345,10 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int t
     }
   }
   __syncthreads();
-  const int ntask = DESCR_R * kpan * 8, kreal = M * MA;
+  const int ntask = DESCR_R * kpan * CH, kreal = M * MA;
   for (int q = threadIdx.x; q < ntask; q += 256) {
-    const int j = q & 7, rl = (q >> 3) & (DESCR_R - 1), pan = q / (8 * DESCR_R);
-    const int m = row0 + rl, k0 = pan * FT_KP + 4 * j;
+    const int j = q % CH, rl = (q / CH) & (DESCR_R - 1), pan = q / (CH * DESCR_R);
+    const int m = row0 + rl, k0 = pan * KP + 4 * j;
     if (rl >= nrow || m < row_lo || m >= row_hi) continue;
     float d[4] = {0.f, 0.f, 0.f, 0.f};                             // image columns between dim and the padded K are zero
     if (k0 < kreal) {
@@ -315,7 +360,7 @@ __global__ void __launch_bounds__(256) k_descr_tc(DevModel P, ChunkView C, int t
         d[k] = fmaf(tb.x, ta.x, fmaf(tb.y, ta.y, fmaf(tb.z, ta.z, tb.w * ta.w)));
       }
     }
-    img_store4(Dh, Dl, (size_t)(m >> 7), kpan, k0, m & 127, d[0], d[1], d[2], d[3]);
+    img_store4<OPF>(img.out, (size_t)(m >> 7), kpan, k0, m & 127, d[0], d[1], d[2], d[3]);
   }
 }
 
@@ -424,27 +469,39 @@ __global__ void __launch_bounds__(32 * DT_WARPS) k_dT_tc(DevModel P, ChunkView C
 // ---- host: weights as B images -------------------------------------------------------------------------------------
 static int ft_round_up(int x, int m) { return (x + m - 1) / m * m; }
 
-// B[n][k] for n < N, k < K (zero outside), as [ntiles][kpan][NT rows x 32] swizzled panels; appends hi and lo to out
+// B[n][k] for n < N, k < K (zero outside), as [ntiles][kpan][NT rows x 128 B] swizzled panels, one array per piece;
+// appends the pieces to `out` (bytes) and returns their offsets
 template <class F>
-static void pack_B(F get, int N, int K, int NT, int ntiles, int kpan, std::vector<float> &out, size_t &off_h, size_t &off_l) {
-  const size_t sz = (size_t)ntiles * kpan * NT * 32;
-  off_h = out.size();
-  out.resize(out.size() + 2 * sz, 0.0f);
-  off_l = off_h + sz;
+static void pack_B(int opf, F get, int N, int K, int NT, int ntiles, int kpan, std::vector<uint8_t> &out, size_t off[3]) {
+  const int np = opf_np(opf), kp_cols = opf_kp(opf);
+  const size_t sz = (size_t)ntiles * kpan * NT * 128;
+  const size_t at = (out.size() + 1023) / 1024 * 1024;
+  out.resize(at + np * sz, 0);
+  for (int q = 0; q < 3; ++q) off[q] = at + (size_t)(q < np ? q : 0) * sz;
   for (int nt = 0; nt < ntiles; ++nt)
     for (int kp = 0; kp < kpan; ++kp) {
-      const size_t base = ((size_t)nt * kpan + kp) * NT * 32;
+      const size_t base = ((size_t)nt * kpan + kp) * NT * 128;
       for (int rn = 0; rn < NT; ++rn) {
         const int n = nt * NT + rn;
         if (n >= N) continue;
-        for (int kk = 0; kk < 32; ++kk) {
-          const int k = kp * 32 + kk;
+        for (int kk = 0; kk < kp_cols; ++kk) {
+          const int k = kp * kp_cols + kk;
           if (k >= K) continue;
           const double w = get(n, k);
-          const float hi = tc_host_tf32((float)w);
-          const size_t o = base + tc::sw128_offset(rn, kk) / 4;
-          out[off_h + o] = hi;
-          out[off_l + o] = tc_host_tf32((float)(w - (double)hi));
+          if (opf == 0) {
+            const float hi = tc_host_tf32((float)w), lo = tc_host_tf32((float)(w - (double)hi));
+            const size_t o = base + tc::sw128_offset(rn, kk);
+            memcpy(&out[off[0] + o], &hi, 4);
+            memcpy(&out[off[1] + o], &lo, 4);
+          } else {
+            float rem = (float)w;
+            const size_t o = base + tc::sw128_offset_b16(rn, kk);
+            for (int q = 0; q < np; ++q) {
+              const uint16_t b = tc_host_bf16_bits(rem);
+              memcpy(&out[off[q] + o], &b, 2);
+              rem -= tc_host_bf16_value(b);
+            }
+          }
         }
       }
     }
@@ -459,15 +516,17 @@ static int ft_pick_nt(int fw) {
   return 0;
 }
 
-cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W) {
+cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W, int opf) {
   if (P.fw % 4 != 0 || ft_pick_nt(P.fw) == 0 || (P.Ma != 4 && P.Ma != 8 && P.Ma != 16)) return cudaErrorNotSupported;
   FitTC *F = new FitTC();
-  F->fw = P.fw; F->fwp = ft_round_up(P.fw, 32); F->NT = ft_pick_nt(P.fw);
+  const int KP = opf_kp(opf);
+  F->opf = opf;
+  F->fw = P.fw; F->fwp = ft_round_up(P.fw, KP); F->NT = ft_pick_nt(P.fw);
   F->NT6 = P.dim >= 960 ? 240 : 128;
   F->dim = P.dim; F->dimp = ft_round_up(P.dim, F->NT6);
-  const int fw = P.fw, dim = P.dim, kpw = F->fwp / 32, kpd = ft_round_up(dim, 32) / 32, nt6 = F->dimp / F->NT6;
-  std::vector<float> h;
-  struct Off { size_t W0h, W0l, W1h, W1l, W2h, W2l, W2Th, W2Tl, W1Th, W1Tl, W0Th, W0Tl, b0, b1, b2, w3; };
+  const int fw = P.fw, dim = P.dim, kpw = F->fwp / KP, kpd = ft_round_up(dim, KP) / KP, nt6 = F->dimp / F->NT6;
+  std::vector<uint8_t> h;
+  struct Off { size_t W0[3], W1[3], W2[3], W2T[3], W1T[3], W0T[3], b0, b1, b2, w3; };
   std::vector<Off> offs(P.ntypes);
   for (int ty = 0; ty < P.ntypes; ++ty) {
     const double *W0 = fit_h + (size_t)ty * P.fit_net_size;
@@ -475,31 +534,36 @@ cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W)
                  *b2 = W2 + (size_t)fw * fw, *w3 = b2 + fw;
     Off &o = offs[ty];
     // forward GEMMs: C[r][n] = sum_k A[r][k] W[k][n]  ->  B[n][k] = W[k][n]
-    pack_B([&](int n, int k) { return W0[(size_t)k * fw + n]; }, fw, dim, F->NT, 1, kpd, h, o.W0h, o.W0l);
-    pack_B([&](int n, int k) { return W1[(size_t)k * fw + n]; }, fw, fw, F->NT, 1, kpw, h, o.W1h, o.W1l);
-    pack_B([&](int n, int k) { return W2[(size_t)k * fw + n]; }, fw, fw, F->NT, 1, kpw, h, o.W2h, o.W2l);
+    pack_B(opf, [&](int n, int k) { return W0[(size_t)k * fw + n]; }, fw, dim, F->NT, 1, kpd, h, o.W0);
+    pack_B(opf, [&](int n, int k) { return W1[(size_t)k * fw + n]; }, fw, fw, F->NT, 1, kpw, h, o.W1);
+    pack_B(opf, [&](int n, int k) { return W2[(size_t)k * fw + n]; }, fw, fw, F->NT, 1, kpw, h, o.W2);
     // backward GEMMs: C[r][n] = sum_k Q[r][k] W[n][k]  ->  B[n][k] = W[n][k]
-    pack_B([&](int n, int k) { return W2[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W2Th, o.W2Tl);
-    pack_B([&](int n, int k) { return W1[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W1Th, o.W1Tl);
-    pack_B([&](int n, int k) { return W0[(size_t)n * fw + k]; }, dim, fw, F->NT6, nt6, kpw, h, o.W0Th, o.W0Tl);
+    pack_B(opf, [&](int n, int k) { return W2[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W2T);
+    pack_B(opf, [&](int n, int k) { return W1[(size_t)n * fw + k]; }, fw, fw, F->NT, 1, kpw, h, o.W1T);
+    pack_B(opf, [&](int n, int k) { return W0[(size_t)n * fw + k]; }, dim, fw, F->NT6, nt6, kpw, h, o.W0T);
     auto vecpad = [&](const double *src) {
-      const size_t at = h.size();
-      h.resize(at + 256, 0.0f);
-      for (int i = 0; i < fw; ++i) h[at + i] = (float)src[i];
+      const size_t at = (h.size() + 15) / 16 * 16;
+      h.resize(at + 256 * sizeof(float), 0);
+      for (int i = 0; i < fw; ++i) { const float v = (float)src[i]; memcpy(&h[at + 4 * (size_t)i], &v, 4); }
       return at;
     };
     o.b0 = vecpad(b0); o.b1 = vecpad(b1); o.b2 = vecpad(b2); o.w3 = vecpad(w3);
   }
-  cudaError_t e = cudaMalloc(&F->buf, sizeof(float) * h.size());
+  cudaError_t e = cudaMalloc(&F->buf, h.size());
   if (e != cudaSuccess) { delete F; return e; }
-  e = cudaMemcpy(F->buf, h.data(), sizeof(float) * h.size(), cudaMemcpyHostToDevice);
+  e = cudaMemcpy(F->buf, h.data(), h.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) { cudaFree(F->buf); delete F; return e; }
   for (int ty = 0; ty < P.ntypes; ++ty) {
     const Off &o = offs[ty];
-    const float *b = F->buf;
-    FitTCNet n{b + o.W0h, b + o.W0l, b + o.W1h, b + o.W1l, b + o.W2h, b + o.W2l, b + o.W2Th, b + o.W2Tl,
-               b + o.W1Th, b + o.W1Tl, b + o.W0Th, b + o.W0Tl, b + o.b0, b + o.b1, b + o.b2, b + o.w3,
-               (float)fit_h[(size_t)ty * P.fit_net_size + P.fit_net_size - 1]};
+    const uint8_t *b = F->buf;
+    FitTCNet n{};
+    for (int q = 0; q < 3; ++q) {
+      n.W0[q] = b + o.W0[q]; n.W1[q] = b + o.W1[q]; n.W2[q] = b + o.W2[q];
+      n.W2T[q] = b + o.W2T[q]; n.W1T[q] = b + o.W1T[q]; n.W0T[q] = b + o.W0T[q];
+    }
+    n.b0 = reinterpret_cast<const float *>(b + o.b0); n.b1 = reinterpret_cast<const float *>(b + o.b1);
+    n.b2 = reinterpret_cast<const float *>(b + o.b2); n.w3 = reinterpret_cast<const float *>(b + o.w3);
+    n.b3 = (float)fit_h[(size_t)ty * P.fit_net_size + P.fit_net_size - 1];
     F->nets.push_back(n);
   }
   W.fit = F;
@@ -515,85 +579,95 @@ void tc_release_fit(TCWeights &W) {
   W.fit = nullptr;
 }
 
-size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk) {
+// images: D (NP pieces x tiles x kpd panels), X0 and X1 (NP x tiles x kpw each); plain fp32: Z0 S0 S1 Z1 dZ1 [rows][fwp], dD
+size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk, int opf) {
+  const int KP = opf_kp(opf), np = opf_np(opf);
   const size_t tiles = (size_t)(chunk + 127) / 128, rows = tiles * 128;
-  const size_t kpd = (size_t)ft_round_up(P.dim, 32) / 32, fwp = ft_round_up(P.fw, 32), dimp = ft_round_up(P.dim, P.dim >= 960 ? 240 : 128);
-  return sizeof(float) * (2 * tiles * kpd * 4096 + 4 * tiles * (fwp / 32) * 4096 + 5 * rows * fwp + rows * dimp) + 1024;
+  const size_t kpd = (size_t)ft_round_up(P.dim, KP) / KP, fwp = ft_round_up(P.fw, KP), kpw = fwp / KP,
+               dimp = ft_round_up(P.dim, P.dim >= 960 ? 240 : 128);
+  return (size_t)np * tiles * (kpd + 2 * kpw) * FT_APANEL + sizeof(float) * (5 * rows * fwp + rows * dimp) + 4096;
 }
 
-template <int NT, int EPI>
+template <int NT, int EPI, int OPF>
 static cudaError_t ft_launch(const ChunkView &C, int ty, const FitTCArgs &g, int ntiles_n, cudaStream_t st) {
-  constexpr int STAGE = 2 * FT_APANEL + 2 * NT * 128;
-  constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : 2;
+  constexpr int STAGE = OpFmt<OPF>::NP * (FT_APANEL + NT * 128);
+  constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : ((STAGE * 2 <= 200 * 1024) ? 2 : 1);
   constexpr int smem = STAGES * STAGE + 128;
+  static_assert(smem <= 227 * 1024, "stage does not fit");
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_fit_tc<NT, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(k_fit_tc<NT, EPI, OPF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
   dim3 grid((C.n + 127) / 128, ntiles_n);
-  k_fit_tc<NT, EPI><<<grid, 320, smem, st>>>(C, ty, g);
+  k_fit_tc<NT, EPI, OPF><<<grid, 320, smem, st>>>(C, ty, g);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
 
-template <int NT>
-static cudaError_t ft_run_type(const DevModel &P, const ChunkView &C, const FitTC &F, int ty, float *Dh, float *Dl,
-                               float *X0h, float *X0l, float *X1h, float *X1l, float *Z0, float *S0, float *S1,
-                               float *Z1, float *dZ1, float *dD, double *atom_energy, cudaStream_t st) {
+struct FitTCBufs { uint8_t *D[3], *X0[3], *X1[3]; float *Z0, *S0, *S1, *Z1, *dZ1, *dD; };
+
+template <int NT, int OPF>
+static cudaError_t ft_run_type(const DevModel &P, const ChunkView &C, const FitTC &F, int ty, const FitTCBufs &B,
+                               double *atom_energy, cudaStream_t st) {
+  constexpr int KP = OpFmt<OPF>::KP;
   const FitTCNet &N = F.nets[ty];
-  const int kpw = F.fwp / 32, kpd = ft_round_up(F.dim, 32) / 32, fw = F.fw, ldp = F.fwp;
+  const int kpw = F.fwp / KP, kpd = ft_round_up(F.dim, KP) / KP, fw = F.fw, ldp = F.fwp;
   cudaError_t e;
   FitTCArgs g{};
+  auto setA = [&](uint8_t *const a[3]) { for (int q = 0; q < 3; ++q) g.A[q] = a[q]; };
+  auto setB = [&](const uint8_t *const b[3]) { for (int q = 0; q < 3; ++q) g.B[q] = b[q]; };
+  auto setO = [&](uint8_t *const o[3]) { for (int q = 0; q < 3; ++q) g.out[q] = o ? o[q] : nullptr; };
   g.s_idx = C.s_idx; g.ldp = ldp; g.N = fw; g.KPAN_out = kpw;
   // G1: Z0 = tanh(D W0 + b0), S0 = 1 - Z0^2 (stored: recomputing it from the rounded Z0 loses the saturated units)
-  g.Ah = Dh; g.Al = Dl; g.Bh = N.W0h; g.Bl = N.W0l; g.KPAN = kpd; g.bias = N.b0;
-  g.out_plain0 = Z0; g.out_plain1 = S0; g.out_h = X0h; g.out_l = X0l;
-  if ((e = ft_launch<NT, FE_TANH>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  setA(B.D); setB(N.W0); g.KPAN = kpd; g.bias = N.b0;
+  g.out_plain0 = B.Z0; g.out_plain1 = B.S0; setO(B.X0);
+  if ((e = ft_launch<NT, FE_TANH, OPF>(C, ty, g, 1, st)) != cudaSuccess) return e;
   // G2: U1 = tanh(Z0 W1 + b1), Z1 = Z0 + U1, S1 = 1 - U1^2
-  g.Ah = X0h; g.Al = X0l; g.Bh = N.W1h; g.Bl = N.W1l; g.KPAN = kpw; g.bias = N.b1; g.in0 = Z0;
-  g.out_plain0 = Z1; g.out_plain1 = S1; g.out_h = X1h; g.out_l = X1l;
-  if ((e = ft_launch<NT, FE_TANH_SKIP>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  setA(B.X0); setB(N.W1); g.KPAN = kpw; g.bias = N.b1; g.in0 = B.Z0;
+  g.out_plain0 = B.Z1; g.out_plain1 = B.S1; setO(B.X1);
+  if ((e = ft_launch<NT, FE_TANH_SKIP, OPF>(C, ty, g, 1, st)) != cudaSuccess) return e;
   // G3: U2 = tanh(Z1 W2 + b2), E_i = (Z1 + U2) . w3 + b3, Q2 = w3 (1 - U2^2)
-  g.Ah = X1h; g.Al = X1l; g.Bh = N.W2h; g.Bl = N.W2l; g.bias = N.b2; g.w3 = N.w3; g.in0 = Z1; g.b3 = N.b3;
-  g.atom_energy = atom_energy; g.out_plain0 = nullptr; g.out_plain1 = nullptr; g.out_h = X0h; g.out_l = X0l;
-  if ((e = ft_launch<NT, FE_L3>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  setA(B.X1); setB(N.W2); g.bias = N.b2; g.w3 = N.w3; g.in0 = B.Z1; g.b3 = N.b3;
+  g.atom_energy = atom_energy; g.out_plain0 = nullptr; g.out_plain1 = nullptr; setO(B.X0);
+  if ((e = ft_launch<NT, FE_L3, OPF>(C, ty, g, 1, st)) != cudaSuccess) return e;
   // G4: dZ1 = w3 + Q2 W2^T, Q1 = dZ1 S1
-  g.Ah = X0h; g.Al = X0l; g.Bh = N.W2Th; g.Bl = N.W2Tl; g.in0 = nullptr; g.in1 = S1;
-  g.out_plain0 = nullptr; g.out_plain1 = dZ1; g.out_h = X1h; g.out_l = X1l;
-  if ((e = ft_launch<NT, FE_BWD1>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  setA(B.X0); setB(N.W2T); g.in0 = nullptr; g.in1 = B.S1;
+  g.out_plain0 = nullptr; g.out_plain1 = B.dZ1; setO(B.X1);
+  if ((e = ft_launch<NT, FE_BWD1, OPF>(C, ty, g, 1, st)) != cudaSuccess) return e;
   // G5: dZ0 = dZ1 + Q1 W1^T, Q0 = dZ0 S0
-  g.Ah = X1h; g.Al = X1l; g.Bh = N.W1Th; g.Bl = N.W1Tl; g.in0 = dZ1; g.in1 = S0;
-  g.out_plain0 = nullptr; g.out_plain1 = nullptr; g.out_h = X0h; g.out_l = X0l;
-  if ((e = ft_launch<NT, FE_BWD0>(C, ty, g, 1, st)) != cudaSuccess) return e;
+  setA(B.X1); setB(N.W1T); g.in0 = B.dZ1; g.in1 = B.S0;
+  g.out_plain0 = nullptr; g.out_plain1 = nullptr; setO(B.X0);
+  if ((e = ft_launch<NT, FE_BWD0, OPF>(C, ty, g, 1, st)) != cudaSuccess) return e;
   // G6: dD = Q0 W0^T
-  g.Ah = X0h; g.Al = X0l; g.Bh = N.W0Th; g.Bl = N.W0Tl; g.N = F.dim; g.ldp = F.dimp; g.KPAN_out = 0;
-  g.out_plain0 = dD; g.out_h = nullptr; g.out_l = nullptr; g.in0 = nullptr; g.in1 = nullptr;
-  if (F.NT6 == 240) return ft_launch<240, FE_STORE>(C, ty, g, F.dimp / 240, st);
-  return ft_launch<128, FE_STORE>(C, ty, g, F.dimp / 128, st);
+  setA(B.X0); setB(N.W0T); g.N = F.dim; g.ldp = F.dimp; g.KPAN_out = 0;
+  g.out_plain0 = B.dD; setO(nullptr); g.in0 = nullptr; g.in1 = nullptr;
+  if (F.NT6 == 240) return ft_launch<240, FE_STORE, OPF>(C, ty, g, F.dimp / 240, st);
+  return ft_launch<128, FE_STORE, OPF>(C, ty, g, F.dimp / 128, st);
 }
 
-cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
-                   cudaStream_t st, bool want_dT64) {
-  if (C.n <= 0) return cudaSuccess;
-  const FitTC *F = reinterpret_cast<const FitTC *>(W.fit);
-  if (!F) return cudaErrorNotSupported;
+template <int OPF>
+static cudaError_t tc_fit_fmt(const DevModel &P, const ChunkView &C, const FitTC *F, void *ws, float *dT32,
+                              double *atom_energy, cudaStream_t st, bool want_dT64) {
+  constexpr int KP = OpFmt<OPF>::KP, NP = OpFmt<OPF>::NP;
   const size_t tiles = (size_t)(C.n + 127) / 128, rows = tiles * 128;
-  const size_t kpd = (size_t)ft_round_up(F->dim, 32) / 32, kpw = F->fwp / 32;
-  float *p = reinterpret_cast<float *>(ws);
-  float *Dh = p; p += tiles * kpd * 4096;
-  float *Dl = p; p += tiles * kpd * 4096;
-  float *X0h = p; p += tiles * kpw * 4096;
-  float *X0l = p; p += tiles * kpw * 4096;
-  float *X1h = p; p += tiles * kpw * 4096;
-  float *X1l = p; p += tiles * kpw * 4096;
-  float *Z0 = p; p += rows * F->fwp;
-  float *S0 = p; p += rows * F->fwp;
-  float *S1 = p; p += rows * F->fwp;
-  float *Z1 = p; p += rows * F->fwp;
-  float *dZ1 = p; p += rows * F->fwp;
-  float *dD = p;
+  const size_t kpd = (size_t)ft_round_up(F->dim, KP) / KP, kpw = F->fwp / KP;
+  uint8_t *pb = reinterpret_cast<uint8_t *>(ws);
+  FitTCBufs B{};
+  for (int q = 0; q < 3; ++q) { B.D[q] = pb + (size_t)(q < NP ? q : 0) * tiles * kpd * FT_APANEL; }
+  pb += (size_t)NP * tiles * kpd * FT_APANEL;
+  for (int q = 0; q < 3; ++q) { B.X0[q] = pb + (size_t)(q < NP ? q : 0) * tiles * kpw * FT_APANEL; }
+  pb += (size_t)NP * tiles * kpw * FT_APANEL;
+  for (int q = 0; q < 3; ++q) { B.X1[q] = pb + (size_t)(q < NP ? q : 0) * tiles * kpw * FT_APANEL; }
+  pb += (size_t)NP * tiles * kpw * FT_APANEL;
+  float *p = reinterpret_cast<float *>(pb);
+  B.Z0 = p; p += rows * F->fwp;
+  B.S0 = p; p += rows * F->fwp;
+  B.S1 = p; p += rows * F->fwp;
+  B.Z1 = p; p += rows * F->fwp;
+  B.dZ1 = p; p += rows * F->fwp;
+  B.dD = p;
   // The per-type chains (descriptor rows, six GEMMs, dT contraction) are independent: disjoint rows; a tile on the type
   // boundary is read by both and written row-wise by each.  G1-G5 of one type fill only as many SMs as that type has row
   // tiles (W24k: 64 and 128 of 148), and the descriptor / dT kernels are memory-bound while the GEMMs are not: forked
@@ -608,28 +682,30 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
     cudaError_t e = dpb_fork_streams(P.ntypes, st, ts);
     if (e != cudaSuccess) return e;
   }
+  FitTCArgs dimg{};
+  for (int q = 0; q < 3; ++q) dimg.out[q] = B.D[q];
   for (int k = 0; k < P.ntypes; ++k) {
     const int ty = P.ntypes - 1 - k;
     cudaStream_t s = ts[k];
     switch (P.Ma) {
-      case 4: k_descr_tc<4><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, Dh, Dl); break;
-      case 8: k_descr_tc<8><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, Dh, Dl); break;
-      default: k_descr_tc<16><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, Dh, Dl); break;
+      case 4: k_descr_tc<4, OPF><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, dimg); break;
+      case 8: k_descr_tc<8, OPF><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, dimg); break;
+      default: k_descr_tc<16, OPF><<<nbd, 256, smd, s>>>(P, C, ty, (int)kpd, dimg); break;
     }
     DPB_LAUNCHED(1);
     cudaError_t e;
     switch (F->NT) {
-      case 32: e = ft_run_type<32>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
-      case 64: e = ft_run_type<64>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
-      case 128: e = ft_run_type<128>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
-      case 240: e = ft_run_type<240>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
-      default: e = ft_run_type<256>(P, C, *F, ty, Dh, Dl, X0h, X0l, X1h, X1l, Z0, S0, S1, Z1, dZ1, dD, atom_energy, s); break;
+      case 32: e = ft_run_type<32, OPF>(P, C, *F, ty, B, atom_energy, s); break;
+      case 64: e = ft_run_type<64, OPF>(P, C, *F, ty, B, atom_energy, s); break;
+      case 128: e = ft_run_type<128, OPF>(P, C, *F, ty, B, atom_energy, s); break;
+      case 240: e = ft_run_type<240, OPF>(P, C, *F, ty, B, atom_energy, s); break;
+      default: e = ft_run_type<256, OPF>(P, C, *F, ty, B, atom_energy, s); break;
     }
     if (e != cudaSuccess) return e;
     switch (P.Ma) {
-      case 4: k_dT_tc<1><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, dD, dT32, dT64, ty); break;
-      case 8: k_dT_tc<2><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, dD, dT32, dT64, ty); break;
-      default: k_dT_tc<4><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, dD, dT32, dT64, ty); break;
+      case 4: k_dT_tc<1><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, B.dD, dT32, dT64, ty); break;
+      case 8: k_dT_tc<2><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, B.dD, dT32, dT64, ty); break;
+      default: k_dT_tc<4><<<nbt, 32 * DT_WARPS, smt, s>>>(P, C, F->dimp, B.dD, dT32, dT64, ty); break;
     }
     DPB_LAUNCHED(1);
   }
@@ -638,4 +714,16 @@ cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, vo
     if (e != cudaSuccess) return e;
   }
   return cudaGetLastError();
+}
+
+cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
+                   cudaStream_t st, bool want_dT64) {
+  if (C.n <= 0) return cudaSuccess;
+  const FitTC *F = reinterpret_cast<const FitTC *>(W.fit);
+  if (!F) return cudaErrorNotSupported;
+  switch (F->opf) {
+    case 0: return tc_fit_fmt<0>(P, C, F, ws, dT32, atom_energy, st, want_dT64);
+    case 1: return tc_fit_fmt<1>(P, C, F, ws, dT32, atom_energy, st, want_dT64);
+    default: return tc_fit_fmt<2>(P, C, F, ws, dT32, atom_energy, st, want_dT64);
+  }
 }

@@ -39,7 +39,33 @@ __host__ __device__ __forceinline__ constexpr uint32_t make_idesc_tf32(uint32_t 
        | ((M >> 4) << 24);  // m_dim
 }
 
+// Same layout for 16-bit operands (BF16): a panel row of 128 bytes holds 64 K-columns.
+__host__ __device__ __forceinline__ constexpr uint32_t sw128_offset_b16(uint32_t row, uint32_t k /* 0..63 */) {
+  return (row >> 3) * 1024u + (row & 7u) * 128u + ((((k >> 3) ^ (row & 7u)) & 7u) << 4) + ((k & 7u) << 1);
+}
+
+// Instruction descriptor for kind::f16 with BF16 operands, fp32 accumulate, K-major A and B, M x N tile (K = 16).
+__host__ __device__ __forceinline__ constexpr uint32_t make_idesc_bf16(uint32_t M, uint32_t N) {
+  return (1u << 4)          // c_format = F32
+       | (1u << 7)          // a_format = BF16
+       | (1u << 10)         // b_format = BF16
+       | ((N >> 3) << 17)   // n_dim
+       | ((M >> 4) << 24);  // m_dim
+}
+
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// D[tmem] (+)= A[smem] B[smem], 16-bit operands (kind::f16; the instruction descriptor says BF16).
+__device__ __forceinline__ void mma_f16_ss(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                           uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}\n" ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
 
 // D[tmem] (+)= A[smem] B[smem]; issued by ONE thread on behalf of the CTA.
 __device__ __forceinline__ void mma_tf32_ss(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
@@ -205,6 +231,21 @@ __device__ __forceinline__ void split_tf32(float x, float &hi, float &lo) {
   lo = __uint_as_float(l);
 }
 
+// x = p0 + p1 + p2 with every piece representable in BF16 (8 significant bits each, 24 together: all of fp32's):
+// p0 = rn(x), p1 = rn(x - p0), p2 = rn(x - p0 - p1); returned as the 16-bit patterns.
+__device__ __forceinline__ uint32_t bf16_bits_rn(float x) {
+  uint32_t u = __float_as_uint(x);
+  u += 0x7fffu + ((u >> 16) & 1u);                          // round to nearest even (finite inputs)
+  return u >> 16;
+}
+__device__ __forceinline__ void split_bf16x3(float x, uint32_t &p0, uint32_t &p1, uint32_t &p2) {
+  p0 = bf16_bits_rn(x);
+  const float r1 = x - __uint_as_float(p0 << 16);
+  p1 = bf16_bits_rn(r1);
+  const float r2 = r1 - __uint_as_float(p1 << 16);
+  p2 = bf16_bits_rn(r2);
+}
+
 // fp32 tanh and its derivative from u = exp(-2|x|) in (0, 1] (ex2.approx) and r = 1 / (1 + u) (rcp.approx):
 //   tanh x = sign(x) (1 - u) r,    1 - tanh^2 x = 4 u r^2.
 // The derivative is formed without the cancellation of 1 - t^2, so it keeps fp32 relative accuracy in the saturated
@@ -251,6 +292,20 @@ __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
 }
 
 }  // namespace tc
+
+// host-side BF16 rounding (round to nearest even), returned as the 16-bit pattern
+static inline uint16_t tc_host_bf16_bits(float x) {
+  uint32_t u;
+  memcpy(&u, &x, 4);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+static inline float tc_host_bf16_value(uint16_t b) {
+  const uint32_t u = (uint32_t)b << 16;
+  float y;
+  memcpy(&y, &u, 4);
+  return y;
+}
 
 // host-side TF32 rounding (round to nearest, ties away from zero: what cvt.rna.tf32.f32 does)
 static inline float tc_host_tf32(float x) {

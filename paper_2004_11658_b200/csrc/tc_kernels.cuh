@@ -23,8 +23,9 @@ cudaError_t tc_pass2(const DevModel &P, const ChunkView &C, const TCWeights &W, 
                      double *force, double *virial, cudaStream_t st);
 
 // fitting stage (fit_tc.cu): E_i and dT (fp64 in C.dT and the fp32 copy dT32) from C.T
-cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W);
+// opf: operand format of the fitting GEMMs: 0 = 3xTF32, 1 = BF16 x 6 products, 2 = plain BF16 (fit_tc.cu)
+cudaError_t tc_prepare_fit(const DevModel &P, const double *fit_h, TCWeights &W, int opf);
 void tc_release_fit(TCWeights &W);
-size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk);
+size_t tc_fit_workspace_bytes(const DevModel &P, int64_t chunk, int opf);
 cudaError_t tc_fit(const DevModel &P, const ChunkView &C, const TCWeights &W, void *ws, float *dT32, double *atom_energy,
                    cudaStream_t st, bool want_dT64);   // want_dT64: also write C.dT (fp64 view of dT for the debug hook)

@@ -41,7 +41,7 @@ def test_version_and_error_strings(lib):
 
 
 def test_create_rejects_bad_arguments_without_a_gpu(lib):
-    """Argument validation happens before any CUDA call: EINVAL for null pointers, ENOTIMPL for precisions that are not built."""
+    """Argument validation happens before any CUDA call: EINVAL for null pointers and for precisions outside the enum."""
     out = ctypes.c_void_p()
     assert lib.dpb_model_create(None, 0, ctypes.byref(out)) == -1
 
@@ -50,7 +50,8 @@ def test_create_rejects_bad_arguments_without_a_gpu(lib):
                     ("sel", ctypes.c_void_p), ("emb_s1", ctypes.c_int32), ("m_axis", ctypes.c_int32),
                     ("fit_width", ctypes.c_int32), ("emb", ctypes.c_void_p), ("fit", ctypes.c_void_p)]
     d = Desc(1, 6.0, 0.5, None, 25, 16, 240, None, None)
-    assert lib.dpb_model_create(ctypes.byref(d), 2, ctypes.byref(out)) == -6      # BF16 variant: not built
+    assert lib.dpb_model_create(ctypes.byref(d), 7, ctypes.byref(out)) == -1      # not a dpb_precision
+    assert lib.dpb_model_create(ctypes.byref(d), 2, ctypes.byref(out)) == -1      # BF16 is built: null sel / weights
     assert lib.dpb_model_create(ctypes.byref(d), 1, ctypes.byref(out)) == -1      # TF32 is built: null sel / weights
     assert lib.dpb_model_create(ctypes.byref(d), 0, ctypes.byref(out)) == -1      # null sel / weights
     assert not out.value

@@ -48,14 +48,14 @@ def _eval(m, coord, types, box, spec=None, debug=False):
     return res
 
 
-def _check(ref, got):
+def _check(ref, got, vir_tol=1e-4):
     assert np.array_equal(got["nlist"], ref["nlist"]), "nlist must be bit-exact also in mixed precision"
     e_ref = ref["energy"]
     assert abs(e_ref) >= 1e-3 * np.abs(ref["atom_energy"]).sum()
     assert abs(got["energy"][0] - e_ref) <= E_REL * abs(e_ref)
     assert np.abs(got["force"] - ref["force"]).max() <= F_ABS
     assert np.abs(got["atom_energy"] - ref["atom_energy"]).max() <= 1e-4 * max(1.0, np.abs(ref["atom_energy"]).max())
-    assert np.abs(got["virial"] - ref["virial"]).max() <= 1e-4 * max(1.0, np.abs(ref["virial"]).max())
+    assert np.abs(got["virial"] - ref["virial"]).max() <= vir_tol * max(1.0, np.abs(ref["virial"]).max())
     assert np.abs(got["force"].sum(0)).max() <= 1e-9          # F_j -= f, F_i += f in fp64: exact up to fp64 rounding
 
 
@@ -143,12 +143,12 @@ def test_mixed_full_size(name, conditioned):
     assert got["info"].n_overflow == 0
 
 
-def test_mixed_unsupported_shapes_and_bf16_are_reported():
+def test_mixed_unsupported_shapes_are_reported():
     from paper_2004_11658_b200 import DPBError
-    from paper_2004_11658_b200.binding import TF32, BF16
+    from paper_2004_11658_b200.binding import TF32, BF16, BF16_PLAIN
     from conftest import small_model
     spec, emb, fit = small_model(ntypes=1, s1=5, m_axis=3, fit_width=9)
-    for prec in (TF32, BF16):
+    for prec in (TF32, BF16, BF16_PLAIN):
         with pytest.raises(DPBError) as e:
             _model(spec, emb, fit, prec)
         assert e.value.status == -6
@@ -191,3 +191,50 @@ def test_mixed_config5_copper_864k():
     assert abs(e32 - e64) <= E_REL * abs(e64)
     assert (res["tf32"]["force"] - res["f64"]["force"]).abs().max().item() <= F_ABS
     assert res["tf32"]["force"].sum(0).abs().max().item() <= 1e-7
+
+
+# ---- BASELINE.json configs[3] "and a BF16 variant" (DPB_BF16 / DPB_BF16_PLAIN, include/dpb.h) ------------------------------
+@pytest.mark.parametrize("conditioned", [False, True])
+def test_bf16x6_small_boxes_vs_oracle(conditioned):
+    """DPB_BF16 (fitting GEMMs with BF16 operands split into three pieces, six products, tcgen05 kind::f16) against the
+    oracle under the mixed-precision bars, W192 (two species, tiles holding both) and the 864-atom copper box."""
+    from oracle import Oracle
+    from paper_2004_11658_b200.binding import BF16
+    for name in ("W192", "Cu32k"):
+        spec = MODELS[name]
+        coord, types, box = gen.make_system("W192") if name == "W192" else gen.copper_box(6, 0.05, seed=gen.SEED_BASE + 2)
+        emb, fit = gen.make_weights(spec)
+        if conditioned:
+            fit = gen.condition_fit_w0(spec, fit)
+        ref = Oracle.from_spec(spec, emb, fit).eval(coord, types, box)
+        m = _model(spec, emb, fit, BF16)
+        # north_star's bars are on E and F; the virial bound is ours: 1.2e-4 measured on copper with the literal
+        # (saturated) weight set, 3e-5 with 3xTF32 — same order, hence 3e-4 here
+        _check(ref, _eval(m, coord, types, box), vir_tol=3e-4)
+        m.close()
+
+
+@pytest.mark.parametrize("conditioned", [False, True])
+def test_bf16_full_size_w24k(conditioned):
+    """configs[3] at full size (W24k, literal and conditioned weights), every output element against the oracle:
+    DPB_BF16 (x6) must meet the mixed-precision bars (E 1e-5 relative, F 1e-3 eV/A); DPB_BF16_PLAIN (one BF16 piece per
+    operand in the fitting GEMMs) is MEASURED: its errors are recorded here and must exceed those of the split by more
+    than an order of magnitude in E_i — the reason the variant that ships is the split one."""
+    from conftest import oracle_full
+    from paper_2004_11658_b200.binding import BF16, BF16_PLAIN
+    spec, emb, fit, coord, types, box, ref = oracle_full("W24k", conditioned)
+    m = _model(spec, emb, fit, BF16)
+    got = _eval(m, coord, types, box)
+    m.close()
+    _check(ref, got, vir_tol=3e-4)
+    m = _model(spec, emb, fit, BF16_PLAIN)
+    plain = _eval(m, coord, types, box)
+    m.close()
+    assert np.array_equal(plain["nlist"], ref["nlist"])
+    err = lambda o: (abs(o["energy"][0] - ref["energy"]) / abs(ref["energy"]), np.abs(o["force"] - ref["force"]).max(),
+                     np.abs(o["atom_energy"] - ref["atom_energy"]).max())
+    e6, f6, ei6 = err(got)
+    e1, f1, ei1 = err(plain)
+    print(f"W24k conditioned={conditioned}: BF16x6 E {e6:.2e} F {f6:.2e} E_i {ei6:.2e} | plain BF16 E {e1:.2e} F {f1:.2e} E_i {ei1:.2e}")
+    assert np.isfinite(e1) and np.isfinite(f1)
+    assert ei1 > 10.0 * ei6
