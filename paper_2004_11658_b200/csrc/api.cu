@@ -131,7 +131,7 @@ struct dpb_model {
   Buf v2ws;
   // workspace
   Buf key, count, start, cursor, s_idx, s_xyz, stats, ei;
-  Buf nl, nlp, dr, nreal, T, dT;
+  Buf nl, nlp, dr, nreal, T, dT, counters;
   int dt_pad_alloc = -1;          // layout the dT buffer was last used with (pad rows must be zero: cleared on a change)
   Buf v0[9];
   Buf v1ws;
@@ -242,7 +242,7 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
 extern "C" int dpb_model_destroy(dpb_model *m) {
   if (!m) return DPB_OK;
   Buf *all[] = {&m->emb, &m->fit, &m->key, &m->count, &m->start, &m->cursor, &m->s_idx, &m->s_xyz, &m->stats, &m->ei,
-                &m->nl, &m->nlp, &m->dr, &m->v2ws, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
+                &m->nl, &m->nlp, &m->dr, &m->v2ws, &m->counters, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
                 &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
                 &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass,
                 &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_owner, &m->cell_f, &m->cell_cnt};
@@ -458,6 +458,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   int dt_pad = 0;
   CU(m->nl.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
   CU(m->nlp.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
+  CU(m->counters.reserve(sizeof(int) * 128), "workspace");
   CU(m->dr.reserve(sizeof(double4) * (size_t)chunk * P.nm), "workspace");
   CU(m->nreal.reserve(sizeof(int) * (size_t)chunk * P.ntypes), "workspace");
   if (!nlist_only) {
@@ -544,6 +545,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.dt_pad = dt_pad;
     C.dt_rows = dt_pad ? 4 * dt_pad : P.M;
     C.nlp = m->nlp.as<int>();
+    C.counters = m->counters.as<int>();
+    if (!nlist_only) CU(cudaMemsetAsync(C.counters, 0, sizeof(int) * 128, st), "memset counters");
     C.fslot = nullptr;
     C.pos_of = m->pos_of.as<int>();
     C.stats = stats;

@@ -73,6 +73,7 @@ struct ChunkView {
   // the atom with the lower sorted position evaluates the pair once and adds g (x) R~_ji to T_j with red.global.add.f64
   const int *pos_of;       // [N] sorted position of original atom index (nullptr: no reuse)
   const DevStats *stats;   // reuse is taken only while stats->n_overflow == 0 (a dropped neighbour breaks the symmetry)
+  int *counters;           // [128] work-item counters of the embedding launches (pass 1: net, pass 2: 64 + net), zeroed per chunk
   int reuse;               // pass 1
   int reuse2;              // pass 2 (k_pass2_dmma_ru): both directions of a same-species pair from one evaluation
 };

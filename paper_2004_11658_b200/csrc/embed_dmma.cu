@@ -22,7 +22,7 @@
 #include <vector>
 
 #ifndef P1_WARPS
-#define P1_WARPS 8            // warps per CTA, pass 1
+#define P1_WARPS 12           // warps per CTA, pass 1 (168 registers; 8 warps at 204-218: 3-4 % slower, 16: no better)
 #endif
 #ifndef P2_WARPS
 #define P2_WARPS 8            // warps per CTA, pass 2
@@ -78,6 +78,15 @@ __device__ __forceinline__ void stage_net(double *W, const double *__restrict__ 
   }
   __syncthreads();                                       // the initialised barrier is visible to every waiter
   tc::mbar_wait(mbar, 0);
+}
+
+// Work items are handed out dynamically: a warp takes the next (atom, segment) from a counter in global memory.  A static
+// round-robin leaves a tail of 1 / (items per warp) — 15-20 % for the 8,192 oxygen atoms of the water box on 148 x 12 warps
+// — and the pair reuse makes the items unequal (an atom evaluates between none and all of its same-species pairs).
+__device__ __forceinline__ int next_item(int *counter, int lane) {
+  int v = 0;
+  if (lane == 0) v = atomicAdd(counter, 1);
+  return __shfl_sync(0xffffffffu, v, 0);
 }
 
 static int sp_for(int s1) {
@@ -190,7 +199,8 @@ __device__ __forceinline__ void env_row4(const DevModel &P, const double4 v, dou
 // accumulation of this launch into T is a reduction.  Taken only while no neighbour was dropped (n_overflow == 0).
 template <int SP, int RB, bool RU>
 __global__ void __launch_bounds__((32 * P1_WARPS), 1)
-k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate, int nseg) {
+k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, int accumulate, int nseg,
+             int *counter) {
   using L = EL<SP>;
   extern __shared__ __align__(16) double smem[];
   double *W = smem;
@@ -223,7 +233,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 
   // work item = (atom, segment of its section): nseg > 1 splits the rows of an atom over several warps when the chunk has
   // too few atoms to fill the GPU (configs[0]: 192 atoms); T is then accumulated with reductions (accumulate == 2)
-  for (int item = blockIdx.x * P1_WARPS + warp; item < (row_hi - row_lo) * nseg; item += gridDim.x * P1_WARPS) {
+  for (int item = next_item(counter, lane); item < (row_hi - row_lo) * nseg; item = next_item(counter, lane)) {
     const int qa = row_lo + item / nseg;
     int n = C.nreal[(size_t)qa * P.ntypes + t];
     int s_lo = 0;
@@ -235,24 +245,32 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
     if (s_lo >= n && accumulate) continue;               // (store mode still has to write the zero tile)
     const double4 *dr = C.dr + (size_t)qa * P.nm + P.sec_start[t];
     if (RU && ru) {                                      // keep the slots whose pair this atom evaluates
-      const int *nlr = C.nl + (size_t)qa * P.nm + P.sec_start[t];
+      // the sorted positions of the neighbours (written by k_nlist next to their input indices): the loads of up to
+      // eight 32-slot batches are issued together — one memory latency per atom instead of two dependent ones per batch
+      const int *nlpr = C.nlp + (size_t)qa * P.nm + P.sec_start[t];
       int nk = 0;
       __syncwarp();
-      for (int base = s_lo; base < n; base += 32) {
-        const int slot = base + lane;
-        bool keep = false;
-        int qj = -1;
-        if (slot < n) {
-          qj = C.pos_of[nlr[slot]] - C.p0;
+      for (int base0 = s_lo; base0 < n; base0 += 256) {
+        int pj[8];
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+          const int slot = base0 + 32 * b + lane;
+          pj[b] = slot < n ? nlpr[slot] - C.p0 : -1;
+        }
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+          const int slot = base0 + 32 * b + lane;
+          if (base0 + 32 * b >= n) break;
+          int qj = pj[b];
           if (qj < 0 || qj >= C.n) qj = -1;              // not a centre of this chunk (other chunk, ghost): one direction
-          keep = qj < 0 || qj > qa;
+          const bool keep = slot < n && (qj < 0 || qj > qa);
+          const unsigned mk = __ballot_sync(0xffffffffu, keep);
+          if (keep) {
+            const int pos = nk + __popc(mk & ((1u << lane) - 1u));
+            ksl[pos] = slot; krow[pos] = qj;
+          }
+          nk += __popc(mk);
         }
-        const unsigned mk = __ballot_sync(0xffffffffu, keep);
-        if (keep) {
-          const int pos = nk + __popc(mk & ((1u << lane) - 1u));
-          ksl[pos] = slot; krow[pos] = qj;
-        }
-        nk += __popc(mk);
       }
       n = nk;
       __syncwarp();
@@ -268,13 +286,26 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 #pragma unroll
         for (int c = 0; c < 4; ++c) Tacc[ch][u][c] = 0.0;
 
+    // the (d, r) row of the NEXT block is fetched while this one is computed: no block starts with a global round trip
+    double4 dvn[RB];
+#pragma unroll
+    for (int rb = 0; rb < RB; ++rb) {
+      const int row = g + 8 * rb;
+      dvn[rb] = make_double4(0.0, 0.0, 0.0, 1.0);
+      if (row < n) dvn[rb] = dr[(RU && ru) ? ksl[row] : row];
+    }
     for (int r0 = 0; r0 < n; r0 += 8 * RB) {
       double x[RB];
 #pragma unroll
       for (int rb = 0; rb < RB; ++rb) {
         const int row = r0 + g + 8 * rb;
         double e[4] = {0.0, 0.0, 0.0, 0.0};
-        if (row < n) env_row4(P, dr[(RU && ru) ? ksl[row] : row], e);
+        const double4 dvc = dvn[rb];
+        {
+          const int rown = row + 8 * RB;
+          if (rown < n) dvn[rb] = dr[(RU && ru) ? ksl[rown] : rown];
+        }
+        if (row < n) env_row4(P, dvc, e);
         x[rb] = e[0];
         if (q == 0) {
           double *dst = envt + (g + 8 * rb) * 4;
@@ -352,19 +383,26 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
           }
         }
         if (RU && ru) {                                  // T_k += g (x) R~_ki, 8 positions x 4 components per instruction
+          // The phase must be SHORT: while a warp is in it, it feeds the fp64 pipe nothing.  Row targets come from one
+          // load per lane + shuffles, and all shared-memory loads of a row (its R~ component, SP values of g) are issued
+          // before the first reduction (the compiler keeps loads behind atomics in program order).
           const int comp = lane & 3;
-#pragma unroll 1
+          const int myq = (lane < 8 * RB && r0 + lane < n) ? krow[r0 + lane] : -1;
+#pragma unroll 2
           for (int row = 0; row < 8 * RB; ++row) {
-            if (r0 + row >= n) break;
-            const int qj = krow[r0 + row];
+            const int qj = __shfl_sync(0xffffffffu, myq, row);
             if (qj < 0) continue;
-            const double ev = comp == 0 ? envt[row * 4] : -envt[row * 4 + comp];
-            double *Tj = C.T + (size_t)qj * M * 4;
+            const double e0 = envt[row * 4 + comp];
             const double *gr = gt + row * L::LDG + (lane >> 2);
+            double gv[SP];
+#pragma unroll
+            for (int k = 0; k < SP; ++k) gv[k] = gr[8 * k];
+            const double ev = comp == 0 ? e0 : -e0;
+            double *Tj = C.T + (size_t)qj * M * 4;
 #pragma unroll
             for (int k = 0; k < SP; ++k) {
               const int o = toff[ch][k];
-              if (o >= 0) atomicAdd(Tj + o, gr[8 * k] * ev);
+              if (o >= 0) atomicAdd(Tj + o, gv[k] * ev);
             }
           }
         }
@@ -403,7 +441,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 template <int SP>
 __global__ void __launch_bounds__((32 * P2_WARPS), 1)
 k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
-             double *__restrict__ virial, int nseg) {
+             double *__restrict__ virial, int nseg, int *counter) {
   using L = EL<SP>;
   extern __shared__ __align__(16) double smem[];
   double *W = smem;
@@ -421,7 +459,7 @@ k_pass2_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 #pragma unroll
   for (int k = 0; k < 9; ++k) vir[k] = 0.0;
 
-  for (int item = blockIdx.x * P2_WARPS + warp; item < (row_hi - row_lo) * nseg; item += gridDim.x * P2_WARPS) {
+  for (int item = next_item(counter, lane); item < (row_hi - row_lo) * nseg; item = next_item(counter, lane)) {
     const int qa = row_lo + item / nseg;                 // work item = (atom, segment of its section), as in pass 1
     int n = C.nreal[(size_t)qa * P.ntypes + t];
     int s_lo = 0;
@@ -609,7 +647,8 @@ struct P2R {
   static constexpr int SLICE = 32 * NBA + 16;                // doubles per staged row slice (+128 B: rows on distinct banks)
   static constexpr int RING = 64;                            // kept rows in flight per warp
   // per warp: own dT tile [16 SP][4] | dT_j slices [8][SLICE] | ring (d, r) [RING] | ring j [RING] | ring row of j | mbarrier
-  static constexpr int per_warp = 64 * SP + 8 * SLICE + 4 * RING + RING / 2 + RING / 2 + 2;
+  //           | staging of 32 raw slots: (d, r) [32], j [32], sorted position of j [32]
+  static constexpr int per_warp = 64 * SP + 8 * SLICE + 4 * RING + RING / 2 + RING / 2 + 2 + 4 * 32 + 16 + 16;
 };
 
 // value and tangent MMAs of NB n-blocks (starting at n-block NB0 of the half), then the epilogue over their 2 NB slots
@@ -672,7 +711,7 @@ __device__ __forceinline__ void p2r_chunk(const double *__restrict__ W2h, const 
 template <int SP>
 __global__ void __launch_bounds__((32 * P2_WARPS), 1)
 k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a, double *__restrict__ force,
-                double *__restrict__ virial, int nseg) {
+                double *__restrict__ virial, int nseg, int *counter) {
   using L = EL<SP>;
   using R = P2R<SP>;
   extern __shared__ __align__(16) double smem[];
@@ -684,6 +723,9 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   int *rjn = reinterpret_cast<int *>(rdv + R::RING);                    //   input index of the neighbour (force scatter)
   int *rqj = rjn + R::RING;                                             //   its row in this chunk when both directions run, else -1
   uint64_t *mbar = reinterpret_cast<uint64_t *>(rqj + R::RING);
+  double4 *sdr = reinterpret_cast<double4 *>(mbar + 2);                 // staged raw slots (cp.async, one batch ahead)
+  int *snl = reinterpret_cast<int *>(sdr + 32);
+  int *snlp = snl + 32;
   __shared__ double vred[P2_WARPS][9];
   __shared__ uint64_t wbar;
   if (lane == 0) tc::mbar_init(mbar, 1);
@@ -700,7 +742,7 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 #pragma unroll
   for (int k = 0; k < 9; ++k) vir[k] = 0.0;
 
-  for (int item = blockIdx.x * P2_WARPS + warp; item < (row_hi - row_lo) * nseg; item += gridDim.x * P2_WARPS) {
+  for (int item = next_item(counter, lane); item < (row_hi - row_lo) * nseg; item = next_item(counter, lane)) {
     const int qa = row_lo + item / nseg;                 // work item = (atom, segment of its section), as in pass 1
     int n = C.nreal[(size_t)qa * P.ntypes + t];
     int s_lo = 0;
@@ -718,18 +760,39 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       const double4 *src = reinterpret_cast<const double4 *>(C.dT + (size_t)qa * dt_tile);
       for (int p = lane; p < 16 * SP; p += 32) *reinterpret_cast<double4 *>(dTt + 4 * p) = src[p];
     }
-    // kept rows: sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs
-    int head = 0, cnt = 0, rawpos = s_lo, sweep = ru ? 0 : 1;
-    bool done = false;
-    auto refill = [&]() {
+    // kept rows: sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs.  The raw
+    // slots travel global -> shared one batch of 32 AHEAD of their use (cp.async issued before a row block is computed,
+    // consumed after it), so that the compaction into the ring never waits for a memory round trip.
+    int head = 0, cnt = 0, rawpos = s_lo, sweep = ru ? 0 : 1, st_base = 0, st_sweep = 0;
+    bool done = false, staged = false;
+    auto stage = [&]() {
+      if (done || staged) return;
       const int slot = rawpos + lane;
+      if (slot < n) {
+        emb_cp16(sdr + lane, dr + slot);
+        emb_cp16(reinterpret_cast<double *>(sdr + lane) + 2, reinterpret_cast<const double *>(dr + slot) + 2);
+        emb_cp4(snl + lane, nl + slot);
+        emb_cp4(snlp + lane, nlp + slot);
+      }
+      emb_cp_commit();
+      st_base = rawpos; st_sweep = sweep; staged = true;
+      rawpos += 32;
+      if (rawpos >= n) {
+        if (ru && sweep == 0) { sweep = 1; rawpos = s_lo; } else done = true;
+      }
+    };
+    auto consume = [&]() {
+      if (!staged) return;
+      emb_cp_wait<0>();
+      __syncwarp();
+      const int slot = st_base + lane;
       bool keep = false;
       int qj = -1;
       if (slot < n) {
         if (ru) {
-          const int pj = nlp[slot] - C.p0;
+          const int pj = snlp[lane] - C.p0;
           const bool inchunk = pj >= 0 && pj < C.n;
-          if (sweep == 0) { keep = inchunk && ((((qa + pj) & 1) == 0) == (qa < pj)); qj = pj; }
+          if (st_sweep == 0) { keep = inchunk && ((((qa + pj) & 1) == 0) == (qa < pj)); qj = pj; }
           else keep = !inchunk;
         } else {
           keep = true;
@@ -738,13 +801,14 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       const unsigned mk = __ballot_sync(0xffffffffu, keep);
       if (keep) {
         const int pos = (head + cnt + __popc(mk & ((1u << lane) - 1u))) & (R::RING - 1);
-        rdv[pos] = dr[slot]; rjn[pos] = nl[slot]; rqj[pos] = qj;
+        rdv[pos] = sdr[lane]; rjn[pos] = snl[lane]; rqj[pos] = qj;
       }
       cnt += __popc(mk);
-      rawpos += 32;
-      if (rawpos >= n) {
-        if (ru && sweep == 0) { sweep = 1; rawpos = s_lo; } else done = true;
-      }
+      staged = false;
+      __syncwarp();                                      // ring rows visible; the staging area may be refilled
+    };
+    auto fill = [&]() {
+      while (cnt < 16 && (staged || !done)) { stage(); consume(); }
     };
     // both-direction rows of the block at the ring head, and (lanes 0..7) the row of neighbour j of ring row `lane`
     int myqj = -1;
@@ -761,8 +825,8 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       __syncwarp();
       if (myqj >= 0) tc::bulk_g2s(jbuf + lane * R::SLICE, C.dT + (size_t)myqj * dt_tile + 16 * slot0, bytes, mbar);
     };
-    while (cnt < 16 && !done) refill();
-    __syncwarp();
+    fill();
+    if (cnt <= 32) stage();
     unsigned bmask = block_mask();
     issue(bmask, 0);
     double fi[3] = {0.0, 0.0, 0.0};
@@ -839,8 +903,9 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       // advance the ring and start the next block's first slices before the scalar tail of this one
       head = (head + nrows) & (R::RING - 1);
       cnt -= nrows;
-      while (cnt < 16 && !done) refill();
-      __syncwarp();
+      consume();
+      fill();
+      if (cnt <= 32) stage();
       bmask = block_mask();
       issue(bmask, 0);
       if (valid && q == 0) {
@@ -913,7 +978,7 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
   using L = EL<SP>;
   const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P1_WARPS * L::tile1s);
   const size_t smem_ru = smem + sizeof(int) * 2 * (size_t)P.nm * P1_WARPS;
-  const bool reuse = C.reuse && C.pos_of && smem_ru <= 227 * 1024;
+  const bool reuse = C.reuse && C.nlp && smem_ru <= 227 * 1024;
   static bool configured = false;
   static size_t configured_ru = 0;
   if (!configured) {
@@ -944,10 +1009,12 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
       const double *net = W.emb + (size_t)(a * P.ntypes + t) * W.net_stride;
       cudaStream_t s = nseg > 1 ? ts[(a * P.ntypes + t) % ns] : ts[P.ntypes - 1 - a];
       if (reuse && a == t)
-        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, s>>>(P, C, net, a, t, nseg > 1 ? 2 : 1, nseg);
+        k_pass1_dmma<SP, 1, true><<<grid, (32 * P1_WARPS), smem_ru, s>>>(P, C, net, a, t, nseg > 1 ? 2 : 1, nseg,
+                                                                        C.counters + a * P.ntypes + t);
       else
         k_pass1_dmma<SP, 1, false><<<grid, (32 * P1_WARPS), smem, s>>>(P, C, net, a, t,
-                                                                      nseg > 1 ? 2 : (reuse ? 1 : t > 0), nseg);
+                                                                      nseg > 1 ? 2 : (reuse ? 1 : t > 0), nseg,
+                                                                      C.counters + a * P.ntypes + t);
       DPB_LAUNCHED(1);
     }
   if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;
@@ -988,10 +1055,10 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
       cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
       if (reuse && a == t)
         k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, force,
-                                                                     virial, nseg);
+                                                                     virial, nseg, C.counters + 64 + net);
       else
         k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
-                                                              virial, nseg);
+                                                              virial, nseg, C.counters + 64 + net);
       DPB_LAUNCHED(1);
     }
   if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;
