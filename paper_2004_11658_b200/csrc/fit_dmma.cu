@@ -193,8 +193,12 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
 }
 
 // S5: D[b][a] = sum_c T[b][c] T[a][c] (Eq. 4; flatten b M^< + a, reading R7), zero-padded to dimp.
-__global__ void k_descr_v1(DevModel P, ChunkView C, int dimp, double *__restrict__ D) {
+__global__ void k_descr_v1(DevModel P, ChunkView C, int ty, int dimp, double *__restrict__ D) {
   const int q = blockIdx.x;
+  {                                                         // one launch per species, on that species' stream
+    const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+    if (q < row_lo || q >= row_hi) return;
+  }
   __shared__ double Ts[256 * 5 + 16];            // row stride 5 doubles: the 16 rows a = 0..15 hit 16 distinct bank pairs
   const double *T = C.T + (size_t)q * P.M * 4;
   for (int k = threadIdx.x; k < P.M * 4; k += blockDim.x) Ts[(k >> 2) * 5 + (k & 3)] = T[k];
@@ -212,8 +216,12 @@ __global__ void k_descr_v1(DevModel P, ChunkView C, int dimp, double *__restrict
 
 // S7: dT[b][c] = sum_a dD[b][a] T[a][c] + [b < M^<] sum_b' dD[b'][b] T[b'][c].  The second term (M^< x 4 outputs, M terms
 // each) is split over all threads in partial sums so that it does not serialise behind M^< x 4 threads.
-__global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restrict__ dD) {
+__global__ void k_dT_v1(DevModel P, ChunkView C, int ty, int dimp, const double *__restrict__ dD) {
   const int q = blockIdx.x;
+  {
+    const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+    if (q < row_lo || q >= row_hi) return;                  // (block-uniform: before any barrier)
+  }
   extern __shared__ double sm2[];
   double *Ts = sm2;                      // [M][4]
   const int ldr = P.Ma + 1;              // padded row stride: rows b, b + 1, ... fall into different banks
@@ -250,12 +258,16 @@ __global__ void k_dT_v1(DevModel P, ChunkView C, int dimp, const double *__restr
 // (a, c) summed over the lane's rows, at the end across the lanes that share a0.  Only T is staged in shared memory.
 #define DTV_WARPS 8
 template <int LPR>
-__global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView C, int dimp, const double *__restrict__ dD) {
+__global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView C, int ty, int dimp, const double *__restrict__ dD) {
   extern __shared__ double sm2[];
   constexpr int Ma = 2 * LPR, RPI = 32 / LPR;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = blockIdx.x * DTV_WARPS + warp;
   if (q >= C.n) return;
+  {                                                         // one launch per species, at the tail of that species' chain
+    const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+    if (q < row_lo || q >= row_hi) return;
+  }
   const int M = P.M;
   double *Ts = sm2 + (size_t)warp * (M + 2 * Ma) * 4;      // [M][4]
   double *f1 = Ts + 4 * M, *t2 = f1 + 4 * Ma;              // [Ma][4] first term of rows b < M^<; [Ma][4] second term
@@ -470,11 +482,19 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
   double *Q2 = p;                        // second Q buffer
   cudaError_t e;
 
-  k_descr_v1<<<C.n, 256, 0, st>>>(P, C, dimp, D);
-  DPB_LAUNCHED(1);
   const bool splitk = C.n <= FIT_SMALL_N && !C.fslot;    // (not in deterministic mode: the partial sums are reductions)
   if (splitk && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
-  // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint
+  // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint.  The
+  // descriptor and dT kernels (memory-bound) belong to the chains: one species' run beside the other's GEMMs
+  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
+  static size_t configured = 0;
+  if (sm > 48 * 1024 && sm > configured) {
+    e = cudaFuncSetAttribute(k_dT_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    configured = sm;
+  }
+  const size_t sms = sizeof(double) * DTV_WARPS * 4 * ((size_t)P.M + 2 * P.Ma);
+  const unsigned nbs = (unsigned)((C.n + DTV_WARPS - 1) / DTV_WARPS);
   cudaStream_t ts[DPB_MAX_TYPES];
   if ((e = dpb_fork_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
   for (int k = 0; k < P.ntypes; ++k) {
@@ -482,6 +502,8 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     cudaStream_t s = ts[k];
     const FitNet &N = F->nets[ty];
     GemmArgs g;
+    k_descr_v1<<<C.n, 256, 0, s>>>(P, C, ty, dimp, D);
+    DPB_LAUNCHED(1);
     // G1: Z0 = tanh(D W0 + b0).  Small systems: split-K over 8 CTAs (K = dim is a serial loop of dim / 16 tiles for
     // the few CTAs a 192-atom box offers), partial sums added into the cleared Z0, bias and tanh in a second kernel.
     g = GemmArgs{D, dimp, N.W0, fwp, dimp, fwp, N.b0, nullptr, nullptr, fwp, Z0, nullptr, fwp};
@@ -507,21 +529,12 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     // G6: dD = Q W0^T
     g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
     if ((e = gemm<8, EPI_STORE>(C, ty, g, s)) != cudaSuccess) return e;
+    if (P.Ma == 16 && sms <= 48 * 1024) k_dT_v1s<8><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
+    else if (P.Ma == 8 && sms <= 48 * 1024) k_dT_v1s<4><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
+    else if (P.Ma == 4 && sms <= 48 * 1024) k_dT_v1s<2><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
+    else k_dT_v1<<<C.n, 256, sm, s>>>(P, C, ty, dimp, dD);
+    DPB_LAUNCHED(1);
   }
   if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
-  const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
-  static size_t configured = 0;
-  if (sm > 48 * 1024 && sm > configured) {
-    e = cudaFuncSetAttribute(k_dT_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return e;
-    configured = sm;
-  }
-  const size_t sms = sizeof(double) * DTV_WARPS * 4 * ((size_t)P.M + 2 * P.Ma);
-  const unsigned nbs = (unsigned)((C.n + DTV_WARPS - 1) / DTV_WARPS);
-  if (P.Ma == 16 && sms <= 48 * 1024) k_dT_v1s<8><<<nbs, 32 * DTV_WARPS, sms, st>>>(P, C, dimp, dD);
-  else if (P.Ma == 8 && sms <= 48 * 1024) k_dT_v1s<4><<<nbs, 32 * DTV_WARPS, sms, st>>>(P, C, dimp, dD);
-  else if (P.Ma == 4 && sms <= 48 * 1024) k_dT_v1s<2><<<nbs, 32 * DTV_WARPS, sms, st>>>(P, C, dimp, dD);
-  else k_dT_v1<<<C.n, 256, sm, st>>>(P, C, dimp, dD);
-  DPB_LAUNCHED(1);
   return cudaGetLastError();
 }
