@@ -710,7 +710,7 @@ __device__ __forceinline__ void p2r_chunk(const double *__restrict__ W2h, const 
 
 template <int SP>
 __global__ void __launch_bounds__((32 * P2_WARPS), 1)
-k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a, double *__restrict__ force,
+k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
                 double *__restrict__ virial, int nseg, int *counter) {
   using L = EL<SP>;
   using R = P2R<SP>;
@@ -733,9 +733,9 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   stage_net(W, netp, L::total, &wbar);
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
-  const int t = a;
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
-  const bool ru = C.stats->n_overflow == 0ull;           // a dropped neighbour breaks the symmetry of the lists
+  // pairs are shared for the nets (a, a) only, and only while no neighbour was dropped (that breaks the list symmetry)
+  const bool ru = a == t && C.stats->n_overflow == 0ull;
   const size_t dt_tile = (size_t)C.dt_rows * 4;          // doubles per dT tile (= 64 SP)
   unsigned parity = 0;
   double vir[9];
@@ -1053,8 +1053,12 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     for (int t = P.ntypes - 1; t >= 0; --t) {
       const int net = a * P.ntypes + t;
       cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
+#ifdef EXP_RU_AS_PLAIN
+      if (reuse)
+#else
       if (reuse && a == t)
-        k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, force,
+#endif
+        k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
                                                                      virial, nseg, C.counters + 64 + net);
       else
         k_pass2_dmma<SP><<<grid, (32 * P2_WARPS), smem, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
