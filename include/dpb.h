@@ -101,7 +101,13 @@ int dpb_model_set_chunk(dpb_model *model, int64_t chunk_atoms);
  * synchronisation per evaluation (the batch sizes).  All compute the same path; tests compare each with the oracle. */
 int dpb_model_set_variant(dpb_model *model, int variant);
 
-/* Deterministic reduction (DPB_FP64, variant 1): forces and virial are summed in a fixed order instead of with fp64
+/* Reproducibility.  In the default mode two evaluations of the same input differ at the 1e-16 relative level, in F and the
+ * virial (fp64 atomics in the force scatter) AND in E and E_i: with the same-species pair reuse (on by default) and, for
+ * small systems, with the row segments and the split-K first fitting layer, T (Eq. 4's G^T R~) and the first-layer
+ * pre-activations are accumulated with fp64 reductions whose order varies from run to run.  The deterministic mode below
+ * switches all of these off (fixed summation order everywhere): bitwise identical E, E_i, F and virial.
+ *
+ * Deterministic reduction (DPB_FP64, variant 1): forces and virial are summed in a fixed order instead of with fp64
  * atomics, so two evaluations of the same input agree bit for bit (the paper reports E / F / virial reproducible to
  * 15 / 10 / 13 digits; the default atomics mode differs at the 1e-16 relative level from run to run).
  * Costs about N * Nm * 28 bytes of extra workspace and one gather kernel.  Exact only when no neighbour was dropped
@@ -117,17 +123,20 @@ int dpb_model_set_deterministic(dpb_model *model, int on);
  * dpb_eval_local, dpb_eval_host and dpb_md_run always run eagerly. */
 int dpb_model_set_graph(dpb_model *model, int mode);
 
-/* Same-species pair reuse in pass 1 (DPB_FP64, variant 1; on by default, off while the deterministic reduction is on).
+/* Same-species pair reuse (DPB_FP64, variant 1; on by default, off while the deterministic reduction is on).
  * The embedding net of a pair depends on s(r_ij) = s(r_ji) only (Eq. 5 and 8-9), so for the nets
- * G^{a,a} one evaluation serves both directions: the atom with the lower sorted position adds g (x) R~_ik to its own
- * T_i (Eq. 4's G^T R~) and g (x) R~_ki to T_k with fp64 reductions.  Only pairs whose two atoms are centres of the same
- * chunk are shared; it is switched off on the device for an evaluation in which a neighbour was dropped by a full type
- * section (n_overflow > 0), because the two lists are then not symmetric.  T is summed in a different (and, with the
- * reductions, run-to-run varying) order: results move at the 1e-15 relative level.  Other precisions ignore it.
- *   on = 0  off
- *   on = 1  (default) evaluations that run as a single chunk (dpb_model_set_chunk): with several chunks only the pairs
- *           inside a chunk can be shared and the bookkeeping costs more than it saves (measured on the 864,000-atom box)
- *   on = 2  always (pairs across a chunk boundary are evaluated in both directions)
+ * G^{a,a} one evaluation serves both directions.  Pass 1: the atom with the lower sorted position adds g (x) R~_ik to its
+ * own T_i (Eq. 4's G^T R~) and g (x) R~_ki to T_k with fp64 reductions.  Pass 2: one atom of the pair runs the value and
+ * tangent chains and applies the backward epilogue with its own dE/dT tile and with the neighbour's (read from memory);
+ * the pair force is f_ik - f_ki.  Only pairs whose two atoms are centres of the same chunk are shared; it is switched
+ * off on the device for an evaluation in which a neighbour was dropped by a full type section (n_overflow > 0), because
+ * the two lists are then not symmetric.  T is summed in a different (and, with the reductions, run-to-run varying)
+ * order: results move at the 1e-15 relative level.  Other precisions ignore it.
+ *   on = 0  off (both passes)
+ *   on = 1  (default) pass 2 always; pass 1 in evaluations that run as a single chunk (dpb_model_set_chunk): with several
+ *           chunks only the pairs inside a chunk can be shared and pass 1's bookkeeping (clearing T, every accumulation a
+ *           reduction) costs more than it saves (measured on the 864,000-atom box in 27 chunks)
+ *   on = 2  both passes always (pairs across a chunk boundary are evaluated in both directions)
  * Returns DPB_EINVAL for any other value. */
 int dpb_model_set_pair_reuse(dpb_model *model, int on);
 

@@ -27,7 +27,6 @@ unsigned long long g_dpb_launches = 0;
 
 // Auxiliary streams and events are per device (one process per GPU is the design, but a process that drives several
 // devices must not wait on another device's stream).
-#define DPB_MAX_DEVICES 32
 struct ForkState {
   cudaStream_t aux[DPB_MAX_TYPES];
   cudaEvent_t ev_fork, ev_join[DPB_MAX_TYPES];

@@ -104,6 +104,15 @@ cudaError_t launch_cell_images(int64_t n, const double *frac, const int *type, c
 cudaError_t launch_cell_fold(int64_t nall, int64_t n, const int *owner, const double *fall, double *force,
                              cudaStream_t st);
 
+// Per-device launch configuration: cudaFuncSetAttribute and the SM count belong to a device, so the "already done" flags
+// of the launchers are kept per device (a process that drives several GPUs creates models on each of them).
+#define DPB_MAX_DEVICES 32
+static inline int dpb_device() {
+  int d = 0;
+  if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= DPB_MAX_DEVICES) d = 0;
+  return d;
+}
+
 // Process-wide count of kernels launched by this library (reported by dpb_kernel_launches()).
 extern unsigned long long g_dpb_launches;
 #define DPB_LAUNCHED(n) (g_dpb_launches += (unsigned long long)(n))

@@ -963,7 +963,8 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 }
 
 // ---------------------------------------------------------------------------------------------------------
-static int g_sm_count = 0;
+static int g_sm_count_d[DPB_MAX_DEVICES] = {};      // per device
+#define g_sm_count (g_sm_count_d[dpb_device()])
 
 // Segments per atom (work items per atom and net): 1 when the chunk has enough atoms to give every warp of the GPU two
 // of them (counting all nets); up to 8 for small chunks (configs[0]: 192 atoms on 148 SMs x 8 warps).
@@ -979,8 +980,10 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
   const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P1_WARPS * L::tile1s);
   const size_t smem_ru = smem + sizeof(int) * 2 * (size_t)P.nm * P1_WARPS;
   const bool reuse = C.reuse && C.nlp && smem_ru <= 227 * 1024;
-  static bool configured = false;
-  static size_t configured_ru = 0;
+  static bool configured_d[DPB_MAX_DEVICES] = {};
+  bool &configured = configured_d[dpb_device()];
+  static size_t configured_ru_d[DPB_MAX_DEVICES] = {};
+  size_t &configured_ru = configured_ru_d[dpb_device()];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass1_dmma<SP, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -1026,7 +1029,8 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
                              cudaStream_t st) {
   using L = EL<SP>;
   const size_t smem = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * (L::tile2 + EMB_STG));
-  static bool configured = false;
+  static bool configured_d[DPB_MAX_DEVICES] = {};
+  bool &configured = configured_d[dpb_device()];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -1035,7 +1039,8 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
   using R = P2R<SP>;
   const size_t smem_ru = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * R::per_warp);
   const bool reuse = C.reuse2 && !C.fslot && C.nlp && C.dt_pad == 4 * SP && smem_ru <= 227 * 1024;
-  static bool configured_ru = false;
+  static bool configured_ru_d[DPB_MAX_DEVICES] = {};
+  bool &configured_ru = configured_ru_d[dpb_device()];
   if (reuse && !configured_ru) {
     cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_ru<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ru);
     if (e != cudaSuccess) return e;

@@ -520,13 +520,15 @@ k_pass1_tc(DevModel P, ChunkView C, const float *__restrict__ all_img, size_t ne
   if (warp == 0) tc::tmem_dealloc<512>(tmem);
 }
 
-static int g_tc_sms = 0;
+static int g_tc_sms_d[DPB_MAX_DEVICES] = {};        // per device
+#define g_tc_sms (g_tc_sms_d[dpb_device()])
 
 template <int S1>
 static cudaError_t run_pass1_tc(const DevModel &P, const ChunkView &C, const TCWeights &W, const int *off,
                                 const int *pidx, cudaStream_t st) {
   using L = TL<S1>;
-  static bool configured = false;
+  static bool configured_d[DPB_MAX_DEVICES] = {};
+  bool &configured = configured_d[dpb_device()];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass1_tc<S1>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::smem_bytes);
     if (e != cudaSuccess) return e;
@@ -888,7 +890,8 @@ template <int S1>
 static cudaError_t run_pass2_tc(const DevModel &P, const ChunkView &C, const TCWeights &W, const int *off,
                                 const int *pidx, const float *dT32, double *force, double *virial, cudaStream_t st) {
   using L = TL<S1>;
-  static bool configured = false;
+  static bool configured_d[DPB_MAX_DEVICES] = {};
+  bool &configured = configured_d[dpb_device()];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_pass2_tc<S1>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::smem_bytes);
     if (e != cudaSuccess) return e;

@@ -427,7 +427,8 @@ template <int WM, int NBW, int EPI, int FIT_BK = 16>
 static cudaError_t gemm_t(const ChunkView &C, int ty, const GemmArgs &g, cudaStream_t st, int splitk = 1) {
   constexpr int BN = 16 * NBW, FIT_BM = 16 * WM;
   const size_t smem = sizeof(double) * FIT_STAGES * (FIT_BM * (FIT_BK + 4) + FIT_BK * (BN + 4));
-  static bool configured = false;
+  static bool configured_d[DPB_MAX_DEVICES] = {};
+  bool &configured = configured_d[dpb_device()];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_fit_gemm<WM, NBW, EPI, FIT_BK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem);
@@ -487,7 +488,8 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
   // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint.  The
   // descriptor and dT kernels (memory-bound) belong to the chains: one species' run beside the other's GEMMs
   const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
-  static size_t configured = 0;
+  static size_t configured_d[DPB_MAX_DEVICES] = {};
+  size_t &configured = configured_d[dpb_device()];
   if (sm > 48 * 1024 && sm > configured) {
     e = cudaFuncSetAttribute(k_dT_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;

@@ -594,7 +594,8 @@ static cudaError_t ft_launch(const ChunkView &C, int ty, const FitTCArgs &g, int
   constexpr int STAGES = (STAGE * 3 <= 200 * 1024) ? 3 : ((STAGE * 2 <= 200 * 1024) ? 2 : 1);
   constexpr int smem = STAGES * STAGE + 128;
   static_assert(smem <= 227 * 1024, "stage does not fit");
-  static bool configured = false;
+  static bool configured_d[DPB_MAX_DEVICES] = {};
+  bool &configured = configured_d[dpb_device()];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_fit_tc<NT, EPI, OPF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;

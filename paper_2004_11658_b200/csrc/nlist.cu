@@ -346,7 +346,8 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
                          const NlRaw *raw) {
   if (C.n <= 0) return cudaSuccess;
   const size_t smem = (size_t)cap * (sizeof(NlHit) + 2 * sizeof(int)) + sizeof(int) * (3 * 18 * (size_t)P.ntypes * G.ngrp + 1);
-  static size_t configured = 0;
+  static size_t configured_d[DPB_MAX_DEVICES] = {};
+  size_t &configured = configured_d[dpb_device()];
   if (smem > 48 * 1024 && smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_nlist<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_nlist<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
