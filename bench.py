@@ -1,9 +1,13 @@
 #!/usr/bin/env python
 """bench.py — throughput of one DP energy / force / virial evaluation (the whole hot path, S1..S9) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload W24k|Cu32k|W192|Cu864k] [--variant 0|1]
-                    [--precision fp64|tf32]      # tf32 = BASELINE.json configs[3] (mixed precision, tcgen05 kernels)
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload W24k|Cu32k|W192|Cu864k] [--variant 0|1|2]
+                    [--precision fp64|tf32|bf16]   # tf32 / bf16 = BASELINE.json configs[3] (mixed precision, tcgen05 kernels)
     python bench.py --impl reference ...     # times the CPU oracle (the baseline arm) on a bounded sample
+
+The default run (W24k, fp64: the headline line) appends a `configs` object with short legs over every other
+BASELINE.json config (W192, Cu32k, W24k tf32 / bf16, Cu864k); --no-configs skips them.  --variant 2 adds a `strawman`
+object (the paper's own pipeline against the fused path).
 
 A "step" is one dpb_eval over one freshly perturbed copy of the workload's box (BASELINE.json config: positions
 perturbed by sigma = 0.01 A between calls, neighbour build included every call).  Inputs are resident in HBM for

@@ -2,6 +2,9 @@
 // One dpb_eval = S1 (cell sort) once, then for each chunk of atoms (sorted by type, then cell):
 //   S2 nlist -> S3-S5 pass 1 (T) -> S5-S7 fitting fwd/bwd (E_i, dT) -> S8-S9 pass 2 (F, virial); finally E = sum E_i.
 // Everything is enqueued on the caller's stream; no host synchronisation unless the caller asks for `info`.
+// The chunk size is automatic (effective_chunk); small evaluations are replayed from a CUDA graph (eval_graphed);
+// dpb_eval_cell builds lattice images and dispatches to the sub-region mode of run_eval; variant 2 (strawman.cu) is the
+// paper's padded-dense pipeline.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>

@@ -16,6 +16,11 @@
 // Pass 2 differentiates the embedding net in forward mode: its input is the scalar s(r), so the tangent row
 // h' = dh/dx runs through the same GEMM chain as the value row (second m-block, same B fragments), and
 //   dE/dx = sum_o (dT R~)[o] g'[o],   dE/dR~[c] = sum_o dT[o][c] g[o]          (O9 of DESIGN.md / SURVEY.md §8(c)).
+//
+// Kernels: k_pass1_dmma<SP, RB, RU> (RU: same-species pair reuse, T_j += g (x) R~_ji by fp64 reductions),
+// k_pass2_dmma<SP> and k_pass2_dmma_ru<SP> (pair reuse: the second direction reads dT_j slices staged by the TMA
+// engine).  One launch per net; a warp takes work items (atom, or a segment of an atom's rows for small chunks) from a
+// counter in global memory; the net's weights are staged by one TMA bulk copy per CTA.  DESIGN.md sections 6 and 12.
 #include "v1_kernels.cuh"
 #include "tc_common.cuh"
 
