@@ -548,6 +548,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.dt_rows = dt_pad ? 4 * dt_pad : P.M;
     C.nlp = m->nlp.as<int>();
     C.counters = m->counters.as<int>();
+    C.sub_part = 0; C.sub_nparts = 1;
     if (!nlist_only) CU(cudaMemsetAsync(C.counters, 0, sizeof(int) * 128, st), "memset counters");
     C.fslot = nullptr;
     C.pos_of = m->pos_of.as<int>();

@@ -73,6 +73,7 @@ struct ChunkView {
   // the atom with the lower sorted position evaluates the pair once and adds g (x) R~_ji to T_j with red.global.add.f64
   const int *pos_of;       // [N] sorted position of original atom index (nullptr: no reuse)
   const DevStats *stats;   // reuse is taken only while stats->n_overflow == 0 (a dropped neighbour breaks the symmetry)
+  int sub_part, sub_nparts; // the fitting kernels of one launch cover part sub_part of sub_nparts of a species' rows (default 0 of 1)
   int *counters;           // [128] work-item counters of the embedding launches (pass 1: net, pass 2: 64 + net), zeroed per chunk
   int reuse;               // pass 1
   int reuse2;              // pass 2 (k_pass2_dmma_ru): both directions of a same-species pair from one evaluation
@@ -171,6 +172,16 @@ __device__ __forceinline__ void dp_displacement(const double xi[3], const double
   }
   double r2 = __fma_rn(d[2], d[2], __fma_rn(d[1], d[1], __dmul_rn(d[0], d[0])));
   r = __dsqrt_rn(r2);
+}
+
+// Part `sub_part` of `sub_nparts` of the row range [lo, hi) of a species (cut at multiples of 32 rows from lo).
+__device__ __forceinline__ void dpb_sub_range(const ChunkView &C, int &lo, int &hi) {
+  if (C.sub_nparts <= 1) return;
+  const int n = hi > lo ? hi - lo : 0;
+  const int per = ((n + C.sub_nparts - 1) / C.sub_nparts + 31) / 32 * 32;
+  const int a = lo + C.sub_part * per, b = a + per;
+  lo = a < hi ? a : hi;
+  hi = (C.sub_part == C.sub_nparts - 1 || b > hi) ? hi : b;
 }
 
 // Offset (in doubles) of dT[q][b][0] in the chunk's dT buffer (layouts: ChunkView::dt_pad).

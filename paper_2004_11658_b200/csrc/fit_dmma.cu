@@ -68,7 +68,8 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
   extern __shared__ __align__(16) double smem[];
   double *As = smem;                                        // [STAGES][BM][LDA]
   double *Bs = smem + FIT_STAGES * FIT_BM * FIT_LDA;        // [STAGES][BK][LDB]
-  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
   const int m0 = row_lo + blockIdx.x * FIT_BM;
   if (m0 >= row_hi) return;
   const int n0 = blockIdx.y * BN;
@@ -196,7 +197,8 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
 __global__ void k_descr_v1(DevModel P, ChunkView C, int ty, int dimp, double *__restrict__ D) {
   const int q = blockIdx.x;
   {                                                         // one launch per species, on that species' stream
-    const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+    int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
     if (q < row_lo || q >= row_hi) return;
   }
   __shared__ double Ts[256 * 5 + 16];            // row stride 5 doubles: the 16 rows a = 0..15 hit 16 distinct bank pairs
@@ -219,7 +221,8 @@ __global__ void k_descr_v1(DevModel P, ChunkView C, int ty, int dimp, double *__
 __global__ void k_dT_v1(DevModel P, ChunkView C, int ty, int dimp, const double *__restrict__ dD) {
   const int q = blockIdx.x;
   {
-    const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+    int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
     if (q < row_lo || q >= row_hi) return;                  // (block-uniform: before any barrier)
   }
   extern __shared__ double sm2[];
@@ -265,7 +268,8 @@ __global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView
   const int q = blockIdx.x * DTV_WARPS + warp;
   if (q >= C.n) return;
   {                                                         // one launch per species, at the tail of that species' chain
-    const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+    int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
     if (q < row_lo || q >= row_hi) return;
   }
   const int M = P.M;
@@ -339,7 +343,8 @@ __global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView
 
 // Z0 = tanh(X + b0) in place, after a split-K G1 (small systems): rows of species ty.
 __global__ void k_bias_tanh_v1(ChunkView C, int ty, int fwp, const double *__restrict__ bias, double *__restrict__ Z) {
-  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
   const int q = row_lo + blockIdx.x;
   if (q >= row_hi) return;
   for (int o = threadIdx.x; o < fwp; o += blockDim.x) Z[(size_t)q * fwp + o] = dp_tanh(Z[(size_t)q * fwp + o] + bias[o]);
@@ -348,7 +353,8 @@ __global__ void k_bias_tanh_v1(ChunkView C, int ty, int fwp, const double *__res
 // E_i = Z2 . w3 + b3 (output layer, reading R4): one warp per atom.
 __global__ void k_rowdot_v1(ChunkView C, int ty, int fwp, const double *__restrict__ Z2, const double *__restrict__ w3,
                             double b3, double *__restrict__ atom_energy) {
-  const int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
   const int q = row_lo + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (q >= row_hi) return;
   const int lane = threadIdx.x & 31;
@@ -456,7 +462,7 @@ cudaError_t v1_plain_gemm(int64_t rows, const double *A, int lda, const double *
                           const double *Cin, double *Cout, int ldc, const int *range, cudaStream_t st) {
   if (rows <= 0) return cudaSuccess;
   ChunkView C{};
-  C.p0 = 0; C.n = (int)rows; C.type_start = range;
+  C.p0 = 0; C.n = (int)rows; C.type_start = range; C.sub_part = 0; C.sub_nparts = 1;
   GemmArgs g{A, lda, B, ldb, K, N, nullptr, Cin, nullptr, ldc, Cout, nullptr, ldc};
   if (N <= 32) return Cin ? gemm_t<2, 2, EPI_ADD>(C, 0, g, st) : gemm_t<2, 2, EPI_STORE>(C, 0, g, st);
   if (N <= 64) return Cin ? gemm_t<2, 4, EPI_ADD>(C, 0, g, st) : gemm_t<2, 4, EPI_STORE>(C, 0, g, st);
@@ -464,9 +470,10 @@ cudaError_t v1_plain_gemm(int64_t rows, const double *A, int lda, const double *
   return Cin ? gemm_t<2, 8, EPI_ADD>(C, 0, g, st) : gemm_t<2, 8, EPI_STORE>(C, 0, g, st);
 }
 
-cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, const double *fit, void *ws,
+cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, const double *fit, void *ws,
                    double *atom_energy, cudaStream_t st) {
   (void)fit;
+  const ChunkView &C = Cin;
   if (C.n <= 0) return cudaSuccess;
   const FitWeights *F = reinterpret_cast<const FitWeights *>(W.fit);
   if (!F) return cudaErrorNotSupported;
@@ -497,13 +504,21 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
   }
   const size_t sms = sizeof(double) * DTV_WARPS * 4 * ((size_t)P.M + 2 * P.Ma);
   const unsigned nbs = (unsigned)((C.n + DTV_WARPS - 1) / DTV_WARPS);
+  // A single-species system has no second chain to overlap with: its rows are split into two parts that run as two chains
+  // on forked streams (the memory-bound descriptor / dT kernels and the GEMM tails of one beside the GEMMs of the other:
+  // Cu32k fitting 3.52 -> 3.30 ms).  With two species the chains already overlap; splitting them further was measured
+  // and is slower (W24k 2.12 -> 2.17 ms in 2 parts, 2.28 in 4).
+  const int split = P.ntypes == 1 && C.n >= 4096 ? 2 : 1;
+  const int nbatch = P.ntypes * split;
   cudaStream_t ts[DPB_MAX_TYPES];
-  if ((e = dpb_fork_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
-  for (int k = 0; k < P.ntypes; ++k) {
-    const int ty = P.ntypes - 1 - k;
+  if ((e = dpb_fork_streams(nbatch, st, ts)) != cudaSuccess) return e;
+  for (int k = 0; k < nbatch; ++k) {
+    const int ty = P.ntypes - 1 - k / split, part = k % split;
     cudaStream_t s = ts[k];
     const FitNet &N = F->nets[ty];
     GemmArgs g;
+    ChunkView C = Cin;
+    C.sub_part = part; C.sub_nparts = split;
     k_descr_v1<<<C.n, 256, 0, s>>>(P, C, ty, dimp, D);
     DPB_LAUNCHED(1);
     // G1: Z0 = tanh(D W0 + b0).  Small systems: split-K over 8 CTAs (K = dim is a serial loop of dim / 16 tiles for
@@ -537,6 +552,6 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, co
     else k_dT_v1<<<C.n, 256, sm, s>>>(P, C, ty, dimp, dD);
     DPB_LAUNCHED(1);
   }
-  if ((e = dpb_join_streams(P.ntypes, st, ts)) != cudaSuccess) return e;
+  if ((e = dpb_join_streams(nbatch, st, ts)) != cudaSuccess) return e;
   return cudaGetLastError();
 }
