@@ -967,6 +967,337 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// Pass 2, row-stream kernel (every net; chunks large enough that a work item is a whole atom).  The kept rows of the atoms a
+// warp takes (pair reuse as in k_pass2_dmma_ru for a == t) form ONE stream of 8-row blocks: only the last block of a
+// WARP is ragged, not the last block of every atom and net (W24k: 8.6 % of the pass-2 rows were padding, Cu32k 4 %).
+// A block may therefore hold rows of two atoms (never more: it is cut short otherwise): the dE/dT slices of the (at
+// most two) centre atoms of a block come from L2 by the same TMA copies as the neighbours' slices, per N chunk, instead
+// of a per-atom tile in shared memory; F_i is added per row.
+template <int SP>
+struct P2S {
+  static constexpr int NBA = (SP + 1) / 2, NBB = SP - NBA;   // n-blocks of the two N chunks of a half (SP n-blocks)
+  static constexpr int SLICE = 32 * NBA + 16;                // doubles per staged row slice (+128 B: rows on distinct banks)
+  static constexpr int RING = 64;
+  // per warp: dT_i slices [2][SLICE] | dT_j slices [8][SLICE] | ring (d, r) [RING] | ring ints j, row of j, centre row, i [RING]
+  //           | mbarrier | staging of 32 raw slots: (d, r) [32], j [32], sorted position of j [32]
+  static constexpr int per_warp = 10 * SLICE + 4 * RING + 2 * RING + 2 + 4 * 32 + 16 + 16;
+};
+
+template <int SP, int NB, int NB0>
+__device__ __forceinline__ void p2s_chunk(const double *__restrict__ W2h, const double *__restrict__ b2h,
+                                          const double *__restrict__ irow, const double *__restrict__ jrow,
+                                          const bool anyboth, uint64_t *mbar, unsigned &parity,
+                                          const double (&h1v)[2 * SP], const double (&h1t)[2 * SP],
+                                          const double (&e)[4], const int g, const int q, double (&pr)[5],
+                                          double (&pj)[5]) {
+  using L = EL<SP>;
+  double av[2 * NB], at[2 * NB];
+#pragma unroll
+  for (int nb = 0; nb < NB; ++nb) {
+    const double2 bb = *reinterpret_cast<const double2 *>(b2h + 8 * (NB0 + nb) + 2 * q);
+    av[2 * nb] = bb.x; av[2 * nb + 1] = bb.y;
+    at[2 * nb] = 0.0; at[2 * nb + 1] = 0.0;
+  }
+#pragma unroll
+  for (int ks = 0; ks < 2 * SP; ++ks) {
+#pragma unroll
+    for (int nb = 0; nb < NB; ++nb) {
+      const double b = W2h[(4 * ks + q) * L::LD2 + 8 * (NB0 + nb) + g];
+      dmma884(av[2 * nb], av[2 * nb + 1], h1v[ks], b);
+      dmma884(at[2 * nb], at[2 * nb + 1], h1t[ks], b);
+    }
+  }
+  tc::mbar_wait(mbar, parity);                              // the slices of this chunk (dT_i always, dT_j if any) have landed
+  parity ^= 1u;
+#pragma unroll
+  for (int s = 0; s < 2 * NB; ++s) {
+    const int sl = 2 * NB0 + s;                             // slot inside the half: the skip comes from slot sl of layer 1
+    const double t2 = dp_tanh(av[s]);
+    const double gv = h1v[sl] + t2;
+    const double gp = fma(fma(-t2, t2, 1.0), at[s], h1t[sl]);
+    av[s] = gv; at[s] = gp;
+    const double4 d4 = *reinterpret_cast<const double4 *>(irow + 4 * (4 * s + q));
+    pr[0] = fma(d4.x, gv, pr[0]);
+    pr[1] = fma(d4.y, gv, pr[1]);
+    pr[2] = fma(d4.z, gv, pr[2]);
+    pr[3] = fma(d4.w, gv, pr[3]);
+    const double dg = fma(d4.x, e[0], fma(d4.y, e[1], fma(d4.z, e[2], d4.w * e[3])));
+    pr[4] = fma(dg, gp, pr[4]);
+  }
+  if (anyboth) {                                            // direction j -> i: dT_j, R~_ji = (s, -s d/r)
+#pragma unroll
+    for (int s = 0; s < 2 * NB; ++s) {
+      const double4 d4 = *reinterpret_cast<const double4 *>(jrow + 4 * (4 * s + q));
+      pj[0] = fma(d4.x, av[s], pj[0]);
+      pj[1] = fma(d4.y, av[s], pj[1]);
+      pj[2] = fma(d4.z, av[s], pj[2]);
+      pj[3] = fma(d4.w, av[s], pj[3]);
+      const double dg = fma(d4.x, e[0], -fma(d4.y, e[1], fma(d4.z, e[2], d4.w * e[3])));
+      pj[4] = fma(dg, at[s], pj[4]);
+    }
+  }
+}
+
+template <int SP>
+__global__ void __launch_bounds__((32 * P2_WARPS), 1)
+k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
+                double *__restrict__ virial, int *counter) {
+  using L = EL<SP>;
+  using R = P2S<SP>;
+  extern __shared__ __align__(16) double smem[];
+  double *W = smem;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
+  double *ibuf = smem + ((L::total + 1) & ~1) + warp * R::per_warp;     // [2][SLICE] dT slices of the block's centre atoms
+  double *jbuf = ibuf + 2 * R::SLICE;                                   // [8][SLICE] dT slices of the rows' neighbours
+  double4 *rdv = reinterpret_cast<double4 *>(jbuf + 8 * R::SLICE);      // ring of kept rows: (d, r)
+  int *rjn = reinterpret_cast<int *>(rdv + R::RING);                    //   input index of the neighbour
+  int *rqj = rjn + R::RING;                                             //   its row in this chunk when both directions run, else -1
+  int *rqa = rqj + R::RING;                                             //   row of the centre atom in this chunk
+  int *rio = rqa + R::RING;                                             //   input index of the centre atom
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(rio + R::RING);
+  double4 *sdr = reinterpret_cast<double4 *>(mbar + 2);                 // staged raw slots (cp.async, one batch ahead)
+  int *snl = reinterpret_cast<int *>(sdr + 32);
+  int *snlp = snl + 32;
+  __shared__ double vred[P2_WARPS][9];
+  __shared__ uint64_t wbar;
+  if (lane == 0) tc::mbar_init(mbar, 1);
+  tc::fence_mbar_init();
+  stage_net(W, netp, L::total, &wbar);
+  const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
+               *b2p = W + L::ob2;
+  const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
+  const bool ru = a == t && C.stats->n_overflow == 0ull;
+  const size_t dt_tile = (size_t)C.dt_rows * 4;
+  unsigned parity = 0;
+  double vir[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) vir[k] = 0.0;
+
+  // The ring of kept rows lives across work items: a warp takes one atom at a time from the counter (fine-grained, for the
+  // tail of the launch), and the rows an atom leaves over (< 8) are computed together with the first rows of the warp's
+  // next atom, whichever that is — rows carry their centre atom.  Only the last block of a WARP is ragged.
+  const int natom = max(row_hi - row_lo, 0);
+  int head = 0, cnt = 0;
+  int qa = 0, n = 0, io = 0, rawpos = 0, sweep = 1;      // the atom being swept: chunk row, real slots, input index
+  bool have = false, nomore = false;
+  {
+    // next atom with rows, or nomore
+    auto next_atom = [&]() {
+      have = false;
+      while (!nomore && !have) {
+        const int item = next_item(counter, lane);
+        if (item >= natom) { nomore = true; break; }
+        qa = row_lo + item;
+        n = C.nreal[(size_t)qa * P.ntypes + t];
+        if (n > 0) { io = C.s_idx[C.p0 + qa]; rawpos = 0; sweep = ru ? 0 : 1; have = true; }
+      }
+    };
+    // one batch of 32 raw slots of the current atom: global -> shared (cp.async), kept rows -> ring
+    auto batch = [&]() {
+      const int slot = rawpos + lane;
+      if (slot < n) {
+        const size_t o = (size_t)qa * P.nm + P.sec_start[t] + slot;
+        emb_cp16(sdr + lane, C.dr + o);
+        emb_cp16(reinterpret_cast<double *>(sdr + lane) + 2, reinterpret_cast<const double *>(C.dr + o) + 2);
+        emb_cp4(snl + lane, C.nl + o);
+        emb_cp4(snlp + lane, C.nlp + o);
+      }
+      emb_cp_commit();
+      emb_cp_wait<0>();
+      __syncwarp();
+      bool keep = false;
+      int qj = -1;
+      if (slot < n) {
+        if (ru) {
+          const int pj = snlp[lane] - C.p0;
+          const bool inchunk = pj >= 0 && pj < C.n;
+          // sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs
+          if (sweep == 0) { keep = inchunk && ((((qa + pj) & 1) == 0) == (qa < pj)); qj = pj; }
+          else keep = !inchunk;
+        } else {
+          keep = true;
+        }
+      }
+      const unsigned mk = __ballot_sync(0xffffffffu, keep);
+      if (keep) {
+        const int pos = (head + cnt + __popc(mk & ((1u << lane) - 1u))) & (R::RING - 1);
+        rdv[pos] = sdr[lane]; rjn[pos] = snl[lane]; rqj[pos] = qj; rqa[pos] = qa; rio[pos] = io;
+      }
+      cnt += __popc(mk);
+      __syncwarp();
+      rawpos += 32;
+      if (rawpos >= n) {
+        if (ru && sweep == 0) { sweep = 1; rawpos = 0; } else have = false;
+      }
+    };
+    auto fill = [&]() {
+      while (cnt < 16 && !nomore) {
+        if (!have) { next_atom(); continue; }
+        batch();
+      }
+    };
+    // the block at the ring head: its rows (at most 8, of at most two atoms), which of them run both directions, and
+    // (lanes 0..7) the neighbour row, (lanes 8, 9) the centre rows whose dT slices the TMA fetches
+    int nrows = 0, myrow = -1, islot = 0;
+    unsigned bmask = 0;
+    auto block_setup = [&]() {
+      const int avail = min(cnt, 8);
+      const int rq = lane < avail ? rqa[(head + lane) & (R::RING - 1)] : -1;
+      const int a0 = __shfl_sync(0xffffffffu, rq, 0);
+      const unsigned m0 = __ballot_sync(0xffffffffu, lane < avail && rq == a0);
+      const unsigned rest = ((1u << avail) - 1u) & ~m0;
+      int a1 = -1;
+      unsigned m1 = 0;
+      if (rest) {
+        a1 = __shfl_sync(0xffffffffu, rq, __ffs(rest) - 1);
+        m1 = __ballot_sync(0xffffffffu, lane < avail && rq == a1);
+      }
+      nrows = __popc(m0 | m1);                              // rows are ordered by atom: a prefix of the ring
+      const int qjl = lane < nrows ? rqj[(head + lane) & (R::RING - 1)] : -1;
+      bmask = __ballot_sync(0xffffffffu, qjl >= 0);
+      myrow = qjl;                                          // lanes 0..7: row of the neighbour (or -1)
+      if (lane == 8) myrow = nrows > 0 ? a0 : -1;
+      if (lane == 9) myrow = a1;
+      const int rqg = __shfl_sync(0xffffffffu, rq, g);      // centre row of this thread's tile row
+      islot = (g < nrows && rqg == a1) ? 1 : 0;
+    };
+    auto issue = [&](const int k) {                         // N chunk k (0..3) of the block at the ring head
+      if (nrows == 0) return;
+      const int slot0 = (k >> 1) * 2 * SP + ((k & 1) ? 2 * R::NBA : 0);
+      const unsigned bytes = ((k & 1) ? R::NBB : R::NBA) * 256u;
+      const unsigned want = __ballot_sync(0xffffffffu, lane < 10 && myrow >= 0);
+      if (lane == 0) tc::mbar_arrive_expect_tx(mbar, (unsigned)__popc(want) * bytes);
+      __syncwarp();
+      if (lane < 10 && myrow >= 0) {
+        double *dst = lane < 8 ? jbuf + lane * R::SLICE : ibuf + (lane - 8) * R::SLICE;
+        tc::bulk_g2s(dst, C.dT + (size_t)myrow * dt_tile + 16 * slot0, bytes, mbar);
+      }
+    };
+    fill();
+    block_setup();
+    issue(0);
+
+    while (cnt > 0) {
+      const int nr = nrows;
+      const bool valid = g < nr;
+      const bool both = (bmask >> g) & 1u;
+      const bool anyboth = bmask != 0u;
+      double e[4] = {0.0, 0.0, 0.0, 0.0};
+      double4 dv = make_double4(0.0, 0.0, 0.0, 1.0);
+      int jn = 0, ri_io = 0;
+      if (valid) {
+        const int ri = (head + g) & (R::RING - 1);
+        dv = rdv[ri]; jn = rjn[ri]; ri_io = rio[ri];
+        env_row4(P, dv, e);
+      }
+      double h0v[SP], h0t[SP];
+#pragma unroll
+      for (int s = 0; s < SP; ++s) {
+        const double w0 = W0p[4 * s + q], bb = b0p[4 * s + q];
+        const double t0 = dp_tanh(fma(e[0], w0, bb));
+        h0v[s] = t0;
+        h0t[s] = fma(-t0, t0, 1.0) * w0;
+      }
+      double h1v[2 * SP], h1t[2 * SP];
+#pragma unroll
+      for (int nb = 0; nb < L::NB1; ++nb) {
+        const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
+        h1v[2 * nb] = bb.x; h1v[2 * nb + 1] = bb.y;
+        h1t[2 * nb] = 0.0; h1t[2 * nb + 1] = 0.0;
+      }
+#pragma unroll
+      for (int ks = 0; ks < SP; ++ks) {
+#pragma unroll
+        for (int nb = 0; nb < L::NB1; ++nb) {
+          const double b = W1p[(4 * ks + q) * L::LD1 + 8 * nb + g];
+          dmma884(h1v[2 * nb], h1v[2 * nb + 1], h0v[ks], b);
+          dmma884(h1t[2 * nb], h1t[2 * nb + 1], h0t[ks], b);
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < 2 * SP; ++s) {
+        const double t1 = dp_tanh(h1v[s]);
+        h1v[s] = h0v[s % SP] + t1;
+        h1t[s] = fma(fma(-t1, t1, 1.0), h1t[s], h0t[s % SP]);
+      }
+      double pr[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      double pj[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      const double *irow = ibuf + islot * R::SLICE, *jrow = jbuf + g * R::SLICE;
+#pragma unroll 1
+      for (int half = 0; half < 2; ++half) {
+        const double *W2h = W2p + 8 * half * SP, *b2h = b2p + 8 * half * SP;
+        p2s_chunk<SP, R::NBA, 0>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, e, g, q, pr, pj);
+        __syncwarp();
+        issue(2 * half + 1);
+        if (R::NBB > 0) p2s_chunk<SP, R::NBB, R::NBA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, e, g, q, pr, pj);
+        __syncwarp();
+        if (half == 0) issue(2);
+      }
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        pr[k] += __shfl_xor_sync(0xffffffffu, pr[k], 1);
+        pr[k] += __shfl_xor_sync(0xffffffffu, pr[k], 2);
+      }
+      if (anyboth) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+          pj[k] += __shfl_xor_sync(0xffffffffu, pj[k], 1);
+          pj[k] += __shfl_xor_sync(0xffffffffu, pj[k], 2);
+        }
+      }
+      head = (head + nr) & (R::RING - 1);
+      cnt -= nr;
+      fill();
+      block_setup();
+      issue(0);
+      if (valid && q == 0) {
+        const double r = dv.w, ir = 1.0 / r;
+        double w, dw;
+        dp_switch(r, P.rcs, P.rc, w, dw);
+        const double s = w * ir, qq = s * ir;
+        const double sp = dw * ir - w * ir * ir;
+        const double qp = sp * ir - s * ir * ir;
+        const double dot = pr[1] * dv.x + pr[2] * dv.y + pr[3] * dv.z;
+        const double cm = ((pr[0] + pr[4]) * sp + qp * dot) * ir;
+        double f0 = fma(cm, dv.x, qq * pr[1]), f1 = fma(cm, dv.y, qq * pr[2]), f2 = fma(cm, dv.z, qq * pr[3]);
+        if (both) {
+          const double dotj = -(pj[1] * dv.x + pj[2] * dv.y + pj[3] * dv.z);
+          const double cmj = ((pj[0] + pj[4]) * sp + qp * dotj) * ir;
+          f0 -= fma(-cmj, dv.x, qq * pj[1]);
+          f1 -= fma(-cmj, dv.y, qq * pj[2]);
+          f2 -= fma(-cmj, dv.z, qq * pj[3]);
+        }
+        if (force) {
+          atomicAdd(&force[3 * (size_t)jn + 0], -f0);
+          atomicAdd(&force[3 * (size_t)jn + 1], -f1);
+          atomicAdd(&force[3 * (size_t)jn + 2], -f2);
+          atomicAdd(&force[3 * (size_t)ri_io + 0], f0);
+          atomicAdd(&force[3 * (size_t)ri_io + 1], f1);
+          atomicAdd(&force[3 * (size_t)ri_io + 2], f2);
+        }
+        vir[0] -= dv.x * f0; vir[1] -= dv.x * f1; vir[2] -= dv.x * f2;
+        vir[3] -= dv.y * f0; vir[4] -= dv.y * f1; vir[5] -= dv.y * f2;
+        vir[6] -= dv.z * f0; vir[7] -= dv.z * f1; vir[8] -= dv.z * f2;
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 9; ++k) {
+    double v = vir[k];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if (lane == 0) vred[warp][k] = v;
+  }
+  __syncthreads();
+  if (tid < 9 && virial) {
+    double v = 0.0;
+    for (int w = 0; w < P2_WARPS; ++w) v += vred[w][tid];
+    atomicAdd(&virial[tid], v);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 static int g_sm_count_d[DPB_MAX_DEVICES] = {};      // per device
 #define g_sm_count (g_sm_count_d[dpb_device()])
@@ -1052,6 +1383,17 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     configured_ru = true;
   }
   const int nseg = C.fslot ? 1 : seg_count(C.n, P2_WARPS, P.ntypes * P.ntypes);
+  using S = P2S<SP>;
+  const size_t smem_st = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * S::per_warp);
+  // the row-stream kernel serves every net when an item is a run of whole atoms (no row segments, no per-slot output)
+  const bool stream = reuse && nseg == 1 && smem_st <= 227 * 1024;
+  static bool configured_st_d[DPB_MAX_DEVICES] = {};
+  bool &configured_st = configured_st_d[dpb_device()];
+  if (stream && !configured_st) {
+    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_st<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_st);
+    if (e != cudaSuccess) return e;
+    configured_st = true;
+  }
   const int grid = (int)min((long long)g_sm_count, ((long long)C.n * nseg + P2_WARPS - 1) / P2_WARPS);
   // the nets are independent here (forces and virial are atomic sums, slot stores are disjoint): a stream per net, so
   // that the tail of every launch is filled by the others
@@ -1063,11 +1405,10 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     for (int t = P.ntypes - 1; t >= 0; --t) {
       const int net = a * P.ntypes + t;
       cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
-#ifdef EXP_RU_AS_PLAIN
-      if (reuse)
-#else
-      if (reuse && a == t)
-#endif
+      if (stream)
+        k_pass2_dmma_st<SP><<<grid, (32 * P2_WARPS), smem_st, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
+                                                                     virial, C.counters + 64 + net);
+      else if (reuse && a == t)
         k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
                                                                      virial, nseg, C.counters + 64 + net);
       else
