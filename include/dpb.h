@@ -111,7 +111,10 @@ int dpb_model_set_variant(dpb_model *model, int variant);
  * atomics, so two evaluations of the same input agree bit for bit (the paper reports E / F / virial reproducible to
  * 15 / 10 / 13 digits; the default atomics mode differs at the 1e-16 relative level from run to run).
  * Costs about N * Nm * 28 bytes of extra workspace and one gather kernel.  Exact only when no neighbour was dropped
- * by a full type section (info.n_overflow == 0).  Other precisions / variants: dpb_eval returns DPB_ENOTIMPL. */
+ * by a full type section (info.n_overflow == 0).  Other precisions / variants: dpb_eval returns DPB_ENOTIMPL.
+ * dpb_eval_local and dpb_eval_cell take part: the formatted lists of the ghost atoms are built as well (list only; by
+ * the same symmetry a ghost's list names the local atoms whose lists contain it), N above is then nall, and n_overflow
+ * also counts neighbours dropped from a ghost's list.  dpb_eval_cell lays out and folds its images in a fixed order. */
 int dpb_model_set_deterministic(dpb_model *model, int on);
 
 /* CUDA-graph replay of dpb_eval (calls with info == NULL and the stage timers off).  The first call with a given set of
@@ -145,7 +148,9 @@ int dpb_model_set_pair_reuse(dpb_model *model, int on);
  *     atom_virial[i][a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b],     sum_i atom_virial[i] = virial of dpb_eval.
  * atom_virial: DEVICE fp64 [N][9] that the following dpb_eval calls fill (indexed by the input atom order), or NULL to
  * switch the output off.  The caller owns the buffer and keeps it alive.  Produced by the gather of the deterministic
- * reduction: dpb_eval returns DPB_ENOTIMPL while a buffer is set and dpb_model_set_deterministic is off. */
+ * reduction: dpb_eval returns DPB_ENOTIMPL while a buffer is set and dpb_model_set_deterministic is off.
+ * dpb_eval_local fills the rows of the nloc local atoms only ([nloc][9]; the terms of an atom's own neighbourhood, ghost
+ * neighbours included), dpb_eval_cell the rows of the N atoms of the cell. */
 int dpb_model_set_atom_virial(dpb_model *model, double *atom_virial);
 
 /* One evaluation (the paper's problem statement: coordinates, types and box in; E, E_i, F_i and the virial out).
@@ -197,7 +202,7 @@ int dpb_eval_host(dpb_model *model, void *stream, int64_t natoms, const double *
  *   virial       DEVICE fp64 [9]       the local atoms' part, -sum_{i<nloc} sum_k d_ik (x) dE_i/dd_ik
  *   nlist        DEVICE int32 [nloc][Nm], indices into [0, nall)
  * Summed over the sub-regions of a periodic system (ghost forces added to their owners) the outputs equal dpb_eval's.
- * Ownership, asynchrony and info as for dpb_eval.  Not available with the deterministic reduction (DPB_ENOTIMPL). */
+ * Ownership, asynchrony and info as for dpb_eval. */
 int dpb_eval_local(dpb_model *model, void *stream, int64_t nloc, int64_t nall, const double *coord,
                    const int32_t *type, const double bounds[6], double *energy, double *atom_energy, double *force,
                    double *virial, int32_t *nlist, dpb_eval_info *info);
@@ -212,8 +217,9 @@ int dpb_eval_local(dpb_model *model, void *stream, int64_t nloc, int64_t nall, c
  *   coord, type  DEVICE, [N][3] / [N]; raw positions (wrapped internally)
  *   energy [1], atom_energy [N], force [N][3], virial [9]: DEVICE, as dpb_eval (any may be NULL)
  *   info         HOST or NULL; n_real_pairs etc. refer to the N atoms of the cell
- * One host synchronisation (the number of images sizes the evaluation), otherwise asynchronous on `stream`.
- * Not available with the deterministic reduction (DPB_ENOTIMPL). */
+ * One host synchronisation (the number of images sizes the evaluation), otherwise asynchronous on `stream`.  An atom's
+ * images take consecutive rows in shift order and are folded back in that order, so the result does not depend on the
+ * scheduling (bitwise reproducible together with dpb_model_set_deterministic). */
 int dpb_eval_cell(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,
                   const double cell[9], double *energy, double *atom_energy, double *force, double *virial,
                   dpb_eval_info *info);

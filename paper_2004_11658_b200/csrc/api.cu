@@ -145,7 +145,7 @@ struct dpb_model {
   // deterministic mode: inverse of s_idx, full-size lists, per-slot dE_i/dd_ik, per-atom virial parts
   Buf pos_of, nl_all, nreal_all, fslot, vpart;
   Buf md_raw, md_nraw, md_xyz0, md_force, md_scal, md_mass;
-  Buf cell_frac, cell_x, cell_t, cell_owner, cell_f, cell_cnt;   // dpb_eval_cell: local + image atoms
+  Buf cell_frac, cell_x, cell_t, cell_off, cell_f;   // dpb_eval_cell: local + image atoms
   int md_cap_raw = 0;
   double md_skin = 0.0;
   DevGrid md_grid;
@@ -218,7 +218,7 @@ extern "C" int dpb_model_create(const dpb_model_desc *d, int precision, dpb_mode
   const size_t fb = sizeof(double) * (size_t)P.fit_net_size * P.ntypes;
   cudaError_t e = m->emb.reserve(eb);
   if (e == cudaSuccess) e = m->fit.reserve(fb);
-  if (e == cudaSuccess) e = m->stats.reserve(sizeof(DevStats));
+  if (e == cudaSuccess) e = m->stats.reserve(2 * sizeof(DevStats));      // [1]: ghost rows of the deterministic local mode
   if (e == cudaSuccess) e = cudaMemcpy(m->emb.p, d->emb_weights, eb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(m->fit.p, d->fit_weights, fb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = v1_prepare_weights(P, d->emb_weights, d->fit_weights, m->v1);
@@ -247,7 +247,7 @@ extern "C" int dpb_model_destroy(dpb_model *m) {
                 &m->nl, &m->nlp, &m->dr, &m->v2ws, &m->counters, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
                 &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
                 &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass,
-                &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_owner, &m->cell_f, &m->cell_cnt};
+                &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_off, &m->cell_f};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
@@ -446,7 +446,6 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   const bool det = m->deterministic && !nlist_only;
   if (det && (m->precision != DPB_FP64 || m->variant != 1 || !m->v1.ready))
     return fail(DPB_ENOTIMPL, "the deterministic reduction is built for DPB_FP64, variant 1");
-  if (det && nloc >= 0) return fail(DPB_ENOTIMPL, "the deterministic reduction is built for the periodic box");
   if (m->atom_virial && !nlist_only && !det)
     return fail(DPB_ENOTIMPL, "the per-atom virial comes from the deterministic reduction: switch it on "
                               "(dpb_model_set_deterministic) or clear the buffer");
@@ -458,10 +457,14 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     CU(m->vpart.reserve(sizeof(double) * 9 * (size_t)(N + 1)), "workspace");
   }
   int dt_pad = 0;
+  // deterministic sub-region mode: the ghosts' lists are built too (list only), in chunks of their own
+  const int64_t nghost = (det && nloc > 0) ? natoms - nloc : 0;
+  const int64_t gchunk = chunk_cap < nghost ? chunk_cap : nghost;
+  const int64_t lrows = chunk > gchunk ? chunk : gchunk;
   CU(m->nl.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
-  CU(m->nlp.reserve(sizeof(int) * (size_t)chunk * P.nm), "workspace");
+  CU(m->nlp.reserve(sizeof(int) * (size_t)lrows * P.nm), "workspace");
   CU(m->counters.reserve(sizeof(int) * 128), "workspace");
-  CU(m->dr.reserve(sizeof(double4) * (size_t)chunk * P.nm), "workspace");
+  CU(m->dr.reserve(sizeof(double4) * (size_t)lrows * P.nm), "workspace");
   CU(m->nreal.reserve(sizeof(int) * (size_t)chunk * P.ntypes), "workspace");
   if (!nlist_only) {
     CU(m->T.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
@@ -486,7 +489,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     }
   }
   DevStats *stats = m->stats.as<DevStats>();
-  if (nl_mode == 0) CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");   // MD: kept over the run
+  if (nl_mode == 0) CU(cudaMemsetAsync(stats, 0, 2 * sizeof(DevStats), st), "memset stats");   // MD: kept over the run
   NlRaw raw{};
   if (nl_mode != 0) {
     raw.raw = m->md_raw.as<int>(); raw.nraw = m->md_nraw.as<int>(); raw.cap = m->md_cap_raw;
@@ -604,8 +607,24 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
     }
   }
-  if (det)
-    CU(launch_force_gather(P, G, natoms, m->s_idx.as<int>(), m->pos_of.as<int>(), start + nkeys + 1,
+  for (int64_t p0 = nloc; nghost > 0 && p0 < natoms; p0 += gchunk) {      // ghost rows of the full-size list
+    ChunkView C{};
+    C.p0 = (int)p0;
+    C.n = (int)((natoms - p0) < gchunk ? (natoms - p0) : gchunk);
+    C.s_idx = m->s_idx.as<int>();
+    C.type_start = start + nkeys + 1;
+    C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
+    C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;
+    C.dr = m->dr.as<double4>();
+    C.nlp = m->nlp.as<int>();
+    C.pos_of = m->pos_of.as<int>();
+    C.sub_nparts = 1;
+    C.stats = stats + 1;
+    CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nullptr, stats + 1, st, 0, nullptr), "nlist of the ghosts");
+  }
+  if (nghost > 0) CU(launch_merge_ghost_stats(stats, st), "ghost statistics");
+  if (det && ncentre > 0)
+    CU(launch_force_gather(P, G, natoms, ncentre, m->s_idx.as<int>(), m->pos_of.as<int>(), start + nkeys + 1,
                            m->s_xyz.as<double>(), m->nl_all.as<int>(), m->nreal_all.as<int>(), m->fslot.as<double>(),
                            force, m->atom_virial ? m->atom_virial : m->vpart.as<double>(), virial, st),
        "deterministic force gather");
@@ -779,27 +798,26 @@ extern "C" int dpb_eval_cell(dpb_model *m, void *stream, int64_t natoms, const d
     }
   }
   for (int c = 0; c < 3; ++c) { bounds[c] -= 1e-9 * (1.0 + big); bounds[3 + c] += 1e-9 * (1.0 + big); }
-  const long long cap = natoms * (nshift - 1);
-  if (natoms + cap > 2000000000ll) return fail(DPB_EINVAL, "dpb_eval_cell: too many lattice images (%lld)", cap);
-  const size_t rows = (size_t)(natoms + cap) + 1;
   CU(m->cell_frac.reserve(sizeof(double) * 3 * ((size_t)natoms + 1)), "cell workspace");
-  CU(m->cell_x.reserve(sizeof(double) * 3 * rows), "cell workspace");
-  CU(m->cell_t.reserve(sizeof(int) * rows), "cell workspace");
-  CU(m->cell_owner.reserve(sizeof(int) * rows), "cell workspace");
-  CU(m->cell_f.reserve(sizeof(double) * 3 * rows), "cell workspace");
-  CU(m->cell_cnt.reserve(16), "cell workspace");
-  CU(launch_cell_wrap(natoms, coord, type, G, m->cell_frac.as<double>(), m->cell_x.as<double>(), m->cell_t.as<int>(),
-                      m->cell_owner.as<int>(), st), "cell wrap");
-  CU(launch_cell_images(natoms, m->cell_frac.as<double>(), type, G, cap, m->cell_x.as<double>(), m->cell_t.as<int>(),
-                        m->cell_owner.as<int>(), m->cell_cnt.as<unsigned long long>(), st), "cell images");
-  unsigned long long nimg = 0;                             // the number of images sizes the evaluation: one host sync
-  CU(cudaMemcpyAsync(&nimg, m->cell_cnt.p, sizeof(nimg), cudaMemcpyDeviceToHost, st), "image count");
+  CU(m->cell_off.reserve(sizeof(int) * ((size_t)natoms + 1)), "cell workspace");
+  int *off = m->cell_off.as<int>();
+  CU(launch_cell_wrap(natoms, coord, G, m->cell_frac.as<double>(), st), "cell wrap");
+  CU(launch_cell_images(natoms, m->cell_frac.as<double>(), type, G, off, nullptr, nullptr, 0, st), "cell image count");
+  int nimg = 0;                                            // the number of images sizes the evaluation: one host sync
+  CU(cudaMemcpyAsync(&nimg, off + natoms, sizeof(int), cudaMemcpyDeviceToHost, st), "image count");
   CU(cudaStreamSynchronize(st), "stream synchronise");
   const int64_t nall = natoms + (int64_t)nimg;
+  if (nall > 2000000000ll - 1)                             // (k_cell_scan saturates the count at 2e9)
+    return fail(DPB_EINVAL, "dpb_eval_cell: too many lattice images (at least %lld)", (long long)nimg);
+  CU(m->cell_x.reserve(sizeof(double) * 3 * ((size_t)nall + 1)), "cell workspace");
+  CU(m->cell_t.reserve(sizeof(int) * ((size_t)nall + 1)), "cell workspace");
+  CU(m->cell_f.reserve(sizeof(double) * 3 * ((size_t)nall + 1)), "cell workspace");
+  CU(launch_cell_images(natoms, m->cell_frac.as<double>(), type, G, off, m->cell_x.as<double>(), m->cell_t.as<int>(), 1,
+                        st), "cell images");
   int rc = run_eval(m, st, nall, m->cell_x.as<double>(), m->cell_t.as<int>(), bounds, energy, atom_energy,
                     force ? m->cell_f.as<double>() : nullptr, virial, nullptr, false, 0, natoms);
   if (rc != DPB_OK) return rc;
-  if (force) CU(launch_cell_fold(nall, natoms, m->cell_owner.as<int>(), m->cell_f.as<double>(), force, st), "cell fold");
+  if (force) CU(launch_cell_fold(natoms, off, m->cell_f.as<double>(), force, st), "cell fold");
   if (info) return finish_info(m, st, natoms, info);
   return DPB_OK;
 }

@@ -98,12 +98,12 @@ struct CellGeom {
   double margin[3];          // r_c / h_c, h_c = perpendicular height of the cell along lattice direction c
   int nshell[3];             // ceil(r_c / h_c) image shells
 };
-cudaError_t launch_cell_wrap(int64_t n, const double *coord, const int *type, const CellGeom &G, double *frac,
-                             double *xall, int *tall, int *owner, cudaStream_t st);
-cudaError_t launch_cell_images(int64_t n, const double *frac, const int *type, const CellGeom &G, int64_t cap,
-                               double *xall, int *tall, int *owner, unsigned long long *count, cudaStream_t st);
-cudaError_t launch_cell_fold(int64_t nall, int64_t n, const int *owner, const double *fall, double *force,
-                             cudaStream_t st);
+cudaError_t launch_cell_wrap(int64_t n, const double *coord, const CellGeom &G, double *frac, cudaStream_t st);
+// fill = 0: off[i] = first image row of atom i (relative to row n), off[n] = number of images; fill = 1: write the rows
+// (the wrapped atoms in rows [0, n), their images behind them)
+cudaError_t launch_cell_images(int64_t n, const double *frac, const int *type, const CellGeom &G, int *off, double *xall,
+                               int *tall, int fill, cudaStream_t st);
+cudaError_t launch_cell_fold(int64_t n, const int *off, const double *fall, double *force, cudaStream_t st);
 
 // Per-device launch configuration: cudaFuncSetAttribute and the SM count belong to a device, so the "already done" flags
 // of the launchers are kept per device (a process that drives several GPUs creates models on each of them).
@@ -123,7 +123,8 @@ cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
                              DevStats *stats, cudaStream_t st, int *pos_of = nullptr);
 // deterministic force / virial reduction (det.cu)
-cudaError_t launch_force_gather(const DevModel &P, const DevGrid &G, int64_t natoms, const int *s_idx, const int *pos_of,
+cudaError_t launch_merge_ghost_stats(DevStats *stats, cudaStream_t st);
+cudaError_t launch_force_gather(const DevModel &P, const DevGrid &G, int64_t natoms, int64_t nloc, const int *s_idx, const int *pos_of,
                                 const int *type_start, const double *s_xyz, const int *nl_all, const int *nreal_all,
                                 const double *fslot, double *force, double *vpart, double *virial, cudaStream_t st);
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,

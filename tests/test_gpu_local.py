@@ -139,10 +139,53 @@ def test_isolated_cluster_and_degenerate_cases():
     bad[3] -= 1.0
     with pytest.raises(pk.DPBError):
         _gpu_local(m, x, types, 50, bad)
-    # sub-region mode and the deterministic reduction do not combine
+    # the same degenerate cases with the deterministic reduction
     m.set_deterministic(True)
-    with pytest.raises(pk.DPBError):
-        _gpu_local(m, x, types, 50, bounds)
+    _check(ref, _gpu_local(m, x, types, 50, bounds), 0)
+    got0 = _gpu_local(m, x, types, 0, bounds)
+    assert got0["energy"][0] == 0.0 and not got0["force"].any() and not got0["virial"].any()
+    one = _gpu_local(m, x[:1], types[:1], 1, np.concatenate([x[0], x[0]]))
+    assert abs(one["energy"][0] - ref1["energy"]) <= 1e-10 * max(1.0, abs(ref1["energy"])) and not one["force"].any()
+    m.set_deterministic(False)
+
+
+@pytest.mark.parametrize("chunk", [0, 40])
+def test_deterministic_reduction_in_subregions(chunk):
+    """Deterministic reduction + per-atom virial in sub-region mode (the ghosts' lists are built too and name, by the
+    list symmetry, the local atoms that push on each ghost): W192 in 2 x 2 x 2 bricks against the oracle's
+    dpo_eval_local, ghost forces included; two runs agree bit for bit; the per-atom virial of a brick's local atoms
+    equals the periodic box's dpo_atom_virial of the same atoms and sums to the brick's virial.  chunk = 40: local and
+    ghost rows in several chunks."""
+    import paper_2004_11658_b200 as pk
+    from oracle import Oracle
+    torch = _torch()
+    spec = MODELS["W192"]
+    coord, types, box = gen.make_system("W192")
+    emb, fit = gen.make_weights(spec)
+    fit = gen.condition_fit_w0(spec, fit)
+    orc = Oracle.from_spec(spec, emb, fit)
+    av_ref = orc.atom_virial(coord, types, box)
+    m = pk.DPModel.from_spec(spec, emb, fit)
+    if chunk:
+        m.set_chunk(chunk)
+    m.set_deterministic(True)
+    for lo, hi in bricks(box, (2, 2, 2)):
+        loc, own, x, t, bounds = _domain(coord, types, box, lo, hi, spec.rcut)
+        nloc = len(loc)
+        ref = orc.eval_local(x, t, nloc)
+        av = torch.full((len(x), 9), float("nan"), dtype=torch.float64, device="cuda")
+        m.set_atom_virial(av)
+        got = _gpu_local(m, x, t, nloc, bounds)
+        _check(ref, got, 0)
+        avh = av.cpu().numpy()
+        assert np.isnan(avh[nloc:]).all(), "only the local atoms' rows are written"
+        scale = max(1.0, np.abs(av_ref).max())
+        assert np.abs(avh[:nloc].reshape(-1, 3, 3) - av_ref[loc].reshape(-1, 3, 3)).max() <= 1e-10 * scale
+        assert np.abs(avh[:nloc].sum(axis=0).reshape(3, 3) - got["virial"]).max() <= 1e-10 * scale
+        again = _gpu_local(m, x, t, nloc, bounds)
+        for k in ("energy", "atom_energy", "force", "virial"):
+            assert np.array_equal(got[k], again[k]), k
+        m.set_atom_virial(None)
     m.set_deterministic(False)
 
 
@@ -309,6 +352,24 @@ def test_triclinic_cell_through_explicit_images():
     assert abs(got["energy"].item() - per["energy"].item()) <= 1e-10 * abs(per["energy"].item())
     assert (got["force"] - per["force"]).abs().max().item() <= 2e-9
     assert (got["virial"] - per["virial"]).abs().max().item() <= 1e-10 * max(1.0, per["virial"].abs().max().item())
+    # (3) the deterministic reduction in a general cell (image rows and the fold are in a fixed order too): bitwise
+    # reproducible, same parity, and the per-atom virial [N][9] against the oracle's dpo_atom_virial on the box
+    from oracle import Oracle as _O
+    av_ref = _O.from_spec(spec, emb, fit).atom_virial(coord, types, box)
+    m.set_deterministic(True)
+    av = torch.zeros((len(coord), 9), dtype=torch.float64, device="cuda")
+    m.set_atom_virial(av)
+    sheared = np.array([a[0], a[1] + a[0], a[2] + a[1] - a[0]])
+    d1 = eval_cell(m, dc, dt, sheared)
+    d1 = {k: v.clone() for k, v in d1.items() if hasattr(v, "clone")}
+    d2 = eval_cell(m, dc, dt, sheared)
+    torch.cuda.synchronize()
+    for k in ("energy", "atom_energy", "force", "virial"):
+        assert torch.equal(d1[k], d2[k]), k
+    assert (d1["force"] - per["force"]).abs().max().item() <= 2e-9
+    assert np.abs(av.cpu().numpy().reshape(-1, 3, 3) - av_ref).max() <= 1e-10 * max(1.0, np.abs(av_ref).max())
+    m.set_atom_virial(None)
+    m.set_deterministic(False)
 
 
 def test_subregion_in_several_chunks():
