@@ -260,6 +260,27 @@ int dpb_dd_add_forces(void *stream, int64_t k, const int32_t *idx, const double 
 int dpb_build_nlist(dpb_model *model, void *stream, int64_t natoms, const double *coord, const int32_t *type,
                     const double box[9], int32_t *nlist, int64_t *n_overflow);
 
+/* dpb_build_nlist without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  Same kernels, same result (Alg. 1: cell binning,
+ * neighbour search, sort by (type, distance, index), -1 padding); the scratch of the kernels lives in one file-scope
+ * device array of 9.9 MB that every GPU which loads this library holds until the process exits, instead of in the
+ * model's workspace.  The call performs no cudaMalloc / cudaFree and calls no allocating library routine; it does not
+ * touch the model's workspace (the model only supplies r_c, sel and the number of types).
+ *   Limits: natoms <= 4096, natoms * Nm <= 262144, ntypes * (cells of the search grid) <= 16384.  Beyond any of them:
+ *           DPB_EINVAL with a message naming the limit; nothing is launched.  dpb_build_nlist has no such limits.
+ *   coord, type  DEVICE fp64 [N][3] / int32 [N];  box HOST fp64 [9] as for dpb_eval (DPB_EBOX otherwise)
+ *   nlist        DEVICE int32 [N][Nm], caller-owned output
+ *   status       DEVICE int64 [4], caller-owned, may be NULL: real pairs, neighbours dropped by a full type section,
+ *                error bits (1: a type index outside [0, ntypes), 2: an atom has more in-range candidates than the
+ *                staging capacity — its row is then written empty), largest candidate count of any (atom, type).
+ *                The call never synchronises: the deferred input errors are reported here, not by the return code.
+ * Every call on a device shares the one array, which keeps the previous call's contents (what must start at zero is
+ * cleared on `stream` first): calls that overlap on the GPU — different streams, different models, different host
+ * threads — race.  Serialise them (one stream, or events).  The first call on a device looks up the array's device
+ * address (cudaGetSymbolAddress) and sets the kernels' shared-memory limit: make that call outside graph capture. */
+int dpb_build_nlist_static(const dpb_model *model, void *stream, int64_t natoms, const double *coord,
+                           const int32_t *type, const double box[9], int32_t *nlist, int64_t *status);
+
 /* Test / profiling hook, not part of the contract: DEVICE buffers (any may be NULL) that the following
  * dpb_eval calls also fill, indexed by the ORIGINAL atom index:
  *   T  [N][M][4]   = G^T R~                    (Eq. 4, left factor)

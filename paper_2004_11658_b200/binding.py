@@ -89,6 +89,7 @@ def load_library():
     lib.dpb_eval_host.argtypes = lib.dpb_eval.argtypes
     lib.dpb_eval_cell.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp, vp, vp, C.POINTER(_Info)]
     lib.dpb_build_nlist.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, C.POINTER(i64)]
+    lib.dpb_build_nlist_static.argtypes = [vp, vp, i64, vp, vp, C.POINTER(C.c_double), vp, vp]
     lib.dpb_md_run.argtypes = [vp, vp, i64, vp, vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                C.POINTER(_MDParams), vp, C.POINTER(_MDInfo)]
     d = C.c_double
@@ -331,6 +332,20 @@ class DPModel:
                                       C.c_void_p(types.data_ptr()), bp, C.c_void_p(nlist.data_ptr()), C.byref(ovf))
         self._chk(rc)
         return nlist, int(ovf.value)
+
+    def build_nlist_static(self, coord, types, box, nlist, status=None):
+        """dpb_build_nlist_static: Alg. 1 with no allocation (scratch in a fixed device array; at most 4096 atoms and
+        natoms * Nm <= 262144).  nlist (CUDA int32 [N][Nm]) and status (CUDA int64 [4] or None) are the caller's."""
+        torch = _torch()
+        n = int(coord.shape[0])
+        assert nlist.is_cuda and nlist.dtype == torch.int32 and nlist.is_contiguous() and nlist.numel() >= n * self.nm
+        assert status is None or (status.is_cuda and status.dtype == torch.int64 and status.numel() >= 4)
+        b, bp = self._box(box)
+        rc = self.lib.dpb_build_nlist_static(self._h, self._stream(), n, C.c_void_p(coord.data_ptr()),
+                                             C.c_void_p(types.data_ptr()), bp, C.c_void_p(nlist.data_ptr()),
+                                             C.c_void_p(status.data_ptr()) if status is not None else None)
+        self._chk(rc)
+        return nlist
 
     def md_run(self, coord, vel, types, mass, box, dt_fs, nsteps, thermo_every=1, rebuild_every=1, skin=0.0):
         """dpb_md_run: velocity-Verlet NVE on torch CUDA tensors coord / vel (float64 [N,3], updated IN PLACE).

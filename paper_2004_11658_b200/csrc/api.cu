@@ -901,6 +901,109 @@ extern "C" int dpb_build_nlist(dpb_model *m, void *stream, int64_t natoms, const
   return DPB_OK;
 }
 
+// ---- dpb_build_nlist_static: Alg. 1 without any allocation -------------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+// The kernels are those of dpb_build_nlist (k_keys / k_scan / k_fill / k_nlist); what differs is where their scratch
+// lives: not in the model's workspace (Buf::reserve -> cudaMalloc) but in ONE file-scope device array of fixed size that
+// every GPU which loads the library holds until the process exits.  Limits (checked, DPB_EINVAL beyond them):
+#define DPB_STATIC_MAX_ATOMS 4096                     // natoms
+#define DPB_STATIC_MAX_SLOTS (1 << 18)                // natoms * Nm       (W192: 26,496)
+#define DPB_STATIC_MAX_KEYS 16384                     // ntypes * cells of the search grid
+// Layout of the array (byte offsets, every piece 256-byte aligned):
+#define SN_AL(x) (((size_t)(x) + 255) & ~(size_t)255)
+#define SN_STATS 0
+#define SN_KEY (SN_STATS + SN_AL(sizeof(DevStats)))
+#define SN_SIDX (SN_KEY + SN_AL(4 * (DPB_STATIC_MAX_ATOMS + 1)))
+#define SN_SXYZ (SN_SIDX + SN_AL(4 * (DPB_STATIC_MAX_ATOMS + 1)))
+#define SN_COUNT (SN_SXYZ + SN_AL(24 * (DPB_STATIC_MAX_ATOMS + 1)))
+#define SN_START (SN_COUNT + SN_AL(4 * (DPB_STATIC_MAX_KEYS + 1)))
+#define SN_CURSOR (SN_START + SN_AL(4 * (DPB_STATIC_MAX_KEYS + 1 + DPB_MAX_TYPES + 1)))
+#define SN_NREAL (SN_CURSOR + SN_AL(4 * (DPB_STATIC_MAX_KEYS + 1)))
+#define SN_NL (SN_NREAL + SN_AL(4 * DPB_STATIC_MAX_ATOMS * DPB_MAX_TYPES))
+#define SN_DR (SN_NL + SN_AL(4 * (size_t)DPB_STATIC_MAX_SLOTS))
+#define SN_TOTAL (SN_DR + SN_AL(32 * (size_t)DPB_STATIC_MAX_SLOTS))            // 9.9 MB
+static __device__ __align__(256) unsigned char g_static_scratch[SN_TOTAL];
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static unsigned char *g_static_ptr[DPB_MAX_DEVICES] = {};
+
+static int static_scratch(unsigned char **out) {
+  int dev = 0;
+  CU(cudaGetDevice(&dev), "cudaGetDevice");
+  if (dev < 0 || dev >= DPB_MAX_DEVICES) return fail(DPB_EINVAL, "device index %d beyond DPB_MAX_DEVICES", dev);
+  if (!g_static_ptr[dev]) {
+    void *p = nullptr;
+    CU(cudaGetSymbolAddress(&p, g_static_scratch), "cudaGetSymbolAddress of the static scratch");
+    if (!p) return fail(DPB_ECUDA, "cudaGetSymbolAddress returned a null address");
+    g_static_ptr[dev] = static_cast<unsigned char *>(p);
+  }
+  *out = g_static_ptr[dev];
+  return DPB_OK;
+}
+
+// status[0..3] = real pairs, dropped neighbours (n_overflow), error bits (1: type out of range, 2: staging cap), largest
+// candidate count of any (atom, type)
+__global__ void k_static_status(const DevStats *__restrict__ s, int ntypes, long long *__restrict__ status) {
+  int mx = 0;
+  for (int t = 0; t < ntypes; ++t) mx = s->max_nei[t] > mx ? s->max_nei[t] : mx;
+  status[0] = (long long)s->n_real_pairs;
+  status[1] = (long long)s->n_overflow;
+  status[2] = (s->err_type ? 1 : 0) | (s->err_cap ? 2 : 0);
+  status[3] = mx;
+}
+
+extern "C" int dpb_build_nlist_static(const dpb_model *m, void *stream, int64_t natoms, const double *coord,
+                                      const int32_t *type, const double box[9], int32_t *nlist, int64_t *status) {
+  if (!m || !box) return fail(DPB_EINVAL, "dpb_build_nlist_static: null model / box");
+  const DevModel &P = m->P;
+  if (natoms < 0) return fail(DPB_EINVAL, "dpb_build_nlist_static: natoms < 0");
+  if (natoms > DPB_STATIC_MAX_ATOMS)
+    return fail(DPB_EINVAL, "dpb_build_nlist_static: %lld atoms exceed the static scratch (at most %d atoms); use "
+                            "dpb_build_nlist", (long long)natoms, DPB_STATIC_MAX_ATOMS);
+  if (natoms * (int64_t)P.nm > DPB_STATIC_MAX_SLOTS)
+    return fail(DPB_EINVAL, "dpb_build_nlist_static: natoms * Nm = %lld exceeds the static scratch (at most %d slots); "
+                            "use dpb_build_nlist", (long long)(natoms * P.nm), DPB_STATIC_MAX_SLOTS);
+  if (natoms > 0 && (!coord || !type || !nlist)) return fail(DPB_EINVAL, "dpb_build_nlist_static: null coord / type / nlist");
+  DevGrid G;
+  int rc = make_grid(P, box, G, P.rc);
+  if (rc != DPB_OK) return rc;
+  const int nkeys = P.ntypes * G.ncell;
+  if (nkeys > DPB_STATIC_MAX_KEYS)
+    return fail(DPB_EINVAL, "dpb_build_nlist_static: ntypes * cells = %d exceeds the static scratch (at most %d); use "
+                            "dpb_build_nlist", nkeys, DPB_STATIC_MAX_KEYS);
+  unsigned char *base = nullptr;
+  if ((rc = static_scratch(&base)) != DPB_OK) return rc;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  DevStats *stats = reinterpret_cast<DevStats *>(base + SN_STATS);
+  int *start = reinterpret_cast<int *>(base + SN_START);
+  // the array keeps the last call's contents: the statistics start at zero (the cell counts are cleared by the sort)
+  CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), st), "memset stats");
+  CU(launch_cell_sort(P, G, natoms, coord, type, reinterpret_cast<int *>(base + SN_KEY),
+                      reinterpret_cast<int *>(base + SN_COUNT), start, reinterpret_cast<int *>(base + SN_CURSOR),
+                      reinterpret_cast<int *>(base + SN_SIDX), reinterpret_cast<double *>(base + SN_SXYZ), stats, st,
+                      nullptr), "cell sort");
+  ChunkView C{};
+  C.p0 = 0;
+  C.n = (int)natoms;
+  C.s_idx = reinterpret_cast<int *>(base + SN_SIDX);
+  C.type_start = start + nkeys + 1;
+  C.nl = reinterpret_cast<int *>(base + SN_NL);
+  C.dr = reinterpret_cast<double4 *>(base + SN_DR);
+  C.nreal = reinterpret_cast<int *>(base + SN_NREAL);
+  C.nlp = nullptr;
+  C.stats = stats;
+  C.sub_nparts = 1;
+  CU(launch_nlist(P, G, C, reinterpret_cast<double *>(base + SN_SXYZ), start, neighbour_cap(P), nlist, stats, st, 0,
+                  nullptr), "nlist");
+  if (status) {
+    k_static_status<<<1, 1, 0, st>>>(stats, P.ntypes, reinterpret_cast<long long *>(status));
+    DPB_LAUNCHED(1);
+    CU(cudaGetLastError(), "status");
+  }
+  return DPB_OK;
+}
+
 extern "C" int dpb_eval_host(dpb_model *m, void *stream, int64_t natoms, const double *coord_h, const int32_t *type_h,
                              const double box[9], double *energy_h, double *atom_energy_h, double *force_h,
                              double *virial_h, int32_t *nlist_h, dpb_eval_info *info) {
