@@ -281,6 +281,9 @@ def run_dd(args, spec, name, coord, types, box, dev, model, world, rank):
 STAGES = ["cell_sort", "nlist", "pass1_env_embed_T", "fit_fwd_bwd", "pass2_embed_bwd_force", "reduce"]
 
 
+STORED_ACT = None        # --stored-act: None = library default (on), 0 / 1 = dpb_model_set_stored_activations
+
+
 def measure(name, precision, variant, steps, warmup, dev, rank=0, world=1, stage_every=10, want_e2e=False):
     """Time `steps` evaluations of workload `name` (each on a freshly perturbed copy of its box, L2 flushed in between,
     CUDA events on the launching stream, W untimed warm-up calls).  Returns a dict; times are this rank's."""
@@ -295,6 +298,8 @@ def measure(name, precision, variant, steps, warmup, dev, rank=0, world=1, stage
     mixed = precision != "fp64"
     model = DPModel.from_spec(spec, emb, fit, precision={"fp64": 0, "tf32": 1, "bf16": 2, "bf16_plain": 3}[precision])
     model.set_variant(variant)
+    if STORED_ACT is not None:
+        model.set_stored_activations(STORED_ACT)
 
     # pool of freshly perturbed copies (reading R24: fresh perturbation of the base positions per call)
     pool = min(steps + warmup, 16 if n < 200000 else 3)
@@ -576,6 +581,8 @@ def main():
     ap.add_argument("--workload", default="W24k", choices=sorted(MODELS))
     ap.add_argument("--precision", default="fp64", choices=["fp64", "tf32", "bf16", "bf16_plain"])
     ap.add_argument("--variant", type=int, default=1)
+    ap.add_argument("--stored-act", type=int, default=None, choices=[0, 1],
+                    help="fp64 variant 1: pass 2 reads the activations pass 1 stored (default: the library's, on)")
     ap.add_argument("--no-configs", dest="configs", action="store_false",
                     help="skip the short legs over the other BASELINE.json configs (W192, Cu32k, W24k mixed, Cu864k) that the "
                          "default run appends as a `configs` object")
@@ -589,6 +596,8 @@ def main():
                     help="also time the domain-decomposed step (one brick per rank, ghost exchange + dpb_eval_local + "
                          "reverse force exchange + all-reduce) and report it in an extra 'dd' object")
     args = ap.parse_args()
+    global STORED_ACT
+    STORED_ACT = args.stored_act
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

@@ -143,6 +143,16 @@ int dpb_model_set_graph(dpb_model *model, int mode);
  * Returns DPB_EINVAL for any other value. */
 int dpb_model_set_pair_reuse(dpb_model *model, int on);
 
+/* Stored activations (DPB_FP64, variant 1; on by default).  Pass 2 differentiates the embedding net (Eq. 8-9,
+ * PAPER.md:113-123) along the value chain of pass 1.  on = 1: pass 1 writes the tanh outputs of the three layers of every
+ * row it evaluates (7 s1 fp64 numbers per pair, streamed: written once, read once) and pass 2 reads them instead of
+ * running the value chain and its tanh again; the arithmetic that remains is the same, so results do not change beyond
+ * the summation order of the pair reuse.  Taken per evaluation when the records of a chunk (chunk * Nm * 14 * s1 * 8
+ * bytes, padded) fit into the workspace budget (half of the memory that was free when the model was created), the chunk
+ * has at least 4096 centres, the pair reuse is on and the deterministic reduction is off; otherwise, and with on = 0,
+ * pass 2 recomputes (the paper's Eq. 13 tensors are then never written).  Returns DPB_EINVAL for any other value. */
+int dpb_model_set_stored_activations(dpb_model *model, int on);
+
 /* Per-atom virial.  The paper gives no per-atom split (the virial is only named through the
  * ProdVirial operator); this library assigns every term to its centre atom:
  *     atom_virial[i][a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b],     sum_i atom_virial[i] = virial of dpb_eval.

@@ -76,6 +76,7 @@ def load_library():
     lib.dpb_model_set_variant.argtypes = [vp, i32]
     lib.dpb_model_set_deterministic.argtypes = [vp, i32]
     lib.dpb_model_set_pair_reuse.argtypes = [vp, i32]
+    lib.dpb_model_set_stored_activations.argtypes = [vp, i32]
     lib.dpb_model_set_atom_virial.argtypes = [vp, vp]
     lib.dpb_model_set_timing.argtypes = [vp, i32]
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
@@ -164,6 +165,10 @@ class DPModel:
 
     def set_deterministic(self, on: bool):
         self._chk(self.lib.dpb_model_set_deterministic(self._h, int(bool(on))))
+
+    def set_stored_activations(self, on: bool):
+        """dpb_model_set_stored_activations: pass 2 reads the embedding activations pass 1 stored (default on)."""
+        self._chk(self.lib.dpb_model_set_stored_activations(self._h, int(bool(on))))
 
     def set_pair_reuse(self, on: int):
         """dpb_model_set_pair_reuse: 0 off, 1 single-chunk evaluations (default), 2 always."""

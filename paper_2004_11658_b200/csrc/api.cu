@@ -121,7 +121,7 @@ struct dpb_model {
   int graph_mode = 1;                        // 0 off, 1 evaluations of at most DPB_GRAPH_AUTO_ATOMS atoms, 2 always
   unsigned long long cfg_epoch = 1, graph_clock = 0;
   std::vector<GraphEntry> graphs;
-  int precision = 0, variant = 1, timing = 0, deterministic = 0, pair_reuse = 1;
+  int precision = 0, variant = 1, timing = 0, deterministic = 0, pair_reuse = 1, stored_act = 1;
   double *atom_virial = nullptr;        // caller's [N][9] buffer (dpb_model_set_atom_virial)
   int64_t chunk = 0;            // atoms per pass; 0 = automatic (effective_chunk)
   size_t ws_budget = 0;         // bytes the per-chunk workspace may take in automatic mode (half of the memory free at creation)
@@ -134,6 +134,7 @@ struct dpb_model {
   // workspace
   Buf key, count, start, cursor, s_idx, s_xyz, stats, ei;
   Buf nl, nlp, dr, nreal, T, dT, counters;
+  Buf act;                      // activation records of the chunk (ChunkView::act)
   int dt_pad_alloc = -1;          // layout the dT buffer was last used with (pad rows must be zero: cleared on a change)
   Buf v0[9];
   Buf v1ws;
@@ -247,7 +248,7 @@ extern "C" int dpb_model_destroy(dpb_model *m) {
                 &m->nl, &m->nlp, &m->dr, &m->v2ws, &m->counters, &m->nreal, &m->T, &m->dT, &m->v1ws, &m->pairs, &m->dT32, &m->tcfit, &m->h_coord, &m->h_type, &m->h_out,
                 &m->pos_of, &m->nl_all, &m->nreal_all, &m->fslot, &m->vpart,
                 &m->md_raw, &m->md_nraw, &m->md_xyz0, &m->md_force, &m->md_scal, &m->md_mass,
-                &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_off, &m->cell_f};
+                &m->cell_frac, &m->cell_x, &m->cell_t, &m->cell_off, &m->cell_f, &m->act};
   for (Buf *b : all) b->release();
   for (Buf &b : m->v0) b.release();
   v1_release_weights(m->v1);
@@ -302,6 +303,15 @@ extern "C" int dpb_model_set_pair_reuse(dpb_model *m, int on) {
   if (!m) return fail(DPB_EINVAL, "null model");
   if (on < 0 || on > 2) return fail(DPB_EINVAL, "pair reuse: 0 (off), 1 (single-chunk evaluations) or 2 (always)");
   m->pair_reuse = on;
+  ++m->cfg_epoch;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_stored_activations(dpb_model *m, int on) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  if (on < 0 || on > 1) return fail(DPB_EINVAL, "stored activations: 0 (off) or 1 (when the records fit)");
+  m->stored_act = on;
+  if (!on) m->act.release();
   ++m->cfg_epoch;
   return DPB_OK;
 }
@@ -466,6 +476,18 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   CU(m->counters.reserve(sizeof(int) * 128), "workspace");
   CU(m->dr.reserve(sizeof(double4) * (size_t)lrows * P.nm), "workspace");
   CU(m->nreal.reserve(sizeof(int) * (size_t)chunk * P.ntypes), "workspace");
+  // Stored activations (dpb_model_set_stored_activations): one record per (centre, slot) of the chunk, taken when the
+  // records fit into the workspace budget and the chunk is large enough for whole-atom work items
+  int act_stride = 0;
+  if (!nlist_only && m->stored_act && m->precision == DPB_FP64 && m->variant == 1 && m->v1.ready && !det &&
+      m->pair_reuse >= 1 && chunk >= 4096 && (size_t)chunk * P.nm < 2000000000ull) {
+    const int sp = m->v1.SP, stride = 4 * (((sp + 1) & ~1) + 6 * sp);
+    const size_t bytes = sizeof(double) * (size_t)chunk * P.nm * stride;
+    if (bytes <= m->ws_budget) {
+      CU(m->act.reserve(bytes), "workspace of the stored activations");
+      act_stride = stride;
+    }
+  }
   if (!nlist_only) {
     CU(m->T.reserve(sizeof(double) * (size_t)chunk * P.M * 4), "workspace");
     // fp64 variant 1 keeps dT in the padded lane order of the DMMA kernels (ChunkView::dt_pad); the pad rows are zero
@@ -558,6 +580,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.stats = stats;
     C.reuse = (!det && (m->pair_reuse == 2 || (m->pair_reuse == 1 && nchunks == 1))) ? 1 : 0;
     C.reuse2 = (!det && m->pair_reuse >= 1) ? 1 : 0;     // pass 2 only reads dT_j: no bookkeeping, any chunking
+    C.act = act_stride ? m->act.as<double>() : nullptr;
+    C.act_stride = act_stride;
     if (det) {                                           // full-size lists: the gather needs every atom's row
       C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
       C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;

@@ -77,6 +77,11 @@ struct ChunkView {
   int *counters;           // [128] work-item counters of the embedding launches (pass 1: net, pass 2: 64 + net), zeroed per chunk
   int reuse;               // pass 1
   int reuse2;              // pass 2 (k_pass2_dmma_ru): both directions of a same-species pair from one evaluation
+  // Stored activations (fp64 variant 1, embed_dmma.cu): pass 1 writes the tanh outputs of the three
+  // embedding layers of every row it evaluates, pass 2 reads them instead of recomputing the value chain.  Record of
+  // slot (row, section slot) at act + ((size_t)row * nm + slot) * act_stride; nullptr: pass 2 recomputes.
+  double *act;
+  int act_stride;          // doubles per record: 4 * (even(SP) + 6 SP)
 };
 
 // The per-type fitting chains are independent (disjoint rows) and one type's GEMM launch fills only as many SMs as that

@@ -54,7 +54,20 @@ struct EL {
   static constexpr int tile1 = 16 * LDG + 16 * 4;        // pass 1, per warp: g tile [16][LDG] + env tile [16][4] (RB = 2)
   static constexpr int tile1s = 8 * LDG + 8 * 4;         // same for RB = 1
   static constexpr int tile2 = 16 * SP * 4;              // pass 2, per warp: dT tile [16 SP][4]
+  // Stored activations (ChunkView::act): per row and lane quarter q the tanh outputs t0 [SP] (padded to an even count),
+  // t1 [2 SP], t2 [4 SP] in slot order; element e of quarter q at (e / 2) * 8 + 2 q + e % 2, so that one 16-byte access
+  // per lane covers 64 contiguous bytes per row (8 rows: 512 bytes per warp instruction).
+  static constexpr int A0 = (SP + 1) & ~1;               // elements of t0 per lane
+  static constexpr int AE = A0 + 6 * SP;                 // elements per lane
+  static constexpr int REC = 4 * AE;                     // doubles per record
 };
+
+// streaming (evict-first) 16-byte accesses to the activation records: written once, read once, never reused — they must
+// not push the dT tiles and the lists out of L2
+__device__ __forceinline__ void act_store(double *p, const double a, const double b) {
+  __stcs(reinterpret_cast<double2 *>(p), make_double2(a, b));
+}
+__device__ __forceinline__ double2 act_load(const double *p) { return __ldcs(reinterpret_cast<const double2 *>(p)); }
 
 // Row staging of the embedding passes: the (d, r) rows and neighbour indices of the next 32 slots are copied global ->
 // shared with cp.async (no registers in flight) while the current 32 are processed, so that no 8-row block starts with
@@ -217,6 +230,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
              warp * 2 * P.nm;
   int *krow = ksl + P.nm;
   const bool ru = RU && C.stats->n_overflow == 0ull;
+  const bool store_act = C.act != nullptr && nseg == 1;     // pass 2 reads the records only when items are whole atoms
   // RU: offset inside a T tile of the element this lane adds in step k of N chunk ch (position p = lane / 4 + 8 k of
   // the g tile, component lane % 4), or -1 for a pad
   int toff[RU ? 2 : 1][RU ? SP : 1];
@@ -301,6 +315,7 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
     }
     for (int r0 = 0; r0 < n; r0 += 8 * RB) {
       double x[RB];
+      double *recp[RB];                                  // this lane's piece of the row's activation record, or nullptr
 #pragma unroll
       for (int rb = 0; rb < RB; ++rb) {
         const int row = r0 + g + 8 * rb;
@@ -310,6 +325,9 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
           const int rown = row + 8 * RB;
           if (rown < n) dvn[rb] = dr[(RU && ru) ? ksl[rown] : rown];
         }
+        recp[rb] = nullptr;
+        if (store_act && row < n)
+          recp[rb] = C.act + ((size_t)qa * P.nm + P.sec_start[t] + ((RU && ru) ? ksl[row] : s_lo + row)) * L::REC + 2 * q;
         if (row < n) env_row4(P, dvc, e);
         x[rb] = e[0];
         if (q == 0) {
@@ -325,6 +343,12 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
 #pragma unroll
         for (int rb = 0; rb < RB; ++rb) h0[rb][s] = dp_tanh(fma(x[rb], w0, bb));
       }
+#pragma unroll
+      for (int rb = 0; rb < RB; ++rb)
+        if (recp[rb]) {
+#pragma unroll
+          for (int s = 0; s < SP; s += 2) act_store(recp[rb] + 4 * s, h0[rb][s], s + 1 < SP ? h0[rb][s + 1] : 0.0);
+        }
       // layer 1 (Eq. 9): h1 = (h0, h0) + tanh(h0 W1 + b1)
       double h1[RB][2 * SP];
 #pragma unroll
@@ -343,9 +367,14 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         }
       }
 #pragma unroll
-      for (int s = 0; s < 2 * SP; ++s)
+      for (int s = 0; s < 2 * SP; s += 2)
 #pragma unroll
-        for (int rb = 0; rb < RB; ++rb) h1[rb][s] = h0[rb][s % SP] + dp_tanh(h1[rb][s]);
+        for (int rb = 0; rb < RB; ++rb) {
+          const double ta = dp_tanh(h1[rb][s]), tb = dp_tanh(h1[rb][s + 1]);
+          if (recp[rb]) act_store(recp[rb] + 4 * (L::A0 + s), ta, tb);
+          h1[rb][s] = h0[rb][s % SP] + ta;
+          h1[rb][s + 1] = h0[rb][(s + 1) % SP] + tb;
+        }
       // layer 2 (Eq. 9) in two N chunks of SP n-blocks: g = (h1, h1) + tanh(h1 W2 + b2); T += g (x) R~
 #pragma unroll
       for (int ch = 0; ch < 2; ++ch) {
@@ -368,9 +397,14 @@ k_pass1_dmma(DevModel P, ChunkView C, const double *__restrict__ netp, int a, in
         __syncwarp();                                    // previous chunk's T update has finished reading gt
         // slot ch*2SP + s of layer 2 takes its skip from slot s of layer 1 (same copy structure)
 #pragma unroll
-        for (int s = 0; s < 2 * SP; ++s)
+        for (int s = 0; s < 2 * SP; s += 2)
 #pragma unroll
-          for (int rb = 0; rb < RB; ++rb) gt[(g + 8 * rb) * L::LDG + 4 * s + q] = h1[rb][s] + dp_tanh(acc[rb][s]);
+          for (int rb = 0; rb < RB; ++rb) {
+            const double ta = dp_tanh(acc[rb][s]), tb = dp_tanh(acc[rb][s + 1]);
+            if (recp[rb]) act_store(recp[rb] + 4 * (L::A0 + 2 * SP + ch * 2 * SP + s), ta, tb);
+            gt[(g + 8 * rb) * L::LDG + 4 * s + q] = h1[rb][s] + ta;
+            gt[(g + 8 * rb) * L::LDG + 4 * (s + 1) + q] = h1[rb][s + 1] + tb;
+          }
         __syncwarp();
 #pragma unroll
         for (int row = 0; row < 8 * RB; ++row) {
@@ -980,24 +1014,28 @@ struct P2S {
   static constexpr int NBA = (SP + 1) / 2, NBB = SP - NBA;   // n-blocks of the two N chunks of a half (SP n-blocks)
   static constexpr int SLICE = 32 * NBA + 16;                // doubles per staged row slice (+128 B: rows on distinct banks)
   static constexpr int RING = 64;
-  // per warp: dT_i slices [2][SLICE] | dT_j slices [8][SLICE] | ring (d, r) [RING] | ring ints j, row of j, centre row, i [RING]
-  //           | mbarrier | staging of 32 raw slots: (d, r) [32], j [32], sorted position of j [32]
-  static constexpr int per_warp = 10 * SLICE + 4 * RING + 2 * RING + 2 + 4 * 32 + 16 + 16;
+  // per warp: dT_i slices [2][SLICE] | dT_j slices [8][SLICE] | ring (d, r) [RING] | ring ints j, row of j, centre row, i,
+  //           record index [RING] | mbarrier | staging of 32 raw slots: (d, r) [32], j [32], sorted position of j [32]
+  static constexpr int per_warp = 10 * SLICE + 4 * RING + 2 * RING + RING / 2 + 2 + 4 * 32 + 16 + 16;
 };
 
-template <int SP, int NB, int NB0>
+// SA: the value chain is not run; t2v holds the stored tanh outputs of this chunk's slots (ChunkView::act).
+template <int SP, int NB, int NB0, bool SA>
 __device__ __forceinline__ void p2s_chunk(const double *__restrict__ W2h, const double *__restrict__ b2h,
                                           const double *__restrict__ irow, const double *__restrict__ jrow,
                                           const bool anyboth, uint64_t *mbar, unsigned &parity,
                                           const double (&h1v)[2 * SP], const double (&h1t)[2 * SP],
+                                          const double (&t2v)[2 * NB],
                                           const double (&e)[4], const int g, const int q, double (&pr)[5],
                                           double (&pj)[5]) {
   using L = EL<SP>;
   double av[2 * NB], at[2 * NB];
 #pragma unroll
   for (int nb = 0; nb < NB; ++nb) {
-    const double2 bb = *reinterpret_cast<const double2 *>(b2h + 8 * (NB0 + nb) + 2 * q);
-    av[2 * nb] = bb.x; av[2 * nb + 1] = bb.y;
+    if (!SA) {
+      const double2 bb = *reinterpret_cast<const double2 *>(b2h + 8 * (NB0 + nb) + 2 * q);
+      av[2 * nb] = bb.x; av[2 * nb + 1] = bb.y;
+    }
     at[2 * nb] = 0.0; at[2 * nb + 1] = 0.0;
   }
 #pragma unroll
@@ -1005,7 +1043,7 @@ __device__ __forceinline__ void p2s_chunk(const double *__restrict__ W2h, const 
 #pragma unroll
     for (int nb = 0; nb < NB; ++nb) {
       const double b = W2h[(4 * ks + q) * L::LD2 + 8 * (NB0 + nb) + g];
-      dmma884(av[2 * nb], av[2 * nb + 1], h1v[ks], b);
+      if (!SA) dmma884(av[2 * nb], av[2 * nb + 1], h1v[ks], b);
       dmma884(at[2 * nb], at[2 * nb + 1], h1t[ks], b);
     }
   }
@@ -1014,7 +1052,7 @@ __device__ __forceinline__ void p2s_chunk(const double *__restrict__ W2h, const 
 #pragma unroll
   for (int s = 0; s < 2 * NB; ++s) {
     const int sl = 2 * NB0 + s;                             // slot inside the half: the skip comes from slot sl of layer 1
-    const double t2 = dp_tanh(av[s]);
+    const double t2 = SA ? t2v[s] : dp_tanh(av[s]);
     const double gv = h1v[sl] + t2;
     const double gp = fma(fma(-t2, t2, 1.0), at[s], h1t[sl]);
     av[s] = gv; at[s] = gp;
@@ -1040,7 +1078,7 @@ __device__ __forceinline__ void p2s_chunk(const double *__restrict__ W2h, const 
   }
 }
 
-template <int SP>
+template <int SP, bool SA>
 __global__ void __launch_bounds__((32 * P2_WARPS), 1)
 k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
                 double *__restrict__ virial, int *counter) {
@@ -1056,7 +1094,8 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   int *rqj = rjn + R::RING;                                             //   its row in this chunk when both directions run, else -1
   int *rqa = rqj + R::RING;                                             //   row of the centre atom in this chunk
   int *rio = rqa + R::RING;                                             //   input index of the centre atom
-  uint64_t *mbar = reinterpret_cast<uint64_t *>(rio + R::RING);
+  int *rrec = rio + R::RING;                                            //   index of the row's activation record (SA)
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(rrec + R::RING);
   double4 *sdr = reinterpret_cast<double4 *>(mbar + 2);                 // staged raw slots (cp.async, one batch ahead)
   int *snl = reinterpret_cast<int *>(sdr + 32);
   int *snlp = snl + 32;
@@ -1113,8 +1152,9 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
         if (ru) {
           const int pj = snlp[lane] - C.p0;
           const bool inchunk = pj >= 0 && pj < C.n;
-          // sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs
-          if (sweep == 0) { keep = inchunk && ((((qa + pj) & 1) == 0) == (qa < pj)); qj = pj; }
+          // sweep 0 keeps the pairs this atom evaluates in both directions, sweep 1 the one-direction pairs.
+          // SA: the evaluating atom is the one whose row pass 1 stored — the lower row, as in k_pass1_dmma<.., RU>
+          if (sweep == 0) { keep = inchunk && (SA ? qa < pj : ((((qa + pj) & 1) == 0) == (qa < pj))); qj = pj; }
           else keep = !inchunk;
         } else {
           keep = true;
@@ -1124,6 +1164,7 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       if (keep) {
         const int pos = (head + cnt + __popc(mk & ((1u << lane) - 1u))) & (R::RING - 1);
         rdv[pos] = sdr[lane]; rjn[pos] = snl[lane]; rqj[pos] = qj; rqa[pos] = qa; rio[pos] = io;
+        if (SA) rrec[pos] = qa * P.nm + P.sec_start[t] + slot;
       }
       cnt += __popc(mk);
       __syncwarp();
@@ -1192,19 +1233,40 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
         dv = rdv[ri]; jn = rjn[ri]; ri_io = rio[ri];
         env_row4(P, dv, e);
       }
+      // SA: this lane's piece of the row's activation record (written by pass 1)
+      const double *recp = nullptr;
+      if (SA && valid) recp = C.act + (size_t)rrec[(head + g) & (R::RING - 1)] * L::REC + 2 * q;
+      double t01[SA ? L::A0 + 2 * SP : 2];                  // t0 [A0] | t1 [2 SP]
+      double t2a[2 * R::NBA], t2b[2 * R::NBB];              // NBB >= 1 for every SP in use
+      if (SA) {
+#pragma unroll
+        for (int s = 0; s < L::A0 + 2 * SP; s += 2) {
+          double2 v = make_double2(0.0, 0.0);
+          if (recp) v = act_load(recp + 4 * s);
+          t01[s] = v.x; t01[s + 1] = v.y;
+        }
+#pragma unroll
+        for (int s = 0; s < 2 * R::NBA; s += 2) {           // N chunk 0 of layer 2
+          double2 v = make_double2(0.0, 0.0);
+          if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + s));
+          t2a[s] = v.x; t2a[s + 1] = v.y;
+        }
+      }
       double h0v[SP], h0t[SP];
 #pragma unroll
       for (int s = 0; s < SP; ++s) {
         const double w0 = W0p[4 * s + q], bb = b0p[4 * s + q];
-        const double t0 = dp_tanh(fma(e[0], w0, bb));
+        const double t0 = SA ? t01[s] : dp_tanh(fma(e[0], w0, bb));
         h0v[s] = t0;
         h0t[s] = fma(-t0, t0, 1.0) * w0;
       }
       double h1v[2 * SP], h1t[2 * SP];
 #pragma unroll
       for (int nb = 0; nb < L::NB1; ++nb) {
-        const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
-        h1v[2 * nb] = bb.x; h1v[2 * nb + 1] = bb.y;
+        if (!SA) {
+          const double2 bb = *reinterpret_cast<const double2 *>(b1p + 8 * nb + 2 * q);
+          h1v[2 * nb] = bb.x; h1v[2 * nb + 1] = bb.y;
+        }
         h1t[2 * nb] = 0.0; h1t[2 * nb + 1] = 0.0;
       }
 #pragma unroll
@@ -1212,13 +1274,13 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 #pragma unroll
         for (int nb = 0; nb < L::NB1; ++nb) {
           const double b = W1p[(4 * ks + q) * L::LD1 + 8 * nb + g];
-          dmma884(h1v[2 * nb], h1v[2 * nb + 1], h0v[ks], b);
+          if (!SA) dmma884(h1v[2 * nb], h1v[2 * nb + 1], h0v[ks], b);
           dmma884(h1t[2 * nb], h1t[2 * nb + 1], h0t[ks], b);
         }
       }
 #pragma unroll
       for (int s = 0; s < 2 * SP; ++s) {
-        const double t1 = dp_tanh(h1v[s]);
+        const double t1 = SA ? t01[L::A0 + s] : dp_tanh(h1v[s]);
         h1v[s] = h0v[s % SP] + t1;
         h1t[s] = fma(fma(-t1, t1, 1.0), h1t[s], h0t[s % SP]);
       }
@@ -1228,10 +1290,26 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 #pragma unroll 1
       for (int half = 0; half < 2; ++half) {
         const double *W2h = W2p + 8 * half * SP, *b2h = b2p + 8 * half * SP;
-        p2s_chunk<SP, R::NBA, 0>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, e, g, q, pr, pj);
+        if (SA) {                                           // the stored t2 of a chunk are fetched one chunk ahead
+#pragma unroll
+          for (int s = 0; s < 2 * R::NBB; s += 2) {
+            double2 v = make_double2(0.0, 0.0);
+            if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + half * 2 * SP + 2 * R::NBA + s));
+            t2b[s] = v.x; t2b[s + 1] = v.y;
+          }
+        }
+        p2s_chunk<SP, R::NBA, 0, SA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, t2a, e, g, q, pr, pj);
         __syncwarp();
         issue(2 * half + 1);
-        if (R::NBB > 0) p2s_chunk<SP, R::NBB, R::NBA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, e, g, q, pr, pj);
+        if (SA && half == 0) {
+#pragma unroll
+          for (int s = 0; s < 2 * R::NBA; s += 2) {
+            double2 v = make_double2(0.0, 0.0);
+            if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + 2 * SP + s));
+            t2a[s] = v.x; t2a[s + 1] = v.y;
+          }
+        }
+        p2s_chunk<SP, R::NBB, R::NBA, SA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, t2b, e, g, q, pr, pj);
         __syncwarp();
         if (half == 0) issue(2);
       }
@@ -1387,10 +1465,15 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
   const size_t smem_st = sizeof(double) * (((L::total + 1) & ~1) + P2_WARPS * S::per_warp);
   // the row-stream kernel serves every net when an item is a run of whole atoms (no row segments, no per-slot output)
   const bool stream = reuse && nseg == 1 && smem_st <= 227 * 1024;
+  // stored activations: pass 1 wrote a record for every row it evaluated (same nseg == 1 condition there)
+  const bool sa = stream && C.act != nullptr && C.act_stride == L::REC &&
+                  seg_count(C.n, P1_WARPS, P.ntypes * P.ntypes) == 1;
   static bool configured_st_d[DPB_MAX_DEVICES] = {};
   bool &configured_st = configured_st_d[dpb_device()];
   if (stream && !configured_st) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_st<SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_st);
+    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_st);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_st);
     if (e != cudaSuccess) return e;
     configured_st = true;
   }
@@ -1405,9 +1488,12 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     for (int t = P.ntypes - 1; t >= 0; --t) {
       const int net = a * P.ntypes + t;
       cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
-      if (stream)
-        k_pass2_dmma_st<SP><<<grid, (32 * P2_WARPS), smem_st, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
-                                                                     virial, C.counters + 64 + net);
+      if (sa)
+        k_pass2_dmma_st<SP, true><<<grid, (32 * P2_WARPS), smem_st, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t,
+                                                                           force, virial, C.counters + 64 + net);
+      else if (stream)
+        k_pass2_dmma_st<SP, false><<<grid, (32 * P2_WARPS), smem_st, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t,
+                                                                            force, virial, C.counters + 64 + net);
       else if (reuse && a == t)
         k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
                                                                      virial, nseg, C.counters + 64 + net);
