@@ -220,7 +220,8 @@ def test_full_size_parity_every_element(name, conditioned):
     default pair reuse) and on the weight set it times (literal) as well as the conditioned one: EVERY output element
     against the oracle's whole evaluation — nlist bit-exact on all rows, E, E_i, every force component, the virial
     (Eq. 10; ProdForce / ProdVirial :240), T and dT through the debug buffers on sampled rows.
-    The pair reuse is also switched off and on again; the two kernel generations are compared as an extra."""
+    The pair reuse and the stored activations are also switched off and on again (one chunk and several); the two kernel
+    generations are compared as an extra."""
     from conftest import oracle_full
     torch = _torch()
     spec, emb, fit, coord, types, box, ref = oracle_full(name, conditioned)
@@ -236,6 +237,18 @@ def test_full_size_parity_every_element(name, conditioned):
     for reuse in (0, 2):
         m.set_pair_reuse(reuse)
         _check_full(ref, _gpu_eval(m, coord, types, box))
+    # stored activations (default on: the runs above) off, and on again in several chunks — pass 1 then evaluates every
+    # row (pair_reuse 1) or shares inside a chunk only (2), pass 2 reads the records of the rows of the lower atom
+    m.set_pair_reuse(1)
+    m.set_stored_activations(False)
+    _check_full(ref, _gpu_eval(m, coord, types, box))
+    m.set_stored_activations(True)
+    m.set_chunk(8192)
+    for reuse in (1, 2):
+        m.set_pair_reuse(reuse)
+        got = _gpu_eval(m, coord, types, box)
+        assert got["info"].n_chunks >= 3
+        _check_full(ref, got)
     m.close()
     if not conditioned:
         m0 = _models(spec, emb, fit, 0)[1]
