@@ -187,7 +187,9 @@ def workload_config(name, args):
             "parallelism": "replicas only (1 GPU per replica, no collectives)",
             "l2": "flushed between timed steps (256 MiB write)", "variant": getattr(args, "variant", 1),
             "precision": getattr(args, "precision", "fp64"),
-            "pair_reuse": "nets (a,a): pass 2 always, pass 1 in single-chunk evaluations (library default; fp64 variant 1)"}
+            "pair_reuse": "nets (a,a): pass 2 always, pass 1 in single-chunk evaluations (library default; fp64 variant 1)",
+            "stored_activations": ("library default (on when the records fit the workspace budget)" if STORED_ACT is None
+                                   else bool(STORED_ACT))}
 
 
 # ---- molecular dynamics: the paper's own unit, steps/s and ns/day ----------------------
@@ -198,6 +200,8 @@ def run_md(args, spec, name, coord, types, box, dev, emb, fit, mixed):
     import torch
     from paper_2004_11658_b200 import DPModel
     model = DPModel.from_spec(spec, emb, gen.condition_fit_w0(spec, fit), precision={"fp64": 0, "tf32": 1, "bf16": 2, "bf16_plain": 3}[args.precision])
+    if STORED_ACT is not None:
+        model.set_stored_activations(STORED_ACT)
     masses = gen.MASSES[name]
     dt_fs = 0.5 if spec.ntypes == 2 else 1.0                     # 0.5 fs water, 1.0 fs copper
     vel = gen.maxwell_boltzmann(types, masses, 330.0, seed=gen.SEED_BASE + 500)
@@ -506,10 +510,11 @@ def run_cuda(args):
             line["roofline"]["note"] = (
                 "fp64 pipe: DFMA and DMMA share one pipe (measured 37.0 TF/s at 1965 MHz, profiles/r1_fp64_peaks.md); "
                 "`achieved` = ALGORITHMIC flops of the stage (SURVEY.md 8(d): both directions of every pair, no recompute, "
-                "no padding, tanh not counted) / its CUDA-event time.  The kernels execute more than that: pass 2 recomputes "
-                "the forward chain and carries a tangent chain, tanh costs 19 pipe slots, 25 -> 28 padding on water; with "
-                "the same-species pair reuse they execute fewer chains than the algorithmic count for the nets (a,a) — so "
-                "this is a throughput figure, not a pipe-utilisation figure (that is ncu's, profiles/)")
+                "no padding, tanh not counted) / its CUDA-event time.  What the kernels execute differs: tanh costs 19 pipe "
+                "slots, 25 -> 28 padding on water; with the same-species pair reuse they execute fewer chains than the "
+                "algorithmic count for the nets (a,a); pass 2 reads the activations pass 1 stored (value chain and tanh not "
+                "re-run: its DRAM traffic is those records) unless --stored-act 0 or they do not fit — so this is a "
+                "throughput figure, not a pipe-utilisation figure (that is ncu's, profiles/)")
         else:
             line["roofline"]["note"] = (
                 f"algorithmic flops of the stage / its CUDA-event time against the dense tensor peak ({how}); the tensor "

@@ -19,7 +19,8 @@
 //
 // Kernels: k_pass1_dmma<SP, RB, RU> (RU: same-species pair reuse, T_j += g (x) R~_ji by fp64 reductions),
 // k_pass2_dmma<SP> and k_pass2_dmma_ru<SP> (pair reuse: the second direction reads dT_j slices staged by the TMA
-// engine).  One launch per net; a warp takes work items (atom, or a segment of an atom's rows for small chunks) from a
+// engine), k_pass2_dmma_st<SP, SA> (row stream over the atoms a warp takes; SA: the tanh outputs of the value chain are
+// read from the records pass 1 stored, ChunkView::act, and only the tangent chain runs).  One launch per net; a warp takes work items (atom, or a segment of an atom's rows for small chunks) from a
 // counter in global memory; the net's weights are staged by one TMA bulk copy per CTA.  DESIGN.md sections 6 and 12.
 #include "v1_kernels.cuh"
 #include "tc_common.cuh"
