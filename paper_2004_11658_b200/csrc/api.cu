@@ -484,8 +484,10 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     const int sp = m->v1.SP, stride = 4 * (((sp + 1) & ~1) + 6 * sp);
     const size_t bytes = sizeof(double) * (size_t)chunk * P.nm * stride;
     if (bytes <= m->ws_budget) {
-      CU(m->act.reserve(bytes), "workspace of the stored activations");
-      act_stride = stride;
+      const cudaError_t ea = m->act.reserve(bytes);
+      if (ea == cudaSuccess) act_stride = stride;
+      else if (ea == cudaErrorMemoryAllocation) cudaGetLastError();      // no room today: pass 2 recomputes
+      else return cuda_fail(ea, "workspace of the stored activations");
     }
   }
   if (!nlist_only) {
