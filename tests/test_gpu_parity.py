@@ -256,6 +256,38 @@ def test_full_size_parity_every_element(name, conditioned):
         m0.close()
 
 
+@pytest.mark.parametrize("s1,sel", [(8, (40, 60, 30)), (16, (40, 60, 30)), (8, (5, 7, 4))])
+def test_stored_activations_other_net_widths_and_overflow(s1, sel):
+    """The stored-activation kernels in their other instantiations (s1 = 8, 16: SP = 2, 4; the BASELINE configs use 7
+    and 8) on a 5,400-atom, 3-species box (a chunk of >= 4,096 centres is what switches them on), and with sections so
+    short that neighbours are dropped: the pair reuse then switches itself off on the device while pass 2 still reads the
+    records.  Every output element against the oracle, stored activations on and off."""
+    spec, emb, fit = small_model(ntypes=3, s1=s1, m_axis=4, fit_width=16, sel=sel, rcut=4.0, rcut_smth=1.0, seed=12,
+                                 fit_scale=0.05)
+    c0, t0, b0 = random_box(200, 10.0, 3, seed=31, min_dist=1.1)
+    shifts = np.array([[i, j, k] for i in range(3) for j in range(3) for k in range(3)], dtype=np.float64) * 10.0
+    coord = (c0[None, :, :] + shifts[:, None, :]).reshape(-1, 3)
+    coord = coord + np.random.default_rng(5).normal(0.0, 0.02, size=coord.shape)
+    types = np.tile(t0, 27)
+    box = np.diag([30.0, 30.0, 30.0]).reshape(-1)
+    orc, m = _models(spec, emb, fit, 1)
+    ref = orc.eval(coord, types, box)
+    _, ovf = orc.build_nlist(coord, types, box)
+    assert (ovf > 0) == (sel[0] < 10)
+    torch = _torch()
+    on = _gpu_eval(m, coord, types, box)
+    _check_full(ref, on, n_overflow=ovf)
+    free_on = torch.cuda.mem_get_info()[0]
+    m.set_stored_activations(False)                            # releases the records: that they existed shows the path ran
+    off = _gpu_eval(m, coord, types, box)
+    _check_full(ref, off, n_overflow=ovf)
+    sp = (s1 + 3) // 4
+    records = len(coord) * sum(sel) * 4 * (((sp + 1) & ~1) + 6 * sp) * 8
+    assert torch.cuda.mem_get_info()[0] - free_on >= 0.9 * records
+    assert np.abs(on["force"] - off["force"]).max() <= 1e-12 * max(1.0, np.abs(off["force"]).max())
+    m.close()
+
+
 def test_eval_host_matches_device_entry():
     """dpb_eval_host (host buffers, copies inside) returns the same numbers as dpb_eval."""
     torch = _torch()
