@@ -1014,14 +1014,15 @@ k_pass2_dmma_ru(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 // A block may therefore hold rows of two atoms (never more: it is cut short otherwise): the dE/dT slices of the (at
 // most two) centre atoms of a block come from L2 by the same TMA copies as the neighbours' slices, per N chunk, instead
 // of a per-atom tile in shared memory; F_i is added per row.
-template <int SP>
+template <int SP, bool BOTH = true>
 struct P2S {
+  static constexpr int JR = BOTH ? 8 : 0;                    // staged dT_j rows (none for a net without shared pairs)
   static constexpr int NBA = (SP + 1) / 2, NBB = SP - NBA;   // n-blocks of the two N chunks of a half (SP n-blocks)
   static constexpr int SLICE = 32 * NBA + 16;                // doubles per staged row slice (+128 B: rows on distinct banks)
   static constexpr int RING = 64;
   // per warp: dT_i slices [2][SLICE] | dT_j slices [8][SLICE] | ring (d, r) [RING] | ring ints j, row of j, centre row, i,
   //           record index [RING] | mbarrier | staging of 32 raw slots: (d, r) [32], j [32], sorted position of j [32]
-  static constexpr int per_warp = 10 * SLICE + 4 * RING + 2 * RING + RING / 2 + 2 + 4 * 32 + 16 + 16;
+  static constexpr int per_warp = (2 + JR) * SLICE + 4 * RING + 2 * RING + RING / 2 + 2 + 4 * 32 + 16 + 16;
 };
 
 // SA: the value chain is not run; t2v holds the stored tanh outputs of this chunk's slots (ChunkView::act).
@@ -1083,18 +1084,20 @@ __device__ __forceinline__ void p2s_chunk(const double *__restrict__ W2h, const 
   }
 }
 
-template <int SP, bool SA>
-__global__ void __launch_bounds__((32 * P2_WARPS), 1)
+// NW warps per CTA; BOTH = false: a net without shared pairs (a != t) — no dT_j slices, no second direction, and with SA
+// few enough registers and little enough shared memory for 12 warps
+template <int SP, bool SA, int NW, bool BOTH>
+__global__ void __launch_bounds__((32 * NW), 1)
 k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a, int t, double *__restrict__ force,
                 double *__restrict__ virial, int *counter) {
   using L = EL<SP>;
-  using R = P2S<SP>;
+  using R = P2S<SP, BOTH>;
   extern __shared__ __align__(16) double smem[];
   double *W = smem;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
   double *ibuf = smem + ((L::total + 1) & ~1) + warp * R::per_warp;     // [2][SLICE] dT slices of the block's centre atoms
   double *jbuf = ibuf + 2 * R::SLICE;                                   // [8][SLICE] dT slices of the rows' neighbours
-  double4 *rdv = reinterpret_cast<double4 *>(jbuf + 8 * R::SLICE);      // ring of kept rows: (d, r)
+  double4 *rdv = reinterpret_cast<double4 *>(jbuf + R::JR * R::SLICE);      // ring of kept rows: (d, r)
   int *rjn = reinterpret_cast<int *>(rdv + R::RING);                    //   input index of the neighbour
   int *rqj = rjn + R::RING;                                             //   its row in this chunk when both directions run, else -1
   int *rqa = rqj + R::RING;                                             //   row of the centre atom in this chunk
@@ -1104,7 +1107,7 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   double4 *sdr = reinterpret_cast<double4 *>(mbar + 2);                 // staged raw slots (cp.async, one batch ahead)
   int *snl = reinterpret_cast<int *>(sdr + 32);
   int *snlp = snl + 32;
-  __shared__ double vred[P2_WARPS][9];
+  __shared__ double vred[NW][9];
   __shared__ uint64_t wbar;
   if (lane == 0) tc::mbar_init(mbar, 1);
   tc::fence_mbar_init();
@@ -1112,7 +1115,7 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   const double *W0p = W + L::oW0, *b0p = W + L::ob0, *W1p = W + L::oW1, *b1p = W + L::ob1, *W2p = W + L::oW2,
                *b2p = W + L::ob2;
   const int row_lo = max(C.p0, C.type_start[a]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[a + 1]) - C.p0;
-  const bool ru = a == t && C.stats->n_overflow == 0ull;
+  const bool ru = BOTH && a == t && C.stats->n_overflow == 0ull;
   const size_t dt_tile = (size_t)C.dt_rows * 4;
   unsigned parity = 0;
   double vir[9];
@@ -1202,8 +1205,8 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
       }
       nrows = __popc(m0 | m1);                              // rows are ordered by atom: a prefix of the ring
       const int qjl = lane < nrows ? rqj[(head + lane) & (R::RING - 1)] : -1;
-      bmask = __ballot_sync(0xffffffffu, qjl >= 0);
-      myrow = qjl;                                          // lanes 0..7: row of the neighbour (or -1)
+      bmask = BOTH ? __ballot_sync(0xffffffffu, qjl >= 0) : 0u;
+      myrow = BOTH ? qjl : -1;                              // lanes 0..7: row of the neighbour (or -1)
       if (lane == 8) myrow = nrows > 0 ? a0 : -1;
       if (lane == 9) myrow = a1;
       const int rqg = __shfl_sync(0xffffffffu, rq, g);      // centre row of this thread's tile row
@@ -1228,8 +1231,8 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
     while (cnt > 0) {
       const int nr = nrows;
       const bool valid = g < nr;
-      const bool both = (bmask >> g) & 1u;
-      const bool anyboth = bmask != 0u;
+      const bool both = BOTH && ((bmask >> g) & 1u);
+      const bool anyboth = BOTH && bmask != 0u;
       // SA: the records are streamed from DRAM (written once by pass 1, read once here): the 8 ring rows behind this block
       // are prefetched into L2 now, one block (about 2,500 cycles) before their loads
       if (SA && lane < 8 && 8 + lane < cnt)
@@ -1299,25 +1302,31 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
 #pragma unroll 1
       for (int half = 0; half < 2; ++half) {
         const double *W2h = W2p + 8 * half * SP, *b2h = b2p + 8 * half * SP;
-        if (SA) {                                           // the stored t2 of a chunk are fetched one chunk ahead
-#pragma unroll
-          for (int s = 0; s < 2 * R::NBB; s += 2) {
-            double2 v = make_double2(0.0, 0.0);
-            if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + half * 2 * SP + 2 * R::NBA + s));
-            t2b[s] = v.x; t2b[s + 1] = v.y;
-          }
-        }
-        p2s_chunk<SP, R::NBA, 0, SA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, t2a, e, g, q, pr, pj);
-        __syncwarp();
-        issue(2 * half + 1);
-        if (SA && half == 0) {
+        // the stored t2 of a chunk are fetched one chunk ahead (BOTH: 2 warps per scheduler) or just before the chunk's
+        // DMMAs, which then cover the load (!BOTH: 12 warps at 168 registers — the lookahead's registers would spill)
+        auto load_t2a = [&](const int hf) {
 #pragma unroll
           for (int s = 0; s < 2 * R::NBA; s += 2) {
             double2 v = make_double2(0.0, 0.0);
-            if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + 2 * SP + s));
+            if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + hf * 2 * SP + s));
             t2a[s] = v.x; t2a[s + 1] = v.y;
           }
-        }
+        };
+        auto load_t2b = [&](const int hf) {
+#pragma unroll
+          for (int s = 0; s < 2 * R::NBB; s += 2) {
+            double2 v = make_double2(0.0, 0.0);
+            if (recp) v = act_load(recp + 4 * (L::A0 + 2 * SP + hf * 2 * SP + 2 * R::NBA + s));
+            t2b[s] = v.x; t2b[s + 1] = v.y;
+          }
+        };
+        if (SA && !BOTH && half == 1) load_t2a(1);
+        if (SA && BOTH) load_t2b(half);
+        p2s_chunk<SP, R::NBA, 0, SA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, t2a, e, g, q, pr, pj);
+        __syncwarp();
+        issue(2 * half + 1);
+        if (SA && BOTH && half == 0) load_t2a(1);
+        if (SA && !BOTH) load_t2b(half);
         p2s_chunk<SP, R::NBB, R::NBA, SA>(W2h, b2h, irow, jrow, anyboth, mbar, parity, h1v, h1t, t2b, e, g, q, pr, pj);
         __syncwarp();
         if (half == 0) issue(2);
@@ -1380,7 +1389,7 @@ k_pass2_dmma_st(DevModel P, ChunkView C, const double *__restrict__ netp, int a,
   __syncthreads();
   if (tid < 9 && virial) {
     double v = 0.0;
-    for (int w = 0; w < P2_WARPS; ++w) v += vred[w][tid];
+    for (int w = 0; w < NW; ++w) v += vred[w][tid];
     atomicAdd(&virial[tid], v);
   }
 }
@@ -1477,12 +1486,20 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
   // stored activations: pass 1 wrote a record for every row it evaluated (same nseg == 1 condition there)
   const bool sa = stream && C.act != nullptr && C.act_stride == L::REC &&
                   seg_count(C.n, P1_WARPS, P.ntypes * P.ntypes) == 1;
+  // nets a != t with stored activations: no staged neighbour slices and no second direction -> 12 warps per CTA
+  constexpr int NW1 = 12;
+  const size_t smem_one = sizeof(double) * (((L::total + 1) & ~1) + NW1 * P2S<SP, false>::per_warp);
   static bool configured_st_d[DPB_MAX_DEVICES] = {};
   bool &configured_st = configured_st_d[dpb_device()];
   if (stream && !configured_st) {
-    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_st);
+    cudaError_t e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, false, P2_WARPS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_st);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_st);
+      e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, true, P2_WARPS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)smem_st);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_pass2_dmma_st<SP, true, NW1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)smem_one);
     if (e != cudaSuccess) return e;
     configured_st = true;
   }
@@ -1497,12 +1514,15 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
     for (int t = P.ntypes - 1; t >= 0; --t) {
       const int net = a * P.ntypes + t;
       cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
-      if (sa)
-        k_pass2_dmma_st<SP, true><<<grid, (32 * P2_WARPS), smem_st, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t,
-                                                                           force, virial, C.counters + 64 + net);
+      if (sa && a != t)
+        k_pass2_dmma_st<SP, true, NW1, false><<<grid, (32 * NW1), smem_one, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a,
+                                                                                   t, force, virial, C.counters + 64 + net);
+      else if (sa)
+        k_pass2_dmma_st<SP, true, P2_WARPS, true><<<grid, (32 * P2_WARPS), smem_st, s>>>(
+            P, C, W.emb + (size_t)net * W.net_stride, a, t, force, virial, C.counters + 64 + net);
       else if (stream)
-        k_pass2_dmma_st<SP, false><<<grid, (32 * P2_WARPS), smem_st, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t,
-                                                                            force, virial, C.counters + 64 + net);
+        k_pass2_dmma_st<SP, false, P2_WARPS, true><<<grid, (32 * P2_WARPS), smem_st, s>>>(
+            P, C, W.emb + (size_t)net * W.net_stride, a, t, force, virial, C.counters + 64 + net);
       else if (reuse && a == t)
         k_pass2_dmma_ru<SP><<<grid, (32 * P2_WARPS), smem_ru, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a, t, force,
                                                                      virial, nseg, C.counters + 64 + net);
