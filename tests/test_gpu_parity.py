@@ -198,6 +198,8 @@ def test_errors_are_reported_not_thrown_from_c():
     _, m = _models(spec, emb, fit, 1)
     coord = torch.zeros((4, 3), dtype=torch.float64, device="cuda")
     types = torch.zeros((4,), dtype=torch.int32, device="cuda")
+    for setter, bad in ((m.lib.dpb_model_set_stored_activations, 2), (m.lib.dpb_model_set_pair_reuse, 3)):
+        assert setter(m._h, bad) == -1 and b"0" in m.lib.dpb_last_error()   # DPB_EINVAL, message names the values
     with pytest.raises(DPBError) as e:
         m.eval(coord, types, np.diag([7.0] * 3).reshape(9))                  # r_c = 4 >= L/2
     assert e.value.status == -2
