@@ -86,11 +86,14 @@ int dpb_model_destroy(dpb_model *model);
 /* Nm = sum_t sel[t]. */
 int dpb_model_nm(const dpb_model *model);
 
-/* Upper bound on the atoms processed per pass (bounds the workspace: about 73 KB per atom for the copper model).
- * chunk_atoms = 0 (the default) sizes it automatically: the largest chunk whose workspace fits in half of the device
- * memory that was free when the model was created, at least 32768 atoms (the 864,000-atom copper box then runs as one
- * chunk in 63 GB of the B200's 180 GB).  Larger chunks are faster: the same-species pair reuse shares only pairs whose
- * two atoms are centres of the same chunk.  Returns DPB_EINVAL if chunk < 0. */
+/* Upper bound on the atoms processed per pass (bounds the workspace: about 73 KB per atom for the copper model, plus the
+ * activation records where they are stored: Nm * 1.6-1.8 KB per atom).
+ * chunk_atoms = 0 (the default) sizes it automatically inside a budget of half of the device memory that was free when
+ * the model was created: one chunk if workspace and activation records of all centres fit (W24k, Cu32k); otherwise equal
+ * chunks of the largest size whose workspace and records fit, if that is at least 32768 atoms (the 864,000-atom copper
+ * box: 10 chunks of 87,040, 88 GB in use, 326 ms); otherwise the largest chunk whose workspace alone fits, at least
+ * 32768 atoms, and pass 2 recomputes.  Larger chunks are faster: the same-species pair reuse shares only pairs whose two
+ * atoms are centres of the same chunk.  Returns DPB_EINVAL if chunk < 0. */
 int dpb_model_set_chunk(dpb_model *model, int64_t chunk_atoms);
 
 /* Select the kernel generation: 0 = plain reference kernels ("v0": unfused, thread-per-output FMA loops),
@@ -136,9 +139,9 @@ int dpb_model_set_graph(dpb_model *model, int mode);
  * the two lists are then not symmetric.  T is summed in a different (and, with the reductions, run-to-run varying)
  * order: results move at the 1e-15 relative level.  Other precisions ignore it.
  *   on = 0  off (both passes)
- *   on = 1  (default) pass 2 always; pass 1 in evaluations that run as a single chunk (dpb_model_set_chunk): with several
- *           chunks only the pairs inside a chunk can be shared and pass 1's bookkeeping (clearing T, every accumulation a
- *           reduction) costs more than it saves (measured on the 864,000-atom box in 27 chunks)
+ *   on = 1  (default) pass 2 always; pass 1 in evaluations that run as a single chunk or in chunks of at least 32768
+ *           centres (dpb_model_set_chunk): only the pairs inside a chunk can be shared, and with thin chunks pass 1's
+ *           bookkeeping (clearing T, every accumulation a reduction) costs more than the sharing saves
  *   on = 2  both passes always (pairs across a chunk boundary are evaluated in both directions)
  * Returns DPB_EINVAL for any other value. */
 int dpb_model_set_pair_reuse(dpb_model *model, int on);
@@ -147,10 +150,11 @@ int dpb_model_set_pair_reuse(dpb_model *model, int on);
  * PAPER.md:113-123) along the value chain of pass 1.  on = 1: pass 1 writes the tanh outputs of the three layers of every
  * row it evaluates (7 s1 fp64 numbers per pair, streamed: written once, read once) and pass 2 reads them instead of
  * running the value chain and its tanh again; the arithmetic that remains is the same, so results do not change beyond
- * the summation order of the pair reuse.  Taken per evaluation when the records of a chunk (chunk * Nm * 14 * s1 * 8
- * bytes, padded) fit into the workspace budget (half of the memory that was free when the model was created), the chunk
- * has at least 4096 centres, the pair reuse is on and the deterministic reduction is off; otherwise, and with on = 0,
- * pass 2 recomputes (the paper's Eq. 13 tensors are then never written).  Returns DPB_EINVAL for any other value. */
+ * the summation order of the pair reuse.  Taken per evaluation when the records of a chunk (chunk * Nm * 7 * s1 * 8
+ * bytes, padded: 1,600 B per slot for s1 = 25) fit into the workspace budget (half of the memory that was free when the
+ * model was created; the automatic chunk size is chosen so that they do, see dpb_model_set_chunk), the chunk has at least
+ * 4096 centres, the pair reuse is on and the deterministic reduction is off; otherwise, and with on = 0, pass 2
+ * recomputes (the paper's Eq. 13 tensors are then never written).  Returns DPB_EINVAL for any other value. */
 int dpb_model_set_stored_activations(dpb_model *model, int on);
 
 /* Per-atom virial.  The paper gives no per-atom split (the virial is only named through the

@@ -84,12 +84,12 @@ static unsigned long long g_ws_epoch = 1;
 struct Buf {
   void *p = nullptr;
   size_t cap = 0;
-  cudaError_t reserve(size_t bytes, bool zero = false) {
+  cudaError_t reserve(size_t bytes, bool zero = false, bool exact = false) {
     if (bytes <= cap) return cudaSuccess;
     ++g_ws_epoch;
     if (p) cudaFree(p);
     p = nullptr; cap = 0;
-    size_t want = bytes + bytes / 8 + 256;
+    size_t want = exact ? bytes : bytes + bytes / 8 + 256;      // exact: the activation records (tens of GB)
     cudaError_t e = cudaMalloc(&p, want);
     if (e == cudaSuccess) cap = want;
     if (e == cudaSuccess && zero) e = cudaMemset(p, 0, want);      // (re)allocation only: synchronous, rare
@@ -162,7 +162,20 @@ static int nm_of(const DevModel &P) { return P.nm; }
 // rows, T, dT and the fitting activations: 73 KB per atom for the copper model in fp64) stays inside the budget fixed
 // at model creation, at least 32768 atoms.  Larger chunks are faster, not only smaller in launch count: the
 // same-species pair reuse only shares pairs whose two atoms are centres of the same chunk.
-static int64_t effective_chunk(const dpb_model *m) {
+// doubles per activation record (ChunkView::act_stride), or 0 when the stored activations cannot apply to this model
+static int act_record_doubles(const dpb_model *m) {
+  if (!m->stored_act || m->precision != DPB_FP64 || m->variant != 1 || !m->v1.ready || m->deterministic ||
+      m->pair_reuse < 1)
+    return 0;
+  const int sp = m->v1.SP;
+  return 4 * (((sp + 1) & ~1) + 6 * sp);
+}
+
+// ncentre > 0: the number of centres of the evaluation.  When the activation records (stored activations, DESIGN.md
+// section 12) of ONE chunk over all centres do not fit the budget but those of a chunk of at least 32768 centres do, the
+// evaluation is cut into equal chunks of that size: on the 864,000-atom copper box 10 chunks of 87,040 with the records
+// (326 ms) beat one chunk without them (365 ms) although the pairs across a chunk boundary are evaluated twice.
+static int64_t effective_chunk(const dpb_model *m, int64_t ncentre = -1) {
   if (m->chunk > 0) return m->chunk;
   if (m->precision != DPB_FP64) return 32768;            // mixed precision: the tile / pair-list kernels are sized for this
   const DevModel &P = m->P;
@@ -176,7 +189,19 @@ static int64_t effective_chunk(const dpb_model *m) {
   }
   int64_t c = (int64_t)(m->ws_budget / (per + 1));
   c -= c % 1024;
-  return c < 32768 ? 32768 : c;
+  c = c < 32768 ? 32768 : c;
+  const int rec = act_record_doubles(m);
+  if (rec > 0 && ncentre > 0) {
+    int64_t c_sa = (int64_t)(m->ws_budget / (per + (size_t)P.nm * rec * sizeof(double) + 1));
+    c_sa -= c_sa % 1024;
+    if (ncentre > c_sa && c_sa >= 32768) {
+      const int64_t nch = (ncentre + c_sa - 1) / c_sa;
+      int64_t bal = (ncentre + nch - 1) / nch;               // equal chunks
+      bal = (bal + 1023) / 1024 * 1024;
+      c = bal <= c_sa ? bal : c_sa;
+    }
+  }
+  return c;
 }
 
 extern "C" int dpb_model_nm(const dpb_model *m) { return m ? nm_of(m->P) : DPB_EINVAL; }
@@ -443,7 +468,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   const int N = (int)natoms;
   const int nkeys = P.ntypes * G.ngrp * G.ncell;
   const int64_t ncentre = nloc >= 0 ? nloc : natoms;
-  const int64_t chunk_cap = effective_chunk(m);
+  const int64_t chunk_cap = effective_chunk(m, nlist_only ? -1 : ncentre);
   const int64_t chunk = chunk_cap < ncentre ? chunk_cap : (ncentre > 0 ? ncentre : 1);
 
   CU(m->key.reserve(sizeof(int) * (size_t)(N + 1)), "workspace");
@@ -479,12 +504,11 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   // Stored activations (dpb_model_set_stored_activations): one record per (centre, slot) of the chunk, taken when the
   // records fit into the workspace budget and the chunk is large enough for whole-atom work items
   int act_stride = 0;
-  if (!nlist_only && m->stored_act && m->precision == DPB_FP64 && m->variant == 1 && m->v1.ready && !det &&
-      m->pair_reuse >= 1 && chunk >= 4096 && (size_t)chunk * P.nm < 2000000000ull) {
-    const int sp = m->v1.SP, stride = 4 * (((sp + 1) & ~1) + 6 * sp);
+  if (!nlist_only && act_record_doubles(m) > 0 && chunk >= 4096 && (size_t)chunk * P.nm < 2000000000ull) {
+    const int stride = act_record_doubles(m);
     const size_t bytes = sizeof(double) * (size_t)chunk * P.nm * stride;
     if (bytes <= m->ws_budget) {
-      const cudaError_t ea = m->act.reserve(bytes);
+      const cudaError_t ea = m->act.reserve(bytes, false, true);
       if (ea == cudaSuccess) act_stride = stride;
       else if (ea == cudaErrorMemoryAllocation) cudaGetLastError();      // no room today: pass 2 recomputes
       else return cuda_fail(ea, "workspace of the stored activations");
@@ -580,7 +604,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.fslot = nullptr;
     C.pos_of = m->pos_of.as<int>();
     C.stats = stats;
-    C.reuse = (!det && (m->pair_reuse == 2 || (m->pair_reuse == 1 && nchunks == 1))) ? 1 : 0;
+    C.reuse = (!det && (m->pair_reuse == 2 || (m->pair_reuse == 1 && (nchunks == 1 || chunk >= 32768)))) ? 1 : 0;
     C.reuse2 = (!det && m->pair_reuse >= 1) ? 1 : 0;     // pass 2 only reads dT_j: no bookkeeping, any chunking
     C.act = act_stride ? m->act.as<double>() : nullptr;
     C.act_stride = act_stride;
@@ -674,7 +698,7 @@ static int finish_info(dpb_model *m, cudaStream_t st, int64_t natoms, dpb_eval_i
     info->n_real_pairs = (int64_t)hs.n_real_pairs;
     info->n_overflow = (int64_t)hs.n_overflow;
     for (int t = 0; t < 8 && t < DPB_MAX_TYPES; ++t) info->max_nei[t] = hs.max_nei[t];
-    const int64_t chunk = effective_chunk(m);
+    const int64_t chunk = effective_chunk(m, natoms);
     info->n_chunks = (int32_t)((natoms + chunk - 1) / chunk);
   }
   return DPB_OK;
