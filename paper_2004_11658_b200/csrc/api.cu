@@ -158,10 +158,6 @@ struct dpb_model {
 
 static int nm_of(const DevModel &P) { return P.nm; }
 
-// Atoms per chunk.  An explicit dpb_model_set_chunk wins; otherwise the largest chunk whose workspace (lists, (d, r)
-// rows, T, dT and the fitting activations: 73 KB per atom for the copper model in fp64) stays inside the budget fixed
-// at model creation, at least 32768 atoms.  Larger chunks are faster, not only smaller in launch count: the
-// same-species pair reuse only shares pairs whose two atoms are centres of the same chunk.
 // doubles per activation record (ChunkView::act_stride), or 0 when the stored activations cannot apply to this model
 static int act_record_doubles(const dpb_model *m) {
   if (!m->stored_act || m->precision != DPB_FP64 || m->variant != 1 || !m->v1.ready || m->deterministic ||
@@ -171,6 +167,10 @@ static int act_record_doubles(const dpb_model *m) {
   return 4 * (((sp + 1) & ~1) + 6 * sp);
 }
 
+// Atoms per chunk.  An explicit dpb_model_set_chunk wins; otherwise the largest chunk whose workspace (lists, (d, r)
+// rows, T, dT and the fitting activations: 73 KB per atom for the copper model in fp64) stays inside the budget fixed
+// at model creation, at least 32768 atoms.  Larger chunks are faster, not only smaller in launch count: the
+// same-species pair reuse only shares pairs whose two atoms are centres of the same chunk.
 // ncentre > 0: the number of centres of the evaluation.  When the activation records (stored activations, DESIGN.md
 // section 12) of ONE chunk over all centres do not fit the budget but those of a chunk of at least 32768 centres do, the
 // evaluation is cut into equal chunks of that size: on the 864,000-atom copper box 10 chunks of 87,040 with the records
