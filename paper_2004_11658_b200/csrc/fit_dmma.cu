@@ -16,6 +16,7 @@
 // pipeline; shared-memory leading dimensions are 4 (mod 16) doubles, which makes the fragment loads conflict-free.
 #include "v1_kernels.cuh"
 
+#include <cooperative_groups.h>
 #include <vector>
 
 #define FIT_STAGES 3
@@ -366,6 +367,175 @@ __global__ void k_rowdot_v1(ChunkView C, int ty, int fwp, const double *__restri
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Small systems (BASELINE.json configs[0]): the middle of the fitting chain — bias + tanh of G1, G2, G3, the E_i row dot,
+// G4 and G5 — as ONE kernel on thread-block clusters.  A cluster of fwp / 48 CTAs owns a tile of 16 atoms; CTA r owns the
+// columns [48 r, 48 r + 48) of every layer (6 warps = 6 n-blocks, two m-blocks each) and streams only those columns of
+// the four w x w matrices (halves of K through a 3-buffer cp.async pipeline that runs ahead across the layers).  A layer's
+// full-width output, the next layer's A operand, is assembled in every CTA's shared memory by distributed-shared-memory
+// stores, one cluster barrier per layer; U1, Z1 / dZ1, U2 and Z0 of the own columns stay in registers.  Replaces six
+// dependent launches (10-14 us each at 192 atoms, bound by their latency) by one.  E_i is summed in a fixed order
+// (lanes, warps, then the cluster's CTAs at rank 0): no reductions.
+#define MID_WARPS 6
+#define MID_COLS (8 * MID_WARPS)
+#define MID_LDB (MID_COLS + 4)
+
+__global__ void __launch_bounds__(32 * MID_WARPS, 1)
+k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restrict__ Z0pre, double *__restrict__ Q,
+                  double *__restrict__ atom_energy) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
+  dpb_sub_range(C, row_lo, row_hi);
+  const int m0 = row_lo + blockIdx.y * 16;
+  if (m0 >= row_hi) return;                                  // the whole cluster (same blockIdx.y) leaves together
+  const int ncl = (int)cluster.num_blocks(), r = (int)cluster.block_rank();
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
+  const int lda = fwp + 4, kh = fwp / 2;
+  extern __shared__ __align__(16) double smem[];
+  double *bufA = smem, *bufB = bufA + 16 * lda;              // full-width activations [16][lda]
+  double *Bs = bufB + 16 * lda;                              // 3 x [kh][MID_LDB]: one half (in K) of a matrix' own columns
+  double *red = Bs + 3 * kh * MID_LDB;                       // [MID_WARPS][16] row sums of the warps
+  double *clred = red + MID_WARPS * 16;                      // [8][16] row sums of the cluster's CTAs (used at rank 0)
+  const int c0 = MID_COLS * r;                               // first own column
+
+  auto load_half = [&](int h) {                              // h = 2 layer + half; matrices W1, W2, W2^T, W1^T
+    if (h < 8) {
+      const double *Wm = (h >> 1) == 0 ? N.W1 : (h >> 1) == 1 ? N.W2 : (h >> 1) == 2 ? N.W2T : N.W1T;
+      const double *src = Wm + (size_t)(h & 1) * kh * fwp + c0;
+      double *dst = Bs + (h % 3) * kh * MID_LDB;
+      for (int c = tid; c < kh * (MID_COLS / 2); c += 32 * MID_WARPS) {
+        const int k = c / (MID_COLS / 2), nn = (c - k * (MID_COLS / 2)) * 2;
+        cp_async16(dst + k * MID_LDB + nn, src + (size_t)k * fwp + nn, true);
+      }
+    }
+    cp_async_commit();
+  };
+  load_half(0);
+  load_half(1);
+  // Z0 = tanh(pre-activation + b0), the whole tile in every CTA of the cluster (16 x fwp tanh: cheaper than an exchange)
+  for (int c = tid; c < 16 * (fwp / 2); c += 32 * MID_WARPS) {
+    const int m = c / (fwp / 2), n = (c - m * (fwp / 2)) * 2;
+    double2 v = make_double2(0.0, 0.0);
+    if (m0 + m < row_hi) v = *reinterpret_cast<const double2 *>(Z0pre + (size_t)(m0 + m) * fwp + n);
+    const double2 b = *reinterpret_cast<const double2 *>(N.b0 + n);
+    *reinterpret_cast<double2 *>(bufA + m * lda + n) = make_double2(dp_tanh(v.x + b.x), dp_tanh(v.y + b.y));
+  }
+  const int col = c0 + 8 * w + 2 * q;                        // this thread's columns col, col + 1; rows g, g + 8
+  double z0[2][2], u1[2][2], z1[2][2], acc[2][2][2];         // [m-block][column]; acc: [k parity][m-block][column]
+
+  auto gemm_half = [&](const double *A, int h) {             // acc += A[:, half of K] . B half (own columns)
+    cp_async_wait<1>();
+    __syncthreads();                                         // half h has landed; everyone is done with buffer (h + 2) % 3
+    load_half(h + 2);
+    const double *as = A + g * lda + (h & 1) * kh + q;
+    const double *bs = Bs + (h % 3) * kh * MID_LDB + q * MID_LDB + 8 * w + g;
+#pragma unroll 3
+    for (int ks = 0; ks < kh / 4; ks += 2) {                 // kh / 4 is even: two independent accumulator sets
+      const double be = bs[4 * ks * MID_LDB], bo = bs[4 * (ks + 1) * MID_LDB];
+      dmma884f(acc[0][0][0], acc[0][0][1], as[4 * ks], be);
+      dmma884f(acc[0][1][0], acc[0][1][1], as[8 * lda + 4 * ks], be);
+      dmma884f(acc[1][0][0], acc[1][0][1], as[4 * ks + 4], bo);
+      dmma884f(acc[1][1][0], acc[1][1][1], as[8 * lda + 4 * ks + 4], bo);
+    }
+  };
+  auto clear_acc = [&]() {
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+      for (int mb = 0; mb < 2; ++mb) { acc[p][mb][0] = 0.0; acc[p][mb][1] = 0.0; }
+  };
+  auto broadcast = [&](double *buf, const double (&v)[2][2]) {   // own columns of a full-width tile, into every CTA
+    for (int rr = 0; rr < ncl; ++rr) {
+      double *peer = cluster.map_shared_rank(buf, rr);
+#pragma unroll
+      for (int mb = 0; mb < 2; ++mb)
+        *reinterpret_cast<double2 *>(peer + (g + 8 * mb) * lda + col) = make_double2(v[mb][0], v[mb][1]);
+    }
+  };
+
+  // G2: U1 = tanh(Z0 W1 + b1), Z1 = Z0 + U1
+  clear_acc();
+  gemm_half(bufA, 0);                                        // (its barrier also publishes the Z0 tile)
+#pragma unroll
+  for (int mb = 0; mb < 2; ++mb) { z0[mb][0] = bufA[(g + 8 * mb) * lda + col]; z0[mb][1] = bufA[(g + 8 * mb) * lda + col + 1]; }
+  gemm_half(bufA, 1);
+  {
+    const double2 b = *reinterpret_cast<const double2 *>(N.b1 + col);
+#pragma unroll
+    for (int mb = 0; mb < 2; ++mb) {
+      u1[mb][0] = dp_tanh(acc[0][mb][0] + acc[1][mb][0] + b.x);
+      u1[mb][1] = dp_tanh(acc[0][mb][1] + acc[1][mb][1] + b.y);
+      z1[mb][0] = z0[mb][0] + u1[mb][0];
+      z1[mb][1] = z0[mb][1] + u1[mb][1];
+    }
+    broadcast(bufB, z1);
+  }
+  cluster.sync();
+  // G3: U2 = tanh(Z1 W2 + b2), Z2 = Z1 + U2, E_i = Z2 . w3 + b3, Q2 = w3 (1 - U2^2)
+  const double2 w3 = *reinterpret_cast<const double2 *>(N.w3 + col);
+  clear_acc();
+  gemm_half(bufB, 2);
+  gemm_half(bufB, 3);
+  {
+    const double2 b = *reinterpret_cast<const double2 *>(N.b2 + col);
+    double q2[2][2], es[2];
+#pragma unroll
+    for (int mb = 0; mb < 2; ++mb) {
+      const double ua = dp_tanh(acc[0][mb][0] + acc[1][mb][0] + b.x), ub = dp_tanh(acc[0][mb][1] + acc[1][mb][1] + b.y);
+      es[mb] = fma(z1[mb][0] + ua, w3.x, (z1[mb][1] + ub) * w3.y);
+      q2[mb][0] = w3.x * (1.0 - ua * ua);
+      q2[mb][1] = w3.y * (1.0 - ub * ub);
+      es[mb] += __shfl_xor_sync(0xffffffffu, es[mb], 1);
+      es[mb] += __shfl_xor_sync(0xffffffffu, es[mb], 2);
+    }
+    if (q == 0) { red[w * 16 + g] = es[0]; red[w * 16 + g + 8] = es[1]; }
+    broadcast(bufA, q2);
+    __syncthreads();
+    if (tid < 16) {
+      double s = 0.0;
+#pragma unroll
+      for (int ww = 0; ww < MID_WARPS; ++ww) s += red[ww * 16 + tid];
+      cluster.map_shared_rank(clred, 0)[r * 16 + tid] = s;
+    }
+  }
+  cluster.sync();
+  if (r == 0 && tid < 16 && m0 + tid < row_hi) {
+    double s = N.b3;
+    for (int rr = 0; rr < ncl; ++rr) s += clred[rr * 16 + tid];
+    atom_energy[C.s_idx[C.p0 + m0 + tid]] = s;
+  }
+  // G4: dZ1 = w3 + Q2 W2^T, Q1 = dZ1 (1 - U1^2)
+  clear_acc();
+  gemm_half(bufA, 4);
+  gemm_half(bufA, 5);
+  {
+    double q1[2][2];
+#pragma unroll
+    for (int mb = 0; mb < 2; ++mb) {
+      z1[mb][0] = w3.x + acc[0][mb][0] + acc[1][mb][0];        // dZ1
+      z1[mb][1] = w3.y + acc[0][mb][1] + acc[1][mb][1];
+      q1[mb][0] = z1[mb][0] * (1.0 - u1[mb][0] * u1[mb][0]);
+      q1[mb][1] = z1[mb][1] * (1.0 - u1[mb][1] * u1[mb][1]);
+    }
+    broadcast(bufB, q1);
+  }
+  cluster.sync();
+  // G5: dZ0 = dZ1 + Q1 W1^T, Q0 = dZ0 (1 - Z0^2): the A operand of G6
+  clear_acc();
+  gemm_half(bufB, 6);
+  gemm_half(bufB, 7);
+#pragma unroll
+  for (int mb = 0; mb < 2; ++mb) {
+    const int m = m0 + g + 8 * mb;
+    if (m >= row_hi) continue;
+    const double da = z1[mb][0] + acc[0][mb][0] + acc[1][mb][0], db = z1[mb][1] + acc[0][mb][1] + acc[1][mb][1];
+    *reinterpret_cast<double2 *>(Q + (size_t)m * fwp + col) =
+        make_double2(da * (1.0 - z0[mb][0] * z0[mb][0]), db * (1.0 - z0[mb][1] * z0[mb][1]));
+  }
+  cp_async_wait<0>();
+}
+
+// ---------------------------------------------------------------------------------------------------------
 static int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 // The padded fitting weights hang off V1Weights::fit (opaque pointer declared in v1_kernels.cuh).
@@ -491,6 +661,19 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
   cudaError_t e;
 
   const bool splitk = C.n <= FIT_SMALL_N && !C.fslot;    // (not in deterministic mode: the partial sums are reductions)
+  // small systems: the middle of the chain as one cluster kernel when the width is a multiple of 48 (clusters of <= 8 CTAs)
+  const size_t smem_mid = sizeof(double) * (2 * 16 * (size_t)(fwp + 4) + 3 * (size_t)(fwp / 2) * MID_LDB + 16 * (MID_WARPS + 8));
+  const bool mid = splitk && fwp % MID_COLS == 0 && fwp / MID_COLS <= 8 && smem_mid <= 227 * 1024;
+  if (mid) {
+    static bool mid_configured_d[DPB_MAX_DEVICES] = {};
+    bool &mid_configured = mid_configured_d[dpb_device()];
+    if (!mid_configured) {
+      if ((e = cudaFuncSetAttribute(k_fit_mid_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024))) !=
+          cudaSuccess)
+        return e;
+      mid_configured = true;
+    }
+  }
   if (splitk && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
   // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint.  The
   // descriptor and dT kernels (memory-bound) belong to the chains: one species' run beside the other's GEMMs
@@ -524,6 +707,22 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
     // G1: Z0 = tanh(D W0 + b0).  Small systems: split-K over 8 CTAs (K = dim is a serial loop of dim / 16 tiles for
     // the few CTAs a 192-atom box offers), partial sums added into the cleared Z0, bias and tanh in a second kernel.
     g = GemmArgs{D, dimp, N.W0, fwp, dimp, fwp, N.b0, nullptr, nullptr, fwp, Z0, nullptr, fwp};
+    if (splitk && mid) {
+      // bias + tanh of G1, G2, G3, E_i, G4, G5 in one cluster kernel (k_fit_mid_cluster): Z0 holds the pre-activation sums
+      if ((e = gemm_t<1, 3, EPI_ATOMIC, 80>(C, ty, g, s, 8)) != cudaSuccess) return e;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)(fwp / MID_COLS), (unsigned)((C.n + 15) / 16), 1);
+      cfg.blockDim = dim3(32 * MID_WARPS, 1, 1);
+      cfg.dynamicSmemBytes = smem_mid;
+      cfg.stream = s;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = (unsigned)(fwp / MID_COLS); at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      if ((e = cudaLaunchKernelEx(&cfg, k_fit_mid_cluster, C, ty, fwp, N, (const double *)Z0, Q, atom_energy)) != cudaSuccess)
+        return e;
+      DPB_LAUNCHED(1);
+    } else {
     if (splitk) {
       if ((e = gemm_t<1, 3, EPI_ATOMIC, 80>(C, ty, g, s, 8)) != cudaSuccess) return e;
       k_bias_tanh_v1<<<C.n, 64, 0, s>>>(C, ty, fwp, N.b0, Z0);
@@ -543,6 +742,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
     // G5: dZ0 = dZ1 + Q' W1^T; Q = dZ0 (1 - Z0^2)
     g = GemmArgs{Q2, fwp, N.W1T, fwp, fwp, fwp, nullptr, Z1, Z0, fwp, nullptr, Q, fwp};
     if ((e = gemm<15, EPI_BWD>(C, ty, g, s)) != cudaSuccess) return e;
+    }
     // G6: dD = Q W0^T
     g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
     if ((e = gemm<8, EPI_STORE>(C, ty, g, s)) != cudaSuccess) return e;
