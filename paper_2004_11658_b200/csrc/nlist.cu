@@ -32,10 +32,8 @@ __device__ __forceinline__ bool displacement_in_range(const double xi[3], const 
 }
 
 // ---------------------------------------------------------------------------------------------------------
-__global__ void k_keys(DevModel P, DevGrid G, int n, const double *__restrict__ coord, const int *__restrict__ type,
-                       int *__restrict__ key, int *__restrict__ count, DevStats *stats) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+__device__ __forceinline__ int sort_key(const DevModel &P, const DevGrid &G, int i, const double *__restrict__ coord,
+                                        const int *__restrict__ type, DevStats *stats) {
   int ic[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
@@ -53,15 +51,21 @@ __global__ void k_keys(DevModel P, DevGrid G, int n, const double *__restrict__ 
     t = 0;
   }
   if (G.ngrp == 2 && i >= G.nloc) t += P.ntypes;                   // ghosts: behind every local atom
-  int k = t * G.ncell + (ic[0] * G.nc[1] + ic[1]) * G.nc[2] + ic[2];
+  return t * G.ncell + (ic[0] * G.nc[1] + ic[1]) * G.nc[2] + ic[2];
+}
+
+__global__ void k_keys(DevModel P, DevGrid G, int n, const double *__restrict__ coord, const int *__restrict__ type,
+                       int *__restrict__ key, int *__restrict__ count, DevStats *stats) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int k = sort_key(P, G, i, coord, type, stats);
   key[i] = k;
   atomicAdd(&count[k], 1);
 }
 
 // Exclusive scan of count[0..nkeys) by one block; also writes cursor = start and type_start[t] = start[t*ncell].
-__global__ void k_scan(int nkeys, int ncell, int ntypes, const int *__restrict__ count, int *__restrict__ start,
-                       int *__restrict__ cursor, int *__restrict__ type_start) {
-  __shared__ int part[1024];
+__device__ __forceinline__ void scan_block(int nkeys, int ncell, int ntypes, const int *count, int *start, int *cursor,
+                                           int *type_start, int *part) {
   const int tid = threadIdx.x;
   const int seg = (nkeys + 1023) / 1024;
   const int lo = tid * seg, hi = min(nkeys, lo + seg);
@@ -88,10 +92,14 @@ __global__ void k_scan(int nkeys, int ncell, int ntypes, const int *__restrict__
   }
 }
 
-__global__ void k_fill(int n, const double *__restrict__ coord, const int *__restrict__ key, int *__restrict__ cursor,
-                       int *__restrict__ s_idx, double *__restrict__ s_xyz, int *__restrict__ pos_of) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+__global__ void k_scan(int nkeys, int ncell, int ntypes, const int *__restrict__ count, int *__restrict__ start,
+                       int *__restrict__ cursor, int *__restrict__ type_start) {
+  __shared__ int part[1024];
+  scan_block(nkeys, ncell, ntypes, count, start, cursor, type_start, part);
+}
+
+__device__ __forceinline__ void fill_one(int i, const double *__restrict__ coord, const int *key, int *cursor,
+                                         int *__restrict__ s_idx, double *__restrict__ s_xyz, int *__restrict__ pos_of) {
   int p = atomicAdd(&cursor[key[i]], 1);   // order inside a (type, cell) bucket is irrelevant: Alg. 1's key is total
   s_idx[p] = i;
   if (pos_of) pos_of[i] = p;
@@ -100,13 +108,46 @@ __global__ void k_fill(int n, const double *__restrict__ coord, const int *__res
   s_xyz[3 * (size_t)p + 2] = coord[3 * (size_t)i + 2];
 }
 
+__global__ void k_fill(int n, const double *__restrict__ coord, const int *__restrict__ key, int *__restrict__ cursor,
+                       int *__restrict__ s_idx, double *__restrict__ s_xyz, int *__restrict__ pos_of) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  fill_one(i, coord, key, cursor, s_idx, s_xyz, pos_of);
+}
+
+// Small systems: keys, scan and fill by ONE block (a 192-atom evaluation is bound by its chain of dependent launches:
+// three launches and a memset become one; same arithmetic, same arrays).
+#define SORT_SMALL_N 4096
+__global__ void __launch_bounds__(1024)
+k_sort_small(DevModel P, DevGrid G, int n, int nkeys, const double *__restrict__ coord, const int *__restrict__ type,
+             int *key, int *count, int *start, int *cursor, int *__restrict__ s_idx, double *__restrict__ s_xyz,
+             DevStats *stats, int *__restrict__ pos_of) {
+  __shared__ int part[1024];
+  for (int k = threadIdx.x; k < nkeys; k += 1024) count[k] = 0;
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += 1024) {
+    const int k = sort_key(P, G, i, coord, type, stats);
+    key[i] = k;
+    atomicAdd(&count[k], 1);
+  }
+  __syncthreads();
+  scan_block(nkeys, G.ncell, P.ntypes * G.ngrp, count, start, cursor, start + nkeys + 1, part);
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += 1024) fill_one(i, coord, key, cursor, s_idx, s_xyz, pos_of);
+}
+
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
                              DevStats *stats, cudaStream_t st, int *pos_of) {
   const int nkeys = P.ntypes * G.ngrp * G.ncell;
+  const int n = (int)natoms;
+  if (n > 0 && n <= SORT_SMALL_N && nkeys <= 4 * SORT_SMALL_N) {
+    k_sort_small<<<1, 1024, 0, st>>>(P, G, n, nkeys, coord, type, key, count, start, cursor, s_idx, s_xyz, stats, pos_of);
+    DPB_LAUNCHED(1);
+    return cudaGetLastError();
+  }
   cudaError_t e = cudaMemsetAsync(count, 0, sizeof(int) * (size_t)nkeys, st);
   if (e != cudaSuccess) return e;
-  const int n = (int)natoms;
   if (n > 0) k_keys<<<(n + 255) / 256, 256, 0, st>>>(P, G, n, coord, type, key, count, stats);
   // type_start lives right behind start[nkeys + 1]
   k_scan<<<1, 1024, 0, st>>>(nkeys, G.ncell, P.ntypes * G.ngrp, count, start, cursor, start + nkeys + 1);
