@@ -584,6 +584,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   }
   const int cap = neighbour_cap(P);
   int ci = 0;
+  bool energy_done = false;
   for (int64_t p0 = 0; p0 < ncentre; p0 += chunk, ++ci) {
     ChunkView C;
     C.p0 = (int)p0;
@@ -653,7 +654,17 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
       CU(v1_fit(P, C, m->v1, m->fit.as<double>(), m->v1ws.p, ei, st), "fit");
       CU(launch_scatter_debug(P, C, m->dbgT, m->dbgdT, st), "debug scatter");
       if (timing) cudaEventRecord(m->evs[4 + 4 * ci], st);
+      // Small single-chunk evaluations: E = sum E_i (complete once the fitting stage has run) goes on a forked stream
+      // beside pass 2 instead of behind it — one dependent launch less in a chain that is bound by its launches.
+      cudaStream_t es[DPB_MAX_TYPES];
+      const bool early_e = energy && !timing && nchunks == 1 && ncentre <= 4096;
+      if (early_e) {
+        CU(dpb_fork_streams(2, st, es), "fork");
+        CU(launch_reduce_energy(ncentre, ei, energy, es[1]), "energy reduction");
+        energy_done = true;
+      }
       CU(v1_pass2(P, C, m->v1, force, virial, st), "pass2");
+      if (early_e) CU(dpb_join_streams(2, st, es), "join");
       if (timing) cudaEventRecord(m->evs[5 + 4 * ci], st);
     }
   }
@@ -679,7 +690,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
                            force, m->atom_virial ? m->atom_virial : m->vpart.as<double>(), virial, st),
        "deterministic force gather");
   if (!nlist_only) {
-    if (energy) CU(launch_reduce_energy(ncentre, ei, energy, st), "energy reduction");
+    if (energy && !energy_done) CU(launch_reduce_energy(ncentre, ei, energy, st), "energy reduction");
     if (timing) cudaEventRecord(m->evs[2 + 4 * nchunks], st);
   }
   return DPB_OK;
