@@ -369,15 +369,17 @@ __global__ void k_rowdot_v1(ChunkView C, int ty, int fwp, const double *__restri
 // ---------------------------------------------------------------------------------------------------------
 // Small systems (BASELINE.json configs[0]): the middle of the fitting chain — bias + tanh of G1, G2, G3, the E_i row dot,
 // G4 and G5 — as ONE kernel on thread-block clusters.  A cluster of fwp / 48 CTAs owns a tile of 16 atoms; CTA r owns the
-// columns [48 r, 48 r + 48) of every layer (6 warps = 6 n-blocks, two m-blocks each) and streams only those columns of
-// the four w x w matrices (halves of K through a 3-buffer cp.async pipeline that runs ahead across the layers).  A layer's
-// full-width output, the next layer's A operand, is assembled in every CTA's shared memory by distributed-shared-memory
-// stores, one cluster barrier per layer; U1, Z1 / dZ1, U2 and Z0 of the own columns stay in registers.  Replaces six
-// dependent launches (10-14 us each at 192 atoms, bound by their latency) by one.  E_i is summed in a fixed order
-// (lanes, warps, then the cluster's CTAs at rank 0): no reductions.
-#define MID_WARPS 6
-#define MID_COLS (8 * MID_WARPS)
+// columns [48 r, 48 r + 48) of every layer (12 warps = 6 n-blocks x 2 m-blocks: three warps per scheduler) and streams
+// only those columns of the four w x w matrices (halves of K through a 3-buffer cp.async pipeline that runs ahead across
+// the layers).  A layer's full-width output, the next layer's A operand, is assembled in every CTA's shared memory by
+// distributed-shared-memory stores, one cluster barrier per layer; U1, Z1 / dZ1, U2 and Z0 of the own columns stay in
+// registers.  Replaces six dependent launches (10-14 us each at 192 atoms, bound by their latency) by one.  E_i is summed
+// in a fixed order (lanes, warps, then the cluster's CTAs at rank 0): no reductions.
+#define MID_NB 6                                              // n-blocks (8 columns) per CTA
+#define MID_WARPS (2 * MID_NB)
+#define MID_COLS (8 * MID_NB)
 #define MID_LDB (MID_COLS + 4)
+#define MID_ZI 5                                              // loads of the Z0 tile per thread (16 x 240 / 2 / 384)
 
 __global__ void __launch_bounds__(32 * MID_WARPS, 1)
 k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restrict__ Z0pre, double *__restrict__ Q,
@@ -390,12 +392,13 @@ k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restri
   if (m0 >= row_hi) return;                                  // the whole cluster (same blockIdx.y) leaves together
   const int ncl = (int)cluster.num_blocks(), r = (int)cluster.block_rank();
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
+  const int nbk = w % MID_NB, row = g + 8 * (w / MID_NB);    // this warp's n-block and m-block: the thread's tile row
   const int lda = fwp + 4, kh = fwp / 2;
   extern __shared__ __align__(16) double smem[];
   double *bufA = smem, *bufB = bufA + 16 * lda;              // full-width activations [16][lda]
   double *Bs = bufB + 16 * lda;                              // 3 x [kh][MID_LDB]: one half (in K) of a matrix' own columns
-  double *red = Bs + 3 * kh * MID_LDB;                       // [MID_WARPS][16] row sums of the warps
-  double *clred = red + MID_WARPS * 16;                      // [8][16] row sums of the cluster's CTAs (used at rank 0)
+  double *red = Bs + 3 * kh * MID_LDB;                       // [MID_NB][16] row sums of the warps
+  double *clred = red + MID_NB * 16;                         // [8][16] row sums of the cluster's CTAs (used at rank 0)
   const int c0 = MID_COLS * r;                               // first own column
 
   auto load_half = [&](int h) {                              // h = 2 layer + half; matrices W1, W2, W2^T, W1^T
@@ -412,62 +415,68 @@ k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restri
   };
   load_half(0);
   load_half(1);
-  // Z0 = tanh(pre-activation + b0), the whole tile in every CTA of the cluster (16 x fwp tanh: cheaper than an exchange)
-  for (int c = tid; c < 16 * (fwp / 2); c += 32 * MID_WARPS) {
-    const int m = c / (fwp / 2), n = (c - m * (fwp / 2)) * 2;
-    double2 v = make_double2(0.0, 0.0);
-    if (m0 + m < row_hi) v = *reinterpret_cast<const double2 *>(Z0pre + (size_t)(m0 + m) * fwp + n);
-    const double2 b = *reinterpret_cast<const double2 *>(N.b0 + n);
-    *reinterpret_cast<double2 *>(bufA + m * lda + n) = make_double2(dp_tanh(v.x + b.x), dp_tanh(v.y + b.y));
+  // Z0 = tanh(pre-activation + b0), the whole tile in every CTA of the cluster (16 x fwp tanh: cheaper than an exchange);
+  // all loads of a thread first, then the arithmetic: one memory latency, not one per element
+  {
+    const int total = 16 * (fwp / 2);
+    double2 v[MID_ZI], b[MID_ZI];
+#pragma unroll
+    for (int u = 0; u < MID_ZI; ++u) {
+      const int c = tid + u * 32 * MID_WARPS;
+      const int m = c / (fwp / 2), n = (c - m * (fwp / 2)) * 2;
+      v[u] = make_double2(0.0, 0.0); b[u] = v[u];
+      if (c < total) {
+        b[u] = *reinterpret_cast<const double2 *>(N.b0 + n);
+        if (m0 + m < row_hi) v[u] = *reinterpret_cast<const double2 *>(Z0pre + (size_t)(m0 + m) * fwp + n);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < MID_ZI; ++u) {
+      const int c = tid + u * 32 * MID_WARPS;
+      const int m = c / (fwp / 2), n = (c - m * (fwp / 2)) * 2;
+      if (c < total)
+        *reinterpret_cast<double2 *>(bufA + m * lda + n) = make_double2(dp_tanh(v[u].x + b[u].x), dp_tanh(v[u].y + b[u].y));
+    }
+    for (int c = tid + MID_ZI * 32 * MID_WARPS; c < total; c += 32 * MID_WARPS) {      // (wider than 240: not launched)
+      const int m = c / (fwp / 2), n = (c - m * (fwp / 2)) * 2;
+      double2 x = make_double2(0.0, 0.0);
+      if (m0 + m < row_hi) x = *reinterpret_cast<const double2 *>(Z0pre + (size_t)(m0 + m) * fwp + n);
+      const double2 bb = *reinterpret_cast<const double2 *>(N.b0 + n);
+      *reinterpret_cast<double2 *>(bufA + m * lda + n) = make_double2(dp_tanh(x.x + bb.x), dp_tanh(x.y + bb.y));
+    }
   }
-  const int col = c0 + 8 * w + 2 * q;                        // this thread's columns col, col + 1; rows g, g + 8
-  double z0[2][2], u1[2][2], z1[2][2], acc[2][2][2];         // [m-block][column]; acc: [k parity][m-block][column]
+  const int col = c0 + 8 * nbk + 2 * q;                      // this thread's columns col, col + 1 of row `row`
+  double z0[2], u1[2], z1[2], acc[2][2];                     // [column]; acc: [k parity][column]
 
   auto gemm_half = [&](const double *A, int h) {             // acc += A[:, half of K] . B half (own columns)
     cp_async_wait<1>();
     __syncthreads();                                         // half h has landed; everyone is done with buffer (h + 2) % 3
     load_half(h + 2);
-    const double *as = A + g * lda + (h & 1) * kh + q;
-    const double *bs = Bs + (h % 3) * kh * MID_LDB + q * MID_LDB + 8 * w + g;
-#pragma unroll 3
+    const double *as = A + row * lda + (h & 1) * kh + q;
+    const double *bs = Bs + (h % 3) * kh * MID_LDB + q * MID_LDB + 8 * nbk + g;
+#pragma unroll 5
     for (int ks = 0; ks < kh / 4; ks += 2) {                 // kh / 4 is even: two independent accumulator sets
-      const double be = bs[4 * ks * MID_LDB], bo = bs[4 * (ks + 1) * MID_LDB];
-      dmma884f(acc[0][0][0], acc[0][0][1], as[4 * ks], be);
-      dmma884f(acc[0][1][0], acc[0][1][1], as[8 * lda + 4 * ks], be);
-      dmma884f(acc[1][0][0], acc[1][0][1], as[4 * ks + 4], bo);
-      dmma884f(acc[1][1][0], acc[1][1][1], as[8 * lda + 4 * ks + 4], bo);
+      dmma884f(acc[0][0], acc[0][1], as[4 * ks], bs[4 * ks * MID_LDB]);
+      dmma884f(acc[1][0], acc[1][1], as[4 * ks + 4], bs[4 * (ks + 1) * MID_LDB]);
     }
   };
-  auto clear_acc = [&]() {
-#pragma unroll
-    for (int p = 0; p < 2; ++p)
-#pragma unroll
-      for (int mb = 0; mb < 2; ++mb) { acc[p][mb][0] = 0.0; acc[p][mb][1] = 0.0; }
-  };
-  auto broadcast = [&](double *buf, const double (&v)[2][2]) {   // own columns of a full-width tile, into every CTA
-    for (int rr = 0; rr < ncl; ++rr) {
-      double *peer = cluster.map_shared_rank(buf, rr);
-#pragma unroll
-      for (int mb = 0; mb < 2; ++mb)
-        *reinterpret_cast<double2 *>(peer + (g + 8 * mb) * lda + col) = make_double2(v[mb][0], v[mb][1]);
-    }
+  auto clear_acc = [&]() { acc[0][0] = 0.0; acc[0][1] = 0.0; acc[1][0] = 0.0; acc[1][1] = 0.0; };
+  auto broadcast = [&](double *buf, const double (&v)[2]) {  // own columns of a full-width tile, into every CTA
+    for (int rr = 0; rr < ncl; ++rr)
+      *reinterpret_cast<double2 *>(cluster.map_shared_rank(buf, rr) + row * lda + col) = make_double2(v[0], v[1]);
   };
 
   // G2: U1 = tanh(Z0 W1 + b1), Z1 = Z0 + U1
   clear_acc();
   gemm_half(bufA, 0);                                        // (its barrier also publishes the Z0 tile)
-#pragma unroll
-  for (int mb = 0; mb < 2; ++mb) { z0[mb][0] = bufA[(g + 8 * mb) * lda + col]; z0[mb][1] = bufA[(g + 8 * mb) * lda + col + 1]; }
+  z0[0] = bufA[row * lda + col]; z0[1] = bufA[row * lda + col + 1];
   gemm_half(bufA, 1);
   {
     const double2 b = *reinterpret_cast<const double2 *>(N.b1 + col);
-#pragma unroll
-    for (int mb = 0; mb < 2; ++mb) {
-      u1[mb][0] = dp_tanh(acc[0][mb][0] + acc[1][mb][0] + b.x);
-      u1[mb][1] = dp_tanh(acc[0][mb][1] + acc[1][mb][1] + b.y);
-      z1[mb][0] = z0[mb][0] + u1[mb][0];
-      z1[mb][1] = z0[mb][1] + u1[mb][1];
-    }
+    u1[0] = dp_tanh(acc[0][0] + acc[1][0] + b.x);
+    u1[1] = dp_tanh(acc[0][1] + acc[1][1] + b.y);
+    z1[0] = z0[0] + u1[0];
+    z1[1] = z0[1] + u1[1];
     broadcast(bufB, z1);
   }
   cluster.sync();
@@ -478,23 +487,18 @@ k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restri
   gemm_half(bufB, 3);
   {
     const double2 b = *reinterpret_cast<const double2 *>(N.b2 + col);
-    double q2[2][2], es[2];
-#pragma unroll
-    for (int mb = 0; mb < 2; ++mb) {
-      const double ua = dp_tanh(acc[0][mb][0] + acc[1][mb][0] + b.x), ub = dp_tanh(acc[0][mb][1] + acc[1][mb][1] + b.y);
-      es[mb] = fma(z1[mb][0] + ua, w3.x, (z1[mb][1] + ub) * w3.y);
-      q2[mb][0] = w3.x * (1.0 - ua * ua);
-      q2[mb][1] = w3.y * (1.0 - ub * ub);
-      es[mb] += __shfl_xor_sync(0xffffffffu, es[mb], 1);
-      es[mb] += __shfl_xor_sync(0xffffffffu, es[mb], 2);
-    }
-    if (q == 0) { red[w * 16 + g] = es[0]; red[w * 16 + g + 8] = es[1]; }
+    const double ua = dp_tanh(acc[0][0] + acc[1][0] + b.x), ub = dp_tanh(acc[0][1] + acc[1][1] + b.y);
+    double es = fma(z1[0] + ua, w3.x, (z1[1] + ub) * w3.y);
+    const double q2[2] = {w3.x * (1.0 - ua * ua), w3.y * (1.0 - ub * ub)};
+    es += __shfl_xor_sync(0xffffffffu, es, 1);
+    es += __shfl_xor_sync(0xffffffffu, es, 2);
+    if (q == 0) red[nbk * 16 + row] = es;
     broadcast(bufA, q2);
     __syncthreads();
     if (tid < 16) {
       double s = 0.0;
 #pragma unroll
-      for (int ww = 0; ww < MID_WARPS; ++ww) s += red[ww * 16 + tid];
+      for (int nb = 0; nb < MID_NB; ++nb) s += red[nb * 16 + tid];
       cluster.map_shared_rank(clred, 0)[r * 16 + tid] = s;
     }
   }
@@ -509,14 +513,9 @@ k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restri
   gemm_half(bufA, 4);
   gemm_half(bufA, 5);
   {
-    double q1[2][2];
-#pragma unroll
-    for (int mb = 0; mb < 2; ++mb) {
-      z1[mb][0] = w3.x + acc[0][mb][0] + acc[1][mb][0];        // dZ1
-      z1[mb][1] = w3.y + acc[0][mb][1] + acc[1][mb][1];
-      q1[mb][0] = z1[mb][0] * (1.0 - u1[mb][0] * u1[mb][0]);
-      q1[mb][1] = z1[mb][1] * (1.0 - u1[mb][1] * u1[mb][1]);
-    }
+    z1[0] = w3.x + acc[0][0] + acc[1][0];                    // dZ1
+    z1[1] = w3.y + acc[0][1] + acc[1][1];
+    const double q1[2] = {z1[0] * (1.0 - u1[0] * u1[0]), z1[1] * (1.0 - u1[1] * u1[1])};
     broadcast(bufB, q1);
   }
   cluster.sync();
@@ -524,13 +523,10 @@ k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restri
   clear_acc();
   gemm_half(bufB, 6);
   gemm_half(bufB, 7);
-#pragma unroll
-  for (int mb = 0; mb < 2; ++mb) {
-    const int m = m0 + g + 8 * mb;
-    if (m >= row_hi) continue;
-    const double da = z1[mb][0] + acc[0][mb][0] + acc[1][mb][0], db = z1[mb][1] + acc[0][mb][1] + acc[1][mb][1];
-    *reinterpret_cast<double2 *>(Q + (size_t)m * fwp + col) =
-        make_double2(da * (1.0 - z0[mb][0] * z0[mb][0]), db * (1.0 - z0[mb][1] * z0[mb][1]));
+  if (m0 + row < row_hi) {
+    const double da = z1[0] + acc[0][0] + acc[1][0], db = z1[1] + acc[0][1] + acc[1][1];
+    *reinterpret_cast<double2 *>(Q + (size_t)(m0 + row) * fwp + col) =
+        make_double2(da * (1.0 - z0[0] * z0[0]), db * (1.0 - z0[1] * z0[1]));
   }
   cp_async_wait<0>();
 }
@@ -662,7 +658,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
 
   const bool splitk = C.n <= FIT_SMALL_N && !C.fslot;    // (not in deterministic mode: the partial sums are reductions)
   // small systems: the middle of the chain as one cluster kernel when the width is a multiple of 48 (clusters of <= 8 CTAs)
-  const size_t smem_mid = sizeof(double) * (2 * 16 * (size_t)(fwp + 4) + 3 * (size_t)(fwp / 2) * MID_LDB + 16 * (MID_WARPS + 8));
+  const size_t smem_mid = sizeof(double) * (2 * 16 * (size_t)(fwp + 4) + 3 * (size_t)(fwp / 2) * MID_LDB + 16 * (MID_NB + 8));
   const bool mid = splitk && fwp % MID_COLS == 0 && fwp / MID_COLS <= 8 && smem_mid <= 227 * 1024;
   if (mid) {
     static bool mid_configured_d[DPB_MAX_DEVICES] = {};
