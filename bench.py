@@ -474,12 +474,15 @@ def run_cuda(args):
         achieved = flops[dom] / dom_t / 1e12 if dom_t > 0 else None
         total_flops = sum(flops.values())
         traffic, traffic_src = None, None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "r2_traffic.csv")
         if os.path.exists(tpath):
             try:
-                tj = json.load(open(tpath))
-                traffic = tj.get(f"{name}:{args.precision if mixed else 'v' + str(args.variant)}:{dom}")
-                traffic_src = tj.get("source")
+                want = f"{name}:{args.precision if mixed else 'v' + str(args.variant)}:{dom}"
+                for ln in open(tpath).read().splitlines()[1:]:
+                    key, val = ln.rsplit(",", 1)
+                    if key == want:
+                        traffic = int(val)
+                traffic_src = "profiles/r2_traffic.md (dram__bytes_read.sum + dram__bytes_write.sum, one evaluation)"
             except Exception:
                 traffic = None
         line = {
