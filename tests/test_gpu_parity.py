@@ -290,6 +290,22 @@ def test_stored_activations_other_net_widths_and_overflow(s1, sel):
     m.close()
 
 
+@pytest.mark.parametrize("fit_width", [48, 96, 144])
+def test_small_system_cluster_kernel_other_widths(fit_width):
+    """The cluster kernel of the small-system fitting chain (k_fit_mid_cluster: widths that are multiples of 48, clusters of
+    w / 48 CTAs; BASELINE configs[0] runs it with 5) with clusters of 1, 2 and 3 CTAs, on a 2-species box whose species
+    have ragged last tiles (70 + 50 atoms: tiles of 16 rows), every output element against the oracle."""
+    spec, emb, fit = small_model(ntypes=2, s1=8, m_axis=4, fit_width=fit_width, sel=(30, 40), rcut=4.0, rcut_smth=1.0,
+                                 seed=17, fit_scale=0.05)
+    coord, types, box = random_box(120, 11.0, 2, seed=4, min_dist=1.1)
+    types[:70] = 0; types[70:] = 1
+    orc, m = _models(spec, emb, fit, 1)
+    ref = orc.eval(coord, types, box)
+    got = _gpu_eval(m, coord, types, box)
+    _check_full(ref, got)
+    m.close()
+
+
 def test_eval_host_matches_device_entry():
     """dpb_eval_host (host buffers, copies inside) returns the same numbers as dpb_eval."""
     torch = _torch()
