@@ -537,7 +537,19 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     }
   }
   DevStats *stats = m->stats.as<DevStats>();
-  if (nl_mode == 0) CU(cudaMemsetAsync(stats, 0, 2 * sizeof(DevStats), st), "memset stats");   // MD: kept over the run
+  // Small single-chunk periodic evaluations: the memsets (each a node in the chain of dependent launches) are folded into
+  // the cell-sort and list kernels (ZeroJobs, common.cuh)
+  const bool fold = !nlist_only && nl_mode == 0 && nloc < 0 && natoms > 0 && natoms <= 4096 && chunk >= ncentre &&
+                    m->precision == DPB_FP64 && m->variant == 1 && m->v1.ready && !det;
+  ZeroJobs zj{};
+  if (fold) {
+    zj.stats = stats; zj.stats_bytes = (int)(2 * sizeof(DevStats));
+    zj.counters = m->counters.as<int>(); zj.ncounters = 128;
+    zj.T = m->T.as<double>(); zj.t_len = P.M * 4;
+    zj.Z0 = v1_fit_preact(m->v1, m->v1ws.p, ncentre, &zj.z_len);
+    zj.force = force; zj.virial = virial;
+  }
+  if (nl_mode == 0 && !fold) CU(cudaMemsetAsync(stats, 0, 2 * sizeof(DevStats), st), "memset stats");   // MD: kept over the run
   NlRaw raw{};
   if (nl_mode != 0) {
     raw.raw = m->md_raw.as<int>(); raw.nraw = m->md_nraw.as<int>(); raw.cap = m->md_cap_raw;
@@ -564,7 +576,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
                             st), "gather");
   } else {
     CU(launch_cell_sort(P, G, natoms, coord, type, m->key.as<int>(), m->count.as<int>(), start, m->cursor.as<int>(),
-                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st, m->pos_of.as<int>()),
+                        m->s_idx.as<int>(), m->s_xyz.as<double>(), stats, st, m->pos_of.as<int>(), fold ? &zj : nullptr),
        "cell sort");
     if (nl_mode == 1 && natoms > 0)
       CU(cudaMemcpyAsync(m->md_xyz0.p, m->s_xyz.p, sizeof(double) * 3 * (size_t)natoms, cudaMemcpyDeviceToDevice, st),
@@ -578,7 +590,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
   }
 
   double *ei = atom_energy ? atom_energy : m->ei.as<double>();
-  if (!nlist_only) {
+  if (!nlist_only && !fold) {
     if (force) CU(cudaMemsetAsync(force, 0, sizeof(double) * 3 * (size_t)natoms, st), "memset force");
     if (virial) CU(cudaMemsetAsync(virial, 0, sizeof(double) * 9, st), "memset virial");
   }
@@ -601,7 +613,7 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.nlp = m->nlp.as<int>();
     C.counters = m->counters.as<int>();
     C.sub_part = 0; C.sub_nparts = 1;
-    if (!nlist_only) CU(cudaMemsetAsync(C.counters, 0, sizeof(int) * 128, st), "memset counters");
+    if (!nlist_only && !fold) CU(cudaMemsetAsync(C.counters, 0, sizeof(int) * 128, st), "memset counters");
     C.fslot = nullptr;
     C.pos_of = m->pos_of.as<int>();
     C.stats = stats;
@@ -609,13 +621,14 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.reuse2 = (!det && m->pair_reuse >= 1) ? 1 : 0;     // pass 2 only reads dT_j: no bookkeeping, any chunking
     C.act = act_stride ? m->act.as<double>() : nullptr;
     C.act_stride = act_stride;
+    C.prezero = fold ? 1 : 0;
     if (det) {                                           // full-size lists: the gather needs every atom's row
       C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
       C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;
       C.fslot = m->fslot.as<double>() + 3 * (size_t)p0 * P.nm;
     }
-    CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st, nl_mode, nl_mode ? &raw : nullptr),
-       "nlist");
+    CU(launch_nlist(P, G, C, m->s_xyz.as<double>(), start, cap, nlist, stats, st, nl_mode, nl_mode ? &raw : nullptr,
+                    fold ? &zj : nullptr), "nlist");
     if (nlist_only) continue;
     if (timing) cudaEventRecord(m->evs[2 + 4 * ci], st);
     if (m->precision != DPB_FP64) {

@@ -82,6 +82,19 @@ struct ChunkView {
   // slot (row, section slot) at act + ((size_t)row * nm + slot) * act_stride; nullptr: pass 2 recomputes.
   double *act;
   int act_stride;          // doubles per record: 4 * (even(SP) + 6 SP)
+  int prezero;             // T and the split-K pre-activations were cleared by the list kernel (ZeroJobs): no memsets
+};
+
+// Small single-chunk evaluations are a chain of dependent graph nodes, and every memset is one of them (stats, counters,
+// force, virial, T, the split-K pre-activations: 15 us of a 230 us evaluation of 192 atoms).  The cell-sort and list kernels
+// clear these on the side instead.  Null pointers: nothing to do.
+struct ZeroJobs {
+  void *stats; int stats_bytes;        // k_sort_small, before the keys (multiple of 4 bytes)
+  int *counters; int ncounters;        // k_sort_small
+  double *T; int t_len;                // k_nlist<0>: block q clears T[q][0 .. t_len)
+  double *Z0; int z_len;               // k_nlist<0>: block q clears Z0[q][0 .. z_len)
+  double *force;                       // k_nlist<0>: block q clears force[q][0..3) (one block per atom of the evaluation)
+  double *virial;                      // k_nlist<0>: block 0 clears virial[0..9)
 };
 
 // The per-type fitting chains are independent (disjoint rows) and one type's GEMM launch fills only as many SMs as that
@@ -126,7 +139,7 @@ extern unsigned long long g_dpb_launches;
 // ---- launchers implemented in the .cu files (all asynchronous on `st`; return cudaGetLastError()) ----------
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
-                             DevStats *stats, cudaStream_t st, int *pos_of = nullptr);
+                             DevStats *stats, cudaStream_t st, int *pos_of = nullptr, const ZeroJobs *zero = nullptr);
 // deterministic force / virial reduction (det.cu)
 cudaError_t launch_merge_ghost_stats(DevStats *stats, cudaStream_t st);
 cudaError_t launch_force_gather(const DevModel &P, const DevGrid &G, int64_t natoms, int64_t nloc, const int *s_idx, const int *pos_of,
@@ -134,7 +147,7 @@ cudaError_t launch_force_gather(const DevModel &P, const DevGrid &G, int64_t nat
                                 const double *fslot, double *force, double *vpart, double *virial, cudaStream_t st);
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
                          const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode = 0,
-                         const NlRaw *raw = nullptr);
+                         const NlRaw *raw = nullptr, const ZeroJobs *zero = nullptr);
 cudaError_t launch_gather_sorted(int64_t natoms, const double *coord, const int *s_idx, double *s_xyz,
                                  const double *xyz0, DevStats *stats, cudaStream_t st);
 

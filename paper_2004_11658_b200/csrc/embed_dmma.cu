@@ -1427,7 +1427,7 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
     configured_ru = smem_ru;
   }
   const int nseg = C.fslot ? 1 : seg_count(C.n, P1_WARPS, P.ntypes * P.ntypes);   // deterministic mode: no reductions into T
-  if (reuse || nseg > 1) {                               // every accumulation into T is then an addition
+  if ((reuse || nseg > 1) && !C.prezero) {               // every accumulation into T is then an addition
     cudaError_t e = cudaMemsetAsync(C.T, 0, sizeof(double) * (size_t)C.n * P.M * 4, st);
     if (e != cudaSuccess) return e;
   }

@@ -636,6 +636,15 @@ cudaError_t v1_plain_gemm(int64_t rows, const double *A, int lda, const double *
   return Cin ? gemm_t<2, 8, EPI_ADD>(C, 0, g, st) : gemm_t<2, 8, EPI_STORE>(C, 0, g, st);
 }
 
+// The buffer of the first layer's pre-activations (split-K sums) inside the workspace of a chunk of n atoms, and its
+// row length: what a caller clears on the side instead of the memset below (ChunkView::prezero).
+double *v1_fit_preact(const V1Weights &W, void *ws, int64_t n, int *row_len) {
+  const FitWeights *F = reinterpret_cast<const FitWeights *>(W.fit);
+  if (!F || !ws) return nullptr;
+  *row_len = F->fwp;
+  return reinterpret_cast<double *>(ws) + 2 * (size_t)n * F->dimp;
+}
+
 cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, const double *fit, void *ws,
                    double *atom_energy, cudaStream_t st) {
   (void)fit;
@@ -670,7 +679,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
       mid_configured = true;
     }
   }
-  if (splitk && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
+  if (splitk && !C.prezero && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
   // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint.  The
   // descriptor and dT kernels (memory-bound) belong to the chains: one species' run beside the other's GEMMs
   const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);

@@ -121,9 +121,11 @@ __global__ void k_fill(int n, const double *__restrict__ coord, const int *__res
 __global__ void __launch_bounds__(1024)
 k_sort_small(DevModel P, DevGrid G, int n, int nkeys, const double *__restrict__ coord, const int *__restrict__ type,
              int *key, int *count, int *start, int *cursor, int *__restrict__ s_idx, double *__restrict__ s_xyz,
-             DevStats *stats, int *__restrict__ pos_of) {
+             DevStats *stats, int *__restrict__ pos_of, ZeroJobs Z) {
   __shared__ int part[1024];
   for (int k = threadIdx.x; k < nkeys; k += 1024) count[k] = 0;
+  if (Z.stats) for (int k = threadIdx.x; k < Z.stats_bytes / 4; k += 1024) reinterpret_cast<int *>(Z.stats)[k] = 0;
+  if (Z.counters) for (int k = threadIdx.x; k < Z.ncounters; k += 1024) Z.counters[k] = 0;
   __syncthreads();
   for (int i = threadIdx.x; i < n; i += 1024) {
     const int k = sort_key(P, G, i, coord, type, stats);
@@ -138,15 +140,19 @@ k_sort_small(DevModel P, DevGrid G, int n, int nkeys, const double *__restrict__
 
 cudaError_t launch_cell_sort(const DevModel &P, const DevGrid &G, int64_t natoms, const double *coord, const int *type,
                              int *key, int *count, int *start, int *cursor, int *s_idx, double *s_xyz,
-                             DevStats *stats, cudaStream_t st, int *pos_of) {
+                             DevStats *stats, cudaStream_t st, int *pos_of, const ZeroJobs *zero) {
   const int nkeys = P.ntypes * G.ngrp * G.ncell;
   const int n = (int)natoms;
+  ZeroJobs Z{};
+  if (zero) Z = *zero;
   if (n > 0 && n <= SORT_SMALL_N && nkeys <= 4 * SORT_SMALL_N) {
-    k_sort_small<<<1, 1024, 0, st>>>(P, G, n, nkeys, coord, type, key, count, start, cursor, s_idx, s_xyz, stats, pos_of);
+    k_sort_small<<<1, 1024, 0, st>>>(P, G, n, nkeys, coord, type, key, count, start, cursor, s_idx, s_xyz, stats, pos_of, Z);
     DPB_LAUNCHED(1);
     return cudaGetLastError();
   }
   cudaError_t e = cudaMemsetAsync(count, 0, sizeof(int) * (size_t)nkeys, st);
+  if (e == cudaSuccess && Z.stats) e = cudaMemsetAsync(Z.stats, 0, (size_t)Z.stats_bytes, st);
+  if (e == cudaSuccess && Z.counters) e = cudaMemsetAsync(Z.counters, 0, sizeof(int) * (size_t)Z.ncounters, st);
   if (e != cudaSuccess) return e;
   if (n > 0) k_keys<<<(n + 255) / 256, 256, 0, st>>>(P, G, n, coord, type, key, count, stats);
   // type_start lives right behind start[nkeys + 1]
@@ -173,8 +179,15 @@ struct __align__(16) NlHit { double r; int j; int t; };
 template <int MODE>
 __global__ void __launch_bounds__(NL_THREADS, MODE == 0 ? 10 : 1)   // 48 registers: 10 blocks per SM (64 gave 8: +11 %)
 k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, const int *__restrict__ start, int cap,
-        int *__restrict__ nlist_out, DevStats *stats, NlRaw R) {
+        int *__restrict__ nlist_out, DevStats *stats, NlRaw R, ZeroJobs Z) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  if (MODE == 0 && (Z.T || Z.Z0 || Z.force || Z.virial)) {          // small evaluations: the memsets of the later stages
+    const int zb = blockIdx.x, zt = threadIdx.x, zn = blockDim.x;
+    if (Z.T) for (int k = zt; k < Z.t_len; k += zn) Z.T[(size_t)zb * Z.t_len + k] = 0.0;
+    if (Z.Z0) for (int k = zt; k < Z.z_len; k += zn) Z.Z0[(size_t)zb * Z.z_len + k] = 0.0;
+    if (Z.force && zt < 3) Z.force[3 * (size_t)zb + zt] = 0.0;
+    if (Z.virial && zb == 0 && zt < 9) Z.virial[zt] = 0.0;
+  }
   NlHit *hit = reinterpret_cast<NlHit *>(smem_raw);               // [cap] (distance, atom index j, type of j)
   int *hp = reinterpret_cast<int *>(hit + cap);                   // [cap] sorted position of j
   int *order = hp + cap;                                          // [cap] hits grouped by (type, distance bucket)
@@ -384,8 +397,10 @@ k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, co
 
 cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C, const double *s_xyz,
                          const int *start, int cap, int *nlist_out, DevStats *stats, cudaStream_t st, int mode,
-                         const NlRaw *raw) {
+                         const NlRaw *raw, const ZeroJobs *zero) {
   if (C.n <= 0) return cudaSuccess;
+  ZeroJobs Z{};
+  if (zero && mode == 0) Z = *zero;
   const size_t smem = (size_t)cap * (sizeof(NlHit) + 2 * sizeof(int)) + sizeof(int) * (3 * 18 * (size_t)P.ntypes * G.ngrp + 1);
   static size_t configured_d[DPB_MAX_DEVICES] = {};
   size_t &configured = configured_d[dpb_device()];
@@ -401,9 +416,9 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
   // one block per atom: 64 threads when the lists are short (water: ~660 candidates for ~90 hits; 192 -> 182 us on W24k),
   // 128 otherwise (copper, ~1,200 candidates: 64 threads take 586 instead of 416 us on Cu32k)
   const int nthr = P.nm <= 192 ? 64 : NL_THREADS;
-  if (mode == 1) k_nlist<1><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R);
-  else if (mode == 2) k_nlist<2><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R);
-  else k_nlist<0><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R);
+  if (mode == 1) k_nlist<1><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
+  else if (mode == 2) k_nlist<2><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
+  else k_nlist<0><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
 }

@@ -17,6 +17,7 @@ void v1_release_fit(V1Weights &W);
 cudaError_t v1_prepare_weights(const DevModel &P, const double *emb_h, const double *fit_h, V1Weights &W);
 void v1_release_weights(V1Weights &W);
 size_t v1_workspace_bytes(const DevModel &P, int64_t chunk);
+double *v1_fit_preact(const V1Weights &W, void *ws, int64_t n, int *row_len);
 cudaError_t v1_pass1(const DevModel &P, const ChunkView &C, const V1Weights &W, cudaStream_t st);
 cudaError_t v1_fit(const DevModel &P, const ChunkView &C, const V1Weights &W, const double *fit, void *ws,
                    double *atom_energy, cudaStream_t st);
