@@ -176,12 +176,14 @@ struct __align__(16) NlHit { double r; int j; int t; };
 // MODE 0: candidates from the cell stencil (cells >= r_c).  MODE 1 (MD, rebuild step): cells >= r_c + skin; every
 // candidate within r_c + skin is also appended to the atom's raw list (the paper's LAMMPS skin list, PAPER.md:193,
 // :298).  MODE 2 (MD, reuse step): candidates are the raw list — Alg. 1 proper: format a raw list.
-template <int MODE>
+// ZERO: the instantiation of small evaluations that also clears the later stages' buffers (ZeroJobs); the other one must
+// not see that code at all (its 48 registers and 10 blocks per SM are tuned: +4-6 % with the test compiled in).
+template <int MODE, bool ZERO = false>
 __global__ void __launch_bounds__(NL_THREADS, MODE == 0 ? 10 : 1)   // 48 registers: 10 blocks per SM (64 gave 8: +11 %)
 k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, const int *__restrict__ start, int cap,
         int *__restrict__ nlist_out, DevStats *stats, NlRaw R, ZeroJobs Z) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  if (MODE == 0 && (Z.T || Z.Z0 || Z.force || Z.virial)) {          // small evaluations: the memsets of the later stages
+  if (ZERO) {                                                       // small evaluations: the memsets of the later stages
     const int zb = blockIdx.x, zt = threadIdx.x, zn = blockDim.x;
     if (Z.T) for (int k = zt; k < Z.t_len; k += zn) Z.T[(size_t)zb * Z.t_len + k] = 0.0;
     if (Z.Z0) for (int k = zt; k < Z.z_len; k += zn) Z.Z0[(size_t)zb * Z.z_len + k] = 0.0;
@@ -408,6 +410,7 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
     cudaError_t e = cudaFuncSetAttribute(k_nlist<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_nlist<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_nlist<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_nlist<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
@@ -418,6 +421,7 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
   const int nthr = P.nm <= 192 ? 64 : NL_THREADS;
   if (mode == 1) k_nlist<1><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
   else if (mode == 2) k_nlist<2><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
+  else if (zero) k_nlist<0, true><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
   else k_nlist<0><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
