@@ -668,18 +668,32 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
   const bool splitk = C.n <= FIT_SMALL_N && !C.fslot;    // (not in deterministic mode: the partial sums are reductions)
   // small systems: the middle of the chain as one cluster kernel when the width is a multiple of 48 (clusters of <= 8 CTAs)
   const size_t smem_mid = sizeof(double) * (2 * 16 * (size_t)(fwp + 4) + 3 * (size_t)(fwp / 2) * MID_LDB + 16 * (MID_NB + 8));
-  const bool mid = splitk && fwp % MID_COLS == 0 && fwp / MID_COLS <= 8 && smem_mid <= 227 * 1024;
+  bool mid = splitk && fwp % MID_COLS == 0 && fwp / MID_COLS <= 8 && smem_mid <= 227 * 1024;
   if (mid) {
-    static bool mid_configured_d[DPB_MAX_DEVICES] = {};
-    bool &mid_configured = mid_configured_d[dpb_device()];
-    if (!mid_configured) {
-      if ((e = cudaFuncSetAttribute(k_fit_mid_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024))) !=
-          cudaSuccess)
-        return e;
-      mid_configured = true;
+    // once per device and width: the shared-memory limit, and whether a cluster of this size can be resident at all (a
+    // device or partition where it cannot falls back to the separate launches)
+    static int mid_state_d[DPB_MAX_DEVICES] = {}, mid_fwp_d[DPB_MAX_DEVICES] = {};
+    int &mid_state = mid_state_d[dpb_device()], &mid_fwp = mid_fwp_d[dpb_device()];
+    if (mid_state == 0 || mid_fwp != fwp) {
+      mid_fwp = fwp;
+      mid_state = -1;
+      if (cudaFuncSetAttribute(k_fit_mid_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)) ==
+          cudaSuccess) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(fwp / MID_COLS), 1, 1);
+        cfg.blockDim = dim3(32 * MID_WARPS, 1, 1);
+        cfg.dynamicSmemBytes = smem_mid;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)(fwp / MID_COLS); at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int nclusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&nclusters, k_fit_mid_cluster, &cfg) == cudaSuccess && nclusters > 0) mid_state = 1;
+      }
+      if (mid_state < 0) cudaGetLastError();
     }
+    mid = mid_state > 0;
   }
-  if (splitk && !C.prezero && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
   // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint.  The
   // descriptor and dT kernels (memory-bound) belong to the chains: one species' run beside the other's GEMMs
   const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
