@@ -694,6 +694,7 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
     }
     mid = mid_state > 0;
   }
+  if (splitk && !C.prezero && (e = cudaMemsetAsync(Z0, 0, sizeof(double) * n * fwp, st)) != cudaSuccess) return e;
   // per-type chains on forked streams (common.cuh); their rows, hence every buffer row they touch, are disjoint.  The
   // descriptor and dT kernels (memory-bound) belong to the chains: one species' run beside the other's GEMMs
   const size_t sm = sizeof(double) * ((size_t)P.M * 4 + (size_t)P.M * (P.Ma + 1) + 256 + 4 * P.Ma);
