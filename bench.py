@@ -189,7 +189,8 @@ def workload_config(name, args):
             "precision": getattr(args, "precision", "fp64"),
             "pair_reuse": "nets (a,a): pass 2 always, pass 1 in single-chunk evaluations (library default; fp64 variant 1)",
             "stored_activations": ("library default (on when the records fit the workspace budget)" if STORED_ACT is None
-                                   else bool(STORED_ACT))}
+                                   else bool(STORED_ACT)),
+            "species_pipeline": "library default (on in the timed steps; the stage timers of stage_us separate the stages)"}
 
 
 # ---- molecular dynamics: the paper's own unit, steps/s and ns/day ----------------------

@@ -157,6 +157,15 @@ int dpb_model_set_pair_reuse(dpb_model *model, int on);
  * recomputes (the paper's Eq. 13 tensors are then never written).  Returns DPB_EINVAL for any other value. */
 int dpb_model_set_stored_activations(dpb_model *model, int on);
 
+/* Species pipeline (DPB_FP64, variant 1, more than one species, chunks of at least 4096 centres; on by default).  Pass 1,
+ * the fitting chain and pass 2 of centre type a touch only rows of type a — T_a, the fitting buffers of a, dE/dT_a; with
+ * the pair reuse the neighbour's rows are of type a as well — so with on = 1 they run back to back on the stream of type
+ * a, without the barriers between the stages, and the streams join after pass 2 (Eq. 1 sums over atoms: the
+ * species are independent until then).  Same arithmetic, same results up to the order of the force reductions.  Switched
+ * off while the stage timers or the debug buffers are on.  on = 0: the three stages are separated by joins (what the
+ * stage times of bench.py describe).  Returns DPB_EINVAL for any other value. */
+int dpb_model_set_species_pipeline(dpb_model *model, int on);
+
 /* Per-atom virial.  The paper gives no per-atom split (the virial is only named through the
  * ProdVirial operator); this library assigns every term to its centre atom:
  *     atom_virial[i][a][b] = -sum_k d_ik[a] (dE_i/dd_ik)[b],     sum_i atom_virial[i] = virial of dpb_eval.

@@ -77,6 +77,7 @@ def load_library():
     lib.dpb_model_set_deterministic.argtypes = [vp, i32]
     lib.dpb_model_set_pair_reuse.argtypes = [vp, i32]
     lib.dpb_model_set_stored_activations.argtypes = [vp, i32]
+    lib.dpb_model_set_species_pipeline.argtypes = [vp, i32]
     lib.dpb_model_set_atom_virial.argtypes = [vp, vp]
     lib.dpb_model_set_timing.argtypes = [vp, i32]
     lib.dpb_model_stage_us.argtypes = [vp, C.POINTER(C.c_float)]
@@ -165,6 +166,10 @@ class DPModel:
 
     def set_deterministic(self, on: bool):
         self._chk(self.lib.dpb_model_set_deterministic(self._h, int(bool(on))))
+
+    def set_species_pipeline(self, on: bool):
+        """dpb_model_set_species_pipeline: the stages of one centre type back to back on its stream (default on)."""
+        self._chk(self.lib.dpb_model_set_species_pipeline(self._h, int(bool(on))))
 
     def set_stored_activations(self, on: bool):
         """dpb_model_set_stored_activations: pass 2 reads the embedding activations pass 1 stored (default on)."""

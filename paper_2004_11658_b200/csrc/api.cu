@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -73,6 +74,18 @@ cudaError_t dpb_join_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX
   }
   return cudaSuccess;
 }
+cudaError_t dpb_forked_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]) {
+  s[0] = st;
+  if (ntypes <= 1) return cudaSuccess;
+  ForkState *F;
+  cudaError_t e = fork_state(&F);
+  if (e != cudaSuccess) return e;
+  for (int ty = 1; ty < ntypes; ++ty) {
+    if (!F->aux[ty]) return cudaErrorInvalidResourceHandle;
+    s[ty] = F->aux[ty];
+  }
+  return cudaSuccess;
+}
 extern "C" int64_t dpb_kernel_launches(void) { return (int64_t)g_dpb_launches; }
 
 extern "C" const char *dpb_last_error(void) { return g_err; }
@@ -122,6 +135,7 @@ struct dpb_model {
   unsigned long long cfg_epoch = 1, graph_clock = 0;
   std::vector<GraphEntry> graphs;
   int precision = 0, variant = 1, timing = 0, deterministic = 0, pair_reuse = 1, stored_act = 1;
+  int species_pipe = 1;         // dpb_model_set_species_pipeline
   double *atom_virial = nullptr;        // caller's [N][9] buffer (dpb_model_set_atom_virial)
   int64_t chunk = 0;            // atoms per pass; 0 = automatic (effective_chunk)
   size_t ws_budget = 0;         // bytes the per-chunk workspace may take in automatic mode (half of the memory free at creation)
@@ -328,6 +342,14 @@ extern "C" int dpb_model_set_pair_reuse(dpb_model *m, int on) {
   if (!m) return fail(DPB_EINVAL, "null model");
   if (on < 0 || on > 2) return fail(DPB_EINVAL, "pair reuse: 0 (off), 1 (single-chunk evaluations) or 2 (always)");
   m->pair_reuse = on;
+  ++m->cfg_epoch;
+  return DPB_OK;
+}
+
+extern "C" int dpb_model_set_species_pipeline(dpb_model *m, int on) {
+  if (!m) return fail(DPB_EINVAL, "null model");
+  if (on < 0 || on > 1) return fail(DPB_EINVAL, "species pipeline: 0 (off) or 1 (on)");
+  m->species_pipe = on;
   ++m->cfg_epoch;
   return DPB_OK;
 }
@@ -622,6 +644,8 @@ static int run_eval(dpb_model *m, cudaStream_t st, int64_t natoms, const double 
     C.act = act_stride ? m->act.as<double>() : nullptr;
     C.act_stride = act_stride;
     C.prezero = fold ? 1 : 0;
+    C.typed_pipe = (P.ntypes > 1 && C.n >= 4096 && !timing && !det && m->precision == DPB_FP64 && m->variant == 1 &&
+                    m->v1.ready && !m->dbgT && !m->dbgD && !m->dbgdT && m->species_pipe) ? 1 : 0;
     if (det) {                                           // full-size lists: the gather needs every atom's row
       C.nl = m->nl_all.as<int>() + (size_t)p0 * P.nm;
       C.nreal = m->nreal_all.as<int>() + (size_t)p0 * P.ntypes;

@@ -83,6 +83,10 @@ struct ChunkView {
   double *act;
   int act_stride;          // doubles per record: 4 * (even(SP) + 6 SP)
   int prezero;             // T and the split-K pre-activations were cleared by the list kernel (ZeroJobs): no memsets
+  // Species pipeline (ntypes > 1, large chunks): pass 1, the fitting chain and pass 2 of centre type a touch only rows of
+  // type a (T_a, the fitting buffers of a, dT_a — with the pair reuse T_j and dT_j are of type a too), so they run back to
+  // back on the stream of type a without the barriers between the stages; the streams join after pass 2.
+  int typed_pipe;
 };
 
 // Small single-chunk evaluations are a chain of dependent graph nodes, and every memset is one of them (stats, counters,
@@ -102,6 +106,8 @@ struct ZeroJobs {
 // streams that wait for everything enqueued on st so far; join: st waits for everything enqueued on them.
 cudaError_t dpb_fork_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]);
 cudaError_t dpb_join_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]);
+// the streams of an earlier fork that has not been joined yet (no event is recorded, nothing waits)
+cudaError_t dpb_forked_streams(int ntypes, cudaStream_t st, cudaStream_t s[DPB_MAX_TYPES]);
 
 // dd.cu: pack / unpack kernels of the domain decomposition's ghost exchange
 cudaError_t launch_dd_pack(int64_t n, const double *coord, const int *type, int dim, double cut_minus, double cut_plus,

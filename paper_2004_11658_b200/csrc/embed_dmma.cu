@@ -1452,7 +1452,7 @@ static cudaError_t run_pass1(const DevModel &P, const ChunkView &C, const V1Weig
                                                                       C.counters + a * P.ntypes + t);
       DPB_LAUNCHED(1);
     }
-  if ((e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;
+  if (!(C.typed_pipe && nseg == 1) && (e = dpb_join_streams(ns, st, ts)) != cudaSuccess) return e;
   return cudaGetLastError();
 }
 
@@ -1507,13 +1507,14 @@ static cudaError_t run_pass2(const DevModel &P, const ChunkView &C, const V1Weig
   // the nets are independent here (forces and virial are atomic sums, slot stores are disjoint): a stream per net, so
   // that the tail of every launch is filled by the others
   cudaStream_t ts[DPB_MAX_TYPES];
-  const int ns = min(P.ntypes * P.ntypes, DPB_MAX_TYPES);
-  cudaError_t e = dpb_fork_streams(ns, st, ts);
+  const bool typed = C.typed_pipe && nseg == 1;            // species pipeline: the streams of pass 1 / fitting, not joined yet
+  const int ns = typed ? P.ntypes : min(P.ntypes * P.ntypes, DPB_MAX_TYPES);
+  cudaError_t e = typed ? dpb_forked_streams(ns, st, ts) : dpb_fork_streams(ns, st, ts);
   if (e != cudaSuccess) return e;
   for (int a = P.ntypes - 1; a >= 0; --a)
     for (int t = P.ntypes - 1; t >= 0; --t) {
       const int net = a * P.ntypes + t;
-      cudaStream_t s = ts[(P.ntypes * P.ntypes - 1 - net) % ns];
+      cudaStream_t s = typed ? ts[P.ntypes - 1 - a] : ts[(P.ntypes * P.ntypes - 1 - net) % ns];
       if (sa && a != t)
         k_pass2_dmma_st<SP, true, NW1, false><<<grid, (32 * NW1), smem_one, s>>>(P, C, W.emb + (size_t)net * W.net_stride, a,
                                                                                    t, force, virial, C.counters + 64 + net);

@@ -714,7 +714,8 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
   const int split = P.ntypes == 1 && C.n >= 4096 ? 2 : 1;
   const int nbatch = P.ntypes * split;
   cudaStream_t ts[DPB_MAX_TYPES];
-  if ((e = dpb_fork_streams(nbatch, st, ts)) != cudaSuccess) return e;
+  const bool typed = C.typed_pipe && split == 1 && !splitk;   // species pipeline: pass 1 left the streams forked
+  if ((e = typed ? dpb_forked_streams(nbatch, st, ts) : dpb_fork_streams(nbatch, st, ts)) != cudaSuccess) return e;
   for (int k = 0; k < nbatch; ++k) {
     const int ty = P.ntypes - 1 - k / split, part = k % split;
     cudaStream_t s = ts[k];
@@ -772,6 +773,6 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
     else k_dT_v1<<<C.n, 256, sm, s>>>(P, C, ty, dimp, dD);
     DPB_LAUNCHED(1);
   }
-  if ((e = dpb_join_streams(nbatch, st, ts)) != cudaSuccess) return e;
+  if (!typed && (e = dpb_join_streams(nbatch, st, ts)) != cudaSuccess) return e;
   return cudaGetLastError();
 }

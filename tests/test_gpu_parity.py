@@ -245,6 +245,9 @@ def test_full_size_parity_every_element(name, conditioned):
     m.set_stored_activations(False)
     _check_full(ref, _gpu_eval(m, coord, types, box))
     m.set_stored_activations(True)
+    m.set_species_pipeline(False)                              # (default on: every run above, for the water box)
+    _check_full(ref, _gpu_eval(m, coord, types, box))
+    m.set_species_pipeline(True)
     m.set_chunk(8192)
     for reuse in (1, 2):
         m.set_pair_reuse(reuse)
