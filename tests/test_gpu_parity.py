@@ -293,6 +293,33 @@ def test_stored_activations_other_net_widths_and_overflow(s1, sel):
     m.close()
 
 
+def test_exactly_4096_atoms_where_the_small_and_the_large_paths_meet():
+    """4,096 atoms, two species: the evaluation is at once a 'small' one (graph replay, folded memsets, energy sum beside
+    pass 2) and a 'large' one (whole-atom work items, stored activations, species pipeline).  Every output element against
+    the oracle, eagerly and replayed from the graph."""
+    torch = _torch()
+    spec, emb, fit = small_model(ntypes=2, s1=8, m_axis=4, fit_width=16, sel=(40, 60), rcut=4.0, rcut_smth=1.0, seed=23,
+                                 fit_scale=0.05)
+    c0, t0, b0 = random_box(256, 11.0, 2, seed=41, min_dist=1.1)
+    shifts = np.array([[i, j, k] for i in range(2) for j in range(2) for k in range(4)], dtype=np.float64) * 11.0
+    coord = (c0[None, :, :] + shifts[:, None, :]).reshape(-1, 3)
+    coord = coord + np.random.default_rng(6).normal(0.0, 0.02, size=coord.shape)
+    types = np.tile(t0, 16)
+    box = np.diag([22.0, 22.0, 44.0]).reshape(-1)
+    assert len(coord) == 4096
+    orc, m = _models(spec, emb, fit, 1)
+    ref = orc.eval(coord, types, box)
+    _check_full(ref, _gpu_eval(m, coord, types, box))
+    dc, dt = torch.tensor(coord, device="cuda"), torch.tensor(types.astype(np.int32), device="cuda")
+    out = None
+    for _ in range(3):                                         # eager, captured, replayed
+        out = m.eval(dc, dt, box, out=out)
+        torch.cuda.synchronize()
+        assert abs(out["energy"].item() - ref["energy"]) <= E_REL * abs(ref["energy"])
+        assert np.abs(out["force"].cpu().numpy() - ref["force"]).max() <= F_ABS
+    m.close()
+
+
 @pytest.mark.parametrize("fit_width", [48, 96, 144])
 def test_small_system_cluster_kernel_other_widths(fit_width):
     """The cluster kernel of the small-system fitting chain (k_fit_mid_cluster: widths that are multiples of 48, clusters of
