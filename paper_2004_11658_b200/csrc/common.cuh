@@ -138,6 +138,25 @@ static inline int dpb_device() {
   return d;
 }
 
+// Programmatic dependent launch (small evaluations: a chain of dependent launches on one stream).  A kernel launched
+// with dpb_launch_pdl may be scheduled while its predecessor on the stream still runs; it must call pdl_wait() before it
+// touches anything the predecessor writes (or writes anything the predecessor reads).  pdl_wait() is a no-op in a kernel
+// launched the ordinary way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// ... and the predecessor says when its successor may be scheduled (it still waits in pdl_wait for the whole grid to end)
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <class... KArgs, class... Args>
+static inline cudaError_t dpb_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                         bool pdl, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // Process-wide count of kernels launched by this library (reported by dpb_kernel_launches()).
 extern unsigned long long g_dpb_launches;
 #define DPB_LAUNCHED(n) (g_dpb_launches += (unsigned long long)(n))

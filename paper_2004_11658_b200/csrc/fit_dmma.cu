@@ -64,6 +64,7 @@ struct GemmArgs {
 template <int WM, int NBW, int EPI, int FIT_BK>
 __global__ void __launch_bounds__(64 * WM, FIT_BK == 16 ? 2 : 1)
 k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
+  if (FIT_BK != 16) { pdl_wait(); pdl_trigger(); }          // the small-system instantiations are launched with dpb_launch_pdl
   constexpr int FIT_BM = 16 * WM, FIT_THREADS = 64 * WM, FIT_LDA = FIT_BK + 4;
   constexpr int BN = 16 * NBW, LDB = BN + 4;
   extern __shared__ __align__(16) double smem[];
@@ -196,6 +197,7 @@ k_fit_gemm(ChunkView C, int ty, GemmArgs g) {
 
 // S5: D[b][a] = sum_c T[b][c] T[a][c] (Eq. 4; flatten b M^< + a, reading R7), zero-padded to dimp.
 __global__ void k_descr_v1(DevModel P, ChunkView C, int ty, int dimp, double *__restrict__ D) {
+  pdl_trigger();                                           // (small systems: G1 behind it is launched with dpb_launch_pdl)
   const int q = blockIdx.x;
   {                                                         // one launch per species, on that species' stream
     int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
@@ -265,6 +267,7 @@ template <int LPR>
 __global__ void __launch_bounds__(32 * DTV_WARPS) k_dT_v1s(DevModel P, ChunkView C, int ty, int dimp, const double *__restrict__ dD) {
   extern __shared__ double sm2[];
   constexpr int Ma = 2 * LPR, RPI = 32 / LPR;
+  pdl_wait();                                               // (small systems launch it with dpb_launch_pdl behind G6)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = blockIdx.x * DTV_WARPS + warp;
   if (q >= C.n) return;
@@ -388,6 +391,8 @@ k_fit_mid_cluster(ChunkView C, int ty, int fwp, FitNet N, const double *__restri
   cg::cluster_group cluster = cg::this_cluster();
   int row_lo = max(C.p0, C.type_start[ty]) - C.p0, row_hi = min(C.p0 + C.n, C.type_start[ty + 1]) - C.p0;
   dpb_sub_range(C, row_lo, row_hi);
+  pdl_wait();                                                // launched behind the split-K G1 with the programmatic attribute
+  pdl_trigger();
   const int m0 = row_lo + blockIdx.y * 16;
   if (m0 >= row_hi) return;                                  // the whole cluster (same blockIdx.y) leaves together
   const int ncl = (int)cluster.num_blocks(), r = (int)cluster.block_rank();
@@ -608,6 +613,10 @@ static cudaError_t gemm_t(const ChunkView &C, int ty, const GemmArgs &g, cudaStr
     configured = true;
   }
   dim3 grid((C.n + FIT_BM - 1) / FIT_BM, (g.N + BN - 1) / BN, splitk);
+  if (FIT_BK != 16) {
+    cudaError_t el = dpb_launch_pdl(k_fit_gemm<WM, NBW, EPI, FIT_BK>, grid, dim3(64 * WM), smem, st, true, C, ty, g);
+    if (el != cudaSuccess) return el;
+  } else
   k_fit_gemm<WM, NBW, EPI, FIT_BK><<<grid, 64 * WM, smem, st>>>(C, ty, g);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
@@ -736,10 +745,12 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
       cfg.blockDim = dim3(32 * MID_WARPS, 1, 1);
       cfg.dynamicSmemBytes = smem_mid;
       cfg.stream = s;
-      cudaLaunchAttribute at[1];
+      cudaLaunchAttribute at[2];
       at[0].id = cudaLaunchAttributeClusterDimension;
       at[0].val.clusterDim.x = (unsigned)(fwp / MID_COLS); at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-      cfg.attrs = at; cfg.numAttrs = 1;
+      at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+      at[1].val.programmaticStreamSerializationAllowed = 1;
+      cfg.attrs = at; cfg.numAttrs = 2;
       if ((e = cudaLaunchKernelEx(&cfg, k_fit_mid_cluster, C, ty, fwp, N, (const double *)Z0, Q, atom_energy)) != cudaSuccess)
         return e;
       DPB_LAUNCHED(1);
@@ -767,7 +778,11 @@ cudaError_t v1_fit(const DevModel &P, const ChunkView &Cin, const V1Weights &W, 
     // G6: dD = Q W0^T
     g = GemmArgs{Q, fwp, N.W0T, dimp, fwp, dimp, nullptr, nullptr, nullptr, dimp, dD, nullptr, dimp};
     if ((e = gemm<8, EPI_STORE>(C, ty, g, s)) != cudaSuccess) return e;
-    if (P.Ma == 16 && sms <= 48 * 1024) k_dT_v1s<8><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
+    if (P.Ma == 16 && sms <= 48 * 1024 && C.n <= FIT_SMALL_N) {
+      if ((e = dpb_launch_pdl(k_dT_v1s<8>, dim3(nbs), dim3(32 * DTV_WARPS), sms, s, true, P, C, ty, dimp, (const double *)dD)) !=
+          cudaSuccess)
+        return e;
+    } else if (P.Ma == 16 && sms <= 48 * 1024) k_dT_v1s<8><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
     else if (P.Ma == 8 && sms <= 48 * 1024) k_dT_v1s<4><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
     else if (P.Ma == 4 && sms <= 48 * 1024) k_dT_v1s<2><<<nbs, 32 * DTV_WARPS, sms, s>>>(P, C, ty, dimp, dD);
     else k_dT_v1<<<C.n, 256, sm, s>>>(P, C, ty, dimp, dD);

@@ -123,6 +123,7 @@ k_sort_small(DevModel P, DevGrid G, int n, int nkeys, const double *__restrict__
              int *key, int *count, int *start, int *cursor, int *__restrict__ s_idx, double *__restrict__ s_xyz,
              DevStats *stats, int *__restrict__ pos_of, ZeroJobs Z) {
   __shared__ int part[1024];
+  pdl_trigger();                                           // the list kernel behind may be scheduled now (it waits in pdl_wait)
   for (int k = threadIdx.x; k < nkeys; k += 1024) count[k] = 0;
   if (Z.stats) for (int k = threadIdx.x; k < Z.stats_bytes / 4; k += 1024) reinterpret_cast<int *>(Z.stats)[k] = 0;
   if (Z.counters) for (int k = threadIdx.x; k < Z.ncounters; k += 1024) Z.counters[k] = 0;
@@ -183,6 +184,7 @@ __global__ void __launch_bounds__(NL_THREADS, MODE == 0 ? 10 : 1)   // 48 regist
 k_nlist(DevModel P, DevGrid G, ChunkView C, const double *__restrict__ s_xyz, const int *__restrict__ start, int cap,
         int *__restrict__ nlist_out, DevStats *stats, NlRaw R, ZeroJobs Z) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  if (ZERO) pdl_wait();                                             // launched behind k_sort_small with dpb_launch_pdl
   if (ZERO) {                                                       // small evaluations: the memsets of the later stages
     const int zb = blockIdx.x, zt = threadIdx.x, zn = blockDim.x;
     if (Z.T) for (int k = zt; k < Z.t_len; k += zn) Z.T[(size_t)zb * Z.t_len + k] = 0.0;
@@ -421,7 +423,11 @@ cudaError_t launch_nlist(const DevModel &P, const DevGrid &G, const ChunkView &C
   const int nthr = P.nm <= 192 ? 64 : NL_THREADS;
   if (mode == 1) k_nlist<1><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
   else if (mode == 2) k_nlist<2><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
-  else if (zero) k_nlist<0, true><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
+  else if (zero) {
+    cudaError_t el = dpb_launch_pdl(k_nlist<0, true>, dim3(C.n), dim3(nthr), smem, st, true, P, G, C, s_xyz, start, cap,
+                                    nlist_out, stats, R, Z);
+    if (el != cudaSuccess) return el;
+  }
   else k_nlist<0><<<C.n, nthr, smem, st>>>(P, G, C, s_xyz, start, cap, nlist_out, stats, R, Z);
   DPB_LAUNCHED(1);
   return cudaGetLastError();
